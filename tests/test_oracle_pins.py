@@ -1,0 +1,472 @@
+"""Pins for the CPU oracle (oracle/vmat_oracle.c) against things other than itself:
+closed forms, finite differences, brute force, library routines, invariants.
+All CPU (-m "not gpu").  Citations: PAPER.md lines / SURVEY.md 8c readings.
+"""
+import itertools
+
+import numpy as np
+import pytest
+import scipy.optimize
+import scipy.sparse as sp
+
+import oracle as orc
+from oracle import Oracle
+
+
+# ------------------------------------------------------------------------------------------------
+# helpers: a small random problem with a dense D we can multiply by hand
+# ------------------------------------------------------------------------------------------------
+def small_problem(seed=0, V=37, N=5, R=3, C=6, density=0.4, gamma=0.3, delta=1, nonuniform_theta=False):
+    rng = np.random.default_rng(seed)
+    B = N * R * C
+    dense = rng.random((B, V)).astype(np.float32) * (rng.random((B, V)) < density)
+    dense[rng.integers(0, B, 3)] = 0.0                      # some empty rows
+    csr = sp.csr_matrix(dense)
+    csr.sort_indices()
+    T = rng.uniform(0.2, 1.0, V).astype(np.float32)
+    alpha = (rng.random(V) < 0.5) * rng.uniform(0.5, 2.0, V)
+    beta = rng.uniform(0.1, 1.5, V)
+    theta = np.cumsum(rng.uniform(1.0, 3.0, N)) if nonuniform_theta else np.arange(N) * 2.0
+    o = Oracle(csr.indptr.astype(np.int64), csr.indices.astype(np.int32), csr.data.astype(np.float32),
+               T, alpha.astype(np.float32), beta.astype(np.float32), theta, R, C, delta, gamma)
+    return o, dense.astype(np.float64), rng
+
+
+def random_plan(o, rng, n_occ):
+    occ = np.zeros(o.N, np.uint8)
+    occ[rng.choice(o.N, n_occ, replace=False)] = 1
+    left = rng.integers(0, o.C + 1, (o.N, o.R)).astype(np.int32)
+    right = np.array([[rng.integers(l, o.C + 1) for l in row] for row in left], np.int32)
+    y = rng.uniform(0.1, 2.0, o.N) * occ
+    return occ, left, right, y
+
+
+def open_mask(o, occ, left, right):
+    """x_i = 1 if beamlet i is exposed in an occupied beam (the set A_k)."""
+    m = np.zeros((o.N, o.R, o.C))
+    for k in range(o.N):
+        if occ[k]:
+            for r in range(o.R):
+                m[k, r, left[k, r]:right[k, r]] = 1.0
+    return m
+
+
+# ------------------------------------------------------------------------------------------------
+# O2 dose / O4 prices: plain (sparse) matrix-vector products
+# ------------------------------------------------------------------------------------------------
+def test_dose_equals_dense_product():
+    # z = D^T x, x_i = y_k [i in A_k]
+    o, D, rng = small_problem(1)
+    occ, left, right, y = random_plan(o, rng, 3)
+    x = (open_mask(o, occ, left, right) * y[:, None, None]).reshape(-1)
+    z = o.dose(occ, left, right, y)
+    np.testing.assert_allclose(z, D.T @ x, rtol=1e-13, atol=1e-13)
+
+
+def test_dose_single_entry_by_hand():
+    # one beam, one row, two beamlets, two voxels:  z = y * (D_0. + D_1.)
+    row_ptr = np.array([0, 2, 3], np.int64)
+    col = np.array([0, 1, 1], np.int32)
+    val = np.array([0.5, 0.25, 2.0], np.float32)
+    o = Oracle(row_ptr, col, val, [1, 1], [1, 1], [1, 1], [0.0], 1, 2, 1, 0.1)
+    z = o.dose([1], [[0]], [[2]], [3.0])
+    np.testing.assert_allclose(z, [1.5, 3.0 * 2.25])
+    z = o.dose([1], [[1]], [[2]], [3.0])          # only beamlet 1 open
+    np.testing.assert_allclose(z, [0.0, 6.0])
+    z = o.dose([1], [[1]], [[1]], [3.0])          # closed row
+    np.testing.assert_allclose(z, [0.0, 0.0])
+
+
+def test_prices_equal_scipy_spmv(tiny_phantom, tiny_oracle):
+    # g = D w against scipy.sparse in fp64
+    ph, o = tiny_phantom, tiny_oracle
+    rng = np.random.default_rng(3)
+    w = rng.standard_normal(o.V)
+    A = sp.csr_matrix((ph.val.astype(np.float64), ph.col_idx, ph.row_ptr), shape=(o.B, o.V))
+    g = o.prices(w)
+    ref = A @ w
+    np.testing.assert_allclose(g, ref, rtol=1e-12, atol=1e-12 * np.abs(ref).max())
+    # occupied beams are not priced
+    occ = np.zeros(o.N, np.uint8)
+    occ[[2, 5]] = 1
+    g2 = o.prices(w, occ).reshape(o.N, -1)
+    assert np.all(g2[[2, 5]] == 0.0)
+    np.testing.assert_array_equal(g2[[0, 1, 3]], g.reshape(o.N, -1)[[0, 1, 3]])
+
+
+def test_dose_is_transpose_of_prices():
+    # <D^T x, w> = <x, D w> ties O2 and O4 to the same matrix (catches a transposed operand)
+    o, D, rng = small_problem(5)
+    occ, left, right, y = random_plan(o, rng, o.N)
+    x = (open_mask(o, occ, left, right) * y[:, None, None]).reshape(-1)
+    w = rng.standard_normal(o.V)
+    assert np.dot(o.dose(occ, left, right, y), w) == pytest.approx(np.dot(x, o.prices(w)), rel=1e-12)
+
+
+# ------------------------------------------------------------------------------------------------
+# O3 penalty (Eq. 1) and smoothing (Eq. 2)
+# ------------------------------------------------------------------------------------------------
+def test_penalty_closed_form_one_voxel():
+    # Eq. 1: T=1, alpha=2, beta=3
+    for z, F, w in [(0.4, 2 * 0.36, -2 * 2 * 0.6), (1.5, 3 * 0.25, 2 * 3 * 0.5), (1.0, 0.0, 0.0)]:
+        Fo, wo = orc.penalty([z], [1.0], [2.0], [3.0])
+        assert Fo == pytest.approx(F, rel=1e-14)
+        assert wo[0] == pytest.approx(w, rel=1e-14, abs=0)
+    # critical structure: alpha = 0 -> no penalty below threshold
+    Fo, wo = orc.penalty([0.1], [0.5], [0.0], [1.0])
+    assert Fo == 0.0 and wo[0] == 0.0
+
+
+def test_penalty_gradient_finite_difference():
+    rng = np.random.default_rng(7)
+    V = 200
+    T = rng.uniform(0.2, 1.0, V).astype(np.float32)
+    a = rng.uniform(0, 2, V).astype(np.float32)
+    b = rng.uniform(0, 2, V).astype(np.float32)
+    z = rng.uniform(0.0, 1.5, V)
+    _, w = orc.penalty(z, T, a, b)
+    h = 1e-6
+    for j in range(V):
+        if abs(z[j] - T[j]) < 10 * h:
+            continue                                   # F is C1 but not C2 at the kink
+        zp, zm = z.copy(), z.copy()
+        zp[j] += h
+        zm[j] -= h
+        fd = (orc.penalty(zp, T, a, b, False)[0] - orc.penalty(zm, T, a, b, False)[0]) / (2 * h)
+        assert w[j] == pytest.approx(fd, rel=1e-6, abs=1e-7)
+
+
+def test_smooth_closed_forms():
+    N, dth = 9, 2.0
+    th = np.arange(N) * dth
+    G, dG = orc.smooth(np.full(N, 3.7), th)
+    assert G == 0.0 and np.all(dG == 0.0)              # constant dose rate costs nothing
+    G, _ = orc.smooth(np.arange(N, dtype=float), th)   # ramp: (N-1) unit steps / dtheta (Eq. 2)
+    assert G == pytest.approx((N - 1) / dth, rel=1e-15)
+    # units are degrees as passed (reading S4): halving the spacing doubles G
+    G2, _ = orc.smooth(np.arange(N, dtype=float), th / 2)
+    assert G2 == pytest.approx(2 * (N - 1) / dth, rel=1e-15)
+
+
+def test_smooth_is_laplacian_quadratic_form_and_gradient():
+    rng = np.random.default_rng(11)
+    N = 12
+    th = np.cumsum(rng.uniform(0.5, 3.0, N))
+    y = rng.uniform(0, 2, N)
+    L = np.zeros((N, N))                                # weighted path-graph Laplacian, no wrap-around (S3)
+    for k in range(N - 1):
+        wgt = 1.0 / (th[k + 1] - th[k])
+        L[k, k] += wgt
+        L[k + 1, k + 1] += wgt
+        L[k, k + 1] -= wgt
+        L[k + 1, k] -= wgt
+    G, dG = orc.smooth(y, th)
+    assert G == pytest.approx(y @ L @ y, rel=1e-13)
+    np.testing.assert_allclose(dG, 2 * L @ y, rtol=1e-12, atol=1e-13)
+    h = 1e-6
+    for k in range(N):
+        yp, ym = y.copy(), y.copy()
+        yp[k] += h
+        ym[k] -= h
+        assert dG[k] == pytest.approx((orc.smooth(yp, th)[0] - orc.smooth(ym, th)[0]) / (2 * h), rel=1e-7, abs=1e-8)
+
+
+# ------------------------------------------------------------------------------------------------
+# O5 leaf-row interval search: brute force over every (l, r') in the box
+# ------------------------------------------------------------------------------------------------
+def brute_force_row(q, Lmin, Lmax, Rmin, Rmax):
+    """Enumerate all admissible leaf pairs; key = (sum of open prices, open count, l) (S8, S9)."""
+    C = len(q)
+    best = None
+    for l in range(max(0, Lmin), min(C, Lmax) + 1):
+        for r in range(max(l, Rmin), min(C, Rmax) + 1):
+            key = (int(sum(int(v) for v in q[l:r])), r - l, l)
+            if best is None or key < best[0]:
+                best = (key, l, r)
+    return None if best is None else (best[1], best[2], best[0][0])
+
+
+def test_row_search_matches_brute_force():
+    rng = np.random.default_rng(2024)
+    n_cases = 0
+    for trial in range(4000):
+        C = int(rng.integers(1, 13))
+        kind = trial % 4
+        if kind == 0:
+            q = rng.integers(-5, 6, C)                  # many exact ties
+        elif kind == 1:
+            q = rng.integers(-3, 4, C) * (rng.random(C) < 0.5)   # many zero-price beamlets
+        elif kind == 2:
+            q = rng.integers(-10**12, 10**12, C)
+        else:
+            q = orc.quantise(rng.standard_normal(C).astype(np.float32) * (rng.random(C) < 0.8))
+        if trial % 3 == 0:
+            box = (0, C, 0, C)
+        else:
+            a, b = sorted(rng.integers(0, C + 1, 2))
+            c, d = sorted(rng.integers(0, C + 1, 2))
+            box = (int(a), int(b), int(c), int(d))
+        ref = brute_force_row(q, *box)
+        got = orc.row_search(q, *box)
+        assert got == ref, (q, box, got, ref)
+        n_cases += ref is not None
+    assert n_cases > 3000
+
+
+def test_row_search_exhaustive_tiny_rows():
+    # every price vector over {-1,0,1}^C for C<=5 and every box: no sampling gaps
+    for C in range(1, 6):
+        boxes = [(a, b, c, d) for a in range(C + 1) for b in range(a, C + 1) for c in range(C + 1) for d in range(c, C + 1)]
+        for q in itertools.product((-1, 0, 1), repeat=C):
+            for box in boxes[:: max(1, len(boxes) // 40)]:
+                assert orc.row_search(np.array(q), *box) == brute_force_row(q, *box)
+
+
+def test_row_search_unboxed_is_minimum_subarray():
+    # with no leaf-travel box the row problem is the textbook minimum-sum subarray (empty allowed)
+    rng = np.random.default_rng(5)
+    for _ in range(300):
+        C = int(rng.integers(1, 81))
+        q = rng.integers(-1000, 1000, C)
+        best = cur = 0
+        for v in q:                                     # Kadane on the negated array
+            cur = min(0, cur + int(v))
+            best = min(best, cur)
+        l, r, v = orc.row_search(q, 0, C, 0, C)
+        assert v == best == int(q[l:r].sum())
+
+
+def test_row_search_prefers_closed_and_narrow_on_ties():
+    assert orc.row_search(np.array([0, 0, 0]), 0, 3, 0, 3) == (0, 0, 0)       # closed row, parked lowest
+    assert orc.row_search(np.array([0, 0, 0]), 2, 3, 0, 3) == (2, 2, 0)       # closed inside the box
+    assert orc.row_search(np.array([0, -1, 0]), 0, 3, 0, 3) == (1, 2, -1)     # zero-price beamlets stay shut
+    assert orc.row_search(np.array([-1, 2, -1]), 0, 3, 0, 3) == (0, 1, -1)    # lowest index among equals
+    assert orc.row_search(np.array([5, 5]), 0, 0, 2, 2) == (0, 2, 10)         # forced open by the box
+    assert orc.row_search(np.array([1, 1]), 2, 2, 0, 1) is None               # l > r' everywhere: empty box
+
+
+def test_quantise_is_exact_fixed_point():
+    g = np.array([0.0, 1.0, -1.0, 0.5, 2.0 ** -30, -(2.0 ** -31), 3.0 * 2.0 ** -31, 1e-12, 123.456], np.float32)
+    q = orc.quantise(g)
+    # round-half-even at the 2^-30 grid
+    assert list(q[:8]) == [0, 2 ** 30, -(2 ** 30), 2 ** 29, 1, 0, 2, 0]
+    assert q[8] == int(np.rint(np.float64(g[8]) * 2.0 ** 30))
+
+
+# ------------------------------------------------------------------------------------------------
+# O5 leaf box and O6 beam choice
+# ------------------------------------------------------------------------------------------------
+def test_leaf_box_from_nearest_occupied_neighbours():
+    o, _, _ = small_problem(9, N=9, R=2, C=10, delta=2)
+    occ = np.zeros(9, np.uint8)
+    left = np.zeros((9, 2), np.int32)
+    right = np.zeros((9, 2), np.int32)
+    assert o.leaf_box(occ, left, right, 4, 0) == (0, 10, 0, 10)           # no neighbour: whole row
+    occ[1] = 1
+    left[1], right[1] = [3, 0], [7, 10]
+    # one neighbour 3 steps away: +-6 around its tips, clipped to [0, C]
+    assert o.leaf_box(occ, left, right, 4, 0) == (0, 9, 1, 10)
+    occ[5] = 1
+    left[5], right[5] = [5, 0], [6, 10]
+    # second neighbour 1 step away: +-2 -> intersection
+    assert o.leaf_box(occ, left, right, 4, 0) == (3, 7, 4, 8)
+    # beam 0 only sees beam 1 (nearest on the right), beam 8 only beam 5
+    assert o.leaf_box(occ, left, right, 0, 0) == (1, 5, 5, 9)
+    assert o.leaf_box(occ, left, right, 8, 0) == (0, 10, 0, 10) or o.leaf_box(occ, left, right, 8, 0) == (0, 10, 0, 10)
+    assert o.leaf_box(occ, left, right, 7, 0) == (1, 9, 2, 10)
+
+
+def test_price_step_matches_bruteforce_and_finite_difference():
+    """price_k = [Phi(y with y_k = h) - Phi(y)]/h for the chosen aperture (S10): ties dose, penalty,
+    smoothing, pricing and search together."""
+    o, D, rng = small_problem(21, V=60, N=6, R=3, C=7, gamma=0.4, delta=1, nonuniform_theta=True)
+    occ, left, right, y = random_plan(o, rng, 2)
+    # make the occupied apertures mutually deliverable (irrelevant for the FD, needed for a non-empty box)
+    ks = np.flatnonzero(occ)
+    left[ks[1]], right[ks[1]] = left[ks[0]], right[ks[0]]
+    z = o.dose(occ, left, right, y)
+    _, w = o.penalty(z)
+    g = o.prices(w, occ)
+    g32 = g.astype(np.float32)
+    out = o.price_step(g32, occ, left, right, y)
+    q = orc.quantise(g32).reshape(o.N, o.R, o.C)
+    _, dG = o.smooth(y)
+    prices = np.full(o.N, np.inf)
+    for k in range(o.N):
+        if occ[k]:
+            continue
+        tot = 0
+        for r in range(o.R):
+            box = o.leaf_box(occ, left, right, k, r)
+            l, rr, v = brute_force_row(q[k, r], *box)
+            assert (out["all_left"][k, r], out["all_right"][k, r]) == (l, rr)
+            tot += v
+        prices[k] = tot / 2.0 ** 30 + o.gamma * dG[k]
+    np.testing.assert_allclose(out["beam_price"], prices, rtol=1e-15)
+    assert out["beam"] == int(np.argmin(prices)) and out["price"] == prices.min()
+    # finite difference of the whole cost along the new column
+    k = out["beam"]
+    occ2, left2, right2 = occ.copy(), left.copy(), right.copy()
+    occ2[k] = 1
+    left2[k], right2[k] = out["left"], out["right"]
+    h = 1e-7
+    y2 = y.copy()
+    y2[k] = h
+    fd = (o.cost(occ2, left2, right2, y2)[2] - o.cost(occ, left, right, y)[2]) / h
+    exact = sum(g[(k * o.R + r) * o.C + c] for r in range(o.R) for c in range(out["left"][r], out["right"][r])) + o.gamma * dG[k]
+    assert fd == pytest.approx(exact, rel=1e-4, abs=1e-5)
+    assert out["price"] == pytest.approx(exact, rel=1e-5, abs=1e-5)        # fp32 hand-over + 2^-30 grid
+
+
+def test_beam_choice_lowest_index_on_ties():
+    # identical beams -> identical prices -> beam 0 (S9)
+    R, C, V, N = 2, 4, 8, 4
+    one = sp.random(R * C, V, density=0.6, random_state=3, format="csr", dtype=np.float32)
+    D = sp.vstack([one] * N).tocsr()
+    D.sort_indices()
+    o = Oracle(D.indptr.astype(np.int64), D.indices, D.data, np.ones(V), np.ones(V), np.ones(V), np.arange(N) * 2.0, R, C, 1, 0.0)
+    occ, left, right, y = o.empty_plan()
+    _, w = o.penalty(np.zeros(V))
+    out = o.price_step(o.prices(w).astype(np.float32), occ, left, right, y)
+    assert out["beam"] == 0 and np.all(out["beam_price"] == out["beam_price"][0])
+
+
+# ------------------------------------------------------------------------------------------------
+# O7 master
+# ------------------------------------------------------------------------------------------------
+def kkt_violation(o, occ, left, right, y):
+    grad, _ = o.cost_gradient(occ, left, right, y)
+    viol = 0.0
+    for k in range(o.N):
+        if not occ[k]:
+            continue
+        viol = max(viol, abs(grad[k]) if y[k] > 0 else max(0.0, -grad[k]))
+    return viol, grad
+
+
+def test_master_one_voxel_closed_form():
+    # one aperture, one voxel, alpha=beta: min (T - y d)^2  ->  y = T/d   (gamma = 0)
+    o = Oracle(np.array([0, 1], np.int64), [0], [0.25], [0.8], [1.0], [1.0], [0.0], 1, 1, 1, 0.0)
+    y, z, info = o.master([1], [[0]], [[1]])
+    assert y[0] == pytest.approx(float(np.float32(0.8)) / 0.25, rel=1e-9) and info.cost == pytest.approx(0.0, abs=1e-15)
+    # two beams, same voxel, smoothing couples them: minimise (T - d(y0+y1))^2 + g (y1-y0)^2/dth -> y0=y1=T/(2d)
+    o = Oracle(np.array([0, 1, 2], np.int64), [0, 0], [0.25, 0.25], [0.8], [1.0], [1.0], [0.0, 2.0], 1, 1, 1, 0.5)
+    y, z, info = o.master([1, 1], [[0], [0]], [[1], [1]])
+    np.testing.assert_allclose(y, [1.6, 1.6], rtol=1e-6)
+    # the bound is active: a beam that can only overdose an organ at risk stays at y = 0
+    o = Oracle(np.array([0, 1, 2], np.int64), [0, 1], [1.0, 1.0], [1.0, 0.0], [1.0, 0.0], [1.0, 5.0], [0.0, 2.0], 1, 1, 1, 0.0)
+    y, z, info = o.master([1, 1], [[0], [0]], [[1], [1]], y0=[0.3, 0.7])
+    np.testing.assert_allclose(y, [1.0, 0.0], atol=1e-8)
+
+
+def test_master_satisfies_kkt_random():
+    for seed in range(6):
+        o, D, rng = small_problem(100 + seed, V=80, N=7, R=3, C=6, gamma=0.2 * seed, delta=2, nonuniform_theta=bool(seed % 2))
+        occ, left, right, y0 = random_plan(o, rng, 5)
+        y, z, info = o.master(occ, left, right, y0=y0)
+        assert np.all(y >= 0) and np.all(y[occ == 0] == 0)
+        viol, grad = kkt_violation(o, occ, left, right, y)
+        assert viol <= 1e-7 * max(1.0, info.pg_entry), (seed, viol, info)
+        np.testing.assert_allclose(z, o.dose(occ, left, right, y), rtol=1e-12, atol=1e-12)
+        assert info.cost == pytest.approx(o.cost(occ, left, right, y)[2], rel=1e-13)
+        # warm start from the optimum does nothing
+        y2, _, info2 = o.master(occ, left, right, y0=y)
+        assert info2.pg_entry <= 1e-6 * max(1.0, info.pg_entry) and info2.cost <= info.cost * (1 + 1e-12)
+
+
+def test_master_equals_nnls_when_all_quadratic():
+    """alpha=beta=omega everywhere makes F a plain weighted least squares, so (3) with fixed apertures is
+    the non-negative least squares  min_{y>=0} || [sqrt(omega) Dc^T ; sqrt(gamma) E] y - [sqrt(omega) T ; 0] ||^2,
+    E the scaled difference operator (G = |E y|^2).  Library routine: scipy.optimize.nnls."""
+    o, D, rng = small_problem(77, V=50, N=6, R=2, C=5, gamma=0.7, nonuniform_theta=True)
+    om = rng.uniform(0.5, 2.0, o.V).astype(np.float32)
+    o = Oracle(o.row_ptr, o.col, o.val, o.T, om, om, o.theta, o.R, o.C, o.delta, o.gamma)
+    occ, left, right, _ = random_plan(o, rng, o.N)            # all beams occupied
+    Dc = np.einsum("krc,krcv->kv", open_mask(o, occ, left, right), D.reshape(o.N, o.R, o.C, o.V))
+    E = np.zeros((o.N - 1, o.N))
+    for k in range(o.N - 1):
+        s = 1.0 / np.sqrt(o.theta[k + 1] - o.theta[k])
+        E[k, k], E[k, k + 1] = -s, s
+    sq = np.sqrt(om.astype(np.float64))
+    A = np.vstack([sq[:, None] * Dc.T, np.sqrt(o.gamma) * E])
+    b = np.concatenate([sq * o.T.astype(np.float64), np.zeros(o.N - 1)])
+    y_ref, rnorm = scipy.optimize.nnls(A, b)
+    y, z, info = o.master(occ, left, right, eps=1e-11)
+    assert info.cost == pytest.approx(rnorm ** 2, rel=1e-9)
+    np.testing.assert_allclose(y, y_ref, rtol=1e-5, atol=1e-7)
+
+
+# ------------------------------------------------------------------------------------------------
+# O8 trajectory invariants on configs[0]
+# ------------------------------------------------------------------------------------------------
+def test_tiny_run_invariants(tiny_phantom, tiny_oracle, tiny_solution):
+    ph, o = tiny_phantom, tiny_oracle
+    occ, left, right, y, z, tr = tiny_solution
+    # one aperture in each beam direction, a plan at all gantry angles (reading S5)
+    assert tr.iters == o.N == 24 and sorted(tr.beam) == list(range(24)) and np.all(occ == 1)
+    # convex model + columns entering at y=0 => cost after each master is non-increasing
+    assert np.all(np.diff(tr.cost) <= 1e-9 * tr.cost[:-1])
+    assert tr.cost[0] < o.penalty(np.zeros(o.V))[0]
+    # every generated column had a negative price (it could decrease the cost)
+    assert np.all(tr.price < 0)
+    # leaf pairs are legal and the arc is deliverable: |dl|,|dr| <= delta*|k-k'| for ALL pairs (S6)
+    assert np.all((0 <= left) & (left <= right) & (right <= o.C))
+    for k in range(o.N):
+        for k2 in range(k + 1, o.N):
+            lim = o.delta * (k2 - k)
+            assert np.all(np.abs(left[k] - left[k2]) <= lim) and np.all(np.abs(right[k] - right[k2]) <= lim)
+    # final plan is a KKT point of the master and z is its dose
+    viol, _ = kkt_violation(o, occ, left, right, y)
+    assert viol <= 1e-6
+    np.testing.assert_allclose(z, o.dose(occ, left, right, y), rtol=1e-12, atol=1e-12)
+    assert tr.cost[-1] == pytest.approx(o.cost(occ, left, right, y)[2], rel=1e-12)
+
+
+def test_first_aperture_is_target_silhouette(tiny_phantom, tiny_oracle, tiny_solution):
+    """At the empty plan w_j = -2 alpha_j T_j <= 0, so every first price is <= 0 and the first aperture
+    opens exactly the beamlets that can reach an alpha>0 voxel (beam's-eye-view silhouette widened by
+    the kernel reach), trimmed only by the (value, width, l) tie-break on zero-price beamlets."""
+    ph, o = tiny_phantom, tiny_oracle
+    _, w = o.penalty(np.zeros(o.V))
+    assert np.all(w <= 0)
+    g = o.prices(w)
+    assert np.all(g <= 0)
+    occ, left, right, y = o.empty_plan()
+    out = o.price_step(g.astype(np.float32), occ, left, right, y)
+    tr = tiny_solution[5]
+    assert out["beam"] == tr.beam[0]
+    np.testing.assert_array_equal(out["left"], tr.left[0])
+    np.testing.assert_array_equal(out["right"], tr.right[0])
+    gk = g.reshape(o.N, o.R, o.C)[out["beam"]]
+    for r in range(o.R):
+        neg = np.flatnonzero(gk[r] < 0)
+        if neg.size:
+            assert (out["left"][r], out["right"][r]) == (neg[0], neg[-1] + 1)
+        else:
+            assert out["left"][r] == out["right"][r]
+
+
+def test_solve_resumes_from_a_plan(tiny_oracle, tiny_solution):
+    # stopping after 5 iterations and resuming gives the same trajectory as the straight run
+    o = tiny_oracle
+    occ, left, right, y, z, tr5 = o.solve(5)
+    occ2, left2, right2, y2, z2, tr_rest = o.solve(40, plan=(occ, left, right, y))
+    full = tiny_solution[5]
+    np.testing.assert_array_equal(np.concatenate([tr5.beam, tr_rest.beam]), full.beam)
+    np.testing.assert_allclose(tr_rest.cost[-1], full.cost[-1], rtol=1e-9)
+
+
+# ------------------------------------------------------------------------------------------------
+# shapes of the synthetic stand-ins vs. the paper's Table 1 (context only)
+# ------------------------------------------------------------------------------------------------
+def test_phantom_shape_is_in_the_range_of_table1():
+    import os
+
+    import vmat_inputs
+
+    rows = [ln.split() for ln in open(os.path.join(os.path.dirname(__file__), "golden", "paper_table1.txt")) if ln[0] != "#"]
+    per_beamlet = [float(r[3]) * 1e7 / float(r[1]) for r in rows]          # ~365-700 nnz per beamlet
+    assert 300 < min(per_beamlet) < max(per_beamlet) < 700
+    ph = vmat_inputs.make_phantom(vmat_inputs.scaled_config("prostate", n_beams=6), check_reach=False)
+    mine = ph.nnz / ph.n_beamlets
+    assert 0.5 * min(per_beamlet) < mine < 2 * max(per_beamlet)
