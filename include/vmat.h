@@ -1,0 +1,187 @@
+/*
+ * vmat.h — C ABI of the B200-native column-generation VMAT hot path.
+ *
+ * Method: Men, Romeijn, Jia, Jiang, "Ultra-fast treatment plan optimization for VMAT"
+ * (arxiv 1005.4396).  Citations "PAPER.md:N" are lines of the paper text; "S<n>" are the
+ * readings of DESIGN.md section 3 taken where the paper is silent.
+ *
+ * One column-generation iteration is
+ *   (a) dose      z_j = sum_k y_k sum_{i in A_k} D_ij
+ *   (b) gradient  w_j = dF/dz_j of the one-sided quadratic penalty (Eq. 1),
+ *                 s_k = gamma dG/dy_k of the dose-rate smoothing term (Eq. 2)
+ *   (c) pricing   g_i = sum_j D_ij w_j for every beamlet of every un-occupied beam
+ *   (d) search    per leaf row the contiguous open interval of least total price inside the
+ *                 leaf-travel box, per-beam sum, best un-occupied beam
+ *   (e) master    min_{y>=0} F(z(y)) + gamma G(y) over the generated apertures by gradient
+ *                 projection                                        (Eq. 3 :86-91)
+ * Every step runs in hand-written sm_100a CUDA kernels on ONE GPU.  There is no CPU fallback:
+ * without a CUDA device every compute entry point returns VMAT_ECUDA.
+ *
+ * Conventions
+ *   sizes      V voxels, N beams (gantry angles), R leaf rows per beam, C beamlets per row,
+ *              B = N*R*C beamlets; beamlet id i = (k*R + r)*C + c.
+ *   leaves     a row's pair (left, right) = (l, r'), integers in [0, C]; column c is open iff
+ *              l <= c < r'; l == r' is a closed row parked at l (S8).
+ *   pointers   every pointer argument is marked HOST or DEVICE.  DEVICE pointers must belong to
+ *              the CUDA device that was current when vmat_create ran.
+ *   stream     all device work of a plan is ordered on the cudaStream_t given to vmat_create
+ *              (NULL = legacy default stream).  Calls that return host values synchronise that
+ *              stream before returning; the others are stream-ordered.
+ *   ownership  the caller owns every array it passes.  vmat_create copies / re-lays-out its
+ *              inputs and keeps no caller pointer.  The plan owns the device memory it
+ *              allocates and frees it in vmat_destroy.  Output buffers are caller-allocated.
+ *   threads    a plan is not thread-safe; different plans are independent.
+ *   errors     every call returns an int: VMAT_OK, VMAT_DONE, or a negative code; no exception
+ *              crosses the boundary; on error the out-parameters are unspecified but no memory
+ *              is leaked.  vmat_last_error gives a message.
+ */
+#ifndef VMAT_H
+#define VMAT_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define VMAT_OK       0
+#define VMAT_DONE     1   /* nothing to do: every beam already holds an aperture               */
+#define VMAT_EINVAL  (-1) /* null pointer, bad size, malformed CSR, NaN/Inf, negative weights,  */
+                          /* non-ascending theta, leaf pairs outside [0,C] or breaking travel   */
+#define VMAT_ENOMEM  (-2) /* host or device allocation failed                                   */
+#define VMAT_ECUDA   (-3) /* CUDA runtime error (message carries the CUDA error string)         */
+#define VMAT_ESTATE  (-4) /* call not valid in the plan's current state                         */
+
+#define VMAT_HOST    0
+#define VMAT_DEVICE  1
+
+#define VMAT_MAX_COLS 255  /* C <= 255: one warp scans one leaf row                             */
+
+typedef struct vmat_plan vmat_plan;          /* opaque; owns all device state */
+
+/* The optimisation problem of PAPER.md:69-93. */
+typedef struct {
+    int64_t n_voxels, n_beams, n_rows, n_cols;   /* V, N, R, C                                   */
+    /* D, the dose-deposition matrix, beamlet-major CSR.  mem_space says where
+     * row_ptr/col_idx/val/T/alpha/beta live (all six in the same space).                      */
+    const int64_t *row_ptr;   /* B+1, row_ptr[0] = 0, non-decreasing                            */
+    const int32_t *col_idx;   /* nnz voxel ids in [0,V), strictly ascending within a row        */
+    const float   *val;       /* nnz, finite                                                    */
+    const float   *T;         /* V prescription / threshold dose T_j (Eq. 1)                    */
+    const float   *alpha;     /* V underdose weight alpha_j >= 0                                */
+    const float   *beta;      /* V overdose weight  beta_j  >= 0                                */
+    const double  *theta_deg; /* HOST, N gantry angles in degrees, strictly ascending (S4)      */
+    int32_t max_leaf_travel;  /* Delta >= 0: beamlets a leaf may move per angular step (S6)     */
+    double  gamma;            /* weight of the smoothing term, >= 0 (Eq. 3)        */
+    int32_t mem_space;        /* VMAT_HOST or VMAT_DEVICE                                       */
+} vmat_problem;
+
+/* Tunables.  Zero-initialise, then call vmat_default_options. */
+typedef struct {
+    int32_t validate;          /* 1: check the CSR and the voxel arrays on the device (default 1) */
+    int32_t pricing_kernel;    /* 0 auto, 1 warp-per-beamlet LDG.128, 2 bulk-copy (TMA 1-D) staged */
+    int32_t dose_path;         /* 0 aperture columns (default), 1 direct fixed-point scatter      */
+    double  master_eps;        /* stop when max|projected gradient| <= eps*max(1, value at entry) */
+    int32_t master_max_inner;  /* cap on inner iterations of one master solve                     */
+    int32_t record_phases;     /* 1: vmat_solve brackets each phase with CUDA events              */
+} vmat_options;
+
+/* One deliverable aperture: a beam and one leaf pair per row. */
+typedef struct {
+    int32_t beam;       /* chosen beam k, -1 if none                                            */
+    double  price;      /* its reduced cost: sum of row minima + gamma dG/dy_k (S10)            */
+    int32_t *left;      /* HOST, R entries, caller-allocated                                    */
+    int32_t *right;     /* HOST, R entries, caller-allocated                                    */
+} vmat_aperture;
+
+typedef struct {
+    int32_t inner;          /* inner iterations done                                            */
+    int32_t backtracks;     /* step halvings                                                    */
+    int32_t stop_reason;    /* 0 converged, 1 iteration cap, 2 no descent, 3 line search failed,
+                               4 decrease below fp32 resolution                                 */
+    double  pg_entry, pg_exit;   /* max |projected gradient| at entry / exit                    */
+    double  F, G, cost;     /* at exit: F, G and F + gamma G                                    */
+} vmat_master_stats;
+
+typedef struct {
+    int32_t iters;          /* outer iterations done                                            */
+    double  us_total;       /* device time of the whole call (CUDA events)                      */
+    double  us_price, us_search, us_column, us_master;  /* per phase, only if record_phases     */
+    double  F, G, cost;     /* after the last master solve                                      */
+    /* optional per-iteration trace, HOST, caller-allocated with max_iters entries, or NULL    */
+    int32_t *beam;          /* chosen beam                                                      */
+    double  *price;         /* its price                                                        */
+    double  *trace_F, *trace_G, *trace_cost;   /* after each master solve                       */
+    int32_t *inner;         /* master inner iterations                                          */
+} vmat_solve_stats;
+
+typedef struct {
+    int64_t n_voxels, n_beams, n_rows, n_cols, n_beamlets;
+    int64_t nnz;            /* entries of D as given                                            */
+    int64_t nnz_padded;     /* entries of the device layout (rows padded to multiples of 4)     */
+    int64_t n_support;      /* voxels with a non-empty column of D                              */
+    int64_t device_bytes;   /* device memory owned by the plan                                  */
+} vmat_info;
+
+void vmat_default_options(vmat_options *opt);
+
+/* Build a plan from the problem statement of PAPER.md:69-93: validate, upload, re-lay-out D
+ * (beamlet-major CSR, rows padded to 16-byte multiples, voxel ids compacted to the support of
+ * D), allocate all state.  The plan starts empty: no beam occupied, y = 0, z = 0 (S1).
+ * stream: a cudaStream_t (void*).  *out is set only on VMAT_OK.                               */
+int vmat_create(const vmat_problem *problem, const vmat_options *options /* NULL = defaults */,
+                void *cuda_stream, vmat_plan **out);
+int vmat_destroy(vmat_plan *plan);                      /* NULL-safe */
+int vmat_get_info(const vmat_plan *plan, vmat_info *out);
+
+/* Steps (a)+(b) for the plan's current apertures and dose rates.
+ * z_dev / w_dev: DEVICE, V floats, or NULL.  cost: HOST, {F, G, F + gamma G}, or NULL.        */
+int vmat_dose(vmat_plan *plan, float *z_dev, float *w_dev, double cost[3]);
+
+/* Steps (b)->(c)->(d): prices of all beamlets of un-occupied beams from the
+ * current penalty gradient, the row search, the beam choice.
+ *   w_override_dev  DEVICE V floats or NULL: use this gradient instead of the plan's own
+ *   g_override_dev  DEVICE B floats or NULL: skip the product and search these prices
+ *   g_out_dev       DEVICE B floats or NULL: receives the prices (0 at occupied beams)
+ *   out             receives the chosen aperture (may be NULL when commit = 1)
+ *   commit          0 report only; 1 occupy the beam with this aperture, y_k = 0
+ * Returns VMAT_DONE (out->beam = -1) when no beam is un-occupied.                             */
+int vmat_price(vmat_plan *plan, const float *w_override_dev, const float *g_override_dev,
+               float *g_out_dev, vmat_aperture *out, int commit);
+
+/* Step (c) alone: g = D w for the beamlets of un-occupied beams (0 elsewhere).
+ * w_dev DEVICE V floats (NULL = plan's own gradient), g_dev DEVICE B floats.  Stream-ordered. */
+int vmat_price_spmv(vmat_plan *plan, const float *w_dev, float *g_dev);
+
+/* Step (d) alone on given prices: row optimum of every un-occupied beam.
+ *   g_dev DEVICE B floats; all_left_dev / all_right_dev DEVICE N*R int32 (untouched at occupied
+ *   beams), beam_price_dev DEVICE N doubles (+inf at occupied beams); any output may be NULL.
+ * Stream-ordered; nothing is committed.                                                      */
+int vmat_leaf_search(vmat_plan *plan, const float *g_dev, int32_t *all_left_dev,
+                     int32_t *all_right_dev, double *beam_price_dev);
+
+/* Step (e): solve model (3) for y >= 0 over the occupied beams, warm-started
+ * from the plan's y.  Leaves z, w current.  out may be NULL.                                  */
+int vmat_master(vmat_plan *plan, vmat_master_stats *out);
+
+/* The column-generation loop (S5): up to max_iters iterations of
+ * price -> search -> occupy -> master, continuing from the plan's current state.  All iterations
+ * are enqueued without a host round trip; the call synchronises once at the end.             */
+int vmat_solve(vmat_plan *plan, int32_t max_iters, vmat_solve_stats *out);
+
+/* Plan state: occupied mask (N bytes), leaf pairs (N*R each), dose rates (N doubles); all HOST.
+ * vmat_set_plan validates 0 <= l <= r' <= C and the leaf-travel invariant between successive
+ * occupied beams.  Any pointer of vmat_get_plan may be NULL.                                  */
+int vmat_get_plan(vmat_plan *plan, uint8_t *occupied, int32_t *left, int32_t *right, double *y);
+int vmat_set_plan(vmat_plan *plan, const uint8_t *occupied, const int32_t *left, const int32_t *right,
+                  const double *y);
+
+/* Number of kernel launches this plan has issued since vmat_create (bench bookkeeping).     */
+int64_t vmat_launch_count(const vmat_plan *plan);
+
+const char *vmat_last_error(const vmat_plan *plan);     /* NULL plan: the last create error  */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* VMAT_H */

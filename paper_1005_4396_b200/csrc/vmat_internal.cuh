@@ -1,0 +1,151 @@
+// vmat_internal.cuh — plan state and kernel launchers shared by the translation units of
+// libvmat_b200.so.  Product code: shares nothing with oracle/ (DESIGN.md section 2).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/vmat.h"
+
+namespace vmat {
+
+constexpr int kChunk = 128;           // slots per master chunk: one warp of float4
+constexpr int kMasterThreads = 256;   // 8 warps split the beam loop of one chunk
+constexpr int kMasterWarps = kMasterThreads / 32;
+
+struct Sel {                          // device-side result of the beam choice (step d)
+    int32_t beam;
+    int32_t pad;
+    double price;
+};
+
+struct MasterOut {                    // device-side mirror of vmat_master_stats
+    int32_t inner, backtracks, stop_reason, pad;
+    double pg_entry, pg_exit, F, G, cost;
+};
+
+}  // namespace vmat
+
+struct vmat_plan {
+    // ---- sizes -------------------------------------------------------------------------
+    int64_t V = 0, N = 0, R = 0, C = 0, B = 0, RC = 0;
+    int64_t nnz = 0;        // entries of D as given
+    int64_t nq = 0;         // quads (groups of 4 entries) of the padded layout
+    int64_t S = 0;          // support: voxels with a non-empty column of D
+    int64_t Sp = 0;         // S rounded up to a multiple of kChunk (>= kChunk)
+    int32_t delta = 0;
+    double gamma = 0.0;
+    vmat_options opt{};
+    cudaStream_t stream = nullptr;
+    int sm_count = 0;
+    int device = 0;
+
+    // ---- D, beamlet-major padded CSR in slot space ------------------
+    uint32_t *rowq = nullptr;   // B+1 row starts in quads
+    float4 *val4 = nullptr;     // nq
+    int4 *col4 = nullptr;       // nq, slot ids
+    // bulk-copy pricing kernel: chunk table (beam-aligned groups of whole rows)
+    int32_t *chunk_row0 = nullptr;  // n_chunks+1 first row of each chunk
+    int64_t n_chunks = 0;
+    int32_t chunk_cap_q = 0;        // stage capacity in quads
+
+    // ---- voxel data --------------------------------------------------------------------
+    float *T_V = nullptr, *alpha_V = nullptr, *beta_V = nullptr;   // V each
+    int32_t *slot_of = nullptr;    // V, -1 outside the support
+    int32_t *voxel_of = nullptr;   // S
+    float *T_s = nullptr, *alpha_s = nullptr, *beta_s = nullptr;   // Sp each (padding: 0)
+    double F_out = 0.0;            // sum over voxels outside the support of alpha_j T_j^2 (+ beta part)
+
+    // ---- plan state on the device --------------------------------------------------------
+    uint8_t *occ = nullptr;        // N
+    int32_t *left = nullptr, *right = nullptr;   // N*R
+    double *y = nullptr;           // N
+    double *theta = nullptr;       // N
+
+    // ---- work arrays -----------------------------------------------------------------------
+    float *z_s = nullptr, *zn_s = nullptr, *q_s = nullptr, *w_s = nullptr, *wtmp_s = nullptr;  // Sp each
+    float *g = nullptr;            // B prices
+    float *Dd = nullptr;           // N x Sp aperture-dose columns d_k (row k valid iff col_valid[k])
+    unsigned long long *acc = nullptr;   // Sp fixed-point accumulator (all zero between uses)
+    double fx_scale = 1.0, fx_inv = 1.0;
+
+    int32_t *cand_left = nullptr, *cand_right = nullptr;   // N*R row optima of the last search
+    double *beam_price = nullptr;  // N
+    vmat::Sel *sel = nullptr;
+    unsigned int *ticket = nullptr;
+
+    double *partA = nullptr, *partF = nullptr, *partG = nullptr;   // master partial sums
+    int master_grid = 0;
+    size_t master_smem = 0;
+    vmat::MasterOut *mout = nullptr;
+    double *cost3 = nullptr;       // device {F, G, F+gamma G}
+    double *part_dose = nullptr;   // partial F sums of the dose kernel
+    int dose_blocks = 0;
+
+    // device trace of vmat_solve
+    int32_t *tr_beam = nullptr, *tr_inner = nullptr;
+    double *tr_price = nullptr, *tr_F = nullptr, *tr_G = nullptr, *tr_cost = nullptr;
+    int32_t tr_cap = 0;
+
+    // ---- host mirror ------------------------------------------------------------------------
+    std::vector<uint8_t> h_occ;        // occupied mask as last known to the host
+    std::vector<uint8_t> col_valid;    // Dd row k matches the plan's aperture of beam k
+    bool state_valid = false;          // z_s / w_s match (occ, leaves, y)
+    std::string err;
+    int64_t launches = 0;
+    int64_t bytes = 0;
+    std::vector<void *> allocs;
+};
+
+namespace vmat {
+
+// error plumbing -------------------------------------------------------------------------------
+int fail(vmat_plan *p, int code, const std::string &msg);
+int cuda_fail(vmat_plan *p, cudaError_t e, const char *what);
+void set_create_error(const std::string &msg);
+
+#define VMAT_CUDA(p, call)                                                  \
+    do {                                                                    \
+        cudaError_t e__ = (call);                                           \
+        if (e__ != cudaSuccess) return vmat::cuda_fail((p), e__, #call);    \
+    } while (0)
+
+template <typename T>
+int dev_alloc(vmat_plan *p, T **out, int64_t count) {
+    void *ptr = nullptr;
+    const size_t bytes = (size_t)(count > 0 ? count : 1) * sizeof(T);
+    cudaError_t e = cudaMalloc(&ptr, bytes);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return fail(p, VMAT_ENOMEM, std::string("cudaMalloc failed: ") + cudaGetErrorString(e));
+    }
+    p->allocs.push_back(ptr);
+    p->bytes += (int64_t)bytes;
+    *out = (T *)ptr;
+    return VMAT_OK;
+}
+
+// vmat_layout.cu: validation and the device layout of D ------------------------------------------
+int build_layout(vmat_plan *p, const vmat_problem *pb);
+
+// vmat_price.cu ---------------------------------------------------------------------------------------
+int launch_price_spmv(vmat_plan *p, const float *w_s, float *g);
+int build_chunk_table(vmat_plan *p, const std::vector<uint32_t> &h_rowq);
+
+// vmat_search.cu --------------------------------------------------------------------------------------
+int launch_leaf_search(vmat_plan *p, const float *g, int32_t *all_left, int32_t *all_right, double *beam_price,
+                       int commit, int trace_it);
+
+// vmat_master.cu ------------------------------------------------------------------------------------
+int master_configure(vmat_plan *p);
+int launch_column_build(vmat_plan *p, int beam /* -1: read p->sel */);
+int launch_dose_grad(vmat_plan *p);
+int launch_master(vmat_plan *p, int trace_it);
+int launch_expand(vmat_plan *p, const float *src_s, float *dst_V, int what /*0 z, 1 w*/);
+int launch_compress(vmat_plan *p, const float *src_V, float *dst_s);
+int launch_direct_dose(vmat_plan *p);
+
+}  // namespace vmat

@@ -1,0 +1,301 @@
+// vmat_layout.cu — vmat_create's device work: validate the problem, find the support of D,
+// re-lay-out D as a padded beamlet-major CSR in slot space.
+// Set-up code (runs once per plan); CUB's device scan is used for the two prefix sums.
+#include <cub/device/device_scan.cuh>
+
+#include <cmath>
+#include <cstring>
+
+#include "vmat_internal.cuh"
+
+namespace vmat {
+
+namespace {
+
+enum : unsigned {
+    kBadRowPtr = 1u,
+    kBadCol = 2u,
+    kBadOrder = 4u,
+    kBadVal = 8u,
+    kBadVoxel = 16u,
+};
+
+__global__ void k_check_row_ptr(const int64_t *__restrict__ row_ptr, int64_t B, int64_t nnz, unsigned *flags) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i > B) return;
+    const int64_t a = row_ptr[i];
+    bool bad = a < 0 || a > nnz;
+    if (i == 0 && a != 0) bad = true;
+    if (i == B && a != nnz) bad = true;
+    if (i < B && row_ptr[i + 1] < a) bad = true;
+    if (bad) atomicOr(flags, kBadRowPtr);
+}
+
+// one warp per row: column range, strict order, finite values; marks the support
+__global__ void k_check_rows(const int64_t *__restrict__ row_ptr, const int32_t *__restrict__ col,
+                             const float *__restrict__ val, int64_t B, int64_t V, int validate,
+                             int32_t *__restrict__ reach, unsigned *flags, unsigned *maxabs_bits) {
+    const int lane = threadIdx.x & 31;
+    const int64_t row = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (row >= B) return;
+    const int64_t a = row_ptr[row], b = row_ptr[row + 1];
+    unsigned bad = 0, mx = 0;
+    for (int64_t e = a + lane; e < b; e += 32) {
+        const int32_t c = col[e];
+        const float v = val[e];
+        if (c < 0 || c >= V) {
+            bad |= kBadCol;
+            continue;
+        }
+        if (validate) {
+            if (e > a && col[e - 1] >= c) bad |= kBadOrder;
+            if (!isfinite(v)) bad |= kBadVal;
+        }
+        reach[c] = 1;
+        const unsigned bits = __float_as_uint(fabsf(v));
+        mx = bits > mx ? bits : mx;
+    }
+    if (bad) atomicOr(flags, bad);
+    for (int o = 16; o; o >>= 1) {
+        const unsigned other = __shfl_xor_sync(0xffffffffu, mx, o);
+        mx = other > mx ? other : mx;
+    }
+    if (lane == 0 && mx) atomicMax(maxabs_bits, mx);
+}
+
+__global__ void k_check_voxels(const float *__restrict__ T, const float *__restrict__ alpha,
+                               const float *__restrict__ beta, int64_t V, unsigned *flags) {
+    const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= V) return;
+    const float t = T[j], a = alpha[j], b = beta[j];
+    if (!isfinite(t) || !isfinite(a) || !isfinite(b) || a < 0.f || b < 0.f) atomicOr(flags, kBadVoxel);
+}
+
+__global__ void k_row_quads(const int64_t *__restrict__ row_ptr, int64_t B, uint32_t *__restrict__ cnt) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i > B) return;
+    cnt[i] = i < B ? (uint32_t)((row_ptr[i + 1] - row_ptr[i] + 3) >> 2) : 0u;
+}
+
+// slot_of[j] = exclusive count if reachable else -1; voxel_of[slot] = j; slot-space T/alpha/beta;
+// per-block partial of the constant cost of the voxels outside the support (z_j = 0 there)
+__global__ void k_slots(const int32_t *__restrict__ reach, const int32_t *__restrict__ excl, int64_t V,
+                        const float *__restrict__ T, const float *__restrict__ alpha, const float *__restrict__ beta,
+                        int32_t *__restrict__ slot_of, int32_t *__restrict__ voxel_of, float *__restrict__ T_s,
+                        float *__restrict__ alpha_s, float *__restrict__ beta_s, double *__restrict__ part) {
+    __shared__ double red[256];
+    const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    double f = 0.0;
+    if (j < V) {
+        if (reach[j]) {
+            const int32_t s = excl[j];
+            slot_of[j] = s;
+            voxel_of[s] = (int32_t)j;
+            T_s[s] = T[j];
+            alpha_s[s] = alpha[j];
+            beta_s[s] = beta[j];
+        } else {
+            slot_of[j] = -1;
+            const double t = (double)T[j];
+            const double under = fmax(0.0, t), over = fmax(0.0, -t);   // Eq. 1 at z_j = 0
+            f = (double)alpha[j] * under * under + (double)beta[j] * over * over;
+        }
+    }
+    red[threadIdx.x] = f;
+    __syncthreads();
+    for (int o = 128; o; o >>= 1) {
+        if (threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) part[blockIdx.x] = red[0];
+}
+
+// one warp per row: copy into the padded layout, voxel ids -> slots.  Padding entries repeat the
+// row's last slot with value 0 so that every quad is a valid 16-byte load + 4 valid gathers.
+__global__ void k_fill_padded(const int64_t *__restrict__ row_ptr, const int32_t *__restrict__ col,
+                              const float *__restrict__ val, const int32_t *__restrict__ slot_of,
+                              const uint32_t *__restrict__ rowq, int64_t B, float *__restrict__ val_out,
+                              int32_t *__restrict__ col_out) {
+    const int lane = threadIdx.x & 31;
+    const int64_t row = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (row >= B) return;
+    const int64_t a = row_ptr[row], len = row_ptr[row + 1] - a;
+    const int64_t o = (int64_t)rowq[row] * 4, plen = (int64_t)(rowq[row + 1] - rowq[row]) * 4;
+    for (int64_t e = lane; e < plen; e += 32) {
+        const int64_t src = e < len ? e : len - 1;
+        col_out[o + e] = slot_of[col[a + src]];
+        val_out[o + e] = e < len ? val[a + src] : 0.f;
+    }
+}
+
+}  // namespace
+
+template <typename T>
+static int stage_in(vmat_plan *p, const T *src, int64_t count, int mem_space, const T **dev, std::vector<void *> &tmp) {
+    if (mem_space == VMAT_DEVICE) {
+        *dev = src;
+        return VMAT_OK;
+    }
+    void *d = nullptr;
+    cudaError_t e = cudaMalloc(&d, (size_t)(count > 0 ? count : 1) * sizeof(T));
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return fail(p, VMAT_ENOMEM, std::string("cudaMalloc (staging) failed: ") + cudaGetErrorString(e));
+    }
+    tmp.push_back(d);
+    VMAT_CUDA(p, cudaMemcpyAsync(d, src, (size_t)count * sizeof(T), cudaMemcpyHostToDevice, p->stream));
+    *dev = (const T *)d;
+    return VMAT_OK;
+}
+
+static int build_layout_impl(vmat_plan *p, const vmat_problem *pb, std::vector<void *> &tmp) {
+    const int64_t B = p->B, V = p->V;
+    cudaStream_t st = p->stream;
+    int rc;
+
+    // nnz = row_ptr[B]
+    int64_t nnz = 0;
+    if (pb->mem_space == VMAT_DEVICE) {
+        VMAT_CUDA(p, cudaMemcpyAsync(&nnz, pb->row_ptr + B, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+        VMAT_CUDA(p, cudaStreamSynchronize(st));
+    } else {
+        nnz = pb->row_ptr[B];
+    }
+    if (nnz < 0) return fail(p, VMAT_EINVAL, "row_ptr[B] is negative");
+    if ((nnz + 3) / 4 + B >= (int64_t)0xffffffffll) return fail(p, VMAT_EINVAL, "D too large: padded quads exceed 2^32");
+    p->nnz = nnz;
+
+    const int64_t *d_row_ptr;
+    const int32_t *d_col;
+    const float *d_val, *d_T, *d_alpha, *d_beta;
+    if ((rc = stage_in(p, pb->row_ptr, B + 1, pb->mem_space, &d_row_ptr, tmp))) return rc;
+    if ((rc = stage_in(p, pb->col_idx, nnz, pb->mem_space, &d_col, tmp))) return rc;
+    if ((rc = stage_in(p, pb->val, nnz, pb->mem_space, &d_val, tmp))) return rc;
+    if ((rc = stage_in(p, pb->T, V, pb->mem_space, &d_T, tmp))) return rc;
+    if ((rc = stage_in(p, pb->alpha, V, pb->mem_space, &d_alpha, tmp))) return rc;
+    if ((rc = stage_in(p, pb->beta, V, pb->mem_space, &d_beta, tmp))) return rc;
+
+    // scratch: flags (2 words), reach[V], excl[V], cnt[B+1]
+    unsigned *d_flags;
+    int32_t *d_reach, *d_excl;
+    uint32_t *d_cnt;
+    auto tmp_alloc = [&](void **ptr, size_t bytes) -> int {
+        cudaError_t e = cudaMalloc(ptr, bytes ? bytes : 1);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            return fail(p, VMAT_ENOMEM, std::string("cudaMalloc (scratch) failed: ") + cudaGetErrorString(e));
+        }
+        tmp.push_back(*ptr);
+        return VMAT_OK;
+    };
+    if ((rc = tmp_alloc((void **)&d_flags, 2 * sizeof(unsigned)))) return rc;
+    if ((rc = tmp_alloc((void **)&d_reach, (size_t)V * 4))) return rc;
+    if ((rc = tmp_alloc((void **)&d_excl, (size_t)V * 4))) return rc;
+    if ((rc = tmp_alloc((void **)&d_cnt, (size_t)(B + 1) * 4))) return rc;
+    VMAT_CUDA(p, cudaMemsetAsync(d_flags, 0, 2 * sizeof(unsigned), st));
+    VMAT_CUDA(p, cudaMemsetAsync(d_reach, 0, (size_t)V * 4, st));
+
+    // row_ptr must be sane before any kernel walks the rows
+    k_check_row_ptr<<<(unsigned)((B + 1 + 255) / 256), 256, 0, st>>>(d_row_ptr, B, nnz, d_flags);
+    unsigned h_flags[2] = {0, 0};
+    VMAT_CUDA(p, cudaMemcpyAsync(h_flags, d_flags, sizeof(h_flags), cudaMemcpyDeviceToHost, st));
+    VMAT_CUDA(p, cudaStreamSynchronize(st));
+    if (h_flags[0] & kBadRowPtr) return fail(p, VMAT_EINVAL, "row_ptr must start at 0, be non-decreasing and end at nnz");
+
+    k_check_rows<<<(unsigned)((B + 7) / 8), 256, 0, st>>>(d_row_ptr, d_col, d_val, B, V, p->opt.validate, d_reach,
+                                                         d_flags, d_flags + 1);
+    if (p->opt.validate) k_check_voxels<<<(unsigned)((V + 255) / 256), 256, 0, st>>>(d_T, d_alpha, d_beta, V, d_flags);
+    VMAT_CUDA(p, cudaMemcpyAsync(h_flags, d_flags, sizeof(h_flags), cudaMemcpyDeviceToHost, st));
+    VMAT_CUDA(p, cudaStreamSynchronize(st));
+    VMAT_CUDA(p, cudaGetLastError());
+    if (h_flags[0] & kBadCol) return fail(p, VMAT_EINVAL, "col_idx has a voxel id outside [0, n_voxels)");
+    if (h_flags[0] & kBadOrder) return fail(p, VMAT_EINVAL, "col_idx must be strictly ascending within a row");
+    if (h_flags[0] & kBadVal) return fail(p, VMAT_EINVAL, "val has a NaN or Inf");
+    if (h_flags[0] & kBadVoxel) return fail(p, VMAT_EINVAL, "T/alpha/beta must be finite with alpha, beta >= 0");
+
+    // fixed-point scale of the aperture-column accumulator: |val| * fx_scale <= 2^40
+    float maxabs;
+    std::memcpy(&maxabs, &h_flags[1], 4);
+    int e2 = 0;
+    if (maxabs > 0.f) std::frexp((double)maxabs, &e2);   // maxabs < 2^e2
+    p->fx_scale = std::ldexp(1.0, 40 - e2);
+    p->fx_inv = std::ldexp(1.0, e2 - 40);
+
+    // support: exclusive scan of the reach flags
+    size_t cub_bytes = 0, cub_bytes2 = 0;
+    cub::DeviceScan::ExclusiveSum(nullptr, cub_bytes, d_reach, d_excl, (int)V, st);
+    cub::DeviceScan::ExclusiveSum(nullptr, cub_bytes2, d_cnt, d_cnt, (int)(B + 1), st);
+    if (cub_bytes2 > cub_bytes) cub_bytes = cub_bytes2;
+    void *d_cub;
+    if ((rc = tmp_alloc(&d_cub, cub_bytes))) return rc;
+    VMAT_CUDA(p, cub::DeviceScan::ExclusiveSum(d_cub, cub_bytes, d_reach, d_excl, (int)V, st));
+    int32_t last_excl = 0, last_flag = 0;
+    if (V > 0) {
+        VMAT_CUDA(p, cudaMemcpyAsync(&last_excl, d_excl + V - 1, 4, cudaMemcpyDeviceToHost, st));
+        VMAT_CUDA(p, cudaMemcpyAsync(&last_flag, d_reach + V - 1, 4, cudaMemcpyDeviceToHost, st));
+    }
+    // row starts in quads
+    k_row_quads<<<(unsigned)((B + 1 + 255) / 256), 256, 0, st>>>(d_row_ptr, B, d_cnt);
+    if ((rc = dev_alloc(p, &p->rowq, B + 1))) return rc;
+    VMAT_CUDA(p, cub::DeviceScan::ExclusiveSum(d_cub, cub_bytes, d_cnt, p->rowq, (int)(B + 1), st));
+    uint32_t nq = 0;
+    VMAT_CUDA(p, cudaMemcpyAsync(&nq, p->rowq + B, 4, cudaMemcpyDeviceToHost, st));
+    VMAT_CUDA(p, cudaStreamSynchronize(st));
+    p->S = (int64_t)last_excl + last_flag;
+    p->Sp = ((p->S + kChunk - 1) / kChunk) * kChunk;
+    if (p->Sp < kChunk) p->Sp = kChunk;
+    p->nq = nq;
+
+    // slot maps and slot-space voxel parameters
+    if ((rc = dev_alloc(p, &p->T_V, V))) return rc;
+    if ((rc = dev_alloc(p, &p->alpha_V, V))) return rc;
+    if ((rc = dev_alloc(p, &p->beta_V, V))) return rc;
+    VMAT_CUDA(p, cudaMemcpyAsync(p->T_V, d_T, (size_t)V * 4, cudaMemcpyDeviceToDevice, st));
+    VMAT_CUDA(p, cudaMemcpyAsync(p->alpha_V, d_alpha, (size_t)V * 4, cudaMemcpyDeviceToDevice, st));
+    VMAT_CUDA(p, cudaMemcpyAsync(p->beta_V, d_beta, (size_t)V * 4, cudaMemcpyDeviceToDevice, st));
+    if ((rc = dev_alloc(p, &p->slot_of, V))) return rc;
+    if ((rc = dev_alloc(p, &p->voxel_of, p->Sp))) return rc;
+    if ((rc = dev_alloc(p, &p->T_s, p->Sp))) return rc;
+    if ((rc = dev_alloc(p, &p->alpha_s, p->Sp))) return rc;
+    if ((rc = dev_alloc(p, &p->beta_s, p->Sp))) return rc;
+    VMAT_CUDA(p, cudaMemsetAsync(p->voxel_of, 0, (size_t)p->Sp * 4, st));
+    VMAT_CUDA(p, cudaMemsetAsync(p->T_s, 0, (size_t)p->Sp * 4, st));
+    VMAT_CUDA(p, cudaMemsetAsync(p->alpha_s, 0, (size_t)p->Sp * 4, st));
+    VMAT_CUDA(p, cudaMemsetAsync(p->beta_s, 0, (size_t)p->Sp * 4, st));
+    const unsigned vblocks = (unsigned)((V + 255) / 256);
+    double *d_part;
+    if ((rc = tmp_alloc((void **)&d_part, (size_t)vblocks * 8))) return rc;
+    k_slots<<<vblocks, 256, 0, st>>>(d_reach, d_excl, V, d_T, d_alpha, d_beta, p->slot_of, p->voxel_of, p->T_s,
+                                     p->alpha_s, p->beta_s, d_part);
+    std::vector<double> h_part(vblocks);
+    VMAT_CUDA(p, cudaMemcpyAsync(h_part.data(), d_part, (size_t)vblocks * 8, cudaMemcpyDeviceToHost, st));
+
+    // padded CSR in slot space
+    if ((rc = dev_alloc(p, &p->val4, p->nq))) return rc;
+    if ((rc = dev_alloc(p, &p->col4, p->nq))) return rc;
+    k_fill_padded<<<(unsigned)((B + 7) / 8), 256, 0, st>>>(d_row_ptr, d_col, d_val, p->slot_of, p->rowq, B,
+                                                          (float *)p->val4, (int32_t *)p->col4);
+    VMAT_CUDA(p, cudaStreamSynchronize(st));
+    VMAT_CUDA(p, cudaGetLastError());
+    double f_out = 0.0;
+    for (unsigned b = 0; b < vblocks; ++b) f_out += h_part[b];
+    p->F_out = f_out;
+
+    if (p->opt.pricing_kernel == 2) {
+        std::vector<uint32_t> h_rowq((size_t)B + 1);
+        VMAT_CUDA(p, cudaMemcpyAsync(h_rowq.data(), p->rowq, (size_t)(B + 1) * 4, cudaMemcpyDeviceToHost, st));
+        VMAT_CUDA(p, cudaStreamSynchronize(st));
+        if ((rc = build_chunk_table(p, h_rowq))) return rc;
+    }
+    return VMAT_OK;
+}
+
+int build_layout(vmat_plan *p, const vmat_problem *pb) {
+    std::vector<void *> tmp;
+    const int rc = build_layout_impl(p, pb, tmp);
+    cudaStreamSynchronize(p->stream);
+    for (void *t : tmp) cudaFree(t);
+    return rc;
+}
+
+}  // namespace vmat

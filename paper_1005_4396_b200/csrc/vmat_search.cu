@@ -1,0 +1,325 @@
+// vmat_search.cu — step (d): per leaf row the contiguous open interval of least total price
+// inside the leaf-travel box, the per-beam sum and the choice of the best un-occupied beam
+// ("passing through all feasible beamlets in a row of a given beam from left to
+// right only once", "By checking the shapes of existing neighboring MLC apertures", "the most
+// promising MLC aperture from all un-occupied beam directions").
+//
+// Integer work throughout: prices are quantised to int64 fixed point, q_c = rn(g_c * 2^30), so
+// prefix sums are exact and independent of evaluation order (reading S9 / O5).  One
+// warp owns one leaf row: positions 0..C are dealt to the lanes in blocks of M, the prefix sums
+// P, the running maximum of P[l] over admissible l (later l wins ties) and the minimum of the key
+// (P[r']-P[l], r'-l, l) are warp-shuffle scans/reductions.  One block owns one beam; the last
+// block to finish picks the beam (smallest price, lowest k on ties) and commits it on request.
+#include <math_constants.h>
+
+#include "vmat_internal.cuh"
+
+namespace vmat {
+
+namespace {
+
+constexpr unsigned kFull = 0xffffffffu;
+constexpr int kSearchThreads = 256;
+
+__device__ __forceinline__ long long shfl_up_ll(long long v, int o) {
+    return __shfl_up_sync(kFull, v, o);
+}
+
+// Warp-cooperative search of one row.  All lanes return the same (value, l, r'); l = -1 if the box
+// admits no interval.
+template <int M>
+__device__ __forceinline__ void row_search_warp(const float *__restrict__ g_row, int C, int Lmin, int Lmax, int Rmin,
+                                                int Rmax, int lane, long long &value, int &l_out, int &r_out) {
+    // inclusive local prefix sums of the quantised prices; position p uses price p-1
+    long long loc[M];
+    long long sum = 0;
+#pragma unroll
+    for (int t = 0; t < M; ++t) {
+        const int pos = lane * M + t;
+        long long qv = 0;
+        if (pos >= 1 && pos <= C) qv = __double2ll_rn((double)g_row[pos - 1] * 1073741824.0);
+        sum += qv;
+        loc[t] = sum;
+    }
+    long long incl = sum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const long long n = shfl_up_ll(incl, o);
+        if (lane >= o) incl += n;
+    }
+    const long long off = incl - sum;   // P at the lane's first position = off + loc[0]
+
+    // lane aggregate of the running maximum of P[l] over admissible l, later l wins ties
+    int av = 0, ap = -1;
+    long long aP = 0;
+#pragma unroll
+    for (int t = 0; t < M; ++t) {
+        const int pos = lane * M + t;
+        const long long P = off + loc[t];
+        if (pos <= C && pos >= Lmin && pos <= Lmax && (!av || P >= aP)) {
+            av = 1;
+            aP = P;
+            ap = pos;
+        }
+    }
+    // inclusive scan of the aggregates across lanes: combine(earlier, later) keeps `later` iff it is
+    // valid and (earlier is invalid or later.P >= earlier.P)
+    int sv = av, sp = ap;
+    long long sP = aP;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int nv = __shfl_up_sync(kFull, sv, o), np = __shfl_up_sync(kFull, sp, o);
+        const long long nP = shfl_up_ll(sP, o);
+        if (lane >= o && !(sv && (!nv || sP >= nP))) {
+            sv = nv;
+            sP = nP;
+            sp = np;
+        }
+    }
+    int cv = __shfl_up_sync(kFull, sv, 1), cp = __shfl_up_sync(kFull, sp, 1);
+    long long cP = shfl_up_ll(sP, 1);
+    if (lane == 0) {
+        cv = 0;
+        cp = -1;
+        cP = 0;
+    }
+    // sweep the lane's positions: update the running maximum with pos as l, then try pos as r'
+    int bv = 0, bw = 0, bl = -1;
+    long long bval = 0;
+#pragma unroll
+    for (int t = 0; t < M; ++t) {
+        const int pos = lane * M + t;
+        const long long P = off + loc[t];
+        if (pos <= C && pos >= Lmin && pos <= Lmax && (!cv || P >= cP)) {
+            cv = 1;
+            cP = P;
+            cp = pos;
+        }
+        if (pos <= C && pos >= Rmin && pos <= Rmax && cv) {
+            const long long v = P - cP;
+            const int wd = pos - cp;
+            if (!bv || v < bval || (v == bval && (wd < bw || (wd == bw && cp < bl)))) {
+                bv = 1;
+                bval = v;
+                bw = wd;
+                bl = cp;
+            }
+        }
+    }
+    // lexicographic minimum of (value, width, l) over the lanes
+#pragma unroll
+    for (int o = 16; o; o >>= 1) {
+        const int ov = __shfl_xor_sync(kFull, bv, o), ow = __shfl_xor_sync(kFull, bw, o),
+                  ol = __shfl_xor_sync(kFull, bl, o);
+        const long long oval = __shfl_xor_sync(kFull, bval, o);
+        if (ov && (!bv || oval < bval || (oval == bval && (ow < bw || (ow == bw && ol < bl))))) {
+            bv = 1;
+            bval = oval;
+            bw = ow;
+            bl = ol;
+        }
+    }
+    value = bv ? bval : 0;
+    l_out = bv ? bl : -1;
+    r_out = bv ? bl + bw : -1;
+}
+
+struct SearchArgs {
+    const float *g;
+    const uint8_t *occ_in;
+    uint8_t *occ;
+    int32_t *left, *right;
+    double *y;
+    const double *theta;
+    int N, R, C, delta;
+    double gamma;
+    int32_t *cand_left, *cand_right;   // N*R row optima
+    double *beam_price;                // N
+    int32_t *out_left, *out_right;     // optional copies for the caller (may alias cand_*)
+    double *out_price;
+    Sel *sel;
+    unsigned int *ticket;
+    int commit;
+    int32_t *tr_beam;                  // trace slots (or null)
+    double *tr_price;
+    int trace_it;
+};
+
+template <int M>
+__global__ void __launch_bounds__(kSearchThreads) k_leaf_search(const SearchArgs a) {
+    __shared__ int s_km, s_kp, s_last;
+    __shared__ unsigned long long s_total;
+    __shared__ double s_price[kSearchThreads];
+    __shared__ int s_beam[kSearchThreads];
+    const int k = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int N = a.N, R = a.R, C = a.C;
+    const bool occupied = a.occ[k] != 0;
+
+    if (!occupied) {
+        if (tid == 0) {
+            s_km = -1;
+            s_kp = N;
+            s_total = 0ull;
+        }
+        __syncthreads();
+        // nearest occupied beam on each side (reading S6)
+        for (int kk = tid; kk < N; kk += kSearchThreads)
+            if (a.occ[kk]) {
+                if (kk < k) atomicMax(&s_km, kk);
+                if (kk > k) atomicMin(&s_kp, kk);
+            }
+        __syncthreads();
+        const int km = s_km, kp = s_kp;
+        for (int r = warp; r < R; r += kSearchThreads / 32) {
+            int Lmin = 0, Lmax = C, Rmin = 0, Rmax = C;
+            if (km >= 0) {
+                const int b = a.delta * (k - km), l = a.left[km * R + r], rr = a.right[km * R + r];
+                Lmin = max(Lmin, l - b);
+                Lmax = min(Lmax, l + b);
+                Rmin = max(Rmin, rr - b);
+                Rmax = min(Rmax, rr + b);
+            }
+            if (kp < N) {
+                const int b = a.delta * (kp - k), l = a.left[kp * R + r], rr = a.right[kp * R + r];
+                Lmin = max(Lmin, l - b);
+                Lmax = min(Lmax, l + b);
+                Rmin = max(Rmin, rr - b);
+                Rmax = min(Rmax, rr + b);
+            }
+            long long value;
+            int bl, br;
+            row_search_warp<M>(a.g + ((size_t)k * R + r) * C, C, Lmin, Lmax, Rmin, Rmax, lane, value, bl, br);
+            if (lane == 0) {
+                a.cand_left[k * R + r] = bl;
+                a.cand_right[k * R + r] = br;
+                if (a.out_left) {
+                    a.out_left[k * R + r] = bl;
+                    a.out_right[k * R + r] = br;
+                }
+                atomicAdd(&s_total, (unsigned long long)value);   // exact, order free
+            }
+        }
+        __syncthreads();
+        if (tid == 0) {
+            // price_k = 2^-30 * total + gamma * dG/dy_k, every operation individually rounded
+            // (Eq. 2; reading S10); same order of operations as the definition
+            double dG = 0.0;
+            if (k > 0)
+                dG = __dadd_rn(dG, __ddiv_rn(__dmul_rn(2.0, __dsub_rn(a.y[k], a.y[k - 1])),
+                                             __dsub_rn(a.theta[k], a.theta[k - 1])));
+            if (k + 1 < N)
+                dG = __dsub_rn(dG, __ddiv_rn(__dmul_rn(2.0, __dsub_rn(a.y[k + 1], a.y[k])),
+                                             __dsub_rn(a.theta[k + 1], a.theta[k])));
+            const double smooth = __dmul_rn(a.gamma, dG);
+            const double price = __dadd_rn(ldexp(__ll2double_rn((long long)s_total), -30), smooth);
+            a.beam_price[k] = price;
+            if (a.out_price) a.out_price[k] = price;
+        }
+    } else if (tid == 0) {
+        a.beam_price[k] = CUDART_INF;
+        if (a.out_price) a.out_price[k] = CUDART_INF;
+    }
+
+    // the last block to arrive chooses the beam
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) s_last = atomicAdd(a.ticket, 1u) == gridDim.x - 1;
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    double bp = CUDART_INF;
+    int bk = -1;
+    for (int kk = tid; kk < N; kk += kSearchThreads) {
+        const double pr = __ldcg(a.beam_price + kk);
+        if (!a.occ[kk] && (bk < 0 || pr < bp)) {   // ascending kk: the lowest index wins ties
+            bp = pr;
+            bk = kk;
+        }
+    }
+    s_price[tid] = bp;
+    s_beam[tid] = bk;
+    __syncthreads();
+    for (int o = kSearchThreads / 2; o; o >>= 1) {
+        if (tid < o) {
+            const double op = s_price[tid + o];
+            const int ok = s_beam[tid + o];
+            const int mk = s_beam[tid];
+            if (ok >= 0 && (mk < 0 || op < s_price[tid] || (op == s_price[tid] && ok < mk))) {
+                s_price[tid] = op;
+                s_beam[tid] = ok;
+            }
+        }
+        __syncthreads();
+    }
+    const int best = s_beam[0];
+    const double best_price = s_price[0];
+    if (tid == 0) {
+        a.sel->beam = best;
+        a.sel->price = best >= 0 ? best_price : 0.0;
+        *a.ticket = 0u;
+        if (a.tr_beam) {
+            a.tr_beam[a.trace_it] = best;
+            a.tr_price[a.trace_it] = best >= 0 ? best_price : 0.0;
+        }
+    }
+    if (a.commit && best >= 0) {
+        // occupy the beam with this aperture at y_k = 0
+        for (int r = tid; r < R; r += kSearchThreads) {
+            a.left[best * R + r] = __ldcg(a.cand_left + best * R + r);
+            a.right[best * R + r] = __ldcg(a.cand_right + best * R + r);
+        }
+        if (tid == 0) {
+            a.occ[best] = 1;
+            a.y[best] = 0.0;
+        }
+    }
+}
+
+}  // namespace
+
+int launch_leaf_search(vmat_plan *p, const float *g, int32_t *all_left, int32_t *all_right, double *beam_price,
+                       int commit, int trace_it) {
+    SearchArgs a;
+    a.g = g;
+    a.occ_in = p->occ;
+    a.occ = p->occ;
+    a.left = p->left;
+    a.right = p->right;
+    a.y = p->y;
+    a.theta = p->theta;
+    a.N = (int)p->N;
+    a.R = (int)p->R;
+    a.C = (int)p->C;
+    a.delta = p->delta;
+    a.gamma = p->gamma;
+    a.cand_left = p->cand_left;
+    a.cand_right = p->cand_right;
+    a.beam_price = p->beam_price;
+    a.out_left = all_left;
+    a.out_right = all_right;
+    a.out_price = beam_price;
+    a.sel = p->sel;
+    a.ticket = p->ticket;
+    a.commit = commit;
+    a.tr_beam = trace_it >= 0 ? p->tr_beam : nullptr;
+    a.tr_price = p->tr_price;
+    a.trace_it = trace_it;
+    const int M = (int)((p->C + 1 + 31) / 32);
+    const dim3 grid((unsigned)p->N), block(kSearchThreads);
+    switch (M) {
+        case 1: k_leaf_search<1><<<grid, block, 0, p->stream>>>(a); break;
+        case 2: k_leaf_search<2><<<grid, block, 0, p->stream>>>(a); break;
+        case 3: k_leaf_search<3><<<grid, block, 0, p->stream>>>(a); break;
+        case 4: k_leaf_search<4><<<grid, block, 0, p->stream>>>(a); break;
+        case 5: k_leaf_search<5><<<grid, block, 0, p->stream>>>(a); break;
+        case 6: k_leaf_search<6><<<grid, block, 0, p->stream>>>(a); break;
+        case 7: k_leaf_search<7><<<grid, block, 0, p->stream>>>(a); break;
+        case 8: k_leaf_search<8><<<grid, block, 0, p->stream>>>(a); break;
+        default: return fail(p, VMAT_EINVAL, "n_cols exceeds VMAT_MAX_COLS");
+    }
+    ++p->launches;
+    VMAT_CUDA(p, cudaGetLastError());
+    return VMAT_OK;
+}
+
+}  // namespace vmat

@@ -1,0 +1,343 @@
+"""GPU parity: the CUDA path (through the C ABI, include/vmat.h) against the CPU oracle, element by
+element on the same seeded inputs.  Protocol of DESIGN.md section 4:
+  P1 teacher-forced step parity  — leaf pairs / beam bit-exact on the oracle's fp32 prices;
+                                   z, w, g within 1e-4 (norm-wise, and per element against sum|D||w|)
+  P2 replay parity               — same aperture set => master cost within 1e-4 relative
+  P3 free run                    — final cost within 1e-4 when the aperture sequences coincide
+"""
+import numpy as np
+import pytest
+import scipy.sparse as sp
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-4          # BASELINE.json north_star: "dose, gradient and final cost within 1e-4 relative"
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def vm():
+    import paper_1005_4396_b200 as vm
+
+    vm.load_library()
+    return vm
+
+
+def relnorm(a, ref):
+    ref = np.asarray(ref, np.float64)
+    d = np.max(np.abs(np.asarray(a, np.float64) - ref)) if ref.size else 0.0
+    return d / max(np.max(np.abs(ref)), 1e-300) if ref.size else 0.0
+
+
+def make_plan(vm, o, **kw):
+    return vm.Plan.create(o.row_ptr, o.col, o.val, o.T, o.alpha, o.beta, o.theta, o.R, o.C, o.delta, o.gamma, **kw)
+
+
+def oracle_states(o, iters, every=1):
+    """Plan states along the oracle's own trajectory: list of (occ, left, right, y) after 0, every, 2*every.. iterations."""
+    occ, left, right, y = o.empty_plan()
+    states = [(occ.copy(), left.reshape(o.N, o.R).copy(), right.reshape(o.N, o.R).copy(), y.copy())]
+    plan = (occ, left, right, y)
+    done = 0
+    while done < iters:
+        occ, l, r, y, z, tr = o.solve(every, plan=plan)
+        if tr.iters == 0:
+            break
+        done += tr.iters
+        plan = (occ, l, r, y)
+        states.append((occ.copy(), l.copy(), r.copy(), y.copy()))
+    return states
+
+
+def random_problem(seed, V=300, N=7, R=4, C=11, density=0.15, gamma=0.3, delta=2):
+    from oracle import Oracle
+
+    rng = np.random.default_rng(seed)
+    B = N * R * C
+    dense = rng.random((B, V)).astype(np.float32) * (rng.random((B, V)) < density)
+    dense[rng.integers(0, B, 5)] = 0.0                       # empty rows
+    dense[:, rng.integers(0, V, 20)] = 0.0                   # voxels outside the support
+    csr = sp.csr_matrix(dense)
+    csr.sort_indices()
+    T = rng.uniform(0.2, 1.0, V).astype(np.float32)
+    alpha = ((rng.random(V) < 0.5) * rng.uniform(0.5, 2.0, V)).astype(np.float32)
+    beta = rng.uniform(0.1, 1.5, V).astype(np.float32)
+    theta = np.cumsum(rng.uniform(1.0, 3.0, N))
+    return Oracle(csr.indptr.astype(np.int64), csr.indices.astype(np.int32), csr.data.astype(np.float32),
+                  T, alpha, beta, theta, R, C, delta, gamma)
+
+
+# ------------------------------------------------------------------------------------------------
+# P1 (c): pricing product
+# ------------------------------------------------------------------------------------------------
+def check_prices(torch, plan, o, w64, occ):
+    w32 = w64.astype(np.float32)
+    g_ref = o.prices(w32.astype(np.float64), occ)
+    g = torch.empty(o.B, dtype=torch.float32, device="cuda")
+    plan.price_spmv(g, torch.from_numpy(w32).cuda())
+    g = g.cpu().numpy()
+    assert relnorm(g, g_ref) <= TOL
+    # per element against the magnitude sum_j |D_ij||w_j| (elementwise-relative is meaningless where g cancels)
+    D = sp.csr_matrix((o.val.astype(np.float64), o.col, o.row_ptr), shape=(o.B, o.V))
+    mag = abs(D) @ np.abs(w32.astype(np.float64))
+    mag[np.repeat(np.asarray(occ, bool), o.R * o.C)] = 0.0
+    assert np.all(np.abs(g - g_ref) <= 1e-5 * mag + 1e-30)
+    assert np.all(g[np.repeat(np.asarray(occ, bool), o.R * o.C)] == 0.0)
+
+
+def test_price_spmv_matches_oracle_tiny(torch_cuda, vm, tiny_phantom, tiny_oracle):
+    o = tiny_oracle
+    plan = make_plan(vm, o)
+    for occ, left, right, y in oracle_states(o, 12, every=4):
+        plan.set_plan(occ, left, right, y)
+        z = o.dose(occ, left, right, y)
+        _, w = o.penalty(z)
+        check_prices(torch_cuda, plan, o, w, occ)
+    plan.destroy()
+
+
+def test_price_spmv_random_and_ragged(torch_cuda, vm):
+    for seed in range(4):
+        o = random_problem(seed, C=(5, 11, 33, 70)[seed], R=(1, 4, 3, 2)[seed])
+        plan = make_plan(vm, o)
+        rng = np.random.default_rng(seed)
+        check_prices(torch_cuda, plan, o, rng.normal(size=o.V), np.zeros(o.N, np.uint8))
+        plan.destroy()
+
+
+# ------------------------------------------------------------------------------------------------
+# P1 (d): leaf search and beam choice, bit exact on the oracle's fp32 prices
+# ------------------------------------------------------------------------------------------------
+def check_search(torch, plan, o, occ, left, right, y, g32):
+    ref = o.price_step(g32, occ, left, right, y)
+    plan.set_plan(occ, left, right, y)
+    al = torch.full((o.N * o.R,), -7, dtype=torch.int32, device="cuda")
+    ar = torch.full((o.N * o.R,), -7, dtype=torch.int32, device="cuda")
+    bp = torch.zeros(o.N, dtype=torch.float64, device="cuda")
+    g_dev = torch.from_numpy(g32).cuda()
+    plan.leaf_search(g_dev, al, ar, bp)
+    al, ar, bp = al.cpu().numpy().reshape(o.N, o.R), ar.cpu().numpy().reshape(o.N, o.R), bp.cpu().numpy()
+    free = ~np.asarray(occ, bool)
+    assert np.array_equal(al[free], ref["all_left"][free])
+    assert np.array_equal(ar[free], ref["all_right"][free])
+    assert np.all(al[~free] == -7) and np.all(ar[~free] == -7)          # untouched at occupied beams
+    assert np.array_equal(bp, ref["beam_price"])                         # bit exact, +inf at occupied
+    ap = plan.price(g_override=g_dev, commit=False)
+    if ref["beam"] < 0:
+        assert ap is None
+    else:
+        assert ap.beam == ref["beam"] and ap.price == ref["price"]
+        assert np.array_equal(ap.left, ref["left"]) and np.array_equal(ap.right, ref["right"])
+
+
+def test_leaf_search_bit_exact_along_tiny_trajectory(torch_cuda, vm, tiny_oracle):
+    o = tiny_oracle
+    plan = make_plan(vm, o)
+    for occ, left, right, y in oracle_states(o, 24, every=3):
+        z = o.dose(occ, left, right, y)
+        _, w = o.penalty(z)
+        g32 = o.prices(w, occ).astype(np.float32)
+        check_search(torch_cuda, plan, o, occ, left, right, y, g32)
+    plan.destroy()
+
+
+@pytest.mark.parametrize("C", [1, 5, 31, 32, 33, 63, 64, 80, 97, 255])
+def test_leaf_search_bit_exact_random_prices(torch_cuda, vm, C):
+    # random prices with many exact zeros and repeated values (ties), random legal boxes from an oracle run
+    rng = np.random.default_rng(C)
+    o = random_problem(C, V=64, N=9, R=5, C=C, density=0.05, delta=int(rng.integers(0, 4)))
+    plan = make_plan(vm, o)
+    states = oracle_states(o, 6, every=2)
+    for occ, left, right, y in states:
+        for _ in range(3):
+            g = rng.normal(size=o.B).astype(np.float32)
+            g[rng.random(o.B) < 0.3] = 0.0
+            g = np.round(g * 4) / 4 if rng.random() < 0.5 else g          # coarse values -> many ties
+            check_search(torch_cuda, plan, o, occ, left, right, y, g.astype(np.float32))
+    plan.destroy()
+
+
+def test_all_beams_occupied_is_done(torch_cuda, vm):
+    o = random_problem(11, N=3)
+    occ, l, r, y, z, tr = o.solve(10)
+    assert occ.all()
+    plan = make_plan(vm, o)
+    plan.set_plan(occ, l, r, y)
+    assert plan.price(commit=False) is None
+    st = plan.solve(5)
+    assert st.iters == 0
+    plan.destroy()
+
+
+# ------------------------------------------------------------------------------------------------
+# P1 (a)+(b): dose and penalty gradient
+# ------------------------------------------------------------------------------------------------
+def check_dose(torch, plan, o, occ, left, right, y):
+    plan.set_plan(occ, left, right, y)
+    z = torch.empty(o.V, dtype=torch.float32, device="cuda")
+    w = torch.empty(o.V, dtype=torch.float32, device="cuda")
+    F, G, cost = plan.dose(z, w)
+    z_ref = o.dose(occ, left, right, y)
+    F_ref, w_ref = o.penalty(z_ref)
+    G_ref, _ = o.smooth(y)
+    assert relnorm(z.cpu().numpy(), z_ref) <= TOL
+    assert relnorm(w.cpu().numpy(), w_ref) <= TOL
+    assert abs(F - F_ref) <= TOL * max(abs(F_ref), 1e-12)
+    assert abs(G - G_ref) <= 1e-12 * max(abs(G_ref), 1.0)
+    assert abs(cost - (F_ref + o.gamma * G_ref)) <= TOL * abs(F_ref + o.gamma * G_ref)
+
+
+def test_dose_and_gradient_match_oracle_tiny(torch_cuda, vm, tiny_oracle):
+    o = tiny_oracle
+    plan = make_plan(vm, o)
+    for occ, left, right, y in oracle_states(o, 24, every=6):
+        check_dose(torch_cuda, plan, o, occ, left, right, y)
+    plan.destroy()
+
+
+def test_dose_random_problems_with_unreachable_voxels(torch_cuda, vm):
+    for seed in range(3):
+        o = random_problem(20 + seed)
+        plan = make_plan(vm, o)
+        for occ, left, right, y in oracle_states(o, 5, every=2):
+            check_dose(torch_cuda, plan, o, occ, left, right, y * 1.3)     # off-optimum dose rates too
+        plan.destroy()
+
+
+# ------------------------------------------------------------------------------------------------
+# P2: master problem on the same aperture set
+# ------------------------------------------------------------------------------------------------
+def check_master(plan, o, occ, left, right, y0):
+    y_ref, z_ref, info = o.master(occ, left, right, y0=y0, eps=1e-10)
+    plan.set_plan(occ, left, right, y0)
+    st = plan.master()
+    assert abs(st.cost - info.cost) <= TOL * abs(info.cost)
+    # the GPU's y is a KKT point of the oracle's objective, up to fp32 noise
+    _, _, _, y = plan.get_plan()
+    assert np.all(y >= 0) and np.all(y[~np.asarray(occ, bool)] == 0)
+    _, (_, _, cost_at_y) = o.cost_gradient(occ, left, right, y)
+    assert cost_at_y <= info.cost * (1 + TOL) + 1e-12
+    return st
+
+
+def test_master_matches_oracle_cost_tiny(torch_cuda, vm, tiny_oracle):
+    o = tiny_oracle
+    plan = make_plan(vm, o)
+    for occ, left, right, y in oracle_states(o, 24, every=6)[1:]:
+        check_master(plan, o, occ, left, right, np.zeros(o.N))            # cold start
+        check_master(plan, o, occ, left, right, y * 0.5)                   # warm start off the optimum
+    plan.destroy()
+
+
+def test_master_random_problems(torch_cuda, vm):
+    for seed in range(3):
+        o = random_problem(40 + seed, gamma=(0.0, 0.3, 2.0)[seed])
+        plan = make_plan(vm, o)
+        for occ, left, right, y in oracle_states(o, 7, every=3)[1:]:
+            check_master(plan, o, occ, left, right, np.zeros(o.N))
+        plan.destroy()
+
+
+# ------------------------------------------------------------------------------------------------
+# P3: free run of the whole loop
+# ------------------------------------------------------------------------------------------------
+def test_solve_free_run_tiny(torch_cuda, vm, tiny_oracle, tiny_solution):
+    o = tiny_oracle
+    occ_r, left_r, right_r, y_r, z_r, tr = tiny_solution
+    plan = make_plan(vm, o)
+    st = plan.solve(40)
+    assert st.iters == tr.iters == o.N                                    # one aperture per beam (S5)
+    occ, left, right, y = plan.get_plan()
+    assert occ.all()
+    # post-master cost is non-increasing (convexity; S2)
+    assert np.all(np.diff(st.trace_cost) <= 1e-5 * np.abs(st.trace_cost[:-1]))
+    same = np.array_equal(st.beam, tr.beam) and np.array_equal(left, left_r) and np.array_equal(right, right_r)
+    if same:
+        assert relnorm(st.trace_cost, tr.cost) <= TOL
+        assert abs(st.cost - tr.cost[-1]) <= TOL * abs(tr.cost[-1])
+    else:
+        # report the first diverging iteration: the two candidates must be within fp32 noise of a tie
+        it = int(np.argmax(st.beam != tr.beam)) if not np.array_equal(st.beam, tr.beam) else -1
+        pytest.fail(f"free run diverged from the oracle at iteration {it}: gpu {st.beam.tolist()} oracle {tr.beam.tolist()}")
+    # the leaf-travel invariant holds on the finished arc
+    for k in range(o.N - 1):
+        assert np.all(np.abs(left[k + 1] - left[k]) <= o.delta) and np.all(np.abs(right[k + 1] - right[k]) <= o.delta)
+    plan.destroy()
+
+
+def test_solve_is_reproducible(torch_cuda, vm, tiny_oracle):
+    o = tiny_oracle
+    runs = []
+    for _ in range(2):
+        plan = make_plan(vm, o)
+        st = plan.solve(40)
+        runs.append((st.trace_cost.copy(), plan.get_plan()))
+        plan.destroy()
+    assert np.array_equal(runs[0][0], runs[1][0])                         # bit identical costs
+    for a, b in zip(runs[0][1], runs[1][1]):
+        assert np.array_equal(a, b)
+
+
+def test_device_resident_inputs_give_the_same_plan(torch_cuda, vm, tiny_phantom, tiny_oracle):
+    o = tiny_oracle
+    a = make_plan(vm, o)
+    b = vm.Plan.from_phantom(tiny_phantom, device_arrays=True)
+    sa, sb = a.solve(5), b.solve(5)
+    assert np.array_equal(sa.trace_cost, sb.trace_cost) and np.array_equal(sa.beam, sb.beam)
+    a.destroy()
+    b.destroy()
+
+
+# ------------------------------------------------------------------------------------------------
+# boundary behaviour
+# ------------------------------------------------------------------------------------------------
+def test_create_rejects_malformed_problems(torch_cuda, vm):
+    o = random_problem(3)
+    args = dict(row_ptr=o.row_ptr.copy(), col_idx=o.col.copy(), val=o.val.copy(), T=o.T, alpha=o.alpha, beta=o.beta,
+                theta_deg=o.theta, n_rows=o.R, n_cols=o.C, max_leaf_travel=o.delta, gamma=o.gamma)
+
+    def expect_einval(**over):
+        kw = dict(args)
+        kw.update(over)
+        with pytest.raises(vm.VmatError) as e:
+            vm.Plan.create(**kw)
+        assert e.value.code == vm.VMAT_EINVAL
+
+    rp = o.row_ptr.copy(); rp[3] = rp[4] + 1
+    expect_einval(row_ptr=rp)
+    col = o.col.copy(); col[0] = o.V
+    expect_einval(col_idx=col)
+    col = o.col.copy()
+    i = int(np.argmax(np.diff(o.row_ptr) >= 2)); a = o.row_ptr[i]
+    col[a], col[a + 1] = col[a + 1], col[a]
+    expect_einval(col_idx=col)
+    v = o.val.copy(); v[5] = np.nan
+    expect_einval(val=v)
+    al = o.alpha.copy(); al[1] = -1.0
+    expect_einval(alpha=al)
+    expect_einval(theta_deg=o.theta[::-1].copy())
+    expect_einval(gamma=-0.1)
+    expect_einval(max_leaf_travel=-1)
+
+
+def test_set_plan_rejects_illegal_leaves(torch_cuda, vm):
+    o = random_problem(5, delta=1)
+    plan = make_plan(vm, o)
+    occ = np.zeros(o.N, np.uint8); occ[[1, 2]] = 1
+    left = np.zeros((o.N, o.R), np.int32); right = np.full((o.N, o.R), 3, np.int32)
+    y = np.zeros(o.N)
+    plan.set_plan(occ, left, right, y)                                      # legal
+    bad = right.copy(); bad[2, 0] = 6                                       # travel 3 > delta * 1
+    with pytest.raises(vm.VmatError):
+        plan.set_plan(occ, left, bad, y)
+    bad = left.copy(); bad[1, 1] = 4                                        # left > right
+    with pytest.raises(vm.VmatError):
+        plan.set_plan(occ, bad, right, y)
+    plan.destroy()
