@@ -1,0 +1,347 @@
+#!/usr/bin/env python
+"""Benchmark of the column-generation VMAT hot path (BASELINE.json: "CG iterations/s and plan wall-time;
+pricing SpMV GB/s vs B200 HBM peak").
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config prostate] [--impl reference]
+
+One STEP = one whole plan optimisation on the seeded synthetic phantom: every column-generation
+iteration (price -> leaf search -> aperture column -> master) until each beam holds an aperture
+(configs[1], prostate-like: 180 iterations).  `value` = column-generation iterations per second with
+D resident in HBM; `e2e` = the same through the C ABI from pinned HOST buffers (vmat_create's upload
+and re-layout, the solve, the read-back of the plan, vmat_destroy all inside the timed region).
+N > 1 runs N independent replicas (the path does not shard; no collective).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "column_generation_iterations_per_s"
+UNIT = "iterations/s"
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+# ncu --set full capture of k_price_spmv_warp on this workload, dram__bytes_read.sum + dram__bytes_write.sum
+# per launch, first pricing launch of a solve (all 180 beams un-occupied); see profiles/r01_price_spmv.md
+NCU_TRAFFIC_BYTES_FIRST_LAUNCH = None
+
+
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc = index, None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+            out, _ = self.proc.communicate()
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for line in out.strip().splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def pricing_algorithmic_bytes(nnz, B, V, N, iters):
+    """at outer iteration t the product streams the rows of the N-t un-occupied beams:
+    (N-t)/N * (8 nnz + 8 B + 4 B) + 4 V bytes (values + indices, row pointers, g out, one read of w)."""
+    return [(N - t) / N * (8.0 * nnz + 12.0 * B) + 4.0 * V for t in range(iters)]
+
+
+def make_inputs(config: str, seed: int = 0):
+    import vmat_inputs
+
+    t0 = time.perf_counter()
+    ph = vmat_inputs.make_phantom(config, seed=seed)
+    return ph, time.perf_counter() - t0
+
+
+def oracle_sample(ph, budget_s: float, chunk: int = 5):
+    """The oracle as it stands on the first iterations of the same workload, until `budget_s` of CPU work."""
+    from oracle import Oracle, vmat_oracle
+
+    o = Oracle.from_phantom(ph)
+    plan = None
+    done, t_used = 0, 0.0
+    cost = float("nan")
+    while done < ph.config.n_beams and t_used < budget_s:
+        t0 = time.perf_counter()
+        occ, l, r, y, z, tr = o.solve(chunk, plan=plan)
+        t_used += time.perf_counter() - t0
+        if tr.iters == 0:
+            break
+        done += tr.iters
+        cost = float(tr.cost[-1])
+        plan = (occ, l, r, y)
+    return done, t_used, vmat_oracle.num_threads(), cost
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle on the host cores, same config / metric / unit (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    ph, _ = make_inputs(args.config)
+    budget = args.ref_budget_s
+    for _ in range(args.warmup):
+        oracle_sample(ph, min(2.0, budget))
+    it_total, t_total, cores = 0, 0.0, 1
+    for _ in range(args.steps):
+        it, t, cores, _ = oracle_sample(ph, budget)
+        it_total += it
+        t_total += t
+    value = it_total / t_total
+    sample = (f"first {it_total // max(args.steps, 1)} of {ph.config.n_beams} column-generation iterations per step "
+              f"(~{budget:.0f} s of CPU work), oracle/vmat_oracle.c as it stands (fp64, OpenMP)")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_total / max(args.steps, 1),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(ph, args),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def workload_config(ph, args):
+    c = ph.config
+    return {
+        "workload": f"configs[{ {'tiny': 0, 'prostate': 1, 'hn': 2, 'stress': 4}[c.name] }] {c.name}-like phantom, "
+                    f"{c.n_beams} column-generation iterations per step",
+        "grid": list(c.grid), "voxel_mm": c.voxel_mm, "beams": c.n_beams, "leaf_rows": c.n_rows, "leaf_cols": c.n_cols,
+        "beamlets": ph.n_beamlets, "voxels": ph.n_voxels, "nnz": ph.nnz, "max_leaf_travel": c.max_leaf_travel,
+        "gamma": c.gamma, "seed": ph.seed,
+        "l2": "inputs larger than L2 (D streams >= 0.5 GB per iteration on average); no flush",
+        "parallelism": "replicas" if args.gpus > 1 else "single GPU",
+    }
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="prostate", choices=["tiny", "prostate", "hn", "stress"])
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--cpu-budget-s", type=float, default=15.0, help="CPU seconds for the cpu_baseline sample")
+    ap.add_argument("--ref-budget-s", type=float, default=15.0, help="CPU seconds per step of --impl reference")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "b200":
+        args.warmup = 3
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    import __graft_entry__ as entry
+
+    entry.build()
+    import paper_1005_4396_b200 as vm
+
+    ph, gen_s = make_inputs(args.config)
+    c = ph.config
+    iters = c.n_beams                      # S5: one aperture per beam
+    # pinned host copies of the problem (the e2e leg uploads from these every step)
+    host = [torch.from_numpy(a).pin_memory() for a in (ph.row_ptr, ph.col_idx, ph.val, ph.T, ph.alpha, ph.beta)]
+    h2d_bytes = int(sum(t.numel() * t.element_size() for t in host) + ph.theta_deg.nbytes)
+    d2h_bytes = int(c.n_beams * (1 + 8 + 2 * 4 * c.n_rows) + 3 * 8)
+
+    def create(record_phases=0):
+        opt = vm.default_options()
+        opt.record_phases = record_phases
+        return vm.Plan.create(*[t.numpy() for t in host], ph.theta_deg, c.n_rows, c.n_cols, c.max_leaf_travel, c.gamma,
+                              options=opt)
+
+    empty = (np.zeros(c.n_beams, np.uint8), np.zeros((c.n_beams, c.n_rows), np.int32),
+             np.zeros((c.n_beams, c.n_rows), np.int32), np.zeros(c.n_beams))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident leg: `value` -----------------------------------------------------------
+    t0 = time.perf_counter()
+    plan = create()
+    torch.cuda.synchronize()
+    create_ms = 1e3 * (time.perf_counter() - t0)
+    stream = torch.cuda.current_stream()
+    last = None
+    for _ in range(args.warmup):
+        plan.set_plan(*empty)
+        last = plan.solve(iters, trace=False)
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    barrier()
+    l0 = plan.launch_count
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record(stream)
+    done_iters = 0
+    for _ in range(args.steps):
+        plan.set_plan(*empty)
+        last = plan.solve(iters, trace=False)
+        done_iters += last.iters
+    ev1.record(stream)
+    barrier()
+    ms = ev0.elapsed_time(ev1)
+    launches = plan.launch_count - l0
+    if dist is not None:
+        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+        n = torch.tensor([done_iters, launches], device="cuda", dtype=torch.int64)
+        dist.all_reduce(n)
+        done_iters, launches = int(n[0].item()), int(n[1].item())
+    clocks = sampler.stop() if rank == 0 else None
+    value = done_iters / (ms * 1e-3)
+    final_cost = last.cost
+
+    # ---- per-phase device times (CUDA events on the plan's stream) and the pricing roofline -------
+    plan.destroy()
+    plan = create(record_phases=1)
+    plan.set_plan(*empty)
+    plan.solve(iters, trace=False)
+    ph_us = {"price": 0.0, "search": 0.0, "column": 0.0, "master": 0.0, "total": 0.0}
+    inner_total = 0
+    for _ in range(args.steps):
+        plan.set_plan(*empty)
+        st = plan.solve(iters, trace=True)
+        for k, v in (("price", st.us_price), ("search", st.us_search), ("column", st.us_column),
+                     ("master", st.us_master), ("total", st.us_total)):
+            ph_us[k] += v / args.steps
+        inner_total += int(st.inner.sum())
+    alg = pricing_algorithmic_bytes(ph.nnz, ph.n_beamlets, ph.n_voxels, c.n_beams, iters)
+    peak, peak_src = load_peaks()
+    achieved = sum(alg) / (ph_us["price"] * 1e-6) / 1e9
+    roofline = {
+        "kernel": "k_price_spmv_warp (pricing SpMV, step c)", "bound": "hbm", "achieved": achieved, "peak": peak,
+        "unit": "GB/s", "frac": achieved / peak, "frac_of_8TBs_nominal": achieved / 8000.0,
+        "traffic": NCU_TRAFFIC_BYTES_FIRST_LAUNCH, "peak_source": peak_src,
+        "algorithmic_bytes_per_launch_avg": sum(alg) / iters, "algorithmic_bytes_first_launch": alg[0],
+        "avg_launch_us": ph_us["price"] / iters, "launches_per_step": iters,
+        "how": "CUDA events on the plan's stream around every pricing launch of the phase-timed steps",
+    }
+    phases = {k + "_us_per_step": v for k, v in ph_us.items()}
+    phases["master_inner_iterations_per_step"] = inner_total / args.steps
+    info = {"nnz": plan.nnz, "nnz_padded": plan.nnz_padded, "support_voxels": plan.n_support,
+            "device_bytes": plan.device_bytes}
+    plan.destroy()
+
+    # ---- end-to-end leg from pinned host buffers ----------------------------------------------------
+    e2e = None
+    if not args.no_e2e:
+        def e2e_step():
+            p = create()
+            s = p.solve(iters, trace=False)
+            out = p.get_plan()
+            p.destroy()
+            return s, out
+
+        e2e_step()
+        barrier()
+        t0 = time.perf_counter()
+        n_e2e = max(1, min(args.steps, 3))
+        it_e2e = 0
+        for _ in range(n_e2e):
+            s, _ = e2e_step()
+            it_e2e += s.iters
+        barrier()
+        dt = time.perf_counter() - t0
+        if dist is not None:
+            t = torch.tensor([dt], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+            it_e2e *= world
+        e2e = {"value": it_e2e / dt, "unit": UNIT, "h2d_bytes_per_step": h2d_bytes, "d2h_bytes_per_step": d2h_bytes,
+               "ms_per_step": 1e3 * dt / n_e2e, "steps": n_e2e,
+               "what": "vmat_create from pinned host CSR + vmat_solve + vmat_get_plan + vmat_destroy, wall clock"}
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    cpu_baseline = None
+    if not args.no_cpu_baseline and world == 1:
+        it, t, cores, _ = oracle_sample(ph, args.cpu_budget_s)
+        cpu_baseline = {"value": it / t, "unit": UNIT, "cores": cores, "kind": "oracle",
+                        "sample": f"first {it} of {c.n_beams} column-generation iterations of the same phantom "
+                                  f"({t:.1f} s), oracle/vmat_oracle.c as it stands (fp64, OpenMP)"}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic", "config": workload_config(ph, args),
+        "plan_wall_time_ms": ms / args.steps, "final_cost": final_cost,
+        "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+        "phases": phases, "layout": info, "create_ms": create_ms, "generate_inputs_s": gen_s,
+        "paper_context": "PAPER.md:157 whole plan 18-31 s (CUDA, Tesla C1060) / 5-8 min (MATLAB, Xeon) on clinical "
+                         "cases of 1.8e7-5.5e7 non-zeros; different machine and data, not a target",
+    }
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
