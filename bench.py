@@ -148,6 +148,20 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def aggregate_over_ranks(ms, done_iters, launches, dist, device):
+    """Replicas: the job's time is the MAX over ranks of the device-timed region, its
+    work the SUM of the iterations (and kernel launches) every rank completed.  No data-path collective."""
+    if dist is None:
+        return float(ms), int(done_iters), int(launches)
+    import torch
+
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    n = torch.tensor([done_iters, launches], device=device, dtype=torch.int64)
+    dist.all_reduce(n)
+    return float(t.item()), int(n[0].item()), int(n[1].item())
+
+
 def workload_config(ph, args):
     c = ph.config
     return {
@@ -245,13 +259,7 @@ def main():
     barrier()
     ms = ev0.elapsed_time(ev1)
     launches = plan.launch_count - l0
-    if dist is not None:
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-        n = torch.tensor([done_iters, launches], device="cuda", dtype=torch.int64)
-        dist.all_reduce(n)
-        done_iters, launches = int(n[0].item()), int(n[1].item())
+    ms, done_iters, launches = aggregate_over_ranks(ms, done_iters, launches, dist, "cuda")
     clocks = sampler.stop() if rank == 0 else None
     value = done_iters / (ms * 1e-3)
     final_cost = last.cost
@@ -307,11 +315,7 @@ def main():
             it_e2e += s.iters
         barrier()
         dt = time.perf_counter() - t0
-        if dist is not None:
-            t = torch.tensor([dt], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
-            it_e2e *= world
+        dt, it_e2e, _ = aggregate_over_ranks(dt, it_e2e, 0, dist, "cuda")
         e2e = {"value": it_e2e / dt, "unit": UNIT, "h2d_bytes_per_step": h2d_bytes, "d2h_bytes_per_step": d2h_bytes,
                "ms_per_step": 1e3 * dt / n_e2e, "steps": n_e2e,
                "what": "vmat_create from pinned host CSR + vmat_solve + vmat_get_plan + vmat_destroy, wall clock"}

@@ -79,7 +79,8 @@ typedef struct {
 /* Tunables.  Zero-initialise, then call vmat_default_options. */
 typedef struct {
     int32_t validate;          /* 1: check the CSR and the voxel arrays on the device (default 1) */
-    int32_t pricing_kernel;    /* 0 auto, 1 warp-per-beamlet LDG.128, 2 bulk-copy (TMA 1-D) staged */
+    int32_t pricing_kernel;    /* 0 default; 1..5 lanes-per-beamlet x loads-in-flight variants of the
+                                  pricing product (32x2, 32x4, 16x2, 16x4, 8x4), for measurement   */
     int32_t dose_path;         /* 0 aperture columns (default), 1 direct fixed-point scatter      */
     double  master_eps;        /* stop when max|projected gradient| <= eps*max(1, value at entry) */
     int32_t master_max_inner;  /* cap on inner iterations of one master solve                     */

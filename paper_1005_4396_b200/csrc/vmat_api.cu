@@ -145,6 +145,7 @@ int vmat_create(const vmat_problem *pb, const vmat_options *options, void *cuda_
 #define A(ptr, n) \
     if ((rc = dev_alloc(p, &(ptr), (n)))) return bail(rc)
     A(p->occ, N);
+    A(p->free_list, N);
     A(p->left, NR);
     A(p->right, NR);
     A(p->y, N);
@@ -194,6 +195,7 @@ int vmat_create(const vmat_problem *pb, const vmat_options *options, void *cuda_
     if ((e = cudaMemcpyAsync(p->theta, pb->theta_deg, (size_t)N * 8, cudaMemcpyHostToDevice, st)) != cudaSuccess)
         return bail(cuda_fail(p, e, "cudaMemcpyAsync(theta)"));
     if ((rc = master_configure(p))) return bail(rc);
+    if ((rc = launch_free_list(p))) return bail(rc);
     if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return bail(cuda_fail(p, e, "cudaStreamSynchronize"));
     p->h_occ.assign((size_t)N, 0);
     p->col_valid.assign((size_t)N, 0);
@@ -244,7 +246,9 @@ int vmat_price_spmv(vmat_plan *p, const float *w_dev, float *g_dev) {
         if ((rc = launch_compress(p, w_dev, p->wtmp_s))) return rc;
         w_s = p->wtmp_s;
     } else if ((rc = ensure_state(p))) return rc;
-    return launch_price_spmv(p, w_s, g_dev);
+    // the kernel covers the un-occupied beams only: the caller's buffer gets its zeros here
+    VMAT_CUDA(p, cudaMemsetAsync(g_dev, 0, (size_t)p->B * 4, p->stream));
+    return launch_price_spmv(p, w_s, g_dev, (int)unoccupied(p));
 }
 
 int vmat_leaf_search(vmat_plan *p, const float *g_dev, int32_t *all_left_dev, int32_t *all_right_dev,
@@ -273,7 +277,8 @@ int vmat_price(vmat_plan *p, const float *w_override_dev, const float *g_overrid
             if ((rc = launch_compress(p, w_override_dev, p->wtmp_s))) return rc;
             w_s = p->wtmp_s;
         } else if ((rc = ensure_state(p))) return rc;
-        if ((rc = launch_price_spmv(p, w_s, p->g))) return rc;
+        if (g_out_dev) VMAT_CUDA(p, cudaMemsetAsync(p->g, 0, (size_t)p->B * 4, p->stream));
+        if ((rc = launch_price_spmv(p, w_s, p->g, (int)unoccupied(p)))) return rc;
         g = p->g;
     }
     if (g_out_dev && g_out_dev != g)
@@ -325,7 +330,8 @@ int vmat_master(vmat_plan *p, vmat_master_stats *out) {
 int vmat_solve(vmat_plan *p, int32_t max_iters, vmat_solve_stats *out) {
     if (!p) return VMAT_EINVAL;
     if (max_iters < 0) return fail(p, VMAT_EINVAL, "max_iters must be >= 0");
-    int64_t todo = unoccupied(p);
+    const int64_t n_free0 = unoccupied(p);
+    int64_t todo = n_free0;
     if (todo > max_iters) todo = max_iters;
     int rc;
     cudaStream_t st = p->stream;
@@ -367,7 +373,7 @@ int vmat_solve(vmat_plan *p, int32_t max_iters, vmat_solve_stats *out) {
     TRY(ensure_state(p));
     for (int64_t it = 0; it < todo; ++it) {
         if (phases) TRYC(cudaEventRecord(evs[it * 5 + 0], st));
-        TRY(launch_price_spmv(p, p->w_s, p->g));                                   // (c)
+        TRY(launch_price_spmv(p, p->w_s, p->g, (int)(n_free0 - it)));              // (c)
         if (phases) TRYC(cudaEventRecord(evs[it * 5 + 1], st));
         TRY(launch_leaf_search(p, p->g, nullptr, nullptr, nullptr, 1, (int)it));   // (d), commits
         if (phases) TRYC(cudaEventRecord(evs[it * 5 + 2], st));
@@ -471,7 +477,7 @@ int vmat_set_plan(vmat_plan *p, const uint8_t *occupied, const int32_t *left, co
     p->h_occ = oo;
     p->col_valid.assign((size_t)N, 0);
     p->state_valid = false;
-    return VMAT_OK;
+    return launch_free_list(p);
 }
 
 int64_t vmat_launch_count(const vmat_plan *p) { return p ? p->launches : 0; }

@@ -13,8 +13,15 @@
 namespace vmat {
 
 constexpr int kChunk = 128;           // slots per master chunk: one warp of float4
-constexpr int kMasterThreads = 256;   // 8 warps split the beam loop of one chunk
+constexpr int kGroup = 8;             // chunks a master block works on at a time
+constexpr int kMasterThreads = 512;   // 16 warps split the beam loop of one group of chunks
 constexpr int kMasterWarps = kMasterThreads / 32;
+constexpr int kOutPerThread = kGroup * kChunk / kMasterThreads;
+
+struct ColStat {                      // statistics of one aperture-dose column d_k (fixed-point units)
+    unsigned long long l1, linf;      // sum and max of |d_k|
+    int32_t clo, chi;                 // first and last chunk with a non-zero entry (INT_MAX, -1 if none)
+};
 
 struct Sel {                          // device-side result of the beam choice (step d)
     int32_t beam;
@@ -47,10 +54,6 @@ struct vmat_plan {
     uint32_t *rowq = nullptr;   // B+1 row starts in quads
     float4 *val4 = nullptr;     // nq
     int4 *col4 = nullptr;       // nq, slot ids
-    // bulk-copy pricing kernel: chunk table (beam-aligned groups of whole rows)
-    int32_t *chunk_row0 = nullptr;  // n_chunks+1 first row of each chunk
-    int64_t n_chunks = 0;
-    int32_t chunk_cap_q = 0;        // stage capacity in quads
 
     // ---- voxel data --------------------------------------------------------------------
     float *T_V = nullptr, *alpha_V = nullptr, *beta_V = nullptr;   // V each
@@ -61,6 +64,7 @@ struct vmat_plan {
 
     // ---- plan state on the device --------------------------------------------------------
     uint8_t *occ = nullptr;        // N
+    int32_t *free_list = nullptr;  // N: un-occupied beams, ascending (first N - #occupied entries valid)
     int32_t *left = nullptr, *right = nullptr;   // N*R
     double *y = nullptr;           // N
     double *theta = nullptr;       // N
@@ -77,7 +81,11 @@ struct vmat_plan {
     vmat::Sel *sel = nullptr;
     unsigned int *ticket = nullptr;
 
-    double *partA = nullptr, *partF = nullptr, *partG = nullptr;   // master partial sums
+    long long *accbuf = nullptr;       // 3 x (N + 2) fixed-point sums of the master kernel
+    unsigned int *phase = nullptr;     // rotation counter of accbuf
+    vmat::ColStat *colstat = nullptr;  // N
+    unsigned int *vbounds = nullptr;   // bit patterns of max|T|, max(alpha, beta)
+    float Tmax = 0.f, abmax = 0.f;
     int master_grid = 0;
     size_t master_smem = 0;
     vmat::MasterOut *mout = nullptr;
@@ -132,8 +140,8 @@ int dev_alloc(vmat_plan *p, T **out, int64_t count) {
 int build_layout(vmat_plan *p, const vmat_problem *pb);
 
 // vmat_price.cu ---------------------------------------------------------------------------------------
-int launch_price_spmv(vmat_plan *p, const float *w_s, float *g);
-int build_chunk_table(vmat_plan *p, const std::vector<uint32_t> &h_rowq);
+int launch_price_spmv(vmat_plan *p, const float *w_s, float *g, int n_free);
+int launch_free_list(vmat_plan *p);
 
 // vmat_search.cu --------------------------------------------------------------------------------------
 int launch_leaf_search(vmat_plan *p, const float *g, int32_t *all_left, int32_t *all_right, double *beam_price,

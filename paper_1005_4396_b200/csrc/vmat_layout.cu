@@ -281,12 +281,6 @@ static int build_layout_impl(vmat_plan *p, const vmat_problem *pb, std::vector<v
     for (unsigned b = 0; b < vblocks; ++b) f_out += h_part[b];
     p->F_out = f_out;
 
-    if (p->opt.pricing_kernel == 2) {
-        std::vector<uint32_t> h_rowq((size_t)B + 1);
-        VMAT_CUDA(p, cudaMemcpyAsync(h_rowq.data(), p->rowq, (size_t)(B + 1) * 4, cudaMemcpyDeviceToHost, st));
-        VMAT_CUDA(p, cudaStreamSynchronize(st));
-        if ((rc = build_chunk_table(p, h_rowq))) return rc;
-    }
     return VMAT_OK;
 }
 

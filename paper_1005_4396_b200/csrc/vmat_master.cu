@@ -5,18 +5,25 @@
 //   penalty gradient       w_j = -2 alpha_j max(0,T_j-z_j) + 2 beta_j max(0,z_j-T_j)      (Eq. 1)
 //   master problem         min_{y>=0} F(z(y)) + gamma G(y), gradient projection (Eq. 3)
 //
-// Layout: the columns are DENSE rows over the support of D, Dd[k][slot], fp32.
-// Both products of one inner iteration — q = Dc^T d (per slot) and grad = Dc w (per beam) — stream
-// the same rows with coalesced float4 loads, both are tiled over chunks of 128 slots, and every
-// reduction runs in a fixed order, so a solve is bit-reproducible from run to run.
+// Layout: the columns are DENSE rows over the support of D, Dd[k][slot], fp32,
+// cut into chunks of 128 slots (one warp of float4).  Each column carries the range of chunks it
+// touches, so both products of one inner iteration — q = Dc^T d (per slot) and grad = Dc w (per
+// beam) — skip the part of a row that is all zero.  Chunks are dealt to the blocks round-robin
+// (the touched slots cluster in the slabs the apertures irradiate), a block works on groups of
+// kGroup chunks at a time with the beam loop split over its warps, so every lane keeps kGroup
+// independent 16-byte loads in flight.
 //
-// The whole master solve is ONE persistent cooperative kernel: blocks own fixed slot ranges, the
-// K-vectors (y, direction, gradient) live in every block's shared memory and all scalar decisions
-// (step length, sufficient decrease, conjugacy, stop) are taken redundantly by every block from
-// the same partial sums in the same order, so control flow is uniform with two grid barriers per
-// inner iteration and no host round trip.
+// The whole master solve is ONE persistent cooperative kernel: the K-vectors (y, direction,
+// gradient) live in every block's shared memory and all scalar decisions (step length, sufficient
+// decrease, conjugacy, stop) are taken redundantly by every block from the same sums, so control
+// flow is uniform with two grid barriers per inner iteration and no host round trip.  Sums over
+// the grid (F, the curvature, the K gradient entries) are accumulated with 64-bit FIXED-POINT
+// atomics whose scale every block derives from the same bound: integer addition is order free, so
+// a solve is bit-reproducible from run to run although the blocks arrive in any order.
 #include <cooperative_groups.h>
 #include <math_constants.h>
+
+#include <climits>
 
 #include "vmat_internal.cuh"
 
@@ -34,9 +41,18 @@ constexpr unsigned kFull = 0xffffffffu;
 __global__ void __launch_bounds__(256)
 k_column_scatter(const uint32_t *__restrict__ rowq, const float4 *__restrict__ val4, const int4 *__restrict__ col4,
                  const Sel *__restrict__ sel, int beam, const int32_t *__restrict__ left,
-                 const int32_t *__restrict__ right, int R, int C, double fx_scale, unsigned long long *__restrict__ acc) {
+                 const int32_t *__restrict__ right, int R, int C, double fx_scale, unsigned long long *__restrict__ acc,
+                 ColStat *__restrict__ colstat) {
     const int k = sel ? sel->beam : beam;
     if (k < 0) return;
+    if (blockIdx.x == 0 && threadIdx.x == 0) {   // statistics of the column, filled by k_column_finish
+        ColStat cs;
+        cs.l1 = 0ull;
+        cs.linf = 0ull;
+        cs.clo = INT_MAX;
+        cs.chi = -1;
+        colstat[k] = cs;
+    }
     const int lane = threadIdx.x & 31;
     const int idx = blockIdx.x * 8 + (threadIdx.x >> 5);
     if (idx >= R * C) return;
@@ -54,16 +70,57 @@ k_column_scatter(const uint32_t *__restrict__ rowq, const float4 *__restrict__ v
     }
 }
 
+// Dd[k][.] = fixed-point accumulator as fp32; clears the accumulator; gathers the column's
+// statistics (exact integer sums / extrema, hence order free): sum and max of |d_k|, first and
+// last chunk with a non-zero entry.  One block = 256 slots = 2 chunks.
 __global__ void __launch_bounds__(256)
 k_column_finish(unsigned long long *__restrict__ acc, long long Sp, const Sel *__restrict__ sel, int beam,
-                double fx_inv, float *__restrict__ Dd) {
+                double fx_inv, float *__restrict__ Dd, ColStat *__restrict__ colstat) {
     const int k = sel ? sel->beam : beam;
     if (k < 0) return;
+    __shared__ unsigned long long s_sum[8], s_max[8];
+    __shared__ int s_lo[8], s_hi[8];
     const long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= Sp) return;
-    const long long v = (long long)acc[s];
-    Dd[(size_t)k * Sp + s] = (float)((double)v * fx_inv);
-    acc[s] = 0ull;
+    unsigned long long mag = 0ull;
+    if (s < Sp) {
+        const long long v = (long long)acc[s];
+        Dd[(size_t)k * Sp + s] = (float)((double)v * fx_inv);
+        acc[s] = 0ull;
+        mag = (unsigned long long)(v < 0 ? -v : v);
+    }
+    const int chunk = (int)(s / kChunk);
+    unsigned long long sum = mag, mx = mag;
+    int lo = mag ? chunk : INT_MAX, hi = mag ? chunk : -1;
+#pragma unroll
+    for (int o = 16; o; o >>= 1) {
+        sum += __shfl_xor_sync(kFull, sum, o);
+        const unsigned long long om = __shfl_xor_sync(kFull, mx, o);
+        mx = om > mx ? om : mx;
+        lo = min(lo, __shfl_xor_sync(kFull, lo, o));
+        hi = max(hi, __shfl_xor_sync(kFull, hi, o));
+    }
+    const int warp = threadIdx.x >> 5;
+    if ((threadIdx.x & 31) == 0) {
+        s_sum[warp] = sum;
+        s_max[warp] = mx;
+        s_lo[warp] = lo;
+        s_hi[warp] = hi;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int i = 1; i < 8; ++i) {
+            sum += s_sum[i];
+            mx = s_max[i] > mx ? s_max[i] : mx;
+            lo = min(lo, s_lo[i]);
+            hi = max(hi, s_hi[i]);
+        }
+        if (mx) {
+            atomicAdd(&colstat[k].l1, sum);
+            atomicMax(&colstat[k].linf, mx);
+            atomicMin(&colstat[k].clo, lo);
+            atomicMax(&colstat[k].chi, hi);
+        }
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -92,6 +149,26 @@ __global__ void k_compress(const float *__restrict__ src_V, const int32_t *__res
     dst_s[s] = s < S ? src_V[voxel_of[s]] : 0.f;
 }
 
+// max |T| and max(alpha, beta) over the support (bounds for the fixed-point scales of the master)
+__global__ void k_voxel_bounds(const float *__restrict__ T, const float *__restrict__ alpha,
+                               const float *__restrict__ beta, long long Sp, unsigned int *__restrict__ out2) {
+    const long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    float t = 0.f, ab = 0.f;
+    if (s < Sp) {
+        t = fabsf(T[s]);
+        ab = fmaxf(alpha[s], beta[s]);
+    }
+#pragma unroll
+    for (int o = 16; o; o >>= 1) {
+        t = fmaxf(t, __shfl_xor_sync(kFull, t, o));
+        ab = fmaxf(ab, __shfl_xor_sync(kFull, ab, o));
+    }
+    if ((threadIdx.x & 31) == 0) {   // non-negative floats order like their bit patterns
+        atomicMax(out2, __float_as_uint(t));
+        atomicMax(out2 + 1, __float_as_uint(ab));
+    }
+}
+
 // ------------------------------------------------------------------------------------------------
 // the master kernel
 // ------------------------------------------------------------------------------------------------
@@ -104,10 +181,13 @@ struct MasterArgs {
     const uint8_t *occ;
     double *y;
     const double *theta;
+    const ColStat *colstat;
     int N;
-    double gamma, F_out, eps;
+    double gamma, F_out, eps, fx_inv;
+    float Tmax, abmax;
     int max_inner;
-    double *partA, *partF, *partG;
+    long long *accbuf;          // 3 rotating records of (N + 2) fixed-point sums: F, curvature, grad[0..K)
+    unsigned int *phase;        // rotation counter, persists from launch to launch
     MasterOut *out;
     double *cost3;
     double *trF, *trG, *trC;
@@ -144,39 +224,69 @@ __device__ __forceinline__ double block_max(double v, double *red) {
 }
 __device__ __forceinline__ double block_min(double v, double *red) { return -block_max(-v, red); }
 
+// scale 2^(60-e) for sums whose magnitude is bounded by `bound` < 2^e; flags a non-finite bound
+__device__ __forceinline__ double fx_scale_for(double bound, int &bad) {
+    if (!(bound < 1e300)) bad = 1;
+    int e = 0;
+    frexp(fmax(bound, 1e-18), &e);
+    return ldexp(1.0, 60 - e);
+}
+__device__ __forceinline__ void fx_add(long long *dst, double v, double scale) {
+    atomicAdd(reinterpret_cast<unsigned long long *>(dst), (unsigned long long)__double2ll_rn(v * scale));
+}
+__device__ __forceinline__ double fx_get(const long long *src, double scale) {
+    return (double)__ldcg(src) / scale;   // scale is a power of two: exact
+}
+
 struct Smem {
-    double *y, *d, *grad, *pg, *yn, *gn, *dG, *dt, *gacc, *red;
-    float *part, *wchunk, *coef;
-    int *sk;
+    double *y, *d, *grad, *pg, *yn, *gn, *dG, *dt, *gacc, *linf, *red;
+    float *part, *wbuf, *coef;
+    int *sk, *lo, *hi;
 };
 
-// value[slot] = sum_i coef[i] * Dd[sk[i]][slot] for the 128 slots of chunk c; the beam loop is split
-// over the warps, partials meet in shared memory and are added in warp order.  Result valid for
-// tid < 128 (slot = c*128 + tid).  Ends with the block in sync.
-__device__ __forceinline__ float combine_chunk(const MasterArgs &a, const Smem &sm, int K, int c) {
+// chunk handled by this block as member `ch` of its group `g`: chunks are dealt round-robin
+__device__ __forceinline__ int chunk_of(int g, int ch) { return (int)blockIdx.x + (g * kGroup + ch) * (int)gridDim.x; }
+
+// value[o] = sum_i coef[i] * Dd[sk[i]][slot(o)] for the kGroup*128 slots of group g, o = tid + r*kMasterThreads.
+// The beam loop is split over the warps; partials meet in shared memory and are added in warp order.
+// The caller must __syncthreads() before sm.part is written again.
+__device__ __forceinline__ void combine_group(const MasterArgs &a, const Smem &sm, int K, int g,
+                                              float (&out)[kOutPerThread]) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const float4 *base = reinterpret_cast<const float4 *>(a.Dd + (size_t)c * kChunk) + lane;
+    const float4 *Dd4 = reinterpret_cast<const float4 *>(a.Dd) + lane;
     const size_t stride4 = (size_t)a.Sp / 4;
-    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll 4
+    const int cb = chunk_of(g, 0), G = (int)gridDim.x;
+    float4 acc[kGroup];
+#pragma unroll
+    for (int ch = 0; ch < kGroup; ++ch) acc[ch] = make_float4(0.f, 0.f, 0.f, 0.f);
     for (int i = warp; i < K; i += kMasterWarps) {
         const float cf = sm.coef[i];
-        if (cf != 0.f) {
-            const float4 v = __ldg(base + (size_t)sm.sk[i] * stride4);
-            acc.x = fmaf(cf, v.x, acc.x);
-            acc.y = fmaf(cf, v.y, acc.y);
-            acc.z = fmaf(cf, v.z, acc.z);
-            acc.w = fmaf(cf, v.w, acc.w);
+        if (cf == 0.f) continue;
+        const int lo = sm.lo[i], hi = sm.hi[i];
+        const float4 *row = Dd4 + (size_t)sm.sk[i] * stride4;
+#pragma unroll
+        for (int ch = 0; ch < kGroup; ++ch) {
+            const int c = cb + ch * G;
+            if (c >= lo && c <= hi) {
+                const float4 v = __ldg(row + (size_t)c * (kChunk / 4));
+                acc[ch].x = fmaf(cf, v.x, acc[ch].x);
+                acc[ch].y = fmaf(cf, v.y, acc[ch].y);
+                acc[ch].z = fmaf(cf, v.z, acc[ch].z);
+                acc[ch].w = fmaf(cf, v.w, acc[ch].w);
+            }
         }
     }
-    reinterpret_cast<float4 *>(sm.part)[warp * 32 + lane] = acc;
-    __syncthreads();
-    float r = 0.f;
-    if (tid < kChunk) {
 #pragma unroll
-        for (int wv = 0; wv < kMasterWarps; ++wv) r += sm.part[wv * kChunk + tid];
+    for (int ch = 0; ch < kGroup; ++ch) reinterpret_cast<float4 *>(sm.part)[(warp * kGroup + ch) * 32 + lane] = acc[ch];
+    __syncthreads();
+#pragma unroll
+    for (int r = 0; r < kOutPerThread; ++r) {
+        const int o = tid + r * kMasterThreads, ch = o >> 7, s = o & (kChunk - 1);
+        float v = 0.f;
+#pragma unroll
+        for (int wv = 0; wv < kMasterWarps; ++wv) v += sm.part[(wv * kGroup + ch) * kChunk + s];
+        out[r] = v;
     }
-    return r;
 }
 
 __device__ __forceinline__ void penalty(float z, float T, float al, float be, float &w, double &F) {
@@ -186,45 +296,63 @@ __device__ __forceinline__ void penalty(float z, float T, float al, float be, fl
 }
 
 // One pass over the block's chunks that evaluates the objective at a new dose:
-//   from_y:  z_new = sum_k y_k d_k            (coef must hold y)             -> stored to zdst, w to a.w
+//   FROM_Y:  z_new = sum_k y_k d_k            (coef must hold y)             -> stored to zdst, w to a.w
 //   else:    z_new = zsrc + t q               (line-search trial)            -> stored to zdst
-// and in the same pass F (partial, fp64) and the block's share of grad = Dc w_new.
-__device__ __forceinline__ void eval_pass(const MasterArgs &a, const Smem &sm, int K, int c0, int c1, bool from_y,
-                                          const float *zsrc, float *zdst, float tf, double *partF, double *partG) {
+// and in the same pass F and the block's share of grad = Dc w_new, both added to the record `rec`
+// in fixed point (scales scF, scG).
+template <bool FROM_Y>
+__device__ __forceinline__ void eval_pass(const MasterArgs &a, const Smem &sm, int K, int ngroups, const float *zsrc,
+                                          float *zdst, float tf, long long *rec, double scF, double scG) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const float4 *Dd4 = reinterpret_cast<const float4 *>(a.Dd) + lane;
     const size_t stride4 = (size_t)a.Sp / 4;
+    const int G = (int)gridDim.x;
     for (int i = tid; i < K; i += kMasterThreads) sm.gacc[i] = 0.0;
     double F = 0.0;
     __syncthreads();
-    for (int c = c0; c < c1; ++c) {
-        float zv = 0.f;
-        if (from_y) zv = combine_chunk(a, sm, K, c);
-        if (tid < kChunk) {
-            const size_t s = (size_t)c * kChunk + tid;
-            if (!from_y) zv = fmaf(tf, a.q[s], zsrc[s]);
-            float wv;
-            double f;
-            penalty(zv, a.T[s], a.alpha[s], a.beta[s], wv, f);
-            F += f;
-            zdst[s] = zv;
-            if (from_y) a.w[s] = wv;
-            sm.wchunk[tid] = wv;
+    for (int g = 0; g < ngroups; ++g) {
+        float zv[kOutPerThread];
+        if (FROM_Y) combine_group(a, sm, K, g, zv);
+#pragma unroll
+        for (int r = 0; r < kOutPerThread; ++r) {
+            const int o = tid + r * kMasterThreads, c = chunk_of(g, o >> 7);
+            float wv = 0.f;
+            if (c < a.nchunks) {
+                const size_t s = (size_t)c * kChunk + (o & (kChunk - 1));
+                const float z = FROM_Y ? zv[r] : fmaf(tf, a.q[s], zsrc[s]);
+                double f;
+                penalty(z, a.T[s], a.alpha[s], a.beta[s], wv, f);
+                F += f;
+                zdst[s] = z;
+                if (FROM_Y) a.w[s] = wv;
+            }
+            sm.wbuf[o] = wv;
         }
         __syncthreads();
-        const float4 w4 = reinterpret_cast<const float4 *>(sm.wchunk)[lane];
-        const float4 *base = reinterpret_cast<const float4 *>(a.Dd + (size_t)c * kChunk) + lane;
-#pragma unroll 4
+        float4 w4[kGroup];
+#pragma unroll
+        for (int ch = 0; ch < kGroup; ++ch) w4[ch] = reinterpret_cast<const float4 *>(sm.wbuf)[ch * 32 + lane];
+        const int cb = chunk_of(g, 0);
         for (int i = warp; i < K; i += kMasterWarps) {
-            const float4 v = __ldg(base + (size_t)sm.sk[i] * stride4);
-            double dot = (double)(v.x * w4.x + v.y * w4.y) + (double)(v.z * w4.z + v.w * w4.w);
+            const int lo = sm.lo[i], hi = sm.hi[i];
+            const float4 *row = Dd4 + (size_t)sm.sk[i] * stride4;
+            double dot = 0.0;
+#pragma unroll
+            for (int ch = 0; ch < kGroup; ++ch) {
+                const int c = cb + ch * G;
+                if (c >= lo && c <= hi) {
+                    const float4 v = __ldg(row + (size_t)c * (kChunk / 4));
+                    dot += (double)(v.x * w4[ch].x + v.y * w4[ch].y + v.z * w4[ch].z + v.w * w4[ch].w);
+                }
+            }
             dot = warp_sum(dot);
             if (lane == 0) sm.gacc[i] += dot;   // index i is owned by this warp
         }
         __syncthreads();
     }
     F = block_sum(F, sm.red);
-    if (tid == 0) partF[blockIdx.x] = F;
-    for (int i = tid; i < K; i += kMasterThreads) partG[(size_t)blockIdx.x * a.N + i] = sm.gacc[i];
+    if (tid == 0) fx_add(rec, F, scF);
+    for (int i = tid; i < K; i += kMasterThreads) fx_add(rec + 2 + i, sm.gacc[i], scG);
 }
 
 // G(v) = sum_k (v_{k+1}-v_k)^2 / (theta_{k+1}-theta_k)   (Eq. 2; S2, S3)
@@ -246,14 +374,14 @@ __device__ __forceinline__ void smooth_dG(const double *v, const Smem &sm, int N
     __syncthreads();
 }
 
-__global__ void __launch_bounds__(kMasterThreads) k_master(const MasterArgs a) {
+__global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a) {
     cg::grid_group grid = cg::this_grid();
     extern __shared__ float4 smem_raw[];   // 16-byte aligned: float4 tiles first, then doubles, floats, ints
     const int N = a.N, tid = threadIdx.x;
     Smem sm;
     sm.part = reinterpret_cast<float *>(smem_raw);
-    sm.wchunk = sm.part + kMasterWarps * kChunk;
-    sm.y = reinterpret_cast<double *>(sm.wchunk + kChunk);
+    sm.wbuf = sm.part + kMasterWarps * kGroup * kChunk;
+    sm.y = reinterpret_cast<double *>(sm.wbuf + kGroup * kChunk);
     sm.d = sm.y + N;
     sm.grad = sm.d + N;
     sm.pg = sm.grad + N;
@@ -262,9 +390,12 @@ __global__ void __launch_bounds__(kMasterThreads) k_master(const MasterArgs a) {
     sm.dG = sm.gn + N;
     sm.dt = sm.dG + N;
     sm.gacc = sm.dt + N;
-    sm.red = sm.gacc + N;
+    sm.linf = sm.gacc + N;
+    sm.red = sm.linf + N;
     sm.coef = reinterpret_cast<float *>(sm.red + kMasterWarps);
     sm.sk = reinterpret_cast<int *>(sm.coef + N);
+    sm.lo = sm.sk + N;
+    sm.hi = sm.lo + N;
     __shared__ int sK;
 
     // occupied beams in ascending order
@@ -288,30 +419,53 @@ __global__ void __launch_bounds__(kMasterThreads) k_master(const MasterArgs a) {
     }
     __syncthreads();
     const int K = sK;
+    // per occupied beam: touched chunk range, max |d_k|; over all: max sum |d_k|
+    double l1l = 0.0;
+    for (int i = tid; i < K; i += kMasterThreads) {
+        const ColStat cs = a.colstat[sm.sk[i]];
+        sm.lo[i] = cs.clo;
+        sm.hi[i] = cs.chi;
+        sm.linf[i] = (double)cs.linf * a.fx_inv * 1.000001;
+        l1l = fmax(l1l, (double)cs.l1 * a.fx_inv * 1.000001);
+    }
+    const double l1max = block_max(l1l, sm.red);
+    const double Tm = (double)a.Tmax, ab = (double)a.abmax, Spd = (double)a.Sp;
 
-    // this block's chunks
     const int G = gridDim.x;
-    const int per = (a.nchunks + G - 1) / G;
-    const int c0 = min(a.nchunks, (int)blockIdx.x * per), c1 = min(a.nchunks, c0 + per);
-    const int nb = (a.nchunks + per - 1) / per;   // blocks that own chunks
-    double *partF[2] = {a.partF, a.partF + G};
-    double *partG[2] = {a.partG, a.partG + (size_t)G * N};
-    int buf = 0;
+    const int ngroups = (a.nchunks + G * kGroup - 1) / (G * kGroup);
+    const int recn = N + 2;
+    unsigned ph = *a.phase;   // written by the previous launch, stream ordered
+    int bad = 0;
 
-    auto reduce_eval = [&](int b, const double *yv, double &F, double &Gv) {
-        // F, and gn = Dc w + gamma dG(yv) at occupied beams (0 elsewhere)
+    // start a pass: the record that collects its sums; block 0 clears the record of the next pass
+    auto begin_pass = [&]() -> long long * {
+        if (blockIdx.x == 0) {
+            long long *nx = a.accbuf + (size_t)((ph + 1) % 3) * recn;
+            for (int i = tid; i < recn; i += kMasterThreads) nx[i] = 0;
+        }
+        return a.accbuf + (size_t)(ph % 3) * recn;
+    };
+    // sum_i |v_i| * max|d_i|  >=  max_j |sum_i v_i d_ij|
+    auto dose_bound = [&](const double *v) {
         double s = 0.0;
-        for (int i = tid; i < nb; i += kMasterThreads) s += __ldcg(partF[b] + i);
-        F = block_sum(s, sm.red) + a.F_out;
+        for (int i = tid; i < K; i += kMasterThreads) s += fabs(v[sm.sk[i]]) * sm.linf[i];
+        return block_sum(s, sm.red);
+    };
+    auto eval_scales = [&](double zb, double &scF, double &scG) {
+        const double dev = Tm + zb;
+        scF = fx_scale_for(1.01 * Spd * ab * dev * dev, bad);
+        scG = fx_scale_for(2.02 * ab * dev * l1max, bad);
+    };
+    auto read_eval = [&](const long long *rec, double scF, double scG, const double *yv, double &F, double &Gv) {
+        // F, and gn = Dc w + gamma dG(yv) at occupied beams (0 elsewhere)
+        F = fx_get(rec, scF) + a.F_out;
         Gv = smooth_G(yv, sm, N);
         smooth_dG(yv, sm, N);
         for (int k = tid; k < N; k += kMasterThreads) sm.gn[k] = 0.0;
         __syncthreads();
         for (int i = tid; i < K; i += kMasterThreads) {
-            double g = 0.0;
-            for (int bb = 0; bb < nb; ++bb) g += __ldcg(partG[b] + (size_t)bb * N + i);
             const int k = sm.sk[i];
-            sm.gn[k] = g + a.gamma * sm.dG[k];
+            sm.gn[k] = fx_get(rec + 2 + i, scG) + a.gamma * sm.dG[k];
         }
         __syncthreads();
     };
@@ -319,13 +473,16 @@ __global__ void __launch_bounds__(kMasterThreads) k_master(const MasterArgs a) {
     float *zcur = a.z, *znext = a.zn;
 
     // objective and gradient at the incoming y
+    double scF, scG;
+    eval_scales(dose_bound(sm.y), scF, scG);
     for (int i = tid; i < K; i += kMasterThreads) sm.coef[i] = (float)sm.y[sm.sk[i]];
     __syncthreads();
-    eval_pass(a, sm, K, c0, c1, true, nullptr, zcur, 0.f, partF[buf], partG[buf]);
+    long long *rec = begin_pass();
+    eval_pass<true>(a, sm, K, ngroups, nullptr, zcur, 0.f, rec, scF, scG);
     grid.sync();
+    ++ph;
     double F, Gs;
-    reduce_eval(buf, sm.y, F, Gs);
-    buf ^= 1;
+    read_eval(rec, scF, scG, sm.y, F, Gs);
     double Phi = F + a.gamma * Gs;
 
     double pgl = 0.0;
@@ -343,7 +500,7 @@ __global__ void __launch_bounds__(kMasterThreads) k_master(const MasterArgs a) {
     const double c1a = 1e-4, noise = 2e-7;
     int inner = 0, backtracks = 0, stop = 0, stall = 0;
 
-    while (pgmax > tol) {
+    while (pgmax > tol && !bad) {
         if (inner >= a.max_inner) {
             stop = 1;
             break;
@@ -365,26 +522,33 @@ __global__ void __launch_bounds__(kMasterThreads) k_master(const MasterArgs a) {
             }
         }
         // q = Dc^T d and the curvature of the quadratic piece at t = 0
+        const double qb = dose_bound(sm.d), yb = dose_bound(sm.y);
+        const double scC = fx_scale_for(1.01 * Spd * ab * qb * qb, bad);
         for (int i = tid; i < K; i += kMasterThreads) sm.coef[i] = (float)sm.d[sm.sk[i]];
         __syncthreads();
+        rec = begin_pass();
         double curv = 0.0;
-        for (int c = c0; c < c1; ++c) {
-            const float qv = combine_chunk(a, sm, K, c);
-            if (tid < kChunk) {
-                const size_t sl = (size_t)c * kChunk + tid;
-                const float zv = zcur[sl], Tv = a.T[sl];
-                const float om = zv < Tv ? a.alpha[sl] : (zv > Tv ? a.beta[sl] : 0.f);
-                curv += (double)om * (double)qv * (double)qv;
-                a.q[sl] = qv;
+        for (int g = 0; g < ngroups; ++g) {
+            float qv[kOutPerThread];
+            combine_group(a, sm, K, g, qv);
+#pragma unroll
+            for (int r = 0; r < kOutPerThread; ++r) {
+                const int o = tid + r * kMasterThreads, c = chunk_of(g, o >> 7);
+                if (c < a.nchunks) {
+                    const size_t sl = (size_t)c * kChunk + (o & (kChunk - 1));
+                    const float zv = zcur[sl], Tv = a.T[sl];
+                    const float om = zv < Tv ? a.alpha[sl] : (zv > Tv ? a.beta[sl] : 0.f);
+                    curv += (double)om * (double)qv[r] * (double)qv[r];
+                    a.q[sl] = qv[r];
+                }
             }
             __syncthreads();
         }
         curv = block_sum(curv, sm.red);
-        if (tid == 0) a.partA[blockIdx.x] = curv;
+        if (tid == 0) fx_add(rec + 1, curv, scC);
         grid.sync();
-        s = 0.0;
-        for (int i = tid; i < nb; i += kMasterThreads) s += __ldcg(a.partA + i);
-        const double curvF = block_sum(s, sm.red);
+        ++ph;
+        const double curvF = fx_get(rec + 1, scC);
         const double phi2 = 2.0 * curvF + 2.0 * a.gamma * smooth_G(sm.d, sm, N);   // d^T L d = G(d)
         double tl = CUDART_INF;
         for (int k = tid; k < N; k += kMasterThreads)
@@ -396,6 +560,8 @@ __global__ void __launch_bounds__(kMasterThreads) k_master(const MasterArgs a) {
             t = tmax;
             hit = 1;
         }
+        eval_scales(yb + t * qb, scF, scG);   // |z + t q| <= sum_i (|y_i| + t |d_i|) max|d_i|; t only shrinks below
+        if (bad) break;
         // backtracking on the true cost
         bool accepted = false;
         double Fn = 0.0, Gn = 0.0, Phin = 0.0;
@@ -406,10 +572,11 @@ __global__ void __launch_bounds__(kMasterThreads) k_master(const MasterArgs a) {
                 sm.yn[k] = v;
             }
             __syncthreads();
-            eval_pass(a, sm, K, c0, c1, false, zcur, znext, (float)t, partF[buf], partG[buf]);
+            rec = begin_pass();
+            eval_pass<false>(a, sm, K, ngroups, zcur, znext, (float)t, rec, scF, scG);
             grid.sync();
-            reduce_eval(buf, sm.yn, Fn, Gn);
-            buf ^= 1;
+            ++ph;
+            read_eval(rec, scF, scG, sm.yn, Fn, Gn);
             Phin = Fn + a.gamma * Gn;
             if (Phin <= Phi + c1a * t * phi1) accepted = true;
             else if (Phin <= Phi + noise * fabs(Phi)) {
@@ -468,19 +635,24 @@ __global__ void __launch_bounds__(kMasterThreads) k_master(const MasterArgs a) {
             break;
         }
     }
+    if (bad) stop = 5;
 
     // z, w and the cost from the final y (no drift from the z += t q updates)
-    if (inner > 0 || zcur != a.z) {
+    if ((inner > 0 || zcur != a.z) && !bad) {
+        eval_scales(dose_bound(sm.y), scF, scG);
         for (int i = tid; i < K; i += kMasterThreads) sm.coef[i] = (float)sm.y[sm.sk[i]];
         __syncthreads();
-        eval_pass(a, sm, K, c0, c1, true, nullptr, a.z, 0.f, partF[buf], partG[buf]);
+        rec = begin_pass();
+        eval_pass<true>(a, sm, K, ngroups, nullptr, a.z, 0.f, rec, scF, scG);
         grid.sync();
-        reduce_eval(buf, sm.y, F, Gs);
+        ++ph;
+        read_eval(rec, scF, scG, sm.y, F, Gs);
         Phi = F + a.gamma * Gs;
     }
     if (blockIdx.x == 0) {
         for (int k = tid; k < N; k += kMasterThreads) a.y[k] = sm.y[k];
         if (tid == 0) {
+            *a.phase = ph % 3;
             MasterOut o;
             o.inner = inner;
             o.backtracks = backtracks;
@@ -506,28 +678,43 @@ __global__ void __launch_bounds__(kMasterThreads) k_master(const MasterArgs a) {
 }
 
 size_t master_smem_bytes(int64_t N) {
-    return (size_t)(9 * N + kMasterWarps) * 8 + (size_t)(kMasterWarps * kChunk + kChunk + N) * 4 + (size_t)N * 4;
+    return (size_t)(kMasterWarps * kGroup * kChunk + kGroup * kChunk) * 4   // part, wbuf
+           + (size_t)(10 * N + kMasterWarps) * 8                             // K-vectors, red
+           + (size_t)N * 4 * 4;                                              // coef, sk, lo, hi
 }
 
 }  // namespace
 
 int master_configure(vmat_plan *p) {
     p->master_smem = master_smem_bytes(p->N);
-    if (p->master_smem > 200 * 1024) return fail(p, VMAT_EINVAL, "n_beams too large for the master kernel's shared memory");
+    if (p->master_smem > 220 * 1024) return fail(p, VMAT_EINVAL, "n_beams too large for the master kernel's shared memory");
     VMAT_CUDA(p, cudaFuncSetAttribute(k_master, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->master_smem));
     int per_sm = 0;
     VMAT_CUDA(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_master, kMasterThreads, p->master_smem));
     if (per_sm < 1) return fail(p, VMAT_ECUDA, "master kernel does not fit on an SM");
-    if (per_sm > 2) per_sm = 2;
     const int64_t nchunks = p->Sp / kChunk;
-    int64_t grid = (int64_t)per_sm * p->sm_count;
-    if (grid > nchunks) grid = nchunks;
+    int64_t grid = p->sm_count;                       // one block per SM
+    const int64_t want = (nchunks + kGroup - 1) / kGroup;   // no more blocks than groups of chunks
+    if (grid > want) grid = want;
     if (grid < 1) grid = 1;
     p->master_grid = (int)grid;
     int rc;
-    if ((rc = dev_alloc(p, &p->partA, grid))) return rc;
-    if ((rc = dev_alloc(p, &p->partF, 2 * grid))) return rc;
-    if ((rc = dev_alloc(p, &p->partG, 2 * grid * p->N))) return rc;
+    if ((rc = dev_alloc(p, &p->accbuf, 3 * (p->N + 2)))) return rc;
+    if ((rc = dev_alloc(p, &p->phase, 1))) return rc;
+    if ((rc = dev_alloc(p, &p->colstat, p->N))) return rc;
+    if ((rc = dev_alloc(p, &p->vbounds, 2))) return rc;
+    VMAT_CUDA(p, cudaMemsetAsync(p->accbuf, 0, (size_t)3 * (p->N + 2) * 8, p->stream));
+    VMAT_CUDA(p, cudaMemsetAsync(p->phase, 0, 4, p->stream));
+    VMAT_CUDA(p, cudaMemsetAsync(p->colstat, 0, (size_t)p->N * sizeof(ColStat), p->stream));
+    VMAT_CUDA(p, cudaMemsetAsync(p->vbounds, 0, 8, p->stream));
+    k_voxel_bounds<<<(unsigned)((p->Sp + 255) / 256), 256, 0, p->stream>>>(p->T_s, p->alpha_s, p->beta_s,
+                                                                         (long long)p->Sp, p->vbounds);
+    VMAT_CUDA(p, cudaGetLastError());
+    float hb[2];
+    VMAT_CUDA(p, cudaMemcpyAsync(hb, p->vbounds, 8, cudaMemcpyDeviceToHost, p->stream));
+    VMAT_CUDA(p, cudaStreamSynchronize(p->stream));
+    p->Tmax = hb[0];
+    p->abmax = hb[1];
     return VMAT_OK;
 }
 
@@ -535,9 +722,9 @@ int launch_column_build(vmat_plan *p, int beam) {
     const Sel *sel = beam < 0 ? p->sel : nullptr;
     const unsigned blocks = (unsigned)((p->RC + 7) / 8);
     k_column_scatter<<<blocks, 256, 0, p->stream>>>(p->rowq, p->val4, p->col4, sel, beam, p->left, p->right, (int)p->R,
-                                                   (int)p->C, p->fx_scale, p->acc);
+                                                   (int)p->C, p->fx_scale, p->acc, p->colstat);
     k_column_finish<<<(unsigned)((p->Sp + 255) / 256), 256, 0, p->stream>>>(p->acc, (long long)p->Sp, sel, beam,
-                                                                          p->fx_inv, p->Dd);
+                                                                          p->fx_inv, p->Dd, p->colstat);
     p->launches += 2;
     VMAT_CUDA(p, cudaGetLastError());
     return VMAT_OK;
@@ -563,9 +750,12 @@ static int launch_master_impl(vmat_plan *p, int max_inner, int trace_it) {
     a.F_out = p->F_out;
     a.eps = p->opt.master_eps;
     a.max_inner = max_inner;
-    a.partA = p->partA;
-    a.partF = p->partF;
-    a.partG = p->partG;
+    a.colstat = p->colstat;
+    a.fx_inv = p->fx_inv;
+    a.Tmax = p->Tmax;
+    a.abmax = p->abmax;
+    a.accbuf = p->accbuf;
+    a.phase = p->phase;
     a.out = p->mout;
     a.cost3 = p->cost3;
     a.trF = p->tr_F;

@@ -27,31 +27,33 @@ __device__ __forceinline__ int4 ld_stream_i4(const int4 *ptr) {
     return r;
 }
 
-constexpr int kPriceWarps = 8;
+constexpr int kPriceThreads = 256;
 
-// One warp per beamlet.  UNROLL quads per lane are loaded before any gather is issued.
-template <int UNROLL>
-__global__ void __launch_bounds__(kPriceWarps * 32)
-k_price_spmv_warp(const uint32_t *__restrict__ rowq, const float4 *__restrict__ val4, const int4 *__restrict__ col4,
-                  const float *__restrict__ w, const uint8_t *__restrict__ occ, int RC, long long B,
-                  float *__restrict__ g) {
-    const int lane = threadIdx.x & 31;
-    const long long row = (long long)blockIdx.x * kPriceWarps + (threadIdx.x >> 5);
-    if (row >= B) return;
-    if (occ[row / RC]) {
-        if (lane == 0) g[row] = 0.f;
-        return;
-    }
+// One group of LANES lanes (a warp or half a warp) per beamlet; UNROLL quads per lane are loaded
+// before any gather is issued.  The grid covers only the un-occupied beams: block b works on beam
+// free_list[b / blocks_per_beam] (ascending list kept current by the leaf search's commit), so a
+// launch late in the plan is as short as the rows it has to stream.
+template <int LANES, int UNROLL>
+__global__ void __launch_bounds__(kPriceThreads)
+k_price_spmv(const uint32_t *__restrict__ rowq, const float4 *__restrict__ val4, const int4 *__restrict__ col4,
+             const float *__restrict__ w, const int32_t *__restrict__ free_list, int blocks_per_beam, int RC,
+             float *__restrict__ g) {
+    constexpr int kRowsPerBlock = kPriceThreads / LANES;
+    const int lane = threadIdx.x & (LANES - 1);
+    const int beam = free_list[blockIdx.x / blocks_per_beam];
+    const int local = (blockIdx.x % blocks_per_beam) * kRowsPerBlock + threadIdx.x / LANES;
+    if (local >= RC) return;
+    const long long row = (long long)beam * RC + local;
     const uint32_t a = rowq[row], b = rowq[row + 1];
     float acc = 0.f;
-    for (uint32_t q = a + lane; q < b; q += 32 * UNROLL) {
+    for (uint32_t q = a + lane; q < b; q += LANES * UNROLL) {
         float4 v[UNROLL];
         int4 c[UNROLL];
 #pragma unroll
         for (int u = 0; u < UNROLL; ++u) {
-            if (q + 32 * u < b) {
-                v[u] = ld_stream_f4(val4 + q + 32 * u);
-                c[u] = ld_stream_i4(col4 + q + 32 * u);
+            if (q + LANES * u < b) {
+                v[u] = ld_stream_f4(val4 + q + LANES * u);
+                c[u] = ld_stream_i4(col4 + q + LANES * u);
             } else {
                 v[u] = make_float4(0.f, 0.f, 0.f, 0.f);
                 c[u] = make_int4(0, 0, 0, 0);
@@ -66,23 +68,51 @@ k_price_spmv_warp(const uint32_t *__restrict__ rowq, const float4 *__restrict__ 
         }
     }
 #pragma unroll
-    for (int o = 16; o; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    for (int o = LANES / 2; o; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
     if (lane == 0) g[row] = acc;
+}
+
+// ascending list of the un-occupied beams (after vmat_set_plan; the search keeps it current afterwards)
+__global__ void k_free_list(const uint8_t *__restrict__ occ, int N, int32_t *__restrict__ free_list) {
+    int base = 0;
+    const int lane = threadIdx.x;
+    for (int k0 = 0; k0 < N; k0 += 32) {
+        const int k = k0 + lane;
+        const bool f = k < N && !occ[k];
+        const unsigned m = __ballot_sync(0xffffffffu, f);
+        if (f) free_list[base + __popc(m & ((1u << lane) - 1u))] = k;
+        base += __popc(m);
+    }
+}
+
+template <int LANES, int UNROLL>
+void launch_variant(vmat_plan *p, const float *w_s, float *g, int n_free) {
+    const int rows_per_block = kPriceThreads / LANES;
+    const int bpb = (int)((p->RC + rows_per_block - 1) / rows_per_block);
+    k_price_spmv<LANES, UNROLL><<<(unsigned)(n_free * bpb), kPriceThreads, 0, p->stream>>>(
+        p->rowq, p->val4, p->col4, w_s, p->free_list, bpb, (int)p->RC, g);
 }
 
 }  // namespace
 
-int build_chunk_table(vmat_plan *p, const std::vector<uint32_t> &h_rowq) {
-    (void)p;
-    (void)h_rowq;
+int launch_free_list(vmat_plan *p) {
+    k_free_list<<<1, 32, 0, p->stream>>>(p->occ, (int)p->N, p->free_list);
+    ++p->launches;
+    VMAT_CUDA(p, cudaGetLastError());
     return VMAT_OK;
 }
 
-int launch_price_spmv(vmat_plan *p, const float *w_s, float *g) {
-    if (p->B == 0) return VMAT_OK;
-    const unsigned blocks = (unsigned)((p->B + kPriceWarps - 1) / kPriceWarps);
-    k_price_spmv_warp<2><<<blocks, kPriceWarps * 32, 0, p->stream>>>(p->rowq, p->val4, p->col4, w_s, p->occ, (int)p->RC,
-                                                                      (long long)p->B, g);
+// g_i for the beamlets of the n_free un-occupied beams listed in p->free_list; other entries of g untouched
+int launch_price_spmv(vmat_plan *p, const float *w_s, float *g, int n_free) {
+    if (p->B == 0 || n_free <= 0) return VMAT_OK;
+    switch (p->opt.pricing_kernel) {
+        case 1: launch_variant<32, 2>(p, w_s, g, n_free); break;
+        case 2: launch_variant<32, 4>(p, w_s, g, n_free); break;
+        case 3: launch_variant<16, 2>(p, w_s, g, n_free); break;
+        case 4: launch_variant<16, 4>(p, w_s, g, n_free); break;
+        case 5: launch_variant<8, 4>(p, w_s, g, n_free); break;
+        default: launch_variant<16, 4>(p, w_s, g, n_free); break;
+    }
     ++p->launches;
     VMAT_CUDA(p, cudaGetLastError());
     return VMAT_OK;

@@ -128,6 +128,7 @@ struct SearchArgs {
     const float *g;
     const uint8_t *occ_in;
     uint8_t *occ;
+    int32_t *free_list;                // ascending list of un-occupied beams, rebuilt on commit
     int32_t *left, *right;
     double *y;
     const double *theta;
@@ -272,6 +273,17 @@ __global__ void __launch_bounds__(kSearchThreads) k_leaf_search(const SearchArgs
             a.occ[best] = 1;
             a.y[best] = 0.0;
         }
+        // the pricing product of the next iteration walks this list
+        if (tid < 32) {
+            int base = 0;
+            for (int k0 = 0; k0 < N; k0 += 32) {
+                const int kk = k0 + tid;
+                const bool f = kk < N && kk != best && !a.occ[kk];
+                const unsigned m = __ballot_sync(kFull, f);
+                if (f) a.free_list[base + __popc(m & ((1u << tid) - 1u))] = kk;
+                base += __popc(m);
+            }
+        }
     }
 }
 
@@ -283,6 +295,7 @@ int launch_leaf_search(vmat_plan *p, const float *g, int32_t *all_left, int32_t 
     a.g = g;
     a.occ_in = p->occ;
     a.occ = p->occ;
+    a.free_list = p->free_list;
     a.left = p->left;
     a.right = p->right;
     a.y = p->y;

@@ -1,0 +1,123 @@
+"""GPU parity at BASELINE.json configs[1] (prostate-like phantom: 288,000 beamlets, 1.2e8 non-zeros), i.e. the
+workload and launch configuration bench.py times.  The oracle cannot run the whole 180-iteration plan in a test,
+so:
+  * the first iterations are compared step by step, teacher-forced (the oracle's state is loaded into the plan):
+    prices on every beamlet (one fp64 SpMV of the oracle), leaf pairs / beam prices bit-exact, dose and gradient
+    norm-wise, master cost on the same aperture set;
+  * the full 180-iteration plan is checked on what holds at any size: one aperture per beam, the leaf-travel
+    invariant, non-increasing cost, and the final dose / cost recomputed by the oracle from the GPU's plan.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-4
+
+
+def relnorm(a, ref):
+    ref = np.asarray(ref, np.float64)
+    return np.max(np.abs(np.asarray(a, np.float64) - ref)) / max(np.max(np.abs(ref)), 1e-300)
+
+
+@pytest.fixture(scope="module")
+def setup():
+    import torch
+
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_1005_4396_b200 as vm
+    import vmat_inputs
+    from oracle import Oracle
+
+    ph = vmat_inputs.make_phantom("prostate", seed=0)
+    o = Oracle.from_phantom(ph)
+    plan = vm.Plan.from_phantom(ph)
+    yield torch, vm, ph, o, plan
+    plan.destroy()
+
+
+def test_teacher_forced_steps_fullsize(setup):
+    torch, vm, ph, o, plan = setup
+    occ, left, right, y = o.empty_plan()
+    left, right = left.reshape(o.N, o.R), right.reshape(o.N, o.R)
+    rng = np.random.default_rng(0)
+    for it in range(3):
+        plan.set_plan(occ, left, right, y)
+        # (a)+(b) dose and gradient of the current plan
+        z = torch.empty(o.V, dtype=torch.float32, device="cuda")
+        w = torch.empty(o.V, dtype=torch.float32, device="cuda")
+        F, G, cost = plan.dose(z, w)
+        z_ref = o.dose(occ, left, right, y)
+        F_ref, w_ref = o.penalty(z_ref)
+        G_ref, _ = o.smooth(y)
+        if np.max(np.abs(z_ref)) > 0:
+            assert relnorm(z.cpu().numpy(), z_ref) <= TOL
+        assert relnorm(w.cpu().numpy(), w_ref) <= TOL
+        assert abs(F - F_ref) <= TOL * abs(F_ref)
+        assert abs(cost - (F_ref + o.gamma * G_ref)) <= TOL * abs(F_ref + o.gamma * G_ref)
+        # (c) prices on the oracle's gradient, every beamlet
+        w32 = w_ref.astype(np.float32)
+        g_ref = o.prices(w32.astype(np.float64), occ)
+        g = torch.empty(o.B, dtype=torch.float32, device="cuda")
+        plan.price_spmv(g, torch.from_numpy(w32).cuda())
+        g = g.cpu().numpy()
+        assert relnorm(g, g_ref) <= TOL
+        # sampled rows against the magnitude sum_j |D_ij||w_j|, one by one
+        for i in rng.integers(0, o.B, 200):
+            a, b = o.row_ptr[i], o.row_ptr[i + 1]
+            mag = np.sum(np.abs(o.val[a:b].astype(np.float64)) * np.abs(w32[o.col[a:b]].astype(np.float64)))
+            assert abs(g[i] - g_ref[i]) <= 1e-5 * mag + 1e-30
+        assert np.all(g[np.repeat(occ.astype(bool), o.R * o.C)] == 0.0)
+        # (d) search on the oracle's fp32 prices: bit exact
+        g32 = g_ref.astype(np.float32)
+        ref = o.price_step(g32, occ, left, right, y)
+        al = torch.zeros(o.N * o.R, dtype=torch.int32, device="cuda")
+        ar = torch.zeros(o.N * o.R, dtype=torch.int32, device="cuda")
+        bp = torch.zeros(o.N, dtype=torch.float64, device="cuda")
+        g_dev = torch.from_numpy(g32).cuda()
+        plan.leaf_search(g_dev, al, ar, bp)
+        free = ~occ.astype(bool)
+        assert np.array_equal(al.cpu().numpy().reshape(o.N, o.R)[free], ref["all_left"][free])
+        assert np.array_equal(ar.cpu().numpy().reshape(o.N, o.R)[free], ref["all_right"][free])
+        assert np.array_equal(bp.cpu().numpy(), ref["beam_price"])
+        ap = plan.price(g_override=g_dev, commit=True)
+        assert ap.beam == ref["beam"] and ap.price == ref["price"]
+        assert np.array_equal(ap.left, ref["left"]) and np.array_equal(ap.right, ref["right"])
+        # (e) master on the same aperture set (P2)
+        occ = occ.copy()
+        occ[ap.beam] = 1
+        left, right = left.copy(), right.copy()
+        left[ap.beam], right[ap.beam] = ap.left, ap.right
+        y_ref, _, info = o.master(occ, left, right, y0=y, eps=1e-10)
+        st = plan.master()
+        assert abs(st.cost - info.cost) <= TOL * abs(info.cost)
+        y = y_ref
+
+
+def test_full_plan_properties(setup):
+    torch, vm, ph, o, plan = setup
+    e = o.empty_plan()
+    plan.set_plan(e[0], e[1], e[2], e[3])
+    st = plan.solve(o.N)
+    assert st.iters == o.N
+    occ, left, right, y = plan.get_plan()
+    assert occ.all() and np.all(y >= 0)                                        # one aperture per beam (S5)
+    assert sorted(st.beam.tolist()) == list(range(o.N))
+    assert np.all((0 <= left) & (left <= right) & (right <= o.C))
+    for k in range(o.N - 1):                                                   # deliverable arc (S6)
+        assert np.all(np.abs(left[k + 1] - left[k]) <= o.delta) and np.all(np.abs(right[k + 1] - right[k]) <= o.delta)
+    assert np.all(np.diff(st.trace_cost) <= 1e-5 * np.abs(st.trace_cost[:-1]))  # convexity + S2
+    # the oracle recomputes dose and cost from the GPU's finished plan
+    z = torch.empty(o.V, dtype=torch.float32, device="cuda")
+    F, G, cost = plan.dose(z)
+    z_ref = o.dose(occ, left, right, y)
+    F_ref, _ = o.penalty(z_ref)
+    G_ref, _ = o.smooth(y)
+    assert relnorm(z.cpu().numpy(), z_ref) <= TOL
+    assert abs(cost - (F_ref + o.gamma * G_ref)) <= TOL * abs(F_ref + o.gamma * G_ref)
+    assert abs(st.cost - cost) <= 1e-6 * abs(cost)
+    # the finished y is (up to fp32 noise) the minimiser of the oracle's master problem on this aperture set:
+    # warm-started from it, the oracle's own gradient projection cannot lower the cost by more than TOL
+    _, _, info = o.master(occ, left, right, y0=y, eps=1e-7, max_inner=40)
+    assert info.cost <= cost * (1 + TOL)
+    assert cost <= info.cost * (1 + TOL)
