@@ -222,26 +222,66 @@ __device__ __forceinline__ double block_max(double v, double *red) {
     __syncthreads();
     return s;
 }
-__device__ __forceinline__ double block_min(double v, double *red) { return -block_max(-v, red); }
 
-// scale 2^(60-e) for sums whose magnitude is bounded by `bound` < 2^e; flags a non-finite bound
-__device__ __forceinline__ double fx_scale_for(double bound, int &bad) {
+// scale 2^(60-e) (and its inverse) for sums whose magnitude is bounded by `bound` < 2^e; flags a
+// non-finite bound.  Powers of two built from the exponent field: conversions are exact.
+struct FxScale {
+    double scale, inv;
+};
+__device__ __forceinline__ FxScale fx_scale_for(double bound, int &bad) {
     if (!(bound < 1e300)) bad = 1;
-    int e = 0;
-    frexp(fmax(bound, 1e-18), &e);
-    return ldexp(1.0, 60 - e);
+    const double b = fmin(fmax(bound, 1e-18), 1e300);
+    const int e = ((__double2hiint(b) >> 20) & 0x7ff) - 1022;   // b < 2^e
+    FxScale r;
+    r.scale = __hiloint2double((1023 + 60 - e) << 20, 0);
+    r.inv = __hiloint2double((1023 - 60 + e) << 20, 0);
+    return r;
 }
 __device__ __forceinline__ void fx_add(long long *dst, double v, double scale) {
     atomicAdd(reinterpret_cast<unsigned long long *>(dst), (unsigned long long)__double2ll_rn(v * scale));
 }
-__device__ __forceinline__ double fx_get(const long long *src, double scale) {
-    return (double)__ldcg(src) / scale;   // scale is a power of two: exact
-}
+#ifdef VMAT_MASTER_PROFILE
+__device__ long long g_master_prof[16];
+#define PROF_DECL long long pt_ = clock64(), pacc_[16] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0}
+#define PROF(i)                           \
+    {                                     \
+        const long long n_ = clock64();   \
+        pacc_[i] += n_ - pt_;             \
+        pt_ = n_;                         \
+    }
+#define PROFW(i, j)                       \
+    {                                     \
+        const long long n_ = clock64();   \
+        pacc_[j] += n_ - pt_;             \
+        pacc_[i] += n_ - pt_;             \
+        pt_ = n_;                         \
+    }
+#define PROF_END                                                                  \
+    if (blockIdx.x == 0 && threadIdx.x == 0)                                      \
+        for (int i_ = 0; i_ < 16; ++i_) g_master_prof[i_] += pacc_[i_];
+#else
+#define PROF_DECL
+#define PROF(i)
+#define PROFW(i, j)
+#define PROF_END
+#endif
+
+// scalars every thread of the block needs, written by warp 0 (the block's control warp)
+struct Ctl {
+    double scF, scG, scC;   // fixed-point scales of the pass about to run
+    double iF, iG, iC;      // and their inverses
+    float tf;               // trial step of the line search
+    int state;              // what the block does next (kRunDirection, ...)
+    int accepted;           // the last trial was accepted: the z buffers swap roles
+};
+enum { kRunDirection = 0, kRunTrial = 1, kFinish = 2 };
 
 struct Smem {
-    double *y, *d, *grad, *pg, *yn, *gn, *dG, *dt, *gacc, *linf, *red;
+    double *y, *d, *grad, *pg, *yn, *gn, *dG, *rdt, *gacc, *linf;   // N each (control warp; gacc: all warps)
     float *part, *wbuf, *coef;
-    int *sk, *lo, *hi;
+    int *sk, *lo, *hi, *ik;
+    long long *recv;   // the pass's record of grid sums, fetched by the whole block after the barrier
+    Ctl *ctl;
 };
 
 // chunk handled by this block as member `ch` of its group `g`: chunks are dealt round-robin
@@ -295,6 +335,26 @@ __device__ __forceinline__ void penalty(float z, float T, float al, float be, fl
     F = (double)al * (double)under * (double)under + (double)be * (double)over * (double)over;
 }
 
+// dot of row i of the group (chunks cb, cb+G, ..) with the penalty gradient staged in sm.wbuf
+__device__ __forceinline__ double group_dot(const MasterArgs &a, const Smem &sm, const float4 *Dd4, size_t stride4,
+                                            int i, int cb, int G, int lane) {
+    const int lo = sm.lo[i], hi = sm.hi[i];
+    const float4 *row = Dd4 + (size_t)sm.sk[i] * stride4;
+    float4 v[kGroup];
+#pragma unroll
+    for (int ch = 0; ch < kGroup; ++ch) {
+        const int c = cb + ch * G;
+        v[ch] = (c >= lo && c <= hi) ? __ldg(row + (size_t)c * (kChunk / 4)) : make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+    double dot = 0.0;
+#pragma unroll
+    for (int ch = 0; ch < kGroup; ++ch) {
+        const float4 w4 = reinterpret_cast<const float4 *>(sm.wbuf)[ch * 32 + lane];
+        dot += (double)(v[ch].x * w4.x + v[ch].y * w4.y + v[ch].z * w4.z + v[ch].w * w4.w);
+    }
+    return dot;
+}
+
 // One pass over the block's chunks that evaluates the objective at a new dose:
 //   FROM_Y:  z_new = sum_k y_k d_k            (coef must hold y)             -> stored to zdst, w to a.w
 //   else:    z_new = zsrc + t q               (line-search trial)            -> stored to zdst
@@ -302,7 +362,8 @@ __device__ __forceinline__ void penalty(float z, float T, float al, float be, fl
 // in fixed point (scales scF, scG).
 template <bool FROM_Y>
 __device__ __forceinline__ void eval_pass(const MasterArgs &a, const Smem &sm, int K, int ngroups, const float *zsrc,
-                                          float *zdst, float tf, long long *rec, double scF, double scG) {
+                                          float *zdst, float tf, long long *rec, double scF, double scG,
+                                          double *red) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const float4 *Dd4 = reinterpret_cast<const float4 *>(a.Dd) + lane;
     const size_t stride4 = (size_t)a.Sp / 4;
@@ -329,55 +390,65 @@ __device__ __forceinline__ void eval_pass(const MasterArgs &a, const Smem &sm, i
             sm.wbuf[o] = wv;
         }
         __syncthreads();
-        float4 w4[kGroup];
-#pragma unroll
-        for (int ch = 0; ch < kGroup; ++ch) w4[ch] = reinterpret_cast<const float4 *>(sm.wbuf)[ch * 32 + lane];
         const int cb = chunk_of(g, 0);
-        for (int i = warp; i < K; i += kMasterWarps) {
-            const int lo = sm.lo[i], hi = sm.hi[i];
-            const float4 *row = Dd4 + (size_t)sm.sk[i] * stride4;
-            double dot = 0.0;
+        // two rows per step: 2*kGroup independent loads in flight, two interleaved shuffle chains
+        for (int i = warp; i < K; i += 2 * kMasterWarps) {
+            const int i2 = i + kMasterWarps;
+            double d1 = group_dot(a, sm, Dd4, stride4, i, cb, G, lane);
+            double d2 = i2 < K ? group_dot(a, sm, Dd4, stride4, i2, cb, G, lane) : 0.0;
 #pragma unroll
-            for (int ch = 0; ch < kGroup; ++ch) {
-                const int c = cb + ch * G;
-                if (c >= lo && c <= hi) {
-                    const float4 v = __ldg(row + (size_t)c * (kChunk / 4));
-                    dot += (double)(v.x * w4[ch].x + v.y * w4[ch].y + v.z * w4[ch].z + v.w * w4[ch].w);
-                }
+            for (int o = 16; o; o >>= 1) {
+                d1 += __shfl_xor_sync(kFull, d1, o);
+                d2 += __shfl_xor_sync(kFull, d2, o);
             }
-            dot = warp_sum(dot);
-            if (lane == 0) sm.gacc[i] += dot;   // index i is owned by this warp
+            if (lane == 0) {   // indices i, i2 are owned by this warp
+                sm.gacc[i] += d1;
+                if (i2 < K) sm.gacc[i2] += d2;
+            }
         }
         __syncthreads();
     }
-    F = block_sum(F, sm.red);
+    F = block_sum(F, red);
     if (tid == 0) fx_add(rec, F, scF);
     for (int i = tid; i < K; i += kMasterThreads) fx_add(rec + 2 + i, sm.gacc[i], scG);
 }
 
-// G(v) = sum_k (v_{k+1}-v_k)^2 / (theta_{k+1}-theta_k)   (Eq. 2; S2, S3)
-__device__ __forceinline__ double smooth_G(const double *v, const Smem &sm, int N) {
-    double s = 0.0;
-    for (int k = threadIdx.x; k + 1 < N; k += kMasterThreads) {
-        const double dv = v[k + 1] - v[k];
-        s += dv * dv / sm.dt[k];
-    }
-    return block_sum(s, sm.red);
+// ---- control-warp helpers: every lane of warp 0 ends with the same value, fixed order ------------
+__device__ __forceinline__ double wsum(double v) {
+#pragma unroll
+    for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
+    return v;
 }
-__device__ __forceinline__ void smooth_dG(const double *v, const Smem &sm, int N) {
-    for (int k = threadIdx.x; k < N; k += kMasterThreads) {
-        double s = 0.0;
-        if (k > 0) s += 2.0 * (v[k] - v[k - 1]) / sm.dt[k - 1];
-        if (k + 1 < N) s -= 2.0 * (v[k + 1] - v[k]) / sm.dt[k];
-        sm.dG[k] = s;
+__device__ __forceinline__ double wmax(double v) {
+#pragma unroll
+    for (int o = 16; o; o >>= 1) v = fmax(v, __shfl_xor_sync(kFull, v, o));
+    return v;
+}
+__device__ __forceinline__ double wmin(double v) {
+#pragma unroll
+    for (int o = 16; o; o >>= 1) v = fmin(v, __shfl_xor_sync(kFull, v, o));
+    return v;
+}
+
+// G(v) = sum_k (v_{k+1}-v_k)^2 / (theta_{k+1}-theta_k) and dG/dv_k   (Eq. 2; S2, S3)
+__device__ __forceinline__ double smooth_G(const double *v, const Smem &sm, int N, int lane, bool want_dG) {
+    double s = 0.0;
+    for (int k = lane; k < N; k += 32) {
+        const double e1 = k + 1 < N ? (v[k + 1] - v[k]) * sm.rdt[k] : 0.0;      // (v_{k+1}-v_k)/dtheta_k
+        if (k + 1 < N) s += (v[k + 1] - v[k]) * e1;
+        if (want_dG) {
+            const double e0 = k > 0 ? (v[k] - v[k - 1]) * sm.rdt[k - 1] : 0.0;
+            sm.dG[k] = 2.0 * (e0 - e1);
+        }
     }
-    __syncthreads();
+    __syncwarp();
+    return wsum(s);
 }
 
 __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a) {
     cg::grid_group grid = cg::this_grid();
     extern __shared__ float4 smem_raw[];   // 16-byte aligned: float4 tiles first, then doubles, floats, ints
-    const int N = a.N, tid = threadIdx.x;
+    const int N = a.N, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     Smem sm;
     sm.part = reinterpret_cast<float *>(smem_raw);
     sm.wbuf = sm.part + kMasterWarps * kGroup * kChunk;
@@ -388,14 +459,17 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     sm.yn = sm.pg + N;
     sm.gn = sm.yn + N;
     sm.dG = sm.gn + N;
-    sm.dt = sm.dG + N;
-    sm.gacc = sm.dt + N;
+    sm.rdt = sm.dG + N;
+    sm.gacc = sm.rdt + N;
     sm.linf = sm.gacc + N;
-    sm.red = sm.linf + N;
-    sm.coef = reinterpret_cast<float *>(sm.red + kMasterWarps);
+    double *red = sm.linf + N;
+    sm.recv = reinterpret_cast<long long *>(red + kMasterWarps);
+    sm.ctl = reinterpret_cast<Ctl *>(sm.recv + N + 2);
+    sm.coef = reinterpret_cast<float *>(sm.ctl + 1);
     sm.sk = reinterpret_cast<int *>(sm.coef + N);
     sm.lo = sm.sk + N;
     sm.hi = sm.lo + N;
+    sm.ik = sm.hi + N;
     __shared__ int sK;
 
     // occupied beams in ascending order
@@ -405,7 +479,9 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
             const int k = k0 + tid;
             const bool f = k < N && a.occ[k];
             const unsigned m = __ballot_sync(kFull, f);
-            if (f) sm.sk[base + __popc(m & ((1u << tid) - 1u))] = k;
+            const int i = base + __popc(m & ((1u << tid) - 1u));
+            if (f) sm.sk[i] = k;
+            if (k < N) sm.ik[k] = f ? i : -1;
             base += __popc(m);
         }
         if (tid == 0) sK = base;
@@ -415,27 +491,33 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
         if (!a.occ[k] || !(yk > 0.0)) yk = 0.0;
         sm.y[k] = yk;
         sm.d[k] = 0.0;
-        sm.dt[k] = k + 1 < N ? a.theta[k + 1] - a.theta[k] : 1.0;
+        sm.rdt[k] = k + 1 < N ? 1.0 / (a.theta[k + 1] - a.theta[k]) : 0.0;
     }
     __syncthreads();
     const int K = sK;
-    // per occupied beam: touched chunk range, max |d_k|; over all: max sum |d_k|
+    // per occupied beam: touched chunk range, max |d_k| (0 at un-occupied beams); over all: max sum |d_k|
     double l1l = 0.0;
-    for (int i = tid; i < K; i += kMasterThreads) {
-        const ColStat cs = a.colstat[sm.sk[i]];
-        sm.lo[i] = cs.clo;
-        sm.hi[i] = cs.chi;
-        sm.linf[i] = (double)cs.linf * a.fx_inv * 1.000001;
-        l1l = fmax(l1l, (double)cs.l1 * a.fx_inv * 1.000001);
+    for (int k = tid; k < N; k += kMasterThreads) {
+        const int i = sm.ik[k];
+        double lf = 0.0;
+        if (i >= 0) {
+            const ColStat cs = a.colstat[k];
+            sm.lo[i] = cs.clo;
+            sm.hi[i] = cs.chi;
+            lf = (double)cs.linf * a.fx_inv * 1.000001;
+            l1l = fmax(l1l, (double)cs.l1 * a.fx_inv * 1.000001);
+            sm.coef[i] = (float)sm.y[k];
+        }
+        sm.linf[k] = lf;
     }
-    const double l1max = block_max(l1l, sm.red);
+    const double l1max = block_max(l1l, red);
     const double Tm = (double)a.Tmax, ab = (double)a.abmax, Spd = (double)a.Sp;
 
     const int G = gridDim.x;
     const int ngroups = (a.nchunks + G * kGroup - 1) / (G * kGroup);
     const int recn = N + 2;
     unsigned ph = *a.phase;   // written by the previous launch, stream ordered
-    int bad = 0;
+    float *zcur = a.z, *znext = a.zn;
 
     // start a pass: the record that collects its sums; block 0 clears the record of the next pass
     auto begin_pass = [&]() -> long long * {
@@ -445,87 +527,142 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
         }
         return a.accbuf + (size_t)(ph % 3) * recn;
     };
-    // sum_i |v_i| * max|d_i|  >=  max_j |sum_i v_i d_ij|
-    auto dose_bound = [&](const double *v) {
-        double s = 0.0;
-        for (int i = tid; i < K; i += kMasterThreads) s += fabs(v[sm.sk[i]]) * sm.linf[i];
-        return block_sum(s, sm.red);
-    };
-    auto eval_scales = [&](double zb, double &scF, double &scG) {
-        const double dev = Tm + zb;
-        scF = fx_scale_for(1.01 * Spd * ab * dev * dev, bad);
-        scG = fx_scale_for(2.02 * ab * dev * l1max, bad);
-    };
-    auto read_eval = [&](const long long *rec, double scF, double scG, const double *yv, double &F, double &Gv) {
-        // F, and gn = Dc w + gamma dG(yv) at occupied beams (0 elsewhere)
-        F = fx_get(rec, scF) + a.F_out;
-        Gv = smooth_G(yv, sm, N);
-        smooth_dG(yv, sm, N);
-        for (int k = tid; k < N; k += kMasterThreads) sm.gn[k] = 0.0;
-        __syncthreads();
-        for (int i = tid; i < K; i += kMasterThreads) {
-            const int k = sm.sk[i];
-            sm.gn[k] = fx_get(rec + 2 + i, scG) + a.gamma * sm.dG[k];
-        }
+
+    // after the grid barrier: one round trip to L2 for the whole record, then the control warp works from smem
+    auto fetch_record = [&](const long long *rec) {
+        for (int i = tid; i < K + 2; i += kMasterThreads) sm.recv[i] = __ldcg(rec + i);
         __syncthreads();
     };
 
-    float *zcur = a.z, *znext = a.zn;
-
-    // objective and gradient at the incoming y
-    double scF, scG;
-    eval_scales(dose_bound(sm.y), scF, scG);
-    for (int i = tid; i < K; i += kMasterThreads) sm.coef[i] = (float)sm.y[sm.sk[i]];
-    __syncthreads();
-    long long *rec = begin_pass();
-    eval_pass<true>(a, sm, K, ngroups, nullptr, zcur, 0.f, rec, scF, scG);
-    grid.sync();
-    ++ph;
-    double F, Gs;
-    read_eval(rec, scF, scG, sm.y, F, Gs);
-    double Phi = F + a.gamma * Gs;
-
-    double pgl = 0.0;
-    for (int k = tid; k < N; k += kMasterThreads) {
-        const double gk = sm.gn[k];
-        const double p = (!a.occ[k] || (sm.y[k] <= 0.0 && gk >= 0.0)) ? 0.0 : gk;
-        sm.grad[k] = gk;
-        sm.pg[k] = p;
-        sm.d[k] = -p;
-        pgl = fmax(pgl, fabs(p));
-    }
-    double pgmax = block_max(pgl, sm.red);
-    const double pg_entry = pgmax;
-    const double tol = a.eps * fmax(1.0, pgmax);
+    // ---- control-warp state and steps (warp 0 of every block, all blocks identical) ----------------
+    int bad = 0, inner = 0, backtracks = 0, stop = 0, stall = 0, hit = 0, half = 0;
+    double F = 0.0, Gs = 0.0, Phi = 0.0, pgmax = 0.0, pg_entry = 0.0, tol = 0.0;
+    double phi1 = 0.0, Gd = 0.0, tmax = 0.0, qb = 0.0, yb = 0.0, t = 0.0, Gn = 0.0;
     const double c1a = 1e-4, noise = 2e-7;
-    int inner = 0, backtracks = 0, stop = 0, stall = 0;
 
-    while (pgmax > tol && !bad) {
-        if (inner >= a.max_inner) {
-            stop = 1;
-            break;
+    auto set_eval_scales = [&](double zb) {
+        const double dev = Tm + zb;
+        const FxScale sF = fx_scale_for(1.01 * Spd * ab * dev * dev, bad);
+        const FxScale sG = fx_scale_for(2.02 * ab * dev * l1max, bad);
+        if (lane == 0) {
+            sm.ctl->scF = sF.scale;
+            sm.ctl->iF = sF.inv;
+            sm.ctl->scG = sG.scale;
+            sm.ctl->iG = sG.inv;
         }
-        // slope along d; fall back to steepest descent if d is not a descent direction
-        double s = 0.0;
-        for (int k = tid; k < N; k += kMasterThreads) s += sm.grad[k] * sm.d[k];
-        double phi1 = block_sum(s, sm.red);
-        if (!(phi1 < 0.0)) {
-            s = 0.0;
-            for (int k = tid; k < N; k += kMasterThreads) {
-                sm.d[k] = -sm.pg[k];
-                s += sm.grad[k] * sm.d[k];
+    };
+    // everything the direction pass and the step rule need from (y, grad, d), in one sweep and one
+    // batched reduction: slope phi1 = grad.d, the dose bounds qb, yb (sum_k |v_k| max|d_k| >=
+    // max_j |sum_k v_k d_kj|), Gd = d^T L d = G(d), and the largest feasible step tmax
+    auto direction_sums = [&]() {
+        double s[4] = {0.0, 0.0, 0.0, 0.0}, tl = CUDART_INF;
+#pragma unroll 2
+        for (int k = lane; k < N; k += 32) {
+            const double dk = sm.d[k], yk = sm.y[k], lf = sm.linf[k];
+            s[0] += sm.grad[k] * dk;
+            s[1] += fabs(dk) * lf;
+            s[2] += fabs(yk) * lf;
+            if (k + 1 < N) {
+                const double dv = sm.d[k + 1] - dk;
+                s[3] += dv * dv * sm.rdt[k];
             }
-            phi1 = block_sum(s, sm.red);
+            tl = fmin(tl, dk < 0.0 ? yk / (-dk) : CUDART_INF);
+        }
+#pragma unroll
+        for (int o = 16; o; o >>= 1) {
+#pragma unroll
+            for (int m = 0; m < 4; ++m) s[m] += __shfl_xor_sync(kFull, s[m], o);
+            tl = fmin(tl, __shfl_xor_sync(kFull, tl, o));
+        }
+        phi1 = s[0];
+        qb = s[1];
+        yb = s[2];
+        Gd = s[3];
+        tmax = tl;
+    };
+    // slope along d (steepest descent if d does not descend) and the coefficients / scale of the
+    // direction pass.  Returns false (stop set) if no descent is possible.
+    auto prepare_direction = [&]() {
+        direction_sums();
+        if (!(phi1 < 0.0)) {
+            for (int k = lane; k < N; k += 32) sm.d[k] = -sm.pg[k];
+            __syncwarp();
+            direction_sums();
             if (!(phi1 < 0.0)) {
                 stop = 2;
-                break;
+                return false;
             }
         }
-        // q = Dc^T d and the curvature of the quadratic piece at t = 0
-        const double qb = dose_bound(sm.d), yb = dose_bound(sm.y);
-        const double scC = fx_scale_for(1.01 * Spd * ab * qb * qb, bad);
-        for (int i = tid; i < K; i += kMasterThreads) sm.coef[i] = (float)sm.d[sm.sk[i]];
-        __syncthreads();
+        const FxScale sC = fx_scale_for(1.01 * Spd * ab * qb * qb, bad);
+        for (int i = lane; i < K; i += 32) sm.coef[i] = (float)sm.d[sm.sk[i]];
+        if (lane == 0) {
+            sm.ctl->scC = sC.scale;
+            sm.ctl->iC = sC.inv;
+        }
+        return !bad;
+    };
+    // trial point y + t d (clamped), G and dG there
+    auto prepare_trial = [&]() {
+#pragma unroll 2
+        for (int k = lane; k < N; k += 32) {
+            const double yk = sm.y[k], dk = sm.d[k];
+            double v = yk + t * dk;
+            if (v < 0.0 || (hit && dk < 0.0 && yk / (-dk) <= tmax)) v = 0.0;
+            sm.yn[k] = v;
+        }
+        __syncwarp();
+        Gn = smooth_G(sm.yn, sm, N, lane, true);
+        if (lane == 0) sm.ctl->tf = (float)t;
+    };
+
+    // objective and gradient at the incoming y
+    if (warp == 0) {
+        double s = 0.0;
+        for (int k = lane; k < N; k += 32) s += fabs(sm.y[k]) * sm.linf[k];
+        set_eval_scales(wsum(s));
+        Gs = smooth_G(sm.y, sm, N, lane, true);
+    }
+    __syncthreads();
+    long long *rec = begin_pass();
+    eval_pass<true>(a, sm, K, ngroups, nullptr, zcur, 0.f, rec, sm.ctl->scF, sm.ctl->scG, red);
+    grid.sync();
+    ++ph;
+    fetch_record(rec);
+    if (warp == 0) {
+        const double iG = sm.ctl->iG;
+        double pgl = 0.0;
+        for (int k = lane; k < N; k += 32) {
+            const int i = sm.ik[k];
+            const double gk = i >= 0 ? (double)sm.recv[2 + i] * iG + a.gamma * sm.dG[k] : 0.0;
+            const double p = (i < 0 || (sm.y[k] <= 0.0 && gk >= 0.0)) ? 0.0 : gk;
+            sm.grad[k] = gk;
+            sm.pg[k] = p;
+            sm.d[k] = -p;
+            pgl = fmax(pgl, fabs(p));
+        }
+        __syncwarp();
+        F = (double)sm.recv[0] * sm.ctl->iF + a.F_out;
+        Phi = F + a.gamma * Gs;
+        pgmax = wmax(pgl);
+        pg_entry = pgmax;
+        tol = a.eps * fmax(1.0, pgmax);
+        int state = kRunDirection;
+        if (!(pgmax > tol) || bad) state = kFinish;
+        else if (a.max_inner <= 0) {
+            stop = 1;
+            state = kFinish;
+        } else if (!prepare_direction()) state = kFinish;
+        if (lane == 0) {
+            sm.ctl->state = state;
+            sm.ctl->accepted = 0;
+        }
+    }
+    __syncthreads();
+
+    PROF_DECL;
+    while (sm.ctl->state != kFinish) {
+        PROF(7)
+        // ---- q = Dc^T d and the curvature of the quadratic piece at t = 0 ------------------------------
         rec = begin_pass();
         double curv = 0.0;
         for (int g = 0; g < ngroups; ++g) {
@@ -544,114 +681,157 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
             }
             __syncthreads();
         }
-        curv = block_sum(curv, sm.red);
-        if (tid == 0) fx_add(rec + 1, curv, scC);
+        curv = block_sum(curv, red);
+        if (tid == 0) fx_add(rec + 1, curv, sm.ctl->scC);
+        PROF(0)
         grid.sync();
+        PROF(1)
         ++ph;
-        const double curvF = fx_get(rec + 1, scC);
-        const double phi2 = 2.0 * curvF + 2.0 * a.gamma * smooth_G(sm.d, sm, N);   // d^T L d = G(d)
-        double tl = CUDART_INF;
-        for (int k = tid; k < N; k += kMasterThreads)
-            if (sm.d[k] < 0.0) tl = fmin(tl, sm.y[k] / (-sm.d[k]));
-        const double tmax = block_min(tl, sm.red);
-        double t = phi2 > 0.0 ? -phi1 / phi2 : (isfinite(tmax) ? tmax : 1.0);
-        int hit = 0;
-        if (t >= tmax) {
-            t = tmax;
-            hit = 1;
+        if (warp == 0) {
+            const double curvF = (double)__ldcg(rec + 1) * sm.ctl->iC;
+            const double phi2 = 2.0 * curvF + 2.0 * a.gamma * Gd;
+            t = phi2 > 0.0 ? -phi1 / phi2 : (isfinite(tmax) ? tmax : 1.0);
+            hit = 0;
+            if (t >= tmax) {
+                t = tmax;
+                hit = 1;
+            }
+            half = 0;
+            set_eval_scales(yb + t * qb);   // |z + t q| <= sum_k (|y_k| + t |d_k|) max|d_k|; t only shrinks below
+            prepare_trial();
+            if (lane == 0) sm.ctl->state = bad ? kFinish : kRunTrial;
         }
-        eval_scales(yb + t * qb, scF, scG);   // |z + t q| <= sum_i (|y_i| + t |d_i|) max|d_i|; t only shrinks below
-        if (bad) break;
-        // backtracking on the true cost
-        bool accepted = false;
-        double Fn = 0.0, Gn = 0.0, Phin = 0.0;
-        for (int half = 0; half < 60; ++half) {
-            for (int k = tid; k < N; k += kMasterThreads) {
-                double v = sm.y[k] + t * sm.d[k];
-                if (v < 0.0 || (hit && sm.d[k] < 0.0 && sm.y[k] / (-sm.d[k]) <= tmax)) v = 0.0;
-                sm.yn[k] = v;
+        __syncthreads();
+        PROF(2)
+        // ---- backtracking on the true cost ----------------------------------------------------------------
+        while (sm.ctl->state == kRunTrial) {
+            rec = begin_pass();
+            eval_pass<false>(a, sm, K, ngroups, zcur, znext, sm.ctl->tf, rec, sm.ctl->scF, sm.ctl->scG, red);
+            PROF(3)
+            grid.sync();
+            PROF(4)
+            ++ph;
+            fetch_record(rec);
+            if (warp == 0) {
+                // gn = Dc w + gamma dG at the trial point, and the sums of the acceptance test and of the
+                // Polak-Ribiere+ update, in one sweep and one batched reduction
+                const double iG = sm.ctl->iG;
+                const double Fn = (double)sm.recv[0] * sm.ctl->iF + a.F_out;
+                double s[3] = {0.0, 0.0, 0.0}, pgm = 0.0;
+                int changed = hit;
+#pragma unroll 2
+                for (int k = lane; k < N; k += 32) {
+                    const int i = sm.ik[k];
+                    const double gk = i >= 0 ? (double)sm.recv[2 + i] * iG + a.gamma * sm.dG[k] : 0.0;
+                    const double yk = sm.yn[k], po = sm.pg[k];
+                    const double pn = (i < 0 || (yk <= 0.0 && gk >= 0.0)) ? 0.0 : gk;
+                    sm.gn[k] = gk;
+                    changed |= (pn == 0.0) != (po == 0.0);
+                    s[0] += pn * (pn - po);
+                    s[1] += po * po;
+                    s[2] += gk * sm.d[k];
+                    pgm = fmax(pgm, fabs(pn));
+                }
+#pragma unroll
+                for (int o = 16; o; o >>= 1) {
+#pragma unroll
+                    for (int m = 0; m < 3; ++m) s[m] += __shfl_xor_sync(kFull, s[m], o);
+                    pgm = fmax(pgm, __shfl_xor_sync(kFull, pgm, o));
+                }
+                changed = __any_sync(kFull, changed);
+                PROFW(5, 8)
+                const double Phin = Fn + a.gamma * Gn;
+                // sufficient decrease; below the resolution of Phi accept on the slope instead
+                const bool accepted = Phin <= Phi + c1a * t * phi1 ||
+                                      (Phin <= Phi + noise * fabs(Phi) && fabs(s[2]) <= 0.9 * fabs(phi1));
+                int state;
+                if (accepted) {
+                    // take the step; Polak-Ribiere+ direction on the current face, restart when the active set changes
+                    stall = (Phi - Phin <= 1e-8 * fabs(Phi)) ? stall + 1 : 0;
+                    F = Fn;
+                    Gs = Gn;
+                    Phi = Phin;
+                    pgmax = pgm;
+                    const double bpr = (changed || !(s[1] > 0.0) || s[0] <= 0.0) ? 0.0 : s[0] / s[1];
+#pragma unroll 2
+                    for (int k = lane; k < N; k += 32) {
+                        const double yk = sm.yn[k], gk = sm.gn[k];
+                        const bool off = sm.ik[k] < 0;
+                        const double pn = (off || (yk <= 0.0 && gk >= 0.0)) ? 0.0 : gk;
+                        double dk = -pn + bpr * sm.d[k];
+                        if (off || (yk <= 0.0 && dk < 0.0)) dk = 0.0;   // stay feasible
+                        sm.y[k] = yk;
+                        sm.grad[k] = gk;
+                        sm.pg[k] = pn;
+                        sm.d[k] = dk;
+                    }
+                    __syncwarp();
+                    PROFW(5, 9)
+                    ++inner;
+                    state = kRunDirection;
+                    if (!(pgmax > tol)) state = kFinish;
+                    else if (stall >= 3) {
+                        stop = 4;
+                        state = kFinish;
+                    } else if (inner >= a.max_inner) {
+                        stop = 1;
+                        state = kFinish;
+                    } else if (!prepare_direction()) state = kFinish;
+                } else {
+                    t *= 0.5;
+                    hit = 0;
+                    ++backtracks;
+                    state = kRunTrial;
+                    if (++half >= 60) {
+                        stop = 3;
+                        state = kFinish;
+                    } else prepare_trial();
+                }
+                PROFW(5, 10)
+                if (lane == 0) {
+                    sm.ctl->state = state;
+                    sm.ctl->accepted = accepted ? 1 : 0;
+                }
             }
             __syncthreads();
-            rec = begin_pass();
-            eval_pass<false>(a, sm, K, ngroups, zcur, znext, (float)t, rec, scF, scG);
-            grid.sync();
-            ++ph;
-            read_eval(rec, scF, scG, sm.yn, Fn, Gn);
-            Phin = Fn + a.gamma * Gn;
-            if (Phin <= Phi + c1a * t * phi1) accepted = true;
-            else if (Phin <= Phi + noise * fabs(Phi)) {
-                // below the resolution of Phi: accept on the slope instead
-                s = 0.0;
-                for (int k = tid; k < N; k += kMasterThreads) s += sm.gn[k] * sm.d[k];
-                const double phi1n = block_sum(s, sm.red);
-                if (fabs(phi1n) <= 0.9 * fabs(phi1)) accepted = true;
+            PROF(5)
+            if (sm.ctl->accepted) {
+                float *tmpz = zcur;
+                zcur = znext;
+                znext = tmpz;
             }
-            if (accepted) break;
-            t *= 0.5;
-            hit = 0;
-            ++backtracks;
-        }
-        if (!accepted) {
-            stop = 3;
-            break;
-        }
-        // take the step
-        stall = (Phi - Phin <= 1e-8 * fabs(Phi)) ? stall + 1 : 0;
-        float *tmpz = zcur;
-        zcur = znext;
-        znext = tmpz;
-        F = Fn;
-        Gs = Gn;
-        Phi = Phin;
-        // Polak-Ribiere+ direction on the current face, restart when the active set changes
-        double num = 0.0, den = 0.0, pgm = 0.0;
-        int changed = hit;
-        for (int k = tid; k < N; k += kMasterThreads) {
-            const double yk = sm.yn[k], gk = sm.gn[k];
-            const double pn = (!a.occ[k] || (yk <= 0.0 && gk >= 0.0)) ? 0.0 : gk;
-            const double po = sm.pg[k];
-            if ((pn == 0.0) != (po == 0.0)) changed = 1;
-            num += pn * (pn - po);
-            den += po * po;
-            pgm = fmax(pgm, fabs(pn));
-            sm.y[k] = yk;
-            sm.grad[k] = gk;
-            sm.pg[k] = pn;
-        }
-        changed = __syncthreads_or(changed);
-        num = block_sum(num, sm.red);
-        den = block_sum(den, sm.red);
-        pgmax = block_max(pgm, sm.red);
-        const double bpr = (changed || !(den > 0.0) || num <= 0.0) ? 0.0 : num / den;
-        for (int k = tid; k < N; k += kMasterThreads) {
-            double dk = -sm.pg[k] + bpr * sm.d[k];
-            if (!a.occ[k] || (sm.y[k] <= 0.0 && dk < 0.0)) dk = 0.0;   // stay feasible
-            sm.d[k] = dk;
-        }
-        __syncthreads();
-        ++inner;
-        if (stall >= 3 && pgmax > tol) {
-            stop = 4;
-            break;
         }
     }
-    if (bad) stop = 5;
+    PROF_END
 
     // z, w and the cost from the final y (no drift from the z += t q updates)
-    if ((inner > 0 || zcur != a.z) && !bad) {
-        eval_scales(dose_bound(sm.y), scF, scG);
-        for (int i = tid; i < K; i += kMasterThreads) sm.coef[i] = (float)sm.y[sm.sk[i]];
-        __syncthreads();
+    __syncthreads();
+    if (warp == 0) {
+        if (bad) stop = 5;
+        const int redo = (inner > 0 || zcur != a.z) && !bad;
+        if (redo) {
+            double s = 0.0;
+            for (int k = lane; k < N; k += 32) s += fabs(sm.y[k]) * sm.linf[k];
+            set_eval_scales(wsum(s));
+            Gs = smooth_G(sm.y, sm, N, lane, true);
+            for (int i = lane; i < K; i += 32) sm.coef[i] = (float)sm.y[sm.sk[i]];
+        }
+        if (lane == 0) sm.ctl->accepted = redo;
+    }
+    __syncthreads();
+    if (sm.ctl->accepted) {
         rec = begin_pass();
-        eval_pass<true>(a, sm, K, ngroups, nullptr, a.z, 0.f, rec, scF, scG);
+        eval_pass<true>(a, sm, K, ngroups, nullptr, a.z, 0.f, rec, sm.ctl->scF, sm.ctl->scG, red);
         grid.sync();
         ++ph;
-        read_eval(rec, scF, scG, sm.y, F, Gs);
-        Phi = F + a.gamma * Gs;
+        if (warp == 0) {
+            F = (double)__ldcg(rec) * sm.ctl->iF + a.F_out;
+            Phi = F + a.gamma * Gs;
+        }
     }
-    if (blockIdx.x == 0) {
-        for (int k = tid; k < N; k += kMasterThreads) a.y[k] = sm.y[k];
-        if (tid == 0) {
+    if (blockIdx.x == 0 && warp == 0) {
+        for (int k = lane; k < N; k += 32) a.y[k] = sm.y[k];
+        if (lane == 0) {
             *a.phase = ph % 3;
             MasterOut o;
             o.inner = inner;
@@ -679,8 +859,8 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
 
 size_t master_smem_bytes(int64_t N) {
     return (size_t)(kMasterWarps * kGroup * kChunk + kGroup * kChunk) * 4   // part, wbuf
-           + (size_t)(10 * N + kMasterWarps) * 8                             // K-vectors, red
-           + (size_t)N * 4 * 4;                                              // coef, sk, lo, hi
+           + (size_t)(11 * N + 2 + kMasterWarps) * 8 + sizeof(Ctl)           // K-vectors, recv, red, ctl
+           + (size_t)N * 4 * 5;                                              // coef, sk, lo, hi, ik
 }
 
 }  // namespace
@@ -774,6 +954,16 @@ int launch_master(vmat_plan *p, int trace_it) { return launch_master_impl(p, p->
 
 // steps (a)+(b) alone: the master kernel's evaluation pass with no iteration allowed
 int launch_dose_grad(vmat_plan *p) { return launch_master_impl(p, 0, -1); }
+
+#ifdef VMAT_MASTER_PROFILE
+extern "C" void vmat_debug_master_prof(long long out[16], int reset) {
+    cudaMemcpyFromSymbol(out, g_master_prof, sizeof(long long) * 16);
+    if (reset) {
+        long long z[16] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+        cudaMemcpyToSymbol(g_master_prof, z, sizeof(z));
+    }
+}
+#endif
 
 int launch_expand(vmat_plan *p, const float *src_s, float *dst_V, int what) {
     if (p->V == 0) return VMAT_OK;
