@@ -873,9 +873,8 @@ int master_configure(vmat_plan *p) {
     VMAT_CUDA(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_master, kMasterThreads, p->master_smem));
     if (per_sm < 1) return fail(p, VMAT_ECUDA, "master kernel does not fit on an SM");
     const int64_t nchunks = p->Sp / kChunk;
-    int64_t grid = p->sm_count;                       // one block per SM
-    const int64_t want = (nchunks + kGroup - 1) / kGroup;   // no more blocks than groups of chunks
-    if (grid > want) grid = want;
+    int64_t grid = p->sm_count;                       // one block per SM, chunks dealt round-robin
+    if (grid > nchunks) grid = nchunks;
     if (grid < 1) grid = 1;
     p->master_grid = (int)grid;
     int rc;
