@@ -37,9 +37,9 @@ def load_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-# ncu --set full capture of k_price_spmv_warp on this workload, dram__bytes_read.sum + dram__bytes_write.sum
-# per launch, first pricing launch of a solve (all 180 beams un-occupied); see profiles/r01_price_spmv.md
-NCU_TRAFFIC_BYTES_FIRST_LAUNCH = None
+# ncu --set full capture of k_price_spmv on configs[1] (profiles/r01_price_spmv.md): dram__bytes_read.sum +
+# dram__bytes_write.sum of the first pricing launch of a plan (all 180 beams un-occupied; 994,678,664 algorithmic bytes)
+NCU_TRAFFIC_BYTES_FIRST_LAUNCH = {"prostate": 992105216 + 4085248}
 
 
 class ClockSampler:
@@ -282,9 +282,11 @@ def main():
     peak, peak_src = load_peaks()
     achieved = sum(alg) / (ph_us["price"] * 1e-6) / 1e9
     roofline = {
-        "kernel": "k_price_spmv_warp (pricing SpMV, step c)", "bound": "hbm", "achieved": achieved, "peak": peak,
+        "kernel": "k_price_spmv<16,4> (pricing SpMV, step c)", "bound": "hbm", "achieved": achieved, "peak": peak,
         "unit": "GB/s", "frac": achieved / peak, "frac_of_8TBs_nominal": achieved / 8000.0,
-        "traffic": NCU_TRAFFIC_BYTES_FIRST_LAUNCH, "peak_source": peak_src,
+        "traffic": NCU_TRAFFIC_BYTES_FIRST_LAUNCH.get(c.name),
+        "traffic_note": "ncu dram bytes of the FIRST launch of a plan (compare algorithmic_bytes_first_launch)",
+        "peak_source": peak_src,
         "algorithmic_bytes_per_launch_avg": sum(alg) / iters, "algorithmic_bytes_first_launch": alg[0],
         "avg_launch_us": ph_us["price"] / iters, "launches_per_step": iters,
         "how": "CUDA events on the plan's stream around every pricing launch of the phase-timed steps",
