@@ -278,6 +278,30 @@ def main():
                      ("master", st.us_master), ("total", st.us_total)):
             ph_us[k] += v / args.steps
         inner_total += int(st.inner.sum())
+    # ---- steps (a)+(b) on the finished plan, both layouts (north_star: "chosen by measurement") -------------
+    occ_f, left_f, right_f, _ = plan.get_plan()
+    nnz_open = 0
+    for k in range(c.n_beams):
+        for r in range(c.n_rows):
+            i0 = (k * c.n_rows + r) * c.n_cols
+            nnz_open += int(ph.row_ptr[i0 + right_f[k, r]] - ph.row_ptr[i0 + left_f[k, r]])
+    dose = {"nnz_exposed": nnz_open, "exposed_fraction_of_nnz": nnz_open / ph.nnz}
+    for name, path in (("columns", 0), ("direct_atomics", 1)):
+        for _ in range(3):
+            plan.dose_recompute(path)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        nrep = 20
+        e0.record(stream)
+        for _ in range(nrep):
+            plan.dose_recompute(path)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        dose[name + "_us"] = e0.elapsed_time(e1) * 1e3 / nrep
+    # algorithmic bytes of the direct pass: the exposed rows (8 B per entry) + z, w out and T, alpha, beta in
+    dose_bytes = 8.0 * nnz_open + 20.0 * plan.n_support
+    dose["direct_atomics_GBs"] = dose_bytes / dose["direct_atomics_us"] / 1e3
+    dose["direct_algorithmic_bytes"] = dose_bytes
+    plan.dose_recompute(0)
     alg = pricing_algorithmic_bytes(ph.nnz, ph.n_beamlets, ph.n_voxels, c.n_beams, iters)
     peak, peak_src = load_peaks()
     achieved = sum(alg) / (ph_us["price"] * 1e-6) / 1e9
@@ -340,7 +364,7 @@ def main():
         "dtype": "f32", "data": "synthetic", "config": workload_config(ph, args),
         "plan_wall_time_ms": ms / args.steps, "final_cost": final_cost,
         "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
-        "phases": phases, "layout": info, "create_ms": create_ms, "generate_inputs_s": gen_s,
+        "phases": phases, "dose_pass": dose, "layout": info, "create_ms": create_ms, "generate_inputs_s": gen_s,
         "paper_context": "PAPER.md:157 whole plan 18-31 s (CUDA, Tesla C1060) / 5-8 min (MATLAB, Xeon) on clinical "
                          "cases of 1.8e7-5.5e7 non-zeros; different machine and data, not a target",
     }

@@ -81,7 +81,8 @@ typedef struct {
     int32_t validate;          /* 1: check the CSR and the voxel arrays on the device (default 1) */
     int32_t pricing_kernel;    /* 0 default; 1..5 lanes-per-beamlet x loads-in-flight variants of the
                                   pricing product (32x2, 32x4, 16x2, 16x4, 8x4), for measurement   */
-    int32_t dose_path;         /* 0 aperture columns (default), 1 direct fixed-point scatter      */
+    int32_t dose_path;         /* how vmat_dose forms z: 0 from the aperture-dose columns d_k the
+                                  master keeps (default), 1 straight from D (fixed-point atomics)  */
     double  master_eps;        /* stop when max|projected gradient| <= eps*max(1, value at entry) */
     int32_t master_max_inner;  /* cap on inner iterations of one master solve                     */
     int32_t record_phases;     /* 1: vmat_solve brackets each phase with CUDA events              */
@@ -138,6 +139,12 @@ int vmat_get_info(const vmat_plan *plan, vmat_info *out);
 /* Steps (a)+(b) for the plan's current apertures and dose rates.
  * z_dev / w_dev: DEVICE, V floats, or NULL.  cost: HOST, {F, G, F + gamma G}, or NULL.        */
 int vmat_dose(vmat_plan *plan, float *z_dev, float *w_dev, double cost[3]);
+
+/* Steps (a)+(b) again, even if the plan's z and w are current: dose_path 0 = z = sum_k y_k d_k from
+ * the aperture-dose columns, 1 = z = sum_k y_k sum_{i in A_k} D_i. straight from the CSR rows of
+ * the exposed beamlets, -1 = the plan's option.  Stream-ordered, no host sync;
+ * read the result with vmat_dose.  Exists so that the two layouts can be timed and compared.   */
+int vmat_dose_recompute(vmat_plan *plan, int dose_path);
 
 /* Steps (b)->(c)->(d): prices of all beamlets of un-occupied beams from the
  * current penalty gradient, the row search, the beam choice.

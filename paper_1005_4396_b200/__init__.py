@@ -26,7 +26,8 @@ VMAT_HOST, VMAT_DEVICE = 0, 1
 
 # every symbol include/vmat.h declares
 SYMBOLS = (
-    "vmat_default_options", "vmat_create", "vmat_destroy", "vmat_get_info", "vmat_dose", "vmat_price",
+    "vmat_default_options", "vmat_create", "vmat_destroy", "vmat_get_info", "vmat_dose", "vmat_dose_recompute",
+    "vmat_price",
     "vmat_price_spmv", "vmat_leaf_search", "vmat_master", "vmat_solve", "vmat_get_plan", "vmat_set_plan",
     "vmat_launch_count", "vmat_last_error",
 )
@@ -91,6 +92,7 @@ def load_library():
     L.vmat_destroy.argtypes = [_P]
     L.vmat_get_info.argtypes = [_P, C.POINTER(_Info)]
     L.vmat_dose.argtypes = [_P, _P, _P, _P]
+    L.vmat_dose_recompute.argtypes = [_P, C.c_int]
     L.vmat_price.argtypes = [_P, _P, _P, _P, C.POINTER(_Aperture), C.c_int]
     L.vmat_price_spmv.argtypes = [_P, _P, _P]
     L.vmat_leaf_search.argtypes = [_P, _P, _P, _P, _P]
@@ -102,7 +104,8 @@ def load_library():
     L.vmat_launch_count.restype = C.c_int64
     L.vmat_last_error.argtypes = [_P]
     L.vmat_last_error.restype = C.c_char_p
-    for name in ("vmat_create", "vmat_destroy", "vmat_get_info", "vmat_dose", "vmat_price", "vmat_price_spmv",
+    for name in ("vmat_create", "vmat_destroy", "vmat_get_info", "vmat_dose", "vmat_dose_recompute", "vmat_price",
+                 "vmat_price_spmv",
                  "vmat_leaf_search", "vmat_master", "vmat_solve", "vmat_get_plan", "vmat_set_plan"):
         getattr(L, name).restype = C.c_int
     _lib = L
@@ -262,6 +265,10 @@ class Plan:
         self._check(self._L.vmat_dose(self._h, _dev_ptr(z, "float32", self.V), _dev_ptr(w, "float32", self.V),
                                       C.addressof(cost) if want_cost else None))
         return tuple(cost) if want_cost else None
+
+    def dose_recompute(self, dose_path: int = -1):
+        """vmat_dose_recompute: run steps (a)+(b) again by the given path (0 columns, 1 from D).  Stream-ordered."""
+        self._check(self._L.vmat_dose_recompute(self._h, int(dose_path)))
 
     def price(self, w_override=None, g_override=None, g_out=None, commit: bool = False) -> Optional[Aperture]:
         """vmat_price.  Returns the chosen Aperture, or None when every beam is occupied."""

@@ -41,14 +41,23 @@ static int ensure_columns(vmat_plan *p) {
     return VMAT_OK;
 }
 
-// z, w and the cost for the current (occ, leaves, y)
-static int ensure_state(vmat_plan *p) {
-    if (p->state_valid) return VMAT_OK;
-    int rc = ensure_columns(p);
-    if (rc) return rc;
-    if ((rc = launch_dose_grad(p))) return rc;
+// steps (a)+(b): z, w and the cost for the current (occ, leaves, y), by the aperture-dose columns
+// (path 0) or straight from D (path 1)
+static int evaluate_state(vmat_plan *p, int path) {
+    int rc;
+    if (path == 1) {
+        if ((rc = launch_direct_dose(p))) return rc;
+    } else {
+        if ((rc = ensure_columns(p))) return rc;
+        if ((rc = launch_dose_grad(p))) return rc;
+    }
     p->state_valid = true;
     return VMAT_OK;
+}
+
+static int ensure_state(vmat_plan *p) {
+    if (p->state_valid) return VMAT_OK;
+    return evaluate_state(p, p->opt.dose_path == 1 ? 1 : 0);
 }
 
 static int refresh_host_occ(vmat_plan *p) {
@@ -195,6 +204,7 @@ int vmat_create(const vmat_problem *pb, const vmat_options *options, void *cuda_
     if ((e = cudaMemcpyAsync(p->theta, pb->theta_deg, (size_t)N * 8, cudaMemcpyHostToDevice, st)) != cudaSuccess)
         return bail(cuda_fail(p, e, "cudaMemcpyAsync(theta)"));
     if ((rc = master_configure(p))) return bail(rc);
+    if ((rc = dose_configure(p))) return bail(rc);
     if ((rc = launch_free_list(p))) return bail(rc);
     if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return bail(cuda_fail(p, e, "cudaStreamSynchronize"));
     p->h_occ.assign((size_t)N, 0);
@@ -236,6 +246,12 @@ int vmat_dose(vmat_plan *p, float *z_dev, float *w_dev, double cost[3]) {
         VMAT_CUDA(p, cudaStreamSynchronize(p->stream));
     }
     return VMAT_OK;
+}
+
+int vmat_dose_recompute(vmat_plan *p, int dose_path) {
+    if (!p) return VMAT_EINVAL;
+    if (dose_path < -1 || dose_path > 1) return fail(p, VMAT_EINVAL, "dose_path must be -1, 0 or 1");
+    return evaluate_state(p, dose_path < 0 ? (p->opt.dose_path == 1 ? 1 : 0) : dose_path);
 }
 
 int vmat_price_spmv(vmat_plan *p, const float *w_dev, float *g_dev) {
@@ -371,6 +387,7 @@ int vmat_solve(vmat_plan *p, int32_t max_iters, vmat_solve_stats *out) {
     }
     TRYC(cudaEventRecord(ev0, st));
     TRY(ensure_state(p));
+    TRY(ensure_columns(p));   // the master needs d_k of every occupied beam, whichever path formed z
     for (int64_t it = 0; it < todo; ++it) {
         if (phases) TRYC(cudaEventRecord(evs[it * 5 + 0], st));
         TRY(launch_price_spmv(p, p->w_s, p->g, (int)(n_free0 - it)));              // (c)

@@ -90,7 +90,8 @@ struct vmat_plan {
     size_t master_smem = 0;
     vmat::MasterOut *mout = nullptr;
     double *cost3 = nullptr;       // device {F, G, F+gamma G}
-    double *part_dose = nullptr;   // partial F sums of the dose kernel
+    double *part_dose = nullptr;   // partial F sums of the direct dose pass
+    void *dose_scale = nullptr;    // device scalars of the direct dose pass (vmat_dose.cu)
     int dose_blocks = 0;
 
     // device trace of vmat_solve
@@ -154,6 +155,9 @@ int launch_dose_grad(vmat_plan *p);
 int launch_master(vmat_plan *p, int trace_it);
 int launch_expand(vmat_plan *p, const float *src_s, float *dst_V, int what /*0 z, 1 w*/);
 int launch_compress(vmat_plan *p, const float *src_V, float *dst_s);
+
+// vmat_dose.cu: steps (a)+(b) straight from D (fixed-point atomics path) ------------------------------
+int dose_configure(vmat_plan *p);
 int launch_direct_dose(vmat_plan *p);
 
 }  // namespace vmat

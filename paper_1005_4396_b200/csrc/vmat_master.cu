@@ -981,6 +981,4 @@ int launch_compress(vmat_plan *p, const float *src_V, float *dst_s) {
     return VMAT_OK;
 }
 
-int launch_direct_dose(vmat_plan *p) { return fail(p, VMAT_ESTATE, "direct dose path not built"); }
-
 }  // namespace vmat

@@ -116,6 +116,13 @@ def test_full_plan_properties(setup):
     assert relnorm(z.cpu().numpy(), z_ref) <= TOL
     assert abs(cost - (F_ref + o.gamma * G_ref)) <= TOL * abs(F_ref + o.gamma * G_ref)
     assert abs(st.cost - cost) <= 1e-6 * abs(cost)
+    # the dose straight from D (atomics path) agrees with the oracle and with the column path
+    plan.dose_recompute(1)
+    z1 = torch.empty(o.V, dtype=torch.float32, device="cuda")
+    _, _, cost1 = plan.dose(z1)
+    assert relnorm(z1.cpu().numpy(), z_ref) <= TOL
+    assert abs(cost1 - (F_ref + o.gamma * G_ref)) <= TOL * abs(F_ref + o.gamma * G_ref)
+    plan.dose_recompute(0)
     # the finished y is (up to fp32 noise) the minimiser of the oracle's master problem on this aperture set:
     # warm-started from it, the oracle's own gradient projection cannot lower the cost by more than TOL
     _, _, info = o.master(occ, left, right, y0=y, eps=1e-7, max_inner=40)

@@ -179,10 +179,12 @@ def test_all_beams_occupied_is_done(torch_cuda, vm):
 # ------------------------------------------------------------------------------------------------
 # P1 (a)+(b): dose and penalty gradient
 # ------------------------------------------------------------------------------------------------
-def check_dose(torch, plan, o, occ, left, right, y):
+def check_dose(torch, plan, o, occ, left, right, y, path=-1):
     plan.set_plan(occ, left, right, y)
     z = torch.empty(o.V, dtype=torch.float32, device="cuda")
     w = torch.empty(o.V, dtype=torch.float32, device="cuda")
+    if path >= 0:
+        plan.dose_recompute(path)              # 0: aperture-dose columns, 1: straight from D (atomics path)
     F, G, cost = plan.dose(z, w)
     z_ref = o.dose(occ, left, right, y)
     F_ref, w_ref = o.penalty(z_ref)
@@ -194,21 +196,49 @@ def check_dose(torch, plan, o, occ, left, right, y):
     assert abs(cost - (F_ref + o.gamma * G_ref)) <= TOL * abs(F_ref + o.gamma * G_ref)
 
 
-def test_dose_and_gradient_match_oracle_tiny(torch_cuda, vm, tiny_oracle):
+@pytest.mark.parametrize("path", [0, 1])
+def test_dose_and_gradient_match_oracle_tiny(torch_cuda, vm, tiny_oracle, path):
     o = tiny_oracle
     plan = make_plan(vm, o)
     for occ, left, right, y in oracle_states(o, 24, every=6):
-        check_dose(torch_cuda, plan, o, occ, left, right, y)
+        check_dose(torch_cuda, plan, o, occ, left, right, y, path)
     plan.destroy()
 
 
-def test_dose_random_problems_with_unreachable_voxels(torch_cuda, vm):
+@pytest.mark.parametrize("path", [0, 1])
+def test_dose_random_problems_with_unreachable_voxels(torch_cuda, vm, path):
     for seed in range(3):
         o = random_problem(20 + seed)
         plan = make_plan(vm, o)
         for occ, left, right, y in oracle_states(o, 5, every=2):
-            check_dose(torch_cuda, plan, o, occ, left, right, y * 1.3)     # off-optimum dose rates too
+            check_dose(torch_cuda, plan, o, occ, left, right, y * 1.3, path)     # off-optimum dose rates too
         plan.destroy()
+
+
+def test_direct_dose_option_runs_the_whole_loop(torch_cuda, vm, tiny_oracle):
+    # dose_path = 1 as the plan's own path: the state a resumed plan starts from is established by the direct
+    # pass; the loop then picks the same apertures as with the column path, and the pass is reproducible
+    o = tiny_oracle
+    occ, left, right, y = oracle_states(o, 6, every=6)[1]
+    runs = {}
+    for path in (0, 1, 1):
+        opt = vm.default_options()
+        opt.dose_path = path
+        plan = make_plan(vm, o, options=opt)
+        plan.set_plan(occ, left, right, y)
+        st = plan.solve(40)
+        z = torch_cuda.empty(o.V, dtype=torch_cuda.float32, device="cuda")
+        plan.dose_recompute(path)
+        runs.setdefault(path, []).append((st, plan.dose(z), z.cpu().numpy().copy(), plan.get_plan()))
+        plan.destroy()
+    (s0, c0, z0, p0), (s1, c1, z1, p1), (s2, c2, z2, p2) = runs[0][0], runs[1][0], runs[1][1]
+    assert s0.iters == s1.iters == o.N - 6
+    assert np.array_equal(s0.beam, s1.beam) and np.array_equal(p0[1], p1[1]) and np.array_equal(p0[2], p1[2])
+    assert relnorm(s1.trace_cost, s0.trace_cost) <= 1e-6
+    assert relnorm(z1, z0) <= 1e-6 and abs(c1[2] - c0[2]) <= 1e-6 * abs(c0[2])
+    assert c1 == c2 and np.array_equal(z1, z2)                 # order-free accumulation: bit identical
+    z_ref = o.dose(*p1)
+    assert relnorm(z1, z_ref) <= TOL
 
 
 # ------------------------------------------------------------------------------------------------
