@@ -162,6 +162,92 @@ def aggregate_over_ranks(ms, done_iters, launches, dist, device):
     return float(t.item()), int(n[0].item()), int(n[1].item())
 
 
+def run_sweep(args):
+    """BASELINE.json configs[3]: the pricing product g = D w in isolation on synthetic beamlet-major CSR
+    (row lengths U[200,800], voxel ids in runs of 8-64, w ~ N(0,1)), and the leaf-row search on 180 x 40 rows of
+    40-80 beamlets.  One JSON line per point; GB/s = algorithmic bytes (8 nnz + 12 rows + 4 V) / kernel time."""
+    import torch
+
+    import __graft_entry__ as entry
+
+    entry.build()
+    import paper_1005_4396_b200 as vm
+    import vmat_inputs
+
+    torch.cuda.set_device(0)
+    peak, peak_src = load_peaks()
+    R, C = 80, 200                                     # rows are grouped as "beams" of R*C beamlets
+    for nnz_target in [int(float(x)) for x in args.sweep_nnz.split(",")]:
+        for V in [int(float(x)) for x in args.sweep_voxels.split(",")]:
+            row_ptr, col, val = vmat_inputs.make_sweep_matrix(nnz_target, V, seed=0)
+            rows = row_ptr.size - 1
+            N = (rows + R * C - 1) // (R * C)
+            row_ptr = np.concatenate([row_ptr, np.full(N * R * C - rows, row_ptr[-1], np.int64)])
+            w = vmat_inputs.make_normal(V, seed=1)
+            # alpha = beta = 1 and T = -w/2 make the empty plan's own penalty gradient (Eq. 1 at z = 0) equal w
+            # exactly, so vmat_price_spmv(NULL) is the kernel alone (no staging of a caller-supplied gradient)
+            one = np.ones(V, np.float32)
+            opt = vm.default_options()
+            opt.validate = 0
+            plan = vm.Plan.create(row_ptr, col, val, (-0.5 * w).astype(np.float32), one, one,
+                                  np.arange(N, dtype=np.float64), R, C, 2, 0.1, options=opt)
+            g = torch.empty(N * R * C, dtype=torch.float32, device="cuda")
+            wd = torch.empty(V, dtype=torch.float32, device="cuda")
+            plan.dose(None, wd)
+            assert np.array_equal(wd.cpu().numpy(), w), "plan gradient differs from the sweep's w"
+            for _ in range(3):
+                plan.price_spmv(g)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            nrep = 10
+            e0.record()
+            for _ in range(nrep):
+                plan.price_spmv(g)
+            e1.record()
+            torch.cuda.synchronize()
+            us = e0.elapsed_time(e1) * 1e3 / nrep
+            nnz = int(row_ptr[-1])
+            alg = 8.0 * nnz + 12.0 * rows + 4.0 * V
+            # spot check against the definition on a few rows (fp64 on the host, not the oracle: a plain dot)
+            gh = g.cpu().numpy()
+            for i in np.random.default_rng(0).integers(0, rows, 50):
+                a, b = row_ptr[i], row_ptr[i + 1]
+                ref = float(np.dot(val[a:b].astype(np.float64), w[col[a:b]].astype(np.float64)))
+                mag = float(np.dot(np.abs(val[a:b]).astype(np.float64), np.abs(w[col[a:b]]).astype(np.float64)))
+                assert abs(gh[i] - ref) <= 1e-5 * mag + 1e-30, (i, gh[i], ref)
+            print(json.dumps({"sweep": "pricing_spmv", "nnz": nnz, "rows": rows, "voxels": V, "us": us,
+                              "GBs": alg / us / 1e3, "frac_of_peak": alg / us / 1e3 / peak, "peak": peak,
+                              "peak_source": peak_src, "algorithmic_bytes": alg,
+                              "support_voxels": plan.n_support}), flush=True)
+            plan.destroy()
+            del g, wd
+            torch.cuda.empty_cache()
+    # leaf-row search on 180 x 40 rows
+    for Cs in (40, 60, 80):
+        N, Rs = 180, 40
+        B = N * Rs * Cs
+        opt = vm.default_options()
+        plan = vm.Plan.create(np.zeros(B + 1, np.int64), np.zeros(1, np.int32), np.zeros(1, np.float32),
+                              np.zeros(4, np.float32), np.zeros(4, np.float32), np.zeros(4, np.float32),
+                              np.arange(N, dtype=np.float64) * 2.0, Rs, Cs, 2, 0.1, options=opt)
+        gd = torch.from_numpy(vmat_inputs.make_search_rows(N, Rs, Cs, seed=0)).cuda()
+        al = torch.zeros(N * Rs, dtype=torch.int32, device="cuda")
+        ar = torch.zeros(N * Rs, dtype=torch.int32, device="cuda")
+        bp = torch.zeros(N, dtype=torch.float64, device="cuda")
+        for _ in range(3):
+            plan.leaf_search(gd, al, ar, bp)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        nrep = 50
+        e0.record()
+        for _ in range(nrep):
+            plan.leaf_search(gd, al, ar, bp)
+        e1.record()
+        torch.cuda.synchronize()
+        us = e0.elapsed_time(e1) * 1e3 / nrep
+        print(json.dumps({"sweep": "leaf_search", "beams": N, "leaf_rows": Rs, "leaf_cols": Cs, "us": us,
+                          "rows_per_s": N * Rs / (us * 1e-6)}), flush=True)
+        plan.destroy()
+
+
 def workload_config(ph, args):
     c = ph.config
     return {
@@ -186,7 +272,12 @@ def main():
     ap.add_argument("--ref-budget-s", type=float, default=15.0, help="CPU seconds per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--sweep", action="store_true", help="configs[3]: isolated pricing / search kernel sweep")
+    ap.add_argument("--sweep-nnz", default="5e7,1e8,2.5e8,5e8,1e9")
+    ap.add_argument("--sweep-voxels", default="1048576,2097152,4194304")
     args = ap.parse_args()
+    if args.sweep:
+        return run_sweep(args)
     if args.warmup < 3 and args.impl == "b200":
         args.warmup = 3
     if args.impl == "reference":

@@ -263,8 +263,9 @@ int vmat_price_spmv(vmat_plan *p, const float *w_dev, float *g_dev) {
         w_s = p->wtmp_s;
     } else if ((rc = ensure_state(p))) return rc;
     // the kernel covers the un-occupied beams only: the caller's buffer gets its zeros here
-    VMAT_CUDA(p, cudaMemsetAsync(g_dev, 0, (size_t)p->B * 4, p->stream));
-    return launch_price_spmv(p, w_s, g_dev, (int)unoccupied(p));
+    const int64_t n_free = unoccupied(p);
+    if (n_free < p->N) VMAT_CUDA(p, cudaMemsetAsync(g_dev, 0, (size_t)p->B * 4, p->stream));
+    return launch_price_spmv(p, w_s, g_dev, (int)n_free);
 }
 
 int vmat_leaf_search(vmat_plan *p, const float *g_dev, int32_t *all_left_dev, int32_t *all_right_dev,
