@@ -20,8 +20,7 @@ def relnorm(a, ref):
     return np.max(np.abs(np.asarray(a, np.float64) - ref)) / max(np.max(np.abs(ref)), 1e-300)
 
 
-@pytest.fixture(scope="module")
-def setup():
+def _setup(name):
     import torch
 
     assert torch.cuda.is_available(), "GPU tests need a CUDA device"
@@ -29,19 +28,58 @@ def setup():
     import vmat_inputs
     from oracle import Oracle
 
-    ph = vmat_inputs.make_phantom("prostate", seed=0)
+    ph = vmat_inputs.make_phantom(name, seed=0)
     o = Oracle.from_phantom(ph)
     plan = vm.Plan.from_phantom(ph)
-    yield torch, vm, ph, o, plan
-    plan.destroy()
+    return torch, vm, ph, o, plan
+
+
+@pytest.fixture(scope="module")
+def setup():
+    s = _setup("prostate")
+    yield s
+    s[4].destroy()
+
+
+@pytest.fixture(scope="module")
+def setup_hn():
+    # BASELINE.json configs[2]: head-and-neck-like phantom, 432,000 beamlets, 2.9e8 non-zeros
+    s = _setup("hn")
+    yield s
+    s[4].destroy()
 
 
 def test_teacher_forced_steps_fullsize(setup):
+    _teacher_forced(setup, 3)
+
+
+def test_teacher_forced_steps_head_and_neck(setup_hn):
+    _teacher_forced(setup_hn, 2)
+    # and a stretch of the free-running loop: invariants that hold at any size
+    torch, vm, ph, o, plan = setup_hn
+    st = plan.solve(25)
+    occ, left, right, y = plan.get_plan()
+    assert st.iters == 25 and occ.sum() == 27 and np.all(y >= 0) and np.all(y[occ == 0] == 0)
+    assert np.all(np.diff(st.trace_cost) <= 1e-5 * np.abs(st.trace_cost[:-1]))
+    ks = np.flatnonzero(occ)
+    for a, b in zip(ks[:-1], ks[1:]):                                          # S6 between successive occupied beams
+        lim = o.delta * (b - a)
+        assert np.all(np.abs(left[b] - left[a]) <= lim) and np.all(np.abs(right[b] - right[a]) <= lim)
+    z = torch.empty(o.V, dtype=torch.float32, device="cuda")
+    _, _, cost = plan.dose(z)
+    z_ref = o.dose(occ, left, right, y)
+    F_ref, _ = o.penalty(z_ref)
+    G_ref, _ = o.smooth(y)
+    assert relnorm(z.cpu().numpy(), z_ref) <= TOL
+    assert abs(cost - (F_ref + o.gamma * G_ref)) <= TOL * abs(F_ref + o.gamma * G_ref)
+
+
+def _teacher_forced(setup, n_iters):
     torch, vm, ph, o, plan = setup
     occ, left, right, y = o.empty_plan()
     left, right = left.reshape(o.N, o.R), right.reshape(o.N, o.R)
     rng = np.random.default_rng(0)
-    for it in range(3):
+    for it in range(n_iters):
         plan.set_plan(occ, left, right, y)
         # (a)+(b) dose and gradient of the current plan
         z = torch.empty(o.V, dtype=torch.float32, device="cuda")
