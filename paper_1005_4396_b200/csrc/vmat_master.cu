@@ -183,7 +183,8 @@ struct MasterArgs {
     const double *theta;
     const ColStat *colstat;
     int N;
-    double gamma, F_out, eps, fx_inv;
+    double gamma, F_out, eps, fx_inv, stall_rel;
+    int stall_count;
     float Tmax, abmax;
     int max_inner;
     long long *accbuf;          // 3 rotating records of (N + 2) fixed-point sums: F, curvature, grad[0..K)
@@ -747,7 +748,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
                 int state;
                 if (accepted) {
                     // take the step; Polak-Ribiere+ direction on the current face, restart when the active set changes
-                    stall = (Phi - Phin <= 1e-8 * fabs(Phi)) ? stall + 1 : 0;
+                    stall = (Phi - Phin <= a.stall_rel * fabs(Phi)) ? stall + 1 : 0;
                     F = Fn;
                     Gs = Gn;
                     Phi = Phin;
@@ -770,7 +771,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
                     ++inner;
                     state = kRunDirection;
                     if (!(pgmax > tol)) state = kFinish;
-                    else if (stall >= 3) {
+                    else if (stall >= a.stall_count) {
                         stop = 4;
                         state = kFinish;
                     } else if (inner >= a.max_inner) {
@@ -928,6 +929,8 @@ static int launch_master_impl(vmat_plan *p, int max_inner, int trace_it) {
     a.gamma = p->gamma;
     a.F_out = p->F_out;
     a.eps = p->opt.master_eps;
+    a.stall_rel = p->opt.master_stall_rel;
+    a.stall_count = p->opt.master_stall_count;
     a.max_inner = max_inner;
     a.colstat = p->colstat;
     a.fx_inv = p->fx_inv;
