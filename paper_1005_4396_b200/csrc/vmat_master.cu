@@ -277,6 +277,8 @@ struct Ctl {
 };
 enum { kRunDirection = 0, kRunTrial = 1, kFinish = 2 };
 
+constexpr int kRedSlots = 6;   // values per warp row of the control group's reduction scratch
+
 struct Smem {
     double *y, *d, *grad, *pg, *yn, *gn, *dG, *rdt, *gacc, *linf;   // N each (control warp; gacc: all warps)
     float *part, *wbuf, *coef;
@@ -414,27 +416,45 @@ __device__ __forceinline__ void eval_pass(const MasterArgs &a, const Smem &sm, i
     for (int i = tid; i < K; i += kMasterThreads) fx_add(rec + 2 + i, sm.gacc[i], scG);
 }
 
-// ---- control-warp helpers: every lane of warp 0 ends with the same value, fixed order ------------
-__device__ __forceinline__ double wsum(double v) {
+// ---- control group: the first nw warps of a block (CT = 32 nw threads) share the N-vector work -----
+__device__ __forceinline__ void ctl_sync(int CT) { asm volatile("bar.sync 1, %0;" ::"r"(CT) : "memory"); }
+
+// Batched reduction over the control group: MS sums and one maximum at once, fixed order, every thread of the
+// group receives the results.  One barrier per call: the scratch alternates (tog), so a call never overwrites
+// what a slower warp is still reading from the call before.
+template <int MS>
+__device__ __forceinline__ void ctl_reduce(double (&s)[MS], double &mx, double *cred, int &tog, int nw, int CT) {
+    static_assert(MS < kRedSlots, "scratch row too short");
 #pragma unroll
-    for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
-    return v;
-}
-__device__ __forceinline__ double wmax(double v) {
+    for (int o = 16; o; o >>= 1) {
 #pragma unroll
-    for (int o = 16; o; o >>= 1) v = fmax(v, __shfl_xor_sync(kFull, v, o));
-    return v;
-}
-__device__ __forceinline__ double wmin(double v) {
+        for (int m = 0; m < MS; ++m) s[m] += __shfl_xor_sync(kFull, s[m], o);
+        mx = fmax(mx, __shfl_xor_sync(kFull, mx, o));
+    }
+    double *buf = cred + tog * (kMasterWarps * kRedSlots);
+    tog ^= 1;
+    if ((threadIdx.x & 31) == 0) {
+        double *row = buf + (threadIdx.x >> 5) * kRedSlots;
 #pragma unroll
-    for (int o = 16; o; o >>= 1) v = fmin(v, __shfl_xor_sync(kFull, v, o));
-    return v;
+        for (int m = 0; m < MS; ++m) row[m] = s[m];
+        row[kRedSlots - 1] = mx;
+    }
+    ctl_sync(CT);
+#pragma unroll
+    for (int m = 0; m < MS; ++m) s[m] = 0.0;
+    mx = -CUDART_INF;
+    for (int w = 0; w < nw; ++w) {
+#pragma unroll
+        for (int m = 0; m < MS; ++m) s[m] += buf[w * kRedSlots + m];
+        mx = fmax(mx, buf[w * kRedSlots + kRedSlots - 1]);
+    }
 }
 
-// G(v) = sum_k (v_{k+1}-v_k)^2 / (theta_{k+1}-theta_k) and dG/dv_k   (Eq. 2; S2, S3)
-__device__ __forceinline__ double smooth_G(const double *v, const Smem &sm, int N, int lane, bool want_dG) {
+// this thread's share of G(v) = sum_k (v_{k+1}-v_k)^2 / (theta_{k+1}-theta_k), and dG/dv_k -> sm.dG
+// (Eq. 2; S2, S3)
+__device__ __forceinline__ double smooth_part(const double *v, const Smem &sm, int N, int CT, bool want_dG) {
     double s = 0.0;
-    for (int k = lane; k < N; k += 32) {
+    for (int k = threadIdx.x; k < N; k += CT) {
         const double e1 = k + 1 < N ? (v[k + 1] - v[k]) * sm.rdt[k] : 0.0;      // (v_{k+1}-v_k)/dtheta_k
         if (k + 1 < N) s += (v[k + 1] - v[k]) * e1;
         if (want_dG) {
@@ -442,8 +462,7 @@ __device__ __forceinline__ double smooth_G(const double *v, const Smem &sm, int 
             sm.dG[k] = 2.0 * (e0 - e1);
         }
     }
-    __syncwarp();
-    return wsum(s);
+    return s;
 }
 
 __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a) {
@@ -464,7 +483,8 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     sm.gacc = sm.rdt + N;
     sm.linf = sm.gacc + N;
     double *red = sm.linf + N;
-    sm.recv = reinterpret_cast<long long *>(red + kMasterWarps);
+    double *cred = red + kMasterWarps;   // 2 x kMasterWarps x kRedSlots
+    sm.recv = reinterpret_cast<long long *>(cred + 2 * kMasterWarps * kRedSlots);
     sm.ctl = reinterpret_cast<Ctl *>(sm.recv + N + 2);
     sm.coef = reinterpret_cast<float *>(sm.ctl + 1);
     sm.sk = reinterpret_cast<int *>(sm.coef + N);
@@ -535,7 +555,11 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
         __syncthreads();
     };
 
-    // ---- control-warp state and steps (warp 0 of every block, all blocks identical) ----------------
+    // ---- control group: the first nw warps of every block share the N-vector work (one entry per thread
+    // for N <= 512); every thread of the group carries the same scalars, all blocks take the same decisions
+    const int nw = min(kMasterWarps, (N + 31) / 32), CT = nw * 32;
+    const bool ctl = warp < nw;
+    int tog = 0;
     int bad = 0, inner = 0, backtracks = 0, stop = 0, stall = 0, hit = 0, half = 0;
     double F = 0.0, Gs = 0.0, Phi = 0.0, pgmax = 0.0, pg_entry = 0.0, tol = 0.0;
     double phi1 = 0.0, Gd = 0.0, tmax = 0.0, qb = 0.0, yb = 0.0, t = 0.0, Gn = 0.0;
@@ -545,7 +569,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
         const double dev = Tm + zb;
         const FxScale sF = fx_scale_for(1.01 * Spd * ab * dev * dev, bad);
         const FxScale sG = fx_scale_for(2.02 * ab * dev * l1max, bad);
-        if (lane == 0) {
+        if (tid == 0) {
             sm.ctl->scF = sF.scale;
             sm.ctl->iF = sF.inv;
             sm.ctl->scG = sG.scale;
@@ -556,9 +580,8 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     // batched reduction: slope phi1 = grad.d, the dose bounds qb, yb (sum_k |v_k| max|d_k| >=
     // max_j |sum_k v_k d_kj|), Gd = d^T L d = G(d), and the largest feasible step tmax
     auto direction_sums = [&]() {
-        double s[4] = {0.0, 0.0, 0.0, 0.0}, tl = CUDART_INF;
-#pragma unroll 2
-        for (int k = lane; k < N; k += 32) {
+        double s[4] = {0.0, 0.0, 0.0, 0.0}, ntl = -CUDART_INF;
+        for (int k = tid; k < N; k += CT) {
             const double dk = sm.d[k], yk = sm.y[k], lf = sm.linf[k];
             s[0] += sm.grad[k] * dk;
             s[1] += fabs(dk) * lf;
@@ -567,27 +590,22 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
                 const double dv = sm.d[k + 1] - dk;
                 s[3] += dv * dv * sm.rdt[k];
             }
-            tl = fmin(tl, dk < 0.0 ? yk / (-dk) : CUDART_INF);
+            if (dk < 0.0) ntl = fmax(ntl, -(yk / (-dk)));
         }
-#pragma unroll
-        for (int o = 16; o; o >>= 1) {
-#pragma unroll
-            for (int m = 0; m < 4; ++m) s[m] += __shfl_xor_sync(kFull, s[m], o);
-            tl = fmin(tl, __shfl_xor_sync(kFull, tl, o));
-        }
+        ctl_reduce<4>(s, ntl, cred, tog, nw, CT);
         phi1 = s[0];
         qb = s[1];
         yb = s[2];
         Gd = s[3];
-        tmax = tl;
+        tmax = -ntl;
     };
     // slope along d (steepest descent if d does not descend) and the coefficients / scale of the
     // direction pass.  Returns false (stop set) if no descent is possible.
     auto prepare_direction = [&]() {
         direction_sums();
         if (!(phi1 < 0.0)) {
-            for (int k = lane; k < N; k += 32) sm.d[k] = -sm.pg[k];
-            __syncwarp();
+            for (int k = tid; k < N; k += CT) sm.d[k] = -sm.pg[k];
+            ctl_sync(CT);
             direction_sums();
             if (!(phi1 < 0.0)) {
                 stop = 2;
@@ -595,8 +613,8 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
             }
         }
         const FxScale sC = fx_scale_for(1.01 * Spd * ab * qb * qb, bad);
-        for (int i = lane; i < K; i += 32) sm.coef[i] = (float)sm.d[sm.sk[i]];
-        if (lane == 0) {
+        for (int i = tid; i < K; i += CT) sm.coef[i] = (float)sm.d[sm.sk[i]];
+        if (tid == 0) {
             sm.ctl->scC = sC.scale;
             sm.ctl->iC = sC.inv;
         }
@@ -604,24 +622,26 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     };
     // trial point y + t d (clamped), G and dG there
     auto prepare_trial = [&]() {
-#pragma unroll 2
-        for (int k = lane; k < N; k += 32) {
+        for (int k = tid; k < N; k += CT) {
             const double yk = sm.y[k], dk = sm.d[k];
             double v = yk + t * dk;
             if (v < 0.0 || (hit && dk < 0.0 && yk / (-dk) <= tmax)) v = 0.0;
             sm.yn[k] = v;
         }
-        __syncwarp();
-        Gn = smooth_G(sm.yn, sm, N, lane, true);
-        if (lane == 0) sm.ctl->tf = (float)t;
+        ctl_sync(CT);
+        double sg[1] = {smooth_part(sm.yn, sm, N, CT, true)}, mx = 0.0;
+        ctl_reduce<1>(sg, mx, cred, tog, nw, CT);
+        Gn = sg[0];
+        if (tid == 0) sm.ctl->tf = (float)t;
     };
 
     // objective and gradient at the incoming y
-    if (warp == 0) {
-        double s = 0.0;
-        for (int k = lane; k < N; k += 32) s += fabs(sm.y[k]) * sm.linf[k];
-        set_eval_scales(wsum(s));
-        Gs = smooth_G(sm.y, sm, N, lane, true);
+    if (ctl) {
+        double s[2] = {0.0, smooth_part(sm.y, sm, N, CT, true)}, mx = 0.0;
+        for (int k = tid; k < N; k += CT) s[0] += fabs(sm.y[k]) * sm.linf[k];
+        ctl_reduce<2>(s, mx, cred, tog, nw, CT);
+        set_eval_scales(s[0]);
+        Gs = s[1];
     }
     __syncthreads();
     long long *rec = begin_pass();
@@ -629,10 +649,10 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     grid.sync();
     ++ph;
     fetch_record(rec);
-    if (warp == 0) {
+    if (ctl) {
         const double iG = sm.ctl->iG;
         double pgl = 0.0;
-        for (int k = lane; k < N; k += 32) {
+        for (int k = tid; k < N; k += CT) {
             const int i = sm.ik[k];
             const double gk = i >= 0 ? (double)sm.recv[2 + i] * iG + a.gamma * sm.dG[k] : 0.0;
             const double p = (i < 0 || (sm.y[k] <= 0.0 && gk >= 0.0)) ? 0.0 : gk;
@@ -641,10 +661,11 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
             sm.d[k] = -p;
             pgl = fmax(pgl, fabs(p));
         }
-        __syncwarp();
+        double s0[1] = {0.0};
+        ctl_reduce<1>(s0, pgl, cred, tog, nw, CT);   // its barrier also publishes grad, pg, d to the group
         F = (double)sm.recv[0] * sm.ctl->iF + a.F_out;
         Phi = F + a.gamma * Gs;
-        pgmax = wmax(pgl);
+        pgmax = pgl;
         pg_entry = pgmax;
         tol = a.eps * fmax(1.0, pgmax);
         int state = kRunDirection;
@@ -653,7 +674,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
             stop = 1;
             state = kFinish;
         } else if (!prepare_direction()) state = kFinish;
-        if (lane == 0) {
+        if (tid == 0) {
             sm.ctl->state = state;
             sm.ctl->accepted = 0;
         }
@@ -688,7 +709,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
         grid.sync();
         PROF(1)
         ++ph;
-        if (warp == 0) {
+        if (ctl) {
             const double curvF = (double)__ldcg(rec + 1) * sm.ctl->iC;
             const double phi2 = 2.0 * curvF + 2.0 * a.gamma * Gd;
             t = phi2 > 0.0 ? -phi1 / phi2 : (isfinite(tmax) ? tmax : 1.0);
@@ -700,7 +721,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
             half = 0;
             set_eval_scales(yb + t * qb);   // |z + t q| <= sum_k (|y_k| + t |d_k|) max|d_k|; t only shrinks below
             prepare_trial();
-            if (lane == 0) sm.ctl->state = bad ? kFinish : kRunTrial;
+            if (tid == 0) sm.ctl->state = bad ? kFinish : kRunTrial;
         }
         __syncthreads();
         PROF(2)
@@ -713,33 +734,26 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
             PROF(4)
             ++ph;
             fetch_record(rec);
-            if (warp == 0) {
+            if (ctl) {
                 // gn = Dc w + gamma dG at the trial point, and the sums of the acceptance test and of the
                 // Polak-Ribiere+ update, in one sweep and one batched reduction
                 const double iG = sm.ctl->iG;
                 const double Fn = (double)sm.recv[0] * sm.ctl->iF + a.F_out;
-                double s[3] = {0.0, 0.0, 0.0}, pgm = 0.0;
-                int changed = hit;
-#pragma unroll 2
-                for (int k = lane; k < N; k += 32) {
+                double s[4] = {0.0, 0.0, 0.0, 0.0}, pgm = 0.0;
+                for (int k = tid; k < N; k += CT) {
                     const int i = sm.ik[k];
                     const double gk = i >= 0 ? (double)sm.recv[2 + i] * iG + a.gamma * sm.dG[k] : 0.0;
                     const double yk = sm.yn[k], po = sm.pg[k];
                     const double pn = (i < 0 || (yk <= 0.0 && gk >= 0.0)) ? 0.0 : gk;
                     sm.gn[k] = gk;
-                    changed |= (pn == 0.0) != (po == 0.0);
+                    s[3] += ((pn == 0.0) != (po == 0.0)) ? 1.0 : 0.0;   // entries entering / leaving the face
                     s[0] += pn * (pn - po);
                     s[1] += po * po;
                     s[2] += gk * sm.d[k];
                     pgm = fmax(pgm, fabs(pn));
                 }
-#pragma unroll
-                for (int o = 16; o; o >>= 1) {
-#pragma unroll
-                    for (int m = 0; m < 3; ++m) s[m] += __shfl_xor_sync(kFull, s[m], o);
-                    pgm = fmax(pgm, __shfl_xor_sync(kFull, pgm, o));
-                }
-                changed = __any_sync(kFull, changed);
+                ctl_reduce<4>(s, pgm, cred, tog, nw, CT);
+                const bool changed = hit || s[3] > 0.0;
                 PROFW(5, 8)
                 const double Phin = Fn + a.gamma * Gn;
                 // sufficient decrease; below the resolution of Phi accept on the slope instead
@@ -754,8 +768,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
                     Phi = Phin;
                     pgmax = pgm;
                     const double bpr = (changed || !(s[1] > 0.0) || s[0] <= 0.0) ? 0.0 : s[0] / s[1];
-#pragma unroll 2
-                    for (int k = lane; k < N; k += 32) {
+                    for (int k = tid; k < N; k += CT) {
                         const double yk = sm.yn[k], gk = sm.gn[k];
                         const bool off = sm.ik[k] < 0;
                         const double pn = (off || (yk <= 0.0 && gk >= 0.0)) ? 0.0 : gk;
@@ -766,7 +779,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
                         sm.pg[k] = pn;
                         sm.d[k] = dk;
                     }
-                    __syncwarp();
+                    ctl_sync(CT);
                     PROFW(5, 9)
                     ++inner;
                     state = kRunDirection;
@@ -789,7 +802,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
                     } else prepare_trial();
                 }
                 PROFW(5, 10)
-                if (lane == 0) {
+                if (tid == 0) {
                     sm.ctl->state = state;
                     sm.ctl->accepted = accepted ? 1 : 0;
                 }
@@ -807,17 +820,18 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
 
     // z, w and the cost from the final y (no drift from the z += t q updates)
     __syncthreads();
-    if (warp == 0) {
+    if (ctl) {
         if (bad) stop = 5;
         const int redo = (inner > 0 || zcur != a.z) && !bad;
         if (redo) {
-            double s = 0.0;
-            for (int k = lane; k < N; k += 32) s += fabs(sm.y[k]) * sm.linf[k];
-            set_eval_scales(wsum(s));
-            Gs = smooth_G(sm.y, sm, N, lane, true);
-            for (int i = lane; i < K; i += 32) sm.coef[i] = (float)sm.y[sm.sk[i]];
+            double s[2] = {0.0, smooth_part(sm.y, sm, N, CT, true)}, mx = 0.0;
+            for (int k = tid; k < N; k += CT) s[0] += fabs(sm.y[k]) * sm.linf[k];
+            ctl_reduce<2>(s, mx, cred, tog, nw, CT);
+            set_eval_scales(s[0]);
+            Gs = s[1];
+            for (int i = tid; i < K; i += CT) sm.coef[i] = (float)sm.y[sm.sk[i]];
         }
-        if (lane == 0) sm.ctl->accepted = redo;
+        if (tid == 0) sm.ctl->accepted = redo;
     }
     __syncthreads();
     if (sm.ctl->accepted) {
@@ -825,7 +839,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
         eval_pass<true>(a, sm, K, ngroups, nullptr, a.z, 0.f, rec, sm.ctl->scF, sm.ctl->scG, red);
         grid.sync();
         ++ph;
-        if (warp == 0) {
+        if (ctl) {
             F = (double)__ldcg(rec) * sm.ctl->iF + a.F_out;
             Phi = F + a.gamma * Gs;
         }
@@ -860,7 +874,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
 
 size_t master_smem_bytes(int64_t N) {
     return (size_t)(kMasterWarps * kGroup * kChunk + kGroup * kChunk) * 4   // part, wbuf
-           + (size_t)(11 * N + 2 + kMasterWarps) * 8 + sizeof(Ctl)           // K-vectors, recv, red, ctl
+           + (size_t)(11 * N + 2 + kMasterWarps + 2 * kMasterWarps * kRedSlots) * 8 + sizeof(Ctl)   // K-vectors, recv, red, cred, ctl
            + (size_t)N * 4 * 5;                                              // coef, sk, lo, hi, ik
 }
 
