@@ -88,6 +88,7 @@ struct vmat_plan {
     float Tmax = 0.f, abmax = 0.f;
     int master_grid = 0;
     size_t master_smem = 0;
+    int master_rslots = 0;             // slots per master block kept resident in shared memory (0: none)
     vmat::MasterOut *mout = nullptr;
     double *cost3 = nullptr;       // device {F, G, F+gamma G}
     double *part_dose = nullptr;   // partial F sums of the direct dose pass

@@ -187,6 +187,7 @@ struct MasterArgs {
     int stall_count;
     float Tmax, abmax;
     int max_inner;
+    int rslots;                 // > 0: every block keeps z, q, T, alpha, beta of its own slots in shared memory
     long long *accbuf;          // 3 rotating records of (N + 2) fixed-point sums: F, curvature, grad[0..K)
     unsigned int *phase;        // rotation counter, persists from launch to launch
     MasterOut *out;
@@ -260,7 +261,20 @@ __device__ long long g_master_prof[16];
 #define PROF_END                                                                  \
     if (blockIdx.x == 0 && threadIdx.x == 0)                                      \
         for (int i_ = 0; i_ < 16; ++i_) g_master_prof[i_] += pacc_[i_];
+#define PROFX(j)                          \
+    {                                     \
+        const long long n_ = clock64();   \
+        pacc_[j] += n_ - px_;             \
+        px_ = n_;                         \
+    }
+#define PROFX_START long long px_ = clock64();
+#define PROF_PARAM , long long &pt_, long long (&pacc_)[16]
+#define PROF_ARG , pt_, pacc_
 #else
+#define PROF_PARAM
+#define PROF_ARG
+#define PROFX(j)
+#define PROFX_START
 #define PROF_DECL
 #define PROF(i)
 #define PROFW(i, j)
@@ -282,6 +296,7 @@ constexpr int kRedSlots = 6;   // values per warp row of the control group's red
 struct Smem {
     double *y, *d, *grad, *pg, *yn, *gn, *dG, *rdt, *gacc, *linf;   // N each (control warp; gacc: all warps)
     float *part, *wbuf, *coef;
+    float *rz0, *rz1, *rq, *rT, *ral, *rbe;   // resident copies of the block's own slots (a.rslots each), or unused
     int *sk, *lo, *hi, *ik;
     long long *recv;   // the pass's record of grid sums, fetched by the whole block after the barrier
     Ctl *ctl;
@@ -294,12 +309,13 @@ __device__ __forceinline__ int chunk_of(int g, int ch) { return (int)blockIdx.x 
 // The beam loop is split over the warps; partials meet in shared memory and are added in warp order.
 // The caller must __syncthreads() before sm.part is written again.
 __device__ __forceinline__ void combine_group(const MasterArgs &a, const Smem &sm, int K, int g,
-                                              float (&out)[kOutPerThread]) {
+                                              float (&out)[kOutPerThread] PROF_PARAM) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const float4 *Dd4 = reinterpret_cast<const float4 *>(a.Dd) + lane;
     const size_t stride4 = (size_t)a.Sp / 4;
     const int cb = chunk_of(g, 0), G = (int)gridDim.x;
     float4 acc[kGroup];
+    PROFX_START
 #pragma unroll
     for (int ch = 0; ch < kGroup; ++ch) acc[ch] = make_float4(0.f, 0.f, 0.f, 0.f);
     for (int i = warp; i < K; i += kMasterWarps) {
@@ -319,6 +335,7 @@ __device__ __forceinline__ void combine_group(const MasterArgs &a, const Smem &s
             }
         }
     }
+    PROFX(12)
 #pragma unroll
     for (int ch = 0; ch < kGroup; ++ch) reinterpret_cast<float4 *>(sm.part)[(warp * kGroup + ch) * 32 + lane] = acc[ch];
     __syncthreads();
@@ -330,6 +347,7 @@ __device__ __forceinline__ void combine_group(const MasterArgs &a, const Smem &s
         for (int wv = 0; wv < kMasterWarps; ++wv) v += sm.part[(wv * kGroup + ch) * kChunk + s];
         out[r] = v;
     }
+    PROFX(13)
 }
 
 __device__ __forceinline__ void penalty(float z, float T, float al, float be, float &w, double &F) {
@@ -365,8 +383,10 @@ __device__ __forceinline__ double group_dot(const MasterArgs &a, const Smem &sm,
 // in fixed point (scales scF, scG).
 template <bool FROM_Y>
 __device__ __forceinline__ void eval_pass(const MasterArgs &a, const Smem &sm, int K, int ngroups, const float *zsrc,
-                                          float *zdst, float tf, long long *rec, double scF, double scG,
-                                          double *red) {
+                                          float *zdst, const float *rzsrc, float *rzdst, float tf, long long *rec,
+                                          double scF, double scG, double *red PROF_PARAM) {
+    const bool res = a.rslots > 0;
+    PROFX_START
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const float4 *Dd4 = reinterpret_cast<const float4 *>(a.Dd) + lane;
     const size_t stride4 = (size_t)a.Sp / 4;
@@ -374,25 +394,36 @@ __device__ __forceinline__ void eval_pass(const MasterArgs &a, const Smem &sm, i
     for (int i = tid; i < K; i += kMasterThreads) sm.gacc[i] = 0.0;
     double F = 0.0;
     __syncthreads();
+    PROFX(8)
     for (int g = 0; g < ngroups; ++g) {
         float zv[kOutPerThread];
-        if (FROM_Y) combine_group(a, sm, K, g, zv);
+        if (FROM_Y) combine_group(a, sm, K, g, zv PROF_ARG);
 #pragma unroll
         for (int r = 0; r < kOutPerThread; ++r) {
             const int o = tid + r * kMasterThreads, c = chunk_of(g, o >> 7);
             float wv = 0.f;
             if (c < a.nchunks) {
                 const size_t s = (size_t)c * kChunk + (o & (kChunk - 1));
-                const float z = FROM_Y ? zv[r] : fmaf(tf, a.q[s], zsrc[s]);
+                const int ls = g * (kGroup * kChunk) + o;          // the slot's place in the resident arrays
+                float z, Tv, al, be;
+                if (res) {
+                    z = FROM_Y ? zv[r] : fmaf(tf, sm.rq[ls], rzsrc[ls]);
+                    Tv = sm.rT[ls], al = sm.ral[ls], be = sm.rbe[ls];
+                    rzdst[ls] = z;
+                } else {
+                    z = FROM_Y ? zv[r] : fmaf(tf, a.q[s], zsrc[s]);
+                    Tv = a.T[s], al = a.alpha[s], be = a.beta[s];
+                }
                 double f;
-                penalty(z, a.T[s], a.alpha[s], a.beta[s], wv, f);
+                penalty(z, Tv, al, be, wv, f);
                 F += f;
-                zdst[s] = z;
+                if (FROM_Y || !res) zdst[s] = z;   // evaluations from y publish z and w
                 if (FROM_Y) a.w[s] = wv;
             }
             sm.wbuf[o] = wv;
         }
         __syncthreads();
+        PROFX(9)
         const int cb = chunk_of(g, 0);
         // two rows per step: 2*kGroup independent loads in flight, two interleaved shuffle chains
         for (int i = warp; i < K; i += 2 * kMasterWarps) {
@@ -409,11 +440,14 @@ __device__ __forceinline__ void eval_pass(const MasterArgs &a, const Smem &sm, i
                 if (i2 < K) sm.gacc[i2] += d2;
             }
         }
+        PROFX(10)
         __syncthreads();
     }
+    PROFX(11)
     F = block_sum(F, red);
     if (tid == 0) fx_add(rec, F, scF);
     for (int i = tid; i < K; i += kMasterThreads) fx_add(rec + 2 + i, sm.gacc[i], scG);
+    PROFX(11)
 }
 
 // ---- control group: the first nw warps of a block (CT = 32 nw threads) share the N-vector work -----
@@ -472,7 +506,13 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     Smem sm;
     sm.part = reinterpret_cast<float *>(smem_raw);
     sm.wbuf = sm.part + kMasterWarps * kGroup * kChunk;
-    sm.y = reinterpret_cast<double *>(sm.wbuf + kGroup * kChunk);
+    sm.rz0 = sm.wbuf + kGroup * kChunk;
+    sm.rz1 = sm.rz0 + a.rslots;
+    sm.rq = sm.rz1 + a.rslots;
+    sm.rT = sm.rq + a.rslots;
+    sm.ral = sm.rT + a.rslots;
+    sm.rbe = sm.ral + a.rslots;
+    sm.y = reinterpret_cast<double *>(sm.rbe + a.rslots);
     sm.d = sm.y + N;
     sm.grad = sm.d + N;
     sm.pg = sm.grad + N;
@@ -539,6 +579,19 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     const int recn = N + 2;
     unsigned ph = *a.phase;   // written by the previous launch, stream ordered
     float *zcur = a.z, *znext = a.zn;
+    // resident slot data: T, alpha, beta of the block's own slots are read once, z and q never leave the SM
+    const bool res = a.rslots > 0;
+    float *rzcur = sm.rz0, *rznext = sm.rz1;
+    if (res) {
+        for (int ls = tid; ls < a.rslots; ls += kMasterThreads) {
+            const int c = (int)blockIdx.x + (ls >> 7) * (int)gridDim.x;
+            const bool in = c < a.nchunks;
+            const size_t s = (size_t)c * kChunk + (ls & (kChunk - 1));
+            sm.rT[ls] = in ? a.T[s] : 0.f;
+            sm.ral[ls] = in ? a.alpha[s] : 0.f;
+            sm.rbe[ls] = in ? a.beta[s] : 0.f;
+        }
+    }
 
     // start a pass: the record that collects its sums; block 0 clears the record of the next pass
     auto begin_pass = [&]() -> long long * {
@@ -635,6 +688,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
         if (tid == 0) sm.ctl->tf = (float)t;
     };
 
+    PROF_DECL;
     // objective and gradient at the incoming y
     if (ctl) {
         double s[2] = {0.0, smooth_part(sm.y, sm, N, CT, true)}, mx = 0.0;
@@ -645,7 +699,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     }
     __syncthreads();
     long long *rec = begin_pass();
-    eval_pass<true>(a, sm, K, ngroups, nullptr, zcur, 0.f, rec, sm.ctl->scF, sm.ctl->scG, red);
+    eval_pass<true>(a, sm, K, ngroups, nullptr, zcur, nullptr, rzcur, 0.f, rec, sm.ctl->scF, sm.ctl->scG, red PROF_ARG);
     grid.sync();
     ++ph;
     fetch_record(rec);
@@ -681,30 +735,39 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     }
     __syncthreads();
 
-    PROF_DECL;
     while (sm.ctl->state != kFinish) {
         PROF(7)
         // ---- q = Dc^T d and the curvature of the quadratic piece at t = 0 ------------------------------
         rec = begin_pass();
+        PROFX_START
         double curv = 0.0;
         for (int g = 0; g < ngroups; ++g) {
             float qv[kOutPerThread];
-            combine_group(a, sm, K, g, qv);
+            combine_group(a, sm, K, g, qv PROF_ARG);
 #pragma unroll
             for (int r = 0; r < kOutPerThread; ++r) {
                 const int o = tid + r * kMasterThreads, c = chunk_of(g, o >> 7);
                 if (c < a.nchunks) {
                     const size_t sl = (size_t)c * kChunk + (o & (kChunk - 1));
-                    const float zv = zcur[sl], Tv = a.T[sl];
-                    const float om = zv < Tv ? a.alpha[sl] : (zv > Tv ? a.beta[sl] : 0.f);
+                    const int ls = g * (kGroup * kChunk) + o;
+                    float zv, Tv, al, be;
+                    if (res) {
+                        zv = rzcur[ls], Tv = sm.rT[ls], al = sm.ral[ls], be = sm.rbe[ls];
+                        sm.rq[ls] = qv[r];
+                    } else {
+                        zv = zcur[sl], Tv = a.T[sl], al = a.alpha[sl], be = a.beta[sl];
+                        a.q[sl] = qv[r];
+                    }
+                    const float om = zv < Tv ? al : (zv > Tv ? be : 0.f);
                     curv += (double)om * (double)qv[r] * (double)qv[r];
-                    a.q[sl] = qv[r];
                 }
             }
             __syncthreads();
         }
+        PROFX(14)
         curv = block_sum(curv, red);
         if (tid == 0) fx_add(rec + 1, curv, sm.ctl->scC);
+        PROFX(15)
         PROF(0)
         grid.sync();
         PROF(1)
@@ -728,7 +791,8 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
         // ---- backtracking on the true cost ----------------------------------------------------------------
         while (sm.ctl->state == kRunTrial) {
             rec = begin_pass();
-            eval_pass<false>(a, sm, K, ngroups, zcur, znext, sm.ctl->tf, rec, sm.ctl->scF, sm.ctl->scG, red);
+            eval_pass<false>(a, sm, K, ngroups, zcur, znext, rzcur, rznext, sm.ctl->tf, rec, sm.ctl->scF,
+                             sm.ctl->scG, red PROF_ARG);
             PROF(3)
             grid.sync();
             PROF(4)
@@ -754,8 +818,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
                 }
                 ctl_reduce<4>(s, pgm, cred, tog, nw, CT);
                 const bool changed = hit || s[3] > 0.0;
-                PROFW(5, 8)
-                const double Phin = Fn + a.gamma * Gn;
+                                const double Phin = Fn + a.gamma * Gn;
                 // sufficient decrease; below the resolution of Phi accept on the slope instead
                 const bool accepted = Phin <= Phi + c1a * t * phi1 ||
                                       (Phin <= Phi + noise * fabs(Phi) && fabs(s[2]) <= 0.9 * fabs(phi1));
@@ -780,8 +843,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
                         sm.d[k] = dk;
                     }
                     ctl_sync(CT);
-                    PROFW(5, 9)
-                    ++inner;
+                                        ++inner;
                     state = kRunDirection;
                     if (!(pgmax > tol)) state = kFinish;
                     else if (stall >= a.stall_count) {
@@ -801,8 +863,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
                         state = kFinish;
                     } else prepare_trial();
                 }
-                PROFW(5, 10)
-                if (tid == 0) {
+                                if (tid == 0) {
                     sm.ctl->state = state;
                     sm.ctl->accepted = accepted ? 1 : 0;
                 }
@@ -813,6 +874,9 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
                 float *tmpz = zcur;
                 zcur = znext;
                 znext = tmpz;
+                tmpz = rzcur;
+                rzcur = rznext;
+                rznext = tmpz;
             }
         }
     }
@@ -836,7 +900,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     __syncthreads();
     if (sm.ctl->accepted) {
         rec = begin_pass();
-        eval_pass<true>(a, sm, K, ngroups, nullptr, a.z, 0.f, rec, sm.ctl->scF, sm.ctl->scG, red);
+        eval_pass<true>(a, sm, K, ngroups, nullptr, a.z, nullptr, rzcur, 0.f, rec, sm.ctl->scF, sm.ctl->scG, red PROF_ARG);
         grid.sync();
         ++ph;
         if (ctl) {
@@ -872,8 +936,8 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     }
 }
 
-size_t master_smem_bytes(int64_t N) {
-    return (size_t)(kMasterWarps * kGroup * kChunk + kGroup * kChunk) * 4   // part, wbuf
+size_t master_smem_bytes(int64_t N, int64_t rslots) {
+    return (size_t)(kMasterWarps * kGroup * kChunk + kGroup * kChunk + 6 * rslots) * 4   // part, wbuf, resident slots
            + (size_t)(11 * N + 2 + kMasterWarps + 2 * kMasterWarps * kRedSlots) * 8 + sizeof(Ctl)   // K-vectors, recv, red, cred, ctl
            + (size_t)N * 4 * 5;                                              // coef, sk, lo, hi, ik
 }
@@ -881,17 +945,26 @@ size_t master_smem_bytes(int64_t N) {
 }  // namespace
 
 int master_configure(vmat_plan *p) {
-    p->master_smem = master_smem_bytes(p->N);
-    if (p->master_smem > 220 * 1024) return fail(p, VMAT_EINVAL, "n_beams too large for the master kernel's shared memory");
-    VMAT_CUDA(p, cudaFuncSetAttribute(k_master, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->master_smem));
-    int per_sm = 0;
-    VMAT_CUDA(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_master, kMasterThreads, p->master_smem));
-    if (per_sm < 1) return fail(p, VMAT_ECUDA, "master kernel does not fit on an SM");
     const int64_t nchunks = p->Sp / kChunk;
     int64_t grid = p->sm_count;                       // one block per SM, chunks dealt round-robin
     if (grid > nchunks) grid = nchunks;
     if (grid < 1) grid = 1;
     p->master_grid = (int)grid;
+    // resident slot data (z, z trial, q, T, alpha, beta of a block's own slots) if it fits in 96 KB
+    const int64_t ngroups = (nchunks + grid * kGroup - 1) / (grid * kGroup);
+    int64_t rslots = ngroups * kGroup * kChunk;
+    if (rslots * 6 * 4 > 96 * 1024) rslots = 0;
+    p->master_rslots = (int)rslots;
+    p->master_smem = master_smem_bytes(p->N, rslots);
+    if (p->master_smem > 220 * 1024) {
+        p->master_rslots = 0;
+        p->master_smem = master_smem_bytes(p->N, 0);
+    }
+    if (p->master_smem > 220 * 1024) return fail(p, VMAT_EINVAL, "n_beams too large for the master kernel's shared memory");
+    VMAT_CUDA(p, cudaFuncSetAttribute(k_master, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->master_smem));
+    int per_sm = 0;
+    VMAT_CUDA(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_master, kMasterThreads, p->master_smem));
+    if (per_sm < 1) return fail(p, VMAT_ECUDA, "master kernel does not fit on an SM");
     int rc;
     if ((rc = dev_alloc(p, &p->accbuf, 3 * (p->N + 2)))) return rc;
     if ((rc = dev_alloc(p, &p->phase, 1))) return rc;
@@ -946,6 +1019,7 @@ static int launch_master_impl(vmat_plan *p, int max_inner, int trace_it) {
     a.stall_rel = p->opt.master_stall_rel;
     a.stall_count = p->opt.master_stall_count;
     a.max_inner = max_inner;
+    a.rslots = p->master_rslots;
     a.colstat = p->colstat;
     a.fx_inv = p->fx_inv;
     a.Tmax = p->Tmax;
