@@ -82,12 +82,13 @@ struct vmat_plan {
     unsigned int *ticket = nullptr;
 
     long long *accbuf = nullptr;       // 3 x (N + 2) fixed-point sums of the master kernel
-    unsigned int *phase = nullptr;     // rotation counter of accbuf
+    unsigned int *phase = nullptr;     // rotation counter of accbuf, barrier epoch
     vmat::ColStat *colstat = nullptr;  // N
     unsigned int *vbounds = nullptr;   // bit patterns of max|T|, max(alpha, beta)
     float Tmax = 0.f, abmax = 0.f;
     int master_grid = 0;
     size_t master_smem = 0;
+    int master_cache_segs = 0;         // 512-byte segments of Dd a master block stages in shared memory
     int master_rslots = 0;             // slots per master block kept resident in shared memory (0: none)
     vmat::MasterOut *mout = nullptr;
     double *cost3 = nullptr;       // device {F, G, F+gamma G}

@@ -24,6 +24,8 @@
 #include <math_constants.h>
 
 #include <climits>
+#include <cstdio>
+#include <cstdlib>
 
 #include "vmat_internal.cuh"
 
@@ -188,7 +190,9 @@ struct MasterArgs {
     float Tmax, abmax;
     int max_inner;
     int rslots;                 // > 0: every block keeps z, q, T, alpha, beta of its own slots in shared memory
-    long long *accbuf;          // 3 rotating records of (N + 2) fixed-point sums: F, curvature, grad[0..K)
+    int cache_segs;             // capacity of the shared-memory tile of Dd in 512-byte segments
+    long long *accbuf;          // 3 rotating sets of kSumGroups records of (N + 2) fixed-point sums: F, curvature,
+                                // grad[0..K); a block adds to the record of its group (blockIdx mod kSumGroups)
     unsigned int *phase;        // rotation counter, persists from launch to launch
     MasterOut *out;
     double *cost3;
@@ -292,12 +296,45 @@ struct Ctl {
 enum { kRunDirection = 0, kRunTrial = 1, kFinish = 2 };
 
 constexpr int kRedSlots = 6;   // values per warp row of the control group's reduction scratch
+// Records of grid-wide sums per rotation slot.  Measured: splitting the blocks into 16 groups with one record each
+// (to spread same-address atomics) and a hand-rolled two-level barrier were both slower than one record and the
+// cooperative-groups barrier (12.4 / 14.5 vs 11.7 us per inner iteration at K = 30), so there is one group.
+constexpr int kSumGroups = 1;
+constexpr int kKSplit = 8;     // beam-loop split of the passes; the two halves of the warps take alternate chunks
+constexpr int kNoCache = INT_MIN;
+static_assert(kMasterWarps == 2 * kKSplit, "the passes split the warps in two chunk halves");
+
+// 1-D bulk copies (TMA) global -> shared, completion counted in bytes on an mbarrier
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned bytes, uint64_t *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity) {
+    asm volatile(
+        "{\n.reg .pred p;\nWAIT_%=:\nmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n@p bra DONE_%=;\nbra "
+        "WAIT_%=;\nDONE_%=:\n}" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+
 
 struct Smem {
     double *y, *d, *grad, *pg, *yn, *gn, *dG, *rdt, *gacc, *linf;   // N each (control warp; gacc: all warps)
     float *part, *wbuf, *coef;
     float *rz0, *rz1, *rq, *rT, *ral, *rbe;   // resident copies of the block's own slots (a.rslots each), or unused
-    int *sk, *lo, *hi, *ik;
+    float *tile;       // staged 512-byte segments of the block's part of Dd
+    int *sk, *lo, *hi, *ik;   // lo, hi: block-local range of chunks (j of b + jG) column i touches
+    int *base;         // segment (i, j) lives at tile[(base[i] + j) * 128]; kNoCache if column i is not staged
     long long *recv;   // the pass's record of grid sums, fetched by the whole block after the barrier
     Ctl *ctl;
 };
@@ -305,46 +342,66 @@ struct Smem {
 // chunk handled by this block as member `ch` of its group `g`: chunks are dealt round-robin
 __device__ __forceinline__ int chunk_of(int g, int ch) { return (int)blockIdx.x + (g * kGroup + ch) * (int)gridDim.x; }
 
+// The four chunks (j = g*kGroup + chalf + 2h, h = 0..3) of column i that this warp's half of the group covers:
+// v[h] = the lane's float4 of segment h, zero where the column does not touch the chunk.  Staged columns are
+// read from the shared-memory tile, the others from L2 / HBM; either way the four loads are independent.
+__device__ __forceinline__ void load_half(const MasterArgs &a, const Smem &sm, int i, int g, int chalf, int lane,
+                                          float4 (&v)[kGroup / 2]) {
+    const int lb = max(sm.lo[i] - g * kGroup, 0), hb = min(sm.hi[i] - g * kGroup, kGroup - 1);
+    const unsigned m = hb >= lb ? (((2u << hb) - 1u) & ~((1u << lb) - 1u)) >> chalf : 0u;
+    const int bs = sm.base[i], j0 = g * kGroup + chalf;
+    if (bs != kNoCache) {
+        const float4 *t = reinterpret_cast<const float4 *>(sm.tile) + (bs + j0) * 32 + lane;
+#pragma unroll
+        for (int h = 0; h < kGroup / 2; ++h)
+            v[h] = (m >> (2 * h)) & 1u ? t[2 * h * 32] : make_float4(0.f, 0.f, 0.f, 0.f);
+    } else {
+        const int G = (int)gridDim.x;
+        const float4 *row = reinterpret_cast<const float4 *>(a.Dd + (size_t)sm.sk[i] * a.Sp) +
+                            (size_t)((int)blockIdx.x + j0 * G) * (kChunk / 4) + lane;
+#pragma unroll
+        for (int h = 0; h < kGroup / 2; ++h)
+            v[h] = (m >> (2 * h)) & 1u ? __ldg(row + (size_t)(2 * h * G) * (kChunk / 4)) : make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+}
+
 // value[o] = sum_i coef[i] * Dd[sk[i]][slot(o)] for the kGroup*128 slots of group g, o = tid + r*kMasterThreads.
-// The beam loop is split over the warps; partials meet in shared memory and are added in warp order.
-// The caller must __syncthreads() before sm.part is written again.
+// Warp w takes the beams i = (w mod kKSplit), +kKSplit, .. and every second chunk of the group (even chunks
+// for w < kKSplit, odd ones above), two beams per step so that eight loads are in flight; partials meet in
+// shared memory and are added in a fixed order.  The caller must __syncthreads() before sm.part is written again.
 __device__ __forceinline__ void combine_group(const MasterArgs &a, const Smem &sm, int K, int g,
                                               float (&out)[kOutPerThread] PROF_PARAM) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const float4 *Dd4 = reinterpret_cast<const float4 *>(a.Dd) + lane;
-    const size_t stride4 = (size_t)a.Sp / 4;
-    const int cb = chunk_of(g, 0), G = (int)gridDim.x;
-    float4 acc[kGroup];
+    const int kpart = warp & (kKSplit - 1), chalf = warp / kKSplit;
+    float4 acc[kGroup / 2];
     PROFX_START
 #pragma unroll
-    for (int ch = 0; ch < kGroup; ++ch) acc[ch] = make_float4(0.f, 0.f, 0.f, 0.f);
-    for (int i = warp; i < K; i += kMasterWarps) {
-        const float cf = sm.coef[i];
-        if (cf == 0.f) continue;
-        const int lo = sm.lo[i], hi = sm.hi[i];
-        const float4 *row = Dd4 + (size_t)sm.sk[i] * stride4;
+    for (int h = 0; h < kGroup / 2; ++h) acc[h] = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int i = kpart; i < K; i += 2 * kKSplit) {
+        const int i2 = i + kKSplit < K ? i + kKSplit : i;
+        const float c1 = sm.coef[i], c2 = i + kKSplit < K ? sm.coef[i2] : 0.f;
+        float4 v1[kGroup / 2], v2[kGroup / 2];
+        load_half(a, sm, i, g, chalf, lane, v1);
+        load_half(a, sm, i2, g, chalf, lane, v2);
 #pragma unroll
-        for (int ch = 0; ch < kGroup; ++ch) {
-            const int c = cb + ch * G;
-            if (c >= lo && c <= hi) {
-                const float4 v = __ldg(row + (size_t)c * (kChunk / 4));
-                acc[ch].x = fmaf(cf, v.x, acc[ch].x);
-                acc[ch].y = fmaf(cf, v.y, acc[ch].y);
-                acc[ch].z = fmaf(cf, v.z, acc[ch].z);
-                acc[ch].w = fmaf(cf, v.w, acc[ch].w);
-            }
+        for (int h = 0; h < kGroup / 2; ++h) {
+            acc[h].x = fmaf(c2, v2[h].x, fmaf(c1, v1[h].x, acc[h].x));
+            acc[h].y = fmaf(c2, v2[h].y, fmaf(c1, v1[h].y, acc[h].y));
+            acc[h].z = fmaf(c2, v2[h].z, fmaf(c1, v1[h].z, acc[h].z));
+            acc[h].w = fmaf(c2, v2[h].w, fmaf(c1, v1[h].w, acc[h].w));
         }
     }
     PROFX(12)
 #pragma unroll
-    for (int ch = 0; ch < kGroup; ++ch) reinterpret_cast<float4 *>(sm.part)[(warp * kGroup + ch) * 32 + lane] = acc[ch];
+    for (int h = 0; h < kGroup / 2; ++h)
+        reinterpret_cast<float4 *>(sm.part)[(kpart * kGroup + 2 * h + chalf) * 32 + lane] = acc[h];
     __syncthreads();
 #pragma unroll
     for (int r = 0; r < kOutPerThread; ++r) {
         const int o = tid + r * kMasterThreads, ch = o >> 7, s = o & (kChunk - 1);
         float v = 0.f;
 #pragma unroll
-        for (int wv = 0; wv < kMasterWarps; ++wv) v += sm.part[(wv * kGroup + ch) * kChunk + s];
+        for (int kp = 0; kp < kKSplit; ++kp) v += sm.part[(kp * kGroup + ch) * kChunk + s];
         out[r] = v;
     }
     PROFX(13)
@@ -354,26 +411,6 @@ __device__ __forceinline__ void penalty(float z, float T, float al, float be, fl
     const float under = fmaxf(0.f, T - z), over = fmaxf(0.f, z - T);
     w = -2.f * al * under + 2.f * be * over;                                       // Eq. 1, derivative
     F = (double)al * (double)under * (double)under + (double)be * (double)over * (double)over;
-}
-
-// dot of row i of the group (chunks cb, cb+G, ..) with the penalty gradient staged in sm.wbuf
-__device__ __forceinline__ double group_dot(const MasterArgs &a, const Smem &sm, const float4 *Dd4, size_t stride4,
-                                            int i, int cb, int G, int lane) {
-    const int lo = sm.lo[i], hi = sm.hi[i];
-    const float4 *row = Dd4 + (size_t)sm.sk[i] * stride4;
-    float4 v[kGroup];
-#pragma unroll
-    for (int ch = 0; ch < kGroup; ++ch) {
-        const int c = cb + ch * G;
-        v[ch] = (c >= lo && c <= hi) ? __ldg(row + (size_t)c * (kChunk / 4)) : make_float4(0.f, 0.f, 0.f, 0.f);
-    }
-    double dot = 0.0;
-#pragma unroll
-    for (int ch = 0; ch < kGroup; ++ch) {
-        const float4 w4 = reinterpret_cast<const float4 *>(sm.wbuf)[ch * 32 + lane];
-        dot += (double)(v[ch].x * w4.x + v[ch].y * w4.y + v[ch].z * w4.z + v[ch].w * w4.w);
-    }
-    return dot;
 }
 
 // One pass over the block's chunks that evaluates the objective at a new dose:
@@ -388,10 +425,8 @@ __device__ __forceinline__ void eval_pass(const MasterArgs &a, const Smem &sm, i
     const bool res = a.rslots > 0;
     PROFX_START
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const float4 *Dd4 = reinterpret_cast<const float4 *>(a.Dd) + lane;
-    const size_t stride4 = (size_t)a.Sp / 4;
-    const int G = (int)gridDim.x;
-    for (int i = tid; i < K; i += kMasterThreads) sm.gacc[i] = 0.0;
+    const int kpart = warp & (kKSplit - 1), chalf = warp / kKSplit;
+    for (int i = tid; i < 2 * a.N; i += kMasterThreads) sm.gacc[i] = 0.0;
     double F = 0.0;
     __syncthreads();
     PROFX(8)
@@ -424,21 +459,41 @@ __device__ __forceinline__ void eval_pass(const MasterArgs &a, const Smem &sm, i
         }
         __syncthreads();
         PROFX(9)
-        const int cb = chunk_of(g, 0);
-        // two rows per step: 2*kGroup independent loads in flight, two interleaved shuffle chains
-        for (int i = warp; i < K; i += 2 * kMasterWarps) {
-            const int i2 = i + kMasterWarps;
-            double d1 = group_dot(a, sm, Dd4, stride4, i, cb, G, lane);
-            double d2 = i2 < K ? group_dot(a, sm, Dd4, stride4, i2, cb, G, lane) : 0.0;
+        // this warp's half of the group's gradient (4 chunks), and its beams i = kpart, +kKSplit, ..: two beams
+        // per step (eight independent loads), lane partials in fp32 (16 products), the warp sum in fp64; the
+        // partial dot goes to the row of sm.gacc that belongs to this chunk half
+        float4 w4[kGroup / 2];
 #pragma unroll
-            for (int o = 16; o; o >>= 1) {
-                d1 += __shfl_xor_sync(kFull, d1, o);
-                d2 += __shfl_xor_sync(kFull, d2, o);
+        for (int h = 0; h < kGroup / 2; ++h) w4[h] = reinterpret_cast<const float4 *>(sm.wbuf)[(2 * h + chalf) * 32 + lane];
+        for (int i = kpart; i < K; i += 2 * kKSplit) {
+            const bool has2 = i + kKSplit < K;
+            const int i2 = has2 ? i + kKSplit : i;
+            float4 v1[kGroup / 2], v2[kGroup / 2];
+            load_half(a, sm, i, g, chalf, lane, v1);
+            load_half(a, sm, i2, g, chalf, lane, v2);
+            float4 s1 = make_float4(0.f, 0.f, 0.f, 0.f), s2 = s1;
+#pragma unroll
+            for (int h = 0; h < kGroup / 2; ++h) {
+                s1.x = fmaf(v1[h].x, w4[h].x, s1.x);
+                s1.y = fmaf(v1[h].y, w4[h].y, s1.y);
+                s1.z = fmaf(v1[h].z, w4[h].z, s1.z);
+                s1.w = fmaf(v1[h].w, w4[h].w, s1.w);
+                s2.x = fmaf(v2[h].x, w4[h].x, s2.x);
+                s2.y = fmaf(v2[h].y, w4[h].y, s2.y);
+                s2.z = fmaf(v2[h].z, w4[h].z, s2.z);
+                s2.w = fmaf(v2[h].w, w4[h].w, s2.w);
             }
-            if (lane == 0) {   // indices i, i2 are owned by this warp
-                sm.gacc[i] += d1;
-                if (i2 < K) sm.gacc[i2] += d2;
-            }
+            double d1 = (double)((s1.x + s1.y) + (s1.z + s1.w)), d2 = (double)((s2.x + s2.y) + (s2.z + s2.w));
+            // one butterfly for both rows: after the first exchange the lower half-warp carries row 1, the upper row 2
+            const bool up = lane & 16;
+            double r = (up ? d2 : d1) + __shfl_xor_sync(kFull, up ? d1 : d2, 16);
+            r += __shfl_xor_sync(kFull, r, 8);
+            r += __shfl_xor_sync(kFull, r, 4);
+            r += __shfl_xor_sync(kFull, r, 2);
+            r += __shfl_xor_sync(kFull, r, 1);
+            double *gacc = sm.gacc + chalf * a.N;      // entries i, i2 of this row are owned by this warp
+            if (lane == 0) gacc[i] += r;
+            if (lane == 16 && has2) gacc[i2] += r;
         }
         PROFX(10)
         __syncthreads();
@@ -446,7 +501,7 @@ __device__ __forceinline__ void eval_pass(const MasterArgs &a, const Smem &sm, i
     PROFX(11)
     F = block_sum(F, red);
     if (tid == 0) fx_add(rec, F, scF);
-    for (int i = tid; i < K; i += kMasterThreads) fx_add(rec + 2 + i, sm.gacc[i], scG);
+    for (int i = tid; i < K; i += kMasterThreads) fx_add(rec + 2 + i, sm.gacc[i] + sm.gacc[a.N + i], scG);
     PROFX(11)
 }
 
@@ -500,13 +555,13 @@ __device__ __forceinline__ double smooth_part(const double *v, const Smem &sm, i
 }
 
 __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a) {
-    cg::grid_group grid = cg::this_grid();
     extern __shared__ float4 smem_raw[];   // 16-byte aligned: float4 tiles first, then doubles, floats, ints
     const int N = a.N, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     Smem sm;
     sm.part = reinterpret_cast<float *>(smem_raw);
-    sm.wbuf = sm.part + kMasterWarps * kGroup * kChunk;
-    sm.rz0 = sm.wbuf + kGroup * kChunk;
+    sm.wbuf = sm.part + kKSplit * kGroup * kChunk;
+    sm.tile = sm.wbuf + kGroup * kChunk;
+    sm.rz0 = sm.tile + (size_t)a.cache_segs * kChunk;
     sm.rz1 = sm.rz0 + a.rslots;
     sm.rq = sm.rz1 + a.rslots;
     sm.rT = sm.rq + a.rslots;
@@ -521,7 +576,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     sm.dG = sm.gn + N;
     sm.rdt = sm.dG + N;
     sm.gacc = sm.rdt + N;
-    sm.linf = sm.gacc + N;
+    sm.linf = sm.gacc + 2 * N;   // gacc: one row per chunk half
     double *red = sm.linf + N;
     double *cred = red + kMasterWarps;   // 2 x kMasterWarps x kRedSlots
     sm.recv = reinterpret_cast<long long *>(cred + 2 * kMasterWarps * kRedSlots);
@@ -531,7 +586,9 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     sm.lo = sm.sk + N;
     sm.hi = sm.lo + N;
     sm.ik = sm.hi + N;
+    sm.base = sm.ik + N;
     __shared__ int sK;
+    __shared__ uint64_t tile_bar;
 
     // occupied beams in ascending order
     if (tid < 32) {
@@ -563,8 +620,10 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
         double lf = 0.0;
         if (i >= 0) {
             const ColStat cs = a.colstat[k];
-            sm.lo[i] = cs.clo;
-            sm.hi[i] = cs.chi;
+            // the block's chunks are b + jG: column k touches those with lo <= j <= hi (empty: hi < lo)
+            const int b = (int)blockIdx.x, Gd_ = (int)gridDim.x;
+            sm.lo[i] = cs.clo > b ? (cs.clo - b + Gd_ - 1) / Gd_ : 0;
+            sm.hi[i] = cs.chi >= b ? (cs.chi - b) / Gd_ : -1;
             lf = (double)cs.linf * a.fx_inv * 1.000001;
             l1l = fmax(l1l, (double)cs.l1 * a.fx_inv * 1.000001);
             sm.coef[i] = (float)sm.y[k];
@@ -572,12 +631,57 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
         sm.linf[k] = lf;
     }
     const double l1max = block_max(l1l, red);
+
+    // ---- stage the block's part of Dd in shared memory (TMA bulk copies, one per 512-byte segment) ----
+    // The block's chunks are b + jG; column i touches those with j0_i <= j <= j1_i.  Segments are
+    // packed column after column until the tile is full; the rest stays in L2 / HBM.
+    {
+        const int G = (int)gridDim.x, b = (int)blockIdx.x;
+        if (tid == 0) mbar_init(&tile_bar, 1);
+        __syncthreads();
+        if (warp == 0) {
+            int run = 0, total = 0;
+            for (int i0 = 0; i0 < K; i0 += 32) {
+                const int i = i0 + lane;
+                int j0 = 0, cnt = 0;
+                if (i < K) {
+                    j0 = sm.lo[i];
+                    cnt = max(sm.hi[i] - j0 + 1, 0);
+                }
+                int incl = cnt;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const int n = __shfl_up_sync(kFull, incl, o);
+                    if (lane >= o) incl += n;
+                }
+                const int off = run + incl - cnt;
+                const bool cached = cnt > 0 && off + cnt <= a.cache_segs;
+                if (i < K) sm.base[i] = cached ? off - j0 : kNoCache;
+                total += cached ? cnt : 0;
+                run += __shfl_sync(kFull, incl, 31);
+            }
+#pragma unroll
+            for (int o = 16; o; o >>= 1) total += __shfl_xor_sync(kFull, total, o);
+            if (lane == 0) mbar_expect_tx(&tile_bar, (unsigned)total * (kChunk * 4));
+            __syncwarp();
+            for (int i = lane; i < K; i += 32) {
+                const int bs = sm.base[i];
+                if (bs == kNoCache) continue;
+                const int j0 = sm.lo[i], j1 = sm.hi[i];
+                const float *src = a.Dd + (size_t)sm.sk[i] * a.Sp;
+                for (int j = j0; j <= j1; ++j)
+                    bulk_g2s(sm.tile + (size_t)(bs + j) * kChunk, src + (size_t)(b + j * G) * kChunk, kChunk * 4, &tile_bar);
+            }
+        }
+        __syncthreads();          // sm.base visible to all warps
+        mbar_wait(&tile_bar, 0);  // the staged segments have landed
+    }
     const double Tm = (double)a.Tmax, ab = (double)a.abmax, Spd = (double)a.Sp;
 
     const int G = gridDim.x;
     const int ngroups = (a.nchunks + G * kGroup - 1) / (G * kGroup);
     const int recn = N + 2;
-    unsigned ph = *a.phase;   // written by the previous launch, stream ordered
+    unsigned ph = a.phase[0];      // rotation of the records; written by the previous launch, stream ordered
     float *zcur = a.z, *znext = a.zn;
     // resident slot data: T, alpha, beta of the block's own slots are read once, z and q never leave the SM
     const bool res = a.rslots > 0;
@@ -596,15 +700,22 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     // start a pass: the record that collects its sums; block 0 clears the record of the next pass
     auto begin_pass = [&]() -> long long * {
         if (blockIdx.x == 0) {
-            long long *nx = a.accbuf + (size_t)((ph + 1) % 3) * recn;
-            for (int i = tid; i < recn; i += kMasterThreads) nx[i] = 0;
+            long long *nx = a.accbuf + (size_t)((ph + 1) % 3) * kSumGroups * recn;
+            for (int i = tid; i < kSumGroups * recn; i += kMasterThreads) nx[i] = 0;
         }
-        return a.accbuf + (size_t)(ph % 3) * recn;
+        return a.accbuf + ((size_t)(ph % 3) * kSumGroups + blockIdx.x % kSumGroups) * recn;
     };
 
     // after the grid barrier: one round trip to L2 for the whole record, then the control warp works from smem
     auto fetch_record = [&](const long long *rec) {
-        for (int i = tid; i < K + 2; i += kMasterThreads) sm.recv[i] = __ldcg(rec + i);
+        // sum of the group records (integers: any order gives the same bits); rec is this block's own record
+        const long long *r0 = rec - (size_t)(blockIdx.x % kSumGroups) * recn;
+        for (int i = tid; i < K + 2; i += kMasterThreads) {
+            long long v = 0;
+#pragma unroll
+            for (int gq = 0; gq < kSumGroups; ++gq) v += __ldcg(r0 + (size_t)gq * recn + i);
+            sm.recv[i] = v;
+        }
         __syncthreads();
     };
 
@@ -700,7 +811,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     __syncthreads();
     long long *rec = begin_pass();
     eval_pass<true>(a, sm, K, ngroups, nullptr, zcur, nullptr, rzcur, 0.f, rec, sm.ctl->scF, sm.ctl->scG, red PROF_ARG);
-    grid.sync();
+    cg::this_grid().sync();
     ++ph;
     fetch_record(rec);
     if (ctl) {
@@ -769,11 +880,12 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
         if (tid == 0) fx_add(rec + 1, curv, sm.ctl->scC);
         PROFX(15)
         PROF(0)
-        grid.sync();
+        cg::this_grid().sync();
         PROF(1)
         ++ph;
+        fetch_record(rec);
         if (ctl) {
-            const double curvF = (double)__ldcg(rec + 1) * sm.ctl->iC;
+            const double curvF = (double)sm.recv[1] * sm.ctl->iC;
             const double phi2 = 2.0 * curvF + 2.0 * a.gamma * Gd;
             t = phi2 > 0.0 ? -phi1 / phi2 : (isfinite(tmax) ? tmax : 1.0);
             hit = 0;
@@ -794,7 +906,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
             eval_pass<false>(a, sm, K, ngroups, zcur, znext, rzcur, rznext, sm.ctl->tf, rec, sm.ctl->scF,
                              sm.ctl->scG, red PROF_ARG);
             PROF(3)
-            grid.sync();
+            cg::this_grid().sync();
             PROF(4)
             ++ph;
             fetch_record(rec);
@@ -901,17 +1013,18 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     if (sm.ctl->accepted) {
         rec = begin_pass();
         eval_pass<true>(a, sm, K, ngroups, nullptr, a.z, nullptr, rzcur, 0.f, rec, sm.ctl->scF, sm.ctl->scG, red PROF_ARG);
-        grid.sync();
+        cg::this_grid().sync();
         ++ph;
+        fetch_record(rec);
         if (ctl) {
-            F = (double)__ldcg(rec) * sm.ctl->iF + a.F_out;
+            F = (double)sm.recv[0] * sm.ctl->iF + a.F_out;
             Phi = F + a.gamma * Gs;
         }
     }
     if (blockIdx.x == 0 && warp == 0) {
         for (int k = lane; k < N; k += 32) a.y[k] = sm.y[k];
         if (lane == 0) {
-            *a.phase = ph % 3;
+            a.phase[0] = ph % 3;
             MasterOut o;
             o.inner = inner;
             o.backtracks = backtracks;
@@ -936,10 +1049,10 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     }
 }
 
-size_t master_smem_bytes(int64_t N, int64_t rslots) {
-    return (size_t)(kMasterWarps * kGroup * kChunk + kGroup * kChunk + 6 * rslots) * 4   // part, wbuf, resident slots
-           + (size_t)(11 * N + 2 + kMasterWarps + 2 * kMasterWarps * kRedSlots) * 8 + sizeof(Ctl)   // K-vectors, recv, red, cred, ctl
-           + (size_t)N * 4 * 5;                                              // coef, sk, lo, hi, ik
+size_t master_smem_bytes(int64_t N, int64_t rslots, int64_t cache_segs) {
+    return (size_t)(kKSplit * kGroup * kChunk + kGroup * kChunk + 6 * rslots + cache_segs * kChunk) * 4   // part, wbuf, resident slots, tile
+           + (size_t)(12 * N + 2 + kMasterWarps + 2 * kMasterWarps * kRedSlots) * 8 + sizeof(Ctl)   // K-vectors, recv, red, cred, ctl
+           + (size_t)N * 4 * 6;                                              // coef, sk, lo, hi, ik
 }
 
 }  // namespace
@@ -955,23 +1068,33 @@ int master_configure(vmat_plan *p) {
     int64_t rslots = ngroups * kGroup * kChunk;
     if (rslots * 6 * 4 > 96 * 1024) rslots = 0;
     p->master_rslots = (int)rslots;
-    p->master_smem = master_smem_bytes(p->N, rslots);
-    if (p->master_smem > 220 * 1024) {
+    // what is left of the SM's opt-in shared memory (minus static use and room for L1) holds the tile of Dd
+    int optin = 0;
+    VMAT_CUDA(p, cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, p->device));
+    const size_t budget = (size_t)optin > 8 * 1024 ? (size_t)optin - 8 * 1024 : 0;
+    size_t fixed = master_smem_bytes(p->N, rslots, 0);
+    if (fixed > budget) {
         p->master_rslots = 0;
-        p->master_smem = master_smem_bytes(p->N, 0);
+        fixed = master_smem_bytes(p->N, 0, 0);
     }
-    if (p->master_smem > 220 * 1024) return fail(p, VMAT_EINVAL, "n_beams too large for the master kernel's shared memory");
+    if (fixed > budget) return fail(p, VMAT_EINVAL, "n_beams too large for the master kernel's shared memory");
+    p->master_cache_segs = (int)((budget - fixed) / (kChunk * 4));
+#ifdef VMAT_MASTER_PROFILE
+    if (getenv("VMAT_NO_TILE")) p->master_cache_segs = 0;
+    fprintf(stderr, "master: grid %d smem fixed %zu cache_segs %d rslots %d\n", p->master_grid, fixed, p->master_cache_segs, p->master_rslots);
+#endif
+    p->master_smem = master_smem_bytes(p->N, p->master_rslots, p->master_cache_segs);
     VMAT_CUDA(p, cudaFuncSetAttribute(k_master, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->master_smem));
     int per_sm = 0;
     VMAT_CUDA(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_master, kMasterThreads, p->master_smem));
     if (per_sm < 1) return fail(p, VMAT_ECUDA, "master kernel does not fit on an SM");
     int rc;
-    if ((rc = dev_alloc(p, &p->accbuf, 3 * (p->N + 2)))) return rc;
-    if ((rc = dev_alloc(p, &p->phase, 1))) return rc;
+    if ((rc = dev_alloc(p, &p->accbuf, 3 * kSumGroups * (p->N + 2)))) return rc;
+    if ((rc = dev_alloc(p, &p->phase, 2))) return rc;
     if ((rc = dev_alloc(p, &p->colstat, p->N))) return rc;
     if ((rc = dev_alloc(p, &p->vbounds, 2))) return rc;
-    VMAT_CUDA(p, cudaMemsetAsync(p->accbuf, 0, (size_t)3 * (p->N + 2) * 8, p->stream));
-    VMAT_CUDA(p, cudaMemsetAsync(p->phase, 0, 4, p->stream));
+    VMAT_CUDA(p, cudaMemsetAsync(p->accbuf, 0, (size_t)3 * kSumGroups * (p->N + 2) * 8, p->stream));
+    VMAT_CUDA(p, cudaMemsetAsync(p->phase, 0, 8, p->stream));
     VMAT_CUDA(p, cudaMemsetAsync(p->colstat, 0, (size_t)p->N * sizeof(ColStat), p->stream));
     VMAT_CUDA(p, cudaMemsetAsync(p->vbounds, 0, 8, p->stream));
     k_voxel_bounds<<<(unsigned)((p->Sp + 255) / 256), 256, 0, p->stream>>>(p->T_s, p->alpha_s, p->beta_s,
@@ -1020,6 +1143,7 @@ static int launch_master_impl(vmat_plan *p, int max_inner, int trace_it) {
     a.stall_count = p->opt.master_stall_count;
     a.max_inner = max_inner;
     a.rslots = p->master_rslots;
+    a.cache_segs = p->master_cache_segs;
     a.colstat = p->colstat;
     a.fx_inv = p->fx_inv;
     a.Tmax = p->Tmax;
