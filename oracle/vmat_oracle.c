@@ -15,7 +15,9 @@
  * O2/O4; central finite differences and closed forms for O3; brute-force interval enumeration and
  * the textbook minimum-sum subarray for O5; the one-sided finite difference of the full cost for
  * O6; KKT conditions, scipy NNLS and one/two-aperture closed forms for O7; monotone cost and the
- * leaf-travel invariant for O8.
+ * leaf-travel invariant for O8; for the dose-rate feasibility post-pass: feasibility at
+ * exit, gamma = gamma_0 factor^rounds, infeasibility one round earlier (an independent master solve at
+ * the previous gamma), and the two-beam closed form of the smoothed optimum.
  * PARITY UNPINNED: whole-plan numbers (the paper prints no worked example; Table 1 needs clinical
  * data that is not available).
  *
@@ -445,6 +447,66 @@ void vo_master(const vo_problem *p, const uint8_t *occ, const int32_t *left, con
     vo_columns *cols = columns_new(p->N, p->V);
     for (int64_t k = 0; k < p->N; ++k) if (occ[k]) columns_add(cols, p, k, left, right);
     master_solve(p, cols, occ, y, z, info);
+    columns_free(cols);
+}
+
+/* ---- hard dose-rate feasibility after the last aperture -----------------------------
+ * "In the optimization model, we add dose rate constraints as penalty-based soft constraints in the cost
+ *  function.  However, these constraints need to be satisfied as hard constraints. [...] if the final
+ *  solution is not feasible, the coefficient gamma in the objective function will be automatically
+ *  increased and then the intensity for each aperture will be re-optimized till the solution is feasible."
+ * The constraint itself is PAPER.md:80: "the dose rate variation between neighboring angles is constrained
+ * within a certain range".  Readings (R1-R3): the range is
+ *     |y_{k+1} - y_k| <= rho * (theta_{k+1} - theta_k)   for k = 1..N-1   (rho: intensity change per degree),
+ * "increased" is a multiplication of gamma by `factor` (the paper gives no rule), and the incoming y is
+ * tested first: a feasible plan is returned untouched with zero rounds.
+ *
+ * ratio = max_k |y_{k+1} - y_k| / (rho (theta_{k+1} - theta_k));  feasible iff ratio <= 1 + tol. */
+double vo_rate_ratio(int64_t N, const double *y, const double *theta, double rho) {
+    double r = 0.0;
+    for (int64_t k = 0; k + 1 < N; ++k) {
+        const double v = fabs(y[k + 1] - y[k]) / (rho * (theta[k + 1] - theta[k]));
+        if (v > r) r = v;
+    }
+    return r;
+}
+
+typedef struct {
+    double  rho, factor, tol;      /* in */
+    int64_t max_rounds;            /* in */
+    double  eps;                   /* in: master tolerance */
+    int64_t max_inner;             /* in */
+    int64_t rounds;                /* out: number of times gamma was raised and the master re-solved */
+    int64_t feasible;              /* out */
+    double  gamma;                 /* out: gamma at exit = gamma_0 * factor^rounds */
+    double  ratio;                 /* out: ratio at exit */
+    double  F, G, cost;            /* out: at exit, cost = F + gamma G with the gamma at exit */
+} vo_rate_info;
+
+void vo_enforce_rate(const vo_problem *p, const uint8_t *occ, const int32_t *left, const int32_t *right, double *y,
+                     double *z, vo_rate_info *info) {
+    vo_problem q = *p;
+    vo_columns *cols = columns_new(p->N, p->V);
+    for (int64_t k = 0; k < p->N; ++k) if (occ[k]) columns_add(cols, p, k, left, right);
+    double ratio = vo_rate_ratio(p->N, y, p->theta, info->rho);
+    int64_t rounds = 0;
+    while (ratio > 1.0 + info->tol && rounds < info->max_rounds) {
+        q.gamma *= info->factor;                                   /* "gamma ... automatically increased"   */
+        vo_master_info mi;
+        mi.eps = info->eps;
+        mi.max_inner = info->max_inner;
+        master_solve(&q, cols, occ, y, z, &mi);                    /* "intensity ... re-optimized"          */
+        ++rounds;
+        ratio = vo_rate_ratio(p->N, y, p->theta, info->rho);       /* "till the solution is feasible"       */
+    }
+    columns_dose(cols, occ, y, z);
+    info->rounds = rounds;
+    info->feasible = ratio <= 1.0 + info->tol;
+    info->gamma = q.gamma;
+    info->ratio = ratio;
+    info->F = vo_penalty(p->V, z, p->T, p->alpha, p->beta, NULL);
+    info->G = vo_smooth(p->N, y, p->theta, NULL);
+    info->cost = info->F + q.gamma * info->G;
     columns_free(cols);
 }
 

@@ -40,6 +40,13 @@ class _MasterInfo(_c.Structure):
                 ("F", _c.c_double), ("G", _c.c_double), ("cost", _c.c_double)]
 
 
+class _RateInfo(_c.Structure):
+    _fields_ = [("rho", _c.c_double), ("factor", _c.c_double), ("tol", _c.c_double), ("max_rounds", _c.c_int64),
+                ("eps", _c.c_double), ("max_inner", _c.c_int64), ("rounds", _c.c_int64), ("feasible", _c.c_int64),
+                ("gamma", _c.c_double), ("ratio", _c.c_double), ("F", _c.c_double), ("G", _c.c_double),
+                ("cost", _c.c_double)]
+
+
 class _Trace(_c.Structure):
     _fields_ = [("max_iters", _c.c_int64), ("eps", _c.c_double), ("max_inner", _c.c_int64),
                 ("iters", _c.c_int64), ("beam", _P), ("price", _P), ("F", _P), ("G", _P), ("cost", _P),
@@ -73,6 +80,10 @@ def _load():
         L.vo_master.restype = None
         L.vo_cost_gradient.argtypes = [PP, _P, _P, _P, _P, _P, _P]
         L.vo_cost_gradient.restype = None
+        L.vo_rate_ratio.argtypes = [_c.c_int64, _P, _P, _c.c_double]
+        L.vo_rate_ratio.restype = _c.c_double
+        L.vo_enforce_rate.argtypes = [PP, _P, _P, _P, _P, _P, _c.POINTER(_RateInfo)]
+        L.vo_enforce_rate.restype = None
         L.vo_solve.argtypes = [PP, _P, _P, _P, _P, _P, _c.POINTER(_Trace)]
         L.vo_solve.restype = None
         L.vo_num_threads.restype = _c.c_int
@@ -256,6 +267,23 @@ class Oracle:
         grad, c3 = np.empty(self.N, np.float64), np.empty(3, np.float64)
         self._L.vo_cost_gradient(_c.byref(self._p), _ptr(occ), _ptr(left), _ptr(right), _ptr(y), _ptr(grad), _ptr(c3))
         return grad, tuple(float(c) for c in c3)
+
+    # hard dose-rate feasibility after the last aperture ---------------------------------
+    def rate_ratio(self, y, rho):
+        """max_k |y_{k+1} - y_k| / (rho (theta_{k+1} - theta_k)); the plan is feasible iff this is <= 1."""
+        y = _as(y, np.float64)
+        return float(self._L.vo_rate_ratio(self.N, _ptr(y), _ptr(self.theta), float(rho)))
+
+    def enforce_rate(self, occ, left, right, y, rho, factor=2.0, tol=1e-6, max_rounds=60, eps=1e-9, max_inner=20000):
+        """Raise gamma by `factor` and re-solve the master until |dy| <= rho dtheta everywhere.
+        Returns (y, z, dict(rounds, feasible, gamma, ratio, F, G, cost))."""
+        occ, left, right = self._plan(occ, left, right)
+        y = _as(y, np.float64).copy()
+        z = np.empty(self.V, np.float64)
+        info = _RateInfo(rho=rho, factor=factor, tol=tol, max_rounds=max_rounds, eps=eps, max_inner=max_inner)
+        self._L.vo_enforce_rate(_c.byref(self._p), _ptr(occ), _ptr(left), _ptr(right), _ptr(y), _ptr(z), _c.byref(info))
+        return y, z, dict(rounds=int(info.rounds), feasible=bool(info.feasible), gamma=float(info.gamma),
+                          ratio=float(info.ratio), F=float(info.F), G=float(info.G), cost=float(info.cost))
 
     # O1 + O8 -----------------------------------------------------------------------------------
     def solve(self, max_iters, plan=None, eps=1e-9, max_inner=20000):

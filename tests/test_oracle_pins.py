@@ -470,3 +470,85 @@ def test_phantom_shape_is_in_the_range_of_table1():
     ph = vmat_inputs.make_phantom(vmat_inputs.scaled_config("prostate", n_beams=6), check_reach=False)
     mine = ph.nnz / ph.n_beamlets
     assert 0.5 * min(per_beamlet) < mine < 2 * max(per_beamlet)
+
+
+# ------------------------------------------------------------------------------------------------
+# hard dose-rate feasibility after the last aperture (raise gamma, re-solve the master)
+# ------------------------------------------------------------------------------------------------
+def test_rate_ratio_by_hand():
+    o, _, _ = small_problem(seed=3, N=4, nonuniform_theta=True)
+    y = np.array([0.0, 1.0, 0.5, 2.5])
+    dth = np.diff(o.theta)
+    by_hand = max(abs(1.0 - 0.0) / (0.25 * dth[0]), abs(0.5 - 1.0) / (0.25 * dth[1]), abs(2.5 - 0.5) / (0.25 * dth[2]))
+    assert o.rate_ratio(y, 0.25) == pytest.approx(by_hand, rel=1e-15)
+    assert o.rate_ratio(np.full(4, 0.7), 0.25) == 0.0                       # constant dose rate: no variation
+
+
+def two_beam_problem(gamma):
+    # beam 0 reaches only voxel 0 (D = a), beam 1 only voxel 1 (D = b); alpha = beta = 1: everything is quadratic
+    a, b, T0, T1, dth = 0.5, 0.25, 1.0, 0.25, 2.0
+    o = Oracle(np.array([0, 1, 2], np.int64), [0, 1], [a, b], [T0, T1], [1.0, 1.0], [1.0, 1.0], [0.0, dth], 1, 1, 1, gamma)
+    return o, (a, b, T0, T1, dth)
+
+
+def two_beam_optimum(a, b, T0, T1, dth, gamma):
+    # stationarity of (a y0 - T0)^2 + (b y1 - T1)^2 + gamma (y1 - y0)^2 / dth, written out:
+    #   (a^2 + g) y0 - g y1 = a T0 ;  -g y0 + (b^2 + g) y1 = b T1 ,  g = gamma / dth ; Cramer's rule
+    g = gamma / dth
+    det = (a * a + g) * (b * b + g) - g * g
+    return np.array([(a * T0 * (b * b + g) + g * b * T1) / det, ((a * a + g) * b * T1 + g * a * T0) / det])
+
+
+def test_enforce_rate_two_beam_closed_form():
+    gamma0, rho, factor = 0.01, 0.05, 2.0
+    o, prm = two_beam_problem(gamma0)
+    occ, left, right = [1, 1], [[0], [0]], [[1], [1]]
+    y0, _, _ = o.master(occ, left, right)
+    np.testing.assert_allclose(y0, two_beam_optimum(*prm, gamma0), rtol=1e-8)
+    # the closed form tells how often gamma has to double before |y1 - y0| <= rho dtheta
+    want = 0
+    while abs(np.diff(two_beam_optimum(*prm, gamma0 * factor ** want))[0]) > rho * prm[4]:
+        want += 1
+    assert want >= 3                                                          # the case is not trivial
+    y, z, info = o.enforce_rate(occ, left, right, y0, rho, factor=factor, tol=0.0)
+    assert info["rounds"] == want and info["feasible"]
+    assert info["gamma"] == gamma0 * factor ** want
+    np.testing.assert_allclose(y, two_beam_optimum(*prm, info["gamma"]), rtol=1e-7)
+    assert info["ratio"] == pytest.approx(abs(y[1] - y[0]) / (rho * prm[4]), rel=1e-12) and info["ratio"] <= 1.0
+    assert info["cost"] == pytest.approx((prm[0] * y[0] - prm[2]) ** 2 + (prm[1] * y[1] - prm[3]) ** 2
+                                         + info["gamma"] * (y[1] - y[0]) ** 2 / prm[4], rel=1e-9)
+
+
+def test_enforce_rate_random_problems():
+    for seed in range(4):
+        o, dense, rng = small_problem(seed=50 + seed, N=6, gamma=0.05, nonuniform_theta=bool(seed % 2))
+        occ, left, right, y_any = random_plan(o, rng, o.N)
+        y0, _, _ = o.master(occ, left, right, eps=1e-11)
+        r0 = o.rate_ratio(y0, 1.0)
+        # a limit far above the plan's variation: nothing to do, the plan comes back untouched
+        y, z, info = o.enforce_rate(occ, left, right, y0, rho=10.0 * r0)
+        assert info["rounds"] == 0 and info["feasible"] and info["gamma"] == o.gamma and np.array_equal(y, y0)
+        # a limit at a third of it: gamma has to rise
+        rho = r0 / 3.0
+        y, z, info = o.enforce_rate(occ, left, right, y0, rho=rho, factor=2.0, tol=1e-9, eps=1e-11)
+        assert info["feasible"] and info["rounds"] >= 1
+        assert info["gamma"] == o.gamma * 2.0 ** info["rounds"]
+        assert np.max(np.abs(np.diff(y)) / (rho * np.diff(o.theta))) <= 1.0 + 1e-9      # the definition, by hand
+        assert np.all(y >= 0)
+        np.testing.assert_allclose(z, dense.T @ (open_mask(o, occ, left, right).reshape(-1) * np.repeat(y, o.R * o.C)), rtol=1e-10, atol=1e-12)
+        # y is the master optimum for the gamma at exit (KKT on an oracle built with that gamma) ...
+        o_exit = Oracle(o.row_ptr, o.col, o.val, o.T, o.alpha, o.beta, o.theta, o.R, o.C, o.delta, info["gamma"])
+        viol, _ = kkt_violation(o_exit, occ, left, right, y)
+        assert viol <= 1e-7
+        # ... and one round earlier the optimum was still infeasible (gamma is not raised further than needed)
+        o_prev = Oracle(o.row_ptr, o.col, o.val, o.T, o.alpha, o.beta, o.theta, o.R, o.C, o.delta, info["gamma"] / 2.0)
+        y_prev, _, _ = o_prev.master(occ, left, right, y0=y0, eps=1e-11)
+        assert o.rate_ratio(y_prev, rho) > 1.0 + 1e-9
+
+
+def test_enforce_rate_gives_up_at_the_round_cap():
+    o, prm = two_beam_problem(0.01)
+    occ, left, right = [1, 1], [[0], [0]], [[1], [1]]
+    y0, _, _ = o.master(occ, left, right)
+    y, z, info = o.enforce_rate(occ, left, right, y0, rho=1e-9, max_rounds=3)
+    assert info["rounds"] == 3 and not info["feasible"] and info["gamma"] == 0.01 * 8.0
