@@ -180,6 +180,27 @@ int vmat_master(vmat_plan *plan, vmat_master_stats *out);
  * are enqueued without a host round trip; the call synchronises once at the end.             */
 int vmat_solve(vmat_plan *plan, int32_t max_iters, vmat_solve_stats *out);
 
+/* Hard dose-rate feasibility after the last aperture ("if the final solution is not
+ * feasible, the coefficient gamma in the objective function will be automatically increased and then
+ * the intensity for each aperture will be re-optimized till the solution is feasible").  The constraint
+ * ("the dose rate variation between neighboring angles is constrained within a certain
+ * range") is read as |y_{k+1} - y_k| <= max_variation_per_deg * (theta_{k+1} - theta_k), k = 1..N-1
+ * (R1-R3).  ratio = max_k |y_{k+1}-y_k| / (max_variation_per_deg (theta_{k+1}-theta_k));
+ * while ratio > 1 + tol and fewer than max_rounds rounds were spent: gamma *= gamma_factor, step (e)
+ * runs again (warm start).  The plan's y is tested first: a feasible plan costs zero rounds.  The
+ * plan keeps the gamma at exit.  out may be NULL.  Requires max_variation_per_deg > 0,
+ * gamma_factor > 1, tol >= 0, max_rounds >= 0.  Synchronises the stream once per round.       */
+typedef struct {
+    int32_t rounds;         /* times gamma was raised and the master re-solved                  */
+    int32_t feasible;       /* 1 if ratio <= 1 + tol at exit                                    */
+    int32_t inner_total;    /* master inner iterations over all rounds                          */
+    double  gamma;          /* gamma at exit = gamma at entry * gamma_factor^rounds             */
+    double  ratio;          /* at exit                                                          */
+    double  F, G, cost;     /* at exit, cost = F + gamma G with the gamma at exit               */
+} vmat_rate_stats;
+int vmat_enforce_dose_rate(vmat_plan *plan, double max_variation_per_deg, double gamma_factor, double tol,
+                           int32_t max_rounds, vmat_rate_stats *out);
+
 /* Plan state: occupied mask (N bytes), leaf pairs (N*R each), dose rates (N doubles); all HOST.
  * vmat_set_plan validates 0 <= l <= r' <= C and the leaf-travel invariant between successive
  * occupied beams.  Any pointer of vmat_get_plan may be NULL.                                  */

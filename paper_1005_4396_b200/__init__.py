@@ -28,7 +28,7 @@ VMAT_HOST, VMAT_DEVICE = 0, 1
 SYMBOLS = (
     "vmat_default_options", "vmat_create", "vmat_destroy", "vmat_get_info", "vmat_dose", "vmat_dose_recompute",
     "vmat_price",
-    "vmat_price_spmv", "vmat_leaf_search", "vmat_master", "vmat_solve", "vmat_get_plan", "vmat_set_plan",
+    "vmat_price_spmv", "vmat_leaf_search", "vmat_master", "vmat_enforce_dose_rate", "vmat_solve", "vmat_get_plan", "vmat_set_plan",
     "vmat_launch_count", "vmat_last_error",
 )
 
@@ -62,6 +62,11 @@ class _SolveStats(C.Structure):
                 ("us_column", C.c_double), ("us_master", C.c_double), ("F", C.c_double), ("G", C.c_double),
                 ("cost", C.c_double), ("beam", _P), ("price", _P), ("trace_F", _P), ("trace_G", _P),
                 ("trace_cost", _P), ("inner", _P)]
+
+
+class _RateStats(C.Structure):
+    _fields_ = [("rounds", C.c_int32), ("feasible", C.c_int32), ("inner_total", C.c_int32), ("gamma", C.c_double),
+                ("ratio", C.c_double), ("F", C.c_double), ("G", C.c_double), ("cost", C.c_double)]
 
 
 class _Info(C.Structure):
@@ -98,6 +103,7 @@ def load_library():
     L.vmat_price_spmv.argtypes = [_P, _P, _P]
     L.vmat_leaf_search.argtypes = [_P, _P, _P, _P, _P]
     L.vmat_master.argtypes = [_P, C.POINTER(_MasterStats)]
+    L.vmat_enforce_dose_rate.argtypes = [_P, C.c_double, C.c_double, C.c_double, C.c_int32, C.POINTER(_RateStats)]
     L.vmat_solve.argtypes = [_P, C.c_int32, C.POINTER(_SolveStats)]
     L.vmat_get_plan.argtypes = [_P, _P, _P, _P, _P]
     L.vmat_set_plan.argtypes = [_P, _P, _P, _P, _P]
@@ -107,7 +113,8 @@ def load_library():
     L.vmat_last_error.restype = C.c_char_p
     for name in ("vmat_create", "vmat_destroy", "vmat_get_info", "vmat_dose", "vmat_dose_recompute", "vmat_price",
                  "vmat_price_spmv",
-                 "vmat_leaf_search", "vmat_master", "vmat_solve", "vmat_get_plan", "vmat_set_plan"):
+                 "vmat_leaf_search", "vmat_master", "vmat_enforce_dose_rate", "vmat_solve", "vmat_get_plan",
+                 "vmat_set_plan"):
         getattr(L, name).restype = C.c_int
     _lib = L
     return L
@@ -297,6 +304,16 @@ class Plan:
         s = _MasterStats()
         self._check(self._L.vmat_master(self._h, C.byref(s)))
         return MasterStats(s.inner, s.backtracks, s.stop_reason, s.pg_entry, s.pg_exit, s.F, s.G, s.cost)
+
+    def enforce_dose_rate(self, max_variation_per_deg: float, gamma_factor: float = 2.0, tol: float = 1e-6,
+                          max_rounds: int = 60) -> dict:
+        """vmat_enforce_dose_rate: raise gamma and re-solve the master until the dose-rate variation
+        between neighbouring angles is within the limit.  Returns the stats as a dict."""
+        s = _RateStats()
+        self._check(self._L.vmat_enforce_dose_rate(self._h, float(max_variation_per_deg), float(gamma_factor),
+                                                   float(tol), int(max_rounds), C.byref(s)))
+        return dict(rounds=s.rounds, feasible=bool(s.feasible), inner_total=s.inner_total, gamma=s.gamma,
+                    ratio=s.ratio, F=s.F, G=s.G, cost=s.cost)
 
     def solve(self, max_iters: int, trace: bool = True) -> SolveStats:
         M = max(int(max_iters), 1)

@@ -178,6 +178,7 @@ int vmat_create(const vmat_problem *pb, const vmat_options *options, void *cuda_
     A(p->ticket, 1);
     A(p->mout, 1);
     A(p->cost3, 3);
+    A(p->rate_ratio, 1);
     p->tr_cap = (int32_t)N;
     A(p->tr_beam, N);
     A(p->tr_inner, N);
@@ -344,6 +345,51 @@ int vmat_master(vmat_plan *p, vmat_master_stats *out) {
         out->F = h.F;
         out->G = h.G;
         out->cost = h.cost;
+    }
+    return VMAT_OK;
+}
+
+int vmat_enforce_dose_rate(vmat_plan *p, double rho, double factor, double tol, int32_t max_rounds,
+                           vmat_rate_stats *out) {
+    if (!p) return VMAT_EINVAL;
+    if (!(rho > 0.0) || !std::isfinite(rho)) return fail(p, VMAT_EINVAL, "max_variation_per_deg must be finite and > 0");
+    if (!(factor > 1.0) || !std::isfinite(factor)) return fail(p, VMAT_EINVAL, "gamma_factor must be finite and > 1");
+    if (!(tol >= 0.0) || max_rounds < 0) return fail(p, VMAT_EINVAL, "tol and max_rounds must be >= 0");
+    int rc;
+    if ((rc = ensure_state(p))) return rc;
+    if ((rc = ensure_columns(p))) return rc;
+    auto test = [&](double &ratio) -> int {
+        int r = launch_rate_ratio(p, rho, p->rate_ratio);
+        if (r) return r;
+        VMAT_CUDA(p, cudaMemcpyAsync(&ratio, p->rate_ratio, sizeof(double), cudaMemcpyDeviceToHost, p->stream));
+        VMAT_CUDA(p, cudaStreamSynchronize(p->stream));
+        return VMAT_OK;
+    };
+    double ratio = 0.0;
+    if ((rc = test(ratio))) return rc;
+    int32_t rounds = 0, inner_total = 0;
+    while (ratio > 1.0 + tol && rounds < max_rounds) {
+        p->gamma *= factor;                          // "gamma ... will be automatically increased"
+        if (!std::isfinite(p->gamma)) return fail(p, VMAT_ESTATE, "gamma overflowed while enforcing the dose-rate limit");
+        if ((rc = launch_master(p, -1))) return rc;  // "the intensity for each aperture will be re-optimized"
+        MasterOut h;
+        VMAT_CUDA(p, cudaMemcpyAsync(&h, p->mout, sizeof(MasterOut), cudaMemcpyDeviceToHost, p->stream));
+        if ((rc = test(ratio))) return rc;           // "till the solution is feasible"
+        inner_total += h.inner;
+        ++rounds;
+    }
+    double c3[3];
+    VMAT_CUDA(p, cudaMemcpyAsync(c3, p->cost3, sizeof(c3), cudaMemcpyDeviceToHost, p->stream));
+    VMAT_CUDA(p, cudaStreamSynchronize(p->stream));
+    if (out) {
+        out->rounds = rounds;
+        out->feasible = ratio <= 1.0 + tol ? 1 : 0;
+        out->inner_total = inner_total;
+        out->gamma = p->gamma;
+        out->ratio = ratio;
+        out->F = c3[0];
+        out->G = c3[1];
+        out->cost = c3[2];
     }
     return VMAT_OK;
 }

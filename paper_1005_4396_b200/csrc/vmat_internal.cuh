@@ -92,6 +92,7 @@ struct vmat_plan {
     int master_rslots = 0;             // slots per master block kept resident in shared memory (0: none)
     vmat::MasterOut *mout = nullptr;
     double *cost3 = nullptr;       // device {F, G, F+gamma G}
+    double *rate_ratio = nullptr;  // device scalar of the dose-rate feasibility test
     double *part_dose = nullptr;   // partial F sums of the direct dose pass
     void *dose_scale = nullptr;    // device scalars of the direct dose pass (vmat_dose.cu)
     int dose_blocks = 0;
@@ -157,6 +158,7 @@ int launch_dose_grad(vmat_plan *p);
 int launch_master(vmat_plan *p, int trace_it);
 int launch_expand(vmat_plan *p, const float *src_s, float *dst_V, int what /*0 z, 1 w*/);
 int launch_compress(vmat_plan *p, const float *src_V, float *dst_s);
+int launch_rate_ratio(vmat_plan *p, double rho, double *ratio_dev);
 
 // vmat_dose.cu: steps (a)+(b) straight from D (fixed-point atomics path) ------------------------------
 int dose_configure(vmat_plan *p);

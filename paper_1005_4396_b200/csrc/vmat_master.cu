@@ -151,6 +151,27 @@ __global__ void k_compress(const float *__restrict__ src_V, const int32_t *__res
     dst_s[s] = s < S ? src_V[voxel_of[s]] : 0.f;
 }
 
+// dose-rate feasibility test: ratio = max_k |y_{k+1} - y_k| / (rho (theta_{k+1} - theta_k)),
+// y = 0 at un-occupied beams (S2); one block, maximum taken in a fixed order
+__global__ void __launch_bounds__(256)
+k_rate_ratio(const uint8_t *__restrict__ occ, const double *__restrict__ y, const double *__restrict__ theta, int N,
+             double rho, double *__restrict__ out) {
+    __shared__ double s_max[8];
+    double r = 0.0;
+    for (int k = threadIdx.x; k + 1 < N; k += 256) {
+        const double y0 = occ[k] ? y[k] : 0.0, y1 = occ[k + 1] ? y[k + 1] : 0.0;
+        r = fmax(r, fabs(y1 - y0) / (rho * (theta[k + 1] - theta[k])));
+    }
+#pragma unroll
+    for (int o = 16; o; o >>= 1) r = fmax(r, __shfl_xor_sync(kFull, r, o));
+    if ((threadIdx.x & 31) == 0) s_max[threadIdx.x >> 5] = r;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int i = 1; i < 8; ++i) r = fmax(r, s_max[i]);
+        *out = r;
+    }
+}
+
 // max |T| and max(alpha, beta) over the support (bounds for the fixed-point scales of the master)
 __global__ void k_voxel_bounds(const float *__restrict__ T, const float *__restrict__ alpha,
                                const float *__restrict__ beta, long long Sp, unsigned int *__restrict__ out2) {
@@ -1178,6 +1199,13 @@ extern "C" void vmat_debug_master_prof(long long out[16], int reset) {
     }
 }
 #endif
+
+int launch_rate_ratio(vmat_plan *p, double rho, double *ratio_dev) {
+    k_rate_ratio<<<1, 256, 0, p->stream>>>(p->occ, p->y, p->theta, (int)p->N, rho, ratio_dev);
+    ++p->launches;
+    VMAT_CUDA(p, cudaGetLastError());
+    return VMAT_OK;
+}
 
 int launch_expand(vmat_plan *p, const float *src_s, float *dst_V, int what) {
     if (p->V == 0) return VMAT_OK;

@@ -326,6 +326,48 @@ def test_device_resident_inputs_give_the_same_plan(torch_cuda, vm, tiny_phantom,
 
 
 # ------------------------------------------------------------------------------------------------
+# hard dose-rate feasibility after the last aperture
+# ------------------------------------------------------------------------------------------------
+def test_enforce_dose_rate_matches_oracle(torch_cuda, vm, tiny_oracle, tiny_solution):
+    o = tiny_oracle
+    occ, left, right, y, z, tr = tiny_solution
+    r0 = o.rate_ratio(y, 1.0)
+    plan = make_plan(vm, o)
+    # (1) a limit the plan already meets: zero rounds, nothing changes
+    plan.set_plan(occ, left, right, y)
+    st = plan.enforce_dose_rate(2.0 * r0)
+    assert st["rounds"] == 0 and st["feasible"] and st["gamma"] == o.gamma
+    assert st["ratio"] == pytest.approx(0.5, rel=1e-12)                    # the test itself is fp64 on both sides
+    assert np.array_equal(plan.get_plan()[3], y)
+    # (2) limits that need gamma raised: same number of rounds, same gamma, cost within tolerance, feasible
+    for frac, factor in ((0.5, 2.0), (0.2, 2.0), (0.3, 4.0)):
+        rho = frac * r0
+        y_ref, z_ref, ref = o.enforce_rate(occ, left, right, y, rho, factor=factor, tol=1e-6, eps=1e-10)
+        assert ref["feasible"] and ref["rounds"] >= 1
+        plan2 = make_plan(vm, o)
+        plan2.set_plan(occ, left, right, y)
+        st = plan2.enforce_dose_rate(rho, gamma_factor=factor, tol=1e-6)
+        yd = plan2.get_plan()[3]
+        # the round count is a floating-point decision: it must agree unless the oracle's ratio sat within fp32
+        # noise of the limit one round earlier (not the case for these limits)
+        assert st["rounds"] == ref["rounds"] and st["gamma"] == ref["gamma"] and st["feasible"]
+        assert st["ratio"] <= 1.0 + 1e-6 and o.rate_ratio(yd, rho) == pytest.approx(st["ratio"], rel=1e-12)
+        assert abs(st["cost"] - ref["cost"]) <= TOL * abs(ref["cost"])
+        zd = torch_cuda.empty(o.V, dtype=torch_cuda.float32, device="cuda")
+        plan2.dose(zd)
+        assert relnorm(zd.cpu().numpy(), o.dose(occ, left, right, yd)) <= TOL
+        plan2.destroy()
+    # (3) argument checks and the round cap
+    with pytest.raises(vm.VmatError):
+        plan.enforce_dose_rate(0.0)
+    with pytest.raises(vm.VmatError):
+        plan.enforce_dose_rate(1.0, gamma_factor=1.0)
+    st = plan.enforce_dose_rate(1e-9 * r0, max_rounds=2)
+    assert st["rounds"] == 2 and not st["feasible"] and st["gamma"] == o.gamma * 4.0
+    plan.destroy()
+
+
+# ------------------------------------------------------------------------------------------------
 # boundary behaviour
 # ------------------------------------------------------------------------------------------------
 def test_create_rejects_malformed_problems(torch_cuda, vm):
