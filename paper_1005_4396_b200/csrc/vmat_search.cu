@@ -8,8 +8,10 @@
 // prefix sums are exact and independent of evaluation order (reading S9 / O5).  One
 // warp owns one leaf row: positions 0..C are dealt to the lanes in blocks of M, the prefix sums
 // P, the running maximum of P[l] over admissible l (later l wins ties) and the minimum of the key
-// (P[r']-P[l], r'-l, l) are warp-shuffle scans/reductions.  One block owns one beam; the last
-// block to finish picks the beam (smallest price, lowest k on ties) and commits it on request.
+// (P[r']-P[l], r'-l, l) are warp-shuffle scans/reductions.  A block owns kRowsPerBlock rows of one
+// beam; row optima are added to the beam's total with integer atomics (exact, order free); the last
+// block of a beam forms its price, the last block of all picks the beam (smallest price, lowest k
+// on ties) and commits it on request.
 #include <math_constants.h>
 
 #include "vmat_internal.cuh"
@@ -20,6 +22,7 @@ namespace {
 
 constexpr unsigned kFull = 0xffffffffu;
 constexpr int kSearchThreads = 256;
+constexpr int kRowsPerBlock = kSearchThreads / 32;   // one warp per leaf row
 
 __device__ __forceinline__ long long shfl_up_ll(long long v, int o) {
     return __shfl_up_sync(kFull, v, o);
@@ -139,7 +142,9 @@ struct SearchArgs {
     int32_t *out_left, *out_right;     // optional copies for the caller (may alias cand_*)
     double *out_price;
     Sel *sel;
-    unsigned int *ticket;
+    unsigned int *ticket;              // beams finished
+    unsigned long long *beam_total;    // N: sum of the row optima of a beam (all zero between launches)
+    unsigned int *beam_ticket;         // N: blocks of a beam finished (all zero between launches)
     int commit;
     int32_t *tr_beam;                  // trace slots (or null)
     double *tr_price;
@@ -152,9 +157,13 @@ __global__ void __launch_bounds__(kSearchThreads) k_leaf_search(const SearchArgs
     __shared__ unsigned long long s_total;
     __shared__ double s_price[kSearchThreads];
     __shared__ int s_beam[kSearchThreads];
-    const int k = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int N = a.N, R = a.R, C = a.C;
+    const int RB = (R + kRowsPerBlock - 1) / kRowsPerBlock;       // blocks per beam
+    const int k = blockIdx.x / RB, rb = blockIdx.x - k * RB;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const bool occupied = a.occ[k] != 0;
+    if (occupied && rb > 0) return;                               // block 0 of an occupied beam reports +inf
+    bool beam_done = false;                                       // this block finishes its beam (thread 0)
 
     if (!occupied) {
         if (tid == 0) {
@@ -171,7 +180,8 @@ __global__ void __launch_bounds__(kSearchThreads) k_leaf_search(const SearchArgs
             }
         __syncthreads();
         const int km = s_km, kp = s_kp;
-        for (int r = warp; r < R; r += kSearchThreads / 32) {
+        const int r = rb * kRowsPerBlock + warp;
+        if (r < R) {
             int Lmin = 0, Lmax = C, Rmin = 0, Rmax = C;
             if (km >= 0) {
                 const int b = a.delta * (k - km), l = a.left[km * R + r], rr = a.right[km * R + r];
@@ -202,29 +212,42 @@ __global__ void __launch_bounds__(kSearchThreads) k_leaf_search(const SearchArgs
         }
         __syncthreads();
         if (tid == 0) {
-            // price_k = 2^-30 * total + gamma * dG/dy_k, every operation individually rounded
-            // (Eq. 2; reading S10); same order of operations as the definition
-            double dG = 0.0;
-            if (k > 0)
-                dG = __dadd_rn(dG, __ddiv_rn(__dmul_rn(2.0, __dsub_rn(a.y[k], a.y[k - 1])),
-                                             __dsub_rn(a.theta[k], a.theta[k - 1])));
-            if (k + 1 < N)
-                dG = __dsub_rn(dG, __ddiv_rn(__dmul_rn(2.0, __dsub_rn(a.y[k + 1], a.y[k])),
-                                             __dsub_rn(a.theta[k + 1], a.theta[k])));
-            const double smooth = __dmul_rn(a.gamma, dG);
-            const double price = __dadd_rn(ldexp(__ll2double_rn((long long)s_total), -30), smooth);
-            a.beam_price[k] = price;
-            if (a.out_price) a.out_price[k] = price;
+            atomicAdd(a.beam_total + k, s_total);
+            __threadfence();
+            if (atomicAdd(a.beam_ticket + k, 1u) == (unsigned)RB - 1u) {
+                __threadfence();
+                beam_done = true;
+                const long long total = (long long)atomicExch(a.beam_total + k, 0ull);   // all RB sums are in; reset
+                a.beam_ticket[k] = 0u;
+                // price_k = 2^-30 * total + gamma * dG/dy_k, every operation individually rounded
+                // (Eq. 2; reading S10); same order of operations as the definition
+                double dG = 0.0;
+                if (k > 0)
+                    dG = __dadd_rn(dG, __ddiv_rn(__dmul_rn(2.0, __dsub_rn(a.y[k], a.y[k - 1])),
+                                                 __dsub_rn(a.theta[k], a.theta[k - 1])));
+                if (k + 1 < N)
+                    dG = __dsub_rn(dG, __ddiv_rn(__dmul_rn(2.0, __dsub_rn(a.y[k + 1], a.y[k])),
+                                                 __dsub_rn(a.theta[k + 1], a.theta[k])));
+                const double smooth = __dmul_rn(a.gamma, dG);
+                const double price = __dadd_rn(ldexp(__ll2double_rn(total), -30), smooth);
+                a.beam_price[k] = price;
+                if (a.out_price) a.out_price[k] = price;
+            }
         }
     } else if (tid == 0) {
+        beam_done = true;
         a.beam_price[k] = CUDART_INF;
         if (a.out_price) a.out_price[k] = CUDART_INF;
     }
 
-    // the last block to arrive chooses the beam
-    __threadfence();
-    __syncthreads();
-    if (tid == 0) s_last = atomicAdd(a.ticket, 1u) == gridDim.x - 1;
+    // the block that finishes the last beam chooses among all of them
+    if (tid == 0) {
+        s_last = 0;
+        if (beam_done) {
+            __threadfence();
+            s_last = atomicAdd(a.ticket, 1u) == (unsigned)N - 1u;
+        }
+    }
     __syncthreads();
     if (!s_last) return;
     __threadfence();
@@ -313,12 +336,14 @@ int launch_leaf_search(vmat_plan *p, const float *g, int32_t *all_left, int32_t 
     a.out_price = beam_price;
     a.sel = p->sel;
     a.ticket = p->ticket;
+    a.beam_total = p->beam_total;
+    a.beam_ticket = p->beam_ticket;
     a.commit = commit;
     a.tr_beam = trace_it >= 0 ? p->tr_beam : nullptr;
     a.tr_price = p->tr_price;
     a.trace_it = trace_it;
     const int M = (int)((p->C + 1 + 31) / 32);
-    const dim3 grid((unsigned)p->N), block(kSearchThreads);
+    const dim3 grid((unsigned)(p->N * ((p->R + kRowsPerBlock - 1) / kRowsPerBlock))), block(kSearchThreads);
     switch (M) {
         case 1: k_leaf_search<1><<<grid, block, 0, p->stream>>>(a); break;
         case 2: k_leaf_search<2><<<grid, block, 0, p->stream>>>(a); break;
