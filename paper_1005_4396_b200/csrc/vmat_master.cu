@@ -62,13 +62,27 @@ k_column_scatter(const uint32_t *__restrict__ rowq, const float4 *__restrict__ v
     if (c < left[k * R + r] || c >= right[k * R + r]) return;   // beamlet not exposed (A_k)
     const long long row = ((long long)k * R + r) * C + c;
     const uint32_t a = rowq[row], b = rowq[row + 1];
-    for (uint32_t q = a + lane; q < b; q += 32) {
-        const float4 v = __ldg(val4 + q);
-        const int4 s = __ldg(col4 + q);
-        if (v.x != 0.f) atomicAdd(acc + s.x, (unsigned long long)__double2ll_rn((double)v.x * fx_scale));
-        if (v.y != 0.f) atomicAdd(acc + s.y, (unsigned long long)__double2ll_rn((double)v.y * fx_scale));
-        if (v.z != 0.f) atomicAdd(acc + s.z, (unsigned long long)__double2ll_rn((double)v.z * fx_scale));
-        if (v.w != 0.f) atomicAdd(acc + s.w, (unsigned long long)__double2ll_rn((double)v.w * fx_scale));
+    // four quads per lane in flight before the first atomic (a row is ~100 quads: one round trip, not four)
+    for (uint32_t q = a + lane; q < b; q += 32 * 4) {
+        float4 v[4];
+        int4 s[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            if (q + 32 * u < b) {
+                v[u] = __ldg(val4 + q + 32 * u);
+                s[u] = __ldg(col4 + q + 32 * u);
+            } else {
+                v[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+                s[u] = make_int4(0, 0, 0, 0);
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            if (v[u].x != 0.f) atomicAdd(acc + s[u].x, (unsigned long long)__double2ll_rn((double)v[u].x * fx_scale));
+            if (v[u].y != 0.f) atomicAdd(acc + s[u].y, (unsigned long long)__double2ll_rn((double)v[u].y * fx_scale));
+            if (v[u].z != 0.f) atomicAdd(acc + s[u].z, (unsigned long long)__double2ll_rn((double)v[u].z * fx_scale));
+            if (v[u].w != 0.f) atomicAdd(acc + s[u].w, (unsigned long long)__double2ll_rn((double)v[u].w * fx_scale));
+        }
     }
 }
 
