@@ -326,6 +326,52 @@ def test_device_resident_inputs_give_the_same_plan(torch_cuda, vm, tiny_phantom,
 
 
 # ------------------------------------------------------------------------------------------------
+# degenerate and extreme shapes, every step teacher-forced along the oracle's own trajectory
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kw", [
+    dict(N=1, R=1, C=1, V=5, density=0.9),                 # one beam, one row, one beamlet
+    dict(N=2, R=1, C=255, V=40, density=0.05),             # the widest row a warp scans (VMAT_MAX_COLS)
+    dict(N=9, R=3, C=7, V=130, gamma=0.0),                 # no smoothing term
+    dict(N=9, R=3, C=7, V=130, delta=0),                   # leaves may not move at all between angles
+    dict(N=6, R=2, C=9, V=700, density=0.02),              # support spans several 128-slot chunks, ragged tail
+    dict(N=40, R=2, C=5, V=64, density=0.3, gamma=5.0),    # more beams than a warp, strong smoothing
+])
+def test_edge_shapes_step_by_step(torch_cuda, vm, kw):
+    o = random_problem(77, **kw)
+    plan = make_plan(vm, o)
+    for occ, left, right, y in oracle_states(o, o.N, every=max(1, o.N // 4)):
+        check_dose(torch_cuda, plan, o, occ, left, right, y, 0)
+        check_dose(torch_cuda, plan, o, occ, left, right, y, 1)
+        z = o.dose(occ, left, right, y)
+        _, w = o.penalty(z)
+        check_prices(torch_cuda, plan, o, w, occ)
+        g32 = o.prices(w, occ).astype(np.float32)
+        check_search(torch_cuda, plan, o, occ, left, right, y, g32)
+        if occ.any():
+            check_master(plan, o, occ, left, right, np.zeros(o.N))
+    plan.destroy()
+
+
+def test_empty_dose_matrix(torch_cuda, vm):
+    # D = 0: every price is 0, every row closes at l = r' = 0, y stays 0, the cost is the constant F(z = 0)
+    from oracle import Oracle
+
+    N, R, C, V = 3, 2, 4, 10
+    rng = np.random.default_rng(1)
+    T, al, be = (rng.uniform(0.1, 1.0, V).astype(np.float32) for _ in range(3))
+    o = Oracle(np.zeros(N * R * C + 1, np.int64), np.zeros(0, np.int32), np.zeros(0, np.float32), T, al, be,
+               np.arange(N) * 2.0, R, C, 1, 0.1)
+    occ_r, left_r, right_r, y_r, z_r, tr = o.solve(N)
+    plan = vm.Plan.create(o.row_ptr, np.zeros(1, np.int32), np.zeros(1, np.float32), T, al, be, o.theta, R, C, 1, 0.1)
+    st = plan.solve(N)
+    occ, left, right, y = plan.get_plan()
+    assert st.iters == N and np.array_equal(st.beam, tr.beam)
+    assert np.array_equal(left, left_r) and np.array_equal(right, right_r) and np.all(left == right)
+    assert np.all(y == 0) and st.cost == pytest.approx(tr.cost[-1], rel=1e-6)
+    plan.destroy()
+
+
+# ------------------------------------------------------------------------------------------------
 # hard dose-rate feasibility after the last aperture
 # ------------------------------------------------------------------------------------------------
 def test_enforce_dose_rate_matches_oracle(torch_cuda, vm, tiny_oracle, tiny_solution):
