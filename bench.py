@@ -272,6 +272,8 @@ def main():
     ap.add_argument("--ref-budget-s", type=float, default=15.0, help="CPU seconds per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--master-mode", type=int, default=None, choices=[0, 1],
+                    help="inner iteration of the master kernel (vmat_options.master_mode); default: the library's")
     ap.add_argument("--sweep", action="store_true", help="configs[3]: isolated pricing / search kernel sweep")
     ap.add_argument("--sweep-nnz", default="5e7,1e8,2.5e8,5e8,1e9")
     ap.add_argument("--sweep-voxels", default="1048576,2097152,4194304")
@@ -313,6 +315,8 @@ def main():
     def create(record_phases=0):
         opt = vm.default_options()
         opt.record_phases = record_phases
+        if args.master_mode is not None:
+            opt.master_mode = args.master_mode
         return vm.Plan.create(*[t.numpy() for t in host], ph.theta_deg, c.n_rows, c.n_cols, c.max_leaf_travel, c.gamma,
                               options=opt)
 

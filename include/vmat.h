@@ -89,6 +89,11 @@ typedef struct {
                                   the decrease is below what fp32 dose arithmetic resolves        */
     int32_t master_stall_count;/* stop after this many stalls in a row (stop_reason 4)            */
     int32_t record_phases;     /* 1: vmat_solve brackets each phase with CUDA events              */
+    int32_t master_mode;       /* inner iteration of the master kernel: 0 = two passes over the columns and two
+                                  grid barriers (q = Dc^T d and the curvature, then the trial point), 1 = one
+                                  fused pass and one grid barrier (the next direction is built from the gradient
+                                  the quadratic piece predicts at the trial point; the step length and every
+                                  acceptance / stop decision use the true gradient).  Same minimiser (S11).  */
 } vmat_options;
 
 /* One deliverable aperture: a beam and one leaf pair per row. */
@@ -104,6 +109,7 @@ typedef struct {
     int32_t backtracks;     /* step halvings                                                    */
     int32_t stop_reason;    /* 0 converged, 1 iteration cap, 2 no descent, 3 line search failed,
                                4 decrease below fp32 resolution                                 */
+    int32_t passes;         /* passes over the columns, each ended by a grid barrier            */
     double  pg_entry, pg_exit;   /* max |projected gradient| at entry / exit                    */
     double  F, G, cost;     /* at exit: F, G and F + gamma G                                    */
 } vmat_master_stats;

@@ -44,7 +44,7 @@ class _Problem(C.Structure):
 class Options(C.Structure):
     _fields_ = [("validate", C.c_int32), ("pricing_kernel", C.c_int32), ("dose_path", C.c_int32),
                 ("master_eps", C.c_double), ("master_max_inner", C.c_int32), ("master_stall_rel", C.c_double),
-                ("master_stall_count", C.c_int32), ("record_phases", C.c_int32)]
+                ("master_stall_count", C.c_int32), ("record_phases", C.c_int32), ("master_mode", C.c_int32)]
 
 
 class _Aperture(C.Structure):
@@ -53,7 +53,7 @@ class _Aperture(C.Structure):
 
 class _MasterStats(C.Structure):
     _fields_ = [("inner", C.c_int32), ("backtracks", C.c_int32), ("stop_reason", C.c_int32),
-                ("pg_entry", C.c_double), ("pg_exit", C.c_double), ("F", C.c_double), ("G", C.c_double),
+                ("passes", C.c_int32), ("pg_entry", C.c_double), ("pg_exit", C.c_double), ("F", C.c_double), ("G", C.c_double),
                 ("cost", C.c_double)]
 
 
@@ -144,6 +144,7 @@ class MasterStats:
     F: float
     G: float
     cost: float
+    passes: int = 0
 
 
 @dataclass
@@ -303,7 +304,7 @@ class Plan:
     def master(self) -> MasterStats:
         s = _MasterStats()
         self._check(self._L.vmat_master(self._h, C.byref(s)))
-        return MasterStats(s.inner, s.backtracks, s.stop_reason, s.pg_entry, s.pg_exit, s.F, s.G, s.cost)
+        return MasterStats(s.inner, s.backtracks, s.stop_reason, s.pg_entry, s.pg_exit, s.F, s.G, s.cost, s.passes)
 
     def enforce_dose_rate(self, max_variation_per_deg: float, gamma_factor: float = 2.0, tol: float = 1e-6,
                           max_rounds: int = 60) -> dict:

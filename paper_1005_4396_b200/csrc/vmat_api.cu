@@ -88,6 +88,7 @@ void vmat_default_options(vmat_options *opt) {
     opt->master_stall_rel = 1e-6;    // 100x inside the 1e-4 parity tolerance on the master cost (S11)
     opt->master_stall_count = 2;
     opt->record_phases = 0;
+    opt->master_mode = 0;
 }
 
 int vmat_create(const vmat_problem *pb, const vmat_options *options, void *cuda_stream, vmat_plan **out) {
@@ -131,6 +132,7 @@ int vmat_create(const vmat_problem *pb, const vmat_options *options, void *cuda_
     if (p->opt.master_max_inner < 0) p->opt.master_max_inner = 0;
     if (!(p->opt.master_stall_rel >= 0.0)) p->opt.master_stall_rel = 1e-6;
     if (p->opt.master_stall_count < 1) p->opt.master_stall_count = 2;
+    if (p->opt.master_mode != 1) p->opt.master_mode = 0;
     p->V = pb->n_voxels;
     p->N = pb->n_beams;
     p->R = pb->n_rows;
@@ -166,6 +168,7 @@ int vmat_create(const vmat_problem *pb, const vmat_options *options, void *cuda_
     A(p->z_s, Sp);
     A(p->zn_s, Sp);
     A(p->q_s, Sp);
+    A(p->q2_s, Sp);
     A(p->w_s, Sp);
     A(p->wtmp_s, Sp);
     A(p->g, p->B);
@@ -199,6 +202,7 @@ int vmat_create(const vmat_problem *pb, const vmat_options *options, void *cuda_
     Z(p->z_s, (size_t)Sp * 4);
     Z(p->zn_s, (size_t)Sp * 4);
     Z(p->q_s, (size_t)Sp * 4);
+    Z(p->q2_s, (size_t)Sp * 4);
     Z(p->w_s, (size_t)Sp * 4);
     Z(p->wtmp_s, (size_t)Sp * 4);
     Z(p->g, (size_t)p->B * 4);
@@ -344,6 +348,7 @@ int vmat_master(vmat_plan *p, vmat_master_stats *out) {
         out->inner = h.inner;
         out->backtracks = h.backtracks;
         out->stop_reason = h.stop_reason;
+        out->passes = h.pad;
         out->pg_entry = h.pg_entry;
         out->pg_exit = h.pg_exit;
         out->F = h.F;

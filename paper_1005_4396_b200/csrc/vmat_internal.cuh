@@ -30,7 +30,7 @@ struct Sel {                          // device-side result of the beam choice (
 };
 
 struct MasterOut {                    // device-side mirror of vmat_master_stats
-    int32_t inner, backtracks, stop_reason, pad;
+    int32_t inner, backtracks, stop_reason, pad;   // pad: passes over the columns
     double pg_entry, pg_exit, F, G, cost;
 };
 
@@ -70,7 +70,7 @@ struct vmat_plan {
     double *theta = nullptr;       // N
 
     // ---- work arrays -----------------------------------------------------------------------
-    float *z_s = nullptr, *zn_s = nullptr, *q_s = nullptr, *w_s = nullptr, *wtmp_s = nullptr;  // Sp each
+    float *z_s = nullptr, *zn_s = nullptr, *q_s = nullptr, *q2_s = nullptr, *w_s = nullptr, *wtmp_s = nullptr;  // Sp each
     float *g = nullptr;            // B prices
     float *Dd = nullptr;           // N x Sp aperture-dose columns d_k (row k valid iff col_valid[k])
     unsigned long long *acc = nullptr;   // Sp fixed-point accumulator (all zero between uses)
@@ -83,7 +83,7 @@ struct vmat_plan {
     unsigned long long *beam_total = nullptr;   // N, leaf search: per-beam sums of row optima (zero between launches)
     unsigned int *beam_ticket = nullptr;        // N, leaf search: per-beam block counters (zero between launches)
 
-    long long *accbuf = nullptr;       // 3 x (N + 2) fixed-point sums of the master kernel
+    long long *accbuf = nullptr;       // 3 x (2N + 2) fixed-point sums of the master kernel
     unsigned int *phase = nullptr;     // rotation counter of accbuf, barrier epoch
     vmat::ColStat *colstat = nullptr;  // N
     unsigned int *vbounds = nullptr;   // bit patterns of max|T|, max(alpha, beta)

@@ -214,7 +214,7 @@ struct MasterArgs {
     long long Sp;
     int nchunks;
     const float *T, *alpha, *beta;
-    float *z, *zn, *q, *w;
+    float *z, *zn, *q, *q2, *w;
     const uint8_t *occ;
     double *y;
     const double *theta;
@@ -226,8 +226,9 @@ struct MasterArgs {
     int max_inner;
     int rslots;                 // > 0: every block keeps z, q, T, alpha, beta of its own slots in shared memory
     int cache_segs;             // capacity of the shared-memory tile of Dd in 512-byte segments
-    long long *accbuf;          // 3 rotating sets of kSumGroups records of (N + 2) fixed-point sums: F, curvature,
-                                // grad[0..K); a block adds to the record of its group (blockIdx mod kSumGroups)
+    long long *accbuf;          // 3 rotating sets of kSumGroups records of (2N + 2) fixed-point sums: F, curvature,
+                                // grad[0..K), and (fused mode) the Hessian-vector product [K..2K); a block adds
+                                // to the record of its group (blockIdx mod kSumGroups)
     unsigned int *phase;        // rotation counter, persists from launch to launch
     MasterOut *out;
     double *cost3;
@@ -322,13 +323,14 @@ __device__ long long g_master_prof[16];
 
 // scalars every thread of the block needs, written by warp 0 (the block's control warp)
 struct Ctl {
-    double scF, scG, scC;   // fixed-point scales of the pass about to run
-    double iF, iG, iC;      // and their inverses
+    double scF, scG, scC, scH;   // fixed-point scales of the pass about to run
+    double iF, iG, iC, iH;       // and their inverses
     float tf;               // trial step of the line search
     int state;              // what the block does next (kRunDirection, ...)
     int accepted;           // the last trial was accepted: the z buffers swap roles
+    int probe;              // fused mode: the pass about to run does not move (t = 0), it only opens a new direction
 };
-enum { kRunDirection = 0, kRunTrial = 1, kFinish = 2 };
+enum { kRunDirection = 0, kRunTrial = 1, kFinish = 2, kRunFused = 3 };
 
 constexpr int kRedSlots = 6;   // values per warp row of the control group's reduction scratch
 // Records of grid-wide sums per rotation slot.  Measured: splitting the blocks into 16 groups with one record each
@@ -364,9 +366,11 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity) {
 
 
 struct Smem {
-    double *y, *d, *grad, *pg, *yn, *gn, *dG, *rdt, *gacc, *linf;   // N each (control warp; gacc: all warps)
-    float *part, *wbuf, *coef;
-    float *rz0, *rz1, *rq, *rT, *ral, *rbe;   // resident copies of the block's own slots (a.rslots each), or unused
+    double *y, *d, *grad, *pg, *yn, *gn, *dG, *rdt, *gacc, *linf;   // N each (control warp; gacc: 4N, all warps)
+    double *gF, *gFn, *hd, *hdn, *dnx, *gm;   // fused mode, N each: F-part of the gradient, Hessian-vector products
+                                              // (accepted / pending), next direction, predicted gradient
+    float *part, *wbuf, *ubuf, *coef;
+    float *rz0, *rz1, *rq, *rq1, *rT, *ral, *rbe;   // resident copies of the block's own slots (a.rslots each), or unused
     float *tile;       // staged 512-byte segments of the block's part of Dd
     int *sk, *lo, *hi, *ik;   // lo, hi: block-local range of chunks (j of b + jG) column i touches
     int *base;         // segment (i, j) lives at tile[(base[i] + j) * 128]; kNoCache if column i is not staged
@@ -540,6 +544,122 @@ __device__ __forceinline__ void eval_pass(const MasterArgs &a, const Smem &sm, i
     PROFX(11)
 }
 
+// The pass of the single-barrier iteration (master_mode 1).  For the block's slots, in one sweep:
+//   z_new = zsrc + t qsrc (the trial point of the direction in flight; probe: z_new = zsrc), F and w there,
+//   q_new = Dc^T d_next (coef holds the next direction), the curvature sum_j omega_j q_new_j^2 of the quadratic
+//   piece at z_new, and the block's share of BOTH K-vectors Dc w_new (the true gradient at the trial point) and
+//   Dc (omega . q_new) (half the Hessian of F at z_new applied to d_next), so that one grid barrier per inner
+//   iteration suffices.  Sums go to the record `rec` in fixed point: F, curvature, grad[0..K), Hd[K..2K).
+__device__ __forceinline__ void fused_pass(const MasterArgs &a, const Smem &sm, int K, int ngroups, const float *zsrc,
+                                           float *zdst, const float *rzsrc, float *rzdst, const float *qsrc,
+                                           float *qdst, const float *rqsrc, float *rqdst, float tf, bool probe,
+                                           long long *rec, double scF, double scC, double scG, double scH,
+                                           double *red) {
+    const bool res = a.rslots > 0;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int kpart = warp & (kKSplit - 1), chalf = warp / kKSplit;
+#ifdef VMAT_MASTER_PROFILE
+    long long pt_ = 0, pacc_[16] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+#endif
+    for (int i = tid; i < 4 * a.N; i += kMasterThreads) sm.gacc[i] = 0.0;
+    double F = 0.0, curv = 0.0;
+    __syncthreads();
+    for (int g = 0; g < ngroups; ++g) {
+        float om[kOutPerThread], qv[kOutPerThread];
+#pragma unroll
+        for (int r = 0; r < kOutPerThread; ++r) {
+            const int o = tid + r * kMasterThreads, c = chunk_of(g, o >> 7);
+            float wv = 0.f, omv = 0.f;
+            if (c < a.nchunks) {
+                const size_t s = (size_t)c * kChunk + (o & (kChunk - 1));
+                const int ls = g * (kGroup * kChunk) + o;
+                float z, Tv, al, be;
+                if (res) {
+                    z = probe ? rzsrc[ls] : fmaf(tf, rqsrc[ls], rzsrc[ls]);
+                    Tv = sm.rT[ls], al = sm.ral[ls], be = sm.rbe[ls];
+                    rzdst[ls] = z;
+                } else {
+                    z = probe ? zsrc[s] : fmaf(tf, qsrc[s], zsrc[s]);
+                    Tv = a.T[s], al = a.alpha[s], be = a.beta[s];
+                    zdst[s] = z;
+                }
+                double f;
+                penalty(z, Tv, al, be, wv, f);
+                F += f;
+                omv = z < Tv ? al : (z > Tv ? be : 0.f);
+            }
+            sm.wbuf[o] = wv;
+            om[r] = omv;
+        }
+        combine_group(a, sm, K, g, qv PROF_ARG);   // its barrier also publishes wbuf
+#pragma unroll
+        for (int r = 0; r < kOutPerThread; ++r) {
+            const int o = tid + r * kMasterThreads, c = chunk_of(g, o >> 7);
+            if (c < a.nchunks) {
+                if (res) rqdst[g * (kGroup * kChunk) + o] = qv[r];
+                else qdst[(size_t)c * kChunk + (o & (kChunk - 1))] = qv[r];
+            }
+            curv += (double)om[r] * (double)qv[r] * (double)qv[r];
+            sm.ubuf[o] = om[r] * qv[r];
+        }
+        __syncthreads();
+        // this warp's half of the group (4 chunks) and its beams i = kpart, +kKSplit, ..: two beams per step, each
+        // row read once for both products; lane partials in fp32, warp sums in fp64 by one butterfly for all four
+        float4 w4[kGroup / 2], u4[kGroup / 2];
+#pragma unroll
+        for (int h = 0; h < kGroup / 2; ++h) {
+            w4[h] = reinterpret_cast<const float4 *>(sm.wbuf)[(2 * h + chalf) * 32 + lane];
+            u4[h] = reinterpret_cast<const float4 *>(sm.ubuf)[(2 * h + chalf) * 32 + lane];
+        }
+        for (int i = kpart; i < K; i += 2 * kKSplit) {
+            const bool has2 = i + kKSplit < K;
+            const int i2 = has2 ? i + kKSplit : i;
+            float4 v1[kGroup / 2], v2[kGroup / 2];
+            load_half(a, sm, i, g, chalf, lane, v1);
+            load_half(a, sm, i2, g, chalf, lane, v2);
+            float2 w1 = make_float2(0.f, 0.f), w2 = w1, u1 = w1, u2 = w1;
+#pragma unroll
+            for (int h = 0; h < kGroup / 2; ++h) {
+                w1.x = fmaf(v1[h].x, w4[h].x, fmaf(v1[h].y, w4[h].y, w1.x));
+                w1.y = fmaf(v1[h].z, w4[h].z, fmaf(v1[h].w, w4[h].w, w1.y));
+                w2.x = fmaf(v2[h].x, w4[h].x, fmaf(v2[h].y, w4[h].y, w2.x));
+                w2.y = fmaf(v2[h].z, w4[h].z, fmaf(v2[h].w, w4[h].w, w2.y));
+                u1.x = fmaf(v1[h].x, u4[h].x, fmaf(v1[h].y, u4[h].y, u1.x));
+                u1.y = fmaf(v1[h].z, u4[h].z, fmaf(v1[h].w, u4[h].w, u1.y));
+                u2.x = fmaf(v2[h].x, u4[h].x, fmaf(v2[h].y, u4[h].y, u2.x));
+                u2.y = fmaf(v2[h].z, u4[h].z, fmaf(v2[h].w, u4[h].w, u2.y));
+            }
+            const double dw1 = (double)(w1.x + w1.y), dw2 = (double)(w2.x + w2.y);
+            const double du1 = (double)(u1.x + u1.y), du2 = (double)(u2.x + u2.y);
+            // after the exchange at 16 the lower half-warp carries row 1, the upper row 2; after the exchange at 8
+            // the quarters carry (row 1, w), (row 1, u), (row 2, w), (row 2, u)
+            const bool up = lane & 16, uq = lane & 8;
+            const double rw = (up ? dw2 : dw1) + __shfl_xor_sync(kFull, up ? dw1 : dw2, 16);
+            const double ru = (up ? du2 : du1) + __shfl_xor_sync(kFull, up ? du1 : du2, 16);
+            double r = (uq ? ru : rw) + __shfl_xor_sync(kFull, uq ? rw : ru, 8);
+            r += __shfl_xor_sync(kFull, r, 4);
+            r += __shfl_xor_sync(kFull, r, 2);
+            r += __shfl_xor_sync(kFull, r, 1);
+            double *gw = sm.gacc + chalf * a.N, *gu = sm.gacc + (2 + chalf) * a.N;   // entries owned by this warp
+            if (lane == 0) gw[i] += r;
+            if (lane == 8) gu[i] += r;
+            if (lane == 16 && has2) gw[i2] += r;
+            if (lane == 24 && has2) gu[i2] += r;
+        }
+        __syncthreads();
+    }
+    F = block_sum(F, red);
+    curv = block_sum(curv, red);
+    if (tid == 0) {
+        fx_add(rec, F, scF);
+        fx_add(rec + 1, curv, scC);
+    }
+    for (int i = tid; i < K; i += kMasterThreads) {
+        fx_add(rec + 2 + i, sm.gacc[i] + sm.gacc[a.N + i], scG);
+        fx_add(rec + 2 + K + i, sm.gacc[2 * a.N + i] + sm.gacc[3 * a.N + i], scH);
+    }
+}
+
 // ---- control group: the first nw warps of a block (CT = 32 nw threads) share the N-vector work -----
 __device__ __forceinline__ void ctl_sync(int CT) { asm volatile("bar.sync 1, %0;" ::"r"(CT) : "memory"); }
 
@@ -589,17 +709,20 @@ __device__ __forceinline__ double smooth_part(const double *v, const Smem &sm, i
     return s;
 }
 
+template <int MODE>   // 0: two passes and two grid barriers per inner iteration, 1: one fused pass and one barrier
 __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a) {
     extern __shared__ float4 smem_raw[];   // 16-byte aligned: float4 tiles first, then doubles, floats, ints
     const int N = a.N, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     Smem sm;
     sm.part = reinterpret_cast<float *>(smem_raw);
     sm.wbuf = sm.part + kKSplit * kGroup * kChunk;
-    sm.tile = sm.wbuf + kGroup * kChunk;
+    sm.ubuf = sm.wbuf + kGroup * kChunk;
+    sm.tile = sm.ubuf + kGroup * kChunk;
     sm.rz0 = sm.tile + (size_t)a.cache_segs * kChunk;
     sm.rz1 = sm.rz0 + a.rslots;
     sm.rq = sm.rz1 + a.rslots;
-    sm.rT = sm.rq + a.rslots;
+    sm.rq1 = sm.rq + a.rslots;
+    sm.rT = sm.rq1 + a.rslots;
     sm.ral = sm.rT + a.rslots;
     sm.rbe = sm.ral + a.rslots;
     sm.y = reinterpret_cast<double *>(sm.rbe + a.rslots);
@@ -611,11 +734,17 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     sm.dG = sm.gn + N;
     sm.rdt = sm.dG + N;
     sm.gacc = sm.rdt + N;
-    sm.linf = sm.gacc + 2 * N;   // gacc: one row per chunk half
-    double *red = sm.linf + N;
+    sm.linf = sm.gacc + 4 * N;   // gacc: one row per chunk half (and per product in fused mode)
+    sm.gF = sm.linf + N;
+    sm.gFn = sm.gF + N;
+    sm.hd = sm.gFn + N;
+    sm.hdn = sm.hd + N;
+    sm.dnx = sm.hdn + N;
+    sm.gm = sm.dnx + N;
+    double *red = sm.gm + N;
     double *cred = red + kMasterWarps;   // 2 x kMasterWarps x kRedSlots
     sm.recv = reinterpret_cast<long long *>(cred + 2 * kMasterWarps * kRedSlots);
-    sm.ctl = reinterpret_cast<Ctl *>(sm.recv + N + 2);
+    sm.ctl = reinterpret_cast<Ctl *>(sm.recv + 2 * N + 2);
     sm.coef = reinterpret_cast<float *>(sm.ctl + 1);
     sm.sk = reinterpret_cast<int *>(sm.coef + N);
     sm.lo = sm.sk + N;
@@ -715,8 +844,9 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
 
     const int G = gridDim.x;
     const int ngroups = (a.nchunks + G * kGroup - 1) / (G * kGroup);
-    const int recn = N + 2;
+    const int recn = 2 * N + 2;
     unsigned ph = a.phase[0];      // rotation of the records; written by the previous launch, stream ordered
+    const unsigned ph_entry = ph;
     float *zcur = a.z, *znext = a.zn;
     // resident slot data: T, alpha, beta of the block's own slots are read once, z and q never leave the SM
     const bool res = a.rslots > 0;
@@ -742,10 +872,10 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     };
 
     // after the grid barrier: one round trip to L2 for the whole record, then the control warp works from smem
-    auto fetch_record = [&](const long long *rec) {
+    auto fetch_record = [&](const long long *rec, int count) {
         // sum of the group records (integers: any order gives the same bits); rec is this block's own record
         const long long *r0 = rec - (size_t)(blockIdx.x % kSumGroups) * recn;
-        for (int i = tid; i < K + 2; i += kMasterThreads) {
+        for (int i = tid; i < count; i += kMasterThreads) {
             long long v = 0;
 #pragma unroll
             for (int gq = 0; gq < kSumGroups; ++gq) v += __ldcg(r0 + (size_t)gq * recn + i);
@@ -834,6 +964,79 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
         if (tid == 0) sm.ctl->tf = (float)t;
     };
 
+    // ---- single-barrier iteration (MODE 1) ---------------------------------------------------------------
+    // State between passes: y (accepted point) with its true gradient grad = gF + gamma dG and projected gradient
+    // pg; the direction in flight d with q = Dc^T d in the current q buffer and hd = (Hessian of F at z) d; the
+    // trial step t.  make_trial_and_next sets the trial point yn = y + t d, predicts the gradient there on the
+    // quadratic piece, gm = gF + t hd + gamma dG(yn) (exact while no voxel changes sides of T_j along the step),
+    // and builds from it the NEXT direction dnx (Polak-Ribiere+ on the current face), whose q, curvature and
+    // Hessian-vector product the coming pass computes together with the true F and gradient at yn.  Directions
+    // therefore rest on a prediction, every step length, acceptance test and stop test on true values.  A probe
+    // (pr = 1) is a pass with t = 0 that opens the steepest-descent direction -pg.
+    int probe = 0;
+    auto make_trial_and_next = [&](int pr) {
+        probe = pr;
+        if (pr) {
+            t = 0.0;
+            hit = 0;
+        }
+        for (int k = tid; k < N; k += CT) {
+            const double yk = sm.y[k], dk = sm.d[k];
+            double v = pr ? yk : yk + t * dk;
+            if (!pr && (v < 0.0 || (hit && dk < 0.0 && yk / (-dk) <= tmax))) v = 0.0;
+            sm.yn[k] = v;
+        }
+        ctl_sync(CT);
+        double sg[1] = {smooth_part(sm.yn, sm, N, CT, true)}, mx = 0.0;
+        ctl_reduce<1>(sg, mx, cred, tog, nw, CT);   // its barrier also publishes dG
+        Gn = sg[0];
+        double s[3] = {0.0, 0.0, 0.0};
+        mx = 0.0;
+        for (int k = tid; k < N; k += CT) {
+            const int i = sm.ik[k];
+            const double gmk = i >= 0 ? sm.gF[k] + t * sm.hd[k] + a.gamma * sm.dG[k] : 0.0;
+            const double yk = sm.yn[k], po = sm.pg[k];
+            const double pn = (i < 0 || (yk <= 0.0 && gmk >= 0.0)) ? 0.0 : gmk;
+            sm.gm[k] = gmk;
+            sm.gn[k] = pn;   // scratch until the pass returns the true gradient
+            s[0] += pn * (pn - po);
+            s[1] += po * po;
+            s[2] += ((pn == 0.0) != (po == 0.0)) ? 1.0 : 0.0;
+        }
+        ctl_reduce<3>(s, mx, cred, tog, nw, CT);
+        const bool changed = hit || s[2] > 0.0;
+        double bpr = (pr || changed || !(s[1] > 0.0) || s[0] <= 0.0) ? 0.0 : s[0] / s[1];
+        double qbn = 0.0;
+        for (int pass = 0; pass < 2; ++pass) {
+            double s2[2] = {0.0, 0.0};
+            mx = 0.0;
+            for (int k = tid; k < N; k += CT) {
+                const double pn = sm.gn[k], yk = sm.yn[k];
+                double dk = -pn + bpr * sm.d[k];
+                if (sm.ik[k] < 0 || (yk <= 0.0 && dk < 0.0)) dk = 0.0;   // stay feasible
+                sm.dnx[k] = dk;
+                s2[0] += sm.gm[k] * dk;
+                s2[1] += fabs(dk) * sm.linf[k];
+            }
+            ctl_reduce<2>(s2, mx, cred, tog, nw, CT);
+            qbn = s2[1];
+            if (s2[0] < 0.0 || bpr == 0.0) break;
+            bpr = 0.0;   // the conjugate direction does not descend on the prediction: steepest descent
+        }
+        set_eval_scales(pr ? yb : yb + t * qb);
+        const FxScale sC = fx_scale_for(1.01 * Spd * ab * qbn * qbn, bad);
+        const FxScale sH = fx_scale_for(1.01 * ab * qbn * l1max, bad);
+        for (int i = tid; i < K; i += CT) sm.coef[i] = (float)sm.dnx[sm.sk[i]];
+        if (tid == 0) {
+            sm.ctl->scC = sC.scale;
+            sm.ctl->iC = sC.inv;
+            sm.ctl->scH = sH.scale;
+            sm.ctl->iH = sH.inv;
+            sm.ctl->tf = (float)t;
+            sm.ctl->probe = pr;
+        }
+    };
+
     PROF_DECL;
     // objective and gradient at the incoming y
     if (ctl) {
@@ -841,6 +1044,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
         for (int k = tid; k < N; k += CT) s[0] += fabs(sm.y[k]) * sm.linf[k];
         ctl_reduce<2>(s, mx, cred, tog, nw, CT);
         set_eval_scales(s[0]);
+        yb = s[0];
         Gs = s[1];
     }
     __syncthreads();
@@ -848,7 +1052,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     eval_pass<true>(a, sm, K, ngroups, nullptr, zcur, nullptr, rzcur, 0.f, rec, sm.ctl->scF, sm.ctl->scG, red PROF_ARG);
     cg::this_grid().sync();
     ++ph;
-    fetch_record(rec);
+    fetch_record(rec, K + 2);
     if (ctl) {
         const double iG = sm.ctl->iG;
         double pgl = 0.0;
@@ -857,6 +1061,8 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
             const double gk = i >= 0 ? (double)sm.recv[2 + i] * iG + a.gamma * sm.dG[k] : 0.0;
             const double p = (i < 0 || (sm.y[k] <= 0.0 && gk >= 0.0)) ? 0.0 : gk;
             sm.grad[k] = gk;
+            sm.gF[k] = i >= 0 ? (double)sm.recv[2 + i] * iG : 0.0;
+            sm.hd[k] = 0.0;
             sm.pg[k] = p;
             sm.d[k] = -p;
             pgl = fmax(pgl, fabs(p));
@@ -873,6 +1079,9 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
         else if (a.max_inner <= 0) {
             stop = 1;
             state = kFinish;
+        } else if (MODE == 1) {
+            make_trial_and_next(1);   // open the steepest-descent direction
+            state = bad ? kFinish : kRunFused;
         } else if (!prepare_direction()) state = kFinish;
         if (tid == 0) {
             sm.ctl->state = state;
@@ -881,6 +1090,118 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     }
     __syncthreads();
 
+    if constexpr (MODE == 1) {
+        float *qcur = a.q, *qnext = a.q2, *rqcur = sm.rq, *rqnext = sm.rq1;
+        while (sm.ctl->state != kFinish) {
+            rec = begin_pass();
+            fused_pass(a, sm, K, ngroups, zcur, znext, rzcur, rznext, qcur, qnext, rqcur, rqnext, sm.ctl->tf,
+                       sm.ctl->probe != 0, rec, sm.ctl->scF, sm.ctl->scC, sm.ctl->scG, sm.ctl->scH, red);
+            cg::this_grid().sync();
+            ++ph;
+            fetch_record(rec, 2 * K + 2);
+            if (ctl) {
+                // the true values at the trial point yn, and what the pass found along the next direction dnx
+                const double iG = sm.ctl->iG, iH = sm.ctl->iH;
+                const double Fn = (double)sm.recv[0] * sm.ctl->iF + a.F_out;
+                const double curvF = (double)sm.recv[1] * sm.ctl->iC;
+                double s[1] = {0.0}, pgm = 0.0;
+                for (int k = tid; k < N; k += CT) {
+                    const int i = sm.ik[k];
+                    const double gf = i >= 0 ? (double)sm.recv[2 + i] * iG : 0.0;
+                    const double gk = i >= 0 ? gf + a.gamma * sm.dG[k] : 0.0;
+                    const double yk = sm.yn[k];
+                    const double pn = (i < 0 || (yk <= 0.0 && gk >= 0.0)) ? 0.0 : gk;
+                    sm.gFn[k] = gf;
+                    sm.gn[k] = gk;
+                    sm.hdn[k] = i >= 0 ? 2.0 * (double)sm.recv[2 + K + i] * iH : 0.0;
+                    s[0] += gk * sm.d[k];
+                    pgm = fmax(pgm, fabs(pn));
+                }
+                ctl_reduce<1>(s, pgm, cred, tog, nw, CT);
+                const double Phin = Fn + a.gamma * Gn;
+                // sufficient decrease; below the resolution of Phi accept on the slope instead
+                const bool accepted = probe || Phin <= Phi + c1a * t * phi1 ||
+                                      (Phin <= Phi + noise * fabs(Phi) && fabs(s[0]) <= 0.9 * fabs(phi1));
+                int state = kRunFused;
+                if (accepted) {
+                    const int was_probe = probe;
+                    if (!was_probe) {
+                        stall = (Phi - Phin <= a.stall_rel * fabs(Phi)) ? stall + 1 : 0;
+                        F = Fn;
+                        Gs = Gn;
+                        Phi = Phin;
+                        ++inner;
+                    }
+                    pgmax = pgm;
+                    for (int k = tid; k < N; k += CT) {
+                        const double yk = sm.yn[k], gk = sm.gn[k];
+                        sm.y[k] = yk;
+                        sm.grad[k] = gk;
+                        sm.gF[k] = sm.gFn[k];
+                        sm.hd[k] = sm.hdn[k];
+                        sm.pg[k] = (sm.ik[k] < 0 || (yk <= 0.0 && gk >= 0.0)) ? 0.0 : gk;
+                        sm.d[k] = sm.dnx[k];
+                    }
+                    ctl_sync(CT);
+                    if (!(pgmax > tol)) state = kFinish;
+                    else if (stall >= a.stall_count) {
+                        stop = 4;
+                        state = kFinish;
+                    } else if (inner >= a.max_inner) {
+                        stop = 1;
+                        state = kFinish;
+                    } else {
+                        direction_sums();   // slope, bounds, G(d) and the largest feasible step of the new direction
+                        if (!(phi1 < 0.0)) {
+                            if (was_probe) {
+                                stop = 2;
+                                state = kFinish;
+                            } else make_trial_and_next(1);
+                        } else {
+                            const double phi2 = 2.0 * curvF + 2.0 * a.gamma * Gd;
+                            t = phi2 > 0.0 ? -phi1 / phi2 : (isfinite(tmax) ? tmax : 1.0);
+                            hit = 0;
+                            if (t >= tmax) {
+                                t = tmax;
+                                hit = 1;
+                            }
+                            half = 0;
+                            make_trial_and_next(0);
+                        }
+                    }
+                } else {
+                    t *= 0.5;
+                    hit = 0;
+                    ++backtracks;
+                    if (++half >= 60) {
+                        stop = 3;
+                        state = kFinish;
+                    } else make_trial_and_next(0);
+                }
+                if (bad) state = kFinish;
+                if (tid == 0) {
+                    sm.ctl->state = state;
+                    sm.ctl->accepted = accepted ? 1 : 0;
+                }
+            }
+            __syncthreads();
+            if (sm.ctl->accepted) {
+                float *tmp = zcur;
+                zcur = znext;
+                znext = tmp;
+                tmp = rzcur;
+                rzcur = rznext;
+                rznext = tmp;
+                tmp = qcur;
+                qcur = qnext;
+                qnext = tmp;
+                tmp = rqcur;
+                rqcur = rqnext;
+                rqnext = tmp;
+            }
+        }
+    }
+    if constexpr (MODE == 0)
     while (sm.ctl->state != kFinish) {
         PROF(7)
         // ---- q = Dc^T d and the curvature of the quadratic piece at t = 0 ------------------------------
@@ -918,7 +1239,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
         cg::this_grid().sync();
         PROF(1)
         ++ph;
-        fetch_record(rec);
+        fetch_record(rec, K + 2);
         if (ctl) {
             const double curvF = (double)sm.recv[1] * sm.ctl->iC;
             const double phi2 = 2.0 * curvF + 2.0 * a.gamma * Gd;
@@ -944,7 +1265,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
             cg::this_grid().sync();
             PROF(4)
             ++ph;
-            fetch_record(rec);
+            fetch_record(rec, K + 2);
             if (ctl) {
                 // gn = Dc w + gamma dG at the trial point, and the sums of the acceptance test and of the
                 // Polak-Ribiere+ update, in one sweep and one batched reduction
@@ -1050,7 +1371,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
         eval_pass<true>(a, sm, K, ngroups, nullptr, a.z, nullptr, rzcur, 0.f, rec, sm.ctl->scF, sm.ctl->scG, red PROF_ARG);
         cg::this_grid().sync();
         ++ph;
-        fetch_record(rec);
+        fetch_record(rec, K + 2);
         if (ctl) {
             F = (double)sm.recv[0] * sm.ctl->iF + a.F_out;
             Phi = F + a.gamma * Gs;
@@ -1064,7 +1385,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
             o.inner = inner;
             o.backtracks = backtracks;
             o.stop_reason = stop;
-            o.pad = 0;
+            o.pad = (int)(ph - ph_entry);
             o.pg_entry = pg_entry;
             o.pg_exit = pgmax;
             o.F = F;
@@ -1085,8 +1406,8 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
 }
 
 size_t master_smem_bytes(int64_t N, int64_t rslots, int64_t cache_segs) {
-    return (size_t)(kKSplit * kGroup * kChunk + kGroup * kChunk + 6 * rslots + cache_segs * kChunk) * 4   // part, wbuf, resident slots, tile
-           + (size_t)(12 * N + 2 + kMasterWarps + 2 * kMasterWarps * kRedSlots) * 8 + sizeof(Ctl)   // K-vectors, recv, red, cred, ctl
+    return (size_t)(kKSplit * kGroup * kChunk + 2 * kGroup * kChunk + 7 * rslots + cache_segs * kChunk) * 4   // part, wbuf, ubuf, resident slots, tile
+           + (size_t)(21 * N + 2 + kMasterWarps + 2 * kMasterWarps * kRedSlots) * 8 + sizeof(Ctl)   // K-vectors, recv, red, cred, ctl
            + (size_t)N * 4 * 6;                                              // coef, sk, lo, hi, ik
 }
 
@@ -1101,7 +1422,7 @@ int master_configure(vmat_plan *p) {
     // resident slot data (z, z trial, q, T, alpha, beta of a block's own slots) if it fits in 96 KB
     const int64_t ngroups = (nchunks + grid * kGroup - 1) / (grid * kGroup);
     int64_t rslots = ngroups * kGroup * kChunk;
-    if (rslots * 6 * 4 > 96 * 1024) rslots = 0;
+    if (rslots * 7 * 4 > 96 * 1024) rslots = 0;
     p->master_rslots = (int)rslots;
     // what is left of the SM's opt-in shared memory (minus static use and room for L1) holds the tile of Dd
     int optin = 0;
@@ -1119,16 +1440,19 @@ int master_configure(vmat_plan *p) {
     fprintf(stderr, "master: grid %d smem fixed %zu cache_segs %d rslots %d\n", p->master_grid, fixed, p->master_cache_segs, p->master_rslots);
 #endif
     p->master_smem = master_smem_bytes(p->N, p->master_rslots, p->master_cache_segs);
-    VMAT_CUDA(p, cudaFuncSetAttribute(k_master, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->master_smem));
-    int per_sm = 0;
-    VMAT_CUDA(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_master, kMasterThreads, p->master_smem));
+    VMAT_CUDA(p, cudaFuncSetAttribute(k_master<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->master_smem));
+    VMAT_CUDA(p, cudaFuncSetAttribute(k_master<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->master_smem));
+    int per_sm = 0, per_sm1 = 0;
+    VMAT_CUDA(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_master<0>, kMasterThreads, p->master_smem));
+    VMAT_CUDA(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm1, k_master<1>, kMasterThreads, p->master_smem));
+    if (per_sm1 < per_sm) per_sm = per_sm1;
     if (per_sm < 1) return fail(p, VMAT_ECUDA, "master kernel does not fit on an SM");
     int rc;
-    if ((rc = dev_alloc(p, &p->accbuf, 3 * kSumGroups * (p->N + 2)))) return rc;
+    if ((rc = dev_alloc(p, &p->accbuf, 3 * kSumGroups * (2 * p->N + 2)))) return rc;
     if ((rc = dev_alloc(p, &p->phase, 2))) return rc;
     if ((rc = dev_alloc(p, &p->colstat, p->N))) return rc;
     if ((rc = dev_alloc(p, &p->vbounds, 2))) return rc;
-    VMAT_CUDA(p, cudaMemsetAsync(p->accbuf, 0, (size_t)3 * kSumGroups * (p->N + 2) * 8, p->stream));
+    VMAT_CUDA(p, cudaMemsetAsync(p->accbuf, 0, (size_t)3 * kSumGroups * (2 * p->N + 2) * 8, p->stream));
     VMAT_CUDA(p, cudaMemsetAsync(p->phase, 0, 8, p->stream));
     VMAT_CUDA(p, cudaMemsetAsync(p->colstat, 0, (size_t)p->N * sizeof(ColStat), p->stream));
     VMAT_CUDA(p, cudaMemsetAsync(p->vbounds, 0, 8, p->stream));
@@ -1166,6 +1490,7 @@ static int launch_master_impl(vmat_plan *p, int max_inner, int trace_it) {
     a.z = p->z_s;
     a.zn = p->zn_s;
     a.q = p->q_s;
+    a.q2 = p->q2_s;
     a.w = p->w_s;
     a.occ = p->occ;
     a.y = p->y;
@@ -1193,7 +1518,8 @@ static int launch_master_impl(vmat_plan *p, int max_inner, int trace_it) {
     a.trInner = p->tr_inner;
     a.trace_it = trace_it;
     void *args[] = {&a};
-    VMAT_CUDA(p, cudaLaunchCooperativeKernel((void *)k_master, dim3((unsigned)p->master_grid), dim3(kMasterThreads), args,
+    const void *fn = p->opt.master_mode == 1 ? (const void *)k_master<1> : (const void *)k_master<0>;
+    VMAT_CUDA(p, cudaLaunchCooperativeKernel(fn, dim3((unsigned)p->master_grid), dim3(kMasterThreads), args,
                                              p->master_smem, p->stream));
     ++p->launches;
     return VMAT_OK;
