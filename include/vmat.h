@@ -143,6 +143,11 @@ void vmat_default_options(vmat_options *opt);
 int vmat_create(const vmat_problem *problem, const vmat_options *options /* NULL = defaults */,
                 void *cuda_stream, vmat_plan **out);
 int vmat_destroy(vmat_plan *plan);                      /* NULL-safe */
+
+/* Device memory of all plans comes from one stream-ordered pool per device, which keeps what vmat_destroy
+ * frees so that the next vmat_create costs no driver allocation.  vmat_release_memory returns everything the
+ * pools hold beyond live plans to the driver.  Thread-safe.                                              */
+int vmat_release_memory(void);
 int vmat_get_info(const vmat_plan *plan, vmat_info *out);
 
 /* Steps (a)+(b) for the plan's current apertures and dose rates.

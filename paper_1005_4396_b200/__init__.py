@@ -29,7 +29,7 @@ SYMBOLS = (
     "vmat_default_options", "vmat_create", "vmat_destroy", "vmat_get_info", "vmat_dose", "vmat_dose_recompute",
     "vmat_price",
     "vmat_price_spmv", "vmat_leaf_search", "vmat_master", "vmat_enforce_dose_rate", "vmat_solve", "vmat_get_plan", "vmat_set_plan",
-    "vmat_launch_count", "vmat_last_error",
+    "vmat_launch_count", "vmat_last_error", "vmat_release_memory",
 )
 
 _P = C.c_void_p
@@ -108,6 +108,7 @@ def load_library():
     L.vmat_get_plan.argtypes = [_P, _P, _P, _P, _P]
     L.vmat_set_plan.argtypes = [_P, _P, _P, _P, _P]
     L.vmat_launch_count.argtypes = [_P]
+    L.vmat_release_memory.argtypes = []
     L.vmat_launch_count.restype = C.c_int64
     L.vmat_last_error.argtypes = [_P]
     L.vmat_last_error.restype = C.c_char_p
@@ -118,6 +119,13 @@ def load_library():
         getattr(L, name).restype = C.c_int
     _lib = L
     return L
+
+
+def release_memory() -> None:
+    """vmat_release_memory: hand the device memory that destroyed plans left in the library's pools back to the driver."""
+    rc = load_library().vmat_release_memory()
+    if rc != 0:
+        raise RuntimeError(f"vmat_release_memory failed ({rc})")
 
 
 def default_options() -> Options:

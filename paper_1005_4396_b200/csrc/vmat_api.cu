@@ -3,6 +3,7 @@
 // No arithmetic of the method lives here.
 #include <cmath>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 #include "vmat_internal.cuh"
@@ -24,9 +25,55 @@ int cuda_fail(vmat_plan *p, cudaError_t e, const char *what) {
     return fail(p, VMAT_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
 }
 
+// ---- the device memory pools (one per device, created on first use) ---------------------------------------
+namespace {
+constexpr int kMaxDevices = 64;
+std::mutex g_pool_mutex;
+cudaMemPool_t g_pool[kMaxDevices];
+int g_pool_state[kMaxDevices];   // 0 not tried, 1 pool in use, -1 pools unsupported: cudaMalloc / cudaFree
+
+cudaMemPool_t pool_of(int device) {
+    if (device < 0 || device >= kMaxDevices) return nullptr;
+    std::lock_guard<std::mutex> lock(g_pool_mutex);
+    if (g_pool_state[device] == 0) {
+        g_pool_state[device] = -1;
+        int supported = 0;
+        if (cudaDeviceGetAttribute(&supported, cudaDevAttrMemoryPoolsSupported, device) == cudaSuccess && supported) {
+            cudaMemPoolProps props = {};
+            props.allocType = cudaMemAllocationTypePinned;
+            props.handleTypes = cudaMemHandleTypeNone;
+            props.location.type = cudaMemLocationTypeDevice;
+            props.location.id = device;
+            cudaMemPool_t pool;
+            if (cudaMemPoolCreate(&pool, &props) == cudaSuccess) {
+                unsigned long long keep = ~0ull;
+                cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+                g_pool[device] = pool;
+                g_pool_state[device] = 1;
+            }
+        }
+        cudaGetLastError();
+    }
+    return g_pool_state[device] == 1 ? g_pool[device] : nullptr;
+}
+}  // namespace
+
+cudaError_t pool_alloc(void **ptr, size_t bytes, int device, cudaStream_t stream) {
+    cudaMemPool_t pool = pool_of(device);
+    if (pool) return cudaMallocFromPoolAsync(ptr, bytes, pool, stream);
+    return cudaMalloc(ptr, bytes);
+}
+
+void pool_free(void *ptr, int device, cudaStream_t stream) {
+    if (!ptr) return;
+    if (pool_of(device)) cudaFreeAsync(ptr, stream);
+    else cudaFree(ptr);
+}
+
 static void free_plan(vmat_plan *p) {
     if (!p) return;
-    for (void *ptr : p->allocs) cudaFree(ptr);
+    for (void *ptr : p->allocs) pool_free(ptr, p->device, p->stream);
+    cudaStreamSynchronize(p->stream);
     delete p;
 }
 
@@ -142,11 +189,12 @@ int vmat_create(const vmat_problem *pb, const vmat_options *options, void *cuda_
     p->delta = pb->max_leaf_travel;
     p->gamma = pb->gamma;
     p->stream = (cudaStream_t)cuda_stream;
-    cudaDeviceProp prop;
-    if ((e = cudaGetDevice(&p->device)) != cudaSuccess || (e = cudaGetDeviceProperties(&prop, p->device)) != cudaSuccess)
-        return bail(cuda_fail(p, e, "cudaGetDeviceProperties"));
-    p->sm_count = prop.multiProcessorCount;
-    if (!prop.cooperativeLaunch) return bail(fail(p, VMAT_ECUDA, "device lacks cooperative launch"));
+    int coop = 0;
+    if ((e = cudaGetDevice(&p->device)) != cudaSuccess ||
+        (e = cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, p->device)) != cudaSuccess ||
+        (e = cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, p->device)) != cudaSuccess)
+        return bail(cuda_fail(p, e, "cudaDeviceGetAttribute"));
+    if (!coop) return bail(fail(p, VMAT_ECUDA, "device lacks cooperative launch"));
     if (pb->row_ptr && !(pb->col_idx && pb->val)) {
         // col_idx / val may only be NULL for an empty matrix; checked against nnz in build_layout
         if (pb->mem_space == VMAT_HOST && pb->row_ptr[p->B] != 0)
@@ -224,6 +272,16 @@ int vmat_create(const vmat_problem *pb, const vmat_options *options, void *cuda_
     p->col_valid.assign((size_t)N, 0);
     p->state_valid = false;
     *out = p;
+    return VMAT_OK;
+}
+
+int vmat_release_memory(void) {
+    std::lock_guard<std::mutex> lock(g_pool_mutex);
+    for (int d = 0; d < kMaxDevices; ++d)
+        if (g_pool_state[d] == 1 && cudaMemPoolTrimTo(g_pool[d], 0) != cudaSuccess) {
+            cudaGetLastError();
+            return VMAT_ECUDA;
+        }
     return VMAT_OK;
 }
 

@@ -137,10 +137,10 @@ static int stage_in(vmat_plan *p, const T *src, int64_t count, int mem_space, co
         return VMAT_OK;
     }
     void *d = nullptr;
-    cudaError_t e = cudaMalloc(&d, (size_t)(count > 0 ? count : 1) * sizeof(T));
+    cudaError_t e = pool_alloc(&d, (size_t)(count > 0 ? count : 1) * sizeof(T), p->device, p->stream);
     if (e != cudaSuccess) {
         cudaGetLastError();
-        return fail(p, VMAT_ENOMEM, std::string("cudaMalloc (staging) failed: ") + cudaGetErrorString(e));
+        return fail(p, VMAT_ENOMEM, std::string("device allocation (staging) failed: ") + cudaGetErrorString(e));
     }
     tmp.push_back(d);
     VMAT_CUDA(p, cudaMemcpyAsync(d, src, (size_t)count * sizeof(T), cudaMemcpyHostToDevice, p->stream));
@@ -180,10 +180,10 @@ static int build_layout_impl(vmat_plan *p, const vmat_problem *pb, std::vector<v
     int32_t *d_reach, *d_excl;
     uint32_t *d_cnt;
     auto tmp_alloc = [&](void **ptr, size_t bytes) -> int {
-        cudaError_t e = cudaMalloc(ptr, bytes ? bytes : 1);
+        cudaError_t e = pool_alloc(ptr, bytes ? bytes : 1, p->device, p->stream);
         if (e != cudaSuccess) {
             cudaGetLastError();
-            return fail(p, VMAT_ENOMEM, std::string("cudaMalloc (scratch) failed: ") + cudaGetErrorString(e));
+            return fail(p, VMAT_ENOMEM, std::string("device allocation (scratch) failed: ") + cudaGetErrorString(e));
         }
         tmp.push_back(*ptr);
         return VMAT_OK;
@@ -287,8 +287,8 @@ static int build_layout_impl(vmat_plan *p, const vmat_problem *pb, std::vector<v
 int build_layout(vmat_plan *p, const vmat_problem *pb) {
     std::vector<void *> tmp;
     const int rc = build_layout_impl(p, pb, tmp);
+    for (void *t : tmp) pool_free(t, p->device, p->stream);   // stream ordered: after the kernels that read them
     cudaStreamSynchronize(p->stream);
-    for (void *t : tmp) cudaFree(t);
     return rc;
 }
 

@@ -365,15 +365,27 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity) {
 }
 
 
+// Staged segments sit kSeg floats apart (128 used): with 544-byte strides two threads per segment, reading
+// alternate float4s, touch eight distinct 16-byte bank groups per quarter warp, so the thread-per-segment
+// gradient products below run free of bank conflicts.  The w / u buffers of a group use the same stride.
+constexpr int kSeg = 136;
+constexpr int kSeg4 = kSeg / 4;
+static_assert(kMasterWarps == 2 * kGroup, "the staged products give every chunk of a group two warps");
+
 struct Smem {
     double *y, *d, *grad, *pg, *yn, *gn, *dG, *rdt, *gacc, *linf;   // N each (control warp; gacc: 4N, all warps)
     double *gF, *gFn, *hd, *hdn, *dnx, *gm;   // fused mode, N each: F-part of the gradient, Hessian-vector products
                                               // (accepted / pending), next direction, predicted gradient
-    float *part, *wbuf, *ubuf, *coef;
+    double *gpart, *gpartu;   // 2 per staged segment: partial dots of its two threads with w (and, fused mode, u)
+    float *part2, *wbuf, *ubuf, *coef;
     float *rz0, *rz1, *rq, *rq1, *rT, *ral, *rbe;   // resident copies of the block's own slots (a.rslots each), or unused
-    float *tile;       // staged 512-byte segments of the block's part of Dd
+    float *tile;       // staged 512-byte segments of the block's part of Dd, kSeg floats apart
     int *sk, *lo, *hi, *ik;   // lo, hi: block-local range of chunks (j of b + jG) column i touches
-    int *base;         // segment (i, j) lives at tile[(base[i] + j) * 128]; kNoCache if column i is not staged
+    int *base;         // segment (i, j) is number base[i] + j of the tile; kNoCache if column i is not staged
+    int *coff;         // ngroups*kGroup + 1: entries [coff[j], coff[j+1]) of cseg belong to local chunk j
+    int *cseg;         // staged segments chunk by chunk, beams ascending: segment | i << 16
+    int *gseg;         // staged segments group by group, beams ascending, then chunks: segment | (j - g kGroup) << 16
+    int *unc;          // beams that touch this block's chunks but are not staged, ascending
     long long *recv;   // the pass's record of grid sums, fetched by the whole block after the barrier
     Ctl *ctl;
 };
@@ -381,69 +393,155 @@ struct Smem {
 // chunk handled by this block as member `ch` of its group `g`: chunks are dealt round-robin
 __device__ __forceinline__ int chunk_of(int g, int ch) { return (int)blockIdx.x + (g * kGroup + ch) * (int)gridDim.x; }
 
-// The four chunks (j = g*kGroup + chalf + 2h, h = 0..3) of column i that this warp's half of the group covers:
-// v[h] = the lane's float4 of segment h, zero where the column does not touch the chunk.  Staged columns are
-// read from the shared-memory tile, the others from L2 / HBM; either way the four loads are independent.
+// Columns that are NOT staged.  The four chunks (j = g*kGroup + chalf + 2h, h = 0..3) of column i that this
+// warp's half of the group covers: v[h] = the lane's float4 of segment h, zero where the column does not touch
+// the chunk; the four loads from L2 / HBM are independent.
 __device__ __forceinline__ void load_half(const MasterArgs &a, const Smem &sm, int i, int g, int chalf, int lane,
                                           float4 (&v)[kGroup / 2]) {
     const int lb = max(sm.lo[i] - g * kGroup, 0), hb = min(sm.hi[i] - g * kGroup, kGroup - 1);
     const unsigned m = hb >= lb ? (((2u << hb) - 1u) & ~((1u << lb) - 1u)) >> chalf : 0u;
-    const int bs = sm.base[i], j0 = g * kGroup + chalf;
-    if (bs != kNoCache) {
-        const float4 *t = reinterpret_cast<const float4 *>(sm.tile) + (bs + j0) * 32 + lane;
+    const int j0 = g * kGroup + chalf, G = (int)gridDim.x;
+    const float4 *row = reinterpret_cast<const float4 *>(a.Dd + (size_t)sm.sk[i] * a.Sp) +
+                        (size_t)((int)blockIdx.x + j0 * G) * (kChunk / 4) + lane;
 #pragma unroll
-        for (int h = 0; h < kGroup / 2; ++h)
-            v[h] = (m >> (2 * h)) & 1u ? t[2 * h * 32] : make_float4(0.f, 0.f, 0.f, 0.f);
-    } else {
-        const int G = (int)gridDim.x;
-        const float4 *row = reinterpret_cast<const float4 *>(a.Dd + (size_t)sm.sk[i] * a.Sp) +
-                            (size_t)((int)blockIdx.x + j0 * G) * (kChunk / 4) + lane;
-#pragma unroll
-        for (int h = 0; h < kGroup / 2; ++h)
-            v[h] = (m >> (2 * h)) & 1u ? __ldg(row + (size_t)(2 * h * G) * (kChunk / 4)) : make_float4(0.f, 0.f, 0.f, 0.f);
-    }
+    for (int h = 0; h < kGroup / 2; ++h)
+        v[h] = (m >> (2 * h)) & 1u ? __ldg(row + (size_t)(2 * h * G) * (kChunk / 4)) : make_float4(0.f, 0.f, 0.f, 0.f);
 }
 
 // value[o] = sum_i coef[i] * Dd[sk[i]][slot(o)] for the kGroup*128 slots of group g, o = tid + r*kMasterThreads.
-// Warp w takes the beams i = (w mod kKSplit), +kKSplit, .. and every second chunk of the group (even chunks
-// for w < kKSplit, odd ones above), two beams per step so that eight loads are in flight; partials meet in
-// shared memory and are added in a fixed order.  The caller must __syncthreads() before sm.part is written again.
-__device__ __forceinline__ void combine_group(const MasterArgs &a, const Smem &sm, int K, int g,
+// Staged columns: the two warps of a chunk walk its list of staged segments (every second entry each, beams
+// ascending), one float4 of the segment per lane: only segments the columns really touch are visited; the
+// columns that are not staged (Ku of them) follow by the same split.  The two partials of a chunk meet in
+// shared memory.  The caller must __syncthreads() before sm.part2 is written again.
+__device__ __forceinline__ void combine_group(const MasterArgs &a, const Smem &sm, int Ku, int g,
                                               float (&out)[kOutPerThread] PROF_PARAM) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int kpart = warp & (kKSplit - 1), chalf = warp / kKSplit;
-    float4 acc[kGroup / 2];
     PROFX_START
-#pragma unroll
-    for (int h = 0; h < kGroup / 2; ++h) acc[h] = make_float4(0.f, 0.f, 0.f, 0.f);
-    for (int i = kpart; i < K; i += 2 * kKSplit) {
-        const int i2 = i + kKSplit < K ? i + kKSplit : i;
-        const float c1 = sm.coef[i], c2 = i + kKSplit < K ? sm.coef[i2] : 0.f;
-        float4 v1[kGroup / 2], v2[kGroup / 2];
-        load_half(a, sm, i, g, chalf, lane, v1);
-        load_half(a, sm, i2, g, chalf, lane, v2);
-#pragma unroll
-        for (int h = 0; h < kGroup / 2; ++h) {
-            acc[h].x = fmaf(c2, v2[h].x, fmaf(c1, v1[h].x, acc[h].x));
-            acc[h].y = fmaf(c2, v2[h].y, fmaf(c1, v1[h].y, acc[h].y));
-            acc[h].z = fmaf(c2, v2[h].z, fmaf(c1, v1[h].z, acc[h].z));
-            acc[h].w = fmaf(c2, v2[h].w, fmaf(c1, v1[h].w, acc[h].w));
+    {
+        const int cs = warp & (kGroup - 1), hf = warp / kGroup;
+        const int n1 = sm.coff[g * kGroup + cs + 1];
+        int n = sm.coff[g * kGroup + cs] + hf;
+        const float4 *tile4 = reinterpret_cast<const float4 *>(sm.tile) + lane;
+        float4 s1 = make_float4(0.f, 0.f, 0.f, 0.f), s2 = s1;
+        for (; n + 2 < n1; n += 4) {
+            const int e1 = sm.cseg[n], e2 = sm.cseg[n + 2];
+            const float c1 = sm.coef[e1 >> 16], c2 = sm.coef[e2 >> 16];
+            const float4 v1 = tile4[(e1 & 0xffff) * kSeg4], v2 = tile4[(e2 & 0xffff) * kSeg4];
+            s1.x = fmaf(c1, v1.x, s1.x);
+            s1.y = fmaf(c1, v1.y, s1.y);
+            s1.z = fmaf(c1, v1.z, s1.z);
+            s1.w = fmaf(c1, v1.w, s1.w);
+            s2.x = fmaf(c2, v2.x, s2.x);
+            s2.y = fmaf(c2, v2.y, s2.y);
+            s2.z = fmaf(c2, v2.z, s2.z);
+            s2.w = fmaf(c2, v2.w, s2.w);
         }
+        if (n < n1) {
+            const int e1 = sm.cseg[n];
+            const float c1 = sm.coef[e1 >> 16];
+            const float4 v1 = tile4[(e1 & 0xffff) * kSeg4];
+            s1.x = fmaf(c1, v1.x, s1.x);
+            s1.y = fmaf(c1, v1.y, s1.y);
+            s1.z = fmaf(c1, v1.z, s1.z);
+            s1.w = fmaf(c1, v1.w, s1.w);
+        }
+        if (Ku > 0) {
+            // columns that are not staged: same split, four beams per step, one float4 of the chunk per lane
+            // straight from L2 / HBM; a beam that does not touch the chunk is skipped (warp-uniform test)
+            const int j = g * kGroup + cs;
+            const float4 *Dd4 = reinterpret_cast<const float4 *>(a.Dd) +
+                                (size_t)((int)blockIdx.x + j * (int)gridDim.x) * (kChunk / 4) + lane;
+            const size_t row4 = (size_t)a.Sp / 4;
+            for (int u = hf; u < Ku; u += 8) {
+                float4 v[4];
+                float c[4];
+#pragma unroll
+                for (int x = 0; x < 4; ++x) {
+                    const int uu = u + 2 * x;
+                    c[x] = 0.f;
+                    v[x] = make_float4(0.f, 0.f, 0.f, 0.f);
+                    if (uu < Ku) {
+                        const int i = sm.unc[uu];
+                        if (sm.lo[i] <= j && j <= sm.hi[i]) {
+                            c[x] = sm.coef[i];
+                            v[x] = __ldg(Dd4 + (size_t)sm.sk[i] * row4);
+                        }
+                    }
+                }
+#pragma unroll
+                for (int x = 0; x < 4; x += 2) {
+                    s1.x = fmaf(c[x], v[x].x, s1.x);
+                    s1.y = fmaf(c[x], v[x].y, s1.y);
+                    s1.z = fmaf(c[x], v[x].z, s1.z);
+                    s1.w = fmaf(c[x], v[x].w, s1.w);
+                    s2.x = fmaf(c[x + 1], v[x + 1].x, s2.x);
+                    s2.y = fmaf(c[x + 1], v[x + 1].y, s2.y);
+                    s2.z = fmaf(c[x + 1], v[x + 1].z, s2.z);
+                    s2.w = fmaf(c[x + 1], v[x + 1].w, s2.w);
+                }
+            }
+        }
+        reinterpret_cast<float4 *>(sm.part2)[(hf * kGroup + cs) * 32 + lane] =
+            make_float4(s1.x + s2.x, s1.y + s2.y, s1.z + s2.z, s1.w + s2.w);
     }
     PROFX(12)
-#pragma unroll
-    for (int h = 0; h < kGroup / 2; ++h)
-        reinterpret_cast<float4 *>(sm.part)[(kpart * kGroup + 2 * h + chalf) * 32 + lane] = acc[h];
     __syncthreads();
 #pragma unroll
     for (int r = 0; r < kOutPerThread; ++r) {
         const int o = tid + r * kMasterThreads, ch = o >> 7, s = o & (kChunk - 1);
-        float v = 0.f;
-#pragma unroll
-        for (int kp = 0; kp < kKSplit; ++kp) v += sm.part[(kp * kGroup + ch) * kChunk + s];
-        out[r] = v;
+        out[r] = sm.part2[ch * kChunk + s] + sm.part2[(kGroup + ch) * kChunk + s];
     }
     PROFX(13)
+}
+
+// Gradient products of the staged segments of group g: two threads per segment (alternate float4s), each a plain
+// dot of 64 entries with the group's w (TWO: and u) — no exchange between lanes.  Lane partials over 16 products
+// in fp32, then fp64.  The partials land in sm.gpart (sm.gpartu), two per segment; grad_total adds them per beam.
+template <bool TWO>
+__device__ __forceinline__ void grad_staged(const Smem &sm, int g) {
+    const int n0 = sm.coff[g * kGroup], n2 = 2 * (sm.coff[(g + 1) * kGroup] - n0);
+    const float4 *tile4 = reinterpret_cast<const float4 *>(sm.tile);
+    const float4 *wb4 = reinterpret_cast<const float4 *>(sm.wbuf), *ub4 = reinterpret_cast<const float4 *>(sm.ubuf);
+    for (int t2 = threadIdx.x; t2 < n2; t2 += kMasterThreads) {
+        const int e = sm.gseg[n0 + (t2 >> 1)], hfs = t2 & 1;
+        const int s = e & 0xffff, cs = e >> 16;
+        const float4 *tp = tile4 + s * kSeg4 + hfs, *wp = wb4 + cs * kSeg4 + hfs, *up = ub4 + cs * kSeg4 + hfs;
+        double dw = 0.0, du = 0.0;
+#pragma unroll
+        for (int blk = 0; blk < 4; ++blk) {
+            float4 aw = make_float4(0.f, 0.f, 0.f, 0.f), au = aw;
+#pragma unroll
+            for (int it = 0; it < 4; ++it) {
+                const int x = (blk * 4 + it) * 2;
+                const float4 v = tp[x], w = wp[x];
+                aw.x = fmaf(v.x, w.x, aw.x);
+                aw.y = fmaf(v.y, w.y, aw.y);
+                aw.z = fmaf(v.z, w.z, aw.z);
+                aw.w = fmaf(v.w, w.w, aw.w);
+                if (TWO) {
+                    const float4 u = up[x];
+                    au.x = fmaf(v.x, u.x, au.x);
+                    au.y = fmaf(v.y, u.y, au.y);
+                    au.z = fmaf(v.z, u.z, au.z);
+                    au.w = fmaf(v.w, u.w, au.w);
+                }
+            }
+            dw += (double)((aw.x + aw.y) + (aw.z + aw.w));
+            if (TWO) du += (double)((au.x + au.y) + (au.z + au.w));
+        }
+        sm.gpart[2 * s + hfs] = dw;
+        if (TWO) sm.gpartu[2 * s + hfs] = du;
+    }
+}
+
+// beam i's total over the block: staged columns add the partials of their segments in chunk order, the others
+// the two chunk-half rows of sm.gacc (row0, row0 + 1)
+__device__ __forceinline__ double grad_total(const Smem &sm, const double *gp, int i, int N, int row0) {
+    const int bs = sm.base[i];
+    if (bs == kNoCache) return sm.gacc[row0 * N + i] + sm.gacc[(row0 + 1) * N + i];
+    double s = 0.0;
+    for (int j = sm.lo[i]; j <= sm.hi[i]; ++j) s += gp[2 * (bs + j)] + gp[2 * (bs + j) + 1];
+    return s;
 }
 
 __device__ __forceinline__ void penalty(float z, float T, float al, float be, float &w, double &F) {
@@ -458,7 +556,7 @@ __device__ __forceinline__ void penalty(float z, float T, float al, float be, fl
 // and in the same pass F and the block's share of grad = Dc w_new, both added to the record `rec`
 // in fixed point (scales scF, scG).
 template <bool FROM_Y>
-__device__ __forceinline__ void eval_pass(const MasterArgs &a, const Smem &sm, int K, int ngroups, const float *zsrc,
+__device__ __forceinline__ void eval_pass(const MasterArgs &a, const Smem &sm, int K, int Ku, int ngroups, const float *zsrc,
                                           float *zdst, const float *rzsrc, float *rzdst, float tf, long long *rec,
                                           double scF, double scG, double *red PROF_PARAM) {
     const bool res = a.rslots > 0;
@@ -471,7 +569,7 @@ __device__ __forceinline__ void eval_pass(const MasterArgs &a, const Smem &sm, i
     PROFX(8)
     for (int g = 0; g < ngroups; ++g) {
         float zv[kOutPerThread];
-        if (FROM_Y) combine_group(a, sm, K, g, zv PROF_ARG);
+        if (FROM_Y) combine_group(a, sm, Ku, g, zv PROF_ARG);
 #pragma unroll
         for (int r = 0; r < kOutPerThread; ++r) {
             const int o = tid + r * kMasterThreads, c = chunk_of(g, o >> 7);
@@ -494,19 +592,21 @@ __device__ __forceinline__ void eval_pass(const MasterArgs &a, const Smem &sm, i
                 if (FROM_Y || !res) zdst[s] = z;   // evaluations from y publish z and w
                 if (FROM_Y) a.w[s] = wv;
             }
-            sm.wbuf[o] = wv;
+            sm.wbuf[(o >> 7) * kSeg + (o & (kChunk - 1))] = wv;
         }
         __syncthreads();
         PROFX(9)
-        // this warp's half of the group's gradient (4 chunks), and its beams i = kpart, +kKSplit, ..: two beams
+        grad_staged<false>(sm, g);
+        // columns that are not staged: this warp's half of the group's gradient (4 chunks), and its share of those beams: two beams
         // per step (eight independent loads), lane partials in fp32 (16 products), the warp sum in fp64; the
         // partial dot goes to the row of sm.gacc that belongs to this chunk half
+        if (Ku > 0) {
         float4 w4[kGroup / 2];
 #pragma unroll
-        for (int h = 0; h < kGroup / 2; ++h) w4[h] = reinterpret_cast<const float4 *>(sm.wbuf)[(2 * h + chalf) * 32 + lane];
-        for (int i = kpart; i < K; i += 2 * kKSplit) {
-            const bool has2 = i + kKSplit < K;
-            const int i2 = has2 ? i + kKSplit : i;
+        for (int h = 0; h < kGroup / 2; ++h) w4[h] = reinterpret_cast<const float4 *>(sm.wbuf)[(2 * h + chalf) * kSeg4 + lane];
+        for (int u = kpart; u < Ku; u += 2 * kKSplit) {
+            const bool has2 = u + kKSplit < Ku;
+            const int i = sm.unc[u], i2 = has2 ? sm.unc[u + kKSplit] : i;
             float4 v1[kGroup / 2], v2[kGroup / 2];
             load_half(a, sm, i, g, chalf, lane, v1);
             load_half(a, sm, i2, g, chalf, lane, v2);
@@ -534,13 +634,14 @@ __device__ __forceinline__ void eval_pass(const MasterArgs &a, const Smem &sm, i
             if (lane == 0) gacc[i] += r;
             if (lane == 16 && has2) gacc[i2] += r;
         }
+        }
         PROFX(10)
         __syncthreads();
     }
     PROFX(11)
     F = block_sum(F, red);
     if (tid == 0) fx_add(rec, F, scF);
-    for (int i = tid; i < K; i += kMasterThreads) fx_add(rec + 2 + i, sm.gacc[i] + sm.gacc[a.N + i], scG);
+    for (int i = tid; i < K; i += kMasterThreads) fx_add(rec + 2 + i, grad_total(sm, sm.gpart, i, a.N, 0), scG);
     PROFX(11)
 }
 
@@ -550,7 +651,7 @@ __device__ __forceinline__ void eval_pass(const MasterArgs &a, const Smem &sm, i
 //   piece at z_new, and the block's share of BOTH K-vectors Dc w_new (the true gradient at the trial point) and
 //   Dc (omega . q_new) (half the Hessian of F at z_new applied to d_next), so that one grid barrier per inner
 //   iteration suffices.  Sums go to the record `rec` in fixed point: F, curvature, grad[0..K), Hd[K..2K).
-__device__ __forceinline__ void fused_pass(const MasterArgs &a, const Smem &sm, int K, int ngroups, const float *zsrc,
+__device__ __forceinline__ void fused_pass(const MasterArgs &a, const Smem &sm, int K, int Ku, int ngroups, const float *zsrc,
                                            float *zdst, const float *rzsrc, float *rzdst, const float *qsrc,
                                            float *qdst, const float *rqsrc, float *rqdst, float tf, bool probe,
                                            long long *rec, double scF, double scC, double scG, double scH,
@@ -588,10 +689,10 @@ __device__ __forceinline__ void fused_pass(const MasterArgs &a, const Smem &sm, 
                 F += f;
                 omv = z < Tv ? al : (z > Tv ? be : 0.f);
             }
-            sm.wbuf[o] = wv;
+            sm.wbuf[(o >> 7) * kSeg + (o & (kChunk - 1))] = wv;
             om[r] = omv;
         }
-        combine_group(a, sm, K, g, qv PROF_ARG);   // its barrier also publishes wbuf
+        combine_group(a, sm, Ku, g, qv PROF_ARG);   // its barrier also publishes wbuf
 #pragma unroll
         for (int r = 0; r < kOutPerThread; ++r) {
             const int o = tid + r * kMasterThreads, c = chunk_of(g, o >> 7);
@@ -600,20 +701,22 @@ __device__ __forceinline__ void fused_pass(const MasterArgs &a, const Smem &sm, 
                 else qdst[(size_t)c * kChunk + (o & (kChunk - 1))] = qv[r];
             }
             curv += (double)om[r] * (double)qv[r] * (double)qv[r];
-            sm.ubuf[o] = om[r] * qv[r];
+            sm.ubuf[(o >> 7) * kSeg + (o & (kChunk - 1))] = om[r] * qv[r];
         }
         __syncthreads();
-        // this warp's half of the group (4 chunks) and its beams i = kpart, +kKSplit, ..: two beams per step, each
+        grad_staged<true>(sm, g);
+        // columns that are not staged: this warp's half of the group (4 chunks) and its share of those beams: two beams per step, each
         // row read once for both products; lane partials in fp32, warp sums in fp64 by one butterfly for all four
+        if (Ku > 0) {
         float4 w4[kGroup / 2], u4[kGroup / 2];
 #pragma unroll
         for (int h = 0; h < kGroup / 2; ++h) {
-            w4[h] = reinterpret_cast<const float4 *>(sm.wbuf)[(2 * h + chalf) * 32 + lane];
-            u4[h] = reinterpret_cast<const float4 *>(sm.ubuf)[(2 * h + chalf) * 32 + lane];
+            w4[h] = reinterpret_cast<const float4 *>(sm.wbuf)[(2 * h + chalf) * kSeg4 + lane];
+            u4[h] = reinterpret_cast<const float4 *>(sm.ubuf)[(2 * h + chalf) * kSeg4 + lane];
         }
-        for (int i = kpart; i < K; i += 2 * kKSplit) {
-            const bool has2 = i + kKSplit < K;
-            const int i2 = has2 ? i + kKSplit : i;
+        for (int u = kpart; u < Ku; u += 2 * kKSplit) {
+            const bool has2 = u + kKSplit < Ku;
+            const int i = sm.unc[u], i2 = has2 ? sm.unc[u + kKSplit] : i;
             float4 v1[kGroup / 2], v2[kGroup / 2];
             load_half(a, sm, i, g, chalf, lane, v1);
             load_half(a, sm, i2, g, chalf, lane, v2);
@@ -646,6 +749,7 @@ __device__ __forceinline__ void fused_pass(const MasterArgs &a, const Smem &sm, 
             if (lane == 16 && has2) gw[i2] += r;
             if (lane == 24 && has2) gu[i2] += r;
         }
+        }
         __syncthreads();
     }
     F = block_sum(F, red);
@@ -655,8 +759,8 @@ __device__ __forceinline__ void fused_pass(const MasterArgs &a, const Smem &sm, 
         fx_add(rec + 1, curv, scC);
     }
     for (int i = tid; i < K; i += kMasterThreads) {
-        fx_add(rec + 2 + i, sm.gacc[i] + sm.gacc[a.N + i], scG);
-        fx_add(rec + 2 + K + i, sm.gacc[2 * a.N + i] + sm.gacc[3 * a.N + i], scH);
+        fx_add(rec + 2 + i, grad_total(sm, sm.gpart, i, a.N, 0), scG);
+        fx_add(rec + 2 + K + i, grad_total(sm, sm.gpartu, i, a.N, 2), scH);
     }
 }
 
@@ -714,15 +818,16 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     extern __shared__ float4 smem_raw[];   // 16-byte aligned: float4 tiles first, then doubles, floats, ints
     const int N = a.N, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     Smem sm;
-    sm.part = reinterpret_cast<float *>(smem_raw);
-    sm.wbuf = sm.part + kKSplit * kGroup * kChunk;
-    sm.ubuf = sm.wbuf + kGroup * kChunk;
-    sm.tile = sm.ubuf + kGroup * kChunk;
-    sm.rz0 = sm.tile + (size_t)a.cache_segs * kChunk;
+    constexpr int F1 = MODE == 1 ? 1 : 0;   // what only the single-barrier iteration needs is not laid out in mode 0
+    sm.part2 = reinterpret_cast<float *>(smem_raw);
+    sm.wbuf = sm.part2 + 2 * kGroup * kChunk;
+    sm.ubuf = sm.wbuf + kGroup * kSeg;
+    sm.tile = sm.ubuf + F1 * kGroup * kSeg;
+    sm.rz0 = sm.tile + (size_t)a.cache_segs * kSeg;
     sm.rz1 = sm.rz0 + a.rslots;
     sm.rq = sm.rz1 + a.rslots;
     sm.rq1 = sm.rq + a.rslots;
-    sm.rT = sm.rq1 + a.rslots;
+    sm.rT = sm.rq1 + F1 * a.rslots;
     sm.ral = sm.rT + a.rslots;
     sm.rbe = sm.ral + a.rslots;
     sm.y = reinterpret_cast<double *>(sm.rbe + a.rslots);
@@ -734,14 +839,16 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     sm.dG = sm.gn + N;
     sm.rdt = sm.dG + N;
     sm.gacc = sm.rdt + N;
-    sm.linf = sm.gacc + 4 * N;   // gacc: one row per chunk half (and per product in fused mode)
+    sm.linf = sm.gacc + (2 + 2 * F1) * N;   // gacc: one row per chunk half (and per product in fused mode)
     sm.gF = sm.linf + N;
-    sm.gFn = sm.gF + N;
-    sm.hd = sm.gFn + N;
-    sm.hdn = sm.hd + N;
-    sm.dnx = sm.hdn + N;
-    sm.gm = sm.dnx + N;
-    double *red = sm.gm + N;
+    sm.gFn = sm.gF + F1 * N;
+    sm.hd = sm.gFn + F1 * N;
+    sm.hdn = sm.hd + F1 * N;
+    sm.dnx = sm.hdn + F1 * N;
+    sm.gm = sm.dnx + F1 * N;
+    sm.gpart = sm.gm + F1 * N;
+    sm.gpartu = sm.gpart + 2 * a.cache_segs;
+    double *red = sm.gpartu + F1 * 2 * a.cache_segs;
     double *cred = red + kMasterWarps;   // 2 x kMasterWarps x kRedSlots
     sm.recv = reinterpret_cast<long long *>(cred + 2 * kMasterWarps * kRedSlots);
     sm.ctl = reinterpret_cast<Ctl *>(sm.recv + 2 * N + 2);
@@ -751,7 +858,12 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     sm.hi = sm.lo + N;
     sm.ik = sm.hi + N;
     sm.base = sm.ik + N;
-    __shared__ int sK;
+    sm.unc = sm.base + N;
+    sm.cseg = sm.unc + N;
+    sm.gseg = sm.cseg + a.cache_segs;
+    sm.coff = sm.gseg + a.cache_segs;   // ngroups * kGroup + 1
+    const int ngroups = (a.nchunks + (int)gridDim.x * kGroup - 1) / ((int)gridDim.x * kGroup);
+    __shared__ int sK, sKu;
     __shared__ uint64_t tile_bar;
 
     // occupied beams in ascending order
@@ -834,16 +946,86 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
                 const int j0 = sm.lo[i], j1 = sm.hi[i];
                 const float *src = a.Dd + (size_t)sm.sk[i] * a.Sp;
                 for (int j = j0; j <= j1; ++j)
-                    bulk_g2s(sm.tile + (size_t)(bs + j) * kChunk, src + (size_t)(b + j * G) * kChunk, kChunk * 4, &tile_bar);
+                    bulk_g2s(sm.tile + (size_t)(bs + j) * kSeg, src + (size_t)(b + j * G) * kChunk, kChunk * 4, &tile_bar);
             }
         }
         __syncthreads();          // sm.base visible to all warps
-        mbar_wait(&tile_bar, 0);  // the staged segments have landed
     }
+    // ---- lists over the staged segments, built once per solve in a fixed order (reproducible sums) ----
+    const int nj = ngroups * kGroup;
+    if (warp == 1) {   // beams that touch this block's chunks but are not staged, ascending
+        int run = 0;
+        for (int i0 = 0; i0 < K; i0 += 32) {
+            const int i = i0 + lane;
+            const bool f = i < K && sm.base[i] == kNoCache && sm.hi[i] >= sm.lo[i];
+            const unsigned m = __ballot_sync(kFull, f);
+            if (f) sm.unc[run + __popc(m & ((1u << lane) - 1u))] = i;
+            run += __popc(m);
+        }
+        if (lane == 0) sKu = run;
+    }
+    for (int j = warp; j < nj; j += kMasterWarps) {   // staged segments per local chunk
+        int c = 0;
+        for (int i0 = 0; i0 < K; i0 += 32) {
+            const int i = i0 + lane;
+            const bool f = i < K && sm.base[i] != kNoCache && sm.lo[i] <= j && j <= sm.hi[i];
+            c += __popc(__ballot_sync(kFull, f));
+        }
+        if (lane == 0) sm.coff[j + 1] = c;
+    }
+    __syncthreads();
+    if (warp == 0) {   // running sums: coff[j] = first entry of chunk j
+        int run = 0;
+        for (int j0 = 0; j0 < nj; j0 += 32) {
+            const int j = j0 + lane;
+            int incl = j < nj ? sm.coff[j + 1] : 0;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int n = __shfl_up_sync(kFull, incl, o);
+                if (lane >= o) incl += n;
+            }
+            if (j < nj) sm.coff[j + 1] = run + incl;
+            run += __shfl_sync(kFull, incl, 31);
+        }
+        if (lane == 0) sm.coff[0] = 0;
+    }
+    __syncthreads();
+    for (int j = warp; j < nj; j += kMasterWarps) {   // chunk by chunk, beams ascending
+        int pos = sm.coff[j];
+        for (int i0 = 0; i0 < K; i0 += 32) {
+            const int i = i0 + lane;
+            const bool f = i < K && sm.base[i] != kNoCache && sm.lo[i] <= j && j <= sm.hi[i];
+            const unsigned m = __ballot_sync(kFull, f);
+            if (f) sm.cseg[pos + __popc(m & ((1u << lane) - 1u))] = (sm.base[i] + j) | (i << 16);
+            pos += __popc(m);
+        }
+    }
+    for (int g = warp; g < ngroups; g += kMasterWarps) {   // group by group, beams ascending, then chunks
+        int pos = sm.coff[g * kGroup];
+        for (int i0 = 0; i0 < K; i0 += 32) {
+            const int i = i0 + lane;
+            int ja = 0, cnt = 0;
+            if (i < K && sm.base[i] != kNoCache) {
+                ja = max(sm.lo[i], g * kGroup);
+                cnt = max(min(sm.hi[i], g * kGroup + kGroup - 1) - ja + 1, 0);
+            }
+            int incl = cnt;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int n = __shfl_up_sync(kFull, incl, o);
+                if (lane >= o) incl += n;
+            }
+            const int at = pos + incl - cnt;
+            for (int q = 0; q < cnt; ++q) sm.gseg[at + q] = (sm.base[i] + ja + q) | ((ja + q - g * kGroup) << 16);
+            pos += __shfl_sync(kFull, incl, 31);
+        }
+    }
+    __syncthreads();
+    const int Ku = sKu;
+    mbar_wait(&tile_bar, 0);  // the staged segments have landed (the lists were built while they were in flight)
     const double Tm = (double)a.Tmax, ab = (double)a.abmax, Spd = (double)a.Sp;
 
     const int G = gridDim.x;
-    const int ngroups = (a.nchunks + G * kGroup - 1) / (G * kGroup);
     const int recn = 2 * N + 2;
     unsigned ph = a.phase[0];      // rotation of the records; written by the previous launch, stream ordered
     const unsigned ph_entry = ph;
@@ -1049,7 +1231,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     }
     __syncthreads();
     long long *rec = begin_pass();
-    eval_pass<true>(a, sm, K, ngroups, nullptr, zcur, nullptr, rzcur, 0.f, rec, sm.ctl->scF, sm.ctl->scG, red PROF_ARG);
+    eval_pass<true>(a, sm, K, Ku, ngroups, nullptr, zcur, nullptr, rzcur, 0.f, rec, sm.ctl->scF, sm.ctl->scG, red PROF_ARG);
     cg::this_grid().sync();
     ++ph;
     fetch_record(rec, K + 2);
@@ -1061,8 +1243,10 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
             const double gk = i >= 0 ? (double)sm.recv[2 + i] * iG + a.gamma * sm.dG[k] : 0.0;
             const double p = (i < 0 || (sm.y[k] <= 0.0 && gk >= 0.0)) ? 0.0 : gk;
             sm.grad[k] = gk;
-            sm.gF[k] = i >= 0 ? (double)sm.recv[2 + i] * iG : 0.0;
-            sm.hd[k] = 0.0;
+            if (MODE == 1) {
+                sm.gF[k] = i >= 0 ? (double)sm.recv[2 + i] * iG : 0.0;
+                sm.hd[k] = 0.0;
+            }
             sm.pg[k] = p;
             sm.d[k] = -p;
             pgl = fmax(pgl, fabs(p));
@@ -1094,7 +1278,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
         float *qcur = a.q, *qnext = a.q2, *rqcur = sm.rq, *rqnext = sm.rq1;
         while (sm.ctl->state != kFinish) {
             rec = begin_pass();
-            fused_pass(a, sm, K, ngroups, zcur, znext, rzcur, rznext, qcur, qnext, rqcur, rqnext, sm.ctl->tf,
+            fused_pass(a, sm, K, Ku, ngroups, zcur, znext, rzcur, rznext, qcur, qnext, rqcur, rqnext, sm.ctl->tf,
                        sm.ctl->probe != 0, rec, sm.ctl->scF, sm.ctl->scC, sm.ctl->scG, sm.ctl->scH, red);
             cg::this_grid().sync();
             ++ph;
@@ -1210,7 +1394,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
         double curv = 0.0;
         for (int g = 0; g < ngroups; ++g) {
             float qv[kOutPerThread];
-            combine_group(a, sm, K, g, qv PROF_ARG);
+            combine_group(a, sm, Ku, g, qv PROF_ARG);
 #pragma unroll
             for (int r = 0; r < kOutPerThread; ++r) {
                 const int o = tid + r * kMasterThreads, c = chunk_of(g, o >> 7);
@@ -1259,7 +1443,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
         // ---- backtracking on the true cost ----------------------------------------------------------------
         while (sm.ctl->state == kRunTrial) {
             rec = begin_pass();
-            eval_pass<false>(a, sm, K, ngroups, zcur, znext, rzcur, rznext, sm.ctl->tf, rec, sm.ctl->scF,
+            eval_pass<false>(a, sm, K, Ku, ngroups, zcur, znext, rzcur, rznext, sm.ctl->tf, rec, sm.ctl->scF,
                              sm.ctl->scG, red PROF_ARG);
             PROF(3)
             cg::this_grid().sync();
@@ -1368,7 +1552,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     __syncthreads();
     if (sm.ctl->accepted) {
         rec = begin_pass();
-        eval_pass<true>(a, sm, K, ngroups, nullptr, a.z, nullptr, rzcur, 0.f, rec, sm.ctl->scF, sm.ctl->scG, red PROF_ARG);
+        eval_pass<true>(a, sm, K, Ku, ngroups, nullptr, a.z, nullptr, rzcur, 0.f, rec, sm.ctl->scF, sm.ctl->scG, red PROF_ARG);
         cg::this_grid().sync();
         ++ph;
         fetch_record(rec, K + 2);
@@ -1405,10 +1589,15 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     }
 }
 
-size_t master_smem_bytes(int64_t N, int64_t rslots, int64_t cache_segs) {
-    return (size_t)(kKSplit * kGroup * kChunk + 2 * kGroup * kChunk + 7 * rslots + cache_segs * kChunk) * 4   // part, wbuf, ubuf, resident slots, tile
-           + (size_t)(21 * N + 2 + kMasterWarps + 2 * kMasterWarps * kRedSlots) * 8 + sizeof(Ctl)   // K-vectors, recv, red, cred, ctl
-           + (size_t)N * 4 * 6;                                              // coef, sk, lo, hi, ik
+// shared memory of one master block; mode 1 (single-barrier iteration) lays out more (k_master's carve-up)
+size_t seg_bytes(int mode) { return kSeg * 4 + (mode == 1 ? 2 : 1) * 2 * 8 + 2 * 4; }   // tile, gpart (+ gpartu), cseg + gseg
+
+size_t master_smem_bytes(int64_t N, int64_t rslots, int64_t cache_segs, int64_t ngroups, int mode) {
+    const int f1 = mode == 1 ? 1 : 0;
+    return (size_t)(2 * kGroup * kChunk + (1 + f1) * kGroup * kSeg + (6 + f1) * rslots) * 4   // part2, wbuf (ubuf), resident slots
+           + (size_t)cache_segs * seg_bytes(mode)                                            // tile and the lists over it
+           + (size_t)((13 + 8 * f1) * N + 2 * N + 2 + kMasterWarps + 2 * kMasterWarps * kRedSlots) * 8 + sizeof(Ctl)   // K-vectors, recv, red, cred, ctl
+           + (size_t)N * 4 * 7 + (size_t)(ngroups * kGroup + 1) * 4;         // coef, sk, lo, hi, ik, base, unc; coff
 }
 
 }  // namespace
@@ -1428,18 +1617,20 @@ int master_configure(vmat_plan *p) {
     int optin = 0;
     VMAT_CUDA(p, cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, p->device));
     const size_t budget = (size_t)optin > 8 * 1024 ? (size_t)optin - 8 * 1024 : 0;
-    size_t fixed = master_smem_bytes(p->N, rslots, 0);
+    const int mode = p->opt.master_mode;
+    size_t fixed = master_smem_bytes(p->N, rslots, 0, ngroups, mode);
     if (fixed > budget) {
         p->master_rslots = 0;
-        fixed = master_smem_bytes(p->N, 0, 0);
+        fixed = master_smem_bytes(p->N, 0, 0, ngroups, mode);
     }
     if (fixed > budget) return fail(p, VMAT_EINVAL, "n_beams too large for the master kernel's shared memory");
-    p->master_cache_segs = (int)((budget - fixed) / (kChunk * 4));
+    p->master_cache_segs = (int)((budget - fixed) / seg_bytes(mode));
+    if (p->master_cache_segs > 65535 || ngroups * kGroup > 32767) p->master_cache_segs = 0;   // 16-bit fields of the lists
 #ifdef VMAT_MASTER_PROFILE
     if (getenv("VMAT_NO_TILE")) p->master_cache_segs = 0;
     fprintf(stderr, "master: grid %d smem fixed %zu cache_segs %d rslots %d\n", p->master_grid, fixed, p->master_cache_segs, p->master_rslots);
 #endif
-    p->master_smem = master_smem_bytes(p->N, p->master_rslots, p->master_cache_segs);
+    p->master_smem = master_smem_bytes(p->N, p->master_rslots, p->master_cache_segs, ngroups, mode);
     VMAT_CUDA(p, cudaFuncSetAttribute(k_master<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->master_smem));
     VMAT_CUDA(p, cudaFuncSetAttribute(k_master<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->master_smem));
     int per_sm = 0, per_sm1 = 0;
