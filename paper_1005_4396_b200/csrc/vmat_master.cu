@@ -1075,6 +1075,14 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     double F = 0.0, Gs = 0.0, Phi = 0.0, pgmax = 0.0, pg_entry = 0.0, tol = 0.0;
     double phi1 = 0.0, Gd = 0.0, tmax = 0.0, qb = 0.0, yb = 0.0, t = 0.0, Gn = 0.0;
     const double c1a = 1e-4, noise = 2e-7;
+    // The stall rule (stop at the fp32 resolution of the cost) is calibrated for warm starts, where a step that
+    // lowers the cost by <= stall_rel of it really is the end.  A solve that has already lowered the cost by more
+    // than 1 % started far from the optimum: conjugate directions then pass through plateaus of tiny steps before
+    // the next long one, so the rule is applied 100x more strictly there.
+    double Phi0 = 0.0;
+    auto stall_threshold = [&](double Phin) {
+        return (Phi0 - Phin <= 1e-2 * fabs(Phin)) ? a.stall_rel : 1e-2 * a.stall_rel;
+    };
 
     auto set_eval_scales = [&](double zb) {
         const double dev = Tm + zb;
@@ -1257,6 +1265,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
         Phi = F + a.gamma * Gs;
         pgmax = pgl;
         pg_entry = pgmax;
+        Phi0 = Phi;
         tol = a.eps * fmax(1.0, pgmax);
         int state = kRunDirection;
         if (!(pgmax > tol) || bad) state = kFinish;
@@ -1310,7 +1319,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
                 if (accepted) {
                     const int was_probe = probe;
                     if (!was_probe) {
-                        stall = (Phi - Phin <= a.stall_rel * fabs(Phi)) ? stall + 1 : 0;
+                        stall = (Phi - Phin <= stall_threshold(Phin) * fabs(Phi)) ? stall + 1 : 0;
                         F = Fn;
                         Gs = Gn;
                         Phi = Phin;
@@ -1477,7 +1486,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
                 int state;
                 if (accepted) {
                     // take the step; Polak-Ribiere+ direction on the current face, restart when the active set changes
-                    stall = (Phi - Phin <= a.stall_rel * fabs(Phi)) ? stall + 1 : 0;
+                    stall = (Phi - Phin <= stall_threshold(Phin) * fabs(Phi)) ? stall + 1 : 0;
                     F = Fn;
                     Gs = Gn;
                     Phi = Phin;
