@@ -44,16 +44,19 @@ __global__ void __launch_bounds__(256)
 k_column_scatter(const uint32_t *__restrict__ rowq, const float4 *__restrict__ val4, const int4 *__restrict__ col4,
                  const Sel *__restrict__ sel, int beam, const int32_t *__restrict__ left,
                  const int32_t *__restrict__ right, int R, int C, double fx_scale, unsigned long long *__restrict__ acc,
-                 ColStat *__restrict__ colstat) {
+                 ColStat *__restrict__ colstat, uint32_t *__restrict__ touch, int touch_words) {
     const int k = sel ? sel->beam : beam;
     if (k < 0) return;
-    if (blockIdx.x == 0 && threadIdx.x == 0) {   // statistics of the column, filled by k_column_finish
-        ColStat cs;
-        cs.l1 = 0ull;
-        cs.linf = 0ull;
-        cs.clo = INT_MAX;
-        cs.chi = -1;
-        colstat[k] = cs;
+    if (blockIdx.x == 0) {   // statistics and touched-chunk bitmap of the column, filled by k_column_finish
+        if (threadIdx.x == 0) {
+            ColStat cs;
+            cs.l1 = 0ull;
+            cs.linf = 0ull;
+            cs.clo = INT_MAX;
+            cs.chi = -1;
+            colstat[k] = cs;
+        }
+        for (int w = threadIdx.x; w < touch_words; w += blockDim.x) touch[(size_t)k * touch_words + w] = 0u;
     }
     const int lane = threadIdx.x & 31;
     const int idx = blockIdx.x * 8 + (threadIdx.x >> 5);
@@ -91,7 +94,8 @@ k_column_scatter(const uint32_t *__restrict__ rowq, const float4 *__restrict__ v
 // last chunk with a non-zero entry.  One block = 256 slots = 2 chunks.
 __global__ void __launch_bounds__(256)
 k_column_finish(unsigned long long *__restrict__ acc, long long Sp, const Sel *__restrict__ sel, int beam,
-                double fx_inv, float *__restrict__ Dd, ColStat *__restrict__ colstat) {
+                double fx_inv, float *__restrict__ Dd, ColStat *__restrict__ colstat, uint32_t *__restrict__ touch,
+                int touch_words) {
     const int k = sel ? sel->beam : beam;
     if (k < 0) return;
     __shared__ unsigned long long s_sum[8], s_max[8];
@@ -104,7 +108,9 @@ k_column_finish(unsigned long long *__restrict__ acc, long long Sp, const Sel *_
         acc[s] = 0ull;
         mag = (unsigned long long)(v < 0 ? -v : v);
     }
-    const int chunk = (int)(s / kChunk);
+    const int chunk = (int)(s / kChunk);   // the same for the whole warp
+    if (__any_sync(kFull, mag != 0ull) && (threadIdx.x & 31) == 0)
+        atomicOr(touch + (size_t)k * touch_words + (chunk >> 5), 1u << (chunk & 31));
     unsigned long long sum = mag, mx = mag;
     int lo = mag ? chunk : INT_MAX, hi = mag ? chunk : -1;
 #pragma unroll
@@ -219,6 +225,8 @@ struct MasterArgs {
     double *y;
     const double *theta;
     const ColStat *colstat;
+    const uint32_t *touch;      // per column: bit c set iff chunk c holds a non-zero entry (touch_words words each)
+    int touch_words;
     int N;
     double gamma, F_out, eps, fx_inv, stall_rel;
     int stall_count;
@@ -380,8 +388,11 @@ struct Smem {
     float *part2, *wbuf, *ubuf, *coef;
     float *rz0, *rz1, *rq, *rq1, *rT, *ral, *rbe;   // resident copies of the block's own slots (a.rslots each), or unused
     float *tile;       // staged 512-byte segments of the block's part of Dd, kSeg floats apart
-    int *sk, *lo, *hi, *ik;   // lo, hi: block-local range of chunks (j of b + jG) column i touches
-    int *base;         // segment (i, j) is number base[i] + j of the tile; kNoCache if column i is not staged
+    int *sk, *lo, *hi, *ik;   // lo, hi: block-local range of chunks (j of b + jG) that may hold entries of column i
+    int *nseg;         // how many of them really do
+    unsigned long long *lmask;   // which: bit (j & 63) of word lmask[(j >> 6) * N + i]
+    int *base;         // the touched chunks of column i are segments base[i], base[i] + 1, .. of the tile, in chunk
+                       // order; kNoCache if column i is not staged
     int *coff;         // ngroups*kGroup + 1: entries [coff[j], coff[j+1]) of cseg belong to local chunk j
     int *cseg;         // staged segments chunk by chunk, beams ascending: segment | i << 16
     int *gseg;         // staged segments group by group, beams ascending, then chunks: segment | (j - g kGroup) << 16
@@ -393,13 +404,22 @@ struct Smem {
 // chunk handled by this block as member `ch` of its group `g`: chunks are dealt round-robin
 __device__ __forceinline__ int chunk_of(int g, int ch) { return (int)blockIdx.x + (g * kGroup + ch) * (int)gridDim.x; }
 
+__device__ __forceinline__ bool touches(const Smem &sm, int N, int i, int j) {
+    return (sm.lmask[(j >> 6) * N + i] >> (j & 63)) & 1ull;
+}
+// number of touched chunks of column i before local chunk j
+__device__ __forceinline__ int seg_rank(const Smem &sm, int N, int i, int j) {
+    int r = 0;
+    for (int w = 0; w < (j >> 6); ++w) r += __popcll(sm.lmask[w * N + i]);
+    return r + __popcll(sm.lmask[(j >> 6) * N + i] & ((1ull << (j & 63)) - 1ull));
+}
+
 // Columns that are NOT staged.  The four chunks (j = g*kGroup + chalf + 2h, h = 0..3) of column i that this
 // warp's half of the group covers: v[h] = the lane's float4 of segment h, zero where the column does not touch
 // the chunk; the four loads from L2 / HBM are independent.
 __device__ __forceinline__ void load_half(const MasterArgs &a, const Smem &sm, int i, int g, int chalf, int lane,
                                           float4 (&v)[kGroup / 2]) {
-    const int lb = max(sm.lo[i] - g * kGroup, 0), hb = min(sm.hi[i] - g * kGroup, kGroup - 1);
-    const unsigned m = hb >= lb ? (((2u << hb) - 1u) & ~((1u << lb) - 1u)) >> chalf : 0u;
+    const unsigned m = ((unsigned)(sm.lmask[((g * kGroup) >> 6) * a.N + i] >> ((g * kGroup) & 63)) & 0xffu) >> chalf;
     const int j0 = g * kGroup + chalf, G = (int)gridDim.x;
     const float4 *row = reinterpret_cast<const float4 *>(a.Dd + (size_t)sm.sk[i] * a.Sp) +
                         (size_t)((int)blockIdx.x + j0 * G) * (kChunk / 4) + lane;
@@ -462,7 +482,7 @@ __device__ __forceinline__ void combine_group(const MasterArgs &a, const Smem &s
                     v[x] = make_float4(0.f, 0.f, 0.f, 0.f);
                     if (uu < Ku) {
                         const int i = sm.unc[uu];
-                        if (sm.lo[i] <= j && j <= sm.hi[i]) {
+                        if (touches(sm, a.N, i, j)) {
                             c[x] = sm.coef[i];
                             v[x] = __ldg(Dd4 + (size_t)sm.sk[i] * row4);
                         }
@@ -540,7 +560,7 @@ __device__ __forceinline__ double grad_total(const Smem &sm, const double *gp, i
     const int bs = sm.base[i];
     if (bs == kNoCache) return sm.gacc[row0 * N + i] + sm.gacc[(row0 + 1) * N + i];
     double s = 0.0;
-    for (int j = sm.lo[i]; j <= sm.hi[i]; ++j) s += gp[2 * (bs + j)] + gp[2 * (bs + j) + 1];
+    for (int q = 0; q < sm.nseg[i]; ++q) s += gp[2 * (bs + q)] + gp[2 * (bs + q) + 1];
     return s;
 }
 
@@ -848,7 +868,10 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     sm.gm = sm.dnx + F1 * N;
     sm.gpart = sm.gm + F1 * N;
     sm.gpartu = sm.gpart + 2 * a.cache_segs;
-    double *red = sm.gpartu + F1 * 2 * a.cache_segs;
+    const int ngroups = (a.nchunks + (int)gridDim.x * kGroup - 1) / ((int)gridDim.x * kGroup);
+    const int W64 = (ngroups * kGroup + 63) >> 6;   // 64-bit words of a column's local chunk mask
+    sm.lmask = reinterpret_cast<unsigned long long *>(sm.gpartu + F1 * 2 * a.cache_segs);
+    double *red = reinterpret_cast<double *>(sm.lmask + (size_t)W64 * N);
     double *cred = red + kMasterWarps;   // 2 x kMasterWarps x kRedSlots
     sm.recv = reinterpret_cast<long long *>(cred + 2 * kMasterWarps * kRedSlots);
     sm.ctl = reinterpret_cast<Ctl *>(sm.recv + 2 * N + 2);
@@ -861,8 +884,8 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     sm.unc = sm.base + N;
     sm.cseg = sm.unc + N;
     sm.gseg = sm.cseg + a.cache_segs;
-    sm.coff = sm.gseg + a.cache_segs;   // ngroups * kGroup + 1
-    const int ngroups = (a.nchunks + (int)gridDim.x * kGroup - 1) / ((int)gridDim.x * kGroup);
+    sm.nseg = sm.gseg + a.cache_segs;
+    sm.coff = sm.nseg + N;   // ngroups * kGroup + 1
     __shared__ int sK, sKu;
     __shared__ uint64_t tile_bar;
 
@@ -900,6 +923,21 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
             const int b = (int)blockIdx.x, Gd_ = (int)gridDim.x;
             sm.lo[i] = cs.clo > b ? (cs.clo - b + Gd_ - 1) / Gd_ : 0;
             sm.hi[i] = cs.chi >= b ? (cs.chi - b) / Gd_ : -1;
+            // which of them hold a non-zero entry of the column (the range is half empty: an aperture lights a
+            // strip of every slab it crosses)
+            const uint32_t *tw = a.touch + (size_t)k * a.touch_words;
+            int n = 0;
+            for (int w = 0; w < W64; ++w) {
+                unsigned long long bits = 0ull;
+                const int ja = max(sm.lo[i], w * 64), jb = min(sm.hi[i], w * 64 + 63);
+                for (int j = ja; j <= jb; ++j) {
+                    const int c = b + j * Gd_;
+                    if ((__ldg(tw + (c >> 5)) >> (c & 31)) & 1u) bits |= 1ull << (j & 63);
+                }
+                sm.lmask[w * N + i] = bits;
+                n += __popcll(bits);
+            }
+            sm.nseg[i] = n;
             lf = (double)cs.linf * a.fx_inv * 1.000001;
             l1l = fmax(l1l, (double)cs.l1 * a.fx_inv * 1.000001);
             sm.coef[i] = (float)sm.y[k];
@@ -919,11 +957,8 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
             int run = 0, total = 0;
             for (int i0 = 0; i0 < K; i0 += 32) {
                 const int i = i0 + lane;
-                int j0 = 0, cnt = 0;
-                if (i < K) {
-                    j0 = sm.lo[i];
-                    cnt = max(sm.hi[i] - j0 + 1, 0);
-                }
+                int cnt = 0;
+                if (i < K) cnt = sm.nseg[i];
                 int incl = cnt;
 #pragma unroll
                 for (int o = 1; o < 32; o <<= 1) {
@@ -932,7 +967,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
                 }
                 const int off = run + incl - cnt;
                 const bool cached = cnt > 0 && off + cnt <= a.cache_segs;
-                if (i < K) sm.base[i] = cached ? off - j0 : kNoCache;
+                if (i < K) sm.base[i] = cached ? off : kNoCache;
                 total += cached ? cnt : 0;
                 run += __shfl_sync(kFull, incl, 31);
             }
@@ -945,8 +980,10 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
                 if (bs == kNoCache) continue;
                 const int j0 = sm.lo[i], j1 = sm.hi[i];
                 const float *src = a.Dd + (size_t)sm.sk[i] * a.Sp;
+                int q = 0;
                 for (int j = j0; j <= j1; ++j)
-                    bulk_g2s(sm.tile + (size_t)(bs + j) * kSeg, src + (size_t)(b + j * G) * kChunk, kChunk * 4, &tile_bar);
+                    if (touches(sm, N, i, j))
+                        bulk_g2s(sm.tile + (size_t)(bs + q++) * kSeg, src + (size_t)(b + j * G) * kChunk, kChunk * 4, &tile_bar);
             }
         }
         __syncthreads();          // sm.base visible to all warps
@@ -957,7 +994,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
         int run = 0;
         for (int i0 = 0; i0 < K; i0 += 32) {
             const int i = i0 + lane;
-            const bool f = i < K && sm.base[i] == kNoCache && sm.hi[i] >= sm.lo[i];
+            const bool f = i < K && sm.base[i] == kNoCache && sm.nseg[i] > 0;
             const unsigned m = __ballot_sync(kFull, f);
             if (f) sm.unc[run + __popc(m & ((1u << lane) - 1u))] = i;
             run += __popc(m);
@@ -968,7 +1005,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
         int c = 0;
         for (int i0 = 0; i0 < K; i0 += 32) {
             const int i = i0 + lane;
-            const bool f = i < K && sm.base[i] != kNoCache && sm.lo[i] <= j && j <= sm.hi[i];
+            const bool f = i < K && sm.base[i] != kNoCache && touches(sm, N, i, j);
             c += __popc(__ballot_sync(kFull, f));
         }
         if (lane == 0) sm.coff[j + 1] = c;
@@ -994,9 +1031,9 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
         int pos = sm.coff[j];
         for (int i0 = 0; i0 < K; i0 += 32) {
             const int i = i0 + lane;
-            const bool f = i < K && sm.base[i] != kNoCache && sm.lo[i] <= j && j <= sm.hi[i];
+            const bool f = i < K && sm.base[i] != kNoCache && touches(sm, N, i, j);
             const unsigned m = __ballot_sync(kFull, f);
-            if (f) sm.cseg[pos + __popc(m & ((1u << lane) - 1u))] = (sm.base[i] + j) | (i << 16);
+            if (f) sm.cseg[pos + __popc(m & ((1u << lane) - 1u))] = (sm.base[i] + seg_rank(sm, N, i, j)) | (i << 16);
             pos += __popc(m);
         }
     }
@@ -1004,11 +1041,10 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
         int pos = sm.coff[g * kGroup];
         for (int i0 = 0; i0 < K; i0 += 32) {
             const int i = i0 + lane;
-            int ja = 0, cnt = 0;
-            if (i < K && sm.base[i] != kNoCache) {
-                ja = max(sm.lo[i], g * kGroup);
-                cnt = max(min(sm.hi[i], g * kGroup + kGroup - 1) - ja + 1, 0);
-            }
+            unsigned bits = 0u;   // the column's touched chunks within group g
+            if (i < K && sm.base[i] != kNoCache)
+                bits = (unsigned)(sm.lmask[((g * kGroup) >> 6) * N + i] >> ((g * kGroup) & 63)) & 0xffu;
+            const int cnt = __popc(bits);
             int incl = cnt;
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
@@ -1016,7 +1052,11 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
                 if (lane >= o) incl += n;
             }
             const int at = pos + incl - cnt;
-            for (int q = 0; q < cnt; ++q) sm.gseg[at + q] = (sm.base[i] + ja + q) | ((ja + q - g * kGroup) << 16);
+            if (cnt) {
+                int sg = sm.base[i] + seg_rank(sm, N, i, g * kGroup);
+                for (int q = 0, cs = 0; cs < kGroup; ++cs)
+                    if ((bits >> cs) & 1u) sm.gseg[at + q++] = (sg++) | (cs << 16);
+            }
             pos += __shfl_sync(kFull, incl, 31);
         }
     }
@@ -1606,7 +1646,8 @@ size_t master_smem_bytes(int64_t N, int64_t rslots, int64_t cache_segs, int64_t 
     return (size_t)(2 * kGroup * kChunk + (1 + f1) * kGroup * kSeg + (6 + f1) * rslots) * 4   // part2, wbuf (ubuf), resident slots
            + (size_t)cache_segs * seg_bytes(mode)                                            // tile and the lists over it
            + (size_t)((13 + 8 * f1) * N + 2 * N + 2 + kMasterWarps + 2 * kMasterWarps * kRedSlots) * 8 + sizeof(Ctl)   // K-vectors, recv, red, cred, ctl
-           + (size_t)N * 4 * 7 + (size_t)(ngroups * kGroup + 1) * 4;         // coef, sk, lo, hi, ik, base, unc; coff
+           + (size_t)N * 4 * 8 + (size_t)(ngroups * kGroup + 1) * 4           // coef, sk, lo, hi, ik, base, unc, nseg; coff
+           + (size_t)((ngroups * kGroup + 63) / 64) * N * 8;                  // lmask
 }
 
 }  // namespace
@@ -1651,6 +1692,9 @@ int master_configure(vmat_plan *p) {
     if ((rc = dev_alloc(p, &p->accbuf, 3 * kSumGroups * (2 * p->N + 2)))) return rc;
     if ((rc = dev_alloc(p, &p->phase, 2))) return rc;
     if ((rc = dev_alloc(p, &p->colstat, p->N))) return rc;
+    p->touch_words = (int)((nchunks + 31) / 32);
+    if ((rc = dev_alloc(p, &p->col_touch, p->N * p->touch_words))) return rc;
+    VMAT_CUDA(p, cudaMemsetAsync(p->col_touch, 0, (size_t)p->N * p->touch_words * 4, p->stream));
     if ((rc = dev_alloc(p, &p->vbounds, 2))) return rc;
     VMAT_CUDA(p, cudaMemsetAsync(p->accbuf, 0, (size_t)3 * kSumGroups * (2 * p->N + 2) * 8, p->stream));
     VMAT_CUDA(p, cudaMemsetAsync(p->phase, 0, 8, p->stream));
@@ -1671,9 +1715,9 @@ int launch_column_build(vmat_plan *p, int beam) {
     const Sel *sel = beam < 0 ? p->sel : nullptr;
     const unsigned blocks = (unsigned)((p->RC + 7) / 8);
     k_column_scatter<<<blocks, 256, 0, p->stream>>>(p->rowq, p->val4, p->col4, sel, beam, p->left, p->right, (int)p->R,
-                                                   (int)p->C, p->fx_scale, p->acc, p->colstat);
+                                                   (int)p->C, p->fx_scale, p->acc, p->colstat, p->col_touch, p->touch_words);
     k_column_finish<<<(unsigned)((p->Sp + 255) / 256), 256, 0, p->stream>>>(p->acc, (long long)p->Sp, sel, beam,
-                                                                          p->fx_inv, p->Dd, p->colstat);
+                                                                          p->fx_inv, p->Dd, p->colstat, p->col_touch, p->touch_words);
     p->launches += 2;
     VMAT_CUDA(p, cudaGetLastError());
     return VMAT_OK;
@@ -1705,6 +1749,8 @@ static int launch_master_impl(vmat_plan *p, int max_inner, int trace_it) {
     a.rslots = p->master_rslots;
     a.cache_segs = p->master_cache_segs;
     a.colstat = p->colstat;
+    a.touch = p->col_touch;
+    a.touch_words = p->touch_words;
     a.fx_inv = p->fx_inv;
     a.Tmax = p->Tmax;
     a.abmax = p->abmax;
