@@ -86,7 +86,9 @@ typedef struct {
     double  master_eps;        /* stop when max|projected gradient| <= eps*max(1, value at entry) */
     int32_t master_max_inner;  /* cap on inner iterations of one master solve                     */
     double  master_stall_rel;  /* a step that lowers the cost by <= this fraction of it is a stall:
-                                  the decrease is below what fp32 dose arithmetic resolves        */
+                                  the decrease is below what fp32 dose arithmetic resolves.  Once a
+                                  solve has lowered the cost by more than 1 % (a start far from the
+                                  optimum) the fraction is applied 100x more strictly              */
     int32_t master_stall_count;/* stop after this many stalls in a row (stop_reason 4)            */
     int32_t record_phases;     /* 1: vmat_solve brackets each phase with CUDA events              */
     int32_t master_mode;       /* inner iteration of the master kernel: 0 = two passes over the columns and two
