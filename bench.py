@@ -366,6 +366,7 @@ def main():
     plan.solve(iters, trace=False)
     ph_us = {"price": 0.0, "search": 0.0, "column": 0.0, "master": 0.0, "total": 0.0}
     inner_total = 0
+    m_passes = m_bytes = 0.0
     for _ in range(args.steps):
         plan.set_plan(*empty)
         st = plan.solve(iters, trace=True)
@@ -373,6 +374,8 @@ def main():
                      ("master", st.us_master), ("total", st.us_total)):
             ph_us[k] += v / args.steps
         inner_total += int(st.inner.sum())
+        m_passes += st.master_passes / args.steps
+        m_bytes += st.master_bytes / args.steps
     # ---- steps (a)+(b) on the finished plan, both layouts (north_star: "chosen by measurement") -------------
     occ_f, left_f, right_f, _ = plan.get_plan()
     nnz_open = 0
@@ -409,6 +412,17 @@ def main():
         "algorithmic_bytes_per_launch_avg": sum(alg) / iters, "algorithmic_bytes_first_launch": alg[0],
         "avg_launch_us": ph_us["price"] / iters, "launches_per_step": iters,
         "how": "CUDA events on the plan's stream around every pricing launch of the phase-timed steps",
+    }
+    # the master kernel (step e) takes the larger share of a plan: its algorithmic traffic = the touched 512-byte
+    # segments of the aperture-dose columns x the passes that multiplied them (counted on the device); on
+    # configs[1] those segments sit in shared memory, so this is an effective rate, not DRAM traffic
+    m_gbs = m_bytes / (ph_us["master"] * 1e-6) / 1e9 if ph_us["master"] > 0 else 0.0
+    roofline_master = {
+        "kernel": "k_master (master solve, steps a+b+e)", "bound": "hbm", "achieved": m_gbs, "peak": peak, "unit": "GB/s",
+        "frac": m_gbs / peak, "traffic": None, "algorithmic_bytes_per_step": m_bytes, "passes_per_step": m_passes,
+        "us_per_pass": ph_us["master"] / m_passes if m_passes else None, "launches_per_step": iters,
+        "note": "latency bound: two grid barriers and two control steps per inner iteration "
+                "(profiles/r01c_master.md); bytes = touched column segments x passes, device-counted",
     }
     phases = {k + "_us_per_step": v for k, v in ph_us.items()}
     phases["master_inner_iterations_per_step"] = inner_total / args.steps
@@ -459,7 +473,7 @@ def main():
         "dtype": "f32", "data": "synthetic", "config": workload_config(ph, args),
         "plan_wall_time_ms": ms / args.steps, "final_cost": final_cost,
         "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
-        "phases": phases, "dose_pass": dose, "layout": info, "create_ms": create_ms, "generate_inputs_s": gen_s,
+        "roofline_master": roofline_master, "phases": phases, "dose_pass": dose, "layout": info, "create_ms": create_ms, "generate_inputs_s": gen_s,
         "paper_context": "PAPER.md:157 whole plan 18-31 s (CUDA, Tesla C1060) / 5-8 min (MATLAB, Xeon) on clinical "
                          "cases of 1.8e7-5.5e7 non-zeros; different machine and data, not a target",
     }

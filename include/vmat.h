@@ -126,6 +126,9 @@ typedef struct {
     double  *price;         /* its price                                                        */
     double  *trace_F, *trace_G, *trace_cost;   /* after each master solve                       */
     int32_t *inner;         /* master inner iterations                                          */
+    /* bookkeeping of the master kernel over the call (algorithmic traffic of step e):                  */
+    double  master_passes;  /* passes over the aperture-dose columns, each ended by a grid barrier      */
+    double  master_bytes;   /* bytes of the touched 512-byte column segments those passes multiplied    */
 } vmat_solve_stats;
 
 typedef struct {

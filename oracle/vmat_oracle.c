@@ -309,6 +309,7 @@ static void master_gradient(const vo_problem *p, const vo_columns *c, const uint
 typedef struct {
     double eps;           /* stop when max|projected gradient| <= eps*max(1, the same norm at entry) */
     int64_t max_inner;    /* iteration cap                                                           */
+    double lb, ub;        /* bounds on the dose rates of occupied beams: lb <= y_k <= ub (default 0, +inf)  */
     /* outputs */
     int64_t inner;        /* iterations done                                                         */
     int64_t backtracks;   /* step halvings                                                           */
@@ -332,6 +333,12 @@ typedef struct {
  *   TRUE Phi (c1 = 1e-4);  y += t d (clamped at 0), z += t q.
  * Two products with Dc per inner iteration = the "aperture-dose GEMV pair".
  * y is updated in place; z (V) receives sum_k y_k d_k recomputed from the final y.
+ *
+ * Variant (PAPER.md:159 names "the maximum and minimum dose rate constraints" and leaves them
+ * out of "this preliminary work"): bounds lb <= y_k <= ub on the occupied beams (reading R4 of DESIGN.md:
+ * un-occupied beams deliver nothing, y_k = 0).  Gradient projection on a box instead of on y >= 0: pg_k = 0
+ * also where y_k = ub and grad_k <= 0, t_max also limited by (ub - y_k)/d_k for d_k > 0.  With lb = 0,
+ * ub = +inf every expression below reduces to the one above, bit for bit.
  * ------------------------------------------------------------------------------------------ */
 static void master_solve(const vo_problem *p, const vo_columns *cols, const uint8_t *occ, double *y, double *z,
                          vo_master_info *info) {
@@ -343,8 +350,13 @@ static void master_solve(const vo_problem *p, const vo_columns *cols, const uint
     double *pgn = (double *)malloc(sizeof(double) * N), *d = (double *)calloc(N, sizeof(double));
     double *yn = (double *)malloc(sizeof(double) * N);
     const double c1 = 1e-4;
+    const double lb = info->lb, ub = info->ub;
 
-    for (int64_t k = 0; k < N; ++k) if (!occ[k] || y[k] < 0.0) y[k] = 0.0;
+    for (int64_t k = 0; k < N; ++k) {
+        if (!occ[k]) y[k] = 0.0;
+        else if (y[k] < lb) y[k] = lb;
+        else if (y[k] > ub) y[k] = ub;
+    }
     columns_dose(cols, occ, y, z);
     double F = vo_penalty(V, z, p->T, p->alpha, p->beta, w);
     double G = vo_smooth(N, y, p->theta, dG);
@@ -352,7 +364,7 @@ static void master_solve(const vo_problem *p, const vo_columns *cols, const uint
     master_gradient(p, cols, occ, w, dG, grad);
     double pgmax = 0.0;
     for (int64_t k = 0; k < N; ++k) {
-        pg[k] = (!occ[k] || (y[k] <= 0.0 && grad[k] >= 0.0)) ? 0.0 : grad[k];
+        pg[k] = (!occ[k] || (y[k] <= lb && grad[k] >= 0.0) || (y[k] >= ub && grad[k] <= 0.0)) ? 0.0 : grad[k];
         d[k] = -pg[k];
         if (fabs(pg[k]) > pgmax) pgmax = fabs(pg[k]);
     }
@@ -383,8 +395,10 @@ static void master_solve(const vo_problem *p, const vo_columns *cols, const uint
         }
         const double phi2 = 2.0 * curvF + 2.0 * p->gamma * vo_smooth(N, d, p->theta, NULL); /* d^T L d = G(d) */
         double tmax = INFINITY;
-        for (int64_t k = 0; k < N; ++k)
-            if (d[k] < 0.0 && y[k] / (-d[k]) < tmax) tmax = y[k] / (-d[k]);
+        for (int64_t k = 0; k < N; ++k) {
+            if (d[k] < 0.0 && (y[k] - lb) / (-d[k]) < tmax) tmax = (y[k] - lb) / (-d[k]);
+            if (d[k] > 0.0 && (ub - y[k]) / d[k] < tmax) tmax = (ub - y[k]) / d[k];
+        }
         double t = phi2 > 0.0 ? -phi1 / phi2 : (isfinite(tmax) ? tmax : 1.0);
         int hit = 0;
         if (t >= tmax) { t = tmax; hit = 1; }
@@ -392,7 +406,12 @@ static void master_solve(const vo_problem *p, const vo_columns *cols, const uint
         int accepted = 0;
         double Fn = 0.0, Gn = 0.0, Phin = 0.0;
         for (int half = 0; half < 80; ++half) {
-            for (int64_t k = 0; k < N; ++k) { yn[k] = y[k] + t * d[k]; if (yn[k] < 0.0 || (hit && d[k] < 0.0 && y[k] / (-d[k]) <= tmax)) yn[k] = 0.0; }
+            for (int64_t k = 0; k < N; ++k) {
+                yn[k] = y[k] + t * d[k];
+                if (!occ[k]) continue;
+                if (yn[k] < lb || (hit && d[k] < 0.0 && (y[k] - lb) / (-d[k]) <= tmax)) yn[k] = lb;
+                else if (yn[k] > ub || (hit && d[k] > 0.0 && (ub - y[k]) / d[k] <= tmax)) yn[k] = ub;
+            }
 #pragma omp parallel for schedule(static)
             for (int64_t j = 0; j < V; ++j) zn[j] = z[j] + t * q[j];
             Fn = vo_penalty(V, zn, p->T, p->alpha, p->beta, wn);
@@ -419,7 +438,7 @@ static void master_solve(const vo_problem *p, const vo_columns *cols, const uint
         double num = 0.0, den = 0.0;
         pgmax = 0.0;
         for (int64_t k = 0; k < N; ++k) {
-            pgn[k] = (!occ[k] || (y[k] <= 0.0 && gradn[k] >= 0.0)) ? 0.0 : gradn[k];
+            pgn[k] = (!occ[k] || (y[k] <= lb && gradn[k] >= 0.0) || (y[k] >= ub && gradn[k] <= 0.0)) ? 0.0 : gradn[k];
             if ((pgn[k] == 0.0) != (pg[k] == 0.0)) changed = 1;        /* a bound was hit or released */
             num += pgn[k] * (pgn[k] - pg[k]);
             den += pg[k] * pg[k];
@@ -428,7 +447,7 @@ static void master_solve(const vo_problem *p, const vo_columns *cols, const uint
         const double bpr = (changed || !(den > 0.0) || num <= 0.0) ? 0.0 : num / den;   /* PR+, restart on face change */
         for (int64_t k = 0; k < N; ++k) {
             d[k] = -pgn[k] + bpr * d[k];
-            if (!occ[k] || (y[k] <= 0.0 && d[k] < 0.0)) d[k] = 0.0;      /* stay feasible */
+            if (!occ[k] || (y[k] <= lb && d[k] < 0.0) || (y[k] >= ub && d[k] > 0.0)) d[k] = 0.0;      /* stay feasible */
             grad[k] = gradn[k]; pg[k] = pgn[k];
         }
         ++info->inner;
@@ -495,6 +514,8 @@ void vo_enforce_rate(const vo_problem *p, const uint8_t *occ, const int32_t *lef
         vo_master_info mi;
         mi.eps = info->eps;
         mi.max_inner = info->max_inner;
+        mi.lb = 0.0;
+        mi.ub = INFINITY;
         master_solve(&q, cols, occ, y, z, &mi);                    /* "intensity ... re-optimized"          */
         ++rounds;
         ratio = vo_rate_ratio(p->N, y, p->theta, info->rho);       /* "till the solution is feasible"       */
@@ -581,6 +602,7 @@ void vo_solve(const vo_problem *p, uint8_t *occ, int32_t *left, int32_t *right, 
         double t1 = now_s();
         vo_master_info info; memset(&info, 0, sizeof(info));
         info.eps = tr->eps; info.max_inner = tr->max_inner;
+        info.lb = 0.0; info.ub = INFINITY;
         master_solve(p, cols, occ, y, z, &info);
         double t2 = now_s();
         tr->seconds_price += t1 - t0; tr->seconds_master += t2 - t1;

@@ -35,7 +35,8 @@ class _Problem(_c.Structure):
 
 
 class _MasterInfo(_c.Structure):
-    _fields_ = [("eps", _c.c_double), ("max_inner", _c.c_int64), ("inner", _c.c_int64),
+    _fields_ = [("eps", _c.c_double), ("max_inner", _c.c_int64), ("lb", _c.c_double), ("ub", _c.c_double),
+                ("inner", _c.c_int64),
                 ("backtracks", _c.c_int64), ("pg_entry", _c.c_double), ("pg_exit", _c.c_double),
                 ("F", _c.c_double), ("G", _c.c_double), ("cost", _c.c_double)]
 
@@ -251,12 +252,13 @@ class Oracle:
                     all_left=al.reshape(self.N, self.R), all_right=ar.reshape(self.N, self.R))
 
     # O7 ----------------------------------------------------------------------------------------
-    def master(self, occ, left, right, y0=None, eps=1e-9, max_inner=20000):
-        """Returns (y, z, MasterInfo)."""
+    def master(self, occ, left, right, y0=None, eps=1e-9, max_inner=20000, y_min=0.0, y_max=float("inf")):
+        """Returns (y, z, MasterInfo).  y_min, y_max: bounds on the dose rates of the occupied beams (variant of
+        PAPER.md:159's "maximum and minimum dose rate constraints"; default none but y >= 0)."""
         occ, left, right = self._plan(occ, left, right)
         y = np.zeros(self.N, np.float64) if y0 is None else _as(y0, np.float64).copy()
         z = np.empty(self.V, np.float64)
-        info = _MasterInfo(eps=eps, max_inner=max_inner)
+        info = _MasterInfo(eps=eps, max_inner=max_inner, lb=float(y_min), ub=float(y_max))
         self._L.vo_master(_c.byref(self._p), _ptr(occ), _ptr(left), _ptr(right), _ptr(y), _ptr(z), _c.byref(info))
         return y, z, MasterInfo(info.inner, info.backtracks, info.pg_entry, info.pg_exit, info.F, info.G, info.cost)
 

@@ -61,7 +61,7 @@ class _SolveStats(C.Structure):
     _fields_ = [("iters", C.c_int32), ("us_total", C.c_double), ("us_price", C.c_double), ("us_search", C.c_double),
                 ("us_column", C.c_double), ("us_master", C.c_double), ("F", C.c_double), ("G", C.c_double),
                 ("cost", C.c_double), ("beam", _P), ("price", _P), ("trace_F", _P), ("trace_G", _P),
-                ("trace_cost", _P), ("inner", _P)]
+                ("trace_cost", _P), ("inner", _P), ("master_passes", C.c_double), ("master_bytes", C.c_double)]
 
 
 class _RateStats(C.Structure):
@@ -172,6 +172,8 @@ class SolveStats:
     trace_G: np.ndarray
     trace_cost: np.ndarray
     inner: np.ndarray
+    master_passes: float = 0.0
+    master_bytes: float = 0.0
 
 
 def _is_torch(a) -> bool:
@@ -335,7 +337,7 @@ class Plan:
         self._check(self._L.vmat_solve(self._h, int(max_iters), C.byref(s)))
         n = int(s.iters)
         return SolveStats(n, s.us_total, s.us_price, s.us_search, s.us_column, s.us_master, s.F, s.G, s.cost,
-                          beam[:n], price[:n], tF[:n], tG[:n], tC[:n], inner[:n])
+                          beam[:n], price[:n], tF[:n], tG[:n], tC[:n], inner[:n], s.master_passes, s.master_bytes)
 
     # -- plan state -------------------------------------------------------------------------------
     def get_plan(self):

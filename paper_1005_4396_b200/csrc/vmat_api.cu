@@ -503,6 +503,7 @@ int vmat_solve(vmat_plan *p, int32_t max_iters, vmat_solve_stats *out) {
             return cuda_fail(p, ce__, #call);        \
         }                                            \
     }
+    TRYC(cudaMemsetAsync(p->mcount, 0, 16, st));
     TRYC(cudaEventRecord(ev0, st));
     TRY(ensure_state(p));
     TRY(ensure_columns(p));   // the master needs d_k of every occupied beam, whichever path formed z
@@ -548,6 +549,10 @@ int vmat_solve(vmat_plan *p, int32_t max_iters, vmat_solve_stats *out) {
         out->F = c3[0];
         out->G = c3[1];
         out->cost = c3[2];
+        unsigned long long mc[2];
+        TRYC(cudaMemcpy(mc, p->mcount, sizeof(mc), cudaMemcpyDeviceToHost));
+        out->master_passes = (double)mc[1];
+        out->master_bytes = (double)mc[0] * (double)(kChunk * 4);
         const size_t n = (size_t)todo;
         if (n) {
             if (out->beam) TRYC(cudaMemcpy(out->beam, p->tr_beam, n * 4, cudaMemcpyDeviceToHost));

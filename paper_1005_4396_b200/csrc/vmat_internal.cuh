@@ -85,6 +85,7 @@ struct vmat_plan {
 
     long long *accbuf = nullptr;       // 3 x (2N + 2) fixed-point sums of the master kernel
     unsigned int *phase = nullptr;     // rotation counter of accbuf, barrier epoch
+    unsigned long long *mcount = nullptr;   // master bookkeeping: touched segments x passes, passes
     vmat::ColStat *colstat = nullptr;  // N
     uint32_t *col_touch = nullptr;     // N x touch_words: bit c of row k set iff chunk c of d_k holds a non-zero entry
     int touch_words = 0;

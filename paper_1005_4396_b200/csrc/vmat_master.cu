@@ -238,6 +238,7 @@ struct MasterArgs {
                                 // grad[0..K), and (fused mode) the Hessian-vector product [K..2K); a block adds
                                 // to the record of its group (blockIdx mod kSumGroups)
     unsigned int *phase;        // rotation counter, persists from launch to launch
+    unsigned long long *mcount; // bookkeeping: [0] += touched segments x passes (all blocks), [1] += passes
     MasterOut *out;
     double *cost3;
     double *trF, *trG, *trC;
@@ -886,7 +887,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     sm.gseg = sm.cseg + a.cache_segs;
     sm.nseg = sm.gseg + a.cache_segs;
     sm.coff = sm.nseg + N;   // ngroups * kGroup + 1
-    __shared__ int sK, sKu;
+    __shared__ int sK, sKu, sSegs;
     __shared__ uint64_t tile_bar;
 
     // occupied beams in ascending order
@@ -901,7 +902,10 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
             if (k < N) sm.ik[k] = f ? i : -1;
             base += __popc(m);
         }
-        if (tid == 0) sK = base;
+        if (tid == 0) {
+            sK = base;
+            sSegs = 0;
+        }
     }
     for (int k = tid; k < N; k += kMasterThreads) {
         double yk = a.y[k];
@@ -938,6 +942,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
                 n += __popcll(bits);
             }
             sm.nseg[i] = n;
+            if (n) atomicAdd(&sSegs, n);
             lf = (double)cs.linf * a.fx_inv * 1.000001;
             l1l = fmax(l1l, (double)cs.l1 * a.fx_inv * 1.000001);
             sm.coef[i] = (float)sm.y[k];
@@ -1610,6 +1615,10 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
             Phi = F + a.gamma * Gs;
         }
     }
+    if (tid == 0) {
+        atomicAdd(a.mcount, (unsigned long long)sSegs * (unsigned long long)(ph - ph_entry));
+        if (blockIdx.x == 0) atomicAdd(a.mcount + 1, (unsigned long long)(ph - ph_entry));
+    }
     if (blockIdx.x == 0 && warp == 0) {
         for (int k = lane; k < N; k += 32) a.y[k] = sm.y[k];
         if (lane == 0) {
@@ -1691,6 +1700,8 @@ int master_configure(vmat_plan *p) {
     int rc;
     if ((rc = dev_alloc(p, &p->accbuf, 3 * kSumGroups * (2 * p->N + 2)))) return rc;
     if ((rc = dev_alloc(p, &p->phase, 2))) return rc;
+    if ((rc = dev_alloc(p, &p->mcount, 2))) return rc;
+    VMAT_CUDA(p, cudaMemsetAsync(p->mcount, 0, 16, p->stream));
     if ((rc = dev_alloc(p, &p->colstat, p->N))) return rc;
     p->touch_words = (int)((nchunks + 31) / 32);
     if ((rc = dev_alloc(p, &p->col_touch, p->N * p->touch_words))) return rc;
@@ -1756,6 +1767,7 @@ static int launch_master_impl(vmat_plan *p, int max_inner, int trace_it) {
     a.abmax = p->abmax;
     a.accbuf = p->accbuf;
     a.phase = p->phase;
+    a.mcount = p->mcount;
     a.out = p->mout;
     a.cost3 = p->cost3;
     a.trF = p->tr_F;

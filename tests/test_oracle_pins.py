@@ -397,6 +397,78 @@ def test_master_equals_nnls_when_all_quadratic():
 
 
 # ------------------------------------------------------------------------------------------------
+# variant: bounds on the dose rates of occupied beams (PAPER.md:159 names "the maximum and minimum dose rate
+# constraints" and leaves them out; reading R4)
+# ------------------------------------------------------------------------------------------------
+def test_master_bounds_one_voxel_closed_form():
+    # one aperture, one voxel: min (T - y d)^2 over lb <= y <= ub is the unconstrained y* = T/d clipped to the box
+    o = Oracle(np.array([0, 1], np.int64), [0], [0.25], [0.8], [1.0], [1.0], [0.0], 1, 1, 1, 0.0)
+    ystar = float(np.float32(0.8)) / 0.25
+    for lb, ub in ((0.0, 2.0), (4.0, 9.0), (1.0, 5.0), (0.0, float("inf"))):
+        y, z, info = o.master([1], [[0]], [[1]], y_min=lb, y_max=ub)
+        want = min(max(ystar, lb), ub)
+        assert y[0] == pytest.approx(want, rel=1e-9)
+        assert info.cost == pytest.approx((float(np.float32(0.8)) - want * 0.25) ** 2, rel=1e-9, abs=1e-15)
+    # an un-occupied beam stays at 0 whatever the lower bound (it has no aperture: reading R4)
+    o = Oracle(np.array([0, 1, 2], np.int64), [0, 0], [0.25, 0.25], [0.8], [1.0], [1.0], [0.0, 2.0], 1, 1, 1, 0.0)
+    y, z, info = o.master([1, 0], [[0], [0]], [[1], [1]], y_min=0.5, y_max=2.0)
+    assert y[1] == 0.0 and y[0] == pytest.approx(2.0)
+
+
+def test_master_bounds_satisfy_box_kkt_random():
+    """KKT of min Phi over the box: lb < y_k < ub => dPhi/dy_k = 0; y_k = lb => >= 0; y_k = ub => <= 0."""
+    hit_lo = hit_hi = inside = 0
+    for seed in range(6):
+        o, D, rng = small_problem(300 + seed, V=80, N=7, R=3, C=6, gamma=0.2 * seed, delta=2, nonuniform_theta=bool(seed % 2))
+        occ, left, right, y0 = random_plan(o, rng, 5)
+        yfree, _, free = o.master(occ, left, right, y0=y0)
+        pos = yfree[occ == 1]
+        lb, ub = 0.5 * float(np.median(pos)), 0.9 * float(pos.max())      # both bounds bind somewhere
+        y, z, info = o.master(occ, left, right, y0=y0, y_min=lb, y_max=ub)
+        grad, (F, G, cost) = o.cost_gradient(occ, left, right, y)
+        assert np.all(y[occ == 0] == 0) and np.all(y[occ == 1] >= lb) and np.all(y[occ == 1] <= ub)
+        scale = max(1.0, info.pg_entry)
+        for k in np.nonzero(occ)[0]:
+            if y[k] <= lb:
+                assert grad[k] >= -1e-7 * scale
+                hit_lo += 1
+            elif y[k] >= ub:
+                assert grad[k] <= 1e-7 * scale
+                hit_hi += 1
+            else:
+                assert abs(grad[k]) <= 1e-7 * scale
+                inside += 1
+        assert info.cost == pytest.approx(cost, rel=1e-13) and info.cost >= free.cost * (1 - 1e-12)
+        np.testing.assert_allclose(z, o.dose(occ, left, right, y), rtol=1e-12, atol=1e-12)
+    assert hit_lo and hit_hi and inside                                   # the test saw all three cases
+
+
+def test_master_bounds_equal_bounded_least_squares_when_all_quadratic():
+    """alpha = beta everywhere: (3) with fixed apertures and a box on y is a bounded linear least squares.
+    Library routine: scipy.optimize.lsq_linear."""
+    o, D, rng = small_problem(78, V=50, N=6, R=2, C=5, gamma=0.7, nonuniform_theta=True)
+    om = rng.uniform(0.5, 2.0, o.V).astype(np.float32)
+    o = Oracle(o.row_ptr, o.col, o.val, o.T, om, om, o.theta, o.R, o.C, o.delta, o.gamma)
+    occ, left, right, _ = random_plan(o, rng, o.N)
+    Dc = np.einsum("krc,krcv->kv", open_mask(o, occ, left, right), D.reshape(o.N, o.R, o.C, o.V))
+    E = np.zeros((o.N - 1, o.N))
+    for k in range(o.N - 1):
+        s = 1.0 / np.sqrt(o.theta[k + 1] - o.theta[k])
+        E[k, k], E[k, k + 1] = -s, s
+    sq = np.sqrt(om.astype(np.float64))
+    A = np.vstack([sq[:, None] * Dc.T, np.sqrt(o.gamma) * E])
+    b = np.concatenate([sq * o.T.astype(np.float64), np.zeros(o.N - 1)])
+    yfree, _, _ = o.master(occ, left, right, eps=1e-11)
+    lo, hi = float(yfree.min()), float(yfree.max())
+    for lb, ub in ((lo + 0.5 * (hi - lo), np.inf), (0.0, hi - 0.35 * (hi - lo)), (lo + 0.2 * (hi - lo), hi - 0.2 * (hi - lo))):
+        ref = scipy.optimize.lsq_linear(A, b, bounds=(lb, ub), method="bvls", tol=1e-14)
+        y, z, info = o.master(occ, left, right, eps=1e-11, y_min=lb, y_max=ub)
+        assert info.cost == pytest.approx(2.0 * ref.cost, rel=1e-9)       # lsq_linear reports half the squared norm
+        np.testing.assert_allclose(y, ref.x, rtol=1e-5, atol=1e-7)
+        assert np.any(y <= lb * (1 + 1e-12)) or np.any(y >= ub * (1 - 1e-12))   # a bound binds: not the free optimum
+
+
+# ------------------------------------------------------------------------------------------------
 # O8 trajectory invariants on configs[0]
 # ------------------------------------------------------------------------------------------------
 def test_tiny_run_invariants(tiny_phantom, tiny_oracle, tiny_solution):
