@@ -196,6 +196,15 @@ int vmat_master(vmat_plan *plan, vmat_master_stats *out);
  * are enqueued without a host round trip; the call synchronises once at the end.             */
 int vmat_solve(vmat_plan *plan, int32_t max_iters, vmat_solve_stats *out);
 
+/* Variant (PAPER.md:159 names "the maximum and minimum dose rate constraints" and leaves them out of "this
+ * preliminary work"; reading R4): from now on step (e) solves model (3) over the box
+ * y_min <= y_k <= y_max at the occupied beams (un-occupied beams deliver nothing: y_k = 0), by gradient
+ * projection on that box.  Default 0, +infinity = the paper's y >= 0.  Applies to vmat_master, vmat_solve and
+ * vmat_enforce_dose_rate; the plan's y is brought into the box by the next master solve.  A beam that enters
+ * at y_min > 0 changes the cost on entry, so the post-master cost of vmat_solve is guaranteed non-increasing
+ * only for y_min = 0.  Requires 0 <= y_min <= y_max, y_min finite.                                         */
+int vmat_set_dose_rate_bounds(vmat_plan *plan, double y_min, double y_max);
+
 /* Hard dose-rate feasibility after the last aperture ("if the final solution is not
  * feasible, the coefficient gamma in the objective function will be automatically increased and then
  * the intensity for each aperture will be re-optimized till the solution is feasible").  The constraint

@@ -29,7 +29,7 @@ SYMBOLS = (
     "vmat_default_options", "vmat_create", "vmat_destroy", "vmat_get_info", "vmat_dose", "vmat_dose_recompute",
     "vmat_price",
     "vmat_price_spmv", "vmat_leaf_search", "vmat_master", "vmat_enforce_dose_rate", "vmat_solve", "vmat_get_plan", "vmat_set_plan",
-    "vmat_launch_count", "vmat_last_error", "vmat_release_memory",
+    "vmat_launch_count", "vmat_last_error", "vmat_release_memory", "vmat_set_dose_rate_bounds",
 )
 
 _P = C.c_void_p
@@ -109,6 +109,7 @@ def load_library():
     L.vmat_set_plan.argtypes = [_P, _P, _P, _P, _P]
     L.vmat_launch_count.argtypes = [_P]
     L.vmat_release_memory.argtypes = []
+    L.vmat_set_dose_rate_bounds.argtypes = [_P, C.c_double, C.c_double]
     L.vmat_launch_count.restype = C.c_int64
     L.vmat_last_error.argtypes = [_P]
     L.vmat_last_error.restype = C.c_char_p
@@ -315,6 +316,10 @@ class Plan:
         s = _MasterStats()
         self._check(self._L.vmat_master(self._h, C.byref(s)))
         return MasterStats(s.inner, s.backtracks, s.stop_reason, s.pg_entry, s.pg_exit, s.F, s.G, s.cost, s.passes)
+
+    def set_dose_rate_bounds(self, y_min: float = 0.0, y_max: float = float("inf")) -> None:
+        """vmat_set_dose_rate_bounds: the master solves from now on keep y_min <= y_k <= y_max at occupied beams."""
+        self._check(self._L.vmat_set_dose_rate_bounds(self._h, float(y_min), float(y_max)))
 
     def enforce_dose_rate(self, max_variation_per_deg: float, gamma_factor: float = 2.0, tol: float = 1e-6,
                           max_rounds: int = 60) -> dict:

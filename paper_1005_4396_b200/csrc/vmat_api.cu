@@ -416,6 +416,15 @@ int vmat_master(vmat_plan *p, vmat_master_stats *out) {
     return VMAT_OK;
 }
 
+int vmat_set_dose_rate_bounds(vmat_plan *p, double y_min, double y_max) {
+    if (!p) return VMAT_EINVAL;
+    if (!(y_min >= 0.0) || !(y_max >= y_min) || std::isinf(y_min))
+        return fail(p, VMAT_EINVAL, "dose-rate bounds need 0 <= y_min <= y_max, y_min finite");
+    p->y_min = y_min;
+    p->y_max = y_max;
+    return VMAT_OK;
+}
+
 int vmat_enforce_dose_rate(vmat_plan *p, double rho, double factor, double tol, int32_t max_rounds,
                            vmat_rate_stats *out) {
     if (!p) return VMAT_EINVAL;

@@ -45,6 +45,7 @@ struct vmat_plan {
     int64_t Sp = 0;         // S rounded up to a multiple of kChunk (>= kChunk)
     int32_t delta = 0;
     double gamma = 0.0;
+    double y_min = 0.0, y_max = __builtin_huge_val();   // bounds on the dose rates of occupied beams (vmat_set_dose_rate_bounds)
     vmat_options opt{};
     cudaStream_t stream = nullptr;
     int sm_count = 0;

@@ -229,6 +229,7 @@ struct MasterArgs {
     int touch_words;
     int N;
     double gamma, F_out, eps, fx_inv, stall_rel;
+    double lb, ub;              // bounds on the dose rates of occupied beams (default 0, +inf)
     int stall_count;
     float Tmax, abmax;
     int max_inner;
@@ -909,7 +910,9 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     }
     for (int k = tid; k < N; k += kMasterThreads) {
         double yk = a.y[k];
-        if (!a.occ[k] || !(yk > 0.0)) yk = 0.0;
+        if (!a.occ[k]) yk = 0.0;
+        else if (!(yk > a.lb)) yk = a.lb;
+        else if (yk > a.ub) yk = a.ub;
         sm.y[k] = yk;
         sm.d[k] = 0.0;
         sm.rdt[k] = k + 1 < N ? 1.0 / (a.theta[k + 1] - a.theta[k]) : 0.0;
@@ -1070,7 +1073,6 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     mbar_wait(&tile_bar, 0);  // the staged segments have landed (the lists were built while they were in flight)
     const double Tm = (double)a.Tmax, ab = (double)a.abmax, Spd = (double)a.Sp;
 
-    const int G = gridDim.x;
     const int recn = 2 * N + 2;
     unsigned ph = a.phase[0];      // rotation of the records; written by the previous launch, stream ordered
     const unsigned ph_entry = ph;
@@ -1120,6 +1122,11 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     double F = 0.0, Gs = 0.0, Phi = 0.0, pgmax = 0.0, pg_entry = 0.0, tol = 0.0;
     double phi1 = 0.0, Gd = 0.0, tmax = 0.0, qb = 0.0, yb = 0.0, t = 0.0, Gn = 0.0;
     const double c1a = 1e-4, noise = 2e-7;
+    // gradient projection on the box lb <= y_k <= ub (default: y_k >= 0): a beam at a bound whose gradient points
+    // out of the box does not move (the same test with g = -d_k keeps a direction feasible)
+    const double lb = a.lb, ub = a.ub;
+    const bool has_ub = ub < CUDART_INF;   // the default box has no upper face: skip its divisions
+    auto at_bound = [lb, ub](double yk, double g) { return (yk <= lb && g >= 0.0) || (yk >= ub && g <= 0.0); };
     // The stall rule (stop at the fp32 resolution of the cost) is calibrated for warm starts, where a step that
     // lowers the cost by <= stall_rel of it really is the end.  A solve that has already lowered the cost by more
     // than 1 % started far from the optimum: conjugate directions then pass through plateaus of tiny steps before
@@ -1154,7 +1161,8 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
                 const double dv = sm.d[k + 1] - dk;
                 s[3] += dv * dv * sm.rdt[k];
             }
-            if (dk < 0.0) ntl = fmax(ntl, -(yk / (-dk)));
+            if (dk < 0.0) ntl = fmax(ntl, -((yk - lb) / (-dk)));
+            if (has_ub && dk > 0.0) ntl = fmax(ntl, -((ub - yk) / dk));
         }
         ctl_reduce<4>(s, ntl, cred, tog, nw, CT);
         phi1 = s[0];
@@ -1189,7 +1197,10 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
         for (int k = tid; k < N; k += CT) {
             const double yk = sm.y[k], dk = sm.d[k];
             double v = yk + t * dk;
-            if (v < 0.0 || (hit && dk < 0.0 && yk / (-dk) <= tmax)) v = 0.0;
+            if (sm.ik[k] >= 0) {
+                if (v < lb || (hit && dk < 0.0 && (yk - lb) / (-dk) <= tmax)) v = lb;
+                else if (has_ub && (v > ub || (hit && dk > 0.0 && (ub - yk) / dk <= tmax))) v = ub;
+            }
             sm.yn[k] = v;
         }
         ctl_sync(CT);
@@ -1218,7 +1229,10 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
         for (int k = tid; k < N; k += CT) {
             const double yk = sm.y[k], dk = sm.d[k];
             double v = pr ? yk : yk + t * dk;
-            if (!pr && (v < 0.0 || (hit && dk < 0.0 && yk / (-dk) <= tmax))) v = 0.0;
+            if (!pr && sm.ik[k] >= 0) {
+                if (v < lb || (hit && dk < 0.0 && (yk - lb) / (-dk) <= tmax)) v = lb;
+                else if (has_ub && (v > ub || (hit && dk > 0.0 && (ub - yk) / dk <= tmax))) v = ub;
+            }
             sm.yn[k] = v;
         }
         ctl_sync(CT);
@@ -1231,7 +1245,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
             const int i = sm.ik[k];
             const double gmk = i >= 0 ? sm.gF[k] + t * sm.hd[k] + a.gamma * sm.dG[k] : 0.0;
             const double yk = sm.yn[k], po = sm.pg[k];
-            const double pn = (i < 0 || (yk <= 0.0 && gmk >= 0.0)) ? 0.0 : gmk;
+            const double pn = (i < 0 || at_bound(yk, gmk)) ? 0.0 : gmk;
             sm.gm[k] = gmk;
             sm.gn[k] = pn;   // scratch until the pass returns the true gradient
             s[0] += pn * (pn - po);
@@ -1248,7 +1262,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
             for (int k = tid; k < N; k += CT) {
                 const double pn = sm.gn[k], yk = sm.yn[k];
                 double dk = -pn + bpr * sm.d[k];
-                if (sm.ik[k] < 0 || (yk <= 0.0 && dk < 0.0)) dk = 0.0;   // stay feasible
+                if (sm.ik[k] < 0 || at_bound(yk, -dk)) dk = 0.0;   // stay feasible
                 sm.dnx[k] = dk;
                 s2[0] += sm.gm[k] * dk;
                 s2[1] += fabs(dk) * sm.linf[k];
@@ -1294,7 +1308,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
         for (int k = tid; k < N; k += CT) {
             const int i = sm.ik[k];
             const double gk = i >= 0 ? (double)sm.recv[2 + i] * iG + a.gamma * sm.dG[k] : 0.0;
-            const double p = (i < 0 || (sm.y[k] <= 0.0 && gk >= 0.0)) ? 0.0 : gk;
+            const double p = (i < 0 || at_bound(sm.y[k], gk)) ? 0.0 : gk;
             sm.grad[k] = gk;
             if (MODE == 1) {
                 sm.gF[k] = i >= 0 ? (double)sm.recv[2 + i] * iG : 0.0;
@@ -1348,7 +1362,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
                     const double gf = i >= 0 ? (double)sm.recv[2 + i] * iG : 0.0;
                     const double gk = i >= 0 ? gf + a.gamma * sm.dG[k] : 0.0;
                     const double yk = sm.yn[k];
-                    const double pn = (i < 0 || (yk <= 0.0 && gk >= 0.0)) ? 0.0 : gk;
+                    const double pn = (i < 0 || at_bound(yk, gk)) ? 0.0 : gk;
                     sm.gFn[k] = gf;
                     sm.gn[k] = gk;
                     sm.hdn[k] = i >= 0 ? 2.0 * (double)sm.recv[2 + K + i] * iH : 0.0;
@@ -1377,7 +1391,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
                         sm.grad[k] = gk;
                         sm.gF[k] = sm.gFn[k];
                         sm.hd[k] = sm.hdn[k];
-                        sm.pg[k] = (sm.ik[k] < 0 || (yk <= 0.0 && gk >= 0.0)) ? 0.0 : gk;
+                        sm.pg[k] = (sm.ik[k] < 0 || at_bound(yk, gk)) ? 0.0 : gk;
                         sm.d[k] = sm.dnx[k];
                     }
                     ctl_sync(CT);
@@ -1514,7 +1528,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
                     const int i = sm.ik[k];
                     const double gk = i >= 0 ? (double)sm.recv[2 + i] * iG + a.gamma * sm.dG[k] : 0.0;
                     const double yk = sm.yn[k], po = sm.pg[k];
-                    const double pn = (i < 0 || (yk <= 0.0 && gk >= 0.0)) ? 0.0 : gk;
+                    const double pn = (i < 0 || at_bound(yk, gk)) ? 0.0 : gk;
                     sm.gn[k] = gk;
                     s[3] += ((pn == 0.0) != (po == 0.0)) ? 1.0 : 0.0;   // entries entering / leaving the face
                     s[0] += pn * (pn - po);
@@ -1540,9 +1554,9 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
                     for (int k = tid; k < N; k += CT) {
                         const double yk = sm.yn[k], gk = sm.gn[k];
                         const bool off = sm.ik[k] < 0;
-                        const double pn = (off || (yk <= 0.0 && gk >= 0.0)) ? 0.0 : gk;
+                        const double pn = (off || at_bound(yk, gk)) ? 0.0 : gk;
                         double dk = -pn + bpr * sm.d[k];
-                        if (off || (yk <= 0.0 && dk < 0.0)) dk = 0.0;   // stay feasible
+                        if (off || at_bound(yk, -dk)) dk = 0.0;   // stay feasible
                         sm.y[k] = yk;
                         sm.grad[k] = gk;
                         sm.pg[k] = pn;
@@ -1756,6 +1770,8 @@ static int launch_master_impl(vmat_plan *p, int max_inner, int trace_it) {
     a.eps = p->opt.master_eps;
     a.stall_rel = p->opt.master_stall_rel;
     a.stall_count = p->opt.master_stall_count;
+    a.lb = p->y_min;
+    a.ub = p->y_max;
     a.max_inner = max_inner;
     a.rslots = p->master_rslots;
     a.cache_segs = p->master_cache_segs;

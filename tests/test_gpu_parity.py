@@ -284,6 +284,38 @@ def test_master_random_problems(torch_cuda, vm, mode):
         plan.destroy()
 
 
+@pytest.mark.parametrize("mode", [0, 1])
+def test_master_with_dose_rate_bounds_matches_oracle(torch_cuda, vm, tiny_oracle, mode):
+    """Variant of PAPER.md:159 (bounds on the dose rates, vmat_set_dose_rate_bounds): same aperture set, same box =>
+    master cost within 1e-4 of the oracle's box-constrained optimum, y inside the box, both bounds binding."""
+    o = tiny_oracle
+    plan = make_plan(vm, o, options=mode_options(vm, mode))
+    for occ, left, right, y in oracle_states(o, 24, every=8)[1:]:
+        pos = y[np.asarray(occ, bool)]
+        lb, ub = 0.5 * float(np.median(pos)), 0.8 * float(pos.max())
+        y_ref, z_ref, info = o.master(occ, left, right, y0=y, eps=1e-10, y_min=lb, y_max=ub)
+        free = o.master(occ, left, right, y0=y, eps=1e-10)[2]
+        assert info.cost > free.cost * (1 + 1e-6)                          # the box really binds
+        plan.set_dose_rate_bounds(lb, ub)
+        for y0 in (y, np.zeros(o.N)):
+            plan.set_plan(occ, left, right, y0)
+            st = plan.master()
+            assert abs(st.cost - info.cost) <= TOL * abs(info.cost)
+            _, _, _, yg = plan.get_plan()
+            on = np.asarray(occ, bool)
+            assert np.all(yg[~on] == 0) and np.all(yg[on] >= lb) and np.all(yg[on] <= ub)
+            assert np.any(yg[on] == lb) or np.any(yg[on] == ub)
+            _, (_, _, cost_at_y) = o.cost_gradient(occ, left, right, yg)
+            assert cost_at_y <= info.cost * (1 + TOL)
+        # back to the paper's y >= 0: the free optimum again
+        plan.set_dose_rate_bounds(0.0, float("inf"))
+        plan.set_plan(occ, left, right, y)
+        assert abs(plan.master().cost - free.cost) <= TOL * abs(free.cost)
+    with pytest.raises(Exception):
+        plan.set_dose_rate_bounds(2.0, 1.0)
+    plan.destroy()
+
+
 # ------------------------------------------------------------------------------------------------
 # P3: free run of the whole loop
 # ------------------------------------------------------------------------------------------------
