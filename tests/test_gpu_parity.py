@@ -284,6 +284,38 @@ def test_master_random_problems(torch_cuda, vm, mode):
         plan.destroy()
 
 
+def test_master_support_wider_than_one_mask_word(torch_cuda, vm):
+    """A support of 1.35 M voxels gives every master block more than 64 chunks of its own: the touched-chunk masks
+    take two 64-bit words per column, the passes run over several groups with columns partly staged, partly streamed."""
+    from oracle import Oracle
+
+    rng = np.random.default_rng(5)
+    V, N, R, C = 1_500_000, 3, 2, 4
+    B = N * R * C
+    cols, vals, row_ptr = [], [], [0]
+    band = V // B
+    for i in range(B):
+        own = np.arange(i * band, (i + 1) * band if i < B - 1 else V)          # every voxel is in the support
+        keep = own[rng.random(own.size) < 0.9] if i % 5 else own
+        far = rng.choice(V, 4000, replace=False)                               # and a few far ones: wide chunk ranges
+        c = np.unique(np.concatenate([keep, far]))
+        cols.append(c.astype(np.int32))
+        vals.append(rng.uniform(0.05, 1.0, c.size).astype(np.float32))
+        row_ptr.append(row_ptr[-1] + c.size)
+    T = rng.uniform(0.2, 1.0, V).astype(np.float32)
+    alpha = ((rng.random(V) < 0.5) * rng.uniform(0.5, 2.0, V)).astype(np.float32)
+    beta = rng.uniform(0.1, 1.5, V).astype(np.float32)
+    o = Oracle(np.asarray(row_ptr, np.int64), np.concatenate(cols), np.concatenate(vals), T, alpha, beta,
+               np.array([0.0, 2.0, 5.0]), R, C, 2, 0.3)
+    for mode in (0, 1):
+        plan = make_plan(vm, o, options=mode_options(vm, mode))
+        assert plan.n_support > 148 * 64 * 128                                   # more than 64 chunks per block
+        for occ, left, right, y in oracle_states(o, 3, every=1)[1:]:
+            check_master(plan, o, occ, left, right, np.zeros(o.N))
+            check_master(plan, o, occ, left, right, y * 0.5)
+        plan.destroy()
+
+
 @pytest.mark.parametrize("mode", [0, 1])
 def test_master_with_dose_rate_bounds_matches_oracle(torch_cuda, vm, tiny_oracle, mode):
     """Variant of PAPER.md:159 (bounds on the dose rates, vmat_set_dose_rate_bounds): same aperture set, same box =>
