@@ -171,3 +171,20 @@ def test_full_plan_properties(setup):
     plan.set_plan(occ, left, right, np.zeros(o.N))
     cold = plan.master()
     assert abs(cold.cost - cost) <= TOL * abs(cost), (cold, cost)
+    # the single-barrier iteration (master_mode 1) reaches the same optimum on the same apertures, warm and cold
+    opt = vm.default_options()
+    opt.master_mode = 1
+    fused = vm.Plan.from_phantom(ph, options=opt)
+    for y0 in (y, np.zeros(o.N)):
+        fused.set_plan(occ, left, right, y0)
+        m1 = fused.master()
+        assert abs(m1.cost - cost) <= TOL * abs(cost), (m1, cost)
+    # and so does the box-constrained solve once its box is lifted again (vmat_set_dose_rate_bounds)
+    fused.set_dose_rate_bounds(0.25 * float(np.median(y)), 0.9 * float(y.max()))
+    fused.set_plan(occ, left, right, y)
+    boxed = fused.master()
+    _, _, _, yb = fused.get_plan()
+    assert boxed.cost >= cost * (1 - TOL) and np.all(yb >= 0.25 * np.median(y)) and np.all(yb <= 0.9 * y.max())
+    _, (_, _, cost_b) = o.cost_gradient(occ, left, right, yb)
+    assert abs(boxed.cost - cost_b) <= TOL * abs(cost_b)                       # the oracle prices the boxed plan alike
+    fused.destroy()
