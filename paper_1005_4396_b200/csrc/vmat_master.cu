@@ -64,24 +64,28 @@ k_column_scatter(const uint32_t *__restrict__ rowq, const float4 *__restrict__ v
     const int r = idx / C, c = idx - r * C;
     if (c < left[k * R + r] || c >= right[k * R + r]) return;   // beamlet not exposed (A_k)
     const long long row = ((long long)k * R + r) * C + c;
-    // one entry per lane and step, eight steps in flight before the first atomic: the lanes hold consecutive
-    // entries of the row, whose slots come in runs, so the adds of one instruction share 32-byte sectors of the
-    // accumulator and the L2 merges them (half the sector operations of a quad-per-lane layout, vmat_dose.cu)
-    const float *__restrict__ val = reinterpret_cast<const float *>(val4);
-    const int *__restrict__ col = reinterpret_cast<const int *>(col4);
-    const uint32_t a = rowq[row] * 4u, b = rowq[row + 1] * 4u;
-    for (uint32_t e = a + lane; e < b; e += 32 * 8) {
-        float v[8];
-        int s[8];
+    const uint32_t a = rowq[row], b = rowq[row + 1];
+    // four quads per lane in flight before the first atomic (a row is ~100 quads: one round trip, not four)
+    for (uint32_t q = a + lane; q < b; q += 32 * 4) {
+        float4 v[4];
+        int4 s[4];
 #pragma unroll
-        for (int u = 0; u < 8; ++u) {
-            const bool in = e + 32 * u < b;
-            v[u] = in ? __ldg(val + e + 32 * u) : 0.f;
-            s[u] = in ? __ldg(col + e + 32 * u) : 0;
+        for (int u = 0; u < 4; ++u) {
+            if (q + 32 * u < b) {
+                v[u] = __ldg(val4 + q + 32 * u);
+                s[u] = __ldg(col4 + q + 32 * u);
+            } else {
+                v[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+                s[u] = make_int4(0, 0, 0, 0);
+            }
         }
 #pragma unroll
-        for (int u = 0; u < 8; ++u)
-            if (v[u] != 0.f) atomicAdd(acc + s[u], (unsigned long long)__double2ll_rn((double)v[u] * fx_scale));
+        for (int u = 0; u < 4; ++u) {
+            if (v[u].x != 0.f) atomicAdd(acc + s[u].x, (unsigned long long)__double2ll_rn((double)v[u].x * fx_scale));
+            if (v[u].y != 0.f) atomicAdd(acc + s[u].y, (unsigned long long)__double2ll_rn((double)v[u].y * fx_scale));
+            if (v[u].z != 0.f) atomicAdd(acc + s[u].z, (unsigned long long)__double2ll_rn((double)v[u].z * fx_scale));
+            if (v[u].w != 0.f) atomicAdd(acc + s[u].w, (unsigned long long)__double2ll_rn((double)v[u].w * fx_scale));
+        }
     }
 }
 
