@@ -96,6 +96,10 @@ typedef struct {
                                   fused pass and one grid barrier (the next direction is built from the gradient
                                   the quadratic piece predicts at the trial point; the step length and every
                                   acceptance / stop decision use the true gradient).  Same minimiser (S11).  */
+    int32_t stop_when_priced_out; /* vmat_solve stops as soon as the best aperture's price is >= 0 (the textbook
+                                  column-generation stop).  Default 0: the loop goes on until every beam holds an
+                                  aperture, as the paper wants (reading S5).  With 1 the
+                                  call synchronises the stream once per iteration to read the price.             */
 } vmat_options;
 
 /* One deliverable aperture: a beam and one leaf pair per row. */

@@ -552,6 +552,7 @@ typedef struct {
     int64_t max_iters;
     double eps;               /* master tolerance */
     int64_t max_inner;
+    int64_t stop_when_priced_out; /* option of reading S5: stop as soon as the best price is >= 0 */
     /* outputs, arrays caller-allocated with max_iters entries (leaf arrays max_iters*R) */
     int64_t iters;            /* outer iterations done */
     int32_t *beam;            /* chosen beam */
@@ -574,7 +575,9 @@ static double now_s(void) {
  * O1 + O8 column-generation loop (Fig. 1 is missing from the extraction).
  * O1: start from the empty plan, y = 0, z = 0 (reading S1).  Each iteration: gradient (O3),
  * prices (O4, rounded to fp32 for the search), best aperture (O5, O6), occupy that beam with
- * y_k = 0, master (O7).  Stops when every beam is occupied or after max_iters (reading S5).
+ * y_k = 0, master (O7).  Stops when every beam is occupied or after max_iters (reading S5); with
+ * stop_when_priced_out also as soon as no aperture has a negative price (the textbook column-generation
+ * stop, offered as an option because the paper wants an aperture at every angle).
  * State arrays (occ N, left/right N*R, y N, z V) are caller allocated; on entry they hold the
  * plan to continue from (all zero for a fresh run).
  * ------------------------------------------------------------------------------------------ */
@@ -595,6 +598,7 @@ void vo_solve(const vo_problem *p, uint8_t *occ, int32_t *left, int32_t *right, 
         double price = 0.0;
         const int64_t k = vo_price_step(p, g32, occ, left, right, y, &price, bl, br, NULL, NULL, NULL);
         if (k < 0) break;
+        if (tr->stop_when_priced_out && !(price < 0.0)) break;
         occ[k] = 1; y[k] = 0.0;
         memcpy(left + k * R, bl, sizeof(int32_t) * R);
         memcpy(right + k * R, br, sizeof(int32_t) * R);

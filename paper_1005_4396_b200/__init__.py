@@ -44,7 +44,7 @@ class _Problem(C.Structure):
 class Options(C.Structure):
     _fields_ = [("validate", C.c_int32), ("pricing_kernel", C.c_int32), ("dose_path", C.c_int32),
                 ("master_eps", C.c_double), ("master_max_inner", C.c_int32), ("master_stall_rel", C.c_double),
-                ("master_stall_count", C.c_int32), ("record_phases", C.c_int32), ("master_mode", C.c_int32)]
+                ("master_stall_count", C.c_int32), ("record_phases", C.c_int32), ("master_mode", C.c_int32), ("stop_when_priced_out", C.c_int32)]
 
 
 class _Aperture(C.Structure):

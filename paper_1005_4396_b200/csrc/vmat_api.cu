@@ -136,6 +136,7 @@ void vmat_default_options(vmat_options *opt) {
     opt->master_stall_count = 2;
     opt->record_phases = 0;
     opt->master_mode = 0;
+    opt->stop_when_priced_out = 0;
 }
 
 int vmat_create(const vmat_problem *pb, const vmat_options *options, void *cuda_stream, vmat_plan **out) {
@@ -516,17 +517,28 @@ int vmat_solve(vmat_plan *p, int32_t max_iters, vmat_solve_stats *out) {
     TRYC(cudaEventRecord(ev0, st));
     TRY(ensure_state(p));
     TRY(ensure_columns(p));   // the master needs d_k of every occupied beam, whichever path formed z
+    int64_t done = 0;
     for (int64_t it = 0; it < todo; ++it) {
         if (phases) TRYC(cudaEventRecord(evs[it * 5 + 0], st));
         TRY(launch_price_spmv(p, p->w_s, p->g, (int)(n_free0 - it)));              // (c)
         if (phases) TRYC(cudaEventRecord(evs[it * 5 + 1], st));
+        if (p->opt.stop_when_priced_out) {
+            // option of reading S5: look at the best price before committing (one host round trip)
+            TRY(launch_leaf_search(p, p->g, nullptr, nullptr, nullptr, 0, -1));
+            Sel h_sel;
+            TRYC(cudaMemcpyAsync(&h_sel, p->sel, sizeof(Sel), cudaMemcpyDeviceToHost, st));
+            TRYC(cudaStreamSynchronize(st));
+            if (h_sel.beam < 0 || !(h_sel.price < 0.0)) break;
+        }
         TRY(launch_leaf_search(p, p->g, nullptr, nullptr, nullptr, 1, (int)it));   // (d), commits
         if (phases) TRYC(cudaEventRecord(evs[it * 5 + 2], st));
         TRY(launch_column_build(p, -1));                                           // d_k of the new aperture
         if (phases) TRYC(cudaEventRecord(evs[it * 5 + 3], st));
         TRY(launch_master(p, (int)it));                                            // (e), leaves z, w current
         if (phases) TRYC(cudaEventRecord(evs[it * 5 + 4], st));
+        done = it + 1;
     }
+    todo = done;
     TRYC(cudaEventRecord(ev1, st));
     TRYC(cudaStreamSynchronize(st));
     TRYC(cudaGetLastError());

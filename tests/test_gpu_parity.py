@@ -382,6 +382,44 @@ def test_solve_free_run_tiny(torch_cuda, vm, tiny_oracle, tiny_solution, mode):
     plan.destroy()
 
 
+def test_solve_stop_when_priced_out_option(torch_cuda, vm):
+    """Option of reading S5: vmat_solve ends as soon as no aperture has a negative price; the default goes on until
+    every beam holds an aperture.  Same stop iteration, apertures and cost as the oracle's."""
+    from oracle import Oracle
+
+    N, R, C, V = 5, 1, 3, 10
+    rng = np.random.default_rng(11)
+    D = np.zeros((N * R * C, V), np.float32)
+    for i in range(N * R * C):
+        for j in (range(0, 4) if i // C < 2 else range(4, 10)):        # beams 2..4 reach organ-at-risk voxels only
+            if rng.random() < 0.8:
+                D[i, j] = rng.uniform(0.1, 1.0)
+    csr = sp.csr_matrix(D)
+    csr.sort_indices()
+    T = np.array([1.0] * 4 + [0.0] * 6, np.float32)
+    alpha = np.array([1.0] * 4 + [0.0] * 6, np.float32)
+    beta = np.array([1.0] * 4 + [0.7] * 6, np.float32)
+    o = Oracle(csr.indptr.astype(np.int64), csr.indices.astype(np.int32), csr.data.astype(np.float32), T, alpha, beta,
+               np.arange(N) * 2.0, R, C, 3, 0.0)
+    occ_r, left_r, right_r, y_r, z_r, tr = o.solve(10, stop_when_priced_out=True)
+    assert tr.iters == 2
+    opt = vm.default_options()
+    opt.stop_when_priced_out = 1
+    plan = make_plan(vm, o, options=opt)
+    st = plan.solve(10)
+    occ, left, right, y = plan.get_plan()
+    assert st.iters == tr.iters and np.array_equal(st.beam, tr.beam) and np.array_equal(occ, occ_r)
+    assert np.array_equal(left[occ.astype(bool)], left_r[occ_r.astype(bool)])
+    assert np.array_equal(right[occ.astype(bool)], right_r[occ_r.astype(bool)])
+    assert abs(st.cost - tr.cost[-1]) <= TOL * abs(tr.cost[-1])
+    assert plan.solve(10).iters == 0                                      # still priced out: nothing more to do
+    plan.destroy()
+    plan = make_plan(vm, o)                                               # default: an aperture at every angle
+    st = plan.solve(10)
+    assert st.iters == N and plan.get_plan()[0].all()
+    plan.destroy()
+
+
 @pytest.mark.parametrize("mode", [0, 1])
 def test_solve_is_reproducible(torch_cuda, vm, tiny_oracle, mode):
     o = tiny_oracle

@@ -396,6 +396,44 @@ def test_master_equals_nnls_when_all_quadratic():
     np.testing.assert_allclose(y, y_ref, rtol=1e-5, atol=1e-7)
 
 
+def priced_out_problem(gamma=0.0):
+    """Five beams of one row x three beamlets.  Beams 0 and 1 reach the target voxels 0..3 (alpha > 0), beams 2..4
+    only organ-at-risk voxels 4..9 (alpha = 0, T = 0): whatever the dose, w_j >= 0 there, so every aperture of
+    those beams has a price >= 0 and the closed one (price 0) is the best."""
+    N, R, C, V = 5, 1, 3, 10
+    rng = np.random.default_rng(11)
+    D = np.zeros((N * R * C, V), np.float32)
+    for i in range(N * R * C):
+        cols = range(0, 4) if i // C < 2 else range(4, 10)
+        for j in cols:
+            if rng.random() < 0.8:
+                D[i, j] = rng.uniform(0.1, 1.0)
+    csr = scipy.sparse.csr_matrix(D)
+    csr.sort_indices()
+    T = np.array([1.0] * 4 + [0.0] * 6, np.float32)
+    alpha = np.array([1.0] * 4 + [0.0] * 6, np.float32)
+    beta = np.array([1.0] * 4 + [0.7] * 6, np.float32)
+    return Oracle(csr.indptr.astype(np.int64), csr.indices.astype(np.int32), csr.data.astype(np.float32), T, alpha, beta,
+                  np.arange(N) * 2.0, R, C, 3, gamma)
+
+
+def test_solve_stop_when_priced_out_option():
+    """Option of reading S5 (the textbook column-generation stop): the loop ends as soon as no aperture has a
+    negative price.  Default: it goes on until every beam holds an aperture."""
+    o = priced_out_problem()
+    occ, left, right, y, z, tr = o.solve(10, stop_when_priced_out=True)
+    assert tr.iters == 2 and sorted(tr.beam.tolist()) == [0, 1] and np.all(tr.price < 0)
+    assert occ.tolist() == [1, 1, 0, 0, 0]
+    g = o.prices(o.penalty(z)[1], occ)
+    best = o.price_step(g.astype(np.float32), occ, left, right, y)
+    assert best["price"] >= 0.0 and np.all(g[6:] >= 0)                     # nothing prices out at the stop
+    occ2, left2, right2, y2, z2, tr2 = o.solve(10)
+    assert tr2.iters == 5 and occ2.all()                                   # default: an aperture at every angle
+    assert np.array_equal(tr2.beam[:2], tr.beam) and np.array_equal(tr2.cost[:2], tr.cost)
+    assert np.all(tr2.price[2:] >= 0) and np.all(left2[2:] == right2[2:])  # the late apertures are closed ...
+    assert tr2.cost[-1] == pytest.approx(tr.cost[-1], rel=1e-12)           # ... and buy nothing
+
+
 # ------------------------------------------------------------------------------------------------
 # variant: bounds on the dose rates of occupied beams (PAPER.md:159 names "the maximum and minimum dose rate
 # constraints" and leaves them out; SURVEY.md section 8f #4; DESIGN.md reading R4)
