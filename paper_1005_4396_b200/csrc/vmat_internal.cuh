@@ -96,6 +96,7 @@ struct vmat_plan {
     size_t master_smem = 0;
     int master_cache_segs = 0;         // 512-byte segments of Dd a master block stages in shared memory
     int master_rslots = 0;             // slots per master block kept resident in shared memory (0: none)
+    int master_ul_cap = 0;             // capacity of the master's per-chunk lists of unstaged beams (0: masked loops)
     vmat::MasterOut *mout = nullptr;
     double *cost3 = nullptr;       // device {F, G, F+gamma G}
     double *rate_ratio = nullptr;  // device scalar of the dose-rate feasibility test

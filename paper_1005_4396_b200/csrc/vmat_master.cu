@@ -235,6 +235,7 @@ struct MasterArgs {
     int max_inner;
     int rslots;                 // > 0: every block keeps z, q, T, alpha, beta of its own slots in shared memory
     int cache_segs;             // capacity of the shared-memory tile of Dd in 512-byte segments
+    int ul_cap;                 // capacity of the per-chunk lists of unstaged beams (0: they do not fit, masked loops)
     long long *accbuf;          // 3 rotating sets of kSumGroups records of (2N + 2) fixed-point sums: F, curvature,
                                 // grad[0..K), and (fused mode) the Hessian-vector product [K..2K); a block adds
                                 // to the record of its group (blockIdx mod kSumGroups)
@@ -399,6 +400,8 @@ struct Smem {
     int *cseg;         // staged segments chunk by chunk, beams ascending: segment | i << 16
     int *gseg;         // staged segments group by group, beams ascending, then chunks: segment | (j - g kGroup) << 16
     int *unc;          // beams that touch this block's chunks but are not staged, ascending
+    int *uoff, *ul;    // (when a.ul_cap > 0) entries [uoff[j], uoff[j+1]) of ul: the unstaged beams that touch local chunk j
+    long long *gfx;    // (when a.ul_cap > 0) fixed-point gradient sums of the unstaged beams: N for w (+ N for u)
     long long *recv;   // the pass's record of grid sums, fetched by the whole block after the barrier
     Ctl *ctl;
 };
@@ -428,6 +431,120 @@ __device__ __forceinline__ void load_half(const MasterArgs &a, const Smem &sm, i
 #pragma unroll
     for (int h = 0; h < kGroup / 2; ++h)
         v[h] = (m >> (2 * h)) & 1u ? __ldg(row + (size_t)(2 * h * G) * (kChunk / 4)) : make_float4(0.f, 0.f, 0.f, 0.f);
+}
+
+// ---- columns that are not staged, walked through per-chunk lists (sm.ul) when the lists fit --------------
+// Eight independent 16-byte loads per lane and step, every one of them a touched segment: the streaming part of
+// a pass over a large problem is bound by bytes in flight, and the masked loops above keep only the touched
+// fraction (a third) of theirs in flight.
+
+// q-part of chunk j = g*kGroup + cs for this warp's half of the chunk's unstaged beams: adds into s1, s2
+__device__ __forceinline__ void combine_unstaged_listed(const MasterArgs &a, const Smem &sm, int j, int hf, int lane,
+                                                        float4 &s1, float4 &s2) {
+    const float4 *Dd4 = reinterpret_cast<const float4 *>(a.Dd) +
+                        (size_t)((int)blockIdx.x + j * (int)gridDim.x) * (kChunk / 4) + lane;
+    const size_t row4 = (size_t)a.Sp / 4;
+    const int n1 = sm.uoff[j + 1];
+    for (int n = sm.uoff[j] + hf; n < n1; n += 16) {
+        float4 v[8];
+        float c[8];
+#pragma unroll
+        for (int x = 0; x < 8; ++x) {
+            const int nn = n + 2 * x;
+            c[x] = 0.f;
+            v[x] = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (nn < n1) {
+                const int i = sm.ul[nn];
+                c[x] = sm.coef[i];
+                v[x] = __ldg(Dd4 + (size_t)sm.sk[i] * row4);
+            }
+        }
+#pragma unroll
+        for (int x = 0; x < 8; x += 2) {
+            s1.x = fmaf(c[x], v[x].x, s1.x);
+            s1.y = fmaf(c[x], v[x].y, s1.y);
+            s1.z = fmaf(c[x], v[x].z, s1.z);
+            s1.w = fmaf(c[x], v[x].w, s1.w);
+            s2.x = fmaf(c[x + 1], v[x + 1].x, s2.x);
+            s2.y = fmaf(c[x + 1], v[x + 1].y, s2.y);
+            s2.z = fmaf(c[x + 1], v[x + 1].z, s2.z);
+            s2.w = fmaf(c[x + 1], v[x + 1].w, s2.w);
+        }
+    }
+}
+
+// sums of eight values over the warp in nine exchanges: after the exchanges at 16, 8 and 4 each lane carries one
+// of the eight; lane L ends with the total of value ((L >> 4) & 1) * 4 + ((L >> 3) & 1) * 2 + ((L >> 2) & 1)
+__device__ __forceinline__ double warp_sum8(double (&v)[8], int lane) {
+    const bool b16 = lane & 16, b8 = lane & 8, b4 = lane & 4;
+#pragma unroll
+    for (int x = 0; x < 4; ++x) {
+        const double keep = b16 ? v[x + 4] : v[x], send = b16 ? v[x] : v[x + 4];
+        v[x] = keep + __shfl_xor_sync(kFull, send, 16);
+    }
+#pragma unroll
+    for (int x = 0; x < 2; ++x) {
+        const double keep = b8 ? v[x + 2] : v[x], send = b8 ? v[x] : v[x + 2];
+        v[x] = keep + __shfl_xor_sync(kFull, send, 8);
+    }
+    const double keep = b4 ? v[1] : v[0], send = b4 ? v[0] : v[1];
+    double r = keep + __shfl_xor_sync(kFull, send, 4);
+    r += __shfl_xor_sync(kFull, r, 2);
+    r += __shfl_xor_sync(kFull, r, 1);
+    return r;
+}
+
+// Gradient dots of the unstaged beams of group g: warp (cs, hf) takes every second entry of chunk g*kGroup + cs,
+// eight beams per step; lane partials over 4 products in fp32, the warp sums in fp64 (warp_sum8), then into the
+// beam's FIXED-POINT accumulator in shared memory (integer adds: order free, so the result stays reproducible
+// although several warps add to one beam).  sm.gfx holds N entries for w and, TWO, N more for u.
+template <bool TWO>
+__device__ __forceinline__ void grad_unstaged_listed(const MasterArgs &a, const Smem &sm, int g, double scG, double scH) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int cs = warp & (kGroup - 1), hf = warp / kGroup, j = g * kGroup + cs;
+    const int n1 = sm.uoff[j + 1];
+    int n = sm.uoff[j] + hf;
+    if (n >= n1) return;
+    const float4 w4 = reinterpret_cast<const float4 *>(sm.wbuf)[cs * kSeg4 + lane];
+    float4 u4 = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (TWO) u4 = reinterpret_cast<const float4 *>(sm.ubuf)[cs * kSeg4 + lane];
+    const float4 *Dd4 = reinterpret_cast<const float4 *>(a.Dd) +
+                        (size_t)((int)blockIdx.x + j * (int)gridDim.x) * (kChunk / 4) + lane;
+    const size_t row4 = (size_t)a.Sp / 4;
+    const int mine = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);   // warp_sum8's layout
+    for (; n < n1; n += 16) {
+        float4 v[8];
+        int id[8];
+#pragma unroll
+        for (int x = 0; x < 8; ++x) {
+            const int nn = n + 2 * x;
+            id[x] = -1;
+            v[x] = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (nn < n1) {
+                id[x] = sm.ul[nn];
+                v[x] = __ldg(Dd4 + (size_t)sm.sk[id[x]] * row4);
+            }
+        }
+        double dw[8], du[8];
+#pragma unroll
+        for (int x = 0; x < 8; ++x) {
+            dw[x] = (double)((v[x].x * w4.x + v[x].y * w4.y) + (v[x].z * w4.z + v[x].w * w4.w));
+            if (TWO) du[x] = (double)((v[x].x * u4.x + v[x].y * u4.y) + (v[x].z * u4.z + v[x].w * u4.w));
+        }
+        const double rw = warp_sum8(dw, lane);
+        double ru = 0.0;
+        if (TWO) ru = warp_sum8(du, lane);
+        int my_id = -1;
+#pragma unroll
+        for (int x = 0; x < 8; ++x)
+            if (x == mine) my_id = id[x];
+        if ((lane & 3) == 0 && my_id >= 0) {
+            atomicAdd(reinterpret_cast<unsigned long long *>(sm.gfx) + my_id, (unsigned long long)__double2ll_rn(rw * scG));
+            if (TWO)
+                atomicAdd(reinterpret_cast<unsigned long long *>(sm.gfx) + a.N + my_id,
+                          (unsigned long long)__double2ll_rn(ru * scH));
+        }
+    }
 }
 
 // value[o] = sum_i coef[i] * Dd[sk[i]][slot(o)] for the kGroup*128 slots of group g, o = tid + r*kMasterThreads.
@@ -467,7 +584,9 @@ __device__ __forceinline__ void combine_group(const MasterArgs &a, const Smem &s
             s1.z = fmaf(c1, v1.z, s1.z);
             s1.w = fmaf(c1, v1.w, s1.w);
         }
-        if (Ku > 0) {
+        if (Ku > 0 && a.ul_cap > 0) {
+            combine_unstaged_listed(a, sm, g * kGroup + cs, hf, lane, s1, s2);
+        } else if (Ku > 0) {
             // columns that are not staged: same split, four beams per step, one float4 of the chunk per lane
             // straight from L2 / HBM; a beam that does not touch the chunk is skipped (warp-uniform test)
             const int j = g * kGroup + cs;
@@ -586,6 +705,8 @@ __device__ __forceinline__ void eval_pass(const MasterArgs &a, const Smem &sm, i
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int kpart = warp & (kKSplit - 1), chalf = warp / kKSplit;
     for (int i = tid; i < 2 * a.N; i += kMasterThreads) sm.gacc[i] = 0.0;
+    if (a.ul_cap > 0)
+        for (int i = tid; i < a.N; i += kMasterThreads) sm.gfx[i] = 0;
     double F = 0.0;
     __syncthreads();
     PROFX(8)
@@ -619,10 +740,12 @@ __device__ __forceinline__ void eval_pass(const MasterArgs &a, const Smem &sm, i
         __syncthreads();
         PROFX(9)
         grad_staged<false>(sm, g);
-        // columns that are not staged: this warp's half of the group's gradient (4 chunks), and its share of those beams: two beams
-        // per step (eight independent loads), lane partials in fp32 (16 products), the warp sum in fp64; the
-        // partial dot goes to the row of sm.gacc that belongs to this chunk half
-        if (Ku > 0) {
+        // columns that are not staged: through the per-chunk lists when they fit; otherwise this warp's half of the
+        // group's gradient (4 chunks), and its share of those beams: two beams per step (eight masked loads), lane
+        // partials in fp32 (16 products), the warp sum in fp64 to the row of sm.gacc of this chunk half
+        if (Ku > 0 && a.ul_cap > 0) {
+            grad_unstaged_listed<false>(a, sm, g, scG, 0.0);
+        } else if (Ku > 0) {
         float4 w4[kGroup / 2];
 #pragma unroll
         for (int h = 0; h < kGroup / 2; ++h) w4[h] = reinterpret_cast<const float4 *>(sm.wbuf)[(2 * h + chalf) * kSeg4 + lane];
@@ -663,7 +786,11 @@ __device__ __forceinline__ void eval_pass(const MasterArgs &a, const Smem &sm, i
     PROFX(11)
     F = block_sum(F, red);
     if (tid == 0) fx_add(rec, F, scF);
-    for (int i = tid; i < K; i += kMasterThreads) fx_add(rec + 2 + i, grad_total(sm, sm.gpart, i, a.N, 0), scG);
+    for (int i = tid; i < K; i += kMasterThreads) {
+        if (a.ul_cap > 0 && sm.base[i] == kNoCache)   // already in fixed point
+            atomicAdd(reinterpret_cast<unsigned long long *>(rec + 2 + i), (unsigned long long)sm.gfx[i]);
+        else fx_add(rec + 2 + i, grad_total(sm, sm.gpart, i, a.N, 0), scG);
+    }
     PROFX(11)
 }
 
@@ -685,6 +812,8 @@ __device__ __forceinline__ void fused_pass(const MasterArgs &a, const Smem &sm, 
     long long pt_ = 0, pacc_[16] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
 #endif
     for (int i = tid; i < 4 * a.N; i += kMasterThreads) sm.gacc[i] = 0.0;
+    if (a.ul_cap > 0)
+        for (int i = tid; i < 2 * a.N; i += kMasterThreads) sm.gfx[i] = 0;
     double F = 0.0, curv = 0.0;
     __syncthreads();
     for (int g = 0; g < ngroups; ++g) {
@@ -727,9 +856,12 @@ __device__ __forceinline__ void fused_pass(const MasterArgs &a, const Smem &sm, 
         }
         __syncthreads();
         grad_staged<true>(sm, g);
-        // columns that are not staged: this warp's half of the group (4 chunks) and its share of those beams: two beams per step, each
-        // row read once for both products; lane partials in fp32, warp sums in fp64 by one butterfly for all four
-        if (Ku > 0) {
+        // columns that are not staged: through the per-chunk lists when they fit; otherwise this warp's half of the
+        // group (4 chunks) and its share of those beams: two beams per step, each row read once for both products;
+        // lane partials in fp32, warp sums in fp64 by one butterfly for all four
+        if (Ku > 0 && a.ul_cap > 0) {
+            grad_unstaged_listed<true>(a, sm, g, scG, scH);
+        } else if (Ku > 0) {
         float4 w4[kGroup / 2], u4[kGroup / 2];
 #pragma unroll
         for (int h = 0; h < kGroup / 2; ++h) {
@@ -781,8 +913,13 @@ __device__ __forceinline__ void fused_pass(const MasterArgs &a, const Smem &sm, 
         fx_add(rec + 1, curv, scC);
     }
     for (int i = tid; i < K; i += kMasterThreads) {
-        fx_add(rec + 2 + i, grad_total(sm, sm.gpart, i, a.N, 0), scG);
-        fx_add(rec + 2 + K + i, grad_total(sm, sm.gpartu, i, a.N, 2), scH);
+        if (a.ul_cap > 0 && sm.base[i] == kNoCache) {   // already in fixed point
+            atomicAdd(reinterpret_cast<unsigned long long *>(rec + 2 + i), (unsigned long long)sm.gfx[i]);
+            atomicAdd(reinterpret_cast<unsigned long long *>(rec + 2 + K + i), (unsigned long long)sm.gfx[a.N + i]);
+        } else {
+            fx_add(rec + 2 + i, grad_total(sm, sm.gpart, i, a.N, 0), scG);
+            fx_add(rec + 2 + K + i, grad_total(sm, sm.gpartu, i, a.N, 2), scH);
+        }
     }
 }
 
@@ -873,7 +1010,8 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     const int ngroups = (a.nchunks + (int)gridDim.x * kGroup - 1) / ((int)gridDim.x * kGroup);
     const int W64 = (ngroups * kGroup + 63) >> 6;   // 64-bit words of a column's local chunk mask
     sm.lmask = reinterpret_cast<unsigned long long *>(sm.gpartu + F1 * 2 * a.cache_segs);
-    double *red = reinterpret_cast<double *>(sm.lmask + (size_t)W64 * N);
+    sm.gfx = reinterpret_cast<long long *>(sm.lmask + (size_t)W64 * N);
+    double *red = reinterpret_cast<double *>(sm.gfx + (a.ul_cap > 0 ? (1 + F1) * N : 0));
     double *cred = red + kMasterWarps;   // 2 x kMasterWarps x kRedSlots
     sm.recv = reinterpret_cast<long long *>(cred + 2 * kMasterWarps * kRedSlots);
     sm.ctl = reinterpret_cast<Ctl *>(sm.recv + 2 * N + 2);
@@ -888,6 +1026,8 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     sm.gseg = sm.cseg + a.cache_segs;
     sm.nseg = sm.gseg + a.cache_segs;
     sm.coff = sm.nseg + N;   // ngroups * kGroup + 1
+    sm.uoff = sm.coff + ngroups * kGroup + 1;   // the same, if a.ul_cap > 0
+    sm.ul = sm.uoff + ngroups * kGroup + 1;     // a.ul_cap
     __shared__ int sK, sKu, sSegs;
     __shared__ uint64_t tile_bar;
 
@@ -1017,8 +1157,32 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
             c += __popc(__ballot_sync(kFull, f));
         }
         if (lane == 0) sm.coff[j + 1] = c;
+        if (a.ul_cap > 0) {   // and the unstaged beams that touch it
+            int cu = 0;
+            for (int i0 = 0; i0 < K; i0 += 32) {
+                const int i = i0 + lane;
+                const bool f = i < K && sm.base[i] == kNoCache && touches(sm, N, i, j);
+                cu += __popc(__ballot_sync(kFull, f));
+            }
+            if (lane == 0) sm.uoff[j + 1] = cu;
+        }
     }
     __syncthreads();
+    if (warp == 1 && a.ul_cap > 0) {   // running sums of the unstaged lists
+        int run = 0;
+        for (int j0 = 0; j0 < nj; j0 += 32) {
+            const int j = j0 + lane;
+            int incl = j < nj ? sm.uoff[j + 1] : 0;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int n = __shfl_up_sync(kFull, incl, o);
+                if (lane >= o) incl += n;
+            }
+            if (j < nj) sm.uoff[j + 1] = run + incl;
+            run += __shfl_sync(kFull, incl, 31);
+        }
+        if (lane == 0) sm.uoff[0] = 0;
+    }
     if (warp == 0) {   // running sums: coff[j] = first entry of chunk j
         int run = 0;
         for (int j0 = 0; j0 < nj; j0 += 32) {
@@ -1043,6 +1207,16 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
             const unsigned m = __ballot_sync(kFull, f);
             if (f) sm.cseg[pos + __popc(m & ((1u << lane) - 1u))] = (sm.base[i] + seg_rank(sm, N, i, j)) | (i << 16);
             pos += __popc(m);
+        }
+        if (a.ul_cap > 0) {
+            int pu = sm.uoff[j];
+            for (int i0 = 0; i0 < K; i0 += 32) {
+                const int i = i0 + lane;
+                const bool f = i < K && sm.base[i] == kNoCache && touches(sm, N, i, j);
+                const unsigned m = __ballot_sync(kFull, f);
+                if (f) sm.ul[pu + __popc(m & ((1u << lane) - 1u))] = i;
+                pu += __popc(m);
+            }
         }
     }
     for (int g = warp; g < ngroups; g += kMasterWarps) {   // group by group, beams ascending, then chunks
@@ -1664,13 +1838,14 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
 // shared memory of one master block; mode 1 (single-barrier iteration) lays out more (k_master's carve-up)
 size_t seg_bytes(int mode) { return kSeg * 4 + (mode == 1 ? 2 : 1) * 2 * 8 + 2 * 4; }   // tile, gpart (+ gpartu), cseg + gseg
 
-size_t master_smem_bytes(int64_t N, int64_t rslots, int64_t cache_segs, int64_t ngroups, int mode) {
+size_t master_smem_bytes(int64_t N, int64_t rslots, int64_t cache_segs, int64_t ngroups, int mode, int64_t ul_cap) {
     const int f1 = mode == 1 ? 1 : 0;
     return (size_t)(2 * kGroup * kChunk + (1 + f1) * kGroup * kSeg + (6 + f1) * rslots) * 4   // part2, wbuf (ubuf), resident slots
            + (size_t)cache_segs * seg_bytes(mode)                                            // tile and the lists over it
            + (size_t)((13 + 8 * f1) * N + 2 * N + 2 + kMasterWarps + 2 * kMasterWarps * kRedSlots) * 8 + sizeof(Ctl)   // K-vectors, recv, red, cred, ctl
            + (size_t)N * 4 * 8 + (size_t)(ngroups * kGroup + 1) * 4           // coef, sk, lo, hi, ik, base, unc, nseg; coff
-           + (size_t)((ngroups * kGroup + 63) / 64) * N * 8;                  // lmask
+           + (size_t)((ngroups * kGroup + 63) / 64) * N * 8                   // lmask
+           + (ul_cap > 0 ? (size_t)ul_cap * 4 + (size_t)(ngroups * kGroup + 1) * 4 + (size_t)(1 + f1) * N * 8 : 0);   // ul, uoff, gfx
 }
 
 }  // namespace
@@ -1691,11 +1866,20 @@ int master_configure(vmat_plan *p) {
     VMAT_CUDA(p, cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, p->device));
     const size_t budget = (size_t)optin > 8 * 1024 ? (size_t)optin - 8 * 1024 : 0;
     const int mode = p->opt.master_mode;
-    size_t fixed = master_smem_bytes(p->N, rslots, 0, ngroups, mode);
+    // per-chunk lists of the unstaged beams (one entry per column and local chunk at most) if they fit in 64 KB
+    int64_t ul_cap = p->N * ngroups * kGroup;
+    if (ul_cap * 4 > 64 * 1024) ul_cap = 0;
+    if (getenv("VMAT_MASTER_MASKED_LOOPS")) ul_cap = 0;   // debugging aid: force the fallback path (tests)
+    size_t fixed = master_smem_bytes(p->N, rslots, 0, ngroups, mode, ul_cap);
     if (fixed > budget) {
         p->master_rslots = 0;
-        fixed = master_smem_bytes(p->N, 0, 0, ngroups, mode);
+        fixed = master_smem_bytes(p->N, 0, 0, ngroups, mode, ul_cap);
     }
+    if (fixed > budget) {
+        ul_cap = 0;
+        fixed = master_smem_bytes(p->N, 0, 0, ngroups, mode, 0);
+    }
+    p->master_ul_cap = (int)ul_cap;
     if (fixed > budget) return fail(p, VMAT_EINVAL, "n_beams too large for the master kernel's shared memory");
     p->master_cache_segs = (int)((budget - fixed) / seg_bytes(mode));
     if (p->master_cache_segs > 65535 || ngroups * kGroup > 32767) p->master_cache_segs = 0;   // 16-bit fields of the lists
@@ -1703,7 +1887,7 @@ int master_configure(vmat_plan *p) {
     if (getenv("VMAT_NO_TILE")) p->master_cache_segs = 0;
     fprintf(stderr, "master: grid %d smem fixed %zu cache_segs %d rslots %d\n", p->master_grid, fixed, p->master_cache_segs, p->master_rslots);
 #endif
-    p->master_smem = master_smem_bytes(p->N, p->master_rslots, p->master_cache_segs, ngroups, mode);
+    p->master_smem = master_smem_bytes(p->N, p->master_rslots, p->master_cache_segs, ngroups, mode, ul_cap);
     VMAT_CUDA(p, cudaFuncSetAttribute(k_master<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->master_smem));
     VMAT_CUDA(p, cudaFuncSetAttribute(k_master<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->master_smem));
     int per_sm = 0, per_sm1 = 0;
@@ -1775,6 +1959,7 @@ static int launch_master_impl(vmat_plan *p, int max_inner, int trace_it) {
     a.max_inner = max_inner;
     a.rslots = p->master_rslots;
     a.cache_segs = p->master_cache_segs;
+    a.ul_cap = p->master_ul_cap;
     a.colstat = p->colstat;
     a.touch = p->col_touch;
     a.touch_words = p->touch_words;

@@ -188,3 +188,16 @@ def test_full_plan_properties(setup):
     _, (_, _, cost_b) = o.cost_gradient(occ, left, right, yb)
     assert abs(boxed.cost - cost_b) <= TOL * abs(cost_b)                       # the oracle prices the boxed plan alike
     fused.destroy()
+    # the fallback of the unstaged columns (masked loops, taken when their per-chunk lists do not fit in shared
+    # memory) is forced by an environment variable read at vmat_create
+    import os
+
+    os.environ["VMAT_MASTER_MASKED_LOOPS"] = "1"
+    try:
+        masked = vm.Plan.from_phantom(ph)
+    finally:
+        del os.environ["VMAT_MASTER_MASKED_LOOPS"]
+    masked.set_plan(occ, left, right, np.zeros(o.N))
+    mm = masked.master()
+    assert abs(mm.cost - cost) <= TOL * abs(cost), (mm, cost)
+    masked.destroy()
