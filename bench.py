@@ -422,7 +422,7 @@ def main():
         "frac": m_gbs / peak, "traffic": None, "algorithmic_bytes_per_step": m_bytes, "passes_per_step": m_passes,
         "us_per_pass": ph_us["master"] / m_passes if m_passes else None, "launches_per_step": iters,
         "note": "latency bound: two grid barriers and two control steps per inner iteration "
-                "(profiles/r01c_master.md); bytes = touched column segments x passes, device-counted",
+                "(profiles/r01d_master.md); bytes = touched column segments x passes, device-counted",
     }
     phases = {k + "_us_per_step": v for k, v in ph_us.items()}
     phases["master_inner_iterations_per_step"] = inner_total / args.steps
