@@ -400,7 +400,8 @@ struct Smem {
     int *cseg;         // staged segments chunk by chunk, beams ascending: segment | i << 16
     int *gseg;         // staged segments group by group, beams ascending, then chunks: segment | (j - g kGroup) << 16
     int *unc;          // beams that touch this block's chunks but are not staged, ascending
-    int *uoff, *ul;    // (when a.ul_cap > 0) entries [uoff[j], uoff[j+1]) of ul: the unstaged beams that touch local chunk j
+    int *uoff;         // (when a.ul_cap > 0) entries [uoff[j], uoff[j+1]) of ul: the unstaged beams that touch local chunk j
+    unsigned short *ul;
     long long *gfx;    // (when a.ul_cap > 0) fixed-point gradient sums of the unstaged beams: N for w (+ N for u)
     long long *recv;   // the pass's record of grid sums, fetched by the whole block after the barrier
     Ctl *ctl;
@@ -1027,7 +1028,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     sm.nseg = sm.gseg + a.cache_segs;
     sm.coff = sm.nseg + N;   // ngroups * kGroup + 1
     sm.uoff = sm.coff + ngroups * kGroup + 1;   // the same, if a.ul_cap > 0
-    sm.ul = sm.uoff + ngroups * kGroup + 1;     // a.ul_cap
+    sm.ul = reinterpret_cast<unsigned short *>(sm.uoff + ngroups * kGroup + 1);   // a.ul_cap 16-bit beam numbers, last array
     __shared__ int sK, sKu, sSegs;
     __shared__ uint64_t tile_bar;
 
@@ -1214,7 +1215,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
                 const int i = i0 + lane;
                 const bool f = i < K && sm.base[i] == kNoCache && touches(sm, N, i, j);
                 const unsigned m = __ballot_sync(kFull, f);
-                if (f) sm.ul[pu + __popc(m & ((1u << lane) - 1u))] = i;
+                if (f) sm.ul[pu + __popc(m & ((1u << lane) - 1u))] = (unsigned short)i;
                 pu += __popc(m);
             }
         }
@@ -1845,7 +1846,7 @@ size_t master_smem_bytes(int64_t N, int64_t rslots, int64_t cache_segs, int64_t 
            + (size_t)((13 + 8 * f1) * N + 2 * N + 2 + kMasterWarps + 2 * kMasterWarps * kRedSlots) * 8 + sizeof(Ctl)   // K-vectors, recv, red, cred, ctl
            + (size_t)N * 4 * 8 + (size_t)(ngroups * kGroup + 1) * 4           // coef, sk, lo, hi, ik, base, unc, nseg; coff
            + (size_t)((ngroups * kGroup + 63) / 64) * N * 8                   // lmask
-           + (ul_cap > 0 ? (size_t)ul_cap * 4 + (size_t)(ngroups * kGroup + 1) * 4 + (size_t)(1 + f1) * N * 8 : 0);   // ul, uoff, gfx
+           + (ul_cap > 0 ? (size_t)ul_cap * 2 + 16 + (size_t)(ngroups * kGroup + 1) * 4 + (size_t)(1 + f1) * N * 8 : 0);   // ul, uoff, gfx
 }
 
 }  // namespace
@@ -1856,10 +1857,12 @@ int master_configure(vmat_plan *p) {
     if (grid > nchunks) grid = nchunks;
     if (grid < 1) grid = 1;
     p->master_grid = (int)grid;
-    // resident slot data (z, z trial, q, T, alpha, beta of a block's own slots) if it fits in 96 KB
+    // resident slot data (z, z trial, q, T, alpha, beta of a block's own slots) if it fits in 128 KB: on a large
+    // support the tile holds a few per cent of the columns whatever its size, while slot data read from L2 / HBM
+    // costs every group of every pass a round trip
     const int64_t ngroups = (nchunks + grid * kGroup - 1) / (grid * kGroup);
     int64_t rslots = ngroups * kGroup * kChunk;
-    if (rslots * 7 * 4 > 96 * 1024) rslots = 0;
+    if (rslots * (p->opt.master_mode == 1 ? 7 : 6) * 4 > 128 * 1024) rslots = 0;
     p->master_rslots = (int)rslots;
     // what is left of the SM's opt-in shared memory (minus static use and room for L1) holds the tile of Dd
     int optin = 0;
@@ -1868,7 +1871,7 @@ int master_configure(vmat_plan *p) {
     const int mode = p->opt.master_mode;
     // per-chunk lists of the unstaged beams (one entry per column and local chunk at most) if they fit in 64 KB
     int64_t ul_cap = p->N * ngroups * kGroup;
-    if (ul_cap * 4 > 64 * 1024) ul_cap = 0;
+    if (ul_cap * 2 > 64 * 1024 || p->N > 65535) ul_cap = 0;
     if (getenv("VMAT_MASTER_MASKED_LOOPS")) ul_cap = 0;   // debugging aid: force the fallback path (tests)
     size_t fixed = master_smem_bytes(p->N, rslots, 0, ngroups, mode, ul_cap);
     if (fixed > budget) {
