@@ -400,6 +400,8 @@ struct Smem {
     int *cseg;         // staged segments chunk by chunk, beams ascending: segment | i << 16
     int *gseg;         // staged segments group by group, beams ascending, then chunks: segment | (j - g kGroup) << 16
     int *unc;          // beams that touch this block's chunks but are not staged, ascending
+    int *wst;          // ngroups x (kGroup + 1): warps wst[g][cs] .. wst[g][cs+1]-1 share chunk cs of group g, in proportion to
+                       // the work its lists hold (a staged entry counts 1, an unstaged one 4); fixed per solve
     int *uoff;         // (when a.ul_cap > 0) entries [uoff[j], uoff[j+1]) of ul: the unstaged beams that touch local chunk j
     unsigned short *ul;
     long long *gfx;    // (when a.ul_cap > 0) fixed-point gradient sums of the unstaged beams: N for w (+ N for u)
@@ -439,37 +441,51 @@ __device__ __forceinline__ void load_half(const MasterArgs &a, const Smem &sm, i
 // a pass over a large problem is bound by bytes in flight, and the masked loops above keep only the touched
 // fraction (a third) of theirs in flight.
 
-// q-part of chunk j = g*kGroup + cs for this warp's half of the chunk's unstaged beams: adds into s1, s2
-__device__ __forceinline__ void combine_unstaged_listed(const MasterArgs &a, const Smem &sm, int j, int hf, int lane,
+// this warp's chunk cs of group g, its rank r among the c warps that share the chunk (c = 0: the warp is idle)
+__device__ __forceinline__ void warp_share(const Smem &sm, int g, int warp, int &cs, int &r, int &c) {
+    const int *w = sm.wst + g * (kGroup + 1);
+    cs = 0;
+    r = c = 0;
+#pragma unroll
+    for (int x = 0; x < kGroup; ++x)
+        if (w[x] <= warp && warp < w[x + 1]) {
+            cs = x;
+            r = warp - w[x];
+            c = w[x + 1] - w[x];
+        }
+}
+
+// q-part of chunk j for rank r of the c warps that share the chunk's unstaged beams: adds into s1, s2
+__device__ __forceinline__ void combine_unstaged_listed(const MasterArgs &a, const Smem &sm, int j, int r, int c, int lane,
                                                         float4 &s1, float4 &s2) {
     const float4 *Dd4 = reinterpret_cast<const float4 *>(a.Dd) +
                         (size_t)((int)blockIdx.x + j * (int)gridDim.x) * (kChunk / 4) + lane;
     const size_t row4 = (size_t)a.Sp / 4;
     const int n1 = sm.uoff[j + 1];
-    for (int n = sm.uoff[j] + hf; n < n1; n += 16) {
+    for (int n = sm.uoff[j] + r; n < n1; n += 8 * c) {
         float4 v[8];
-        float c[8];
+        float f[8];
 #pragma unroll
         for (int x = 0; x < 8; ++x) {
-            const int nn = n + 2 * x;
-            c[x] = 0.f;
+            const int nn = n + c * x;
+            f[x] = 0.f;
             v[x] = make_float4(0.f, 0.f, 0.f, 0.f);
             if (nn < n1) {
                 const int i = sm.ul[nn];
-                c[x] = sm.coef[i];
+                f[x] = sm.coef[i];
                 v[x] = __ldg(Dd4 + (size_t)sm.sk[i] * row4);
             }
         }
 #pragma unroll
         for (int x = 0; x < 8; x += 2) {
-            s1.x = fmaf(c[x], v[x].x, s1.x);
-            s1.y = fmaf(c[x], v[x].y, s1.y);
-            s1.z = fmaf(c[x], v[x].z, s1.z);
-            s1.w = fmaf(c[x], v[x].w, s1.w);
-            s2.x = fmaf(c[x + 1], v[x + 1].x, s2.x);
-            s2.y = fmaf(c[x + 1], v[x + 1].y, s2.y);
-            s2.z = fmaf(c[x + 1], v[x + 1].z, s2.z);
-            s2.w = fmaf(c[x + 1], v[x + 1].w, s2.w);
+            s1.x = fmaf(f[x], v[x].x, s1.x);
+            s1.y = fmaf(f[x], v[x].y, s1.y);
+            s1.z = fmaf(f[x], v[x].z, s1.z);
+            s1.w = fmaf(f[x], v[x].w, s1.w);
+            s2.x = fmaf(f[x + 1], v[x + 1].x, s2.x);
+            s2.y = fmaf(f[x + 1], v[x + 1].y, s2.y);
+            s2.z = fmaf(f[x + 1], v[x + 1].z, s2.z);
+            s2.w = fmaf(f[x + 1], v[x + 1].w, s2.w);
         }
     }
 }
@@ -502,9 +518,11 @@ __device__ __forceinline__ double warp_sum8(double (&v)[8], int lane) {
 template <bool TWO>
 __device__ __forceinline__ void grad_unstaged_listed(const MasterArgs &a, const Smem &sm, int g, double scG, double scH) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int cs = warp & (kGroup - 1), hf = warp / kGroup, j = g * kGroup + cs;
-    const int n1 = sm.uoff[j + 1];
-    int n = sm.uoff[j] + hf;
+    int cs, r, c;
+    warp_share(sm, g, warp, cs, r, c);
+    if (c == 0) return;
+    const int j = g * kGroup + cs, n1 = sm.uoff[j + 1];
+    int n = sm.uoff[j] + r;
     if (n >= n1) return;
     const float4 w4 = reinterpret_cast<const float4 *>(sm.wbuf)[cs * kSeg4 + lane];
     float4 u4 = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -513,12 +531,12 @@ __device__ __forceinline__ void grad_unstaged_listed(const MasterArgs &a, const 
                         (size_t)((int)blockIdx.x + j * (int)gridDim.x) * (kChunk / 4) + lane;
     const size_t row4 = (size_t)a.Sp / 4;
     const int mine = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);   // warp_sum8's layout
-    for (; n < n1; n += 16) {
+    for (; n < n1; n += 8 * c) {
         float4 v[8];
         int id[8];
 #pragma unroll
         for (int x = 0; x < 8; ++x) {
-            const int nn = n + 2 * x;
+            const int nn = n + c * x;
             id[x] = -1;
             v[x] = make_float4(0.f, 0.f, 0.f, 0.f);
             if (nn < n1) {
@@ -558,13 +576,14 @@ __device__ __forceinline__ void combine_group(const MasterArgs &a, const Smem &s
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     PROFX_START
     {
-        const int cs = warp & (kGroup - 1), hf = warp / kGroup;
-        const int n1 = sm.coff[g * kGroup + cs + 1];
-        int n = sm.coff[g * kGroup + cs] + hf;
+        int cs, r, c;
+        warp_share(sm, g, warp, cs, r, c);
+        const int n1 = c ? sm.coff[g * kGroup + cs + 1] : 0;
+        int n = c ? sm.coff[g * kGroup + cs] + r : 0;
         const float4 *tile4 = reinterpret_cast<const float4 *>(sm.tile) + lane;
         float4 s1 = make_float4(0.f, 0.f, 0.f, 0.f), s2 = s1;
-        for (; n + 2 < n1; n += 4) {
-            const int e1 = sm.cseg[n], e2 = sm.cseg[n + 2];
+        for (; n + c < n1; n += 2 * c) {
+            const int e1 = sm.cseg[n], e2 = sm.cseg[n + c];
             const float c1 = sm.coef[e1 >> 16], c2 = sm.coef[e2 >> 16];
             const float4 v1 = tile4[(e1 & 0xffff) * kSeg4], v2 = tile4[(e2 & 0xffff) * kSeg4];
             s1.x = fmaf(c1, v1.x, s1.x);
@@ -585,8 +604,9 @@ __device__ __forceinline__ void combine_group(const MasterArgs &a, const Smem &s
             s1.z = fmaf(c1, v1.z, s1.z);
             s1.w = fmaf(c1, v1.w, s1.w);
         }
-        if (Ku > 0 && a.ul_cap > 0) {
-            combine_unstaged_listed(a, sm, g * kGroup + cs, hf, lane, s1, s2);
+        if (c == 0) {
+        } else if (Ku > 0 && a.ul_cap > 0) {
+            combine_unstaged_listed(a, sm, g * kGroup + cs, r, c, lane, s1, s2);
         } else if (Ku > 0) {
             // columns that are not staged: same split, four beams per step, one float4 of the chunk per lane
             // straight from L2 / HBM; a beam that does not touch the chunk is skipped (warp-uniform test)
@@ -594,36 +614,36 @@ __device__ __forceinline__ void combine_group(const MasterArgs &a, const Smem &s
             const float4 *Dd4 = reinterpret_cast<const float4 *>(a.Dd) +
                                 (size_t)((int)blockIdx.x + j * (int)gridDim.x) * (kChunk / 4) + lane;
             const size_t row4 = (size_t)a.Sp / 4;
-            for (int u = hf; u < Ku; u += 8) {
+            for (int u = r; u < Ku; u += 4 * c) {
                 float4 v[4];
-                float c[4];
+                float f[4];
 #pragma unroll
                 for (int x = 0; x < 4; ++x) {
-                    const int uu = u + 2 * x;
-                    c[x] = 0.f;
+                    const int uu = u + c * x;
+                    f[x] = 0.f;
                     v[x] = make_float4(0.f, 0.f, 0.f, 0.f);
                     if (uu < Ku) {
                         const int i = sm.unc[uu];
                         if (touches(sm, a.N, i, j)) {
-                            c[x] = sm.coef[i];
+                            f[x] = sm.coef[i];
                             v[x] = __ldg(Dd4 + (size_t)sm.sk[i] * row4);
                         }
                     }
                 }
 #pragma unroll
                 for (int x = 0; x < 4; x += 2) {
-                    s1.x = fmaf(c[x], v[x].x, s1.x);
-                    s1.y = fmaf(c[x], v[x].y, s1.y);
-                    s1.z = fmaf(c[x], v[x].z, s1.z);
-                    s1.w = fmaf(c[x], v[x].w, s1.w);
-                    s2.x = fmaf(c[x + 1], v[x + 1].x, s2.x);
-                    s2.y = fmaf(c[x + 1], v[x + 1].y, s2.y);
-                    s2.z = fmaf(c[x + 1], v[x + 1].z, s2.z);
-                    s2.w = fmaf(c[x + 1], v[x + 1].w, s2.w);
+                    s1.x = fmaf(f[x], v[x].x, s1.x);
+                    s1.y = fmaf(f[x], v[x].y, s1.y);
+                    s1.z = fmaf(f[x], v[x].z, s1.z);
+                    s1.w = fmaf(f[x], v[x].w, s1.w);
+                    s2.x = fmaf(f[x + 1], v[x + 1].x, s2.x);
+                    s2.y = fmaf(f[x + 1], v[x + 1].y, s2.y);
+                    s2.z = fmaf(f[x + 1], v[x + 1].z, s2.z);
+                    s2.w = fmaf(f[x + 1], v[x + 1].w, s2.w);
                 }
             }
         }
-        reinterpret_cast<float4 *>(sm.part2)[(hf * kGroup + cs) * 32 + lane] =
+        reinterpret_cast<float4 *>(sm.part2)[warp * 32 + lane] =
             make_float4(s1.x + s2.x, s1.y + s2.y, s1.z + s2.z, s1.w + s2.w);
     }
     PROFX(12)
@@ -631,7 +651,10 @@ __device__ __forceinline__ void combine_group(const MasterArgs &a, const Smem &s
 #pragma unroll
     for (int r = 0; r < kOutPerThread; ++r) {
         const int o = tid + r * kMasterThreads, ch = o >> 7, s = o & (kChunk - 1);
-        out[r] = sm.part2[ch * kChunk + s] + sm.part2[(kGroup + ch) * kChunk + s];
+        const int w0 = sm.wst[g * (kGroup + 1) + ch], w1 = sm.wst[g * (kGroup + 1) + ch + 1];
+        float v = 0.f;
+        for (int w = w0; w < w1; ++w) v += sm.part2[w * kChunk + s];   // the chunk's warps, in order
+        out[r] = v;
     }
     PROFX(13)
 }
@@ -1027,7 +1050,8 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     sm.gseg = sm.cseg + a.cache_segs;
     sm.nseg = sm.gseg + a.cache_segs;
     sm.coff = sm.nseg + N;   // ngroups * kGroup + 1
-    sm.uoff = sm.coff + ngroups * kGroup + 1;   // the same, if a.ul_cap > 0
+    sm.wst = sm.coff + ngroups * kGroup + 1;    // ngroups * (kGroup + 1)
+    sm.uoff = sm.wst + ngroups * (kGroup + 1);  // like coff, if a.ul_cap > 0
     sm.ul = reinterpret_cast<unsigned short *>(sm.uoff + ngroups * kGroup + 1);   // a.ul_cap 16-bit beam numbers, last array
     __shared__ int sK, sKu, sSegs;
     __shared__ uint64_t tile_bar;
@@ -1245,6 +1269,50 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     }
     __syncthreads();
     const int Ku = sKu;
+    // the kMasterWarps warps are dealt to the chunks of every group in proportion to the work their lists hold (a
+    // staged entry = 1, an unstaged one = 4; without lists every chunk walks all Ku unstaged beams), at least one
+    // warp per chunk that has any: chunk lists differ several-fold in length and a pass waits for its slowest warp
+    for (int g = tid; g < ngroups; g += kMasterThreads) {
+        int wgt[kGroup], w[kGroup], tot = 0, sum = 0;
+#pragma unroll
+        for (int cs = 0; cs < kGroup; ++cs) {
+            const int j = g * kGroup + cs;
+            int v = sm.coff[j + 1] - sm.coff[j];
+            if (a.ul_cap > 0) v += 4 * (sm.uoff[j + 1] - sm.uoff[j]);
+            else if (chunk_of(g, cs) < a.nchunks) v += 4 * Ku;
+            wgt[cs] = v;
+            tot += v;
+        }
+#pragma unroll
+        for (int cs = 0; cs < kGroup; ++cs) {
+            w[cs] = wgt[cs] > 0 ? max(1, (kMasterWarps * wgt[cs]) / tot) : 0;
+            sum += w[cs];
+        }
+        while (sum > kMasterWarps) {   // take from the chunk with the most warps
+            int b = 0;
+#pragma unroll
+            for (int cs = 1; cs < kGroup; ++cs)
+                if (w[cs] > w[b]) b = cs;
+            --w[b];
+            --sum;
+        }
+        while (tot > 0 && sum < kMasterWarps) {   // give to the chunk with the most work per warp
+            int b = -1;
+#pragma unroll
+            for (int cs = 0; cs < kGroup; ++cs)
+                if (w[cs] > 0 && (b < 0 || (long long)wgt[cs] * w[b] > (long long)wgt[b] * w[cs])) b = cs;
+            ++w[b];
+            ++sum;
+        }
+        int run = 0;
+#pragma unroll
+        for (int cs = 0; cs < kGroup; ++cs) {
+            sm.wst[g * (kGroup + 1) + cs] = run;
+            run += w[cs];
+        }
+        sm.wst[g * (kGroup + 1) + kGroup] = run;
+    }
+    __syncthreads();
     mbar_wait(&tile_bar, 0);  // the staged segments have landed (the lists were built while they were in flight)
     const double Tm = (double)a.Tmax, ab = (double)a.abmax, Spd = (double)a.Sp;
 
@@ -1845,6 +1913,7 @@ size_t master_smem_bytes(int64_t N, int64_t rslots, int64_t cache_segs, int64_t 
            + (size_t)cache_segs * seg_bytes(mode)                                            // tile and the lists over it
            + (size_t)((13 + 8 * f1) * N + 2 * N + 2 + kMasterWarps + 2 * kMasterWarps * kRedSlots) * 8 + sizeof(Ctl)   // K-vectors, recv, red, cred, ctl
            + (size_t)N * 4 * 8 + (size_t)(ngroups * kGroup + 1) * 4           // coef, sk, lo, hi, ik, base, unc, nseg; coff
+           + (size_t)ngroups * (kGroup + 1) * 4                               // wst
            + (size_t)((ngroups * kGroup + 63) / 64) * N * 8                   // lmask
            + (ul_cap > 0 ? (size_t)ul_cap * 2 + 16 + (size_t)(ngroups * kGroup + 1) * 4 + (size_t)(1 + f1) * N * 8 : 0);   // ul, uoff, gfx
 }
