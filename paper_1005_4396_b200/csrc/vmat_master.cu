@@ -5,8 +5,9 @@
 //   penalty gradient       w_j = -2 alpha_j max(0,T_j-z_j) + 2 beta_j max(0,z_j-T_j)      (Eq. 1)
 //   master problem         min_{y>=0} F(z(y)) + gamma G(y), gradient projection (Eq. 3)
 //
-// Layout: the columns are DENSE rows over the support of D, Dd[k][slot], fp32,
-// cut into chunks of 128 slots (one warp of float4).  Each column carries the range of chunks it
+// Layout: the columns are DENSE over the support of D, fp32, cut into chunks of 128 slots
+// (one warp of float4) and stored CHUNK-MAJOR, Dd[chunk][k][128]: the segments of all columns for one chunk are
+// neighbours in memory, so a block that walks a chunk's beams streams one contiguous region.  Each column carries the range of chunks it
 // touches, so both products of one inner iteration — q = Dc^T d (per slot) and grad = Dc w (per
 // beam) — skip the part of a row that is all zero.  Chunks are dealt to the blocks round-robin
 // (the touched slots cluster in the slabs the apertures irradiate), a block works on groups of
@@ -94,8 +95,8 @@ k_column_scatter(const uint32_t *__restrict__ rowq, const float4 *__restrict__ v
 // last chunk with a non-zero entry.  One block = 256 slots = 2 chunks.
 __global__ void __launch_bounds__(256)
 k_column_finish(unsigned long long *__restrict__ acc, long long Sp, const Sel *__restrict__ sel, int beam,
-                double fx_inv, float *__restrict__ Dd, ColStat *__restrict__ colstat, uint32_t *__restrict__ touch,
-                int touch_words) {
+                double fx_inv, float *__restrict__ Dd, int N, ColStat *__restrict__ colstat,
+                uint32_t *__restrict__ touch, int touch_words) {
     const int k = sel ? sel->beam : beam;
     if (k < 0) return;
     __shared__ unsigned long long s_sum[8], s_max[8];
@@ -104,7 +105,7 @@ k_column_finish(unsigned long long *__restrict__ acc, long long Sp, const Sel *_
     unsigned long long mag = 0ull;
     if (s < Sp) {
         const long long v = (long long)acc[s];
-        Dd[(size_t)k * Sp + s] = (float)((double)v * fx_inv);
+        Dd[((size_t)(s / kChunk) * N + k) * kChunk + (s & (kChunk - 1))] = (float)((double)v * fx_inv);   // chunk-major
         acc[s] = 0ull;
         mag = (unsigned long long)(v < 0 ? -v : v);
     }
@@ -429,11 +430,11 @@ __device__ __forceinline__ void load_half(const MasterArgs &a, const Smem &sm, i
                                           float4 (&v)[kGroup / 2]) {
     const unsigned m = ((unsigned)(sm.lmask[((g * kGroup) >> 6) * a.N + i] >> ((g * kGroup) & 63)) & 0xffu) >> chalf;
     const int j0 = g * kGroup + chalf, G = (int)gridDim.x;
-    const float4 *row = reinterpret_cast<const float4 *>(a.Dd + (size_t)sm.sk[i] * a.Sp) +
-                        (size_t)((int)blockIdx.x + j0 * G) * (kChunk / 4) + lane;
+    const float4 *row = reinterpret_cast<const float4 *>(a.Dd) +
+                        ((size_t)((int)blockIdx.x + j0 * G) * a.N + sm.sk[i]) * (kChunk / 4) + lane;
 #pragma unroll
     for (int h = 0; h < kGroup / 2; ++h)
-        v[h] = (m >> (2 * h)) & 1u ? __ldg(row + (size_t)(2 * h * G) * (kChunk / 4)) : make_float4(0.f, 0.f, 0.f, 0.f);
+        v[h] = (m >> (2 * h)) & 1u ? __ldg(row + (size_t)(2 * h * G) * a.N * (kChunk / 4)) : make_float4(0.f, 0.f, 0.f, 0.f);
 }
 
 // ---- columns that are not staged, walked through per-chunk lists (sm.ul) when the lists fit --------------
@@ -459,8 +460,8 @@ __device__ __forceinline__ void warp_share(const Smem &sm, int g, int warp, int 
 __device__ __forceinline__ void combine_unstaged_listed(const MasterArgs &a, const Smem &sm, int j, int r, int c, int lane,
                                                         float4 &s1, float4 &s2) {
     const float4 *Dd4 = reinterpret_cast<const float4 *>(a.Dd) +
-                        (size_t)((int)blockIdx.x + j * (int)gridDim.x) * (kChunk / 4) + lane;
-    const size_t row4 = (size_t)a.Sp / 4;
+                        (size_t)((int)blockIdx.x + j * (int)gridDim.x) * a.N * (kChunk / 4) + lane;   // the chunk's segments
+    const size_t row4 = kChunk / 4;
     const int n1 = sm.uoff[j + 1];
     for (int n = sm.uoff[j] + r; n < n1; n += 8 * c) {
         float4 v[8];
@@ -528,8 +529,8 @@ __device__ __forceinline__ void grad_unstaged_listed(const MasterArgs &a, const 
     float4 u4 = make_float4(0.f, 0.f, 0.f, 0.f);
     if (TWO) u4 = reinterpret_cast<const float4 *>(sm.ubuf)[cs * kSeg4 + lane];
     const float4 *Dd4 = reinterpret_cast<const float4 *>(a.Dd) +
-                        (size_t)((int)blockIdx.x + j * (int)gridDim.x) * (kChunk / 4) + lane;
-    const size_t row4 = (size_t)a.Sp / 4;
+                        (size_t)((int)blockIdx.x + j * (int)gridDim.x) * a.N * (kChunk / 4) + lane;   // the chunk's segments
+    const size_t row4 = kChunk / 4;
     const int mine = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);   // warp_sum8's layout
     for (; n < n1; n += 8 * c) {
         float4 v[8];
@@ -612,8 +613,8 @@ __device__ __forceinline__ void combine_group(const MasterArgs &a, const Smem &s
             // straight from L2 / HBM; a beam that does not touch the chunk is skipped (warp-uniform test)
             const int j = g * kGroup + cs;
             const float4 *Dd4 = reinterpret_cast<const float4 *>(a.Dd) +
-                                (size_t)((int)blockIdx.x + j * (int)gridDim.x) * (kChunk / 4) + lane;
-            const size_t row4 = (size_t)a.Sp / 4;
+                                (size_t)((int)blockIdx.x + j * (int)gridDim.x) * a.N * (kChunk / 4) + lane;
+            const size_t row4 = kChunk / 4;
             for (int u = r; u < Ku; u += 4 * c) {
                 float4 v[4];
                 float f[4];
@@ -1152,11 +1153,11 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
                 const int bs = sm.base[i];
                 if (bs == kNoCache) continue;
                 const int j0 = sm.lo[i], j1 = sm.hi[i];
-                const float *src = a.Dd + (size_t)sm.sk[i] * a.Sp;
+                const float *src = a.Dd + (size_t)sm.sk[i] * kChunk;
                 int q = 0;
                 for (int j = j0; j <= j1; ++j)
                     if (touches(sm, N, i, j))
-                        bulk_g2s(sm.tile + (size_t)(bs + q++) * kSeg, src + (size_t)(b + j * G) * kChunk, kChunk * 4, &tile_bar);
+                        bulk_g2s(sm.tile + (size_t)(bs + q++) * kSeg, src + (size_t)(b + j * G) * N * kChunk, kChunk * 4, &tile_bar);
             }
         }
         __syncthreads();          // sm.base visible to all warps
@@ -1998,7 +1999,7 @@ int launch_column_build(vmat_plan *p, int beam) {
     k_column_scatter<<<blocks, 256, 0, p->stream>>>(p->rowq, p->val4, p->col4, sel, beam, p->left, p->right, (int)p->R,
                                                    (int)p->C, p->fx_scale, p->acc, p->colstat, p->col_touch, p->touch_words);
     k_column_finish<<<(unsigned)((p->Sp + 255) / 256), 256, 0, p->stream>>>(p->acc, (long long)p->Sp, sel, beam,
-                                                                          p->fx_inv, p->Dd, p->colstat, p->col_touch, p->touch_words);
+                                                                          p->fx_inv, p->Dd, (int)p->N, p->colstat, p->col_touch, p->touch_words);
     p->launches += 2;
     VMAT_CUDA(p, cudaGetLastError());
     return VMAT_OK;
