@@ -316,6 +316,57 @@ def test_master_support_wider_than_one_mask_word(torch_cuda, vm):
         plan.destroy()
 
 
+def test_master_with_unstaged_columns_over_several_groups(torch_cuda, vm):
+    """40 beams whose columns touch most of a 400,000-voxel support: every master block owns about 21 chunks (three
+    groups) and about 800 touched column segments, three times what its shared-memory tile holds, so most columns run
+    through the lists of unstaged beams (eight segments in flight per lane, fixed-point beam sums)."""
+    from oracle import Oracle
+
+    rng = np.random.default_rng(9)
+    V, N, R, C = 400_000, 40, 1, 2
+    B = N * R * C
+    cols, vals, row_ptr = [], [], [0]
+    for i in range(B):
+        c = np.nonzero(rng.random(V) < 0.2)[0]
+        if i == 0:
+            c = np.arange(V)                                               # the support is the whole grid
+        cols.append(c.astype(np.int32))
+        vals.append(rng.uniform(0.05, 1.0, c.size).astype(np.float32))
+        row_ptr.append(row_ptr[-1] + c.size)
+    T = rng.uniform(2.0, 8.0, V).astype(np.float32)
+    alpha = ((rng.random(V) < 0.5) * rng.uniform(0.5, 2.0, V)).astype(np.float32)
+    beta = rng.uniform(0.1, 1.5, V).astype(np.float32)
+    o = Oracle(np.asarray(row_ptr, np.int64), np.concatenate(cols), np.concatenate(vals), T, alpha, beta,
+               np.arange(N) * 3.0, R, C, 2, 0.3)
+    occ, left, right, _ = o.empty_plan()
+    occ[:] = 1
+    left = np.zeros((N, R), np.int32)
+    right = np.full((N, R), C, np.int32)                                   # every beamlet exposed
+    import os
+
+    for mode, masked in ((0, False), (1, False), (0, True), (1, True)):
+        # masked: the fallback loops over the unstaged columns (taken when their lists do not fit), forced by an
+        # environment variable that vmat_create reads
+        if masked:
+            os.environ["VMAT_MASTER_MASKED_LOOPS"] = "1"
+        try:
+            plan = make_plan(vm, o, options=mode_options(vm, mode))
+        finally:
+            os.environ.pop("VMAT_MASTER_MASKED_LOOPS", None)
+        st = check_master(plan, o, occ, left, right, np.zeros(N))
+        assert st.inner > 3
+        check_master(plan, o, occ, left, right, rng.uniform(0.0, 2.0, N))
+        # dose and gradient of the GPU's y against the oracle, through the same columns
+        _, _, _, y = plan.get_plan()
+        z = torch_cuda.empty(o.V, dtype=torch_cuda.float32, device="cuda")
+        w = torch_cuda.empty(o.V, dtype=torch_cuda.float32, device="cuda")
+        plan.dose(z, w)
+        z_ref = o.dose(occ, left, right, y)
+        assert relnorm(z.cpu().numpy(), z_ref) <= TOL
+        assert relnorm(w.cpu().numpy(), o.penalty(z_ref)[1]) <= TOL
+        plan.destroy()
+
+
 @pytest.mark.parametrize("mode", [0, 1])
 def test_master_with_dose_rate_bounds_matches_oracle(torch_cuda, vm, tiny_oracle, mode):
     """Variant of PAPER.md:159 (bounds on the dose rates, vmat_set_dose_rate_bounds): same aperture set, same box =>
