@@ -154,6 +154,29 @@ int dev_alloc(vmat_plan *p, T **out, int64_t count) {
     return VMAT_OK;
 }
 
+// Programmatic dependent launch: a kernel launched with launch_pdl may be scheduled while the previous kernel of the
+// stream is still draining (provided that one has called pdl_trigger, or exited); it must call pdl_wait() before it
+// touches anything earlier kernels wrote.  Used on the chain of short dependent kernels of an outer iteration
+// (pricing -> leaf search -> column scatter -> column finish), where the launch gaps weigh as much as the kernels.
+template <typename... KArgs, typename... Args>
+cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, cudaStream_t stream, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+#endif
+
 // vmat_layout.cu: validation and the device layout of D ------------------------------------------
 int build_layout(vmat_plan *p, const vmat_problem *pb);
 

@@ -46,6 +46,8 @@ k_column_scatter(const uint32_t *__restrict__ rowq, const float4 *__restrict__ v
                  const Sel *__restrict__ sel, int beam, const int32_t *__restrict__ left,
                  const int32_t *__restrict__ right, int R, int C, double fx_scale, unsigned long long *__restrict__ acc,
                  ColStat *__restrict__ colstat, uint32_t *__restrict__ touch, int touch_words) {
+    pdl_wait();      // the leaf search's choice
+    pdl_trigger();   // k_column_finish may be scheduled; it waits for the accumulator itself
     const int k = sel ? sel->beam : beam;
     if (k < 0) return;
     if (blockIdx.x == 0) {   // statistics and touched-chunk bitmap of the column, filled by k_column_finish
@@ -97,6 +99,7 @@ __global__ void __launch_bounds__(256)
 k_column_finish(unsigned long long *__restrict__ acc, long long Sp, const Sel *__restrict__ sel, int beam,
                 double fx_inv, float *__restrict__ Dd, int N, ColStat *__restrict__ colstat,
                 uint32_t *__restrict__ touch, int touch_words) {
+    pdl_wait();      // the scatter's adds
     const int k = sel ? sel->beam : beam;
     if (k < 0) return;
     __shared__ unsigned long long s_sum[8], s_max[8];
@@ -1996,10 +1999,11 @@ int master_configure(vmat_plan *p) {
 int launch_column_build(vmat_plan *p, int beam) {
     const Sel *sel = beam < 0 ? p->sel : nullptr;
     const unsigned blocks = (unsigned)((p->RC + 7) / 8);
-    k_column_scatter<<<blocks, 256, 0, p->stream>>>(p->rowq, p->val4, p->col4, sel, beam, p->left, p->right, (int)p->R,
-                                                   (int)p->C, p->fx_scale, p->acc, p->colstat, p->col_touch, p->touch_words);
-    k_column_finish<<<(unsigned)((p->Sp + 255) / 256), 256, 0, p->stream>>>(p->acc, (long long)p->Sp, sel, beam,
-                                                                          p->fx_inv, p->Dd, (int)p->N, p->colstat, p->col_touch, p->touch_words);
+    VMAT_CUDA(p, launch_pdl(k_column_scatter, dim3(blocks), dim3(256), p->stream, p->rowq, p->val4, p->col4, sel, beam, p->left,
+                            p->right, (int)p->R, (int)p->C, p->fx_scale, p->acc, p->colstat, p->col_touch, p->touch_words));
+    VMAT_CUDA(p, launch_pdl(k_column_finish, dim3((unsigned)((p->Sp + 255) / 256)), dim3(256), p->stream, p->acc,
+                            (long long)p->Sp, sel, beam, p->fx_inv, p->Dd, (int)p->N, p->colstat, p->col_touch,
+                            p->touch_words));
     p->launches += 2;
     VMAT_CUDA(p, cudaGetLastError());
     return VMAT_OK;

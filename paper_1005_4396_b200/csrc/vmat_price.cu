@@ -38,6 +38,7 @@ __global__ void __launch_bounds__(kPriceThreads)
 k_price_spmv(const uint32_t *__restrict__ rowq, const float4 *__restrict__ val4, const int4 *__restrict__ col4,
              const float *__restrict__ w, const int32_t *__restrict__ free_list, int blocks_per_beam, int RC,
              float *__restrict__ g) {
+    pdl_trigger();   // the leaf search may be scheduled while this grid drains; it waits for g itself
     constexpr int kRowsPerBlock = kPriceThreads / LANES;
     const int lane = threadIdx.x & (LANES - 1);
     const int beam = free_list[blockIdx.x / blocks_per_beam];

@@ -153,6 +153,8 @@ struct SearchArgs {
 
 template <int M>
 __global__ void __launch_bounds__(kSearchThreads) k_leaf_search(const SearchArgs a) {
+    pdl_wait();      // the prices (launched behind the pricing product by programmatic dependent launch)
+    pdl_trigger();   // the column build may be scheduled; it waits for the choice itself
     __shared__ int s_km, s_kp, s_last;
     __shared__ unsigned long long s_total;
     __shared__ double s_price[kSearchThreads];
@@ -345,14 +347,14 @@ int launch_leaf_search(vmat_plan *p, const float *g, int32_t *all_left, int32_t 
     const int M = (int)((p->C + 1 + 31) / 32);
     const dim3 grid((unsigned)(p->N * ((p->R + kRowsPerBlock - 1) / kRowsPerBlock))), block(kSearchThreads);
     switch (M) {
-        case 1: k_leaf_search<1><<<grid, block, 0, p->stream>>>(a); break;
-        case 2: k_leaf_search<2><<<grid, block, 0, p->stream>>>(a); break;
-        case 3: k_leaf_search<3><<<grid, block, 0, p->stream>>>(a); break;
-        case 4: k_leaf_search<4><<<grid, block, 0, p->stream>>>(a); break;
-        case 5: k_leaf_search<5><<<grid, block, 0, p->stream>>>(a); break;
-        case 6: k_leaf_search<6><<<grid, block, 0, p->stream>>>(a); break;
-        case 7: k_leaf_search<7><<<grid, block, 0, p->stream>>>(a); break;
-        case 8: k_leaf_search<8><<<grid, block, 0, p->stream>>>(a); break;
+        case 1: VMAT_CUDA(p, launch_pdl(k_leaf_search<1>, grid, block, p->stream, a)); break;
+        case 2: VMAT_CUDA(p, launch_pdl(k_leaf_search<2>, grid, block, p->stream, a)); break;
+        case 3: VMAT_CUDA(p, launch_pdl(k_leaf_search<3>, grid, block, p->stream, a)); break;
+        case 4: VMAT_CUDA(p, launch_pdl(k_leaf_search<4>, grid, block, p->stream, a)); break;
+        case 5: VMAT_CUDA(p, launch_pdl(k_leaf_search<5>, grid, block, p->stream, a)); break;
+        case 6: VMAT_CUDA(p, launch_pdl(k_leaf_search<6>, grid, block, p->stream, a)); break;
+        case 7: VMAT_CUDA(p, launch_pdl(k_leaf_search<7>, grid, block, p->stream, a)); break;
+        case 8: VMAT_CUDA(p, launch_pdl(k_leaf_search<8>, grid, block, p->stream, a)); break;
         default: return fail(p, VMAT_EINVAL, "n_cols exceeds VMAT_MAX_COLS");
     }
     ++p->launches;
