@@ -35,6 +35,7 @@ struct DoseScale {
 __global__ void __launch_bounds__(kDoseThreads)
 k_dose_prepare(const uint8_t *__restrict__ occ, const double *__restrict__ y, const double *__restrict__ theta, int N,
                double fx_scale, DoseScale *__restrict__ out) {
+    pdl_trigger();   // the scatter may be scheduled; it waits for the scale itself
     __shared__ double s_max[kDoseThreads / 32], s_sum[kDoseThreads / 32];
     double mx = 0.0, g = 0.0;
     for (int k = threadIdx.x; k < N; k += kDoseThreads) {
@@ -77,6 +78,8 @@ k_dose_scatter(const uint32_t *__restrict__ rowq, const float4 *__restrict__ val
                const uint8_t *__restrict__ occ, const int32_t *__restrict__ left, const int32_t *__restrict__ right,
                const double *__restrict__ y, int R, int C, long long B, const DoseScale *__restrict__ ds,
                unsigned long long *__restrict__ acc) {
+    pdl_wait();
+    pdl_trigger();
     const int lane = threadIdx.x & (kDoseLanes - 1);
     const long long row = (long long)blockIdx.x * (kDoseThreads / kDoseLanes) + threadIdx.x / kDoseLanes;
     if (row >= B) return;
@@ -114,6 +117,8 @@ __global__ void __launch_bounds__(kDoseThreads)
 k_dose_finish(unsigned long long *__restrict__ acc, long long Sp, const DoseScale *__restrict__ ds,
               const float *__restrict__ T, const float *__restrict__ alpha, const float *__restrict__ beta,
               float *__restrict__ z, float *__restrict__ w, double *__restrict__ partF) {
+    pdl_wait();
+    pdl_trigger();
     __shared__ double s_sum[kDoseThreads / 32];
     const long long s = (long long)blockIdx.x * kDoseThreads + threadIdx.x;
     double F = 0.0;
@@ -141,6 +146,7 @@ k_dose_finish(unsigned long long *__restrict__ acc, long long Sp, const DoseScal
 __global__ void __launch_bounds__(kDoseThreads)
 k_dose_cost(const double *__restrict__ partF, int nblocks, double F_out, double gamma, const DoseScale *__restrict__ ds,
             double *__restrict__ cost3) {
+    pdl_wait();
     __shared__ double s_sum[kDoseThreads];
     double f = 0.0;
     for (int i = threadIdx.x; i < nblocks; i += kDoseThreads) f += partF[i];
@@ -175,13 +181,13 @@ int launch_direct_dose(vmat_plan *p) {
     if (p->B > 0) {
         const int rows_per_block = kDoseThreads / kDoseLanes;
         const unsigned blocks = (unsigned)((p->B + rows_per_block - 1) / rows_per_block);
-        k_dose_scatter<<<blocks, kDoseThreads, 0, p->stream>>>(p->rowq, p->val4, p->col4, p->occ, p->left, p->right, p->y,
-                                                              (int)p->R, (int)p->C, (long long)p->B, ds, p->acc);
+        VMAT_CUDA(p, launch_pdl(k_dose_scatter, dim3(blocks), dim3(kDoseThreads), p->stream, p->rowq, p->val4, p->col4, p->occ,
+                                p->left, p->right, p->y, (int)p->R, (int)p->C, (long long)p->B, ds, p->acc));
     }
-    k_dose_finish<<<(unsigned)p->dose_blocks, kDoseThreads, 0, p->stream>>>(p->acc, (long long)p->Sp, ds, p->T_s,
-                                                                           p->alpha_s, p->beta_s, p->z_s, p->w_s,
-                                                                           p->part_dose);
-    k_dose_cost<<<1, kDoseThreads, 0, p->stream>>>(p->part_dose, p->dose_blocks, p->F_out, p->gamma, ds, p->cost3);
+    VMAT_CUDA(p, launch_pdl(k_dose_finish, dim3((unsigned)p->dose_blocks), dim3(kDoseThreads), p->stream, p->acc,
+                            (long long)p->Sp, ds, p->T_s, p->alpha_s, p->beta_s, p->z_s, p->w_s, p->part_dose));
+    VMAT_CUDA(p, launch_pdl(k_dose_cost, dim3(1), dim3(kDoseThreads), p->stream, p->part_dose, p->dose_blocks, p->F_out,
+                            p->gamma, ds, p->cost3));
     p->launches += 4;
     VMAT_CUDA(p, cudaGetLastError());
     return VMAT_OK;
