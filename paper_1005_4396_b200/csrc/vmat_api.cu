@@ -272,6 +272,7 @@ int vmat_create(const vmat_problem *pb, const vmat_options *options, void *cuda_
     p->h_occ.assign((size_t)N, 0);
     p->col_valid.assign((size_t)N, 0);
     p->state_valid = false;
+    p->warm_ok = false;
     *out = p;
     return VMAT_OK;
 }
@@ -390,6 +391,7 @@ int vmat_price(vmat_plan *p, const float *w_override_dev, const float *g_overrid
         p->h_occ[h_sel.beam] = 1;
         p->col_valid[h_sel.beam] = 0;
         // y_k = 0: z, w and the cost are unchanged (S2), the state stays valid
+        p->warm_ok = false;   // but the saved gradient knows nothing of this beam
     }
     return VMAT_OK;
 }
@@ -398,8 +400,9 @@ int vmat_master(vmat_plan *p, vmat_master_stats *out) {
     if (!p) return VMAT_EINVAL;
     int rc = ensure_columns(p);
     if (rc) return rc;
-    if ((rc = launch_master(p, -1))) return rc;
+    if ((rc = launch_master(p, -1, 0))) return rc;
     p->state_valid = true;
+    p->warm_ok = true;
     MasterOut h;
     VMAT_CUDA(p, cudaMemcpyAsync(&h, p->mout, sizeof(MasterOut), cudaMemcpyDeviceToHost, p->stream));
     VMAT_CUDA(p, cudaStreamSynchronize(p->stream));
@@ -423,6 +426,7 @@ int vmat_set_dose_rate_bounds(vmat_plan *p, double y_min, double y_max) {
         return fail(p, VMAT_EINVAL, "dose-rate bounds need 0 <= y_min <= y_max, y_min finite");
     p->y_min = y_min;
     p->y_max = y_max;
+    p->warm_ok = false;   // the next solve may clamp y: evaluate from scratch
     return VMAT_OK;
 }
 
@@ -448,7 +452,7 @@ int vmat_enforce_dose_rate(vmat_plan *p, double rho, double factor, double tol, 
     while (ratio > 1.0 + tol && rounds < max_rounds) {
         p->gamma *= factor;                          // "gamma ... will be automatically increased"
         if (!std::isfinite(p->gamma)) return fail(p, VMAT_ESTATE, "gamma overflowed while enforcing the dose-rate limit");
-        if ((rc = launch_master(p, -1))) return rc;  // "the intensity for each aperture will be re-optimized"
+        if ((rc = launch_master(p, -1, 0))) return rc;  // "the intensity for each aperture will be re-optimized"
         MasterOut h;
         VMAT_CUDA(p, cudaMemcpyAsync(&h, p->mout, sizeof(MasterOut), cudaMemcpyDeviceToHost, p->stream));
         if ((rc = test(ratio))) return rc;           // "till the solution is feasible"
@@ -534,7 +538,8 @@ int vmat_solve(vmat_plan *p, int32_t max_iters, vmat_solve_stats *out) {
         if (phases) TRYC(cudaEventRecord(evs[it * 5 + 2], st));
         TRY(launch_column_build(p, -1));                                           // d_k of the new aperture
         if (phases) TRYC(cudaEventRecord(evs[it * 5 + 3], st));
-        TRY(launch_master(p, (int)it));                                            // (e), leaves z, w current
+        TRY(launch_master(p, (int)it, p->warm_ok ? 1 : 0));                        // (e), leaves z, w current
+        p->warm_ok = true;
         if (phases) TRYC(cudaEventRecord(evs[it * 5 + 4], st));
         done = it + 1;
     }
@@ -638,6 +643,7 @@ int vmat_set_plan(vmat_plan *p, const uint8_t *occupied, const int32_t *left, co
     p->h_occ = oo;
     p->col_valid.assign((size_t)N, 0);
     p->state_valid = false;
+    p->warm_ok = false;
     return launch_free_list(p);
 }
 

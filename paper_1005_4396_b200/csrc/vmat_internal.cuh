@@ -87,6 +87,9 @@ struct vmat_plan {
     long long *accbuf = nullptr;       // 3 x (2N + 2) fixed-point sums of the master kernel
     unsigned int *phase = nullptr;     // rotation counter of accbuf, barrier epoch
     unsigned long long *mcount = nullptr;   // master bookkeeping: touched segments x passes, passes
+    double *gsave = nullptr;           // N: d_k . w the last master solve left (warm entry of the next one in vmat_solve)
+    int *gflag = nullptr;              // device flag: gsave is valid
+    bool warm_ok = false;              // host: nothing but vmat_solve's own steps touched the plan since that solve
     vmat::ColStat *colstat = nullptr;  // N
     uint32_t *col_touch = nullptr;     // N x touch_words: bit c of row k set iff chunk c of d_k holds a non-zero entry
     int touch_words = 0;
@@ -192,7 +195,7 @@ int launch_leaf_search(vmat_plan *p, const float *g, int32_t *all_left, int32_t 
 int master_configure(vmat_plan *p);
 int launch_column_build(vmat_plan *p, int beam /* -1: read p->sel */);
 int launch_dose_grad(vmat_plan *p);
-int launch_master(vmat_plan *p, int trace_it);
+int launch_master(vmat_plan *p, int trace_it, int warm /* 1: inside vmat_solve, right after a committed search */);
 int launch_expand(vmat_plan *p, const float *src_s, float *dst_V, int what /*0 z, 1 w*/);
 int launch_compress(vmat_plan *p, const float *src_V, float *dst_s);
 int launch_rate_ratio(vmat_plan *p, double rho, double *ratio_dev);

@@ -245,6 +245,12 @@ struct MasterArgs {
                                 // to the record of its group (blockIdx mod kSumGroups)
     unsigned int *phase;        // rotation counter, persists from launch to launch
     unsigned long long *mcount; // bookkeeping: [0] += touched segments x passes (all blocks), [1] += passes
+    // warm entry (inside vmat_solve): z, w and cost3 are current for the plan as it was before the leaf search
+    // committed beam sel->beam at y = 0, and gsave holds the F-part of the gradient of the beams occupied then
+    int warm;
+    const Sel *sel;
+    double *gsave;              // N: d_k . w at the y this kernel leaves (valid iff gflag[0] == 1)
+    int *gflag;
     MasterOut *out;
     double *cost3;
     double *trF, *trG, *trC;
@@ -1544,17 +1550,36 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
         Gs = s[1];
     }
     __syncthreads();
-    long long *rec = begin_pass();
-    eval_pass<true>(a, sm, K, Ku, ngroups, nullptr, zcur, nullptr, rzcur, 0.f, rec, sm.ctl->scF, sm.ctl->scG, red PROF_ARG);
-    cg::this_grid().sync();
-    ++ph;
-    fetch_record(rec, K + 2);
+    // Warm entry: the previous solve left z, w, F and d_k . w of its beams current, and the one beam the leaf search
+    // has occupied since enters at y = 0, so the dose has not moved; its own d_k . w is the price the search formed
+    // minus the smoothing term.  The evaluation pass (and its grid barrier) is then not needed.
+    const bool warm = MODE == 0 && a.warm && a.gflag[0] == 1 && a.sel->beam >= 0;
+    long long *rec = nullptr;
+    if (!warm) {
+        rec = begin_pass();
+        eval_pass<true>(a, sm, K, Ku, ngroups, nullptr, zcur, nullptr, rzcur, 0.f, rec, sm.ctl->scF, sm.ctl->scG, red PROF_ARG);
+        cg::this_grid().sync();
+        ++ph;
+        fetch_record(rec, K + 2);
+    } else if (res) {
+        for (int ls = tid; ls < a.rslots; ls += kMasterThreads) {
+            const int c = (int)blockIdx.x + (ls >> 7) * (int)gridDim.x;
+            rzcur[ls] = c < a.nchunks ? a.z[(size_t)c * kChunk + (ls & (kChunk - 1))] : 0.f;
+        }
+    }
     if (ctl) {
         const double iG = sm.ctl->iG;
+        const int knew = warm ? a.sel->beam : -1;
+        const double pnew = warm ? a.sel->price : 0.0;
         double pgl = 0.0;
         for (int k = tid; k < N; k += CT) {
             const int i = sm.ik[k];
-            const double gk = i >= 0 ? (double)sm.recv[2 + i] * iG + a.gamma * sm.dG[k] : 0.0;
+            double gk = 0.0;
+            if (i >= 0) {
+                if (!warm) gk = (double)sm.recv[2 + i] * iG + a.gamma * sm.dG[k];
+                else if (k == knew) gk = pnew;   // = 2^-30 total + gamma dG/dy_k, the reduced cost itself
+                else gk = a.gsave[k] + a.gamma * sm.dG[k];
+            }
             const double p = (i < 0 || at_bound(sm.y[k], gk)) ? 0.0 : gk;
             sm.grad[k] = gk;
             if (MODE == 1) {
@@ -1567,7 +1592,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
         }
         double s0[1] = {0.0};
         ctl_reduce<1>(s0, pgl, cred, tog, nw, CT);   // its barrier also publishes grad, pg, d to the group
-        F = (double)sm.recv[0] * sm.ctl->iF + a.F_out;
+        F = warm ? a.cost3[0] : (double)sm.recv[0] * sm.ctl->iF + a.F_out;
         Phi = F + a.gamma * Gs;
         pgmax = pgl;
         pg_entry = pgmax;
@@ -1874,8 +1899,16 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
         if (ctl) {
             F = (double)sm.recv[0] * sm.ctl->iF + a.F_out;
             Phi = F + a.gamma * Gs;
+            if (blockIdx.x == 0) {   // d_k . w at the final y, for the warm entry of the next solve
+                const double iG = sm.ctl->iG;
+                for (int k = tid; k < N; k += CT) {
+                    const int i = sm.ik[k];
+                    a.gsave[k] = i >= 0 ? (double)sm.recv[2 + i] * iG : 0.0;
+                }
+            }
         }
     }
+    if (blockIdx.x == 0 && tid == 0) a.gflag[0] = sm.ctl->accepted ? 1 : 0;   // no final pass: nothing saved
     if (tid == 0) {
         atomicAdd(a.mcount, (unsigned long long)sSegs * (unsigned long long)(ph - ph_entry));
         if (blockIdx.x == 0) atomicAdd(a.mcount + 1, (unsigned long long)(ph - ph_entry));
@@ -1975,6 +2008,9 @@ int master_configure(vmat_plan *p) {
     if ((rc = dev_alloc(p, &p->accbuf, 3 * kSumGroups * (2 * p->N + 2)))) return rc;
     if ((rc = dev_alloc(p, &p->phase, 2))) return rc;
     if ((rc = dev_alloc(p, &p->mcount, 2))) return rc;
+    if ((rc = dev_alloc(p, &p->gsave, p->N))) return rc;
+    if ((rc = dev_alloc(p, &p->gflag, 1))) return rc;
+    VMAT_CUDA(p, cudaMemsetAsync(p->gflag, 0, 4, p->stream));
     VMAT_CUDA(p, cudaMemsetAsync(p->mcount, 0, 16, p->stream));
     if ((rc = dev_alloc(p, &p->colstat, p->N))) return rc;
     p->touch_words = (int)((nchunks + 31) / 32);
@@ -2009,8 +2045,12 @@ int launch_column_build(vmat_plan *p, int beam) {
     return VMAT_OK;
 }
 
-static int launch_master_impl(vmat_plan *p, int max_inner, int trace_it) {
+static int launch_master_impl(vmat_plan *p, int max_inner, int trace_it, int warm) {
     MasterArgs a;
+    a.warm = warm;
+    a.sel = p->sel;
+    a.gsave = p->gsave;
+    a.gflag = p->gflag;
     a.Dd = p->Dd;
     a.Sp = (long long)p->Sp;
     a.nchunks = (int)(p->Sp / kChunk);
@@ -2061,10 +2101,12 @@ static int launch_master_impl(vmat_plan *p, int max_inner, int trace_it) {
     return VMAT_OK;
 }
 
-int launch_master(vmat_plan *p, int trace_it) { return launch_master_impl(p, p->opt.master_max_inner, trace_it); }
+int launch_master(vmat_plan *p, int trace_it, int warm) {
+    return launch_master_impl(p, p->opt.master_max_inner, trace_it, warm);
+}
 
 // steps (a)+(b) alone: the master kernel's evaluation pass with no iteration allowed
-int launch_dose_grad(vmat_plan *p) { return launch_master_impl(p, 0, -1); }
+int launch_dose_grad(vmat_plan *p) { return launch_master_impl(p, 0, -1, 0); }
 
 #ifdef VMAT_MASTER_PROFILE
 extern "C" void vmat_debug_master_prof(long long out[16], int reset) {
