@@ -353,13 +353,14 @@ struct Ctl {
 };
 enum { kRunDirection = 0, kRunTrial = 1, kFinish = 2, kRunFused = 3 };
 
-constexpr int kRedSlots = 6;   // values per warp row of the control group's reduction scratch
+constexpr int kRedSlots = 8;   // values per warp row of the control group's reduction scratch
 // Records of grid-wide sums per rotation slot.  Measured: splitting the blocks into 16 groups with one record each
 // (to spread same-address atomics) and a hand-rolled two-level barrier were both slower than one record and the
 // cooperative-groups barrier (12.4 / 14.5 vs 11.7 us per inner iteration at K = 30), so there is one group.
 constexpr int kSumGroups = 1;
 constexpr int kKSplit = 8;     // beam-loop split of the passes; the two halves of the warps take alternate chunks
 constexpr int kNoCache = INT_MIN;
+constexpr double kReleaseEta2 = 0.0625;   // release the held beams when |g on the face|^2 <= this x |held inward g|^2
 static_assert(kMasterWarps == 2 * kKSplit, "the passes split the warps in two chunk halves");
 
 // 1-D bulk copies (TMA) global -> shared, completion counted in bytes on an mbarrier
@@ -1795,21 +1796,32 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
                 // Polak-Ribiere+ update, in one sweep and one batched reduction
                 const double iG = sm.ctl->iG;
                 const double Fn = (double)sm.recv[0] * sm.ctl->iF + a.F_out;
-                double s[4] = {0.0, 0.0, 0.0, 0.0}, pgm = 0.0;
+                // The working direction lives on the FACE of the beams that are off their bounds: a beam at a bound is
+                // held there (its entry of the working gradient pf is 0) even if its gradient points inwards, until the
+                // gradient on the face is small against the held inward part (s[4] <= eta^2 s[5]); then the held
+                // beams are released and the conjugate directions restart.  Releasing at once, as the textbook rule
+                // does, made beams near y = 0 enter and leave the face from one step to the next: over a third of all
+                // steps of a configs[1] plan were restarts.  Convergence is still judged on the true projected gradient.
+                double s[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0}, pgm = 0.0;
                 for (int k = tid; k < N; k += CT) {
                     const int i = sm.ik[k];
                     const double gk = i >= 0 ? (double)sm.recv[2 + i] * iG + a.gamma * sm.dG[k] : 0.0;
                     const double yk = sm.yn[k], po = sm.pg[k];
                     const double pn = (i < 0 || at_bound(yk, gk)) ? 0.0 : gk;
+                    const bool atb = yk <= lb || (has_ub && yk >= ub);
+                    const double pf = (i < 0 || atb) ? 0.0 : gk;
                     sm.gn[k] = gk;
-                    s[3] += ((pn == 0.0) != (po == 0.0)) ? 1.0 : 0.0;   // entries entering / leaving the face
-                    s[0] += pn * (pn - po);
+                    s[3] += ((pf == 0.0) != (po == 0.0)) ? 1.0 : 0.0;   // entries entering / leaving the face
+                    s[0] += pf * (pf - po);
                     s[1] += po * po;
                     s[2] += gk * sm.d[k];
+                    s[4] += pf * pf;
+                    if (atb) s[5] += pn * pn;                            // held, but the gradient points inwards
                     pgm = fmax(pgm, fabs(pn));
                 }
-                ctl_reduce<4>(s, pgm, cred, tog, nw, CT);
-                const bool changed = hit || s[3] > 0.0;
+                ctl_reduce<6>(s, pgm, cred, tog, nw, CT);
+                const bool release = s[5] > 0.0 && s[4] <= kReleaseEta2 * s[5];
+                const bool changed = hit || release || s[3] > 0.0;
                                 const double Phin = Fn + a.gamma * Gn;
                 // sufficient decrease; below the resolution of Phi accept on the slope instead
                 const bool accepted = Phin <= Phi + c1a * t * phi1 ||
@@ -1826,7 +1838,8 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
                     for (int k = tid; k < N; k += CT) {
                         const double yk = sm.yn[k], gk = sm.gn[k];
                         const bool off = sm.ik[k] < 0;
-                        const double pn = (off || at_bound(yk, gk)) ? 0.0 : gk;
+                        const bool atb = yk <= lb || (has_ub && yk >= ub);
+                        const double pn = (off || (release ? at_bound(yk, gk) : atb)) ? 0.0 : gk;   // working gradient
                         double dk = -pn + bpr * sm.d[k];
                         if (off || at_bound(yk, -dk)) dk = 0.0;   // stay feasible
                         sm.y[k] = yk;
