@@ -1820,8 +1820,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
                     pgm = fmax(pgm, fabs(pn));
                 }
                 ctl_reduce<6>(s, pgm, cred, tog, nw, CT);
-                const bool release = s[5] > 0.0 && s[4] <= kReleaseEta2 * s[5];
-                const bool changed = hit || release || s[3] > 0.0;
+                bool release = s[5] > 0.0 && s[4] <= kReleaseEta2 * s[5];
                                 const double Phin = Fn + a.gamma * Gn;
                 // sufficient decrease; below the resolution of Phi accept on the slope instead
                 const bool accepted = Phin <= Phi + c1a * t * phi1 ||
@@ -1830,6 +1829,11 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
                 if (accepted) {
                     // take the step; Polak-Ribiere+ direction on the current face, restart when the active set changes
                     stall = (Phi - Phin <= stall_threshold(Phin) * fabs(Phi)) ? stall + 1 : 0;
+                    if (stall >= a.stall_count && s[5] > 0.0 && !release) {
+                        release = true;   // never stop on a face while held beams want in: release them and go on
+                        stall = 0;
+                    }
+                    const bool changed = hit || release || s[3] > 0.0;
                     F = Fn;
                     Gs = Gn;
                     Phi = Phin;
