@@ -37,9 +37,9 @@ def load_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-# ncu --set full capture of k_price_spmv on configs[1] (profiles/r01c_price_spmv.md): dram__bytes_read.sum +
+# ncu --set full capture of k_price_spmv on configs[1] (profiles/r01j_price_spmv.md): dram__bytes_read.sum +
 # dram__bytes_write.sum of the first pricing launch of a plan (all 180 beams un-occupied; 994,678,664 algorithmic bytes)
-NCU_TRAFFIC_BYTES_FIRST_LAUNCH = {"prostate": 992093952 + 4464128}
+NCU_TRAFFIC_BYTES_FIRST_LAUNCH = {"prostate": 992094720 + 4436224}
 
 
 class ClockSampler:
