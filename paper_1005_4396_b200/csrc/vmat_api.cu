@@ -228,6 +228,8 @@ int vmat_create(const vmat_problem *pb, const vmat_options *options, void *cuda_
     A(p->beam_price, N);
     A(p->sel, 1);
     A(p->ticket, 1);
+    A(p->beam_total, N);
+    A(p->beam_ticket, N);
     A(p->mout, 1);
     A(p->cost3, 3);
     A(p->rate_ratio, 1);
@@ -257,6 +259,8 @@ int vmat_create(const vmat_problem *pb, const vmat_options *options, void *cuda_
     Z(p->cand_left, (size_t)NR * 4);
     Z(p->cand_right, (size_t)NR * 4);
     Z(p->ticket, 4);
+    Z(p->beam_total, (size_t)N * 8);
+    Z(p->beam_ticket, (size_t)N * 4);
     Z(p->sel, sizeof(Sel));
 #undef Z
     if ((e = cudaMemcpyAsync(p->theta, pb->theta_deg, (size_t)N * 8, cudaMemcpyHostToDevice, st)) != cudaSuccess)

@@ -81,6 +81,8 @@ struct vmat_plan {
     double *beam_price = nullptr;  // N
     vmat::Sel *sel = nullptr;
     unsigned int *ticket = nullptr;
+    unsigned long long *beam_total = nullptr;   // N, leaf search: per-beam sums of row optima (zero between launches)
+    unsigned int *beam_ticket = nullptr;        // N, leaf search: per-beam block counters (zero between launches)
 
     long long *accbuf = nullptr;       // 3 x (2N + 2) fixed-point sums of the master kernel
     unsigned int *phase = nullptr;     // rotation counter of accbuf, barrier epoch

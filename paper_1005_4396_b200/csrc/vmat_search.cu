@@ -8,11 +8,10 @@
 // prefix sums are exact and independent of evaluation order (reading S9 / O5).  One
 // warp owns one leaf row: positions 0..C are dealt to the lanes in blocks of M, the prefix sums
 // P, the running maximum of P[l] over admissible l (later l wins ties) and the minimum of the key
-// (P[r']-P[l], r'-l, l) are warp-shuffle scans/reductions.  One block owns one beam, its rows dealt
-// evenly to at most 32 warps; row optima are summed as integers in shared memory (exact, order free),
-// the block forms the beam's price, and the block that finishes last picks the beam (smallest price,
-// lowest k on ties) and commits it on request.  No global round trip lies between a row's search and
-// its beam's price.
+// (P[r']-P[l], r'-l, l) are warp-shuffle scans/reductions.  A block owns kRowsPerBlock rows of one
+// beam; row optima are added to the beam's total with integer atomics (exact, order free); the last
+// block of a beam forms its price, the last block of all picks the beam (smallest price, lowest k
+// on ties) and commits it on request.
 #include <math_constants.h>
 
 #include "vmat_internal.cuh"
@@ -22,8 +21,9 @@ namespace vmat {
 namespace {
 
 constexpr unsigned kFull = 0xffffffffu;
-constexpr int kMaxSearchThreads = 1024;   // one block per beam, its leaf rows dealt evenly to at most 32 warps
-constexpr int kMaxListChunks = 64;        // list of un-occupied beams rebuilt in parallel up to N = 2048
+constexpr int kSearchThreads = 256;
+constexpr int kRowsPerBlock = kSearchThreads / 32;   // one warp per leaf row
+constexpr int kMaxListChunks = 64;                   // chunks of 32 beams in the list of un-occupied beams (vmat_create: N <= 2048)
 
 __device__ __forceinline__ long long shfl_up_ll(long long v, int o) {
     return __shfl_up_sync(kFull, v, o);
@@ -32,7 +32,7 @@ __device__ __forceinline__ long long shfl_up_ll(long long v, int o) {
 // Warp-cooperative search of one row.  All lanes return the same (value, l, r'); l = -1 if the box
 // admits no interval.
 template <int M>
-__device__ __forceinline__ void row_search_warp(const float (&gv)[M], int C, int Lmin, int Lmax, int Rmin,
+__device__ __forceinline__ void row_search_warp(const float *__restrict__ g_row, int C, int Lmin, int Lmax, int Rmin,
                                                 int Rmax, int lane, long long &value, int &l_out, int &r_out) {
     // inclusive local prefix sums of the quantised prices; position p uses price p-1
     long long loc[M];
@@ -41,7 +41,7 @@ __device__ __forceinline__ void row_search_warp(const float (&gv)[M], int C, int
     for (int t = 0; t < M; ++t) {
         const int pos = lane * M + t;
         long long qv = 0;
-        if (pos >= 1 && pos <= C) qv = __double2ll_rn((double)gv[t] * 1073741824.0);
+        if (pos >= 1 && pos <= C) qv = __double2ll_rn((double)g_row[pos - 1] * 1073741824.0);
         sum += qv;
         loc[t] = sum;
     }
@@ -144,6 +144,8 @@ struct SearchArgs {
     double *out_price;
     Sel *sel;
     unsigned int *ticket;              // beams finished
+    unsigned long long *beam_total;    // N: sum of the row optima of a beam (all zero between launches)
+    unsigned int *beam_ticket;         // N: blocks of a beam finished (all zero between launches)
     int commit;
     int32_t *tr_beam;                  // trace slots (or null)
     double *tr_price;
@@ -158,58 +160,24 @@ __device__ __forceinline__ void take_better(double &bp, int &bk, double op, int 
     }
 }
 
-// the lane's prices of one row (position p uses price p-1)
 template <int M>
-__device__ __forceinline__ void row_prices(const SearchArgs &a, int k, int r, int lane, float (&gv)[M]) {
-    const int R = a.R, C = a.C;
-    const float *g_row = a.g + ((size_t)k * R + r) * C;
-#pragma unroll
-    for (int t = 0; t < M; ++t) {
-        const int pos = lane * M + t;
-        gv[t] = pos >= 1 && pos <= C ? g_row[pos - 1] : 0.f;
-    }
-}
-
-// the row's leaf-travel box from the nearest occupied beams km < k < kp (reading S6)
-__device__ __forceinline__ void row_box(const SearchArgs &a, int k, int r, int km, int kp, int (&box)[4]) {
-    const int N = a.N, R = a.R, C = a.C;
-    int Lmin = 0, Lmax = C, Rmin = 0, Rmax = C;
-    if (km >= 0) {
-        const int b = a.delta * (k - km), l = a.left[km * R + r], rr = a.right[km * R + r];
-        Lmin = max(Lmin, l - b);
-        Lmax = min(Lmax, l + b);
-        Rmin = max(Rmin, rr - b);
-        Rmax = min(Rmax, rr + b);
-    }
-    if (kp < N) {
-        const int b = a.delta * (kp - k), l = a.left[kp * R + r], rr = a.right[kp * R + r];
-        Lmin = max(Lmin, l - b);
-        Lmax = min(Lmax, l + b);
-        Rmin = max(Rmin, rr - b);
-        Rmax = min(Rmax, rr + b);
-    }
-    box[0] = Lmin;
-    box[1] = Lmax;
-    box[2] = Rmin;
-    box[3] = Rmax;
-}
-
-template <int M>
-__global__ void __launch_bounds__(kMaxSearchThreads) k_leaf_search(const SearchArgs a) {
+__global__ void __launch_bounds__(kSearchThreads) k_leaf_search(const SearchArgs a) {
     pdl_wait();      // the prices (launched behind the pricing product by programmatic dependent launch)
     pdl_trigger();   // the column build may be scheduled; it waits for the choice itself
     __shared__ int s_km, s_kp, s_last;
     __shared__ unsigned long long s_total;
-    __shared__ double s_price[32];
-    __shared__ int s_beam[32];
+    __shared__ double s_price[kRowsPerBlock];
+    __shared__ int s_beam[kRowsPerBlock];
     __shared__ int s_cnt[kMaxListChunks];
     const int N = a.N, R = a.R, C = a.C;
-    const int k = blockIdx.x;                                     // one block per beam
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, W = blockDim.x >> 5;
+    const int RB = (R + kRowsPerBlock - 1) / kRowsPerBlock;       // blocks per beam
+    const int k = blockIdx.x / RB, rb = blockIdx.x - k * RB;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const bool occupied = a.occ[k] != 0;
+    if (occupied && rb > 0) return;                               // block 0 of an occupied beam reports +inf
+    bool beam_done = false;                                       // this block finishes its beam (thread 0)
 
-    if (!a.occ[k]) {
-        float gv[M], gn[M];
-        if (warp < R) row_prices<M>(a, k, warp, lane, gv);   // in flight behind the scan of occ
+    if (!occupied) {
         if (tid == 0) {
             s_km = -1;
             s_kp = N;
@@ -218,30 +186,39 @@ __global__ void __launch_bounds__(kMaxSearchThreads) k_leaf_search(const SearchA
         __syncthreads();
         // nearest occupied beam on each side (reading S6)
         int km_t = -1, kp_t = N;
-        for (int kk = tid; kk < N; kk += blockDim.x)
+        for (int kk = tid; kk < N; kk += kSearchThreads)
             if (a.occ[kk]) {
                 if (kk < k) km_t = max(km_t, kk);
                 if (kk > k) kp_t = min(kp_t, kk);
             }
         km_t = __reduce_max_sync(kFull, km_t);
         kp_t = __reduce_min_sync(kFull, kp_t);
-        if (lane == 0 && warp * 32 < N) {
+        if (lane == 0) {   // one shared-memory atomic per warp that saw an occupied beam
             if (km_t >= 0) atomicMax(&s_km, km_t);
             if (kp_t < N) atomicMin(&s_kp, kp_t);
         }
         __syncthreads();
         const int km = s_km, kp = s_kp;
-        long long total = 0;                                      // this warp's rows (all lanes hold the same value)
-        int box[4], boxn[4];
-        if (warp < R) row_box(a, k, warp, km, kp, box);
-        for (int r = warp; r < R; r += W) {
-            if (r + W < R) {   // in flight behind this row's scans
-                row_prices<M>(a, k, r + W, lane, gn);
-                row_box(a, k, r + W, km, kp, boxn);
+        const int r = rb * kRowsPerBlock + warp;
+        if (r < R) {
+            int Lmin = 0, Lmax = C, Rmin = 0, Rmax = C;
+            if (km >= 0) {
+                const int b = a.delta * (k - km), l = a.left[km * R + r], rr = a.right[km * R + r];
+                Lmin = max(Lmin, l - b);
+                Lmax = min(Lmax, l + b);
+                Rmin = max(Rmin, rr - b);
+                Rmax = min(Rmax, rr + b);
+            }
+            if (kp < N) {
+                const int b = a.delta * (kp - k), l = a.left[kp * R + r], rr = a.right[kp * R + r];
+                Lmin = max(Lmin, l - b);
+                Lmax = min(Lmax, l + b);
+                Rmin = max(Rmin, rr - b);
+                Rmax = min(Rmax, rr + b);
             }
             long long value;
             int bl, br;
-            row_search_warp<M>(gv, C, box[0], box[1], box[2], box[3], lane, value, bl, br);
+            row_search_warp<M>(a.g + ((size_t)k * R + r) * C, C, Lmin, Lmax, Rmin, Rmax, lane, value, bl, br);
             if (lane == 0) {
                 a.cand_left[k * R + r] = bl;
                 a.cand_right[k * R + r] = br;
@@ -249,47 +226,53 @@ __global__ void __launch_bounds__(kMaxSearchThreads) k_leaf_search(const SearchA
                     a.out_left[k * R + r] = bl;
                     a.out_right[k * R + r] = br;
                 }
+                atomicAdd(&s_total, (unsigned long long)value);   // exact, order free
             }
-            total += value;
-#pragma unroll
-            for (int t = 0; t < M; ++t) gv[t] = gn[t];
-#pragma unroll
-            for (int t = 0; t < 4; ++t) box[t] = boxn[t];
         }
-        if (lane == 0 && total) atomicAdd(&s_total, (unsigned long long)total);   // integer: exact, order free
         __syncthreads();
         if (tid == 0) {
-            const long long beam_total = (long long)s_total;
-            // price_k = 2^-30 * total + gamma * dG/dy_k, every operation individually rounded
-            // (Eq. 2; reading S10); same order of operations as the definition
-            double dG = 0.0;
-            if (k > 0)
-                dG = __dadd_rn(dG, __ddiv_rn(__dmul_rn(2.0, __dsub_rn(a.y[k], a.y[k - 1])),
-                                             __dsub_rn(a.theta[k], a.theta[k - 1])));
-            if (k + 1 < N)
-                dG = __dsub_rn(dG, __ddiv_rn(__dmul_rn(2.0, __dsub_rn(a.y[k + 1], a.y[k])),
-                                             __dsub_rn(a.theta[k + 1], a.theta[k])));
-            const double smooth = __dmul_rn(a.gamma, dG);
-            const double price = __dadd_rn(ldexp(__ll2double_rn(beam_total), -30), smooth);
-            a.beam_price[k] = price;
-            if (a.out_price) a.out_price[k] = price;
+            atomicAdd(a.beam_total + k, s_total);
+            __threadfence();
+            if (atomicAdd(a.beam_ticket + k, 1u) == (unsigned)RB - 1u) {
+                __threadfence();
+                beam_done = true;
+                const long long total = (long long)atomicExch(a.beam_total + k, 0ull);   // all RB sums are in; reset
+                a.beam_ticket[k] = 0u;
+                // price_k = 2^-30 * total + gamma * dG/dy_k, every operation individually rounded
+                // (Eq. 2; reading S10); same order of operations as the definition
+                double dG = 0.0;
+                if (k > 0)
+                    dG = __dadd_rn(dG, __ddiv_rn(__dmul_rn(2.0, __dsub_rn(a.y[k], a.y[k - 1])),
+                                                 __dsub_rn(a.theta[k], a.theta[k - 1])));
+                if (k + 1 < N)
+                    dG = __dsub_rn(dG, __ddiv_rn(__dmul_rn(2.0, __dsub_rn(a.y[k + 1], a.y[k])),
+                                                 __dsub_rn(a.theta[k + 1], a.theta[k])));
+                const double smooth = __dmul_rn(a.gamma, dG);
+                const double price = __dadd_rn(ldexp(__ll2double_rn(total), -30), smooth);
+                a.beam_price[k] = price;
+                if (a.out_price) a.out_price[k] = price;
+            }
         }
     } else if (tid == 0) {
+        beam_done = true;
         a.beam_price[k] = CUDART_INF;
         if (a.out_price) a.out_price[k] = CUDART_INF;
     }
 
     // the block that finishes the last beam chooses among all of them
     if (tid == 0) {
-        __threadfence();
-        s_last = atomicAdd(a.ticket, 1u) == (unsigned)N - 1u;
+        s_last = 0;
+        if (beam_done) {
+            __threadfence();
+            s_last = atomicAdd(a.ticket, 1u) == (unsigned)N - 1u;
+        }
     }
     __syncthreads();
     if (!s_last) return;
     __threadfence();
     double bp = CUDART_INF;
     int bk = -1;
-    for (int kk = tid; kk < N; kk += blockDim.x) {
+    for (int kk = tid; kk < N; kk += kSearchThreads) {
         const double pr = __ldcg(a.beam_price + kk);
         if (!a.occ[kk] && (bk < 0 || pr < bp)) {   // ascending kk: the lowest index wins ties
             bp = pr;
@@ -304,8 +287,8 @@ __global__ void __launch_bounds__(kMaxSearchThreads) k_leaf_search(const SearchA
     }
     __syncthreads();
     if (warp == 0) {
-        bp = lane < W ? s_price[lane] : CUDART_INF;
-        bk = lane < W ? s_beam[lane] : -1;
+        bp = lane < kRowsPerBlock ? s_price[lane] : CUDART_INF;
+        bk = lane < kRowsPerBlock ? s_beam[lane] : -1;
 #pragma unroll
         for (int o = 16; o; o >>= 1)
             take_better(bp, bk, __shfl_down_sync(kFull, bp, o), __shfl_down_sync(kFull, bk, o));
@@ -328,42 +311,30 @@ __global__ void __launch_bounds__(kMaxSearchThreads) k_leaf_search(const SearchA
     }
     if (a.commit && best >= 0) {
         // occupy the beam with this aperture at y_k = 0
-        for (int r = tid; r < R; r += blockDim.x) {
+        for (int r = tid; r < R; r += kSearchThreads) {
             a.left[best * R + r] = __ldcg(a.cand_left + best * R + r);
             a.right[best * R + r] = __ldcg(a.cand_right + best * R + r);
         }
         // the pricing product of the next iteration walks this list: chunks of 32 beams, counted by one
         // warp each, then written behind the chunks before them
         const int nch = (N + 31) / 32;
-        if (nch <= kMaxListChunks) {
-            for (int ch = warp; ch < nch; ch += W) {
-                const int kk = ch * 32 + lane;
-                const bool f = kk < N && kk != best && !a.occ[kk];
-                const unsigned m = __ballot_sync(kFull, f);
-                if (lane == 0) s_cnt[ch] = __popc(m);
-            }
-            __syncthreads();
-            for (int ch = warp; ch < nch; ch += W) {
-                int base = 0;
-                for (int c0 = lane; c0 < ch; c0 += 32) base += s_cnt[c0];
-                base = __reduce_add_sync(kFull, base);
-                const int kk = ch * 32 + lane;
-                const bool f = kk < N && kk != best && !a.occ[kk];
-                const unsigned m = __ballot_sync(kFull, f);
-                if (f) a.free_list[base + __popc(m & ((1u << lane) - 1u))] = kk;
-            }
-            __syncthreads();
-        } else if (tid < 32) {
-            int base = 0;
-            for (int k0 = 0; k0 < N; k0 += 32) {
-                const int kk = k0 + tid;
-                const bool f = kk < N && kk != best && !a.occ[kk];
-                const unsigned m = __ballot_sync(kFull, f);
-                if (f) a.free_list[base + __popc(m & ((1u << tid) - 1u))] = kk;
-                base += __popc(m);
-            }
+        for (int ch = warp; ch < nch; ch += kRowsPerBlock) {
+            const int kk = ch * 32 + lane;
+            const bool f = kk < N && kk != best && !a.occ[kk];
+            const unsigned m = __ballot_sync(kFull, f);
+            if (lane == 0) s_cnt[ch] = __popc(m);
         }
-        if (tid == 0) {
+        __syncthreads();
+        for (int ch = warp; ch < nch; ch += kRowsPerBlock) {
+            int base = 0;
+            for (int c0 = lane; c0 < ch; c0 += 32) base += s_cnt[c0];
+            base = __reduce_add_sync(kFull, base);
+            const int kk = ch * 32 + lane;
+            const bool f = kk < N && kk != best && !a.occ[kk];
+            const unsigned m = __ballot_sync(kFull, f);
+            if (f) a.free_list[base + __popc(m & ((1u << lane) - 1u))] = kk;
+        }
+        if (tid == 0) {   // no reader above looks at occ[best]
             a.occ[best] = 1;
             a.y[best] = 0.0;
         }
@@ -396,13 +367,14 @@ int launch_leaf_search(vmat_plan *p, const float *g, int32_t *all_left, int32_t 
     a.out_price = beam_price;
     a.sel = p->sel;
     a.ticket = p->ticket;
+    a.beam_total = p->beam_total;
+    a.beam_ticket = p->beam_ticket;
     a.commit = commit;
     a.tr_beam = trace_it >= 0 ? p->tr_beam : nullptr;
     a.tr_price = p->tr_price;
     a.trace_it = trace_it;
     const int M = (int)((p->C + 1 + 31) / 32);
-    const int rounds = (int)((p->R + 31) / 32);                      // rows per warp
-    const dim3 grid((unsigned)p->N), block(32u * (unsigned)((p->R + rounds - 1) / rounds));
+    const dim3 grid((unsigned)(p->N * ((p->R + kRowsPerBlock - 1) / kRowsPerBlock))), block(kSearchThreads);
     switch (M) {
         case 1: VMAT_CUDA(p, launch_pdl(k_leaf_search<1>, grid, block, p->stream, a)); break;
         case 2: VMAT_CUDA(p, launch_pdl(k_leaf_search<2>, grid, block, p->stream, a)); break;

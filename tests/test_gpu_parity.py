@@ -171,6 +171,31 @@ def test_leaf_search_bit_exact_random_prices(torch_cuda, vm, C):
     plan.destroy()
 
 
+@pytest.mark.parametrize("N,R", [(70, 33), (40, 70), (100, 1)])
+def test_leaf_search_many_rows_and_committed_list(torch_cuda, vm, N, R):
+    # one block per beam: 33 rows = two rows per warp with a ragged second round, 70 rows = three rounds; more
+    # than 32 beams = several chunks of the list of un-occupied beams, which the committing block rebuilds and the
+    # next pricing product walks (no set_plan in between: the list under test is the search's own)
+    o = random_problem(N + R, V=64, N=N, R=R, C=3, density=0.1)
+    plan = make_plan(vm, o)
+    occ, left, right, y = (a.copy() for a in oracle_states(o, 3, every=3)[-1])
+    for _ in range(4):
+        z = o.dose(occ, left, right, y)
+        _, w = o.penalty(z)
+        g32 = o.prices(w, occ).astype(np.float32)
+        check_search(torch_cuda, plan, o, occ, left, right, y, g32)
+        ref = o.price_step(g32, occ, left, right, y)
+        ap = plan.price(g_override=torch_cuda.from_numpy(g32).cuda(), commit=True)
+        assert ap.beam == ref["beam"]
+        occ[ref["beam"]] = 1
+        left[ref["beam"]], right[ref["beam"]] = ref["left"], ref["right"]
+        d_occ, d_left, d_right, d_y = plan.get_plan()
+        assert np.array_equal(np.asarray(d_occ, bool), np.asarray(occ, bool))
+        assert np.array_equal(d_left.reshape(N, R), left) and np.array_equal(d_right.reshape(N, R), right)
+        check_prices(torch_cuda, plan, o, w, occ)
+    plan.destroy()
+
+
 def test_all_beams_occupied_is_done(torch_cuda, vm):
     o = random_problem(11, N=3)
     occ, l, r, y, z, tr = o.solve(10)
