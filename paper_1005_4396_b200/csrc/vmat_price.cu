@@ -27,13 +27,17 @@ __device__ __forceinline__ int4 ld_stream_i4(const int4 *ptr) {
     return r;
 }
 
-constexpr int kPriceThreads = 256;
+// Threads per block: 256 for long launches; 128 once a launch is short (its tail, the last blocks of the grid
+// draining on a few SMs, weighs more the shorter the launch: measured 15.0 against 15.3 ms of pricing per
+// configs[1] plan with 128, 334 against 332 ms on configs[4] when 128 is used throughout).
+constexpr int kPriceThreadsLong = 256, kPriceThreadsShort = 128;
+constexpr long long kShortLaunchRows = 600000;
 
 // One group of LANES lanes (a warp or half a warp) per beamlet; UNROLL quads per lane are loaded
 // before any gather is issued.  The grid covers only the un-occupied beams: block b works on beam
 // free_list[b / blocks_per_beam] (ascending list kept current by the leaf search's commit), so a
 // launch late in the plan is as short as the rows it has to stream.
-template <int LANES, int UNROLL>
+template <int LANES, int UNROLL, int kPriceThreads>
 __global__ void __launch_bounds__(kPriceThreads)
 k_price_spmv(const uint32_t *__restrict__ rowq, const float4 *__restrict__ val4, const int4 *__restrict__ col4,
              const float *__restrict__ w, const int32_t *__restrict__ free_list, int blocks_per_beam, int RC,
@@ -86,12 +90,18 @@ __global__ void k_free_list(const uint8_t *__restrict__ occ, int N, int32_t *__r
     }
 }
 
+template <int LANES, int UNROLL, int THREADS>
+void launch_sized(vmat_plan *p, const float *w_s, float *g, int n_free) {
+    const int rows_per_block = THREADS / LANES;
+    const int bpb = (int)((p->RC + rows_per_block - 1) / rows_per_block);
+    k_price_spmv<LANES, UNROLL, THREADS><<<(unsigned)(n_free * bpb), THREADS, 0, p->stream>>>(
+        p->rowq, p->val4, p->col4, w_s, p->free_list, bpb, (int)p->RC, g);
+}
+
 template <int LANES, int UNROLL>
 void launch_variant(vmat_plan *p, const float *w_s, float *g, int n_free) {
-    const int rows_per_block = kPriceThreads / LANES;
-    const int bpb = (int)((p->RC + rows_per_block - 1) / rows_per_block);
-    k_price_spmv<LANES, UNROLL><<<(unsigned)(n_free * bpb), kPriceThreads, 0, p->stream>>>(
-        p->rowq, p->val4, p->col4, w_s, p->free_list, bpb, (int)p->RC, g);
+    if ((long long)n_free * p->RC <= kShortLaunchRows) launch_sized<LANES, UNROLL, kPriceThreadsShort>(p, w_s, g, n_free);
+    else launch_sized<LANES, UNROLL, kPriceThreadsLong>(p, w_s, g, n_free);
 }
 
 }  // namespace
