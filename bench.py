@@ -39,8 +39,6 @@ def load_peaks():
 
 # ncu --set full capture of k_price_spmv on configs[1] (profiles/r01j_price_spmv.md): dram__bytes_read.sum +
 # dram__bytes_write.sum of the first pricing launch of a plan (all 180 beams un-occupied; 994,678,664 algorithmic bytes)
-# vmat_options.pricing_kernel -> lanes per beamlet, 16-byte loads in flight per lane (vmat_price.cu)
-PRICING_VARIANTS = {0: "16,4", 1: "32,2", 2: "32,4", 3: "16,2", 4: "16,4", 5: "8,4"}
 NCU_TRAFFIC_BYTES_FIRST_LAUNCH = {"prostate": 992094720 + 4436224}
 
 
@@ -276,8 +274,6 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--master-mode", type=int, default=None, choices=[0, 1],
                     help="inner iteration of the master kernel (vmat_options.master_mode); default: the library's")
-    ap.add_argument("--pricing-kernel", type=int, default=None, choices=[0, 1, 2, 3, 4, 5],
-                    help="lanes x loads-in-flight variant of the pricing product (vmat_options.pricing_kernel)")
     ap.add_argument("--sweep", action="store_true", help="configs[3]: isolated pricing / search kernel sweep")
     ap.add_argument("--sweep-nnz", default="5e7,1e8,2.5e8,5e8,1e9")
     ap.add_argument("--sweep-voxels", default="1048576,2097152,4194304")
@@ -321,8 +317,6 @@ def main():
         opt.record_phases = record_phases
         if args.master_mode is not None:
             opt.master_mode = args.master_mode
-        if args.pricing_kernel is not None:
-            opt.pricing_kernel = args.pricing_kernel
         return vm.Plan.create(*[t.numpy() for t in host], ph.theta_deg, c.n_rows, c.n_cols, c.max_leaf_travel, c.gamma,
                               options=opt)
 
@@ -410,7 +404,7 @@ def main():
     peak, peak_src = load_peaks()
     achieved = sum(alg) / (ph_us["price"] * 1e-6) / 1e9
     roofline = {
-        "kernel": "k_price_spmv<%s> (pricing SpMV, step c)" % PRICING_VARIANTS[args.pricing_kernel or 0],
+        "kernel": "k_price_spmv<16,4> (pricing SpMV, step c)",
         "bound": "hbm", "achieved": achieved, "peak": peak,
         "unit": "GB/s", "frac": achieved / peak, "frac_of_8TBs_nominal": achieved / 8000.0,
         "traffic": NCU_TRAFFIC_BYTES_FIRST_LAUNCH.get(c.name),

@@ -79,8 +79,8 @@ typedef struct {
 /* Tunables.  Zero-initialise, then call vmat_default_options. */
 typedef struct {
     int32_t validate;          /* 1: check the CSR and the voxel arrays on the device (default 1) */
-    int32_t pricing_kernel;    /* 0 default; 1..5 lanes-per-beamlet x loads-in-flight variants of the
-                                  pricing product (32x2, 32x4, 16x2, 16x4, 8x4), for measurement   */
+    int32_t d_format;          /* device storage of D: 0 = fp32 value + 32-bit voxel slot per entry (8 bytes,
+                                  the fp32-CSR layout of BASELINE.json north_star, default)          */
     int32_t dose_path;         /* how vmat_dose forms z: 0 from the aperture-dose columns d_k the
                                   master keeps (default), 1 straight from D (fixed-point atomics)  */
     double  master_eps;        /* stop when max|projected gradient| <= eps*max(1, value at entry) */
@@ -91,15 +91,25 @@ typedef struct {
                                   optimum) the fraction is applied 100x more strictly              */
     int32_t master_stall_count;/* stop after this many stalls in a row (stop_reason 4)            */
     int32_t record_phases;     /* 1: vmat_solve brackets each phase with CUDA events              */
-    int32_t master_mode;       /* inner iteration of the master kernel: 0 = two passes over the columns and two
-                                  grid barriers (q = Dc^T d and the curvature, then the trial point), 1 = one
-                                  fused pass and one grid barrier (the next direction is built from the gradient
-                                  the quadratic piece predicts at the trial point; the step length and every
-                                  acceptance / stop decision use the true gradient).  Same minimiser (S11).  */
+    int32_t master_mode;       /* how step (e) reaches the minimiser (same minimiser either way, S11):
+                                  0 = gradient projection with conjugate directions: two passes over the aperture-dose
+                                      columns and two grid barriers per inner iteration;
+                                  1 = (default) semismooth Newton on the reduced problem: F is piecewise quadratic, so
+                                      the master problem restricted to the current piece is a quadratic in the K <= N
+                                      dose rates with matrix 2 Dc diag(omega) Dc^T + 2 gamma L; that matrix is kept
+                                      on the device from solve to solve (updated only where a voxel crossed its T_j),
+                                      one thread block solves the K-dimensional box-constrained quadratic by conjugate
+                                      gradients on its faces, the other blocks evaluate the true cost and gradient at
+                                      the point it proposes: two or three passes per solve instead of about twenty.
+                                      Needs n_beams <= 256 and N^2 floats of shared memory; otherwise mode 0 runs.   */
     int32_t stop_when_priced_out; /* vmat_solve stops as soon as the best aperture's price is >= 0 (the textbook
                                   column-generation stop).  Default 0: the loop goes on until every beam holds an
                                   aperture, as the paper wants (reading S5).  With 1 the
                                   call synchronises the stream once per iteration to read the price.             */
+    int32_t master_unstaged_lists; /* 1 (default): aperture-dose columns that do not fit a master block's shared-memory
+                                  tile are walked through per-chunk lists; 0: through masked loops over all such
+                                  columns (the fallback the kernel takes by itself when the lists do not fit;
+                                  exposed so that tests can reach it).  Same results.                            */
 } vmat_options;
 
 /* One deliverable aperture: a beam and one leaf pair per row. */
@@ -111,10 +121,11 @@ typedef struct {
 } vmat_aperture;
 
 typedef struct {
-    int32_t inner;          /* inner iterations done                                            */
+    int32_t inner;          /* inner iterations done (mode 1: Newton steps taken)               */
     int32_t backtracks;     /* step halvings                                                    */
     int32_t stop_reason;    /* 0 converged, 1 iteration cap, 2 no descent, 3 line search failed,
-                               4 decrease below fp32 resolution                                 */
+                               4 decrease below fp32 resolution, 5 non-finite value,
+                               6 internal hand-over timed out                                   */
     int32_t passes;         /* passes over the columns, each ended by a grid barrier            */
     double  pg_entry, pg_exit;   /* max |projected gradient| at entry / exit                    */
     double  F, G, cost;     /* at exit: F, G and F + gamma G                                    */
@@ -133,6 +144,10 @@ typedef struct {
     /* bookkeeping of the master kernel over the call (algorithmic traffic of step e):                  */
     double  master_passes;  /* passes over the aperture-dose columns, each ended by a grid barrier      */
     double  master_bytes;   /* bytes of the touched 512-byte column segments those passes multiplied    */
+    /* master_mode 1 only: the block that solves the reduced problems                                           */
+    double  master_cg_steps;   /* conjugate-gradient steps on the K-dimensional quadratics                     */
+    double  master_clk_cg, master_clk_wait, master_clk_load;   /* its SM clock cycles in those steps, waiting
+                                  for the passes of the other blocks, and loading the reduced Hessian           */
 } vmat_solve_stats;
 
 typedef struct {
@@ -191,9 +206,19 @@ int vmat_price_spmv(vmat_plan *plan, const float *w_dev, float *g_dev);
 int vmat_leaf_search(vmat_plan *plan, const float *g_dev, int32_t *all_left_dev,
                      int32_t *all_right_dev, double *beam_price_dev);
 
+/* Per-call overrides of the master tunables of vmat_options; a field <= 0 keeps the plan's value. */
+typedef struct {
+    double  eps;            /* stop when max|projected gradient| <= eps*max(1, value at entry)          */
+    int32_t max_inner;      /* cap on inner iterations                                                   */
+    double  stall_rel;      /* see vmat_options.master_stall_rel                                         */
+    int32_t stall_count;    /* see vmat_options.master_stall_count                                       */
+} vmat_master_opts;
+
 /* Step (e): solve model (3) for y >= 0 over the occupied beams, warm-started
- * from the plan's y.  Leaves z, w current.  out may be NULL.                                  */
-int vmat_master(vmat_plan *plan, vmat_master_stats *out);
+ * from the plan's y.  Leaves z, w current.  opts may be NULL (the plan's options); out may be NULL.
+ * y is kept in double precision on both sides of the boundary: the dose rates carry the plan from one
+ * solve to the next, and fp32 would add 6e-8 relative noise per hand-over to a 1e-5 stop test.      */
+int vmat_master(vmat_plan *plan, const vmat_master_opts *opts, vmat_master_stats *out);
 
 /* The column-generation loop (S5): up to max_iters iterations of
  * price -> search -> occupy -> master, continuing from the plan's current state.  All iterations

@@ -186,7 +186,9 @@ int vo_row_search(int64_t C, const int64_t *q, int64_t Lmin, int64_t Lmax, int64
  * with each operation individually rounded (-ffp-contract=off).  Chooses the smallest price,
  * lowest k on ties (S9).  Outputs (any may be NULL): beam_price[N] (+inf at occupied beams),
  * all_left/all_right [N*R] (row optimum of every un-occupied beam; untouched at occupied),
- * best_left/best_right [R].  Returns the chosen beam, or -1 if every beam is occupied.
+ * best_left/best_right [R].  A beam with a row whose leaf-travel box admits no interval is undeliverable
+ * ("all the deliverability constraints"): price +inf, rows reported as (-1, -1), never chosen.
+ * Returns the chosen beam, or -1 if no un-occupied beam is deliverable.
  * ------------------------------------------------------------------------------------------ */
 int64_t vo_price_step(const vo_problem *p, const float *g32, const uint8_t *occ, const int32_t *left,
                       const int32_t *right, const double *y, double *best_price, int32_t *best_left,
@@ -202,14 +204,20 @@ int64_t vo_price_step(const vo_problem *p, const float *g32, const uint8_t *occ,
         if (beam_price) beam_price[k] = INFINITY;
         if (occ[k]) continue;
         int64_t total = 0;
+        int deliverable = 1;
         for (int64_t r = 0; r < R; ++r) {
             int64_t box[4], v = 0;
             vo_leaf_box(p, occ, left, right, k, r, box);
             vo_quantise(C, g32 + (k * R + r) * C, q);
-            vo_row_search(C, q, box[0], box[1], box[2], box[3], &tl[r], &tr[r], &v);
+            if (vo_row_search(C, q, box[0], box[1], box[2], box[3], &tl[r], &tr[r], &v) != 0) {
+                /* the box admits no interval (only possible if the occupied apertures themselves break the
+                 * leaf-travel limit): this beam has no deliverable aperture and cannot be chosen */
+                deliverable = 0; tl[r] = -1; tr[r] = -1; v = 0;
+            }
             total += v;
             if (all_left) { all_left[k * R + r] = tl[r]; all_right[k * R + r] = tr[r]; }
         }
+        if (!deliverable) continue;                                /* beam_price[k] stays +inf */
         const double smooth = p->gamma * dG[k];
         const double price = ldexp((double)total, -30) + smooth;
         if (beam_price) beam_price[k] = price;
@@ -553,6 +561,8 @@ typedef struct {
     double eps;               /* master tolerance */
     int64_t max_inner;
     int64_t stop_when_priced_out; /* option of reading S5: stop as soon as the best price is >= 0 */
+    double lb, ub;            /* bounds on the dose rates of occupied beams in every master solve (variant of
+                                 PAPER.md:159, reading R4; 0 and +inf = the paper's y >= 0)                  */
     /* outputs, arrays caller-allocated with max_iters entries (leaf arrays max_iters*R) */
     int64_t iters;            /* outer iterations done */
     int32_t *beam;            /* chosen beam */
@@ -579,7 +589,9 @@ static double now_s(void) {
  * stop_when_priced_out also as soon as no aperture has a negative price (the textbook column-generation
  * stop, offered as an option because the paper wants an aperture at every angle).
  * State arrays (occ N, left/right N*R, y N, z V) are caller allocated; on entry they hold the
- * plan to continue from (all zero for a fresh run).
+ * plan to continue from (all zero for a fresh run).  With bounds lb <= y_k <= ub on the occupied beams (variant,
+ * reading R4) the prices are unchanged (the reduced cost of the paper at the current y); a beam that enters is
+ * brought into the box by its first master solve.
  * ------------------------------------------------------------------------------------------ */
 void vo_solve(const vo_problem *p, uint8_t *occ, int32_t *left, int32_t *right, double *y, double *z, vo_trace *tr) {
     const int64_t N = p->N, R = p->R, B = p->N * p->R * p->C;
@@ -606,7 +618,7 @@ void vo_solve(const vo_problem *p, uint8_t *occ, int32_t *left, int32_t *right, 
         double t1 = now_s();
         vo_master_info info; memset(&info, 0, sizeof(info));
         info.eps = tr->eps; info.max_inner = tr->max_inner;
-        info.lb = 0.0; info.ub = INFINITY;
+        info.lb = tr->lb; info.ub = tr->ub;                        /* the new beam enters at y = 0 and is brought to lb */
         master_solve(p, cols, occ, y, z, &info);
         double t2 = now_s();
         tr->seconds_price += t1 - t0; tr->seconds_master += t2 - t1;

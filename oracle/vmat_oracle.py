@@ -50,7 +50,7 @@ class _RateInfo(_c.Structure):
 
 class _Trace(_c.Structure):
     _fields_ = [("max_iters", _c.c_int64), ("eps", _c.c_double), ("max_inner", _c.c_int64),
-                ("stop_when_priced_out", _c.c_int64), ("iters", _c.c_int64), ("beam", _P), ("price", _P), ("F", _P), ("G", _P), ("cost", _P),
+                ("stop_when_priced_out", _c.c_int64), ("lb", _c.c_double), ("ub", _c.c_double), ("iters", _c.c_int64), ("beam", _P), ("price", _P), ("F", _P), ("G", _P), ("cost", _P),
                 ("inner", _P), ("it_left", _P), ("it_right", _P),
                 ("seconds_price", _c.c_double), ("seconds_master", _c.c_double)]
 
@@ -288,8 +288,10 @@ class Oracle:
                           ratio=float(info.ratio), F=float(info.F), G=float(info.G), cost=float(info.cost))
 
     # O1 + O8 -----------------------------------------------------------------------------------
-    def solve(self, max_iters, plan=None, eps=1e-9, max_inner=20000, stop_when_priced_out=False):
-        """Run the column-generation loop. Returns (occ, left[N,R], right[N,R], y, z, Trace)."""
+    def solve(self, max_iters, plan=None, eps=1e-9, max_inner=20000, stop_when_priced_out=False, y_min=0.0,
+              y_max=float("inf")):
+        """Run the column-generation loop. Returns (occ, left[N,R], right[N,R], y, z, Trace).  y_min, y_max: bounds on
+        the dose rates of occupied beams in every master solve (variant of PAPER.md:159; default the paper's y >= 0)."""
         if plan is None:
             occ, left, right, y = self.empty_plan()
         else:
@@ -300,7 +302,7 @@ class Oracle:
         beam, inner = np.full(M, -1, np.int32), np.zeros(M, np.int64)
         price, F, G, cost = (np.zeros(M, np.float64) for _ in range(4))
         il, ir = np.zeros(M * R, np.int32), np.zeros(M * R, np.int32)
-        tr = _Trace(max_iters=M, eps=eps, max_inner=max_inner, stop_when_priced_out=int(bool(stop_when_priced_out)), beam=_ptr(beam), price=_ptr(price), F=_ptr(F),
+        tr = _Trace(max_iters=M, eps=eps, max_inner=max_inner, stop_when_priced_out=int(bool(stop_when_priced_out)), lb=float(y_min), ub=float(y_max), beam=_ptr(beam), price=_ptr(price), F=_ptr(F),
                     G=_ptr(G), cost=_ptr(cost), inner=_ptr(inner), it_left=_ptr(il), it_right=_ptr(ir))
         self._L.vo_solve(_c.byref(self._p), _ptr(occ), _ptr(left), _ptr(right), _ptr(y), _ptr(z), _c.byref(tr))
         n = int(tr.iters)

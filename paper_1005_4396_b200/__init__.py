@@ -42,13 +42,18 @@ class _Problem(C.Structure):
 
 
 class Options(C.Structure):
-    _fields_ = [("validate", C.c_int32), ("pricing_kernel", C.c_int32), ("dose_path", C.c_int32),
+    _fields_ = [("validate", C.c_int32), ("d_format", C.c_int32), ("dose_path", C.c_int32),
                 ("master_eps", C.c_double), ("master_max_inner", C.c_int32), ("master_stall_rel", C.c_double),
-                ("master_stall_count", C.c_int32), ("record_phases", C.c_int32), ("master_mode", C.c_int32), ("stop_when_priced_out", C.c_int32)]
+                ("master_stall_count", C.c_int32), ("record_phases", C.c_int32), ("master_mode", C.c_int32), ("stop_when_priced_out", C.c_int32),
+                ("master_unstaged_lists", C.c_int32)]
 
 
 class _Aperture(C.Structure):
     _fields_ = [("beam", C.c_int32), ("price", C.c_double), ("left", _P), ("right", _P)]
+
+
+class _MasterOpts(C.Structure):
+    _fields_ = [("eps", C.c_double), ("max_inner", C.c_int32), ("stall_rel", C.c_double), ("stall_count", C.c_int32)]
 
 
 class _MasterStats(C.Structure):
@@ -61,7 +66,9 @@ class _SolveStats(C.Structure):
     _fields_ = [("iters", C.c_int32), ("us_total", C.c_double), ("us_price", C.c_double), ("us_search", C.c_double),
                 ("us_column", C.c_double), ("us_master", C.c_double), ("F", C.c_double), ("G", C.c_double),
                 ("cost", C.c_double), ("beam", _P), ("price", _P), ("trace_F", _P), ("trace_G", _P),
-                ("trace_cost", _P), ("inner", _P), ("master_passes", C.c_double), ("master_bytes", C.c_double)]
+                ("trace_cost", _P), ("inner", _P), ("master_passes", C.c_double), ("master_bytes", C.c_double),
+                ("master_cg_steps", C.c_double), ("master_clk_cg", C.c_double), ("master_clk_wait", C.c_double),
+                ("master_clk_load", C.c_double)]
 
 
 class _RateStats(C.Structure):
@@ -102,7 +109,7 @@ def load_library():
     L.vmat_price.argtypes = [_P, _P, _P, _P, C.POINTER(_Aperture), C.c_int]
     L.vmat_price_spmv.argtypes = [_P, _P, _P]
     L.vmat_leaf_search.argtypes = [_P, _P, _P, _P, _P]
-    L.vmat_master.argtypes = [_P, C.POINTER(_MasterStats)]
+    L.vmat_master.argtypes = [_P, C.POINTER(_MasterOpts), C.POINTER(_MasterStats)]
     L.vmat_enforce_dose_rate.argtypes = [_P, C.c_double, C.c_double, C.c_double, C.c_int32, C.POINTER(_RateStats)]
     L.vmat_solve.argtypes = [_P, C.c_int32, C.POINTER(_SolveStats)]
     L.vmat_get_plan.argtypes = [_P, _P, _P, _P, _P]
@@ -175,6 +182,10 @@ class SolveStats:
     inner: np.ndarray
     master_passes: float = 0.0
     master_bytes: float = 0.0
+    master_cg_steps: float = 0.0
+    master_clk_cg: float = 0.0
+    master_clk_wait: float = 0.0
+    master_clk_load: float = 0.0
 
 
 def _is_torch(a) -> bool:
@@ -312,9 +323,11 @@ class Plan:
                                              _dev_ptr(all_right, "int32", self.N * self.R),
                                              _dev_ptr(beam_price, "float64", self.N)))
 
-    def master(self) -> MasterStats:
+    def master(self, eps: float = 0.0, max_inner: int = 0, stall_rel: float = 0.0, stall_count: int = 0) -> MasterStats:
+        """vmat_master; the keyword arguments are the per-call overrides of vmat_master_opts (0 = the plan's option)."""
         s = _MasterStats()
-        self._check(self._L.vmat_master(self._h, C.byref(s)))
+        o = _MasterOpts(float(eps), int(max_inner), float(stall_rel), int(stall_count))
+        self._check(self._L.vmat_master(self._h, C.byref(o), C.byref(s)))
         return MasterStats(s.inner, s.backtracks, s.stop_reason, s.pg_entry, s.pg_exit, s.F, s.G, s.cost, s.passes)
 
     def set_dose_rate_bounds(self, y_min: float = 0.0, y_max: float = float("inf")) -> None:
@@ -342,7 +355,8 @@ class Plan:
         self._check(self._L.vmat_solve(self._h, int(max_iters), C.byref(s)))
         n = int(s.iters)
         return SolveStats(n, s.us_total, s.us_price, s.us_search, s.us_column, s.us_master, s.F, s.G, s.cost,
-                          beam[:n], price[:n], tF[:n], tG[:n], tC[:n], inner[:n], s.master_passes, s.master_bytes)
+                          beam[:n], price[:n], tF[:n], tG[:n], tC[:n], inner[:n], s.master_passes, s.master_bytes,
+                          s.master_cg_steps, s.master_clk_cg, s.master_clk_wait, s.master_clk_load)
 
     # -- plan state -------------------------------------------------------------------------------
     def get_plan(self):

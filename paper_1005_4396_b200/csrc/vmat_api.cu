@@ -2,6 +2,8 @@
 // life-cycle, and the order in which the kernels of the other translation units are enqueued.
 // No arithmetic of the method lives here.
 #include <cmath>
+#include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <mutex>
 #include <new>
@@ -128,15 +130,16 @@ extern "C" {
 void vmat_default_options(vmat_options *opt) {
     if (!opt) return;
     opt->validate = 1;
-    opt->pricing_kernel = 0;
+    opt->d_format = 0;
     opt->dose_path = 0;
     opt->master_eps = 1e-5;
     opt->master_max_inner = 500;
     opt->master_stall_rel = 1e-6;    // 100x inside the 1e-4 parity tolerance on the master cost (S11)
     opt->master_stall_count = 2;
     opt->record_phases = 0;
-    opt->master_mode = 0;
+    opt->master_mode = 1;
     opt->stop_when_priced_out = 0;
+    opt->master_unstaged_lists = 1;
 }
 
 int vmat_create(const vmat_problem *pb, const vmat_options *options, void *cuda_stream, vmat_plan **out) {
@@ -181,6 +184,7 @@ int vmat_create(const vmat_problem *pb, const vmat_options *options, void *cuda_
     if (!(p->opt.master_stall_rel >= 0.0)) p->opt.master_stall_rel = 1e-6;
     if (p->opt.master_stall_count < 1) p->opt.master_stall_count = 2;
     if (p->opt.master_mode != 1) p->opt.master_mode = 0;
+    if (p->opt.d_format != 0) return bail(fail(p, VMAT_EINVAL, "d_format must be 0"));
     p->V = pb->n_voxels;
     p->N = pb->n_beams;
     p->R = pb->n_rows;
@@ -396,11 +400,20 @@ int vmat_price(vmat_plan *p, const float *w_override_dev, const float *g_overrid
     return VMAT_OK;
 }
 
-int vmat_master(vmat_plan *p, vmat_master_stats *out) {
+int vmat_master(vmat_plan *p, const vmat_master_opts *opts, vmat_master_stats *out) {
     if (!p) return VMAT_EINVAL;
     int rc = ensure_columns(p);
     if (rc) return rc;
-    if ((rc = launch_master(p, -1, 0))) return rc;
+    const vmat_options keep = p->opt;
+    if (opts) {   // per-call overrides (a field <= 0 keeps the plan's value)
+        if (opts->eps > 0.0) p->opt.master_eps = opts->eps;
+        if (opts->max_inner > 0) p->opt.master_max_inner = opts->max_inner;
+        if (opts->stall_rel > 0.0) p->opt.master_stall_rel = opts->stall_rel;
+        if (opts->stall_count > 0) p->opt.master_stall_count = opts->stall_count;
+    }
+    rc = launch_master(p, -1, 0);
+    p->opt = keep;
+    if (rc) return rc;
     p->state_valid = true;
     p->warm_ok = true;
     MasterOut h;
@@ -517,7 +530,7 @@ int vmat_solve(vmat_plan *p, int32_t max_iters, vmat_solve_stats *out) {
             return cuda_fail(p, ce__, #call);        \
         }                                            \
     }
-    TRYC(cudaMemsetAsync(p->mcount, 0, 16, st));
+    TRYC(cudaMemsetAsync(p->mcount, 0, 128, st));
     TRYC(cudaEventRecord(ev0, st));
     TRY(ensure_state(p));
     TRY(ensure_columns(p));   // the master needs d_k of every occupied beam, whichever path formed z
@@ -575,10 +588,15 @@ int vmat_solve(vmat_plan *p, int32_t max_iters, vmat_solve_stats *out) {
         out->F = c3[0];
         out->G = c3[1];
         out->cost = c3[2];
-        unsigned long long mc[2];
+        unsigned long long mc[16];
         TRYC(cudaMemcpy(mc, p->mcount, sizeof(mc), cudaMemcpyDeviceToHost));
+        if (getenv("VMAT_DEBUG_CLK")) fprintf(stderr, "worker pass clk: block0 %llu  max-over-solves-of-block-total %llu  mean %llu\n", mc[6], mc[7], mc[8] / 147);
         out->master_passes = (double)mc[1];
         out->master_bytes = (double)mc[0] * (double)(kChunk * 4);
+        out->master_cg_steps = (double)mc[2];
+        out->master_clk_cg = (double)mc[3];
+        out->master_clk_wait = (double)mc[4];
+        out->master_clk_load = (double)mc[5];
         const size_t n = (size_t)todo;
         if (n) {
             if (out->beam) TRYC(cudaMemcpy(out->beam, p->tr_beam, n * 4, cudaMemcpyDeviceToHost));
@@ -644,6 +662,8 @@ int vmat_set_plan(vmat_plan *p, const uint8_t *occupied, const int32_t *left, co
     p->col_valid.assign((size_t)N, 0);
     p->state_valid = false;
     p->warm_ok = false;
+    int rc = reset_hessian(p);
+    if (rc) return rc;
     return launch_free_list(p);
 }
 

@@ -96,8 +96,8 @@ k_dose_scatter(const uint32_t *__restrict__ rowq, const float4 *__restrict__ val
     // measured, and the pass ran at the L2 reduction rate, not at the HBM rate.)
     const float *__restrict__ val = reinterpret_cast<const float *>(val4);
     const int *__restrict__ col = reinterpret_cast<const int *>(col4);
-    const uint32_t a = rowq[row] * 4u, b = rowq[row + 1] * 4u;
-    for (uint32_t e = a + lane; e < b; e += kDoseLanes * kDoseEntries) {
+    const uint64_t a = (uint64_t)rowq[row] * 4u, b = (uint64_t)rowq[row + 1] * 4u;   // entries: past 2^32 from 2^30 quads on
+    for (uint64_t e = a + lane; e < b; e += kDoseLanes * kDoseEntries) {
         float v[kDoseEntries];
         int s[kDoseEntries];
 #pragma unroll

@@ -100,6 +100,16 @@ struct vmat_plan {
     int master_cache_segs = 0;         // 512-byte segments of Dd a master block stages in shared memory
     int master_rslots = 0;             // slots per master block kept resident in shared memory (0: none)
     int master_ul_cap = 0;             // capacity of the master's per-chunk lists of unstaged beams (0: masked loops)
+    // mode 1 of the master (k_newton): the Hessian of F over the occupied beams, kept on the device from solve to solve
+    bool master_newton = false;        // the plan runs k_newton (master_mode 1 and the reduced problem fits one block)
+    int master_nblk = 0;               // blocks of the master grid that own chunks (k_newton: all but the solving block)
+    long long *hess = nullptr;         // N x N fixed point
+    float *omref = nullptr;            // Sp: the omega (alpha, beta or 0 per slot) the matrix was built with
+    uint8_t *hvalid = nullptr;         // N: column k is in the matrix
+    double hscale = 1.0, hinv = 1.0;
+    float *wn_s = nullptr;             // Sp: second buffer of w
+    void *mail = nullptr;              // message of the solving block to the working blocks
+    unsigned long long *nsync = nullptr;   // arrival / epoch counters of that hand-over
     vmat::MasterOut *mout = nullptr;
     double *cost3 = nullptr;       // device {F, G, F+gamma G}
     double *rate_ratio = nullptr;  // device scalar of the dose-rate feasibility test
@@ -193,6 +203,7 @@ int launch_leaf_search(vmat_plan *p, const float *g, int32_t *all_left, int32_t 
 
 // vmat_master.cu ------------------------------------------------------------------------------------
 int master_configure(vmat_plan *p);
+int reset_hessian(vmat_plan *p);
 int launch_column_build(vmat_plan *p, int beam /* -1: read p->sel */);
 int launch_dose_grad(vmat_plan *p);
 int launch_master(vmat_plan *p, int trace_it, int warm /* 1: inside vmat_solve, right after a committed search */);

@@ -1,8 +1,6 @@
 // vmat_layout.cu — vmat_create's device work: validate the problem, find the support of D,
 // re-lay-out D as a padded beamlet-major CSR in slot space.
-// Set-up code (runs once per plan); CUB's device scan is used for the two prefix sums.
-#include <cub/device/device_scan.cuh>
-
+// Set-up code (runs once per plan).
 #include <cmath>
 #include <cstring>
 
@@ -128,6 +126,87 @@ __global__ void k_fill_padded(const int64_t *__restrict__ row_ptr, const int32_t
     }
 }
 
+// ---- exclusive prefix sum (the two scans of the set-up: support flags -> slots, row quads -> row starts) --------
+// Three short kernels: every block scans kScanTile elements and records its total, one block scans the totals,
+// every block adds the sum of the blocks before it.  In place is allowed (in == out).
+constexpr int kScanThreads = 256, kScanPer = 4, kScanTile = kScanThreads * kScanPer;
+
+template <typename T>
+__device__ __forceinline__ T block_exclusive_scan(T v, T *warp_tot, T &total) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    T incl = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const T n = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += n;
+    }
+    if (lane == 31) warp_tot[warp] = incl;
+    __syncthreads();
+    T base = 0, tot = 0;
+    for (int w = 0; w < (int)(blockDim.x >> 5); ++w) {
+        const T t = warp_tot[w];
+        if (w < warp) base += t;
+        tot += t;
+    }
+    __syncthreads();
+    total = tot;
+    return base + incl - v;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(kScanThreads) k_scan_tiles(const T *__restrict__ in, T *__restrict__ out, int64_t n,
+                                                             T *__restrict__ tile_sums) {
+    __shared__ T warp_tot[kScanThreads / 32];
+    const int64_t i0 = ((int64_t)blockIdx.x * kScanThreads + threadIdx.x) * kScanPer;
+    T v[kScanPer], sum = 0;
+#pragma unroll
+    for (int u = 0; u < kScanPer; ++u) {
+        v[u] = i0 + u < n ? in[i0 + u] : (T)0;
+        sum += v[u];
+    }
+    T total;
+    T run = block_exclusive_scan(sum, warp_tot, total);
+#pragma unroll
+    for (int u = 0; u < kScanPer; ++u) {
+        if (i0 + u < n) out[i0 + u] = run;
+        run += v[u];
+    }
+    if (threadIdx.x == 0) tile_sums[blockIdx.x] = total;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(kScanThreads) k_scan_sums(T *__restrict__ tile_sums, int64_t ntiles) {
+    __shared__ T warp_tot[kScanThreads / 32];
+    T carry = 0;
+    for (int64_t b0 = 0; b0 < ntiles; b0 += kScanThreads) {
+        const int64_t b = b0 + threadIdx.x;
+        const T v = b < ntiles ? tile_sums[b] : (T)0;
+        T total;
+        const T ex = block_exclusive_scan(v, warp_tot, total);
+        if (b < ntiles) tile_sums[b] = carry + ex;
+        carry += total;
+    }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(kScanThreads) k_scan_add(T *__restrict__ out, int64_t n, const T *__restrict__ tile_sums) {
+    const int64_t i0 = ((int64_t)blockIdx.x * kScanThreads + threadIdx.x) * kScanPer;
+    const T base = tile_sums[blockIdx.x];
+#pragma unroll
+    for (int u = 0; u < kScanPer; ++u)
+        if (i0 + u < n) out[i0 + u] += base;
+}
+
+template <typename T>
+cudaError_t exclusive_scan(const T *in, T *out, int64_t n, T *tile_sums, cudaStream_t st) {
+    if (n <= 0) return cudaSuccess;
+    const int64_t ntiles = (n + kScanTile - 1) / kScanTile;
+    k_scan_tiles<T><<<(unsigned)ntiles, kScanThreads, 0, st>>>(in, out, n, tile_sums);
+    k_scan_sums<T><<<1, kScanThreads, 0, st>>>(tile_sums, ntiles);
+    k_scan_add<T><<<(unsigned)ntiles, kScanThreads, 0, st>>>(out, n, tile_sums);
+    return cudaGetLastError();
+}
+
 }  // namespace
 
 template <typename T>
@@ -222,13 +301,10 @@ static int build_layout_impl(vmat_plan *p, const vmat_problem *pb, std::vector<v
     p->fx_inv = std::ldexp(1.0, e2 - 40);
 
     // support: exclusive scan of the reach flags
-    size_t cub_bytes = 0, cub_bytes2 = 0;
-    cub::DeviceScan::ExclusiveSum(nullptr, cub_bytes, d_reach, d_excl, (int)V, st);
-    cub::DeviceScan::ExclusiveSum(nullptr, cub_bytes2, d_cnt, d_cnt, (int)(B + 1), st);
-    if (cub_bytes2 > cub_bytes) cub_bytes = cub_bytes2;
-    void *d_cub;
-    if ((rc = tmp_alloc(&d_cub, cub_bytes))) return rc;
-    VMAT_CUDA(p, cub::DeviceScan::ExclusiveSum(d_cub, cub_bytes, d_reach, d_excl, (int)V, st));
+    const int64_t scan_tiles = ((V > B + 1 ? V : B + 1) + kScanTile - 1) / kScanTile;
+    void *d_tiles;
+    if ((rc = tmp_alloc(&d_tiles, (size_t)scan_tiles * 4))) return rc;
+    VMAT_CUDA(p, exclusive_scan<int32_t>(d_reach, d_excl, V, (int32_t *)d_tiles, st));
     int32_t last_excl = 0, last_flag = 0;
     if (V > 0) {
         VMAT_CUDA(p, cudaMemcpyAsync(&last_excl, d_excl + V - 1, 4, cudaMemcpyDeviceToHost, st));
@@ -237,7 +313,7 @@ static int build_layout_impl(vmat_plan *p, const vmat_problem *pb, std::vector<v
     // row starts in quads
     k_row_quads<<<(unsigned)((B + 1 + 255) / 256), 256, 0, st>>>(d_row_ptr, B, d_cnt);
     if ((rc = dev_alloc(p, &p->rowq, B + 1))) return rc;
-    VMAT_CUDA(p, cub::DeviceScan::ExclusiveSum(d_cub, cub_bytes, d_cnt, p->rowq, (int)(B + 1), st));
+    VMAT_CUDA(p, exclusive_scan<uint32_t>(d_cnt, p->rowq, B + 1, (uint32_t *)d_tiles, st));
     uint32_t nq = 0;
     VMAT_CUDA(p, cudaMemcpyAsync(&nq, p->rowq + B, 4, cudaMemcpyDeviceToHost, st));
     VMAT_CUDA(p, cudaStreamSynchronize(st));

@@ -26,7 +26,7 @@
 
 #include <climits>
 #include <cstdio>
-#include <cstdlib>
+#include <cmath>
 
 #include "vmat_internal.cuh"
 
@@ -219,6 +219,7 @@ __global__ void k_voxel_bounds(const float *__restrict__ T, const float *__restr
 // ------------------------------------------------------------------------------------------------
 // the master kernel
 // ------------------------------------------------------------------------------------------------
+struct Mail;
 struct MasterArgs {
     const float *Dd;
     long long Sp;
@@ -240,6 +241,8 @@ struct MasterArgs {
     int rslots;                 // > 0: every block keeps z, q, T, alpha, beta of its own slots in shared memory
     int cache_segs;             // capacity of the shared-memory tile of Dd in 512-byte segments
     int ul_cap;                 // capacity of the per-chunk lists of unstaged beams (0: they do not fit, masked loops)
+    int nblk;                   // blocks that own chunks: the whole grid (mode 0) or all but the last block (mode 1,
+                                // whose last block solves the reduced problems)
     long long *accbuf;          // 3 rotating sets of kSumGroups records of (2N + 2) fixed-point sums: F, curvature,
                                 // grad[0..K), and (fused mode) the Hessian-vector product [K..2K); a block adds
                                 // to the record of its group (blockIdx mod kSumGroups)
@@ -256,6 +259,14 @@ struct MasterArgs {
     double *trF, *trG, *trC;
     int32_t *trInner;
     int trace_it;
+    // mode 1 (k_newton)
+    long long *hess;            // N x N (upper triangle used): H_F in fixed point, scale hscale
+    float *omref;               // Sp: the omega H_F was built with
+    uint8_t *hvalid;            // N: the column of beam k is in H_F
+    double hscale, hinv;
+    float *wn;                  // second buffer of w (the trial points write z, w to a.zn, a.wn)
+    Mail *mail;                 // message of the solving block, followed by N floats
+    unsigned long long *sync;   // [0] arrivals, [1] epoch published, [2], [3]: where both stand when a launch begins
 };
 
 __device__ __forceinline__ double warp_sum(double v) {
@@ -303,55 +314,16 @@ __device__ __forceinline__ FxScale fx_scale_for(double bound, int &bad) {
 __device__ __forceinline__ void fx_add(long long *dst, double v, double scale) {
     atomicAdd(reinterpret_cast<unsigned long long *>(dst), (unsigned long long)__double2ll_rn(v * scale));
 }
-#ifdef VMAT_MASTER_PROFILE
-__device__ long long g_master_prof[16];
-#define PROF_DECL long long pt_ = clock64(), pacc_[16] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0}
-#define PROF(i)                           \
-    {                                     \
-        const long long n_ = clock64();   \
-        pacc_[i] += n_ - pt_;             \
-        pt_ = n_;                         \
-    }
-#define PROFW(i, j)                       \
-    {                                     \
-        const long long n_ = clock64();   \
-        pacc_[j] += n_ - pt_;             \
-        pacc_[i] += n_ - pt_;             \
-        pt_ = n_;                         \
-    }
-#define PROF_END                                                                  \
-    if (blockIdx.x == 0 && threadIdx.x == 0)                                      \
-        for (int i_ = 0; i_ < 16; ++i_) g_master_prof[i_] += pacc_[i_];
-#define PROFX(j)                          \
-    {                                     \
-        const long long n_ = clock64();   \
-        pacc_[j] += n_ - px_;             \
-        px_ = n_;                         \
-    }
-#define PROFX_START long long px_ = clock64();
-#define PROF_PARAM , long long &pt_, long long (&pacc_)[16]
-#define PROF_ARG , pt_, pacc_
-#else
-#define PROF_PARAM
-#define PROF_ARG
-#define PROFX(j)
-#define PROFX_START
-#define PROF_DECL
-#define PROF(i)
-#define PROFW(i, j)
-#define PROF_END
-#endif
 
 // scalars every thread of the block needs, written by warp 0 (the block's control warp)
 struct Ctl {
-    double scF, scG, scC, scH;   // fixed-point scales of the pass about to run
-    double iF, iG, iC, iH;       // and their inverses
+    double scF, scG, scC;   // fixed-point scales of the pass about to run
+    double iF, iG, iC;      // and their inverses
     float tf;               // trial step of the line search
     int state;              // what the block does next (kRunDirection, ...)
     int accepted;           // the last trial was accepted: the z buffers swap roles
-    int probe;              // fused mode: the pass about to run does not move (t = 0), it only opens a new direction
 };
-enum { kRunDirection = 0, kRunTrial = 1, kFinish = 2, kRunFused = 3 };
+enum { kRunDirection = 0, kRunTrial = 1, kFinish = 2 };
 
 constexpr int kRedSlots = 8;   // values per warp row of the control group's reduction scratch
 // Records of grid-wide sums per rotation slot.  Measured: splitting the blocks into 16 groups with one record each
@@ -396,11 +368,18 @@ static_assert(kMasterWarps == 2 * kGroup, "the staged products give every chunk 
 
 struct Smem {
     double *y, *d, *grad, *pg, *yn, *gn, *dG, *rdt, *gacc, *linf;   // N each (control warp; gacc: 4N, all warps)
-    double *gF, *gFn, *hd, *hdn, *dnx, *gm;   // fused mode, N each: F-part of the gradient, Hessian-vector products
-                                              // (accepted / pending), next direction, predicted gradient
-    double *gpart, *gpartu;   // 2 per staged segment: partial dots of its two threads with w (and, fused mode, u)
-    float *part2, *wbuf, *ubuf, *coef;
-    float *rz0, *rz1, *rq, *rq1, *rT, *ral, *rbe;   // resident copies of the block's own slots (a.rslots each), or unused
+    double *gpart;            // 2 per staged segment: partial dots of its two threads with w
+    float *part2, *wbuf, *coef;
+    float *ombuf, *fl_dw;     // k_newton: omega of the group's slots; change of omega at each chunk's flipped slots
+    float *ubuf;              // k_newton: omega d_new of the group's slots (d_new: the column that is new to H_F)
+    double *gpartu, *gaccu;   // k_newton: like gpart, gacc for the products with ubuf
+    long long *gfxu;          // k_newton: like gfx
+    unsigned char *fl_slot;   // k_newton: the flipped slots of each chunk of the group (kGroup x kChunk), ascending
+    int *fl_wc;               // k_newton: how many each of the four warps of a chunk found
+    int *hm;                  // k_newton: members of the chunk whose Hessian part is being updated (segment | i << 16)
+    int *hv;                  // k_newton: column i is in the Hessian already
+    float *rz0, *rz1, *rq, *rT, *ral, *rbe;   // resident copies of the block's own slots (a.rslots each), or unused
+    float *rom;               // k_newton: resident copy of a.omref (written through)
     float *tile;       // staged 512-byte segments of the block's part of Dd, kSeg floats apart
     int *sk, *lo, *hi, *ik;   // lo, hi: block-local range of chunks (j of b + jG) that may hold entries of column i
     int *nseg;         // how many of them really do
@@ -415,13 +394,13 @@ struct Smem {
                        // the work its lists hold (a staged entry counts 1, an unstaged one 4); fixed per solve
     int *uoff;         // (when a.ul_cap > 0) entries [uoff[j], uoff[j+1]) of ul: the unstaged beams that touch local chunk j
     unsigned short *ul;
-    long long *gfx;    // (when a.ul_cap > 0) fixed-point gradient sums of the unstaged beams: N for w (+ N for u)
+    long long *gfx;    // (when a.ul_cap > 0) fixed-point gradient sums of the unstaged beams, N
     long long *recv;   // the pass's record of grid sums, fetched by the whole block after the barrier
     Ctl *ctl;
 };
 
 // chunk handled by this block as member `ch` of its group `g`: chunks are dealt round-robin
-__device__ __forceinline__ int chunk_of(int g, int ch) { return (int)blockIdx.x + (g * kGroup + ch) * (int)gridDim.x; }
+__device__ __forceinline__ int chunk_of(const MasterArgs &a, int g, int ch) { return (int)blockIdx.x + (g * kGroup + ch) * a.nblk; }
 
 __device__ __forceinline__ bool touches(const Smem &sm, int N, int i, int j) {
     return (sm.lmask[(j >> 6) * N + i] >> (j & 63)) & 1ull;
@@ -439,7 +418,7 @@ __device__ __forceinline__ int seg_rank(const Smem &sm, int N, int i, int j) {
 __device__ __forceinline__ void load_half(const MasterArgs &a, const Smem &sm, int i, int g, int chalf, int lane,
                                           float4 (&v)[kGroup / 2]) {
     const unsigned m = ((unsigned)(sm.lmask[((g * kGroup) >> 6) * a.N + i] >> ((g * kGroup) & 63)) & 0xffu) >> chalf;
-    const int j0 = g * kGroup + chalf, G = (int)gridDim.x;
+    const int j0 = g * kGroup + chalf, G = a.nblk;
     const float4 *row = reinterpret_cast<const float4 *>(a.Dd) +
                         ((size_t)((int)blockIdx.x + j0 * G) * a.N + sm.sk[i]) * (kChunk / 4) + lane;
 #pragma unroll
@@ -470,7 +449,7 @@ __device__ __forceinline__ void warp_share(const Smem &sm, int g, int warp, int 
 __device__ __forceinline__ void combine_unstaged_listed(const MasterArgs &a, const Smem &sm, int j, int r, int c, int lane,
                                                         float4 &s1, float4 &s2) {
     const float4 *Dd4 = reinterpret_cast<const float4 *>(a.Dd) +
-                        (size_t)((int)blockIdx.x + j * (int)gridDim.x) * a.N * (kChunk / 4) + lane;   // the chunk's segments
+                        (size_t)((int)blockIdx.x + j * a.nblk) * a.N * (kChunk / 4) + lane;   // the chunk's segments
     const size_t row4 = kChunk / 4;
     const int n1 = sm.uoff[j + 1];
     for (int n = sm.uoff[j] + r; n < n1; n += 8 * c) {
@@ -525,9 +504,9 @@ __device__ __forceinline__ double warp_sum8(double (&v)[8], int lane) {
 // Gradient dots of the unstaged beams of group g: warp (cs, hf) takes every second entry of chunk g*kGroup + cs,
 // eight beams per step; lane partials over 4 products in fp32, the warp sums in fp64 (warp_sum8), then into the
 // beam's FIXED-POINT accumulator in shared memory (integer adds: order free, so the result stays reproducible
-// although several warps add to one beam).  sm.gfx holds N entries for w and, TWO, N more for u.
-template <bool TWO>
-__device__ __forceinline__ void grad_unstaged_listed(const MasterArgs &a, const Smem &sm, int g, double scG, double scH) {
+// although several warps add to one beam).  buf: the group's vector (laid out like sm.wbuf), gfx: N sums, scale scG.
+__device__ __forceinline__ void grad_unstaged_listed(const MasterArgs &a, const Smem &sm, int g, const float *buf,
+                                                     long long *gfx, double scG) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     int cs, r, c;
     warp_share(sm, g, warp, cs, r, c);
@@ -535,11 +514,9 @@ __device__ __forceinline__ void grad_unstaged_listed(const MasterArgs &a, const 
     const int j = g * kGroup + cs, n1 = sm.uoff[j + 1];
     int n = sm.uoff[j] + r;
     if (n >= n1) return;
-    const float4 w4 = reinterpret_cast<const float4 *>(sm.wbuf)[cs * kSeg4 + lane];
-    float4 u4 = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (TWO) u4 = reinterpret_cast<const float4 *>(sm.ubuf)[cs * kSeg4 + lane];
+    const float4 w4 = reinterpret_cast<const float4 *>(buf)[cs * kSeg4 + lane];
     const float4 *Dd4 = reinterpret_cast<const float4 *>(a.Dd) +
-                        (size_t)((int)blockIdx.x + j * (int)gridDim.x) * a.N * (kChunk / 4) + lane;   // the chunk's segments
+                        (size_t)((int)blockIdx.x + j * a.nblk) * a.N * (kChunk / 4) + lane;   // the chunk's segments
     const size_t row4 = kChunk / 4;
     const int mine = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);   // warp_sum8's layout
     for (; n < n1; n += 8 * c) {
@@ -555,25 +532,17 @@ __device__ __forceinline__ void grad_unstaged_listed(const MasterArgs &a, const 
                 v[x] = __ldg(Dd4 + (size_t)sm.sk[id[x]] * row4);
             }
         }
-        double dw[8], du[8];
+        double dw[8];
 #pragma unroll
-        for (int x = 0; x < 8; ++x) {
+        for (int x = 0; x < 8; ++x)
             dw[x] = (double)((v[x].x * w4.x + v[x].y * w4.y) + (v[x].z * w4.z + v[x].w * w4.w));
-            if (TWO) du[x] = (double)((v[x].x * u4.x + v[x].y * u4.y) + (v[x].z * u4.z + v[x].w * u4.w));
-        }
         const double rw = warp_sum8(dw, lane);
-        double ru = 0.0;
-        if (TWO) ru = warp_sum8(du, lane);
         int my_id = -1;
 #pragma unroll
         for (int x = 0; x < 8; ++x)
             if (x == mine) my_id = id[x];
-        if ((lane & 3) == 0 && my_id >= 0) {
-            atomicAdd(reinterpret_cast<unsigned long long *>(sm.gfx) + my_id, (unsigned long long)__double2ll_rn(rw * scG));
-            if (TWO)
-                atomicAdd(reinterpret_cast<unsigned long long *>(sm.gfx) + a.N + my_id,
-                          (unsigned long long)__double2ll_rn(ru * scH));
-        }
+        if ((lane & 3) == 0 && my_id >= 0)
+            atomicAdd(reinterpret_cast<unsigned long long *>(gfx) + my_id, (unsigned long long)__double2ll_rn(rw * scG));
     }
 }
 
@@ -583,9 +552,8 @@ __device__ __forceinline__ void grad_unstaged_listed(const MasterArgs &a, const 
 // columns that are not staged (Ku of them) follow by the same split.  The two partials of a chunk meet in
 // shared memory.  The caller must __syncthreads() before sm.part2 is written again.
 __device__ __forceinline__ void combine_group(const MasterArgs &a, const Smem &sm, int Ku, int g,
-                                              float (&out)[kOutPerThread] PROF_PARAM) {
+                                              float (&out)[kOutPerThread]) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    PROFX_START
     {
         int cs, r, c;
         warp_share(sm, g, warp, cs, r, c);
@@ -623,7 +591,7 @@ __device__ __forceinline__ void combine_group(const MasterArgs &a, const Smem &s
             // straight from L2 / HBM; a beam that does not touch the chunk is skipped (warp-uniform test)
             const int j = g * kGroup + cs;
             const float4 *Dd4 = reinterpret_cast<const float4 *>(a.Dd) +
-                                (size_t)((int)blockIdx.x + j * (int)gridDim.x) * a.N * (kChunk / 4) + lane;
+                                (size_t)((int)blockIdx.x + j * a.nblk) * a.N * (kChunk / 4) + lane;
             const size_t row4 = kChunk / 4;
             for (int u = r; u < Ku; u += 4 * c) {
                 float4 v[4];
@@ -657,7 +625,6 @@ __device__ __forceinline__ void combine_group(const MasterArgs &a, const Smem &s
         reinterpret_cast<float4 *>(sm.part2)[warp * 32 + lane] =
             make_float4(s1.x + s2.x, s1.y + s2.y, s1.z + s2.z, s1.w + s2.w);
     }
-    PROFX(12)
     __syncthreads();
 #pragma unroll
     for (int r = 0; r < kOutPerThread; ++r) {
@@ -667,25 +634,23 @@ __device__ __forceinline__ void combine_group(const MasterArgs &a, const Smem &s
         for (int w = w0; w < w1; ++w) v += sm.part2[w * kChunk + s];   // the chunk's warps, in order
         out[r] = v;
     }
-    PROFX(13)
 }
 
 // Gradient products of the staged segments of group g: two threads per segment (alternate float4s), each a plain
-// dot of 64 entries with the group's w (TWO: and u) — no exchange between lanes.  Lane partials over 16 products
-// in fp32, then fp64.  The partials land in sm.gpart (sm.gpartu), two per segment; grad_total adds them per beam.
-template <bool TWO>
-__device__ __forceinline__ void grad_staged(const Smem &sm, int g) {
+// dot of 64 entries with the group's vector buf (laid out like sm.wbuf) — no exchange between lanes.  Lane partials
+// over 16 products in fp32, then fp64.  The partials land in gpart, two per segment; grad_total adds them per beam.
+__device__ __forceinline__ void grad_staged(const Smem &sm, int g, const float *buf, double *gpart) {
     const int n0 = sm.coff[g * kGroup], n2 = 2 * (sm.coff[(g + 1) * kGroup] - n0);
     const float4 *tile4 = reinterpret_cast<const float4 *>(sm.tile);
-    const float4 *wb4 = reinterpret_cast<const float4 *>(sm.wbuf), *ub4 = reinterpret_cast<const float4 *>(sm.ubuf);
+    const float4 *wb4 = reinterpret_cast<const float4 *>(buf);
     for (int t2 = threadIdx.x; t2 < n2; t2 += kMasterThreads) {
         const int e = sm.gseg[n0 + (t2 >> 1)], hfs = t2 & 1;
         const int s = e & 0xffff, cs = e >> 16;
-        const float4 *tp = tile4 + s * kSeg4 + hfs, *wp = wb4 + cs * kSeg4 + hfs, *up = ub4 + cs * kSeg4 + hfs;
-        double dw = 0.0, du = 0.0;
+        const float4 *tp = tile4 + s * kSeg4 + hfs, *wp = wb4 + cs * kSeg4 + hfs;
+        double dw = 0.0;
 #pragma unroll
         for (int blk = 0; blk < 4; ++blk) {
-            float4 aw = make_float4(0.f, 0.f, 0.f, 0.f), au = aw;
+            float4 aw = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
             for (int it = 0; it < 4; ++it) {
                 const int x = (blk * 4 + it) * 2;
@@ -694,27 +659,60 @@ __device__ __forceinline__ void grad_staged(const Smem &sm, int g) {
                 aw.y = fmaf(v.y, w.y, aw.y);
                 aw.z = fmaf(v.z, w.z, aw.z);
                 aw.w = fmaf(v.w, w.w, aw.w);
-                if (TWO) {
-                    const float4 u = up[x];
-                    au.x = fmaf(v.x, u.x, au.x);
-                    au.y = fmaf(v.y, u.y, au.y);
-                    au.z = fmaf(v.z, u.z, au.z);
-                    au.w = fmaf(v.w, u.w, au.w);
-                }
             }
             dw += (double)((aw.x + aw.y) + (aw.z + aw.w));
-            if (TWO) du += (double)((au.x + au.y) + (au.z + au.w));
         }
-        sm.gpart[2 * s + hfs] = dw;
-        if (TWO) sm.gpartu[2 * s + hfs] = du;
+        gpart[2 * s + hfs] = dw;
+    }
+}
+
+// Columns that are not staged, when their per-chunk lists do not fit either: this warp's half of the group's chunks
+// (4 chunks) and its share of those beams, two beams per step (eight masked loads), lane partials in fp32 (16
+// products), the warp sums in fp64 to the row of gacc (2 x N) of this chunk half.  buf: laid out like sm.wbuf.
+__device__ __forceinline__ void grad_unstaged_masked(const MasterArgs &a, const Smem &sm, int g, int Ku, const float *buf,
+                                                     double *gacc2) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int kpart = warp & (kKSplit - 1), chalf = warp / kKSplit;
+    float4 w4[kGroup / 2];
+#pragma unroll
+    for (int h = 0; h < kGroup / 2; ++h) w4[h] = reinterpret_cast<const float4 *>(buf)[(2 * h + chalf) * kSeg4 + lane];
+    for (int u = kpart; u < Ku; u += 2 * kKSplit) {
+        const bool has2 = u + kKSplit < Ku;
+        const int i = sm.unc[u], i2 = has2 ? sm.unc[u + kKSplit] : i;
+        float4 v1[kGroup / 2], v2[kGroup / 2];
+        load_half(a, sm, i, g, chalf, lane, v1);
+        load_half(a, sm, i2, g, chalf, lane, v2);
+        float4 s1 = make_float4(0.f, 0.f, 0.f, 0.f), s2 = s1;
+#pragma unroll
+        for (int h = 0; h < kGroup / 2; ++h) {
+            s1.x = fmaf(v1[h].x, w4[h].x, s1.x);
+            s1.y = fmaf(v1[h].y, w4[h].y, s1.y);
+            s1.z = fmaf(v1[h].z, w4[h].z, s1.z);
+            s1.w = fmaf(v1[h].w, w4[h].w, s1.w);
+            s2.x = fmaf(v2[h].x, w4[h].x, s2.x);
+            s2.y = fmaf(v2[h].y, w4[h].y, s2.y);
+            s2.z = fmaf(v2[h].z, w4[h].z, s2.z);
+            s2.w = fmaf(v2[h].w, w4[h].w, s2.w);
+        }
+        double d1 = (double)((s1.x + s1.y) + (s1.z + s1.w)), d2 = (double)((s2.x + s2.y) + (s2.z + s2.w));
+        // one butterfly for both rows: after the first exchange the lower half-warp carries row 1, the upper row 2
+        const bool up = lane & 16;
+        double r = (up ? d2 : d1) + __shfl_xor_sync(kFull, up ? d1 : d2, 16);
+        r += __shfl_xor_sync(kFull, r, 8);
+        r += __shfl_xor_sync(kFull, r, 4);
+        r += __shfl_xor_sync(kFull, r, 2);
+        r += __shfl_xor_sync(kFull, r, 1);
+        double *row = gacc2 + chalf * a.N;      // entries i, i2 of this row are owned by this warp
+        if (lane == 0) row[i] += r;
+        if (lane == 16 && has2) row[i2] += r;
     }
 }
 
 // beam i's total over the block: staged columns add the partials of their segments in chunk order, the others
 // the two chunk-half rows of sm.gacc (row0, row0 + 1)
-__device__ __forceinline__ double grad_total(const Smem &sm, const double *gp, int i, int N, int row0) {
+__device__ __forceinline__ double grad_total(const Smem &sm, const double *gp, const double *gacc, int i, int N) {
     const int bs = sm.base[i];
-    if (bs == kNoCache) return sm.gacc[row0 * N + i] + sm.gacc[(row0 + 1) * N + i];
+    if (bs == kNoCache) return gacc[i] + gacc[N + i];
     double s = 0.0;
     for (int q = 0; q < sm.nseg[i]; ++q) s += gp[2 * (bs + q)] + gp[2 * (bs + q) + 1];
     return s;
@@ -734,23 +732,20 @@ __device__ __forceinline__ void penalty(float z, float T, float al, float be, fl
 template <bool FROM_Y>
 __device__ __forceinline__ void eval_pass(const MasterArgs &a, const Smem &sm, int K, int Ku, int ngroups, const float *zsrc,
                                           float *zdst, const float *rzsrc, float *rzdst, float tf, long long *rec,
-                                          double scF, double scG, double *red PROF_PARAM) {
+                                          double scF, double scG, double *red) {
     const bool res = a.rslots > 0;
-    PROFX_START
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int kpart = warp & (kKSplit - 1), chalf = warp / kKSplit;
+    const int tid = threadIdx.x;
     for (int i = tid; i < 2 * a.N; i += kMasterThreads) sm.gacc[i] = 0.0;
     if (a.ul_cap > 0)
         for (int i = tid; i < a.N; i += kMasterThreads) sm.gfx[i] = 0;
     double F = 0.0;
     __syncthreads();
-    PROFX(8)
     for (int g = 0; g < ngroups; ++g) {
         float zv[kOutPerThread];
-        if (FROM_Y) combine_group(a, sm, Ku, g, zv PROF_ARG);
+        if (FROM_Y) combine_group(a, sm, Ku, g, zv);
 #pragma unroll
         for (int r = 0; r < kOutPerThread; ++r) {
-            const int o = tid + r * kMasterThreads, c = chunk_of(g, o >> 7);
+            const int o = tid + r * kMasterThreads, c = chunk_of(a, g, o >> 7);
             float wv = 0.f;
             if (c < a.nchunks) {
                 const size_t s = (size_t)c * kChunk + (o & (kChunk - 1));
@@ -773,188 +768,21 @@ __device__ __forceinline__ void eval_pass(const MasterArgs &a, const Smem &sm, i
             sm.wbuf[(o >> 7) * kSeg + (o & (kChunk - 1))] = wv;
         }
         __syncthreads();
-        PROFX(9)
-        grad_staged<false>(sm, g);
-        // columns that are not staged: through the per-chunk lists when they fit; otherwise this warp's half of the
-        // group's gradient (4 chunks), and its share of those beams: two beams per step (eight masked loads), lane
-        // partials in fp32 (16 products), the warp sum in fp64 to the row of sm.gacc of this chunk half
+        grad_staged(sm, g, sm.wbuf, sm.gpart);
+        // columns that are not staged: through the per-chunk lists when they fit, otherwise by masked loops
         if (Ku > 0 && a.ul_cap > 0) {
-            grad_unstaged_listed<false>(a, sm, g, scG, 0.0);
+            grad_unstaged_listed(a, sm, g, sm.wbuf, sm.gfx, scG);
         } else if (Ku > 0) {
-        float4 w4[kGroup / 2];
-#pragma unroll
-        for (int h = 0; h < kGroup / 2; ++h) w4[h] = reinterpret_cast<const float4 *>(sm.wbuf)[(2 * h + chalf) * kSeg4 + lane];
-        for (int u = kpart; u < Ku; u += 2 * kKSplit) {
-            const bool has2 = u + kKSplit < Ku;
-            const int i = sm.unc[u], i2 = has2 ? sm.unc[u + kKSplit] : i;
-            float4 v1[kGroup / 2], v2[kGroup / 2];
-            load_half(a, sm, i, g, chalf, lane, v1);
-            load_half(a, sm, i2, g, chalf, lane, v2);
-            float4 s1 = make_float4(0.f, 0.f, 0.f, 0.f), s2 = s1;
-#pragma unroll
-            for (int h = 0; h < kGroup / 2; ++h) {
-                s1.x = fmaf(v1[h].x, w4[h].x, s1.x);
-                s1.y = fmaf(v1[h].y, w4[h].y, s1.y);
-                s1.z = fmaf(v1[h].z, w4[h].z, s1.z);
-                s1.w = fmaf(v1[h].w, w4[h].w, s1.w);
-                s2.x = fmaf(v2[h].x, w4[h].x, s2.x);
-                s2.y = fmaf(v2[h].y, w4[h].y, s2.y);
-                s2.z = fmaf(v2[h].z, w4[h].z, s2.z);
-                s2.w = fmaf(v2[h].w, w4[h].w, s2.w);
-            }
-            double d1 = (double)((s1.x + s1.y) + (s1.z + s1.w)), d2 = (double)((s2.x + s2.y) + (s2.z + s2.w));
-            // one butterfly for both rows: after the first exchange the lower half-warp carries row 1, the upper row 2
-            const bool up = lane & 16;
-            double r = (up ? d2 : d1) + __shfl_xor_sync(kFull, up ? d1 : d2, 16);
-            r += __shfl_xor_sync(kFull, r, 8);
-            r += __shfl_xor_sync(kFull, r, 4);
-            r += __shfl_xor_sync(kFull, r, 2);
-            r += __shfl_xor_sync(kFull, r, 1);
-            double *gacc = sm.gacc + chalf * a.N;      // entries i, i2 of this row are owned by this warp
-            if (lane == 0) gacc[i] += r;
-            if (lane == 16 && has2) gacc[i2] += r;
+            grad_unstaged_masked(a, sm, g, Ku, sm.wbuf, sm.gacc);
         }
-        }
-        PROFX(10)
         __syncthreads();
     }
-    PROFX(11)
     F = block_sum(F, red);
     if (tid == 0) fx_add(rec, F, scF);
     for (int i = tid; i < K; i += kMasterThreads) {
         if (a.ul_cap > 0 && sm.base[i] == kNoCache)   // already in fixed point
             atomicAdd(reinterpret_cast<unsigned long long *>(rec + 2 + i), (unsigned long long)sm.gfx[i]);
-        else fx_add(rec + 2 + i, grad_total(sm, sm.gpart, i, a.N, 0), scG);
-    }
-    PROFX(11)
-}
-
-// The pass of the single-barrier iteration (master_mode 1).  For the block's slots, in one sweep:
-//   z_new = zsrc + t qsrc (the trial point of the direction in flight; probe: z_new = zsrc), F and w there,
-//   q_new = Dc^T d_next (coef holds the next direction), the curvature sum_j omega_j q_new_j^2 of the quadratic
-//   piece at z_new, and the block's share of BOTH K-vectors Dc w_new (the true gradient at the trial point) and
-//   Dc (omega . q_new) (half the Hessian of F at z_new applied to d_next), so that one grid barrier per inner
-//   iteration suffices.  Sums go to the record `rec` in fixed point: F, curvature, grad[0..K), Hd[K..2K).
-__device__ __forceinline__ void fused_pass(const MasterArgs &a, const Smem &sm, int K, int Ku, int ngroups, const float *zsrc,
-                                           float *zdst, const float *rzsrc, float *rzdst, const float *qsrc,
-                                           float *qdst, const float *rqsrc, float *rqdst, float tf, bool probe,
-                                           long long *rec, double scF, double scC, double scG, double scH,
-                                           double *red) {
-    const bool res = a.rslots > 0;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int kpart = warp & (kKSplit - 1), chalf = warp / kKSplit;
-#ifdef VMAT_MASTER_PROFILE
-    long long pt_ = 0, pacc_[16] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
-#endif
-    for (int i = tid; i < 4 * a.N; i += kMasterThreads) sm.gacc[i] = 0.0;
-    if (a.ul_cap > 0)
-        for (int i = tid; i < 2 * a.N; i += kMasterThreads) sm.gfx[i] = 0;
-    double F = 0.0, curv = 0.0;
-    __syncthreads();
-    for (int g = 0; g < ngroups; ++g) {
-        float om[kOutPerThread], qv[kOutPerThread];
-#pragma unroll
-        for (int r = 0; r < kOutPerThread; ++r) {
-            const int o = tid + r * kMasterThreads, c = chunk_of(g, o >> 7);
-            float wv = 0.f, omv = 0.f;
-            if (c < a.nchunks) {
-                const size_t s = (size_t)c * kChunk + (o & (kChunk - 1));
-                const int ls = g * (kGroup * kChunk) + o;
-                float z, Tv, al, be;
-                if (res) {
-                    z = probe ? rzsrc[ls] : fmaf(tf, rqsrc[ls], rzsrc[ls]);
-                    Tv = sm.rT[ls], al = sm.ral[ls], be = sm.rbe[ls];
-                    rzdst[ls] = z;
-                } else {
-                    z = probe ? zsrc[s] : fmaf(tf, qsrc[s], zsrc[s]);
-                    Tv = a.T[s], al = a.alpha[s], be = a.beta[s];
-                    zdst[s] = z;
-                }
-                double f;
-                penalty(z, Tv, al, be, wv, f);
-                F += f;
-                omv = z < Tv ? al : (z > Tv ? be : 0.f);
-            }
-            sm.wbuf[(o >> 7) * kSeg + (o & (kChunk - 1))] = wv;
-            om[r] = omv;
-        }
-        combine_group(a, sm, Ku, g, qv PROF_ARG);   // its barrier also publishes wbuf
-#pragma unroll
-        for (int r = 0; r < kOutPerThread; ++r) {
-            const int o = tid + r * kMasterThreads, c = chunk_of(g, o >> 7);
-            if (c < a.nchunks) {
-                if (res) rqdst[g * (kGroup * kChunk) + o] = qv[r];
-                else qdst[(size_t)c * kChunk + (o & (kChunk - 1))] = qv[r];
-            }
-            curv += (double)om[r] * (double)qv[r] * (double)qv[r];
-            sm.ubuf[(o >> 7) * kSeg + (o & (kChunk - 1))] = om[r] * qv[r];
-        }
-        __syncthreads();
-        grad_staged<true>(sm, g);
-        // columns that are not staged: through the per-chunk lists when they fit; otherwise this warp's half of the
-        // group (4 chunks) and its share of those beams: two beams per step, each row read once for both products;
-        // lane partials in fp32, warp sums in fp64 by one butterfly for all four
-        if (Ku > 0 && a.ul_cap > 0) {
-            grad_unstaged_listed<true>(a, sm, g, scG, scH);
-        } else if (Ku > 0) {
-        float4 w4[kGroup / 2], u4[kGroup / 2];
-#pragma unroll
-        for (int h = 0; h < kGroup / 2; ++h) {
-            w4[h] = reinterpret_cast<const float4 *>(sm.wbuf)[(2 * h + chalf) * kSeg4 + lane];
-            u4[h] = reinterpret_cast<const float4 *>(sm.ubuf)[(2 * h + chalf) * kSeg4 + lane];
-        }
-        for (int u = kpart; u < Ku; u += 2 * kKSplit) {
-            const bool has2 = u + kKSplit < Ku;
-            const int i = sm.unc[u], i2 = has2 ? sm.unc[u + kKSplit] : i;
-            float4 v1[kGroup / 2], v2[kGroup / 2];
-            load_half(a, sm, i, g, chalf, lane, v1);
-            load_half(a, sm, i2, g, chalf, lane, v2);
-            float2 w1 = make_float2(0.f, 0.f), w2 = w1, u1 = w1, u2 = w1;
-#pragma unroll
-            for (int h = 0; h < kGroup / 2; ++h) {
-                w1.x = fmaf(v1[h].x, w4[h].x, fmaf(v1[h].y, w4[h].y, w1.x));
-                w1.y = fmaf(v1[h].z, w4[h].z, fmaf(v1[h].w, w4[h].w, w1.y));
-                w2.x = fmaf(v2[h].x, w4[h].x, fmaf(v2[h].y, w4[h].y, w2.x));
-                w2.y = fmaf(v2[h].z, w4[h].z, fmaf(v2[h].w, w4[h].w, w2.y));
-                u1.x = fmaf(v1[h].x, u4[h].x, fmaf(v1[h].y, u4[h].y, u1.x));
-                u1.y = fmaf(v1[h].z, u4[h].z, fmaf(v1[h].w, u4[h].w, u1.y));
-                u2.x = fmaf(v2[h].x, u4[h].x, fmaf(v2[h].y, u4[h].y, u2.x));
-                u2.y = fmaf(v2[h].z, u4[h].z, fmaf(v2[h].w, u4[h].w, u2.y));
-            }
-            const double dw1 = (double)(w1.x + w1.y), dw2 = (double)(w2.x + w2.y);
-            const double du1 = (double)(u1.x + u1.y), du2 = (double)(u2.x + u2.y);
-            // after the exchange at 16 the lower half-warp carries row 1, the upper row 2; after the exchange at 8
-            // the quarters carry (row 1, w), (row 1, u), (row 2, w), (row 2, u)
-            const bool up = lane & 16, uq = lane & 8;
-            const double rw = (up ? dw2 : dw1) + __shfl_xor_sync(kFull, up ? dw1 : dw2, 16);
-            const double ru = (up ? du2 : du1) + __shfl_xor_sync(kFull, up ? du1 : du2, 16);
-            double r = (uq ? ru : rw) + __shfl_xor_sync(kFull, uq ? rw : ru, 8);
-            r += __shfl_xor_sync(kFull, r, 4);
-            r += __shfl_xor_sync(kFull, r, 2);
-            r += __shfl_xor_sync(kFull, r, 1);
-            double *gw = sm.gacc + chalf * a.N, *gu = sm.gacc + (2 + chalf) * a.N;   // entries owned by this warp
-            if (lane == 0) gw[i] += r;
-            if (lane == 8) gu[i] += r;
-            if (lane == 16 && has2) gw[i2] += r;
-            if (lane == 24 && has2) gu[i2] += r;
-        }
-        }
-        __syncthreads();
-    }
-    F = block_sum(F, red);
-    curv = block_sum(curv, red);
-    if (tid == 0) {
-        fx_add(rec, F, scF);
-        fx_add(rec + 1, curv, scC);
-    }
-    for (int i = tid; i < K; i += kMasterThreads) {
-        if (a.ul_cap > 0 && sm.base[i] == kNoCache) {   // already in fixed point
-            atomicAdd(reinterpret_cast<unsigned long long *>(rec + 2 + i), (unsigned long long)sm.gfx[i]);
-            atomicAdd(reinterpret_cast<unsigned long long *>(rec + 2 + K + i), (unsigned long long)sm.gfx[a.N + i]);
-        } else {
-            fx_add(rec + 2 + i, grad_total(sm, sm.gpart, i, a.N, 0), scG);
-            fx_add(rec + 2 + K + i, grad_total(sm, sm.gpartu, i, a.N, 2), scH);
-        }
+        else fx_add(rec + 2 + i, grad_total(sm, sm.gpart, sm.gacc, i, a.N), scG);
     }
 }
 
@@ -1007,24 +835,32 @@ __device__ __forceinline__ double smooth_part(const double *v, const Smem &sm, i
     return s;
 }
 
-template <int MODE>   // 0: two passes and two grid barriers per inner iteration, 1: one fused pass and one barrier
-__global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a) {
-    extern __shared__ float4 smem_raw[];   // 16-byte aligned: float4 tiles first, then doubles, floats, ints
+// What both master kernels do first: carve up the block's shared memory, list the occupied beams, stage the block's
+// part of Dd and build the lists over it.  NEWTON: the block also lays out what the Hessian updates of k_newton need.
+struct Setup {
+    int K, Ku, ngroups, segs;   // occupied beams, unstaged beams touching this block, groups of chunks, touched segments
+    double l1max;               // max over occupied beams of sum |d_k|
+    double *red, *cred;         // reduction scratch of the block / of its control group
+};
+
+template <bool NEWTON>
+__device__ __forceinline__ Setup master_setup(const MasterArgs &a, Smem &sm, float4 *smem_raw) {
     const int N = a.N, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    Smem sm;
-    constexpr int F1 = MODE == 1 ? 1 : 0;   // what only the single-barrier iteration needs is not laid out in mode 0
+    constexpr int F1 = NEWTON ? 1 : 0;
     sm.part2 = reinterpret_cast<float *>(smem_raw);
     sm.wbuf = sm.part2 + 2 * kGroup * kChunk;
-    sm.ubuf = sm.wbuf + kGroup * kSeg;
-    sm.tile = sm.ubuf + F1 * kGroup * kSeg;
+    sm.ombuf = sm.wbuf + kGroup * kSeg;             // NEWTON: omega of the group's slots, laid out like wbuf
+    sm.ubuf = sm.ombuf + F1 * kGroup * kSeg;        // NEWTON: omega d_new
+    sm.fl_dw = sm.ubuf + F1 * kGroup * kSeg;        // NEWTON: change of omega at the flipped slots of each chunk
+    sm.tile = sm.fl_dw + F1 * kGroup * kChunk;
     sm.rz0 = sm.tile + (size_t)a.cache_segs * kSeg;
     sm.rz1 = sm.rz0 + a.rslots;
     sm.rq = sm.rz1 + a.rslots;
-    sm.rq1 = sm.rq + a.rslots;
-    sm.rT = sm.rq1 + F1 * a.rslots;
+    sm.rT = sm.rq + a.rslots;
     sm.ral = sm.rT + a.rslots;
     sm.rbe = sm.ral + a.rslots;
-    sm.y = reinterpret_cast<double *>(sm.rbe + a.rslots);
+    sm.rom = sm.rbe + a.rslots;
+    sm.y = reinterpret_cast<double *>(sm.rom + F1 * a.rslots);
     sm.d = sm.y + N;
     sm.grad = sm.d + N;
     sm.pg = sm.grad + N;
@@ -1033,20 +869,16 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     sm.dG = sm.gn + N;
     sm.rdt = sm.dG + N;
     sm.gacc = sm.rdt + N;
-    sm.linf = sm.gacc + (2 + 2 * F1) * N;   // gacc: one row per chunk half (and per product in fused mode)
-    sm.gF = sm.linf + N;
-    sm.gFn = sm.gF + F1 * N;
-    sm.hd = sm.gFn + F1 * N;
-    sm.hdn = sm.hd + F1 * N;
-    sm.dnx = sm.hdn + F1 * N;
-    sm.gm = sm.dnx + F1 * N;
-    sm.gpart = sm.gm + F1 * N;
+    sm.gaccu = sm.gacc + 2 * N;  // gacc: one row per chunk half
+    sm.linf = sm.gaccu + F1 * 2 * N;
+    sm.gpart = sm.linf + N;
     sm.gpartu = sm.gpart + 2 * a.cache_segs;
-    const int ngroups = (a.nchunks + (int)gridDim.x * kGroup - 1) / ((int)gridDim.x * kGroup);
+    const int ngroups = (a.nchunks + a.nblk * kGroup - 1) / (a.nblk * kGroup);
     const int W64 = (ngroups * kGroup + 63) >> 6;   // 64-bit words of a column's local chunk mask
     sm.lmask = reinterpret_cast<unsigned long long *>(sm.gpartu + F1 * 2 * a.cache_segs);
     sm.gfx = reinterpret_cast<long long *>(sm.lmask + (size_t)W64 * N);
-    double *red = reinterpret_cast<double *>(sm.gfx + (a.ul_cap > 0 ? (1 + F1) * N : 0));
+    sm.gfxu = sm.gfx + (a.ul_cap > 0 ? N : 0);
+    double *red = reinterpret_cast<double *>(sm.gfxu + (a.ul_cap > 0 ? F1 * N : 0));
     double *cred = red + kMasterWarps;   // 2 x kMasterWarps x kRedSlots
     sm.recv = reinterpret_cast<long long *>(cred + 2 * kMasterWarps * kRedSlots);
     sm.ctl = reinterpret_cast<Ctl *>(sm.recv + 2 * N + 2);
@@ -1063,7 +895,11 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     sm.coff = sm.nseg + N;   // ngroups * kGroup + 1
     sm.wst = sm.coff + ngroups * kGroup + 1;    // ngroups * (kGroup + 1)
     sm.uoff = sm.wst + ngroups * (kGroup + 1);  // like coff, if a.ul_cap > 0
-    sm.ul = reinterpret_cast<unsigned short *>(sm.uoff + ngroups * kGroup + 1);   // a.ul_cap 16-bit beam numbers, last array
+    sm.hm = sm.uoff + (a.ul_cap > 0 ? ngroups * kGroup + 1 : 0);   // NEWTON: N members of the chunk being updated
+    sm.hv = sm.hm + F1 * N;                                        // NEWTON: N flags, column i is in the Hessian
+    sm.fl_wc = sm.hv + F1 * N;                                     // NEWTON: kGroup x 4 flipped slots per warp of a chunk
+    sm.fl_slot = reinterpret_cast<unsigned char *>(sm.fl_wc + F1 * (kGroup * 4 + 4));   // NEWTON: kGroup x kChunk
+    sm.ul = reinterpret_cast<unsigned short *>(sm.fl_slot + F1 * kGroup * kChunk);   // a.ul_cap 16-bit beam numbers, last array
     __shared__ int sK, sKu, sSegs;
     __shared__ uint64_t tile_bar;
 
@@ -1103,7 +939,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
         if (i >= 0) {
             const ColStat cs = a.colstat[k];
             // the block's chunks are b + jG: column k touches those with lo <= j <= hi (empty: hi < lo)
-            const int b = (int)blockIdx.x, Gd_ = (int)gridDim.x;
+            const int b = (int)blockIdx.x, Gd_ = a.nblk;
             sm.lo[i] = cs.clo > b ? (cs.clo - b + Gd_ - 1) / Gd_ : 0;
             sm.hi[i] = cs.chi >= b ? (cs.chi - b) / Gd_ : -1;
             // which of them hold a non-zero entry of the column (the range is half empty: an aperture lights a
@@ -1134,7 +970,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     // The block's chunks are b + jG; column i touches those with j0_i <= j <= j1_i.  Segments are
     // packed column after column until the tile is full; the rest stays in L2 / HBM.
     {
-        const int G = (int)gridDim.x, b = (int)blockIdx.x;
+        const int G = a.nblk, b = (int)blockIdx.x;
         if (tid == 0) mbar_init(&tile_bar, 1);
         __syncthreads();
         if (warp == 0) {
@@ -1290,7 +1126,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
             const int j = g * kGroup + cs;
             int v = sm.coff[j + 1] - sm.coff[j];
             if (a.ul_cap > 0) v += 4 * (sm.uoff[j + 1] - sm.uoff[j]);
-            else if (chunk_of(g, cs) < a.nchunks) v += 4 * Ku;
+            else if (chunk_of(a, g, cs) < a.nchunks) v += 4 * Ku;
             wgt[cs] = v;
             tot += v;
         }
@@ -1325,6 +1161,27 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     }
     __syncthreads();
     mbar_wait(&tile_bar, 0);  // the staged segments have landed (the lists were built while they were in flight)
+    Setup st;
+    st.K = K;
+    st.Ku = Ku;
+    st.ngroups = ngroups;
+    st.segs = sSegs;
+    st.l1max = l1max;
+    st.red = red;
+    st.cred = cred;
+    return st;
+}
+
+// Mode 0: gradient projection with conjugate directions on the current face; two passes over the columns and two
+// grid barriers per inner iteration (q = Dc^T d and the curvature, then the trial point).
+__global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a) {
+    extern __shared__ float4 smem_raw[];   // 16-byte aligned: float4 tiles first, then doubles, floats, ints
+    const int N = a.N, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    Smem sm;
+    const Setup su = master_setup<false>(a, sm, smem_raw);
+    const int K = su.K, Ku = su.Ku, ngroups = su.ngroups, sSegs = su.segs;
+    const double l1max = su.l1max;
+    double *red = su.red, *cred = su.cred;
     const double Tm = (double)a.Tmax, ab = (double)a.abmax, Spd = (double)a.Sp;
 
     const int recn = 2 * N + 2;
@@ -1336,7 +1193,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     float *rzcur = sm.rz0, *rznext = sm.rz1;
     if (res) {
         for (int ls = tid; ls < a.rslots; ls += kMasterThreads) {
-            const int c = (int)blockIdx.x + (ls >> 7) * (int)gridDim.x;
+            const int c = (int)blockIdx.x + (ls >> 7) * a.nblk;
             const bool in = c < a.nchunks;
             const size_t s = (size_t)c * kChunk + (ls & (kChunk - 1));
             sm.rT[ls] = in ? a.T[s] : 0.f;
@@ -1464,83 +1321,6 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
         if (tid == 0) sm.ctl->tf = (float)t;
     };
 
-    // ---- single-barrier iteration (MODE 1) ---------------------------------------------------------------
-    // State between passes: y (accepted point) with its true gradient grad = gF + gamma dG and projected gradient
-    // pg; the direction in flight d with q = Dc^T d in the current q buffer and hd = (Hessian of F at z) d; the
-    // trial step t.  make_trial_and_next sets the trial point yn = y + t d, predicts the gradient there on the
-    // quadratic piece, gm = gF + t hd + gamma dG(yn) (exact while no voxel changes sides of T_j along the step),
-    // and builds from it the NEXT direction dnx (Polak-Ribiere+ on the current face), whose q, curvature and
-    // Hessian-vector product the coming pass computes together with the true F and gradient at yn.  Directions
-    // therefore rest on a prediction, every step length, acceptance test and stop test on true values.  A probe
-    // (pr = 1) is a pass with t = 0 that opens the steepest-descent direction -pg.
-    int probe = 0;
-    auto make_trial_and_next = [&](int pr) {
-        probe = pr;
-        if (pr) {
-            t = 0.0;
-            hit = 0;
-        }
-        for (int k = tid; k < N; k += CT) {
-            const double yk = sm.y[k], dk = sm.d[k];
-            double v = pr ? yk : yk + t * dk;
-            if (!pr && sm.ik[k] >= 0) {
-                if (v < lb || (hit && dk < 0.0 && (yk - lb) / (-dk) <= tmax)) v = lb;
-                else if (has_ub && (v > ub || (hit && dk > 0.0 && (ub - yk) / dk <= tmax))) v = ub;
-            }
-            sm.yn[k] = v;
-        }
-        ctl_sync(CT);
-        double sg[1] = {smooth_part(sm.yn, sm, N, CT, true)}, mx = 0.0;
-        ctl_reduce<1>(sg, mx, cred, tog, nw, CT);   // its barrier also publishes dG
-        Gn = sg[0];
-        double s[3] = {0.0, 0.0, 0.0};
-        mx = 0.0;
-        for (int k = tid; k < N; k += CT) {
-            const int i = sm.ik[k];
-            const double gmk = i >= 0 ? sm.gF[k] + t * sm.hd[k] + a.gamma * sm.dG[k] : 0.0;
-            const double yk = sm.yn[k], po = sm.pg[k];
-            const double pn = (i < 0 || at_bound(yk, gmk)) ? 0.0 : gmk;
-            sm.gm[k] = gmk;
-            sm.gn[k] = pn;   // scratch until the pass returns the true gradient
-            s[0] += pn * (pn - po);
-            s[1] += po * po;
-            s[2] += ((pn == 0.0) != (po == 0.0)) ? 1.0 : 0.0;
-        }
-        ctl_reduce<3>(s, mx, cred, tog, nw, CT);
-        const bool changed = hit || s[2] > 0.0;
-        double bpr = (pr || changed || !(s[1] > 0.0) || s[0] <= 0.0) ? 0.0 : s[0] / s[1];
-        double qbn = 0.0;
-        for (int pass = 0; pass < 2; ++pass) {
-            double s2[2] = {0.0, 0.0};
-            mx = 0.0;
-            for (int k = tid; k < N; k += CT) {
-                const double pn = sm.gn[k], yk = sm.yn[k];
-                double dk = -pn + bpr * sm.d[k];
-                if (sm.ik[k] < 0 || at_bound(yk, -dk)) dk = 0.0;   // stay feasible
-                sm.dnx[k] = dk;
-                s2[0] += sm.gm[k] * dk;
-                s2[1] += fabs(dk) * sm.linf[k];
-            }
-            ctl_reduce<2>(s2, mx, cred, tog, nw, CT);
-            qbn = s2[1];
-            if (s2[0] < 0.0 || bpr == 0.0) break;
-            bpr = 0.0;   // the conjugate direction does not descend on the prediction: steepest descent
-        }
-        set_eval_scales(pr ? yb : yb + t * qb);
-        const FxScale sC = fx_scale_for(1.01 * Spd * ab * qbn * qbn, bad);
-        const FxScale sH = fx_scale_for(1.01 * ab * qbn * l1max, bad);
-        for (int i = tid; i < K; i += CT) sm.coef[i] = (float)sm.dnx[sm.sk[i]];
-        if (tid == 0) {
-            sm.ctl->scC = sC.scale;
-            sm.ctl->iC = sC.inv;
-            sm.ctl->scH = sH.scale;
-            sm.ctl->iH = sH.inv;
-            sm.ctl->tf = (float)t;
-            sm.ctl->probe = pr;
-        }
-    };
-
-    PROF_DECL;
     // objective and gradient at the incoming y
     if (ctl) {
         double s[2] = {0.0, smooth_part(sm.y, sm, N, CT, true)}, mx = 0.0;
@@ -1553,18 +1333,19 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     __syncthreads();
     // Warm entry: the previous solve left z, w, F and d_k . w of its beams current, and the one beam the leaf search
     // has occupied since enters at y = 0, so the dose has not moved; its own d_k . w is the price the search formed
-    // minus the smoothing term.  The evaluation pass (and its grid barrier) is then not needed.
-    const bool warm = MODE == 0 && a.warm && a.gflag[0] == 1 && a.sel->beam >= 0;
+    // minus the smoothing term.  The evaluation pass (and its grid barrier) is then not needed.  With a lower bound
+    // y_min > 0 (vmat_set_dose_rate_bounds) the new beam enters at y_min and the dose does move: no warm entry.
+    const bool warm = a.warm && a.lb == 0.0 && a.gflag[0] == 1 && a.sel->beam >= 0;
     long long *rec = nullptr;
     if (!warm) {
         rec = begin_pass();
-        eval_pass<true>(a, sm, K, Ku, ngroups, nullptr, zcur, nullptr, rzcur, 0.f, rec, sm.ctl->scF, sm.ctl->scG, red PROF_ARG);
+        eval_pass<true>(a, sm, K, Ku, ngroups, nullptr, zcur, nullptr, rzcur, 0.f, rec, sm.ctl->scF, sm.ctl->scG, red);
         cg::this_grid().sync();
         ++ph;
         fetch_record(rec, K + 2);
     } else if (res) {
         for (int ls = tid; ls < a.rslots; ls += kMasterThreads) {
-            const int c = (int)blockIdx.x + (ls >> 7) * (int)gridDim.x;
+            const int c = (int)blockIdx.x + (ls >> 7) * a.nblk;
             rzcur[ls] = c < a.nchunks ? a.z[(size_t)c * kChunk + (ls & (kChunk - 1))] : 0.f;
         }
     }
@@ -1583,10 +1364,6 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
             }
             const double p = (i < 0 || at_bound(sm.y[k], gk)) ? 0.0 : gk;
             sm.grad[k] = gk;
-            if (MODE == 1) {
-                sm.gF[k] = i >= 0 ? (double)sm.recv[2 + i] * iG : 0.0;
-                sm.hd[k] = 0.0;
-            }
             sm.pg[k] = p;
             sm.d[k] = -p;
             pgl = fmax(pgl, fabs(p));
@@ -1604,9 +1381,6 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
         else if (a.max_inner <= 0) {
             stop = 1;
             state = kFinish;
-        } else if (MODE == 1) {
-            make_trial_and_next(1);   // open the steepest-descent direction
-            state = bad ? kFinish : kRunFused;
         } else if (!prepare_direction()) state = kFinish;
         if (tid == 0) {
             sm.ctl->state = state;
@@ -1615,130 +1389,16 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     }
     __syncthreads();
 
-    if constexpr (MODE == 1) {
-        float *qcur = a.q, *qnext = a.q2, *rqcur = sm.rq, *rqnext = sm.rq1;
-        while (sm.ctl->state != kFinish) {
-            rec = begin_pass();
-            fused_pass(a, sm, K, Ku, ngroups, zcur, znext, rzcur, rznext, qcur, qnext, rqcur, rqnext, sm.ctl->tf,
-                       sm.ctl->probe != 0, rec, sm.ctl->scF, sm.ctl->scC, sm.ctl->scG, sm.ctl->scH, red);
-            cg::this_grid().sync();
-            ++ph;
-            fetch_record(rec, 2 * K + 2);
-            if (ctl) {
-                // the true values at the trial point yn, and what the pass found along the next direction dnx
-                const double iG = sm.ctl->iG, iH = sm.ctl->iH;
-                const double Fn = (double)sm.recv[0] * sm.ctl->iF + a.F_out;
-                const double curvF = (double)sm.recv[1] * sm.ctl->iC;
-                double s[1] = {0.0}, pgm = 0.0;
-                for (int k = tid; k < N; k += CT) {
-                    const int i = sm.ik[k];
-                    const double gf = i >= 0 ? (double)sm.recv[2 + i] * iG : 0.0;
-                    const double gk = i >= 0 ? gf + a.gamma * sm.dG[k] : 0.0;
-                    const double yk = sm.yn[k];
-                    const double pn = (i < 0 || at_bound(yk, gk)) ? 0.0 : gk;
-                    sm.gFn[k] = gf;
-                    sm.gn[k] = gk;
-                    sm.hdn[k] = i >= 0 ? 2.0 * (double)sm.recv[2 + K + i] * iH : 0.0;
-                    s[0] += gk * sm.d[k];
-                    pgm = fmax(pgm, fabs(pn));
-                }
-                ctl_reduce<1>(s, pgm, cred, tog, nw, CT);
-                const double Phin = Fn + a.gamma * Gn;
-                // sufficient decrease; below the resolution of Phi accept on the slope instead
-                const bool accepted = probe || Phin <= Phi + c1a * t * phi1 ||
-                                      (Phin <= Phi + noise * fabs(Phi) && fabs(s[0]) <= 0.9 * fabs(phi1));
-                int state = kRunFused;
-                if (accepted) {
-                    const int was_probe = probe;
-                    if (!was_probe) {
-                        stall = (Phi - Phin <= stall_threshold(Phin) * fabs(Phi)) ? stall + 1 : 0;
-                        F = Fn;
-                        Gs = Gn;
-                        Phi = Phin;
-                        ++inner;
-                    }
-                    pgmax = pgm;
-                    for (int k = tid; k < N; k += CT) {
-                        const double yk = sm.yn[k], gk = sm.gn[k];
-                        sm.y[k] = yk;
-                        sm.grad[k] = gk;
-                        sm.gF[k] = sm.gFn[k];
-                        sm.hd[k] = sm.hdn[k];
-                        sm.pg[k] = (sm.ik[k] < 0 || at_bound(yk, gk)) ? 0.0 : gk;
-                        sm.d[k] = sm.dnx[k];
-                    }
-                    ctl_sync(CT);
-                    if (!(pgmax > tol)) state = kFinish;
-                    else if (stall >= a.stall_count) {
-                        stop = 4;
-                        state = kFinish;
-                    } else if (inner >= a.max_inner) {
-                        stop = 1;
-                        state = kFinish;
-                    } else {
-                        direction_sums();   // slope, bounds, G(d) and the largest feasible step of the new direction
-                        if (!(phi1 < 0.0)) {
-                            if (was_probe) {
-                                stop = 2;
-                                state = kFinish;
-                            } else make_trial_and_next(1);
-                        } else {
-                            const double phi2 = 2.0 * curvF + 2.0 * a.gamma * Gd;
-                            t = phi2 > 0.0 ? -phi1 / phi2 : (isfinite(tmax) ? tmax : 1.0);
-                            hit = 0;
-                            if (t >= tmax) {
-                                t = tmax;
-                                hit = 1;
-                            }
-                            half = 0;
-                            make_trial_and_next(0);
-                        }
-                    }
-                } else {
-                    t *= 0.5;
-                    hit = 0;
-                    ++backtracks;
-                    if (++half >= 60) {
-                        stop = 3;
-                        state = kFinish;
-                    } else make_trial_and_next(0);
-                }
-                if (bad) state = kFinish;
-                if (tid == 0) {
-                    sm.ctl->state = state;
-                    sm.ctl->accepted = accepted ? 1 : 0;
-                }
-            }
-            __syncthreads();
-            if (sm.ctl->accepted) {
-                float *tmp = zcur;
-                zcur = znext;
-                znext = tmp;
-                tmp = rzcur;
-                rzcur = rznext;
-                rznext = tmp;
-                tmp = qcur;
-                qcur = qnext;
-                qnext = tmp;
-                tmp = rqcur;
-                rqcur = rqnext;
-                rqnext = tmp;
-            }
-        }
-    }
-    if constexpr (MODE == 0)
     while (sm.ctl->state != kFinish) {
-        PROF(7)
         // ---- q = Dc^T d and the curvature of the quadratic piece at t = 0 ------------------------------
         rec = begin_pass();
-        PROFX_START
         double curv = 0.0;
         for (int g = 0; g < ngroups; ++g) {
             float qv[kOutPerThread];
-            combine_group(a, sm, Ku, g, qv PROF_ARG);
+            combine_group(a, sm, Ku, g, qv);
 #pragma unroll
             for (int r = 0; r < kOutPerThread; ++r) {
-                const int o = tid + r * kMasterThreads, c = chunk_of(g, o >> 7);
+                const int o = tid + r * kMasterThreads, c = chunk_of(a, g, o >> 7);
                 if (c < a.nchunks) {
                     const size_t sl = (size_t)c * kChunk + (o & (kChunk - 1));
                     const int ls = g * (kGroup * kChunk) + o;
@@ -1756,13 +1416,9 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
             }
             __syncthreads();
         }
-        PROFX(14)
         curv = block_sum(curv, red);
         if (tid == 0) fx_add(rec + 1, curv, sm.ctl->scC);
-        PROFX(15)
-        PROF(0)
         cg::this_grid().sync();
-        PROF(1)
         ++ph;
         fetch_record(rec, K + 2);
         if (ctl) {
@@ -1780,15 +1436,12 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
             if (tid == 0) sm.ctl->state = bad ? kFinish : kRunTrial;
         }
         __syncthreads();
-        PROF(2)
         // ---- backtracking on the true cost ----------------------------------------------------------------
         while (sm.ctl->state == kRunTrial) {
             rec = begin_pass();
             eval_pass<false>(a, sm, K, Ku, ngroups, zcur, znext, rzcur, rznext, sm.ctl->tf, rec, sm.ctl->scF,
-                             sm.ctl->scG, red PROF_ARG);
-            PROF(3)
+                             sm.ctl->scG, red);
             cg::this_grid().sync();
-            PROF(4)
             ++ph;
             fetch_record(rec, K + 2);
             if (ctl) {
@@ -1878,7 +1531,6 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
                 }
             }
             __syncthreads();
-            PROF(5)
             if (sm.ctl->accepted) {
                 float *tmpz = zcur;
                 zcur = znext;
@@ -1889,7 +1541,6 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
             }
         }
     }
-    PROF_END
 
     // z, w and the cost from the final y (no drift from the z += t q updates)
     __syncthreads();
@@ -1909,7 +1560,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     __syncthreads();
     if (sm.ctl->accepted) {
         rec = begin_pass();
-        eval_pass<true>(a, sm, K, Ku, ngroups, nullptr, a.z, nullptr, rzcur, 0.f, rec, sm.ctl->scF, sm.ctl->scG, red PROF_ARG);
+        eval_pass<true>(a, sm, K, Ku, ngroups, nullptr, a.z, nullptr, rzcur, 0.f, rec, sm.ctl->scF, sm.ctl->scG, red);
         cg::this_grid().sync();
         ++ph;
         fetch_record(rec, K + 2);
@@ -1958,44 +1609,898 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
     }
 }
 
-// shared memory of one master block; mode 1 (single-barrier iteration) lays out more (k_master's carve-up)
-size_t seg_bytes(int mode) { return kSeg * 4 + (mode == 1 ? 2 : 1) * 2 * 8 + 2 * 4; }   // tile, gpart (+ gpartu), cseg + gseg
+// ------------------------------------------------------------------------------------------------
+// Mode 1: semismooth Newton on the reduced problem (k_newton)
+// ------------------------------------------------------------------------------------------------
+// F is piecewise quadratic in the dose, so on the piece of the current dose the master problem is the quadratic
+//     min_{lb <= y <= ub}  g.(y' - y) + 1/2 (y' - y)^T (2 H_F + 2 gamma L) (y' - y),
+//     H_F[k][k'] = sum_s omega_s d_k[s] d_k'[s],  omega_s = alpha_s (z_s < T_s), beta_s (z_s > T_s), else 0,
+// over the K <= N occupied beams: a problem in K unknowns that needs no pass over the columns at all once H_F is
+// known.  One block of the grid (the last one) holds H_F in its shared memory and solves that quadratic by
+// conjugate gradients on the faces of the box (Jacobi-preconditioned, fp64 vectors); the other blocks evaluate the
+// TRUE cost and gradient at the point it proposes, in one pass each (z = sum_k y_k d_k formed from y itself, so
+// there is no z += t q drift and no closing pass).  The piece changes only where a voxel crosses its T_s, so a
+// master solve takes two or three such passes instead of the twenty-odd of mode 0 (same minimiser: reading S11).
+//
+// H_F lives in global memory in 64-bit fixed point (integer adds: order free, so a solve stays bit-reproducible) and
+// is kept current INCREMENTALLY: every pass compares omega at its dose with the omega the matrix was built with
+// (a.omref) and, chunk by chunk, adds  sum_{s flipped} (omega_new - omega_ref)_s d_k[s] d_k'[s]  for the pairs of
+// columns that touch the chunk; a column that is not in the matrix yet (the aperture the leaf search has just
+// committed; all of them after vmat_set_plan) enters with all its slots.  Measured on configs[1]: 24 of 830 chunks
+// see a flip in a late pass.
+//
+// Hand-over between the solving block and the working blocks: a message in global memory (struct Mail + the
+// coefficients) published by a release store of a monotone epoch counter the workers spin on, and a monotone arrival
+// counter the solver spins on; no grid-wide barrier.  Both counters run on from launch to launch (bases in a.sync).
+#ifdef VMAT_NEWTON_TRACE
+__device__ unsigned long long g_tr[4][4096];   // per pass: published, last block saw it, last block arrived, solver saw the arrivals
+__device__ unsigned int g_trn;
+__device__ long long g_seg[8];
+__device__ __forceinline__ unsigned long long gtime() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+#define TR(stmt) stmt
+#else
+#define TR(stmt)
+#endif
+struct Mail {
+    double scF, scG;   // fixed-point scales of the pass to run
+    int state;         // kRunTrial: evaluate at the coefficients that follow; kFinish: stop
+    int dst;           // kRunTrial: write z, w to buffer pair dst (0: a.z / a.w, 1: a.zn / a.wn)
+    int cur;           // kFinish: the buffer pair that holds the accepted point
+    int pad;
+};
 
-size_t master_smem_bytes(int64_t N, int64_t rslots, int64_t cache_segs, int64_t ngroups, int mode, int64_t ul_cap) {
-    const int f1 = mode == 1 ? 1 : 0;
-    return (size_t)(2 * kGroup * kChunk + (1 + f1) * kGroup * kSeg + (6 + f1) * rslots) * 4   // part2, wbuf (ubuf), resident slots
-           + (size_t)cache_segs * seg_bytes(mode)                                            // tile and the lists over it
-           + (size_t)((13 + 8 * f1) * N + 2 * N + 2 + kMasterWarps + 2 * kMasterWarps * kRedSlots) * 8 + sizeof(Ctl)   // K-vectors, recv, red, cred, ctl
+__device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long long *p) {
+    unsigned long long v;
+    asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release_u64(unsigned long long *p, unsigned long long v) {
+    asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+// spin until *p >= want.  The wait is bounded (about ten seconds): all blocks of a cooperative launch are resident,
+// so the other side always arrives; the bound only keeps a defect from hanging the device.  false = gave up.
+__device__ __forceinline__ bool spin_until(const unsigned long long *p, unsigned long long want) {
+    for (unsigned n = 0; ld_acquire_u64(p) < want; ++n) {
+        if (n > (1u << 23)) return false;
+        __nanosleep(n < 64 ? 20 : 200);
+    }
+    return true;
+}
+
+// H_F += the change the group's chunks owe it (see above): the pairs of columns already in the matrix take the
+// flipped slots of a chunk.  all_slots: the pairs with a column that is not in the matrix yet take every slot of the
+// chunk with the new omega (the slow, general way in; a single new column comes in through newton_pass's second
+// gradient product instead).
+__device__ __forceinline__ void hess_update(const MasterArgs &a, const Smem &sm, int Ku, int g, bool all_slots) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    __shared__ int s_m;
+    for (int cs = 0; cs < kGroup; ++cs) {
+        const int c = chunk_of(a, g, cs);
+        if (c >= a.nchunks) break;
+        const int j = g * kGroup + cs;
+        const int nf = sm.fl_wc[cs * 4] + sm.fl_wc[cs * 4 + 1] + sm.fl_wc[cs * 4 + 2] + sm.fl_wc[cs * 4 + 3];
+        if (nf == 0 && !all_slots) continue;   // the same for the whole block
+        // the columns that touch the chunk: staged segments first, then the unstaged ones
+        const int nS = sm.coff[j + 1] - sm.coff[j];
+        for (int n = tid; n < nS; n += kMasterThreads) sm.hm[n] = sm.cseg[sm.coff[j] + n];
+        if (a.ul_cap > 0) {
+            const int nU = sm.uoff[j + 1] - sm.uoff[j];
+            for (int n = tid; n < nU; n += kMasterThreads) sm.hm[nS + n] = 0xffff | ((int)sm.ul[sm.uoff[j] + n] << 16);
+            if (tid == 0) s_m = nS + nU;
+        } else if (warp == 0) {
+            int run = nS;
+            for (int u0 = 0; u0 < Ku; u0 += 32) {
+                const int u = u0 + lane, i = u < Ku ? sm.unc[u] : 0;
+                const bool f = u < Ku && touches(sm, a.N, i, j);
+                const unsigned mk = __ballot_sync(kFull, f);
+                if (f) sm.hm[run + __popc(mk & ((1u << lane) - 1u))] = 0xffff | (i << 16);
+                run += __popc(mk);
+            }
+            if (lane == 0) s_m = run;
+        }
+        __syncthreads();
+        const int m = s_m;
+        const float *om = sm.ombuf + cs * kSeg, *fd = sm.fl_dw + cs * kChunk;
+        const unsigned char *fs = sm.fl_slot + cs * kChunk;
+        const float *dch = a.Dd + (size_t)c * a.N * kChunk;   // the chunk's segments in global memory
+        // pairs (ia <= ib) of the m members, dealt to the threads row by row of the upper triangle
+        const int npair = m * (m + 1) / 2;
+        for (int pq = tid; pq < npair; pq += kMasterThreads) {
+            // row ia of the triangle starts at ia m - ia (ia - 1) / 2
+            int ia = (int)((2.0f * m + 1.0f - sqrtf((2.0f * m + 1.0f) * (2.0f * m + 1.0f) - 8.0f * (float)pq)) * 0.5f);
+            while (ia > 0 && ia * m - ia * (ia - 1) / 2 > pq) --ia;
+            while ((ia + 1) * m - (ia + 1) * ia / 2 <= pq) ++ia;
+            const int ib = ia + pq - (ia * m - ia * (ia - 1) / 2);
+            const int ea = sm.hm[ia], eb = sm.hm[ib], ca = ea >> 16, cb = eb >> 16;
+            const bool both = sm.hv[ca] && sm.hv[cb];
+            if (both ? nf == 0 : !all_slots) continue;
+            const float *pa = (ea & 0xffff) == 0xffff ? dch + (size_t)sm.sk[ca] * kChunk : sm.tile + (size_t)(ea & 0xffff) * kSeg;
+            const float *pb = (eb & 0xffff) == 0xffff ? dch + (size_t)sm.sk[cb] * kChunk : sm.tile + (size_t)(eb & 0xffff) * kSeg;
+            double acc = 0.0;
+            if (both) {
+                for (int f = 0; f < nf; ++f) {
+                    const int sl = fs[f];
+                    acc = fma((double)fd[f], (double)(pa[sl] * pb[sl]), acc);
+                }
+            } else {
+                for (int sl = 0; sl < kChunk; ++sl) {
+                    const float w = om[sl];
+                    if (w != 0.f) acc = fma((double)w, (double)(pa[sl] * pb[sl]), acc);
+                }
+            }
+            if (acc != 0.0) {
+                const int ka = sm.sk[ca], kb = sm.sk[cb];
+                atomicAdd(reinterpret_cast<unsigned long long *>(a.hess) + (size_t)min(ka, kb) * a.N + max(ka, kb),
+                          (unsigned long long)__double2ll_rn(acc * a.hscale));
+            }
+        }
+        __syncthreads();
+    }
+}
+
+// One pass of a working block: z = sum_k coef_k d_k for its slots -> zdst; w, F and omega there; its share of
+// grad = Dc w (record `rec`, fixed point); the flips of omega against a.omref and the update of H_F they call for.
+// fresh: compact index of the ONE occupied column that is not in H_F yet (the aperture the leaf search has just
+// committed), -1 if there is none, -2 if there are several (then they enter through hess_update, slot by slot).
+// The row of the one new column is a second gradient product, H_F[new][i] = d_i . (omega d_new).
+__device__ __forceinline__ void newton_pass(const MasterArgs &a, const Smem &sm, int K, int Ku, int ngroups, float *zdst,
+                                            float *wdst, long long *rec, double scF, double scG, double *red, int fresh) {
+    const bool res = a.rslots > 0;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const bool one = fresh >= 0;
+    for (int i = tid; i < 2 * a.N; i += kMasterThreads) {
+        sm.gacc[i] = 0.0;
+        if (one) sm.gaccu[i] = 0.0;
+    }
+    if (a.ul_cap > 0)
+        for (int i = tid; i < a.N; i += kMasterThreads) {
+            sm.gfx[i] = 0;
+            if (one) sm.gfxu[i] = 0;
+        }
+    double F = 0.0;
+    __syncthreads();
+    for (int g = 0; g < ngroups; ++g) {
+        float zv[kOutPerThread], dw[kOutPerThread];
+        unsigned bal[kOutPerThread];
+        combine_group(a, sm, Ku, g, zv);
+#pragma unroll
+        for (int r = 0; r < kOutPerThread; ++r) {
+            const int o = tid + r * kMasterThreads, c = chunk_of(a, g, o >> 7);
+            float wv = 0.f, omn = 0.f;
+            dw[r] = 0.f;
+            if (c < a.nchunks) {
+                const size_t s = (size_t)c * kChunk + (o & (kChunk - 1));
+                const int ls = g * (kGroup * kChunk) + o;
+                const float z = zv[r];
+                float Tv, al, be;
+                if (res) Tv = sm.rT[ls], al = sm.ral[ls], be = sm.rbe[ls];
+                else Tv = a.T[s], al = a.alpha[s], be = a.beta[s];
+                double f;
+                penalty(z, Tv, al, be, wv, f);
+                F += f;
+                omn = z < Tv ? al : (z > Tv ? be : 0.f);
+                const float omo = res ? sm.rom[ls] : a.omref[s];   // every slot belongs to one thread of one block
+                dw[r] = omn - omo;
+                if (dw[r] != 0.f) {
+                    a.omref[s] = omn;
+                    if (res) sm.rom[ls] = omn;
+                }
+                zdst[s] = z;
+                wdst[s] = wv;
+            }
+            sm.wbuf[(o >> 7) * kSeg + (o & (kChunk - 1))] = wv;
+            if (one) {   // omega d_new: the new column's own value at this slot, if it touches the chunk at all
+                const int j = g * kGroup + (o >> 7);
+                float dn = 0.f;
+                if (c < a.nchunks && touches(sm, a.N, fresh, j)) {
+                    const int bs = sm.base[fresh];
+                    dn = bs == kNoCache ? __ldg(a.Dd + ((size_t)c * a.N + sm.sk[fresh]) * kChunk + (o & (kChunk - 1)))
+                                        : sm.tile[(size_t)(bs + seg_rank(sm, a.N, fresh, j)) * kSeg + (o & (kChunk - 1))];
+                }
+                sm.ubuf[(o >> 7) * kSeg + (o & (kChunk - 1))] = omn * dn;
+            } else if (fresh == -2) sm.ombuf[(o >> 7) * kSeg + (o & (kChunk - 1))] = omn;
+            bal[r] = __ballot_sync(kFull, dw[r] != 0.f);
+            if (lane == 0) sm.fl_wc[(o >> 7) * 4 + ((o & (kChunk - 1)) >> 5)] = __popc(bal[r]);
+        }
+        __syncthreads();
+        // the flipped slots of every chunk, in slot order (a fixed order: the sums over them are reproducible)
+        int any = 0;
+#pragma unroll
+        for (int r = 0; r < kOutPerThread; ++r) {
+            if (dw[r] != 0.f) {
+                const int o = tid + r * kMasterThreads, cs = o >> 7, q = (o & (kChunk - 1)) >> 5;
+                int pos = __popc(bal[r] & ((1u << lane) - 1u));
+                for (int x = 0; x < q; ++x) pos += sm.fl_wc[cs * 4 + x];
+                sm.fl_slot[cs * kChunk + pos] = (unsigned char)(o & (kChunk - 1));
+                sm.fl_dw[cs * kChunk + pos] = dw[r];
+                any = 1;
+            }
+        }
+        grad_staged(sm, g, sm.wbuf, sm.gpart);
+        if (one) grad_staged(sm, g, sm.ubuf, sm.gpartu);
+        if (Ku > 0 && a.ul_cap > 0) {
+            grad_unstaged_listed(a, sm, g, sm.wbuf, sm.gfx, scG);
+            if (one) grad_unstaged_listed(a, sm, g, sm.ubuf, sm.gfxu, a.hscale);
+        } else if (Ku > 0) {
+            grad_unstaged_masked(a, sm, g, Ku, sm.wbuf, sm.gacc);
+            if (one) grad_unstaged_masked(a, sm, g, Ku, sm.ubuf, sm.gaccu);
+        }
+        // the barrier that ends the group's products also tells whether any of its slots flipped
+        if (__syncthreads_or(any) || fresh == -2) hess_update(a, sm, Ku, g, fresh == -2);
+    }
+    F = block_sum(F, red);
+    if (tid == 0) fx_add(rec, F, scF);
+    for (int i = tid; i < K; i += kMasterThreads) {
+        const bool fx = a.ul_cap > 0 && sm.base[i] == kNoCache;   // already in fixed point
+        if (fx) atomicAdd(reinterpret_cast<unsigned long long *>(rec + 2 + i), (unsigned long long)sm.gfx[i]);
+        else fx_add(rec + 2 + i, grad_total(sm, sm.gpart, sm.gacc, i, a.N), scG);
+        if (one) {   // row of the new column
+            const int ka = sm.sk[i], kb = sm.sk[fresh];
+            unsigned long long *dst = reinterpret_cast<unsigned long long *>(a.hess) + (size_t)min(ka, kb) * a.N + max(ka, kb);
+            if (fx) {
+                if (sm.gfxu[i]) atomicAdd(dst, (unsigned long long)sm.gfxu[i]);
+            } else {
+                const double v = grad_total(sm, sm.gpartu, sm.gaccu, i, a.N);
+                if (v != 0.0) atomicAdd(dst, (unsigned long long)__double2ll_rn(v * a.hscale));
+            }
+        }
+    }
+}
+
+// ---- the solving block ---------------------------------------------------------------------------------
+constexpr int kSolveRed = 8;   // values per warp row of the solver's reduction scratch
+
+// sums s[0..MS) and one maximum over the block, every thread receives them; fixed order
+template <int MS>
+__device__ __forceinline__ void solver_reduce(double (&s)[MS], double &mx, double *buf, int &tog) {
+    static_assert(MS < kSolveRed, "scratch row too short");
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int o = 16; o; o >>= 1) {
+#pragma unroll
+        for (int m = 0; m < MS; ++m) s[m] += __shfl_xor_sync(kFull, s[m], o);
+        mx = fmax(mx, __shfl_xor_sync(kFull, mx, o));
+    }
+    double *b = buf + tog * (kMasterWarps * kSolveRed);
+    tog ^= 1;
+    if (lane == 0) {
+#pragma unroll
+        for (int m = 0; m < MS; ++m) b[warp * kSolveRed + m] = s[m];
+        b[warp * kSolveRed + kSolveRed - 1] = mx;
+    }
+    __syncthreads();
+    // every warp adds the kMasterWarps rows by a butterfly over 16 lanes (both half-warps hold the same values)
+    const int row = lane & (kMasterWarps - 1);
+#pragma unroll
+    for (int m = 0; m < MS; ++m) {
+        double v = b[row * kSolveRed + m];
+#pragma unroll
+        for (int o = kMasterWarps / 2; o; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
+        s[m] = v;
+    }
+    double v = b[row * kSolveRed + kSolveRed - 1];
+#pragma unroll
+    for (int o = kMasterWarps / 2; o; o >>= 1) v = fmax(v, __shfl_xor_sync(kFull, v, o));
+    mx = v;
+}
+
+// Sums of the conjugate-gradient step over the block, in fp32 (the iteration corrects itself: the residual is updated
+// with the step actually taken): s[0..MS) are added, mx is maximised, the three low bits of flags are OR-ed.  Only the
+// first nv <= 8 warps hold data; they receive everything, the other warps the flags only (loop control).  One
+// barrier; both levels are warp shuffles in a fixed order; the scratch alternates between calls.
+constexpr int kCgRow = 8;   // floats per warp row of the scratch
+template <int MS>
+__device__ __forceinline__ void cg_reduce(float (&s)[MS], float &mx, int &flags, float *buf, int &tog, int nv) {
+    static_assert(MS + 2 <= kCgRow, "scratch row too short");
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    float *b = buf + tog * (8 * kCgRow);
+    tog ^= 1;
+    if (warp < nv) {
+#pragma unroll
+        for (int o = 16; o; o >>= 1) {
+#pragma unroll
+            for (int m = 0; m < MS; ++m) s[m] += __shfl_xor_sync(kFull, s[m], o);
+            mx = fmaxf(mx, __shfl_xor_sync(kFull, mx, o));
+        }
+        const int f = __reduce_or_sync(kFull, flags & 7);
+        if (lane == 0) {
+#pragma unroll
+            for (int m = 0; m < MS; ++m) b[warp * kCgRow + m] = s[m];
+            b[warp * kCgRow + MS] = mx;
+            b[warp * kCgRow + MS + 1] = __int_as_float(f);
+        }
+    }
+    __syncthreads();
+    const int row = lane & 7;   // every group of eight lanes reads the (at most) eight rows
+    const bool in = row < nv;
+    flags = __reduce_or_sync(kFull, in ? __float_as_int(b[row * kCgRow + MS + 1]) : 0);
+    if (warp < nv) {
+        float v[MS], m2 = in ? b[row * kCgRow + MS] : -CUDART_INF_F;
+#pragma unroll
+        for (int m = 0; m < MS; ++m) v[m] = in ? b[row * kCgRow + m] : 0.f;
+#pragma unroll
+        for (int o = 4; o; o >>= 1) {
+#pragma unroll
+            for (int m = 0; m < MS; ++m) v[m] += __shfl_xor_sync(kFull, v[m], o);
+            m2 = fmaxf(m2, __shfl_xor_sync(kFull, m2, o));
+        }
+#pragma unroll
+        for (int m = 0; m < MS; ++m) s[m] = v[m];
+        mx = m2;
+    }
+}
+
+__device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned long long ebase, unsigned long long abase) {
+    const int N = a.N, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    __shared__ int sK, s_timeout;
+    int *timed_out = &s_timeout;
+    if (tid == 0) s_timeout = 0;
+    // vectors over the beams (fp64), then the matrix (fp32, K x Kp, Kp / 4 odd: rows 16-byte aligned and conflict free
+    // for one thread per row), then the maps
+    double *vy = reinterpret_cast<double *>(smem_raw);
+    double *vg = vy + N, *yc = vg + N, *vr = yc + N, *vd = vr + N, *vHd = vd + N, *vpo = vHd + N, *vyn = vpo + N;
+    double *vgn = vyn + N, *vp = vgn + N, *linf = vp + N, *rdt = linf + N, *Minv = rdt + N, *dGb = Minv + N;
+    double *redb = dGb + N;                                  // 2 x kMasterWarps x kSolveRed
+    int *sk = reinterpret_cast<int *>(redb + 2 * kMasterWarps * kSolveRed), *ik = sk + N, *freeo = ik + N, *freen = freeo + N;
+    float *dc = reinterpret_cast<float *>((reinterpret_cast<uintptr_t>(freen + N) + 15) & ~(uintptr_t)15);   // compact direction
+    const int Np = ((N + 3) / 4) | 1;                        // float4s per row at K = N
+    float *cgb = dc + 4 * Np;                                // 2 x 8 x kCgRow floats: scratch of cg_reduce
+    float *hpart = cgb + 2 * 8 * kCgRow;                     // the product with the matrix, and the part of its second half
+    float *hpart2 = hpart + kMasterThreads / 2;
+    float *H32 = hpart2 + kMasterThreads / 2;                // Kp x Kp floats, Kp = 4 Kp4 >= K
+    // occupied beams, ascending
+    if (tid < 32) {
+        int base = 0;
+        for (int k0 = 0; k0 < N; k0 += 32) {
+            const int k = k0 + tid;
+            const bool f = k < N && a.occ[k];
+            const unsigned m = __ballot_sync(kFull, f);
+            if (f) sk[base + __popc(m & ((1u << tid) - 1u))] = k;
+            if (k < N) ik[k] = f ? base + __popc(m & ((1u << tid) - 1u)) : -1;
+            base += __popc(m);
+        }
+        if (tid == 0) sK = base;
+    }
+    const double lb = a.lb, ub = a.ub;
+    const bool has_ub = ub < CUDART_INF;
+    auto at_bound = [lb, ub](double yk, double g) { return (yk <= lb && g >= 0.0) || (yk >= ub && g <= 0.0); };
+    double l1l = 0.0;
+    for (int k = tid; k < N; k += kMasterThreads) {
+        double yk = a.y[k];
+        const bool on = a.occ[k] != 0;
+        if (!on) yk = 0.0;
+        else if (!(yk > lb)) yk = lb;
+        else if (yk > ub) yk = ub;
+        vy[k] = yk;
+        vd[k] = 0.0;
+        rdt[k] = k + 1 < N ? 1.0 / (a.theta[k + 1] - a.theta[k]) : 0.0;
+        double lf = 0.0;
+        if (on) {
+            const ColStat cs = a.colstat[k];
+            lf = (double)cs.linf * a.fx_inv * 1.000001;
+            l1l = fmax(l1l, (double)cs.l1 * a.fx_inv * 1.000001);
+        }
+        linf[k] = lf;
+    }
+    int tog = 0;
+    double none[1] = {0.0};
+    solver_reduce<1>(none, l1l, redb, tog);   // its barrier also publishes sk, ik, vy, rdt, linf
+    const double l1max = l1l;
+    const int K = sK;
+    const int Kp4 = ((K + 3) / 4) | 1, Kp = 4 * Kp4;
+    const double Tm = (double)a.Tmax, ab = (double)a.abmax, Spd = (double)a.Sp;
+    const double c1a = 1e-4, noise = 2e-7;
+    int bad = 0, inner = 0, backtracks = 0, stop = 0, stall = 0, cur = 0;
+    unsigned ph = a.phase[0];
+    const unsigned ph_entry = ph;
+    const int recn = 2 * N + 2;
+    unsigned long long epub = ebase, npass = 0;
+    Mail *mail = a.mail;
+    float *mcoef = reinterpret_cast<float *>(mail + 1);
+    double scF = 1.0, iF = 1.0, scG = 1.0, iG = 1.0;
+    long long clk_wait = 0, clk_load = 0, clk_cg = 0, cg_steps = 0;   // bookkeeping (thread 0): where the solver's time goes
+
+    // G(v) and dG/dv (Eq. 2; S2, S3), and the dose bound sum_k |v_k| max|d_k|
+    auto smooth_of = [&](const double *v, double &G, double &zb) {
+        double s[2] = {0.0, 0.0}, mx = 0.0;
+        for (int k = tid; k < N; k += kMasterThreads) {
+            const double e1 = k + 1 < N ? (v[k + 1] - v[k]) * rdt[k] : 0.0;
+            const double e0 = k > 0 ? (v[k] - v[k - 1]) * rdt[k - 1] : 0.0;
+            if (k + 1 < N) s[0] += (v[k + 1] - v[k]) * e1;
+            dGb[k] = 2.0 * (e0 - e1);
+            s[1] += fabs(v[k]) * linf[k];
+        }
+        solver_reduce<2>(s, mx, redb, tog);
+        G = s[0];
+        zb = s[1];
+    };
+    // tell the workers what to do next: evaluate at v (into buffer pair dst), or finish
+    auto send = [&](int state, int dst, const double *v, double zb) {
+        const double dev = Tm + zb;
+        const FxScale sF = fx_scale_for(1.01 * Spd * ab * dev * dev, bad);
+        const FxScale sG = fx_scale_for(2.02 * ab * dev * l1max, bad);
+        scF = sF.scale, iF = sF.inv, scG = sG.scale, iG = sG.inv;
+        if (bad) state = kFinish;
+        if (v)
+            for (int k = tid; k < N; k += kMasterThreads) mcoef[k] = (float)v[k];
+        if (tid == 0) {
+            mail->scF = scF;
+            mail->scG = scG;
+            mail->state = state;
+            mail->dst = dst;
+            mail->cur = cur;
+        }
+        __syncthreads();
+        ++epub;
+        if (tid == 0) {
+            __threadfence();
+            TR(if (state != kFinish) g_tr[0][(g_trn + npass) & 4095] = gtime();)
+            st_release_u64(a.sync + 1, epub);
+        }
+        return state;
+    };
+    // wait for the pass the last message asked for; F and the F-part of the gradient at its point -> Fv, gout
+    auto receive = [&](double &Fv, double *gout) {
+        ++npass;
+        const long long c0 = clock64();
+        if (tid == 0 && !spin_until(a.sync, abase + (unsigned long long)a.nblk * npass)) *timed_out = 1;
+        TR(if (tid == 0) g_tr[3][(g_trn + npass - 1) & 4095] = gtime();)
+        __syncthreads();
+        clk_wait += clock64() - c0;
+        const long long *rec = a.accbuf + (size_t)(ph % 3) * kSumGroups * recn;
+        ++ph;
+        if (s_timeout) bad = 1;
+        Fv = (double)__ldcg(rec) * iF + a.F_out;
+        for (int k = tid; k < N; k += kMasterThreads) {
+            const int i = ik[k];
+            gout[k] = i >= 0 ? (double)__ldcg(rec + 2 + i) * iG + a.gamma * dGb[k] : 0.0;
+        }
+        __syncthreads();
+    };
+
+    // ---- the incoming point -----------------------------------------------------------------------------
+    double F = 0.0, Gs = 0.0, Phi = 0.0, zb = 0.0, pgmax = 0.0, pg_entry = 0.0, tol = 0.0, Phi0 = 0.0;
+    smooth_of(vy, Gs, zb);
+    int state = send(kRunTrial, 0, vy, zb);
+    if (state != kFinish) {
+        receive(F, vg);
+        Phi = F + a.gamma * Gs;
+        Phi0 = Phi;
+        double pgl = 0.0;
+        for (int k = tid; k < N; k += kMasterThreads)
+            if (ik[k] >= 0 && !at_bound(vy[k], vg[k])) pgl = fmax(pgl, fabs(vg[k]));
+        solver_reduce<1>(none, pgl, redb, tog);
+        pgmax = pg_entry = pgl;
+        tol = a.eps * fmax(1.0, pgmax);
+        if (a.max_inner <= 0 && pgmax > tol) stop = 1;
+    }
+    auto stall_threshold = [&](double Phin) {
+        return (Phi0 - Phin <= 1e-2 * fabs(Phin)) ? a.stall_rel : 1e-2 * a.stall_rel;
+    };
+
+    // ---- Newton iterations ------------------------------------------------------------------------------
+    while (state != kFinish && !stop && pgmax > tol) {
+        // the matrix of the current piece: H32 = H_F over the occupied beams
+        const long long c0 = clock64();
+        {
+            const int npair = K * (K + 1) / 2;
+            for (int e0 = 0; e0 < npair; e0 += 8 * kMasterThreads) {
+                long long v[8];
+                int ri[8], ci[8];
+#pragma unroll
+                for (int u = 0; u < 8; ++u) {
+                    const int e = e0 + u * kMasterThreads + tid;
+                    ri[u] = -1;
+                    v[u] = 0;
+                    if (e < npair) {   // row i of the upper triangle starts at i K - i (i - 1) / 2
+                        int i = (int)((2.0f * K + 1.0f - sqrtf((2.0f * K + 1.0f) * (2.0f * K + 1.0f) - 8.0f * (float)e)) * 0.5f);
+                        while (i > 0 && i * K - i * (i - 1) / 2 > e) --i;
+                        while ((i + 1) * K - (i + 1) * i / 2 <= e) ++i;
+                        ri[u] = i;
+                        ci[u] = i + e - (i * K - i * (i - 1) / 2);
+                        v[u] = __ldcg(a.hess + (size_t)sk[i] * N + sk[ci[u]]);
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < 8; ++u)
+                    if (ri[u] >= 0) {
+                        const float f = (float)((double)v[u] * a.hinv);
+                        H32[ri[u] * Kp + ci[u]] = f;
+                        H32[ci[u] * Kp + ri[u]] = f;
+                    }
+            }
+        }
+        for (int e = tid; e < (Kp - K) * Kp; e += kMasterThreads) H32[(size_t)K * Kp + e] = 0.f;   // rows K..Kp-1 (read with d = 0)
+        for (int k = tid; k < N; k += kMasterThreads) {
+            yc[k] = vy[k];
+            vr[k] = vg[k];
+            vd[k] = 0.0;
+            vpo[k] = 0.0;
+            freeo[k] = 0;
+        }
+        for (int i = tid; i < Kp; i += kMasterThreads) dc[i] = 0.f;
+        __syncthreads();
+        for (int k = tid; k < N; k += kMasterThreads) {
+            const int i = ik[k];
+            double m = 0.0;
+            if (i >= 0) m = 2.0 * (double)H32[i * Kp + i] + 2.0 * a.gamma * ((k > 0 ? rdt[k - 1] : 0.0) + rdt[k]);
+            Minv[k] = m > 0.0 ? 1.0 / m : 1.0;
+        }
+        const long long c1 = clock64();
+        clk_load += c1 - c0;
+        // Conjugate gradients on the faces of the box for the quadratic model at (vy, vg): one beam per thread (the
+        // first nv warps), two threads per row of the matrix (all warps); two sums over the beams and two block barriers
+        // per step.  Step lengths and the ratios to the bounds are formed in fp32: the iteration corrects itself (the
+        // residual is updated with the step actually taken) and a beam that reaches its bound is set on it explicitly.
+        const double qtol = fmax(0.5 * tol, 0.05 * pgmax);
+        const int k = tid;                                   // this thread's beam (k < N: checked on the host)
+        const bool mine = k < N && ik[k] >= 0;
+        const int nv = (N + 31) / 32;                        // warps that hold beams
+        auto ratio = [](double num, double den) { return (double)__fdividef((float)num, (float)den); };
+        // state of this thread's beam
+        double yk = mine ? vy[k] : 0.0, rk = mine ? vg[k] : 0.0, dk = 0.0, pok = 0.0;
+        const double mk = mine ? Minv[k] : 1.0;
+        int fo = 0;
+        float rzold = 0.f;
+        double beta = 0.0;
+        bool restart = true, halt = false;
+        const int maxcg = 4 * K + 20;
+        int it = 0, togc = 0;
+        // first half of a step: projected residual, its sums
+        int fr = mine && !at_bound(yk, rk);
+        double prk = fr ? rk : 0.0, zrk = mk * prk;
+        for (;;) {
+            TR(long long q0 = clock64();)
+            float s[2] = {(float)(zrk * prk), (float)(zrk * pok)};
+            float none_f = 0.f;
+            int fl = (fr != fo ? 1 : 0) | (fabs(prk) > qtol ? 2 : 0) | (halt ? 4 : 0);
+            cg_reduce<2>(s, none_f, fl, cgb, togc, nv);
+            TR(if (tid == 0) g_seg[0] += clock64() - q0; q0 = clock64();)
+            const int chg = fl & 1, big = fl & 2;
+            if (!big || (fl & 4) || it >= maxcg) break;   // (only the warps that hold beams know `halt`: it travels as a flag)
+            beta = (restart || chg || !(rzold > 0.f)) ? 0.0 : (double)fmaxf(0.f, __fdividef(s[0] - s[1], rzold));
+            restart = false;
+            rzold = s[0];
+            dk = fr ? -zrk + beta * dk : 0.0;
+            pok = prk;
+            fo = fr;
+            if (k < N) vd[k] = dk;
+            if (mine) dc[ik[k]] = (float)dk;
+            __syncthreads();
+            ++cg_steps;
+            ++it;
+            TR(if (tid == 0) g_seg[1] += clock64() - q0; q0 = clock64();)
+            // H32 d, fp32.  The matrix is symmetric: thread (r, h) sums H[c][r] d_c over the columns c of its half h, so
+            // that the lanes of a warp read consecutive words of row c (no bank conflict, 128 bytes per request) and
+            // d_c is the same word for the whole warp.  Two halves: threads 0..255 and 256..511.
+            {
+                const int r = tid & (kMasterThreads / 2 - 1), h = tid / (kMasterThreads / 2);
+                const int q0 = h * ((Kp4 + 1) / 2), q1 = min(Kp4, q0 + (Kp4 + 1) / 2);   // float4s of d of this half
+                float acc0 = 0.f, acc1 = 0.f;
+                if (r < K) {
+                    const float4 *d4 = reinterpret_cast<const float4 *>(dc);
+                    const float *hc = H32 + r;
+                    for (int q = q0; q < q1; ++q) {
+                        const float4 dv = d4[q];
+                        const float *h4 = hc + (size_t)(4 * q) * Kp;
+                        acc0 = fmaf(h4[0], dv.x, acc0);
+                        acc1 = fmaf(h4[Kp], dv.y, acc1);
+                        acc0 = fmaf(h4[2 * Kp], dv.z, acc0);
+                        acc1 = fmaf(h4[3 * Kp], dv.w, acc1);
+                    }
+                }
+                if (h == 1 && r < K) hpart2[r] = acc0 + acc1;
+                __syncthreads();
+                if (h == 0 && r < K) hpart[r] = (acc0 + acc1) + hpart2[r];
+            }
+            __syncthreads();
+            TR(if (tid == 0) g_seg[2] += clock64() - q0; q0 = clock64();)
+            double hdk = 0.0;
+            float s2[2] = {0.f, 0.f}, ntl = -CUDART_INF_F;
+            if (mine) {
+                const double e1 = k + 1 < N ? (vd[k + 1] - dk) * rdt[k] : 0.0;
+                const double e0 = k > 0 ? (dk - vd[k - 1]) * rdt[k - 1] : 0.0;
+                hdk = 2.0 * (double)hpart[ik[k]] + 2.0 * a.gamma * (e0 - e1);
+                s2[0] = (float)(dk * hdk);
+                s2[1] = (float)(rk * dk);
+                if (dk < 0.0) ntl = -(float)ratio(yk - lb, -dk);
+                if (has_ub && dk > 0.0) ntl = -(float)ratio(ub - yk, dk);
+            }
+            int nofl = 0;
+            cg_reduce<2>(s2, ntl, nofl, cgb, togc, nv);
+            TR(if (tid == 0) g_seg[3] += clock64() - q0; q0 = clock64();)
+            const float tmaxf = -ntl;                            // fp32: the same bits wherever the ratio is formed
+            const double tmax = (double)tmaxf;
+            if (!(s2[1] < 0.f)) {        // not a descent direction of the model: open steepest descent again, or give up
+                if (beta == 0.0) halt = true;
+                restart = true;
+            } else {
+                double t = s2[0] > 0.f ? (double)__fdividef(-s2[1], s2[0]) : tmax;
+                if (!(t < CUDART_INF)) halt = true;
+                else {
+                    const bool hit = t >= tmax;
+                    if (hit) t = tmax;
+                    if (mine) {
+                        double v = yk + t * dk;
+                        if (v < lb || (hit && dk < 0.0 && (float)ratio(yk - lb, -dk) <= tmaxf)) v = lb;
+                        else if (has_ub && (v > ub || (hit && dk > 0.0 && (float)ratio(ub - yk, dk) <= tmaxf))) v = ub;
+                        yk = v;
+                        rk += t * hdk;
+                    }
+                }
+            }
+            fr = mine && !at_bound(yk, rk);
+            prk = fr ? rk : 0.0;
+            zrk = mk * prk;
+            TR(if (tid == 0) g_seg[4] += clock64() - q0;)
+        }
+        if (k < N) yc[k] = yk;
+        __syncthreads();
+        clk_cg += clock64() - c1;
+        // the step and its slope on the true gradient
+        double sl[1] = {0.0}, mxp = 0.0;
+        if (tid < N) {
+            const double pk = yc[tid] - vy[tid];
+            vp[tid] = pk;
+            sl[0] = vg[tid] * pk;
+            mxp = fabs(pk);
+        }
+        solver_reduce<1>(sl, mxp, redb, tog);
+        const double slope = sl[0];
+        if (!(slope < 0.0) || !(mxp > 0.0)) {
+            stop = 2;
+            break;
+        }
+        // back-tracking on the true cost, from the full step
+        double t = 1.0;
+        int half = 0;
+        for (;;) {
+            if (tid < N) vyn[tid] = half == 0 ? yc[tid] : fmin(fmax(vy[tid] + t * vp[tid], ik[tid] >= 0 ? lb : 0.0), ik[tid] >= 0 ? ub : 0.0);
+            __syncthreads();
+            double Gn, zbn, Fn;
+            smooth_of(vyn, Gn, zbn);
+            state = send(kRunTrial, cur ^ 1, vyn, zbn);
+            if (state == kFinish) break;
+            receive(Fn, vgn);
+            const double Phin = Fn + a.gamma * Gn;
+            double sn[1] = {0.0}, pgm = 0.0;
+            if (tid < N) {
+                sn[0] = vgn[tid] * vp[tid];
+                if (ik[tid] >= 0 && !at_bound(vyn[tid], vgn[tid])) pgm = fabs(vgn[tid]);
+            }
+            solver_reduce<1>(sn, pgm, redb, tog);
+            const bool accepted = Phin <= Phi + c1a * t * slope ||
+                                  (Phin <= Phi + noise * fabs(Phi) && fabs(sn[0]) <= 0.9 * fabs(slope));
+            if (accepted) {
+                stall = (Phi - Phin <= stall_threshold(Phin) * fabs(Phi)) ? stall + 1 : 0;
+                cur ^= 1;
+                if (tid < N) {
+                    vy[tid] = vyn[tid];
+                    vg[tid] = vgn[tid];
+                }
+                F = Fn;
+                Gs = Gn;
+                Phi = Phin;
+                pgmax = pgm;
+                ++inner;
+                __syncthreads();
+                break;
+            }
+            t *= 0.5;
+            ++backtracks;
+            if (++half >= 40) {
+                stop = 3;
+                break;
+            }
+        }
+        if (stop || state == kFinish) break;
+        if (stall >= a.stall_count) stop = 4;
+        else if (inner >= a.max_inner) stop = 1;
+    }
+    if (bad) stop = 5;
+    if (s_timeout) stop = 6;
+    if (state != kFinish) send(kFinish, 0, nullptr, 0.0);
+    // results
+    for (int k = tid; k < N; k += kMasterThreads) {
+        a.y[k] = vy[k];
+        if (a.occ[k]) a.hvalid[k] = 1;   // every occupied beam is in the matrix now (the first pass saw to it)
+    }
+    if (tid == 0) {
+        a.phase[0] = ph % 3;
+        a.sync[2] = epub;
+        a.sync[3] = abase + (unsigned long long)a.nblk * npass;
+        a.gflag[0] = 0;
+        atomicAdd(a.mcount + 1, (unsigned long long)(ph - ph_entry));
+        a.mcount[2] += (unsigned long long)cg_steps;
+        a.mcount[3] += (unsigned long long)clk_cg;
+        a.mcount[4] += (unsigned long long)clk_wait;
+        a.mcount[5] += (unsigned long long)clk_load;
+        TR(g_trn += (unsigned)npass;)
+        MasterOut o;
+        o.inner = inner;
+        o.backtracks = backtracks;
+        o.stop_reason = stop;
+        o.pad = (int)(ph - ph_entry);
+        o.pg_entry = pg_entry;
+        o.pg_exit = pgmax;
+        o.F = F;
+        o.G = Gs;
+        o.cost = Phi;
+        *a.out = o;
+        a.cost3[0] = F;
+        a.cost3[1] = Gs;
+        a.cost3[2] = Phi;
+        if (a.trace_it >= 0) {
+            a.trF[a.trace_it] = F;
+            a.trG[a.trace_it] = Gs;
+            a.trC[a.trace_it] = Phi;
+            a.trInner[a.trace_it] = inner;
+        }
+    }
+}
+
+__global__ void __launch_bounds__(kMasterThreads, 1) k_newton(const MasterArgs a) {
+    extern __shared__ float4 smem_raw[];
+    const int tid = threadIdx.x;
+    const unsigned long long ebase = a.sync[2];   // written by the launch before this one: stream ordered
+    const unsigned long long abase = a.sync[3];
+    if ((int)blockIdx.x == a.nblk) {
+        newton_solver(a, smem_raw, ebase, abase);
+        return;
+    }
+    Smem sm;
+    const Setup su = master_setup<true>(a, sm, smem_raw);
+    const int K = su.K, Ku = su.Ku, ngroups = su.ngroups;
+    // T, alpha, beta of the block's own slots are read once
+    if (a.rslots > 0) {
+        for (int ls = tid; ls < a.rslots; ls += kMasterThreads) {
+            const int c = (int)blockIdx.x + (ls >> 7) * a.nblk;
+            const bool in = c < a.nchunks;
+            const size_t s = (size_t)c * kChunk + (ls & (kChunk - 1));
+            sm.rT[ls] = in ? a.T[s] : 0.f;
+            sm.ral[ls] = in ? a.alpha[s] : 0.f;
+            sm.rbe[ls] = in ? a.beta[s] : 0.f;
+            sm.rom[ls] = in ? a.omref[s] : 0.f;
+        }
+    }
+    // which occupied columns are in H_F already: fresh = the one that is not (-1: none, -2: several)
+    __shared__ int s_fresh;
+    if (tid == 0) s_fresh = INT_MAX;
+    __syncthreads();
+    int missing = 0;
+    for (int i = tid; i < K; i += kMasterThreads) {
+        const int v = a.hvalid[sm.sk[i]] != 0;
+        sm.hv[i] = v;
+        if (!v) {
+            ++missing;
+            atomicMin(&s_fresh, i);
+        }
+    }
+    missing = __syncthreads_count(missing);   // (K <= kMasterThreads: at most one column per thread)
+    int fresh = missing == 0 ? -1 : (missing == 1 ? s_fresh : -2);
+    const int recn = 2 * a.N + 2;
+    unsigned ph = a.phase[0];
+    const unsigned ph_entry = ph;
+    const Mail *mail = a.mail;
+    const float *mcoef = reinterpret_cast<const float *>(mail + 1);
+    unsigned long long e = ebase;
+    int cur = 0;
+    long long wclk = 0;
+    for (;;) {
+        ++e;
+        __shared__ int s_gone;
+        if (tid == 0) s_gone = !spin_until(a.sync + 1, e);
+        TR(const unsigned trp = (g_trn + (unsigned)(e - ebase - 1)) & 4095;)
+        TR(if (tid == 0) atomicMax(&g_tr[1][trp], gtime());)
+        __syncthreads();
+        // the whole message in one round trip to L2: header and this thread's coefficient are loaded before any is used
+        const int mstate = __ldcg(&mail->state), dst = __ldcg(&mail->dst), mcur = __ldcg(&mail->cur);
+        const double scF = __ldcg(&mail->scF), scG = __ldcg(&mail->scG);
+        float cf = 0.f;
+        if (tid < K) cf = __ldcg(mcoef + sm.sk[tid]);   // K <= kMasterThreads / 2
+        const int state = s_gone ? kFinish : mstate;
+        if (state == kFinish) {
+            cur = s_gone ? 0 : mcur;
+            break;
+        }
+        if (tid < K) sm.coef[tid] = cf;
+        if (blockIdx.x == 0) {   // block 0 clears the record of the pass after this one
+            long long *nx = a.accbuf + (size_t)((ph + 1) % 3) * kSumGroups * recn;
+            for (int i = tid; i < kSumGroups * recn; i += kMasterThreads) nx[i] = 0;
+        }
+        long long *rec = a.accbuf + (size_t)(ph % 3) * kSumGroups * recn;
+        ++ph;
+        __syncthreads();
+        const long long w1 = clock64();
+        newton_pass(a, sm, K, Ku, ngroups, dst ? a.zn : a.z, dst ? a.wn : a.w, rec, scF, scG, su.red, fresh);
+        wclk += clock64() - w1;
+        if (fresh != -1) {
+            __syncthreads();
+            for (int i = tid; i < K; i += kMasterThreads) sm.hv[i] = 1;
+            fresh = -1;
+        }
+        __syncthreads();
+        if (tid == 0) {
+            __threadfence();
+            TR(atomicMax(&g_tr[2][trp], gtime());)
+            atomicAdd(a.sync, 1ull);
+        }
+    }
+    // the accepted point sits in the second buffer pair: bring the block's own slots home
+    if (cur) {
+        for (int g = 0; g < ngroups; ++g)
+            for (int o = tid; o < kGroup * kChunk; o += kMasterThreads) {
+                const int c = chunk_of(a, g, o >> 7);
+                if (c < a.nchunks) {
+                    const size_t s = (size_t)c * kChunk + (o & (kChunk - 1));
+                    a.z[s] = a.zn[s];
+                    a.w[s] = a.wn[s];
+                }
+            }
+    }
+    if (tid == 0) atomicAdd(a.mcount, (unsigned long long)su.segs * (unsigned long long)(ph - ph_entry));
+    if (tid == 0) {
+        atomicMax(a.mcount + 7, (unsigned long long)wclk);
+        if (blockIdx.x == 0) a.mcount[6] += (unsigned long long)wclk;
+        atomicAdd(a.mcount + 8, (unsigned long long)wclk);
+    }
+}
+
+// shared memory of one master block (master_setup's carve-up); k_newton's working blocks lay out a little more
+size_t seg_bytes(bool newton) { return kSeg * 4 + (newton ? 2 : 1) * 2 * 8 + 2 * 4; }   // tile, gpart (gpartu), cseg + gseg
+
+size_t master_smem_bytes(int64_t N, int64_t rslots, int64_t cache_segs, int64_t ngroups, bool newton, int64_t ul_cap) {
+    const int f1 = newton ? 1 : 0;
+    return (size_t)(2 * kGroup * kChunk + (1 + 2 * f1) * kGroup * kSeg + f1 * kGroup * kChunk + (6 + f1) * rslots) * 4   // part2, wbuf (ombuf, ubuf, fl_dw), resident slots
+           + (size_t)cache_segs * seg_bytes(newton)                                          // tile and the lists over it
+           + (size_t)((13 + 2 * f1) * N + 2 * N + 2 + kMasterWarps + 2 * kMasterWarps * kRedSlots) * 8 + sizeof(Ctl)   // K-vectors (gaccu), recv, red, cred, ctl
            + (size_t)N * 4 * 8 + (size_t)(ngroups * kGroup + 1) * 4           // coef, sk, lo, hi, ik, base, unc, nseg; coff
            + (size_t)ngroups * (kGroup + 1) * 4                               // wst
            + (size_t)((ngroups * kGroup + 63) / 64) * N * 8                   // lmask
-           + (ul_cap > 0 ? (size_t)ul_cap * 2 + 16 + (size_t)(ngroups * kGroup + 1) * 4 + (size_t)(1 + f1) * N * 8 : 0);   // ul, uoff, gfx
+           + (size_t)f1 * ((size_t)2 * N * 4 + (kGroup * 4 + 4) * 4 + kGroup * kChunk)   // hm, hv, fl_wc, fl_slot
+           + (ul_cap > 0 ? (size_t)ul_cap * 2 + 16 + (size_t)(ngroups * kGroup + 1) * 4 + (size_t)(1 + f1) * N * 8 : 0);   // ul, uoff, gfx (gfxu)
+}
+
+// shared memory of k_newton's solving block (newton_solver's carve-up)
+size_t solver_smem_bytes(int64_t N) {
+    const int64_t Np = ((N + 3) / 4) | 1;
+    return (size_t)(14 * N + 2 * kMasterWarps * kSolveRed) * 8 + (size_t)4 * N * 4 + 16 + (size_t)4 * Np * 4 +
+           (size_t)(kMasterThreads + 2 * 8 * 8) * 4 + (size_t)4 * Np * 4 * Np * 4;
 }
 
 }  // namespace
 
 int master_configure(vmat_plan *p) {
     const int64_t nchunks = p->Sp / kChunk;
-    int64_t grid = p->sm_count;                       // one block per SM, chunks dealt round-robin
+    int optin = 0;
+    VMAT_CUDA(p, cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, p->device));
+    const size_t budget = (size_t)optin > 8 * 1024 ? (size_t)optin - 8 * 1024 : 0;
+    // mode 1 (k_newton) gives one block of the grid to the reduced problems: its matrix must fit that block's shared
+    // memory and its vectors take one thread per beam; larger problems run mode 0
+    bool newton = p->opt.master_mode == 1 && p->sm_count >= 2 && p->N <= kMasterThreads / 2 && solver_smem_bytes(p->N) <= budget;
+    p->master_newton = newton;
+    int64_t grid = p->sm_count - (newton ? 1 : 0);    // one block per SM, chunks dealt round-robin
     if (grid > nchunks) grid = nchunks;
     if (grid < 1) grid = 1;
-    p->master_grid = (int)grid;
+    p->master_nblk = (int)grid;
+    p->master_grid = (int)grid + (newton ? 1 : 0);
     // resident slot data (z, z trial, q, T, alpha, beta of a block's own slots) if it fits in 128 KB: on a large
     // support the tile holds a few per cent of the columns whatever its size, while slot data read from L2 / HBM
     // costs every group of every pass a round trip
     const int64_t ngroups = (nchunks + grid * kGroup - 1) / (grid * kGroup);
     int64_t rslots = ngroups * kGroup * kChunk;
-    if (rslots * (p->opt.master_mode == 1 ? 7 : 6) * 4 > 128 * 1024) rslots = 0;
+    if (rslots * 7 * 4 > 128 * 1024) rslots = 0;
     p->master_rslots = (int)rslots;
     // what is left of the SM's opt-in shared memory (minus static use and room for L1) holds the tile of Dd
-    int optin = 0;
-    VMAT_CUDA(p, cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, p->device));
-    const size_t budget = (size_t)optin > 8 * 1024 ? (size_t)optin - 8 * 1024 : 0;
-    const int mode = p->opt.master_mode;
+    const bool mode = newton;
     // per-chunk lists of the unstaged beams (one entry per column and local chunk at most) if they fit in 64 KB
     int64_t ul_cap = p->N * ngroups * kGroup;
     if (ul_cap * 2 > 64 * 1024 || p->N > 65535) ul_cap = 0;
-    if (getenv("VMAT_MASTER_MASKED_LOOPS")) ul_cap = 0;   // debugging aid: force the fallback path (tests)
+    if (!p->opt.master_unstaged_lists) ul_cap = 0;         // option: force the fallback path (tests)
     size_t fixed = master_smem_bytes(p->N, rslots, 0, ngroups, mode, ul_cap);
     if (fixed > budget) {
         p->master_rslots = 0;
@@ -2009,31 +2514,45 @@ int master_configure(vmat_plan *p) {
     if (fixed > budget) return fail(p, VMAT_EINVAL, "n_beams too large for the master kernel's shared memory");
     p->master_cache_segs = (int)((budget - fixed) / seg_bytes(mode));
     if (p->master_cache_segs > 65535 || ngroups * kGroup > 32767) p->master_cache_segs = 0;   // 16-bit fields of the lists
-#ifdef VMAT_MASTER_PROFILE
-    if (getenv("VMAT_NO_TILE")) p->master_cache_segs = 0;
-    fprintf(stderr, "master: grid %d smem fixed %zu cache_segs %d rslots %d\n", p->master_grid, fixed, p->master_cache_segs, p->master_rslots);
-#endif
     p->master_smem = master_smem_bytes(p->N, p->master_rslots, p->master_cache_segs, ngroups, mode, ul_cap);
-    VMAT_CUDA(p, cudaFuncSetAttribute(k_master<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->master_smem));
-    VMAT_CUDA(p, cudaFuncSetAttribute(k_master<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->master_smem));
-    int per_sm = 0, per_sm1 = 0;
-    VMAT_CUDA(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_master<0>, kMasterThreads, p->master_smem));
-    VMAT_CUDA(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm1, k_master<1>, kMasterThreads, p->master_smem));
-    if (per_sm1 < per_sm) per_sm = per_sm1;
+    if (newton && solver_smem_bytes(p->N) > p->master_smem) p->master_smem = solver_smem_bytes(p->N);
+    // The attribute is a per-function, per-device setting shared by every plan of the process: it is set to the
+    // device's opt-in maximum (the same value from every vmat_create), never to this plan's own size, so that a plan
+    // created later cannot shrink it under a live one.  Each launch passes its own p->master_smem <= optin.
+    cudaFuncAttributes fa0, fa1;
+    VMAT_CUDA(p, cudaFuncGetAttributes(&fa0, k_master));
+    VMAT_CUDA(p, cudaFuncGetAttributes(&fa1, k_newton));
+    VMAT_CUDA(p, cudaFuncSetAttribute(k_master, cudaFuncAttributeMaxDynamicSharedMemorySize, optin - (int)fa0.sharedSizeBytes));
+    VMAT_CUDA(p, cudaFuncSetAttribute(k_newton, cudaFuncAttributeMaxDynamicSharedMemorySize, optin - (int)fa1.sharedSizeBytes));
+    int per_sm = 0;
+    if (newton) VMAT_CUDA(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_newton, kMasterThreads, p->master_smem));
+    else VMAT_CUDA(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_master, kMasterThreads, p->master_smem));
     if (per_sm < 1) return fail(p, VMAT_ECUDA, "master kernel does not fit on an SM");
     int rc;
     if ((rc = dev_alloc(p, &p->accbuf, 3 * kSumGroups * (2 * p->N + 2)))) return rc;
     if ((rc = dev_alloc(p, &p->phase, 2))) return rc;
-    if ((rc = dev_alloc(p, &p->mcount, 2))) return rc;
+    if ((rc = dev_alloc(p, &p->mcount, 16))) return rc;
     if ((rc = dev_alloc(p, &p->gsave, p->N))) return rc;
     if ((rc = dev_alloc(p, &p->gflag, 1))) return rc;
     VMAT_CUDA(p, cudaMemsetAsync(p->gflag, 0, 4, p->stream));
-    VMAT_CUDA(p, cudaMemsetAsync(p->mcount, 0, 16, p->stream));
+    VMAT_CUDA(p, cudaMemsetAsync(p->mcount, 0, 128, p->stream));
     if ((rc = dev_alloc(p, &p->colstat, p->N))) return rc;
     p->touch_words = (int)((nchunks + 31) / 32);
     if ((rc = dev_alloc(p, &p->col_touch, p->N * p->touch_words))) return rc;
     VMAT_CUDA(p, cudaMemsetAsync(p->col_touch, 0, (size_t)p->N * p->touch_words * 4, p->stream));
     if ((rc = dev_alloc(p, &p->vbounds, 2))) return rc;
+    if (newton) {
+        if ((rc = dev_alloc(p, &p->hess, p->N * p->N))) return rc;
+        if ((rc = dev_alloc(p, &p->omref, p->Sp))) return rc;
+        if ((rc = dev_alloc(p, &p->hvalid, p->N))) return rc;
+        if ((rc = dev_alloc(p, &p->wn_s, p->Sp))) return rc;
+        if ((rc = dev_alloc(p, (char **)&p->mail, (int64_t)sizeof(Mail) + 4 * p->N))) return rc;
+        if ((rc = dev_alloc(p, &p->nsync, 4))) return rc;
+        VMAT_CUDA(p, cudaMemsetAsync(p->wn_s, 0, (size_t)p->Sp * 4, p->stream));
+        VMAT_CUDA(p, cudaMemsetAsync(p->mail, 0, sizeof(Mail) + 4 * (size_t)p->N, p->stream));
+        VMAT_CUDA(p, cudaMemsetAsync(p->nsync, 0, 32, p->stream));
+        if ((rc = reset_hessian(p))) return rc;
+    }
     VMAT_CUDA(p, cudaMemsetAsync(p->accbuf, 0, (size_t)3 * kSumGroups * (2 * p->N + 2) * 8, p->stream));
     VMAT_CUDA(p, cudaMemsetAsync(p->phase, 0, 8, p->stream));
     VMAT_CUDA(p, cudaMemsetAsync(p->colstat, 0, (size_t)p->N * sizeof(ColStat), p->stream));
@@ -2046,6 +2565,29 @@ int master_configure(vmat_plan *p) {
     VMAT_CUDA(p, cudaStreamSynchronize(p->stream));
     p->Tmax = hb[0];
     p->abmax = hb[1];
+    // fixed-point scale of H_F: |sum_s omega_s d_k[s] d_k'[s]| <= max(alpha, beta) Sp (R C max|D|)^2 < 2^e
+    // (p->fx_inv = 2^(e2 - 40) with max|D| < 2^e2: vmat_layout.cu)
+    {
+        int e2 = 0, eab = 0, esp = 0, erc = 0;
+        std::frexp(p->fx_inv, &e2);   // fx_inv = 2^(e2' - 40) = 0.5 * 2^(e2' - 39): frexp exponent = e2' - 39
+        e2 += 39;
+        std::frexp((double)(p->abmax > 0.f ? p->abmax : 1.f), &eab);
+        std::frexp((double)p->Sp, &esp);
+        std::frexp((double)p->RC, &erc);
+        const int e = eab + esp + 2 * (erc + e2);
+        p->hscale = std::ldexp(1.0, 60 - e);
+        p->hinv = std::ldexp(1.0, e - 60);
+    }
+    return VMAT_OK;
+}
+
+// H_F, the omega it was built with and the flags of its columns back to "empty" (after vmat_set_plan: the apertures
+// behind the columns may all have changed)
+int reset_hessian(vmat_plan *p) {
+    if (!p->master_newton) return VMAT_OK;
+    VMAT_CUDA(p, cudaMemsetAsync(p->hess, 0, (size_t)p->N * p->N * 8, p->stream));
+    VMAT_CUDA(p, cudaMemsetAsync(p->omref, 0, (size_t)p->Sp * 4, p->stream));
+    VMAT_CUDA(p, cudaMemsetAsync(p->hvalid, 0, (size_t)p->N, p->stream));
     return VMAT_OK;
 }
 
@@ -2110,8 +2652,17 @@ static int launch_master_impl(vmat_plan *p, int max_inner, int trace_it, int war
     a.trC = p->tr_cost;
     a.trInner = p->tr_inner;
     a.trace_it = trace_it;
+    a.nblk = p->master_nblk;
+    a.hess = p->hess;
+    a.omref = p->omref;
+    a.hvalid = p->hvalid;
+    a.hscale = p->hscale;
+    a.hinv = p->hinv;
+    a.wn = p->wn_s;
+    a.mail = (Mail *)p->mail;
+    a.sync = p->nsync;
     void *args[] = {&a};
-    const void *fn = p->opt.master_mode == 1 ? (const void *)k_master<1> : (const void *)k_master<0>;
+    const void *fn = p->master_newton ? (const void *)k_newton : (const void *)k_master;
     VMAT_CUDA(p, cudaLaunchCooperativeKernel(fn, dim3((unsigned)p->master_grid), dim3(kMasterThreads), args,
                                              p->master_smem, p->stream));
     ++p->launches;
@@ -2125,13 +2676,19 @@ int launch_master(vmat_plan *p, int trace_it, int warm) {
 // steps (a)+(b) alone: the master kernel's evaluation pass with no iteration allowed
 int launch_dose_grad(vmat_plan *p) { return launch_master_impl(p, 0, -1, 0); }
 
-#ifdef VMAT_MASTER_PROFILE
-extern "C" void vmat_debug_master_prof(long long out[16], int reset) {
-    cudaMemcpyFromSymbol(out, g_master_prof, sizeof(long long) * 16);
-    if (reset) {
-        long long z[16] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
-        cudaMemcpyToSymbol(g_master_prof, z, sizeof(z));
-    }
+#ifdef VMAT_NEWTON_TRACE
+extern "C" void vmat_debug_newton_trace(unsigned long long *out, unsigned int *n) {
+    cudaMemcpyFromSymbol(out, g_tr, sizeof(unsigned long long) * 4 * 4096);
+    cudaMemcpyFromSymbol(n, g_trn, 4);
+    long long seg[8];
+    cudaMemcpyFromSymbol(seg, g_seg, sizeof(seg));
+    fprintf(stderr, "cg segments (clk, thread 0): R1 %lld d-update %lld matvec %lld R2 %lld update %lld | reduce: level1 %lld barrier %lld level2 %lld\n", seg[0], seg[1], seg[2], seg[3], seg[4], seg[5], seg[6], seg[7]);
+    long long zs[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    cudaMemcpyToSymbol(g_seg, zs, sizeof(zs));
+    unsigned int z = 0;
+    cudaMemcpyToSymbol(g_trn, &z, 4);
+    static unsigned long long zeros[4 * 4096];
+    cudaMemcpyToSymbol(g_tr, zeros, sizeof(zeros));
 }
 #endif
 

@@ -116,14 +116,9 @@ int launch_free_list(vmat_plan *p) {
 // g_i for the beamlets of the n_free un-occupied beams listed in p->free_list; other entries of g untouched
 int launch_price_spmv(vmat_plan *p, const float *w_s, float *g, int n_free) {
     if (p->B == 0 || n_free <= 0) return VMAT_OK;
-    switch (p->opt.pricing_kernel) {
-        case 1: launch_variant<32, 2>(p, w_s, g, n_free); break;
-        case 2: launch_variant<32, 4>(p, w_s, g, n_free); break;
-        case 3: launch_variant<16, 2>(p, w_s, g, n_free); break;
-        case 4: launch_variant<16, 4>(p, w_s, g, n_free); break;
-        case 5: launch_variant<8, 4>(p, w_s, g, n_free); break;
-        default: launch_variant<16, 4>(p, w_s, g, n_free); break;
-    }
+    // 16 lanes per beamlet, 4 x 16-byte loads of values and of indices in flight per lane: the best of the five
+    // lanes x loads variants measured in round 1 (table of rejected variants)
+    launch_variant<16, 4>(p, w_s, g, n_free);
     ++p->launches;
     VMAT_CUDA(p, cudaGetLastError());
     return VMAT_OK;

@@ -164,7 +164,7 @@ template <int M>
 __global__ void __launch_bounds__(kSearchThreads) k_leaf_search(const SearchArgs a) {
     pdl_wait();      // the prices (launched behind the pricing product by programmatic dependent launch)
     pdl_trigger();   // the column build may be scheduled; it waits for the choice itself
-    __shared__ int s_km, s_kp, s_last;
+    __shared__ int s_km, s_kp, s_last, s_bad;
     __shared__ unsigned long long s_total;
     __shared__ double s_price[kRowsPerBlock];
     __shared__ int s_beam[kRowsPerBlock];
@@ -181,6 +181,7 @@ __global__ void __launch_bounds__(kSearchThreads) k_leaf_search(const SearchArgs
         if (tid == 0) {
             s_km = -1;
             s_kp = N;
+            s_bad = 0;
             s_total = 0ull;
         }
         __syncthreads();
@@ -227,13 +228,19 @@ __global__ void __launch_bounds__(kSearchThreads) k_leaf_search(const SearchArgs
                     a.out_right[k * R + r] = br;
                 }
                 atomicAdd(&s_total, (unsigned long long)value);   // exact, order free
+                // The box admits no interval: the beam has no deliverable aperture.  Cannot happen
+                // while the occupied apertures respect the leaf-travel limit among themselves, which vmat_set_plan
+                // checks and the loop preserves (S6); kept so that such a beam could never be chosen.
+                if (bl < 0) s_bad = 1;
             }
         }
         __syncthreads();
         if (tid == 0) {
             atomicAdd(a.beam_total + k, s_total);
+            if (s_bad) atomicOr(a.beam_ticket + k, 0x80000000u);   // bit 31: a row of this beam is undeliverable
             __threadfence();
-            if (atomicAdd(a.beam_ticket + k, 1u) == (unsigned)RB - 1u) {
+            const unsigned int seen = atomicAdd(a.beam_ticket + k, 1u);
+            if ((seen & 0x7fffffffu) == (unsigned)RB - 1u) {
                 __threadfence();
                 beam_done = true;
                 const long long total = (long long)atomicExch(a.beam_total + k, 0ull);   // all RB sums are in; reset
@@ -248,7 +255,8 @@ __global__ void __launch_bounds__(kSearchThreads) k_leaf_search(const SearchArgs
                     dG = __dsub_rn(dG, __ddiv_rn(__dmul_rn(2.0, __dsub_rn(a.y[k + 1], a.y[k])),
                                                  __dsub_rn(a.theta[k + 1], a.theta[k])));
                 const double smooth = __dmul_rn(a.gamma, dG);
-                const double price = __dadd_rn(ldexp(__ll2double_rn(total), -30), smooth);
+                const bool undeliverable = (seen >> 31) != 0u || s_bad;
+                const double price = undeliverable ? CUDART_INF : __dadd_rn(ldexp(__ll2double_rn(total), -30), smooth);
                 a.beam_price[k] = price;
                 if (a.out_price) a.out_price[k] = price;
             }
@@ -274,7 +282,7 @@ __global__ void __launch_bounds__(kSearchThreads) k_leaf_search(const SearchArgs
     int bk = -1;
     for (int kk = tid; kk < N; kk += kSearchThreads) {
         const double pr = __ldcg(a.beam_price + kk);
-        if (!a.occ[kk] && (bk < 0 || pr < bp)) {   // ascending kk: the lowest index wins ties
+        if (!a.occ[kk] && pr < CUDART_INF && (bk < 0 || pr < bp)) {   // ascending kk: the lowest index wins ties
             bp = pr;
             bk = kk;
         }

@@ -53,6 +53,91 @@ def test_teacher_forced_steps_fullsize(setup):
     _teacher_forced(setup, 3)
 
 
+def test_free_run_prefix_matches_oracle_fullsize(setup):
+    """P3 at BASELINE.json configs[1]: the oracle's own free run over the first 60 column-generation iterations
+    against vmat_solve(60) in the launch configuration bench.py times: same beams and leaf pairs, cost trace within
+    1e-4; a parting of the ways is admissible only at a tie within fp32 noise (reported, with the oracle's prices)."""
+    from test_gpu_parity import check_free_run_against_oracle
+
+    torch, vm, ph, o, plan = setup
+    n = 60
+    occ_r, left_r, right_r, y_r, z_r, tr = o.solve(n, eps=1e-9)
+    e = o.empty_plan()
+    plan.set_plan(e[0], e[1], e[2], e[3])
+    st = plan.solve(n)
+    occ, left, right, y = plan.get_plan()
+    assert st.iters == n
+    check_free_run_against_oracle(o, st, (occ, left, right, y), tr,
+                                  lambda m: o.solve(m, eps=1e-9)[:4] if m else o.empty_plan())
+
+
+@pytest.mark.parametrize("seed", [0, 1, 2, 3])
+def test_master_stop_rule_stays_within_tolerance_of_the_converged_cost(seed):
+    """The product default ends a master solve when two accepted steps in a row lower the cost by <= 1e-6 of it
+    (vmat_options.master_stall_rel / _count; S11).  Evidence that this stays inside the 1e-4 parity tolerance
+    on the cost: every 20th outer iteration of configs[1] (seeds 0-3) the state the loop has reached is re-solved by
+    a second plan with the stop rule off and a 100x tighter projected-gradient tolerance; the loop's post-master cost
+    must be within 1e-4 of that converged cost (and can never be below it by more than fp32 noise)."""
+    import torch
+
+    import paper_1005_4396_b200 as vm
+    import vmat_inputs
+
+    ph = vmat_inputs.make_phantom("prostate", seed=seed)
+    loop = vm.Plan.from_phantom(ph)
+    ref = vm.Plan.from_phantom(ph)
+    N = ph.config.n_beams
+    worst = 0.0
+    for done in range(20, N + 1, 20):
+        st = loop.solve(20)
+        assert st.iters == 20
+        occ, left, right, y = loop.get_plan()
+        ref.set_plan(occ, left, right, y)
+        conv = ref.master(eps=1e-7, max_inner=5000, stall_rel=1e-12, stall_count=1000)
+        gap = (st.cost - conv.cost) / abs(conv.cost)
+        worst = max(worst, gap)
+        assert -1e-6 <= gap <= TOL, (seed, done, st.cost, conv.cost, conv)
+    print(f"seed {seed}: worst gap of the loop's post-master cost to the converged cost {worst:.3g}")
+    loop.destroy()
+    ref.destroy()
+
+
+def test_teacher_forced_steps_stress():
+    """BASELINE.json configs[4] (stress phantom: 1,728,000 beamlets, 1.46e9 non-zeros, 360 beams): the only config whose
+    byte offsets into the device layout pass 2^32, whose aperture-dose columns mostly stream from HBM, and whose 360
+    beams take the second trip of the 256-thread loops over beams in the leaf search.  Two teacher-forced iterations
+    (prices of every beamlet, bit-exact search, dose + gradient, master cost on the same apertures), then 20
+    free-running iterations checked on what holds at any size and on the oracle's recomputation of dose and cost."""
+    s = _setup("stress")
+    try:
+        _teacher_forced(s, 2)
+        torch, vm, ph, o, plan = s
+        st = plan.solve(20)
+        occ, left, right, y = plan.get_plan()
+        assert st.iters == 20 and occ.sum() == 22 and np.all(y >= 0) and np.all(y[occ == 0] == 0)
+        assert len(set(st.beam.tolist())) == 20
+        assert np.all(np.diff(st.trace_cost) <= 1e-5 * np.abs(st.trace_cost[:-1]))
+        ks = np.flatnonzero(occ)
+        for a, b in zip(ks[:-1], ks[1:]):
+            lim = o.delta * (b - a)
+            assert np.all(np.abs(left[b] - left[a]) <= lim) and np.all(np.abs(right[b] - right[a]) <= lim)
+        z = torch.empty(o.V, dtype=torch.float32, device="cuda")
+        _, _, cost = plan.dose(z)
+        z_ref = o.dose(occ, left, right, y)
+        F_ref, _ = o.penalty(z_ref)
+        G_ref, _ = o.smooth(y)
+        assert relnorm(z.cpu().numpy(), z_ref) <= TOL
+        assert abs(cost - (F_ref + o.gamma * G_ref)) <= TOL * abs(F_ref + o.gamma * G_ref)
+        assert abs(st.cost - cost) <= 1e-6 * abs(cost)
+        plan.dose_recompute(1)                                                     # straight from D: offsets past 2^32
+        z1 = torch.empty(o.V, dtype=torch.float32, device="cuda")
+        _, _, cost1 = plan.dose(z1)
+        assert relnorm(z1.cpu().numpy(), z_ref) <= TOL
+        assert abs(cost1 - (F_ref + o.gamma * G_ref)) <= TOL * abs(F_ref + o.gamma * G_ref)
+    finally:
+        s[4].destroy()
+
+
 def test_teacher_forced_steps_head_and_neck(setup_hn):
     _teacher_forced(setup_hn, 2)
     # and a stretch of the free-running loop: invariants that hold at any size
@@ -189,14 +274,10 @@ def test_full_plan_properties(setup):
     assert abs(boxed.cost - cost_b) <= TOL * abs(cost_b)                       # the oracle prices the boxed plan alike
     fused.destroy()
     # the fallback of the unstaged columns (masked loops, taken when their per-chunk lists do not fit in shared
-    # memory) is forced by an environment variable read at vmat_create
-    import os
-
-    os.environ["VMAT_MASTER_MASKED_LOOPS"] = "1"
-    try:
-        masked = vm.Plan.from_phantom(ph)
-    finally:
-        del os.environ["VMAT_MASTER_MASKED_LOOPS"]
+    # memory) is forced by vmat_options.master_unstaged_lists = 0
+    opt = vm.default_options()
+    opt.master_unstaged_lists = 0
+    masked = vm.Plan.from_phantom(ph, options=opt)
     masked.set_plan(occ, left, right, np.zeros(o.N))
     mm = masked.master()
     assert abs(mm.cost - cost) <= TOL * abs(cost), (mm, cost)

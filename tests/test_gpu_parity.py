@@ -36,8 +36,44 @@ def relnorm(a, ref):
     return d / max(np.max(np.abs(ref)), 1e-300) if ref.size else 0.0
 
 
+TIE = 1e-6          # fp32 noise of a beam price (a sum of ~1e3 fp32 products, quantised at 2^-30)
+
+
+def check_free_run_against_oracle(o, st, plan_state, tr, oracle_state_at, tie=TIE):
+    """P3: the free runs coincide (beams, leaf pairs, cost trace within TOL), or they part at an
+    iteration where the two candidates are a tie within fp32 noise: the first diverging iteration is reported, the
+    oracle's own prices of the two beams at that iteration differ by at most `tie` relative, and everything before
+    it agrees.  oracle_state_at(it) -> (occ, left, right, y) of the oracle's run after `it` iterations."""
+    occ, left, right, y = plan_state
+    n = min(st.iters, tr.iters)
+    assert st.iters == tr.iters
+    differ = np.flatnonzero(st.beam[:n] != tr.beam[:n])
+    if differ.size == 0:
+        # same beams: the leaf pairs must be the same too, and the costs agree
+        for it in range(n):
+            k = int(tr.beam[it])
+            assert np.array_equal(left[k], tr.left[it]) and np.array_equal(right[k], tr.right[it]), f"iteration {it}"
+        assert relnorm(st.trace_cost, tr.cost) <= TOL
+        assert abs(st.cost - tr.cost[-1]) <= TOL * abs(tr.cost[-1])
+        return -1
+    it = int(differ[0])
+    # the oracle's own state before iteration `it` (its run again, `it` iterations long)
+    occ_o, left_o, right_o, y_o = oracle_state_at(it)
+    z = o.dose(occ_o, left_o, right_o, y_o)
+    _, w = o.penalty(z)
+    ref = o.price_step(o.prices(w, occ_o).astype(np.float32), occ_o, left_o, right_o, y_o)
+    pa, pb = ref["beam_price"][int(st.beam[it])], ref["beam_price"][int(tr.beam[it])]
+    gap = abs(pa - pb) / max(abs(pb), 1e-300)
+    print(f"free run parts from the oracle's at iteration {it}: gpu beam {int(st.beam[it])} (oracle price {pa:.9g}), "
+          f"oracle beam {int(tr.beam[it])} (price {pb:.9g}), relative gap {gap:.3g}")
+    assert gap <= tie, f"iteration {it}: the two candidates are not a tie (gap {gap:.3g} > {tie:g})"
+    if it:
+        assert relnorm(st.trace_cost[:it], tr.cost[:it]) <= TOL
+    return it
+
+
 def mode_options(vm, mode):
-    """master_mode 0 = two passes / two grid barriers per inner iteration, 1 = one fused pass / one barrier."""
+    """master_mode 0 = gradient projection with conjugate directions, 1 = semismooth Newton on the reduced problem."""
     opt = vm.default_options()
     opt.master_mode = mode
     return opt
@@ -367,19 +403,14 @@ def test_master_with_unstaged_columns_over_several_groups(torch_cuda, vm):
     occ[:] = 1
     left = np.zeros((N, R), np.int32)
     right = np.full((N, R), C, np.int32)                                   # every beamlet exposed
-    import os
-
     for mode, masked in ((0, False), (1, False), (0, True), (1, True)):
-        # masked: the fallback loops over the unstaged columns (taken when their lists do not fit), forced by an
-        # environment variable that vmat_create reads
-        if masked:
-            os.environ["VMAT_MASTER_MASKED_LOOPS"] = "1"
-        try:
-            plan = make_plan(vm, o, options=mode_options(vm, mode))
-        finally:
-            os.environ.pop("VMAT_MASTER_MASKED_LOOPS", None)
+        # masked: the fallback loops over the unstaged columns (taken when their lists do not fit), forced by
+        # vmat_options.master_unstaged_lists = 0
+        opt = mode_options(vm, mode)
+        opt.master_unstaged_lists = 0 if masked else 1
+        plan = make_plan(vm, o, options=opt)
         st = check_master(plan, o, occ, left, right, np.zeros(N))
-        assert st.inner > 3
+        assert st.inner > (3 if mode == 0 else 1)              # the Newton mode needs a handful of steps only
         check_master(plan, o, occ, left, right, rng.uniform(0.0, 2.0, N))
         # dose and gradient of the GPU's y against the oracle, through the same columns
         _, _, _, y = plan.get_plan()
@@ -438,24 +469,37 @@ def test_solve_free_run_tiny(torch_cuda, vm, tiny_oracle, tiny_solution, mode):
     assert occ.all()
     # post-master cost is non-increasing (convexity; S2)
     assert np.all(np.diff(st.trace_cost) <= 1e-5 * np.abs(st.trace_cost[:-1]))
-    same = np.array_equal(st.beam, tr.beam) and np.array_equal(left, left_r) and np.array_equal(right, right_r)
-    if same:
-        assert relnorm(st.trace_cost, tr.cost) <= TOL
-        assert abs(st.cost - tr.cost[-1]) <= TOL * abs(tr.cost[-1])
-    else:
-        # P3: a diverging run is admissible only where the two candidates are a tie within fp32 noise (the tiny
-        # phantom is mirror symmetric: beams k and N - k price alike); report the first diverging iteration
-        it = int(np.argmax(st.beam != tr.beam)) if not np.array_equal(st.beam, tr.beam) else -1
-        tie = it >= 0 and abs(st.price[it] - tr.price[it]) <= TOL * abs(tr.price[it])
-        if not (mode == 1 and tie):
-            pytest.fail(f"free run diverged from the oracle at iteration {it}: gpu {st.beam.tolist()} "
-                        f"oracle {tr.beam.tolist()}")
-        assert relnorm(st.trace_cost[:it], tr.cost[:it]) <= TOL
-        assert abs(st.cost - tr.cost[-1]) <= 1e-2 * abs(tr.cost[-1])      # another, equally legal, aperture sequence
+    # (the device's stop rule lets an accepted step raise the cost by at most the fp32 resolution of the dose
+    # arithmetic; 1e-5 is 10x its stall threshold of 1e-6)
+    check_free_run_against_oracle(o, st, (occ, left, right, y), tr, lambda n: o.solve(n)[:4] if n else o.empty_plan())
     # the leaf-travel invariant holds on the finished arc
     for k in range(o.N - 1):
         assert np.all(np.abs(left[k + 1] - left[k]) <= o.delta) and np.all(np.abs(right[k + 1] - right[k]) <= o.delta)
     plan.destroy()
+
+
+def test_solve_with_dose_rate_bounds_matches_oracle(torch_cuda, vm, tiny_oracle, tiny_solution):
+    """vmat_solve under vmat_set_dose_rate_bounds with y_min > 0: a new beam enters at y_min, so the dose moves on
+    entry and every master solve has to start from an evaluation (no warm entry).  Same apertures and cost trace as
+    the oracle's loop with the same box."""
+    o = tiny_oracle
+    y0 = tiny_solution[3]
+    lb, ub = 0.3 * float(np.median(y0)), 0.7 * float(y0.max())
+    occ_r, left_r, right_r, y_r, z_r, tr = o.solve(40, y_min=lb, y_max=ub)
+    for mode in (0, 1):
+        plan = make_plan(vm, o, options=mode_options(vm, mode))
+        plan.set_dose_rate_bounds(lb, ub)
+        st = plan.solve(40)
+        occ, left, right, y = plan.get_plan()
+        assert st.iters == o.N and occ.all() and np.all(y >= lb) and np.all(y <= ub)
+        check_free_run_against_oracle(o, st, (occ, left, right, y), tr,
+                                      lambda n: o.solve(n, y_min=lb, y_max=ub)[:4] if n else o.empty_plan())
+        # the state the loop leaves is the state of its plan: dose and cost recomputed by the oracle
+        z = torch_cuda.empty(o.V, dtype=torch_cuda.float32, device="cuda")
+        F, G, cost = plan.dose(z)
+        assert relnorm(z.cpu().numpy(), o.dose(occ, left, right, y)) <= TOL
+        assert abs(cost - o.cost(occ, left, right, y)[2]) <= TOL * abs(cost) and abs(cost - st.cost) <= 1e-9 * abs(cost)
+        plan.destroy()
 
 
 def test_solve_stop_when_priced_out_option(torch_cuda, vm):

@@ -272,7 +272,8 @@ def test_leaf_box_from_nearest_occupied_neighbours():
     assert o.leaf_box(occ, left, right, 4, 0) == (3, 7, 4, 8)
     # beam 0 only sees beam 1 (nearest on the right), beam 8 only beam 5
     assert o.leaf_box(occ, left, right, 0, 0) == (1, 5, 5, 9)
-    assert o.leaf_box(occ, left, right, 8, 0) == (0, 10, 0, 10) or o.leaf_box(occ, left, right, 8, 0) == (0, 10, 0, 10)
+    assert o.leaf_box(occ, left, right, 8, 0) == (0, 10, 0, 10)           # 3 steps from beam 5: +-6 around (5, 6), clipped
+    assert o.leaf_box(occ, left, right, 8, 1) == (0, 6, 4, 10)            # row 1 of beam 5 is (0, 10)
     assert o.leaf_box(occ, left, right, 7, 0) == (1, 9, 2, 10)
 
 
@@ -334,6 +335,101 @@ def test_beam_choice_lowest_index_on_ties():
 # ------------------------------------------------------------------------------------------------
 # O7 master
 # ------------------------------------------------------------------------------------------------
+def test_price_step_never_chooses_an_undeliverable_beam():
+    """Hand-built occupied neighbours whose leaf-travel boxes do not intersect (they break the travel limit between
+    themselves, which the loop can never produce): the beam between them has no deliverable aperture (PAPER.md:111,
+    "all the deliverability constraints") and must not be chosen however good its prices are."""
+    o, _, rng = small_problem(5, N=5, R=2, C=10, delta=1)
+    occ = np.array([1, 0, 1, 0, 0], np.uint8)
+    left = np.zeros((5, 2), np.int32)
+    right = np.zeros((5, 2), np.int32)
+    left[0], right[0] = [0, 2], [1, 5]
+    left[2], right[2] = [8, 2], [9, 5]                  # row 0: tips 8 apart over 2 steps of 1 beamlet
+    assert o.leaf_box(occ, left, right, 1, 0) == (7, 1, 8, 2)             # Lmin > Lmax: empty
+    assert orc.row_search(np.zeros(10, np.int64), 7, 1, 8, 2) is None
+    g32 = np.zeros(o.B, np.float32)
+    g32[1 * 2 * 10:2 * 2 * 10] = -100.0                # beam 1 would win by far
+    g32[3 * 2 * 10 + 12] = -1.0                        # beam 3, row 1, column 2
+    out = o.price_step(g32, occ, left, right, np.zeros(5))
+    assert out["beam"] == 3 and np.isinf(out["beam_price"][1]) and out["beam_price"][3] == -1.0
+    assert out["all_left"][1][0] == -1 and out["all_right"][1][0] == -1
+    # nothing deliverable at all: no beam
+    occ2 = np.array([1, 0, 1, 1, 1], np.uint8)
+    left[3:], right[3:] = left[2], right[2]
+    assert o.price_step(g32, occ2, left, right, np.zeros(5))["beam"] == -1
+
+
+# ------------------------------------------------------------------------------------------------
+# O7 master problem
+# ------------------------------------------------------------------------------------------------
+def test_cost_gradient_matches_central_differences():
+    """vo_cost_gradient (the gradient the KKT pins read) against central differences of the cost, which is itself
+    pinned by the dense dose product, the one-voxel closed form and the Laplacian form of G."""
+    for seed in range(3):
+        o, D, rng = small_problem(300 + seed, V=70, N=6, R=3, C=5, gamma=0.35, nonuniform_theta=bool(seed % 2))
+        occ, left, right, y = random_plan(o, rng, 4)
+        grad, c3 = o.cost_gradient(occ, left, right, y)
+        assert c3[2] == pytest.approx(o.cost(occ, left, right, y)[2], rel=1e-14)
+        h = 1e-6
+        for k in range(o.N):
+            if not occ[k]:
+                assert grad[k] == 0.0
+                continue
+            e = np.zeros(o.N)
+            e[k] = h
+            fd = (o.cost(occ, left, right, y + e)[2] - o.cost(occ, left, right, y - e)[2]) / (2 * h)
+            assert grad[k] == pytest.approx(fd, rel=2e-6, abs=1e-7), (seed, k)
+
+
+def plain_projected_descent(Dc, T, al, be, Lap, gamma, lb, ub, iters=20000):
+    """TEST-ONLY reference for the master problem ("gradient projection method"; Eq. 3): plain projected
+    steepest descent on the box with Armijo back-tracking along the projection arc (the trial step doubles after an
+    accepted step, halves until sufficient decrease) — no conjugate directions, no active-set logic, nothing shared
+    with the oracle.  Dc: K x V aperture-dose columns.  Stops when a step no longer lowers the cost."""
+    y = np.clip(np.zeros(Dc.shape[0]), lb, ub)
+
+    def phi(y):
+        z = y @ Dc
+        return float(np.sum(al * np.maximum(0, T - z) ** 2 + be * np.maximum(0, z - T) ** 2) + gamma * y @ Lap @ y), z
+
+    f, z = phi(y)
+    t = 1.0
+    for _ in range(iters):
+        w = -2 * al * np.maximum(0, T - z) + 2 * be * np.maximum(0, z - T)
+        g = Dc @ w + 2 * gamma * (Lap @ y)
+        t *= 2.0
+        while True:
+            yn = np.clip(y - t * g, lb, ub)
+            fn, zn = phi(yn)
+            if fn <= f - 1e-4 * float(g @ (y - yn)) or t < 1e-30:
+                break
+            t *= 0.5
+        if not fn < f:
+            break
+        y, f, z = yn, fn, zn
+    return y, f
+
+
+def test_master_reaches_the_cost_of_plain_projected_steepest_descent():
+    """The oracle's master carries conjugate directions and an active-set restart; this pins its optimum to a solver
+    that has neither (and shares no code with it), on small random problems with one-sided penalties (alpha = 0 on
+    half the voxels), with and without the box on the dose rates."""
+    for seed in range(4):
+        o, D, rng = small_problem(400 + seed, V=40, N=5, R=2, C=4, gamma=(0.0, 0.3, 1.0, 0.1)[seed],
+                                  nonuniform_theta=bool(seed % 2))
+        occ, left, right, _ = random_plan(o, rng, o.N)
+        Dc = np.einsum("krc,krcv->kv", open_mask(o, occ, left, right), D.reshape(o.N, o.R, o.C, o.V))
+        Lap = np.zeros((o.N, o.N))
+        for k in range(o.N - 1):
+            s = 1.0 / (o.theta[k + 1] - o.theta[k])
+            Lap[k, k] += s; Lap[k + 1, k + 1] += s; Lap[k, k + 1] -= s; Lap[k + 1, k] -= s
+        T, al, be = (a.astype(np.float64) for a in (o.T, o.alpha, o.beta))
+        for lb, ub in ((0.0, np.inf), (0.02, 0.2)):
+            y_ref, f_ref = plain_projected_descent(Dc, T, al, be, Lap, o.gamma, lb, ub)
+            y, z, info = o.master(occ, left, right, eps=1e-12, y_min=lb, y_max=ub)
+            assert info.cost == pytest.approx(f_ref, rel=1e-9), (seed, lb, ub)
+
+
 def kkt_violation(o, occ, left, right, y):
     grad, _ = o.cost_gradient(occ, left, right, y)
     viol = 0.0
@@ -479,6 +575,29 @@ def test_master_bounds_satisfy_box_kkt_random():
         assert info.cost == pytest.approx(cost, rel=1e-13) and info.cost >= free.cost * (1 - 1e-12)
         np.testing.assert_allclose(z, o.dose(occ, left, right, y), rtol=1e-12, atol=1e-12)
     assert hit_lo and hit_hi and inside                                   # the test saw all three cases
+
+
+def test_solve_with_bounds_keeps_every_master_in_the_box(tiny_oracle, tiny_solution):
+    """The loop with bounds on the dose rates (reading R4): prices are those of the paper, every master solve is the
+    box-constrained one.  Pinned by what must hold whatever the path: y in the box at occupied beams and 0 elsewhere,
+    the recorded cost is the cost of the returned plan, a fresh box-constrained master solve on the final aperture
+    set (itself pinned by the BVLS / KKT tests above) cannot lower it, and lb = 0, ub = inf is the unbounded loop."""
+    o = tiny_oracle
+    occ0, left0, right0, y0, z0, tr0 = tiny_solution
+    occ, left, right, y, z, tr = o.solve(40, y_min=0.0, y_max=float("inf"))
+    assert np.array_equal(tr.beam, tr0.beam) and np.array_equal(left, left0) and np.array_equal(right, right0)
+    np.testing.assert_allclose(tr.cost, tr0.cost, rtol=1e-12)       # (OpenMP sums: the last bits depend on the run)
+    np.testing.assert_allclose(y, y0, rtol=1e-7, atol=1e-10)
+    lb, ub = 0.3 * float(np.median(y0)), 0.7 * float(y0.max())
+    for n in (5, 40):
+        occ, left, right, y, z, tr = o.solve(n, y_min=lb, y_max=ub)
+        on = occ.astype(bool)
+        assert np.all(y[on] >= lb) and np.all(y[on] <= ub) and np.all(y[~on] == 0.0)
+        assert np.any(y[on] == lb) or np.any(y[on] == ub)                        # the box binds
+        assert tr.cost[-1] == pytest.approx(o.cost(occ, left, right, y)[2], rel=1e-12)
+        _, _, info = o.master(occ, left, right, y0=y, eps=1e-10, y_min=lb, y_max=ub)
+        assert info.cost == pytest.approx(tr.cost[-1], rel=1e-7) and info.cost <= tr.cost[-1] * (1 + 1e-12)
+    assert tr.cost[-1] > tr0.cost[-1]                                            # a binding box costs something
 
 
 def test_master_bounds_equal_bounded_least_squares_when_all_quadratic():
