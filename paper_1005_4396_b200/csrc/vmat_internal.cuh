@@ -106,6 +106,7 @@ struct vmat_plan {
     long long *hess = nullptr;         // N x N fixed point
     float *omref = nullptr;            // Sp: the omega (alpha, beta or 0 per slot) the matrix was built with
     uint8_t *hvalid = nullptr;         // N: column k is in the matrix
+    int *hlive = nullptr;              // device flag: the matrix is built (a k_newton launch has run since its last reset)
     double hscale = 1.0, hinv = 1.0;
     float *wn_s = nullptr;             // Sp: second buffer of w
     void *mail = nullptr;              // message of the solving block to the working blocks

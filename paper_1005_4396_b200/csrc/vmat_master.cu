@@ -92,13 +92,28 @@ k_column_scatter(const uint32_t *__restrict__ rowq, const float4 *__restrict__ v
     }
 }
 
+__device__ __forceinline__ double warp_sum8(double (&v)[8], int lane);
+
+// What k_column_finish needs to enter the new column into the Hessian of mode 1 (k_newton); hess == nullptr otherwise.
+struct HessRowArgs {
+    long long *hess;          // N x N fixed point, upper triangle
+    const float *omref;       // Sp: the omega the matrix was built with
+    const uint8_t *occ;       // N
+    uint8_t *hvalid;          // N: column i is in the matrix
+    const int *hlive;         // the matrix is built (a master solve has run since it was last reset)
+    double hscale;
+};
+
 // Dd[k][.] = fixed-point accumulator as fp32; clears the accumulator; gathers the column's
 // statistics (exact integer sums / extrema, hence order free): sum and max of |d_k|, first and
 // last chunk with a non-zero entry.  One block = 256 slots = 2 chunks.
+// Mode 1 of the master: the block also adds its two chunks' share of the new column's row of the Hessian,
+// H_F[k][i] = sum_s omega_s d_k[s] d_i[s] over the columns i already in the matrix, so that the next master solve needs
+// no pass of its own for it (and none at all before its first Newton step).
 __global__ void __launch_bounds__(256)
 k_column_finish(unsigned long long *__restrict__ acc, long long Sp, const Sel *__restrict__ sel, int beam,
                 double fx_inv, float *__restrict__ Dd, int N, ColStat *__restrict__ colstat,
-                uint32_t *__restrict__ touch, int touch_words) {
+                uint32_t *__restrict__ touch, int touch_words, const HessRowArgs hr) {
     pdl_wait();      // the scatter's adds
     const int k = sel ? sel->beam : beam;
     if (k < 0) return;
@@ -106,9 +121,11 @@ k_column_finish(unsigned long long *__restrict__ acc, long long Sp, const Sel *_
     __shared__ int s_lo[8], s_hi[8];
     const long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     unsigned long long mag = 0ull;
+    float dk = 0.f;
     if (s < Sp) {
         const long long v = (long long)acc[s];
-        Dd[((size_t)(s / kChunk) * N + k) * kChunk + (s & (kChunk - 1))] = (float)((double)v * fx_inv);   // chunk-major
+        dk = (float)((double)v * fx_inv);
+        Dd[((size_t)(s / kChunk) * N + k) * kChunk + (s & (kChunk - 1))] = dk;   // chunk-major
         acc[s] = 0ull;
         mag = (unsigned long long)(v < 0 ? -v : v);
     }
@@ -146,6 +163,63 @@ k_column_finish(unsigned long long *__restrict__ acc, long long Sp, const Sel *_
             atomicMin(&colstat[k].clo, lo);
             atomicMax(&colstat[k].chi, hi);
         }
+    }
+    // ---- the new column's row of the Hessian (mode 1) ------------------------------------------------
+    if (hr.hess == nullptr || !*hr.hlive || N > 256) return;   // the same for the whole grid
+    if (blockIdx.x == 0 && threadIdx.x == 0) hr.hvalid[k] = 1;   // (no block reads the flag of k itself)
+    __shared__ int s_live[2], s_cnt[2], s_list[2][256];
+    __shared__ float4 s_u[2][kChunk / 4], s_d[2][kChunk / 4];
+    const int lane = threadIdx.x & 31, half = threadIdx.x >> 7;   // warps 0-3: the block's first chunk, 4-7: its second
+    const int sl = threadIdx.x & (kChunk - 1);
+    const float u = s < Sp ? hr.omref[s] * dk : 0.f;
+    reinterpret_cast<float *>(s_u[half])[sl] = u;
+    reinterpret_cast<float *>(s_d[half])[sl] = dk;
+    if (threadIdx.x < 2) s_live[threadIdx.x] = s_cnt[threadIdx.x] = 0;
+    __syncthreads();
+    if (__any_sync(kFull, u != 0.f) && lane == 0) s_live[half] = 1;
+    __syncthreads();
+    // the columns in the matrix that touch the chunk (any order: what each adds is an integer)
+    if ((int)threadIdx.x < N && (int)threadIdx.x != k && hr.occ[threadIdx.x] && hr.hvalid[threadIdx.x]) {
+        const uint32_t *tw = touch + (size_t)threadIdx.x * touch_words;
+        for (int h = 0; h < 2; ++h) {
+            const int c = 2 * (int)blockIdx.x + h;
+            if (s_live[h] && (long long)c * kChunk < Sp && ((tw[c >> 5] >> (c & 31)) & 1u)) s_list[h][atomicAdd(&s_cnt[h], 1)] = (int)threadIdx.x;
+        }
+    }
+    __syncthreads();
+    if (!s_live[half]) return;
+    // every warp of the chunk takes every fourth column of the list, eight at a time: one float4 of the column's
+    // 512-byte segment per lane (all eight loads in flight), the eight sums over the warp by one butterfly
+    const int c = 2 * (int)blockIdx.x + half, wq = (threadIdx.x >> 5) & 3, n1 = s_cnt[half];
+    const float4 u4 = s_u[half][lane];
+    const float4 *seg = reinterpret_cast<const float4 *>(Dd + (size_t)c * N * kChunk) + lane;
+    const int slot8 = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);   // warp_sum8's layout
+    for (int n = wq; n < n1; n += 32) {
+        double v[8];
+        int id[8];
+#pragma unroll
+        for (int x = 0; x < 8; ++x) {
+            id[x] = n + 4 * x < n1 ? s_list[half][n + 4 * x] : -1;
+            float4 d4 = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (id[x] >= 0) d4 = __ldg(seg + (size_t)id[x] * (kChunk / 4));
+            v[x] = (double)((u4.x * d4.x + u4.y * d4.y) + (u4.z * d4.z + u4.w * d4.w));
+        }
+        const double r = warp_sum8(v, lane);
+        int mine = -1;
+#pragma unroll
+        for (int x = 0; x < 8; ++x)
+            if (x == slot8) mine = id[x];
+        if ((lane & 3) == 0 && mine >= 0 && r != 0.0)
+            atomicAdd(reinterpret_cast<unsigned long long *>(hr.hess) + (size_t)min(mine, k) * N + max(mine, k),
+                      (unsigned long long)__double2ll_rn(r * hr.hscale));
+    }
+    if (wq == 0) {   // the diagonal entry
+        const float4 d4 = s_d[half][lane];
+        double dg = (double)((u4.x * d4.x + u4.y * d4.y) + (u4.z * d4.z + u4.w * d4.w));
+#pragma unroll
+        for (int o = 16; o; o >>= 1) dg += __shfl_xor_sync(kFull, dg, o);
+        if (lane == 0 && dg != 0.0)
+            atomicAdd(reinterpret_cast<unsigned long long *>(hr.hess) + (size_t)k * N + k, (unsigned long long)__double2ll_rn(dg * hr.hscale));
     }
 }
 
@@ -263,6 +337,7 @@ struct MasterArgs {
     long long *hess;            // N x N (upper triangle used): H_F in fixed point, scale hscale
     float *omref;               // Sp: the omega H_F was built with
     uint8_t *hvalid;            // N: the column of beam k is in H_F
+    int *hlive;                 // H_F is built: set by every k_newton launch, cleared when the matrix is reset
     double hscale, hinv;
     float *wn;                  // second buffer of w (the trial points write z, w to a.zn, a.wn)
     Mail *mail;                 // message of the solving block, followed by N floats
@@ -1633,7 +1708,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
 // coefficients) published by a release store of a monotone epoch counter the workers spin on, and a monotone arrival
 // counter the solver spins on; no grid-wide barrier.  Both counters run on from launch to launch (bases in a.sync).
 #ifdef VMAT_NEWTON_TRACE
-__device__ unsigned long long g_tr[4][4096];   // per pass: published, last block saw it, last block arrived, solver saw the arrivals
+__device__ unsigned long long g_tr[8][4096];   // per pass: published, last block saw it, last block arrived, solver saw the arrivals
 __device__ unsigned int g_trn;
 __device__ long long g_seg[8];
 __device__ __forceinline__ unsigned long long gtime() {
@@ -1854,37 +1929,40 @@ __device__ __forceinline__ void newton_pass(const MasterArgs &a, const Smem &sm,
 // ---- the solving block ---------------------------------------------------------------------------------
 constexpr int kSolveRed = 8;   // values per warp row of the solver's reduction scratch
 
-// sums s[0..MS) and one maximum over the block, every thread receives them; fixed order
+// sums s[0..MS) and one maximum over the block, every thread receives them; fixed order.  Only the first nv <= 8
+// warps hold data (one beam per thread); the others skip the first level.
 template <int MS>
-__device__ __forceinline__ void solver_reduce(double (&s)[MS], double &mx, double *buf, int &tog) {
+__device__ __forceinline__ void solver_reduce(double (&s)[MS], double &mx, double *buf, int &tog, int nv) {
     static_assert(MS < kSolveRed, "scratch row too short");
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-#pragma unroll
-    for (int o = 16; o; o >>= 1) {
-#pragma unroll
-        for (int m = 0; m < MS; ++m) s[m] += __shfl_xor_sync(kFull, s[m], o);
-        mx = fmax(mx, __shfl_xor_sync(kFull, mx, o));
-    }
     double *b = buf + tog * (kMasterWarps * kSolveRed);
     tog ^= 1;
-    if (lane == 0) {
+    if (warp < nv) {
 #pragma unroll
-        for (int m = 0; m < MS; ++m) b[warp * kSolveRed + m] = s[m];
-        b[warp * kSolveRed + kSolveRed - 1] = mx;
+        for (int o = 16; o; o >>= 1) {
+#pragma unroll
+            for (int m = 0; m < MS; ++m) s[m] += __shfl_xor_sync(kFull, s[m], o);
+            mx = fmax(mx, __shfl_xor_sync(kFull, mx, o));
+        }
+        if (lane == 0) {
+#pragma unroll
+            for (int m = 0; m < MS; ++m) b[warp * kSolveRed + m] = s[m];
+            b[warp * kSolveRed + kSolveRed - 1] = mx;
+        }
     }
     __syncthreads();
-    // every warp adds the kMasterWarps rows by a butterfly over 16 lanes (both half-warps hold the same values)
-    const int row = lane & (kMasterWarps - 1);
+    const int row = lane & 7;   // every group of eight lanes reads the (at most) eight rows
+    const bool in = row < nv;
 #pragma unroll
     for (int m = 0; m < MS; ++m) {
-        double v = b[row * kSolveRed + m];
+        double v = in ? b[row * kSolveRed + m] : 0.0;
 #pragma unroll
-        for (int o = kMasterWarps / 2; o; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
+        for (int o = 4; o; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
         s[m] = v;
     }
-    double v = b[row * kSolveRed + kSolveRed - 1];
+    double v = in ? b[row * kSolveRed + kSolveRed - 1] : -CUDART_INF;
 #pragma unroll
-    for (int o = kMasterWarps / 2; o; o >>= 1) v = fmax(v, __shfl_xor_sync(kFull, v, o));
+    for (int o = 4; o; o >>= 1) v = fmax(v, __shfl_xor_sync(kFull, v, o));
     mx = v;
 }
 
@@ -1987,8 +2065,9 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
         linf[k] = lf;
     }
     int tog = 0;
+    const int nvs = (N + 31) / 32;   // warps that hold beams (one per thread)
     double none[1] = {0.0};
-    solver_reduce<1>(none, l1l, redb, tog);   // its barrier also publishes sk, ik, vy, rdt, linf
+    solver_reduce<1>(none, l1l, redb, tog, nvs);   // its barrier also publishes sk, ik, vy, rdt, linf
     const double l1max = l1l;
     const int K = sK;
     const int Kp4 = ((K + 3) / 4) | 1, Kp = 4 * Kp4;
@@ -2014,7 +2093,7 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
             dGb[k] = 2.0 * (e0 - e1);
             s[1] += fabs(v[k]) * linf[k];
         }
-        solver_reduce<2>(s, mx, redb, tog);
+        solver_reduce<2>(s, mx, redb, tog, nvs);
         G = s[0];
         zb = s[1];
     };
@@ -2065,15 +2144,29 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
     // ---- the incoming point -----------------------------------------------------------------------------
     double F = 0.0, Gs = 0.0, Phi = 0.0, zb = 0.0, pgmax = 0.0, pg_entry = 0.0, tol = 0.0, Phi0 = 0.0;
     smooth_of(vy, Gs, zb);
-    int state = send(kRunTrial, 0, vy, zb);
+    // Warm entry (inside vmat_solve): the solve before this one left z, w, F and d_k . w of its beams current, the one
+    // beam the leaf search has occupied since enters at y = 0 (so the dose has not moved) with the price the search formed
+    // as its gradient, and k_column_finish has entered its column into H_F: no pass is needed before the first step.
+    const bool warm = a.warm && a.lb == 0.0 && a.gflag[0] == 1 && a.sel->beam >= 0 && a.hvalid[a.sel->beam];
+    int state = kRunTrial;
+    if (warm) {
+        const int knew = a.sel->beam;
+        const double pnew = a.sel->price;
+        for (int k = tid; k < N; k += kMasterThreads)
+            vg[k] = ik[k] < 0 ? 0.0 : (k == knew ? pnew : a.gsave[k] + a.gamma * dGb[k]);
+        F = a.cost3[0];
+        __syncthreads();
+    } else {
+        state = send(kRunTrial, 0, vy, zb);
+        if (state != kFinish) receive(F, vg);
+    }
     if (state != kFinish) {
-        receive(F, vg);
         Phi = F + a.gamma * Gs;
         Phi0 = Phi;
         double pgl = 0.0;
         for (int k = tid; k < N; k += kMasterThreads)
             if (ik[k] >= 0 && !at_bound(vy[k], vg[k])) pgl = fmax(pgl, fabs(vg[k]));
-        solver_reduce<1>(none, pgl, redb, tog);
+        solver_reduce<1>(none, pgl, redb, tog, nvs);
         pgmax = pg_entry = pgl;
         tol = a.eps * fmax(1.0, pgmax);
         if (a.max_inner <= 0 && pgmax > tol) stop = 1;
@@ -2133,47 +2226,49 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
         const long long c1 = clock64();
         clk_load += c1 - c0;
         // Conjugate gradients on the faces of the box for the quadratic model at (vy, vg): one beam per thread (the
-        // first nv warps), two threads per row of the matrix (all warps); two sums over the beams and two block barriers
-        // per step.  Step lengths and the ratios to the bounds are formed in fp32: the iteration corrects itself (the
-        // residual is updated with the step actually taken) and a beam that reaches its bound is set on it explicitly.
+        // first nv warps), all warps on the product with the matrix.  One sum over the beams per step: with the
+        // residual r, the preconditioner M, the direction d and H d at hand, A = sum M r^2, B = sum M r (H d) and
+        // C = sum M (H d)^2 over the face give the Polak-Ribiere numerator of the NEXT residual r + t H d without a
+        // second sum, (r+ - r) M r+ = t (B + t C), and its denominator is A.  Whether the face changed, whether any
+        // entry of the new projected residual is still above the tolerance and whether to give up travel as three bits
+        // OR-ed into a shared word.  Step lengths, the sums and the ratios to the bounds are fp32: the iteration
+        // corrects itself (the residual is updated with the step actually taken) and a beam that reaches its bound is
+        // set on it explicitly.
         const double qtol = fmax(0.5 * tol, 0.05 * pgmax);
         const int k = tid;                                   // this thread's beam (k < N: checked on the host)
         const bool mine = k < N && ik[k] >= 0;
         const int nv = (N + 31) / 32;                        // warps that hold beams
         auto ratio = [](double num, double den) { return (double)__fdividef((float)num, (float)den); };
+        __shared__ int s_fl[2];
+        int tf = 0, togc = 0;
+        auto any_flags = [&](int bits) {                     // OR of the bits over the block; one barrier
+            const int wb = __reduce_or_sync(kFull, bits);
+            if (lane == 0 && wb) atomicOr(&s_fl[tf], wb);
+            __syncthreads();
+            const int r = s_fl[tf];
+            tf ^= 1;
+            if (tid == 0) s_fl[tf] = 0;                      // the word of the next call; nobody touches it before another barrier
+            return r;
+        };
+        if (tid < 2) s_fl[tid] = 0;
+        __syncthreads();
         // state of this thread's beam
-        double yk = mine ? vy[k] : 0.0, rk = mine ? vg[k] : 0.0, dk = 0.0, pok = 0.0;
+        double yk = mine ? vy[k] : 0.0, rk = mine ? vg[k] : 0.0, beta = 0.0;
         const double mk = mine ? Minv[k] : 1.0;
-        int fo = 0;
-        float rzold = 0.f;
-        double beta = 0.0;
-        bool restart = true, halt = false;
-        const int maxcg = 4 * K + 20;
-        int it = 0, togc = 0;
-        // first half of a step: projected residual, its sums
         int fr = mine && !at_bound(yk, rk);
-        double prk = fr ? rk : 0.0, zrk = mk * prk;
-        for (;;) {
+        double prk = fr ? rk : 0.0, dk = -mk * prk;
+        bool halt = false;
+        const int maxcg = 4 * K + 20;
+        int it = 0;
+        int fl = any_flags(fabs(prk) > qtol ? 2 : 0);
+        while ((fl & 2) && !(fl & 4) && it < maxcg) {
             TR(long long q0 = clock64();)
-            float s[2] = {(float)(zrk * prk), (float)(zrk * pok)};
-            float none_f = 0.f;
-            int fl = (fr != fo ? 1 : 0) | (fabs(prk) > qtol ? 2 : 0) | (halt ? 4 : 0);
-            cg_reduce<2>(s, none_f, fl, cgb, togc, nv);
-            TR(if (tid == 0) g_seg[0] += clock64() - q0; q0 = clock64();)
-            const int chg = fl & 1, big = fl & 2;
-            if (!big || (fl & 4) || it >= maxcg) break;   // (only the warps that hold beams know `halt`: it travels as a flag)
-            beta = (restart || chg || !(rzold > 0.f)) ? 0.0 : (double)fmaxf(0.f, __fdividef(s[0] - s[1], rzold));
-            restart = false;
-            rzold = s[0];
-            dk = fr ? -zrk + beta * dk : 0.0;
-            pok = prk;
-            fo = fr;
             if (k < N) vd[k] = dk;
             if (mine) dc[ik[k]] = (float)dk;
             __syncthreads();
             ++cg_steps;
             ++it;
-            TR(if (tid == 0) g_seg[1] += clock64() - q0; q0 = clock64();)
+            TR(if (tid == 0) g_seg[0] += clock64() - q0; q0 = clock64();)
             // H32 d, fp32.  The matrix is symmetric: thread (r, h) sums H[c][r] d_c over the columns c of its half h, so
             // that the lanes of a warp read consecutive words of row c (no bank conflict, 128 bytes per request) and
             // d_c is the same word for the whole warp.  Two halves: threads 0..255 and 256..511.
@@ -2198,31 +2293,42 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
                 if (h == 0 && r < K) hpart[r] = (acc0 + acc1) + hpart2[r];
             }
             __syncthreads();
-            TR(if (tid == 0) g_seg[2] += clock64() - q0; q0 = clock64();)
+            TR(if (tid == 0) g_seg[1] += clock64() - q0; q0 = clock64();)
             double hdk = 0.0;
-            float s2[2] = {0.f, 0.f}, ntl = -CUDART_INF_F;
+            float s5[5] = {0.f, 0.f, 0.f, 0.f, 0.f}, ntl = -CUDART_INF_F;
             if (mine) {
                 const double e1 = k + 1 < N ? (vd[k + 1] - dk) * rdt[k] : 0.0;
                 const double e0 = k > 0 ? (dk - vd[k - 1]) * rdt[k - 1] : 0.0;
                 hdk = 2.0 * (double)hpart[ik[k]] + 2.0 * a.gamma * (e0 - e1);
-                s2[0] = (float)(dk * hdk);
-                s2[1] = (float)(rk * dk);
+                s5[0] = (float)(dk * hdk);
+                s5[1] = (float)(rk * dk);
+                if (fr) {
+                    const double mr = mk * rk;
+                    s5[2] = (float)(mr * rk);
+                    s5[3] = (float)(mr * hdk);
+                    s5[4] = (float)(mk * hdk * hdk);
+                }
                 if (dk < 0.0) ntl = -(float)ratio(yk - lb, -dk);
                 if (has_ub && dk > 0.0) ntl = -(float)ratio(ub - yk, dk);
             }
             int nofl = 0;
-            cg_reduce<2>(s2, ntl, nofl, cgb, togc, nv);
+            TR(if (tid == 0) g_seg[2] += clock64() - q0; q0 = clock64();)
+            cg_reduce<5>(s5, ntl, nofl, cgb, togc, nv);
             TR(if (tid == 0) g_seg[3] += clock64() - q0; q0 = clock64();)
             const float tmaxf = -ntl;                            // fp32: the same bits wherever the ratio is formed
             const double tmax = (double)tmaxf;
-            if (!(s2[1] < 0.f)) {        // not a descent direction of the model: open steepest descent again, or give up
+            bool hit = false;
+            double t = 0.0;
+            if (warp >= nv) {            // no beams, and no sums either: this warp only follows the flags
+            } else if (!(s5[1] < 0.f)) { // not a descent direction of the model: open steepest descent again, or give up
                 if (beta == 0.0) halt = true;
-                restart = true;
             } else {
-                double t = s2[0] > 0.f ? (double)__fdividef(-s2[1], s2[0]) : tmax;
-                if (!(t < CUDART_INF)) halt = true;
-                else {
-                    const bool hit = t >= tmax;
+                t = s5[0] > 0.f ? (double)__fdividef(-s5[1], s5[0]) : tmax;
+                if (!(t < CUDART_INF)) {
+                    halt = true;
+                    t = 0.0;
+                } else {
+                    hit = t >= tmax;
                     if (hit) t = tmax;
                     if (mine) {
                         double v = yk + t * dk;
@@ -2233,10 +2339,15 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
                     }
                 }
             }
-            fr = mine && !at_bound(yk, rk);
-            prk = fr ? rk : 0.0;
-            zrk = mk * prk;
-            TR(if (tid == 0) g_seg[4] += clock64() - q0;)
+            const int fn = mine && !at_bound(yk, rk);
+            prk = fn ? rk : 0.0;
+            TR(if (tid == 0) g_seg[4] += clock64() - q0; q0 = clock64();)
+            fl = any_flags(warp >= nv ? 0 : (fn != fr || hit || t == 0.0 ? 1 : 0) | (fabs(prk) > qtol ? 2 : 0) | (halt ? 4 : 0));
+            // (only the warps that hold beams know the sums; `halt` and the rest of the loop control travel as flags)
+            beta = (fl & 1) || !(s5[2] > 0.f) ? 0.0 : (double)fmaxf(0.f, __fdividef((float)t * (s5[3] + (float)t * s5[4]), s5[2]));
+            dk = fn ? -mk * prk + beta * dk : 0.0;
+            fr = fn;
+            TR(if (tid == 0) g_seg[5] += clock64() - q0;)
         }
         if (k < N) yc[k] = yk;
         __syncthreads();
@@ -2249,7 +2360,7 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
             sl[0] = vg[tid] * pk;
             mxp = fabs(pk);
         }
-        solver_reduce<1>(sl, mxp, redb, tog);
+        solver_reduce<1>(sl, mxp, redb, tog, nvs);
         const double slope = sl[0];
         if (!(slope < 0.0) || !(mxp > 0.0)) {
             stop = 2;
@@ -2272,7 +2383,7 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
                 sn[0] = vgn[tid] * vp[tid];
                 if (ik[tid] >= 0 && !at_bound(vyn[tid], vgn[tid])) pgm = fabs(vgn[tid]);
             }
-            solver_reduce<1>(sn, pgm, redb, tog);
+            solver_reduce<1>(sn, pgm, redb, tog, nvs);
             const bool accepted = Phin <= Phi + c1a * t * slope ||
                                   (Phin <= Phi + noise * fabs(Phi) && fabs(sn[0]) <= 0.9 * fabs(slope));
             if (accepted) {
@@ -2304,16 +2415,23 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
     if (bad) stop = 5;
     if (s_timeout) stop = 6;
     if (state != kFinish) send(kFinish, 0, nullptr, 0.0);
-    // results
+    // results; d_k . w at the point the solve leaves, for the warm entry of the next one
+    const bool evaluated = npass > 0 && !bad && !s_timeout;   // z, w, F and vg belong to vy
+    {
+        double Gx, zbx;
+        smooth_of(vy, Gx, zbx);   // dG/dy at vy (the last point sent may have been a rejected trial)
+    }
     for (int k = tid; k < N; k += kMasterThreads) {
         a.y[k] = vy[k];
-        if (a.occ[k]) a.hvalid[k] = 1;   // every occupied beam is in the matrix now (the first pass saw to it)
+        if (a.occ[k] && npass > 0) a.hvalid[k] = 1;   // every occupied beam is in the matrix now (the first pass saw to it)
+        if (evaluated || warm) a.gsave[k] = ik[k] >= 0 ? vg[k] - a.gamma * dGb[k] : 0.0;
     }
     if (tid == 0) {
         a.phase[0] = ph % 3;
         a.sync[2] = epub;
         a.sync[3] = abase + (unsigned long long)a.nblk * npass;
-        a.gflag[0] = 0;
+        a.gflag[0] = (evaluated || warm) ? 1 : 0;
+        if (npass > 0) a.hlive[0] = 1;
         atomicAdd(a.mcount + 1, (unsigned long long)(ph - ph_entry));
         a.mcount[2] += (unsigned long long)cg_steps;
         a.mcount[3] += (unsigned long long)clk_cg;
@@ -2416,7 +2534,10 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_newton(const MasterArgs a
         ++ph;
         __syncthreads();
         const long long w1 = clock64();
+        TR(if (tid == 0) atomicMax(&g_tr[4][trp], gtime());)
         newton_pass(a, sm, K, Ku, ngroups, dst ? a.zn : a.z, dst ? a.wn : a.w, rec, scF, scG, su.red, fresh);
+        TR(if (tid == 0) atomicMax(&g_tr[5][trp], gtime());)
+        TR(if (tid == 0 && blockIdx.x == 0) g_tr[6][trp] = gtime();)
         wclk += clock64() - w1;
         if (fresh != -1) {
             __syncthreads();
@@ -2545,6 +2666,7 @@ int master_configure(vmat_plan *p) {
         if ((rc = dev_alloc(p, &p->hess, p->N * p->N))) return rc;
         if ((rc = dev_alloc(p, &p->omref, p->Sp))) return rc;
         if ((rc = dev_alloc(p, &p->hvalid, p->N))) return rc;
+        if ((rc = dev_alloc(p, &p->hlive, 1))) return rc;
         if ((rc = dev_alloc(p, &p->wn_s, p->Sp))) return rc;
         if ((rc = dev_alloc(p, (char **)&p->mail, (int64_t)sizeof(Mail) + 4 * p->N))) return rc;
         if ((rc = dev_alloc(p, &p->nsync, 4))) return rc;
@@ -2588,6 +2710,7 @@ int reset_hessian(vmat_plan *p) {
     VMAT_CUDA(p, cudaMemsetAsync(p->hess, 0, (size_t)p->N * p->N * 8, p->stream));
     VMAT_CUDA(p, cudaMemsetAsync(p->omref, 0, (size_t)p->Sp * 4, p->stream));
     VMAT_CUDA(p, cudaMemsetAsync(p->hvalid, 0, (size_t)p->N, p->stream));
+    VMAT_CUDA(p, cudaMemsetAsync(p->hlive, 0, 4, p->stream));
     return VMAT_OK;
 }
 
@@ -2596,9 +2719,16 @@ int launch_column_build(vmat_plan *p, int beam) {
     const unsigned blocks = (unsigned)((p->RC + 7) / 8);
     VMAT_CUDA(p, launch_pdl(k_column_scatter, dim3(blocks), dim3(256), p->stream, p->rowq, p->val4, p->col4, sel, beam, p->left,
                             p->right, (int)p->R, (int)p->C, p->fx_scale, p->acc, p->colstat, p->col_touch, p->touch_words));
+    HessRowArgs hr;
+    hr.hess = p->master_newton ? p->hess : nullptr;
+    hr.omref = p->omref;
+    hr.occ = p->occ;
+    hr.hvalid = p->hvalid;
+    hr.hlive = p->hlive;
+    hr.hscale = p->hscale;
     VMAT_CUDA(p, launch_pdl(k_column_finish, dim3((unsigned)((p->Sp + 255) / 256)), dim3(256), p->stream, p->acc,
                             (long long)p->Sp, sel, beam, p->fx_inv, p->Dd, (int)p->N, p->colstat, p->col_touch,
-                            p->touch_words));
+                            p->touch_words, hr));
     p->launches += 2;
     VMAT_CUDA(p, cudaGetLastError());
     return VMAT_OK;
@@ -2656,6 +2786,7 @@ static int launch_master_impl(vmat_plan *p, int max_inner, int trace_it, int war
     a.hess = p->hess;
     a.omref = p->omref;
     a.hvalid = p->hvalid;
+    a.hlive = p->hlive;
     a.hscale = p->hscale;
     a.hinv = p->hinv;
     a.wn = p->wn_s;
@@ -2678,16 +2809,16 @@ int launch_dose_grad(vmat_plan *p) { return launch_master_impl(p, 0, -1, 0); }
 
 #ifdef VMAT_NEWTON_TRACE
 extern "C" void vmat_debug_newton_trace(unsigned long long *out, unsigned int *n) {
-    cudaMemcpyFromSymbol(out, g_tr, sizeof(unsigned long long) * 4 * 4096);
+    cudaMemcpyFromSymbol(out, g_tr, sizeof(unsigned long long) * 8 * 4096);
     cudaMemcpyFromSymbol(n, g_trn, 4);
     long long seg[8];
     cudaMemcpyFromSymbol(seg, g_seg, sizeof(seg));
-    fprintf(stderr, "cg segments (clk, thread 0): R1 %lld d-update %lld matvec %lld R2 %lld update %lld | reduce: level1 %lld barrier %lld level2 %lld\n", seg[0], seg[1], seg[2], seg[3], seg[4], seg[5], seg[6], seg[7]);
+    fprintf(stderr, "cg segments (clk, thread 0): d-write+barrier %lld matvec %lld local sums %lld reduce %lld update %lld flags+beta %lld\n", seg[0], seg[1], seg[2], seg[3], seg[4], seg[5]);
     long long zs[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     cudaMemcpyToSymbol(g_seg, zs, sizeof(zs));
     unsigned int z = 0;
     cudaMemcpyToSymbol(g_trn, &z, 4);
-    static unsigned long long zeros[4 * 4096];
+    static unsigned long long zeros[8 * 4096];
     cudaMemcpyToSymbol(g_tr, zeros, sizeof(zeros));
 }
 #endif
