@@ -37,9 +37,11 @@ def load_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-# ncu --set full capture of k_price_spmv on configs[1] (profiles/r01j_price_spmv.md): dram__bytes_read.sum +
-# dram__bytes_write.sum of the first pricing launch of a plan (all 180 beams un-occupied; 994,678,664 algorithmic bytes)
+# A number cited from a committed capture, not measured by the run that prints it: `ncu --set full` of k_price_spmv on
+# configs[1], dram__bytes_read.sum + dram__bytes_write.sum of the FIRST pricing launch of a plan (all 180 beams
+# un-occupied; 994,678,664 algorithmic bytes).  The kernel and the layout of D have not changed since that capture.
 NCU_TRAFFIC_BYTES_FIRST_LAUNCH = {"prostate": 992094720 + 4436224}
+NCU_TRAFFIC_SOURCE = "profiles/r01j_price_spmv.md (ncu --set full, commit d77c9b3)"
 
 
 class ClockSampler:
@@ -100,8 +102,21 @@ def make_inputs(config: str, seed: int = 0):
     return ph, time.perf_counter() - t0
 
 
-def oracle_sample(ph, budget_s: float, chunk: int = 5):
-    """The oracle as it stands on the first iterations of the same workload, until `budget_s` of CPU work."""
+def oracle_sample(ph, budget_s: float, chunk: int = 5, threads: int = 0):
+    """The oracle as it stands on the first iterations of the same workload, until `budget_s` of CPU work (the whole
+    plan if the budget allows).  threads > 0: run it on that many OpenMP threads."""
+    from oracle import Oracle, vmat_oracle
+
+    all_threads = vmat_oracle.num_threads()
+    if threads > 0:
+        vmat_oracle.set_num_threads(threads)
+    try:
+        return _oracle_sample(ph, budget_s, chunk)
+    finally:
+        vmat_oracle.set_num_threads(all_threads)
+
+
+def _oracle_sample(ph, budget_s: float, chunk: int):
     from oracle import Oracle, vmat_oracle
 
     o = Oracle.from_phantom(ph)
@@ -268,12 +283,15 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="prostate", choices=["tiny", "prostate", "hn", "stress"])
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--cpu-budget-s", type=float, default=15.0, help="CPU seconds for the cpu_baseline sample")
+    ap.add_argument("--cpu-budget-s", type=float, default=150.0,
+                    help="cap on the CPU seconds of the cpu_baseline leg (the oracle's whole plan if it fits)")
+    ap.add_argument("--cpu-single-thread-s", type=float, default=10.0,
+                    help="CPU seconds of the single-thread prefix of the cpu_baseline leg (0: skip)")
     ap.add_argument("--ref-budget-s", type=float, default=15.0, help="CPU seconds per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--master-mode", type=int, default=None, choices=[0, 1],
-                    help="inner iteration of the master kernel (vmat_options.master_mode); default: the library's")
+                    help="vmat_options.master_mode: 0 conjugate directions, 1 Newton on the reduced problem (the library's default)")
     ap.add_argument("--sweep", action="store_true", help="configs[3]: isolated pricing / search kernel sweep")
     ap.add_argument("--sweep-nnz", default="5e7,1e8,2.5e8,5e8,1e9")
     ap.add_argument("--sweep-voxels", default="1048576,2097152,4194304")
@@ -366,7 +384,8 @@ def main():
     plan.solve(iters, trace=False)
     ph_us = {"price": 0.0, "search": 0.0, "column": 0.0, "master": 0.0, "total": 0.0}
     inner_total = 0
-    m_passes = m_bytes = 0.0
+    m_passes = m_bytes = m_cg = 0.0
+    m_clk = [0.0, 0.0, 0.0]
     for _ in range(args.steps):
         plan.set_plan(*empty)
         st = plan.solve(iters, trace=True)
@@ -376,6 +395,9 @@ def main():
         inner_total += int(st.inner.sum())
         m_passes += st.master_passes / args.steps
         m_bytes += st.master_bytes / args.steps
+        m_cg += st.master_cg_steps / args.steps
+        for i, v in enumerate((st.master_clk_cg, st.master_clk_wait, st.master_clk_load)):
+            m_clk[i] += v / args.steps
     # ---- steps (a)+(b) on the finished plan, both layouts (north_star: "chosen by measurement") -------------
     occ_f, left_f, right_f, _ = plan.get_plan()
     nnz_open = 0
@@ -408,7 +430,9 @@ def main():
         "bound": "hbm", "achieved": achieved, "peak": peak,
         "unit": "GB/s", "frac": achieved / peak, "frac_of_8TBs_nominal": achieved / 8000.0,
         "traffic": NCU_TRAFFIC_BYTES_FIRST_LAUNCH.get(c.name),
-        "traffic_note": "ncu dram bytes of the FIRST launch of a plan (compare algorithmic_bytes_first_launch)",
+        "traffic_source": NCU_TRAFFIC_SOURCE if c.name in NCU_TRAFFIC_BYTES_FIRST_LAUNCH else None,
+        "traffic_note": "cited from that capture, not measured by this run: ncu dram bytes of the FIRST launch of a "
+                        "plan (compare algorithmic_bytes_first_launch)",
         "peak_source": peak_src,
         "algorithmic_bytes_per_launch_avg": sum(alg) / iters, "algorithmic_bytes_first_launch": alg[0],
         "avg_launch_us": ph_us["price"] / iters, "launches_per_step": iters,
@@ -418,13 +442,23 @@ def main():
     # segments of the aperture-dose columns x the passes that multiplied them (counted on the device); on
     # configs[1] those segments sit in shared memory, so this is an effective rate, not DRAM traffic
     m_gbs = m_bytes / (ph_us["master"] * 1e-6) / 1e9 if ph_us["master"] > 0 else 0.0
+    newton = m_cg > 0
     roofline_master = {
-        "kernel": "k_master (master solve, steps a+b+e)", "bound": "hbm", "achieved": m_gbs, "peak": peak, "unit": "GB/s",
+        "kernel": ("k_newton" if newton else "k_master") + " (master solve, steps a+b+e)", "bound": "hbm",
+        "achieved": m_gbs, "peak": peak, "unit": "GB/s",
         "frac": m_gbs / peak, "traffic": None, "algorithmic_bytes_per_step": m_bytes, "passes_per_step": m_passes,
         "us_per_pass": ph_us["master"] / m_passes if m_passes else None, "launches_per_step": iters,
-        "note": "latency bound: two grid barriers and two control steps per inner iteration "
-                "(profiles/r01d_master.md); bytes = touched column segments x passes, device-counted",
+        "note": ("latency bound: a solve is two or three passes over the touched column segments, each followed by "
+                 "conjugate-gradient steps on the K x K reduced problem in one block (DESIGN.md section 7); "
+                 if newton else
+                 "latency bound: two grid barriers and two control steps per inner iteration; ") +
+                "bytes = touched column segments x passes, device-counted",
     }
+    if newton:
+        clk_us = (clocks or {}).get("sm_mhz") or 1965.0
+        roofline_master.update({"cg_steps_per_step": m_cg, "cg_us_per_step": m_clk[0] / clk_us,
+                                "waiting_for_passes_us_per_step": m_clk[1] / clk_us,
+                                "loading_hessian_us_per_step": m_clk[2] / clk_us})
     phases = {k + "_us_per_step": v for k, v in ph_us.items()}
     phases["master_inner_iterations_per_step"] = inner_total / args.steps
     info = {"nnz": plan.nnz, "nnz_padded": plan.nnz_padded, "support_voxels": plan.n_support,
@@ -463,10 +497,17 @@ def main():
 
     cpu_baseline = None
     if not args.no_cpu_baseline and world == 1:
-        it, t, cores, _ = oracle_sample(ph, args.cpu_budget_s)
-        cpu_baseline = {"value": it / t, "unit": UNIT, "cores": cores, "kind": "oracle",
-                        "sample": f"first {it} of {c.n_beams} column-generation iterations of the same phantom "
-                                  f"({t:.1f} s), oracle/vmat_oracle.c as it stands (fp64, OpenMP)"}
+        it, t, cores, ocost = oracle_sample(ph, args.cpu_budget_s)
+        whole = it >= c.n_beams
+        cpu_baseline = {"value": it / t, "unit": UNIT, "cores": cores, "kind": "oracle", "nproc": os.cpu_count(),
+                        "sample": (f"the whole plan, {it} column-generation iterations" if whole else
+                                   f"first {it} of {c.n_beams} column-generation iterations") +
+                                  f" of the same phantom ({t:.1f} s), oracle/vmat_oracle.c as it stands (fp64, OpenMP)",
+                        "iterations": it, "seconds": t, "whole_plan": whole, "final_cost": ocost}
+        if args.cpu_single_thread_s > 0:
+            it1, t1, _, _ = oracle_sample(ph, args.cpu_single_thread_s, chunk=2, threads=1)
+            cpu_baseline["single_thread"] = {"value": it1 / t1, "unit": UNIT, "cores": 1,
+                                             "sample": f"first {it1} iterations on one thread ({t1:.1f} s)"}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,

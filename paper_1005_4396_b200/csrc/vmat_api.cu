@@ -2,8 +2,6 @@
 // life-cycle, and the order in which the kernels of the other translation units are enqueued.
 // No arithmetic of the method lives here.
 #include <cmath>
-#include <cstdio>
-#include <cstdlib>
 #include <cstring>
 #include <mutex>
 #include <new>
@@ -590,7 +588,6 @@ int vmat_solve(vmat_plan *p, int32_t max_iters, vmat_solve_stats *out) {
         out->cost = c3[2];
         unsigned long long mc[16];
         TRYC(cudaMemcpy(mc, p->mcount, sizeof(mc), cudaMemcpyDeviceToHost));
-        if (getenv("VMAT_DEBUG_CLK")) fprintf(stderr, "worker pass clk: block0 %llu  max-over-solves-of-block-total %llu  mean %llu\n", mc[6], mc[7], mc[8] / 147);
         out->master_passes = (double)mc[1];
         out->master_bytes = (double)mc[0] * (double)(kChunk * 4);
         out->master_cg_steps = (double)mc[2];

@@ -25,7 +25,6 @@
 #include <math_constants.h>
 
 #include <climits>
-#include <cstdio>
 #include <cmath>
 
 #include "vmat_internal.cuh"
@@ -1707,19 +1706,6 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
 // Hand-over between the solving block and the working blocks: a message in global memory (struct Mail + the
 // coefficients) published by a release store of a monotone epoch counter the workers spin on, and a monotone arrival
 // counter the solver spins on; no grid-wide barrier.  Both counters run on from launch to launch (bases in a.sync).
-#ifdef VMAT_NEWTON_TRACE
-__device__ unsigned long long g_tr[8][4096];   // per pass: published, last block saw it, last block arrived, solver saw the arrivals
-__device__ unsigned int g_trn;
-__device__ long long g_seg[8];
-__device__ __forceinline__ unsigned long long gtime() {
-    unsigned long long t;
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-    return t;
-}
-#define TR(stmt) stmt
-#else
-#define TR(stmt)
-#endif
 struct Mail {
     double scF, scG;   // fixed-point scales of the pass to run
     int state;         // kRunTrial: evaluate at the coefficients that follow; kFinish: stop
@@ -2117,7 +2103,6 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
         ++epub;
         if (tid == 0) {
             __threadfence();
-            TR(if (state != kFinish) g_tr[0][(g_trn + npass) & 4095] = gtime();)
             st_release_u64(a.sync + 1, epub);
         }
         return state;
@@ -2127,7 +2112,6 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
         ++npass;
         const long long c0 = clock64();
         if (tid == 0 && !spin_until(a.sync, abase + (unsigned long long)a.nblk * npass)) *timed_out = 1;
-        TR(if (tid == 0) g_tr[3][(g_trn + npass - 1) & 4095] = gtime();)
         __syncthreads();
         clk_wait += clock64() - c0;
         const long long *rec = a.accbuf + (size_t)(ph % 3) * kSumGroups * recn;
@@ -2262,13 +2246,11 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
         int it = 0;
         int fl = any_flags(fabs(prk) > qtol ? 2 : 0);
         while ((fl & 2) && !(fl & 4) && it < maxcg) {
-            TR(long long q0 = clock64();)
             if (k < N) vd[k] = dk;
             if (mine) dc[ik[k]] = (float)dk;
             __syncthreads();
             ++cg_steps;
             ++it;
-            TR(if (tid == 0) g_seg[0] += clock64() - q0; q0 = clock64();)
             // H32 d, fp32.  The matrix is symmetric: thread (r, h) sums H[c][r] d_c over the columns c of its half h, so
             // that the lanes of a warp read consecutive words of row c (no bank conflict, 128 bytes per request) and
             // d_c is the same word for the whole warp.  Two halves: threads 0..255 and 256..511.
@@ -2293,7 +2275,6 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
                 if (h == 0 && r < K) hpart[r] = (acc0 + acc1) + hpart2[r];
             }
             __syncthreads();
-            TR(if (tid == 0) g_seg[1] += clock64() - q0; q0 = clock64();)
             double hdk = 0.0;
             float s5[5] = {0.f, 0.f, 0.f, 0.f, 0.f}, ntl = -CUDART_INF_F;
             if (mine) {
@@ -2312,9 +2293,7 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
                 if (has_ub && dk > 0.0) ntl = -(float)ratio(ub - yk, dk);
             }
             int nofl = 0;
-            TR(if (tid == 0) g_seg[2] += clock64() - q0; q0 = clock64();)
             cg_reduce<5>(s5, ntl, nofl, cgb, togc, nv);
-            TR(if (tid == 0) g_seg[3] += clock64() - q0; q0 = clock64();)
             const float tmaxf = -ntl;                            // fp32: the same bits wherever the ratio is formed
             const double tmax = (double)tmaxf;
             bool hit = false;
@@ -2341,13 +2320,11 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
             }
             const int fn = mine && !at_bound(yk, rk);
             prk = fn ? rk : 0.0;
-            TR(if (tid == 0) g_seg[4] += clock64() - q0; q0 = clock64();)
             fl = any_flags(warp >= nv ? 0 : (fn != fr || hit || t == 0.0 ? 1 : 0) | (fabs(prk) > qtol ? 2 : 0) | (halt ? 4 : 0));
             // (only the warps that hold beams know the sums; `halt` and the rest of the loop control travel as flags)
             beta = (fl & 1) || !(s5[2] > 0.f) ? 0.0 : (double)fmaxf(0.f, __fdividef((float)t * (s5[3] + (float)t * s5[4]), s5[2]));
             dk = fn ? -mk * prk + beta * dk : 0.0;
             fr = fn;
-            TR(if (tid == 0) g_seg[5] += clock64() - q0;)
         }
         if (k < N) yc[k] = yk;
         __syncthreads();
@@ -2437,7 +2414,6 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
         a.mcount[3] += (unsigned long long)clk_cg;
         a.mcount[4] += (unsigned long long)clk_wait;
         a.mcount[5] += (unsigned long long)clk_load;
-        TR(g_trn += (unsigned)npass;)
         MasterOut o;
         o.inner = inner;
         o.backtracks = backtracks;
@@ -2507,13 +2483,10 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_newton(const MasterArgs a
     const float *mcoef = reinterpret_cast<const float *>(mail + 1);
     unsigned long long e = ebase;
     int cur = 0;
-    long long wclk = 0;
     for (;;) {
         ++e;
         __shared__ int s_gone;
         if (tid == 0) s_gone = !spin_until(a.sync + 1, e);
-        TR(const unsigned trp = (g_trn + (unsigned)(e - ebase - 1)) & 4095;)
-        TR(if (tid == 0) atomicMax(&g_tr[1][trp], gtime());)
         __syncthreads();
         // the whole message in one round trip to L2: header and this thread's coefficient are loaded before any is used
         const int mstate = __ldcg(&mail->state), dst = __ldcg(&mail->dst), mcur = __ldcg(&mail->cur);
@@ -2533,12 +2506,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_newton(const MasterArgs a
         long long *rec = a.accbuf + (size_t)(ph % 3) * kSumGroups * recn;
         ++ph;
         __syncthreads();
-        const long long w1 = clock64();
-        TR(if (tid == 0) atomicMax(&g_tr[4][trp], gtime());)
         newton_pass(a, sm, K, Ku, ngroups, dst ? a.zn : a.z, dst ? a.wn : a.w, rec, scF, scG, su.red, fresh);
-        TR(if (tid == 0) atomicMax(&g_tr[5][trp], gtime());)
-        TR(if (tid == 0 && blockIdx.x == 0) g_tr[6][trp] = gtime();)
-        wclk += clock64() - w1;
         if (fresh != -1) {
             __syncthreads();
             for (int i = tid; i < K; i += kMasterThreads) sm.hv[i] = 1;
@@ -2547,7 +2515,6 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_newton(const MasterArgs a
         __syncthreads();
         if (tid == 0) {
             __threadfence();
-            TR(atomicMax(&g_tr[2][trp], gtime());)
             atomicAdd(a.sync, 1ull);
         }
     }
@@ -2564,11 +2531,6 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_newton(const MasterArgs a
             }
     }
     if (tid == 0) atomicAdd(a.mcount, (unsigned long long)su.segs * (unsigned long long)(ph - ph_entry));
-    if (tid == 0) {
-        atomicMax(a.mcount + 7, (unsigned long long)wclk);
-        if (blockIdx.x == 0) a.mcount[6] += (unsigned long long)wclk;
-        atomicAdd(a.mcount + 8, (unsigned long long)wclk);
-    }
 }
 
 // shared memory of one master block (master_setup's carve-up); k_newton's working blocks lay out a little more
@@ -2806,22 +2768,6 @@ int launch_master(vmat_plan *p, int trace_it, int warm) {
 
 // steps (a)+(b) alone: the master kernel's evaluation pass with no iteration allowed
 int launch_dose_grad(vmat_plan *p) { return launch_master_impl(p, 0, -1, 0); }
-
-#ifdef VMAT_NEWTON_TRACE
-extern "C" void vmat_debug_newton_trace(unsigned long long *out, unsigned int *n) {
-    cudaMemcpyFromSymbol(out, g_tr, sizeof(unsigned long long) * 8 * 4096);
-    cudaMemcpyFromSymbol(n, g_trn, 4);
-    long long seg[8];
-    cudaMemcpyFromSymbol(seg, g_seg, sizeof(seg));
-    fprintf(stderr, "cg segments (clk, thread 0): d-write+barrier %lld matvec %lld local sums %lld reduce %lld update %lld flags+beta %lld\n", seg[0], seg[1], seg[2], seg[3], seg[4], seg[5]);
-    long long zs[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-    cudaMemcpyToSymbol(g_seg, zs, sizeof(zs));
-    unsigned int z = 0;
-    cudaMemcpyToSymbol(g_trn, &z, 4);
-    static unsigned long long zeros[8 * 4096];
-    cudaMemcpyToSymbol(g_tr, zeros, sizeof(zeros));
-}
-#endif
 
 int launch_rate_ratio(vmat_plan *p, double rho, double *ratio_dev) {
     k_rate_ratio<<<1, 256, 0, p->stream>>>(p->occ, p->y, p->theta, (int)p->N, rho, ratio_dev);
