@@ -79,8 +79,12 @@ typedef struct {
 /* Tunables.  Zero-initialise, then call vmat_default_options. */
 typedef struct {
     int32_t validate;          /* 1: check the CSR and the voxel arrays on the device (default 1) */
-    int32_t d_format;          /* device storage of D: 0 = fp32 value + 32-bit voxel slot per entry (8 bytes,
-                                  the fp32-CSR layout of BASELINE.json north_star, default)          */
+    int32_t d_format;          /* device storage of D for the pricing product: 0 = fp32 value + 32-bit voxel slot per
+                                  entry (8 bytes: the fp32-CSR layout of BASELINE.json north_star, default);
+                                  1 = a second copy in aligned slot pairs with 16-bit pair ids (about 6 bytes per
+                                  entry and 0.6 gathers of the gradient per entry, a separate
+                                  format: same fp32 values, same products, the sums in another order).  Costs
+                                  about 0.8 x the memory of D on top.                                    */
     int32_t dose_path;         /* how vmat_dose forms z: 0 from the aperture-dose columns d_k the
                                   master keeps (default), 1 straight from D (fixed-point atomics)  */
     double  master_eps;        /* stop when max|projected gradient| <= eps*max(1, value at entry) */
@@ -156,6 +160,7 @@ typedef struct {
     int64_t nnz_padded;     /* entries of the device layout (rows padded to multiples of 4)     */
     int64_t n_support;      /* voxels with a non-empty column of D                              */
     int64_t device_bytes;   /* device memory owned by the plan                                  */
+    int64_t pricing_bytes;  /* bytes of D (values, indices, row starts) a pricing product over all rows streams */
 } vmat_info;
 
 void vmat_default_options(vmat_options *opt);

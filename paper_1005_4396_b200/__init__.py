@@ -78,7 +78,7 @@ class _RateStats(C.Structure):
 
 class _Info(C.Structure):
     _fields_ = [(n, C.c_int64) for n in ("n_voxels", "n_beams", "n_rows", "n_cols", "n_beamlets", "nnz",
-                                         "nnz_padded", "n_support", "device_bytes")]
+                                         "nnz_padded", "n_support", "device_bytes", "pricing_bytes")]
 
 
 class VmatError(RuntimeError):
@@ -218,6 +218,7 @@ class Plan:
         self.V, self.N, self.R, self.Cc, self.B = info.n_voxels, info.n_beams, info.n_rows, info.n_cols, info.n_beamlets
         self.nnz, self.nnz_padded, self.n_support, self.device_bytes = (info.nnz, info.nnz_padded, info.n_support,
                                                                         info.device_bytes)
+        self.pricing_bytes = info.pricing_bytes
 
     # -- life cycle ----------------------------------------------------------------------------
     @classmethod

@@ -182,7 +182,7 @@ int vmat_create(const vmat_problem *pb, const vmat_options *options, void *cuda_
     if (!(p->opt.master_stall_rel >= 0.0)) p->opt.master_stall_rel = 1e-6;
     if (p->opt.master_stall_count < 1) p->opt.master_stall_count = 2;
     if (p->opt.master_mode != 1) p->opt.master_mode = 0;
-    if (p->opt.d_format != 0) return bail(fail(p, VMAT_EINVAL, "d_format must be 0"));
+    if (p->opt.d_format != 0 && p->opt.d_format != 1) return bail(fail(p, VMAT_EINVAL, "d_format must be 0 or 1"));
     p->V = pb->n_voxels;
     p->N = pb->n_beams;
     p->R = pb->n_rows;
@@ -206,6 +206,7 @@ int vmat_create(const vmat_problem *pb, const vmat_options *options, void *cuda_
 
     int rc = build_layout(p, pb);
     if (rc) return bail(rc);
+    if (p->opt.d_format == 1 && (rc = build_pairs(p))) return bail(rc);
 
     const int64_t N = p->N, NR = p->N * p->R, Sp = p->Sp;
 #define A(ptr, n) \
@@ -307,6 +308,7 @@ int vmat_get_info(const vmat_plan *p, vmat_info *out) {
     out->nnz_padded = p->nq * 4;
     out->n_support = p->S;
     out->device_bytes = p->bytes;
+    out->pricing_bytes = p->opt.d_format == 1 ? p->pr_groups * 41 + (p->B + 1) * 4 : p->nq * 32 + (p->B + 1) * 4;
     return VMAT_OK;
 }
 

@@ -56,6 +56,13 @@ struct vmat_plan {
     float4 *val4 = nullptr;     // nq
     int4 *col4 = nullptr;       // nq, slot ids
 
+    // ---- d_format 1: second copy of D for the pricing product, aligned slot pairs with 16-bit ids (vmat_layout.cu) ----
+    uint32_t *pr_rowo = nullptr;    // B+1 row starts in groups (four units = up to eight entries)
+    float4 *pr_va = nullptr, *pr_vb = nullptr;   // values of units 0-1 / 2-3 of every group
+    uint2 *pr_ix = nullptr;         // four 16-bit pair ids per group, relative to its panel of 65536 pairs
+    uint8_t *pr_pan = nullptr;      // panel of every group
+    int64_t pr_groups = 0;
+
     // ---- voxel data --------------------------------------------------------------------
     float *T_V = nullptr, *alpha_V = nullptr, *beta_V = nullptr;   // V each
     int32_t *slot_of = nullptr;    // V, -1 outside the support
@@ -193,6 +200,7 @@ __device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.lau
 
 // vmat_layout.cu: validation and the device layout of D ------------------------------------------
 int build_layout(vmat_plan *p, const vmat_problem *pb);
+int build_pairs(vmat_plan *p);
 
 // vmat_price.cu ---------------------------------------------------------------------------------------
 int launch_price_spmv(vmat_plan *p, const float *w_s, float *g, int n_free);

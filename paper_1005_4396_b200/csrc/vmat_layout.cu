@@ -207,6 +207,148 @@ cudaError_t exclusive_scan(const T *in, T *out, int64_t n, T *tile_sums, cudaStr
     return cudaGetLastError();
 }
 
+
+// ---- d_format 1: a second copy of D for the pricing product in aligned slot PAIRS with 16-bit ids ---------------
+// The slot ids of a row of D come in runs of consecutive slots (a beamlet's lateral support along a voxel row): a
+// UNIT is the aligned pair of slots (2m, 2m+1) with the row's two values there (0 where the row has no entry), so one
+// 8-byte gather of w serves up to two entries (0.62 / 0.57 units per entry on configs[1] / [2]).  The pair ids are
+// cut into panels of 65536 pairs; a row's units fall into one run per panel, padded to whole GROUPS of four units
+// (values 0, the run's last id repeated).  A group carries two float4 of values (arrays va, vb: units 0-1 and 2-3),
+// four 16-bit pair ids relative to its panel (array ix) and one byte with the panel (array pan): 41 bytes per group,
+// 6.35 / 5.86 bytes per entry of D against 8.  rowo[i] = first group of row i.
+constexpr int kPanelBits = 16;
+
+// Within a run the units are dealt to the groups in blocks of 16 groups (one per lane of the pricing kernel): unit t
+// of a block of n <= 16 groups sits in group t mod n at position t div n, so that the gather of position u reads n
+// CONSECUTIVE units across the lanes (consecutive pairs of w: a few cache lines instead of one per lane).
+__device__ __forceinline__ void unit_place(int u, int Gp, int &group, int &pos) {
+    const int k = u >> 6, n = min(16, Gp - 16 * k), t = u - 64 * k;
+    group = 16 * k + t % n;
+    pos = t / n;
+}
+
+// one warp per row.  FILL = false: cnt[row] = groups the row needs; FILL = true: write the row's groups.
+template <bool FILL>
+__global__ void k_pairs_build(const uint32_t *__restrict__ rowq, const float4 *__restrict__ val4,
+                              const int4 *__restrict__ col4, int64_t B, uint32_t *__restrict__ cnt,
+                              const uint32_t *__restrict__ rowo, float *__restrict__ va, float *__restrict__ vb,
+                              uint16_t *__restrict__ ix, uint8_t *__restrict__ pan) {
+    const int lane = threadIdx.x & 31;
+    const int64_t row = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (row > B) return;
+    if (row == B) {
+        if (!FILL && lane == 0) cnt[B] = 0u;
+        return;
+    }
+    const int32_t *col = reinterpret_cast<const int32_t *>(col4);
+    const float *val = reinterpret_cast<const float *>(val4);
+    const int64_t a = (int64_t)rowq[row] * 4, b = (int64_t)rowq[row + 1] * 4;
+    uint32_t groups = 0;
+    if (b > a) {
+        int64_t grp = FILL ? (int64_t)rowo[row] : 0;   // first group of the current run
+        const int p1 = (col[b - 1] >> 1) >> kPanelBits;
+        for (int pn = (col[a] >> 1) >> kPanelBits; pn <= p1; ++pn) {
+            // units of the row in this panel: entries ascend, a pair id different from the entry before opens a unit
+            int U = 0, lastp = -1;
+            for (int64_t e0 = a; e0 < b; e0 += 32) {
+                const int64_t e = e0 + lane;
+                const bool in = e < b;
+                const int pair = in ? col[e] >> 1 : -2;
+                int before = __shfl_up_sync(0xffffffffu, pair, 1);
+                if (lane == 0) before = e0 == a ? -1 : lastp;
+                const bool mine = in && (pair >> kPanelBits) == pn;
+                U += __popc(__ballot_sync(0xffffffffu, mine && pair != before));
+                const unsigned inmask = __ballot_sync(0xffffffffu, in);
+                lastp = __shfl_sync(0xffffffffu, pair, 31 - __clz(inmask));
+            }
+            if (U == 0) continue;
+            const int Gp = (U + 3) >> 2;
+            if (FILL) {
+                int done = 0, endpair = 0;
+                lastp = -1;
+                for (int64_t e0 = a; e0 < b; e0 += 32) {
+                    const int64_t e = e0 + lane;
+                    const bool in = e < b;
+                    const int sl = in ? col[e] : -4, pair = sl >> 1;
+                    int before = __shfl_up_sync(0xffffffffu, pair, 1);
+                    if (lane == 0) before = e0 == a ? -1 : lastp;
+                    const bool mine = in && (pair >> kPanelBits) == pn, isnew = mine && pair != before;
+                    const unsigned mnew = __ballot_sync(0xffffffffu, isnew), mm = __ballot_sync(0xffffffffu, mine);
+                    if (mine) {
+                        const int u = done + __popc(mnew & (0xffffffffu >> (31 - lane))) - 1;   // this entry's unit
+                        int g, pos;
+                        unit_place(u, Gp, g, pos);
+                        const float v = val[e];   // one entry per slot: a plain store; the zero padding of the CSR rows
+                        if (v != 0.f) ((pos & 2) ? vb : va)[(grp + g) * 4 + 2 * (pos & 1) + (sl & 1)] = v;   // must not write
+                        if (isnew) ix[(grp + g) * 4 + pos] = (uint16_t)(pair & 0xffff);
+                    }
+                    done += __popc(mnew);
+                    if (mm) endpair = __shfl_sync(0xffffffffu, pair, 31 - __clz(mm));
+                    const unsigned inmask = __ballot_sync(0xffffffffu, in);
+                    lastp = __shfl_sync(0xffffffffu, pair, 31 - __clz(inmask));
+                }
+                for (int u = U + lane; u < 4 * Gp; u += 32) {   // padding units: value 0 (the arrays start zeroed)
+                    int g, pos;
+                    unit_place(u, Gp, g, pos);
+                    ix[(grp + g) * 4 + pos] = (uint16_t)(endpair & 0xffff);
+                }
+                for (int g = lane; g < Gp; g += 32) pan[grp + g] = (uint8_t)pn;
+            }
+            grp += Gp;
+            groups += (uint32_t)Gp;
+        }
+    }
+    if (!FILL && lane == 0) cnt[row] = groups;
+}
+
+}  // namespace
+
+// d_format 1: build the pair copy of D from the padded layout (p->rowq, val4, col4 must be in place)
+int build_pairs(vmat_plan *p) {
+    const int64_t B = p->B;
+    cudaStream_t st = p->stream;
+    if (((p->Sp >> 1) >> kPanelBits) >= 256) return fail(p, VMAT_EINVAL, "d_format 1 needs a support below 2^25 voxels");
+    int rc;
+    uint32_t *cnt = nullptr;
+    void *tiles = nullptr;
+    const int64_t scan_tiles = (B + 1 + kScanTile - 1) / kScanTile;
+    cudaError_t e;
+    if ((e = pool_alloc((void **)&cnt, (size_t)(B + 1) * 4, p->device, st)) != cudaSuccess ||
+        (e = pool_alloc(&tiles, (size_t)scan_tiles * 4, p->device, st)) != cudaSuccess) {
+        cudaGetLastError();
+        pool_free(cnt, p->device, st);
+        return fail(p, VMAT_ENOMEM, std::string("device allocation (scratch) failed: ") + cudaGetErrorString(e));
+    }
+    auto done = [&](int code) {
+        pool_free(cnt, p->device, st);
+        pool_free(tiles, p->device, st);
+        return code;
+    };
+    k_pairs_build<false><<<(unsigned)((B + 1 + 7) / 8), 256, 0, st>>>(p->rowq, p->val4, p->col4, B, cnt, nullptr, nullptr,
+                                                                   nullptr, nullptr, nullptr);
+    if ((rc = dev_alloc(p, &p->pr_rowo, B + 1))) return done(rc);
+    if ((e = exclusive_scan<uint32_t>(cnt, p->pr_rowo, B + 1, (uint32_t *)tiles, st)) != cudaSuccess)
+        return done(cuda_fail(p, e, "exclusive_scan"));
+    uint32_t ng = 0;
+    if ((e = cudaMemcpyAsync(&ng, p->pr_rowo + B, 4, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
+        (e = cudaStreamSynchronize(st)) != cudaSuccess)
+        return done(cuda_fail(p, e, "cudaMemcpyAsync"));
+    p->pr_groups = ng;
+    if ((rc = dev_alloc(p, &p->pr_va, (int64_t)ng))) return done(rc);
+    if ((rc = dev_alloc(p, &p->pr_vb, (int64_t)ng))) return done(rc);
+    if ((rc = dev_alloc(p, &p->pr_ix, (int64_t)ng))) return done(rc);
+    if ((rc = dev_alloc(p, &p->pr_pan, (int64_t)ng))) return done(rc);
+    if ((e = cudaMemsetAsync(p->pr_va, 0, (size_t)ng * 16, st)) != cudaSuccess ||
+        (e = cudaMemsetAsync(p->pr_vb, 0, (size_t)ng * 16, st)) != cudaSuccess)
+        return done(cuda_fail(p, e, "cudaMemsetAsync"));
+    k_pairs_build<true><<<(unsigned)((B + 7) / 8), 256, 0, st>>>(p->rowq, p->val4, p->col4, B, nullptr, p->pr_rowo,
+                                                              (float *)p->pr_va, (float *)p->pr_vb, (uint16_t *)p->pr_ix,
+                                                              p->pr_pan);
+    if ((e = cudaGetLastError()) != cudaSuccess) return done(cuda_fail(p, e, "k_pairs_build"));
+    return done(VMAT_OK);
+}
+
+namespace {
 }  // namespace
 
 template <typename T>

@@ -155,6 +155,58 @@ def test_price_spmv_random_and_ragged(torch_cuda, vm):
         plan.destroy()
 
 
+def test_price_spmv_pair_format(torch_cuda, vm, tiny_oracle):
+    """vmat_options.d_format = 1: the pricing product from the copy of D in aligned slot pairs with
+    16-bit pair ids in panels of 65536 pairs.  Same tolerance as the fp32-CSR layout: on the tiny phantom (one panel),
+    on ragged random rows, and on a support of 300,000 voxels whose rows straddle three panels (runs of a few units
+    per panel, chunks of 32 entries that cross a panel border, empty rows, rows confined to one panel, dense runs of
+    consecutive slots)."""
+    from oracle import Oracle
+
+    opt = vm.default_options()
+    opt.d_format = 1
+    o = tiny_oracle
+    plan = make_plan(vm, o, options=opt)
+    for occ, left, right, y in oracle_states(o, 12, every=6):
+        plan.set_plan(occ, left, right, y)
+        _, w = o.penalty(o.dose(occ, left, right, y))
+        check_prices(torch_cuda, plan, o, w, occ)
+    assert plan.pricing_bytes < 0.8 * 8 * plan.nnz_padded
+    plan.destroy()
+    for seed in range(3):
+        o = random_problem(60 + seed, C=(5, 33, 70)[seed], R=(1, 3, 2)[seed])
+        plan = make_plan(vm, o, options=opt)
+        check_prices(torch_cuda, plan, o, np.random.default_rng(seed).normal(size=o.V), np.zeros(o.N, np.uint8))
+        plan.destroy()
+    rng = np.random.default_rng(3)
+    V, N, R, C = 300_000, 3, 2, 8
+    B = N * R * C
+    cols, vals, row_ptr = [], [], [0]
+    for i in range(B):
+        if i % 7 == 3:
+            c = np.zeros(0, np.int64)                                            # empty row
+        elif i % 5 == 0:
+            c = np.sort(rng.choice(np.arange(140_000, 240_000), 37, replace=False))  # confined to panel 1
+        elif i % 3 == 0:
+            c = np.concatenate([np.arange(131_000, 131_150), np.arange(262_100, 262_200)])  # dense runs across borders
+        else:
+            c = np.sort(rng.choice(V, int(rng.integers(4, 120)), replace=False))     # straddles all panels
+        cols.append(c.astype(np.int32))
+        vals.append(rng.uniform(0.05, 1.0, c.size).astype(np.float32))
+        row_ptr.append(row_ptr[-1] + c.size)
+    cols.append(np.arange(V, dtype=np.int32))                                    # (keeps the support = the whole grid)
+    T = rng.uniform(0.2, 1.0, V).astype(np.float32)
+    o = Oracle(np.asarray(row_ptr[:-1] + [row_ptr[-1]], np.int64), np.concatenate(cols[:-1]), np.concatenate(vals),
+               T, np.ones(V, np.float32), np.ones(V, np.float32), np.arange(N) * 2.0, R, C, 2, 0.1)
+    plan = make_plan(vm, o, options=opt)
+    check_prices(torch_cuda, plan, o, rng.normal(size=V), np.zeros(N, np.uint8))
+    occ = np.zeros(N, np.uint8)
+    occ[1] = 1
+    plan.set_plan(occ, np.zeros((N, R), np.int32), np.full((N, R), C, np.int32), np.zeros(N))
+    check_prices(torch_cuda, plan, o, rng.normal(size=V), occ)
+    plan.destroy()
+
+
 # ------------------------------------------------------------------------------------------------
 # P1 (d): leaf search and beam choice, bit exact on the oracle's fp32 prices
 # ------------------------------------------------------------------------------------------------
