@@ -96,7 +96,7 @@ static int evaluate_state(vmat_plan *p, int path) {
         if ((rc = launch_direct_dose(p))) return rc;
     } else {
         if ((rc = ensure_columns(p))) return rc;
-        if ((rc = launch_dose_grad(p))) return rc;
+        if ((rc = launch_columns_dose(p))) return rc;
     }
     p->state_valid = true;
     return VMAT_OK;

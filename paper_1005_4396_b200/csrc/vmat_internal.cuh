@@ -122,7 +122,9 @@ struct vmat_plan {
     double *cost3 = nullptr;       // device {F, G, F+gamma G}
     double *rate_ratio = nullptr;  // device scalar of the dose-rate feasibility test
     double *part_dose = nullptr;   // partial F sums of the direct dose pass
+    double *part_dose2 = nullptr;  // per-chunk F of the dose pass over the columns
     void *dose_scale = nullptr;    // device scalars of the direct dose pass (vmat_dose.cu)
+    int32_t *dose_list = nullptr;  // B: exposed beamlets of the direct dose pass (its first dose_scale->count entries)
     int dose_blocks = 0;
 
     // device trace of vmat_solve
@@ -214,7 +216,6 @@ int launch_leaf_search(vmat_plan *p, const float *g, int32_t *all_left, int32_t 
 int master_configure(vmat_plan *p);
 int reset_hessian(vmat_plan *p);
 int launch_column_build(vmat_plan *p, int beam /* -1: read p->sel */);
-int launch_dose_grad(vmat_plan *p);
 int launch_master(vmat_plan *p, int trace_it, int warm /* 1: inside vmat_solve, right after a committed search */);
 int launch_expand(vmat_plan *p, const float *src_s, float *dst_V, int what /*0 z, 1 w*/);
 int launch_compress(vmat_plan *p, const float *src_V, float *dst_s);
@@ -223,5 +224,6 @@ int launch_rate_ratio(vmat_plan *p, double rho, double *ratio_dev);
 // vmat_dose.cu: steps (a)+(b) straight from D (fixed-point atomics path) ------------------------------
 int dose_configure(vmat_plan *p);
 int launch_direct_dose(vmat_plan *p);
+int launch_columns_dose(vmat_plan *p);
 
 }  // namespace vmat

@@ -2766,9 +2766,6 @@ int launch_master(vmat_plan *p, int trace_it, int warm) {
     return launch_master_impl(p, p->opt.master_max_inner, trace_it, warm);
 }
 
-// steps (a)+(b) alone: the master kernel's evaluation pass with no iteration allowed
-int launch_dose_grad(vmat_plan *p) { return launch_master_impl(p, 0, -1, 0); }
-
 int launch_rate_ratio(vmat_plan *p, double rho, double *ratio_dev) {
     k_rate_ratio<<<1, 256, 0, p->stream>>>(p->occ, p->y, p->theta, (int)p->N, rho, ratio_dev);
     ++p->launches;
