@@ -114,6 +114,12 @@ typedef struct {
                                   tile are walked through per-chunk lists; 0: through masked loops over all such
                                   columns (the fallback the kernel takes by itself when the lists do not fit;
                                   exposed so that tests can reach it).  Same results.                            */
+    int32_t occupied_only_G;   /* reading of Eq. 2 (S2): 0 (default) = the sum runs over all N gantry
+                                  angles with y_k = 0 at un-occupied beams; 1 = over successive OCCUPIED beams only (an
+                                  un-occupied beam is not part of the arc yet).  With 1 an aperture's price carries the
+                                  derivative of G with its beam put into the arc, a beam that enters at y_k = 0 changes
+                                  G, and the post-master cost of vmat_solve is no longer guaranteed non-increasing.
+                                  vmat_enforce_dose_rate tests all N - 1 successive pairs in either reading.          */
 } vmat_options;
 
 /* One deliverable aperture: a beam and one leaf pair per row. */

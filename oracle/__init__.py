@@ -11,6 +11,7 @@ from .vmat_oracle import (  # noqa: F401
     set_num_threads,
     penalty,
     smooth,
+    smooth_occ,
     quantise,
     row_search,
 )

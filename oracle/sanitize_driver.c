@@ -31,7 +31,7 @@ int main(void) {
     for (int64_t j = 0; j < V; ++j) { T[j] = (float)(0.2 + 0.8 * rnd()); al[j] = rnd() < 0.5 ? (float)(0.5 + rnd()) : 0.f; be[j] = (float)(0.1 + rnd()); }
     double *theta = (double *)malloc(sizeof(double) * N);
     for (int64_t k = 0; k < N; ++k) theta[k] = 2.0 * (double)k + 0.5 * rnd();
-    vo_problem p = {V, N, R, C, row_ptr, col, val, T, al, be, theta, 2, 0.3};
+    vo_problem p = {V, N, R, C, row_ptr, col, val, T, al, be, theta, 2, 0.3, 0};
 
     uint8_t *occ = (uint8_t *)calloc(N, 1);
     int32_t *left = (int32_t *)calloc(N * R, sizeof(int32_t)), *right = (int32_t *)calloc(N * R, sizeof(int32_t));
@@ -71,6 +71,12 @@ int main(void) {
     vo_enforce_rate(&p, occ, left, right, y, z, &ri);
     int64_t box[4];
     vo_leaf_box(&p, occ, left, right, 3, 1, box);
+    /* the other reading of Eq. 2 (smoothing over the occupied beams only): the loop again from an empty plan */
+    p.g_occupied_only = 1;
+    memset(occ, 0, N); memset(y, 0, sizeof(double) * N);
+    tr.max_iters = N;
+    vo_solve(&p, occ, left, right, y, z, &tr);
+    vo_smooth_occ(N, y, theta, occ, dG);
     printf("sanitize_driver ok: %lld iterations, cost %.6f, %lld rounds\n", (long long)tr.iters, c3[2], (long long)ri.rounds);
 
     free(row_ptr); free(col); free(val); free(T); free(al); free(be); free(theta); free(occ); free(left); free(right);

@@ -40,6 +40,8 @@ typedef struct {
     const double  *theta;          /* N gantry angles in degrees, ascending (reading S4)    */
     int32_t delta;                 /* max leaf travel in beamlets per angular step (reading S6)          */
     double  gamma;                 /* weight of the smoothing term (Eq. 3)               */
+    int32_t g_occupied_only;       /* 0: Eq. 2 over all N angles, y = 0 at un-occupied beams (reading S2, default);
+                                      1: over successive OCCUPIED beams only (the other reading of S2)    */
 } vo_problem;
 
 /* ------------------------------------------------------------------------------------------
@@ -100,6 +102,46 @@ double vo_smooth(int64_t N, const double *y, const double *theta, double *dG) {
             dG[k] = s;
         }
     return G;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O3, the other reading of S2: "successive gantry angles" are the successive angles that HOLD an
+ * aperture; an un-occupied beam is not part of the arc yet and takes no part in Eq. 2:
+ *   G(y) = sum over successive occupied beams p < k of (y_k - y_p)^2 / (theta_k - theta_p).
+ * dG[k] for an occupied beam is dG/dy_k.  For an UN-occupied beam it is the derivative, at y_k = 0, of G with beam k
+ * put into the arc between its nearest occupied neighbours: the smoothing part of the price of an aperture there
+ * (reading S10).  Entering at y_k = 0 then changes G (unless the neighbours are at 0 too), so the post-master cost
+ * of the loop is no longer guaranteed to be non-increasing in this reading.  Operations individually rounded, in
+ * the order of vo_smooth.  dG may be NULL.
+ * ------------------------------------------------------------------------------------------ */
+double vo_smooth_occ(int64_t N, const double *y, const double *theta, const uint8_t *occ, double *dG) {
+    double G = 0.0;
+    int64_t prev = -1;
+    for (int64_t k = 0; k < N; ++k) {
+        if (!occ[k]) continue;
+        if (prev >= 0) {
+            const double d = y[k] - y[prev];
+            G += d * d / (theta[k] - theta[prev]);
+        }
+        prev = k;
+    }
+    if (dG)
+        for (int64_t k = 0; k < N; ++k) {
+            int64_t p = k - 1, n = k + 1;
+            while (p >= 0 && !occ[p]) --p;
+            while (n < N && !occ[n]) ++n;
+            const double yk = occ[k] ? y[k] : 0.0;
+            double s = 0.0;
+            if (p >= 0) s = s + 2.0 * (yk - y[p]) / (theta[k] - theta[p]);
+            if (n < N) s = s - 2.0 * (y[n] - yk) / (theta[n] - theta[k]);
+            dG[k] = s;
+        }
+    return G;
+}
+
+/* G and dG in the reading the problem asks for */
+static double smooth_of(const vo_problem *p, const uint8_t *occ, const double *y, double *dG) {
+    return p->g_occupied_only ? vo_smooth_occ(p->N, y, p->theta, occ, dG) : vo_smooth(p->N, y, p->theta, dG);
 }
 
 /* ------------------------------------------------------------------------------------------
@@ -197,7 +239,7 @@ int64_t vo_price_step(const vo_problem *p, const float *g32, const uint8_t *occ,
     double *dG = (double *)malloc(sizeof(double) * N);
     int64_t *q = (int64_t *)malloc(sizeof(int64_t) * C);
     int32_t *tl = (int32_t *)malloc(sizeof(int32_t) * R), *tr = (int32_t *)malloc(sizeof(int32_t) * R);
-    vo_smooth(N, y, p->theta, dG);
+    smooth_of(p, occ, y, dG);
     int64_t best = -1;
     double bp = 0.0;
     for (int64_t k = 0; k < N; ++k) {
@@ -367,7 +409,7 @@ static void master_solve(const vo_problem *p, const vo_columns *cols, const uint
     }
     columns_dose(cols, occ, y, z);
     double F = vo_penalty(V, z, p->T, p->alpha, p->beta, w);
-    double G = vo_smooth(N, y, p->theta, dG);
+    double G = smooth_of(p, occ, y, dG);
     double Phi = F + p->gamma * G;
     master_gradient(p, cols, occ, w, dG, grad);
     double pgmax = 0.0;
@@ -401,7 +443,7 @@ static void master_solve(const vo_problem *p, const vo_columns *cols, const uint
             const double om = z[j] < (double)p->T[j] ? (double)p->alpha[j] : (z[j] > (double)p->T[j] ? (double)p->beta[j] : 0.0);
             curvF += om * q[j] * q[j];
         }
-        const double phi2 = 2.0 * curvF + 2.0 * p->gamma * vo_smooth(N, d, p->theta, NULL); /* d^T L d = G(d) */
+        const double phi2 = 2.0 * curvF + 2.0 * p->gamma * smooth_of(p, occ, d, NULL); /* d^T L d = G(d) */
         double tmax = INFINITY;
         for (int64_t k = 0; k < N; ++k) {
             if (d[k] < 0.0 && (y[k] - lb) / (-d[k]) < tmax) tmax = (y[k] - lb) / (-d[k]);
@@ -423,7 +465,7 @@ static void master_solve(const vo_problem *p, const vo_columns *cols, const uint
 #pragma omp parallel for schedule(static)
             for (int64_t j = 0; j < V; ++j) zn[j] = z[j] + t * q[j];
             Fn = vo_penalty(V, zn, p->T, p->alpha, p->beta, wn);
-            Gn = vo_smooth(N, yn, p->theta, dG);
+            Gn = smooth_of(p, occ, yn, dG);
             Phin = Fn + p->gamma * Gn;
             if (Phin <= Phi + c1 * t * phi1) { accepted = 1; break; }
             /* below the resolution of Phi: accept on the slope instead (|phi'(t)| <= 0.9 |phi'(0)|) */
@@ -463,7 +505,7 @@ static void master_solve(const vo_problem *p, const vo_columns *cols, const uint
     info->pg_exit = pgmax;
     columns_dose(cols, occ, y, z);                                     /* z from the final y, no drift */
     info->F = vo_penalty(V, z, p->T, p->alpha, p->beta, NULL);
-    info->G = vo_smooth(N, y, p->theta, NULL);
+    info->G = smooth_of(p, occ, y, NULL);
     info->cost = info->F + p->gamma * info->G;
     free(w); free(q); free(zn); free(wn); free(dG); free(grad); free(gradn); free(pg); free(pgn); free(d); free(yn);
 }
@@ -534,7 +576,7 @@ void vo_enforce_rate(const vo_problem *p, const uint8_t *occ, const int32_t *lef
     info->gamma = q.gamma;
     info->ratio = ratio;
     info->F = vo_penalty(p->V, z, p->T, p->alpha, p->beta, NULL);
-    info->G = vo_smooth(p->N, y, p->theta, NULL);
+    info->G = smooth_of(p, occ, y, NULL);
     info->cost = info->F + q.gamma * info->G;
     columns_free(cols);
 }
@@ -548,7 +590,7 @@ void vo_cost_gradient(const vo_problem *p, const uint8_t *occ, const int32_t *le
     for (int64_t k = 0; k < p->N; ++k) if (occ[k]) columns_add(cols, p, k, left, right);
     columns_dose(cols, occ, y, z);
     const double F = vo_penalty(p->V, z, p->T, p->alpha, p->beta, w);
-    const double G = vo_smooth(p->N, y, p->theta, dG);
+    const double G = smooth_of(p, occ, y, dG);
     master_gradient(p, cols, occ, w, dG, grad);
     if (cost3) { cost3[0] = F; cost3[1] = G; cost3[2] = F + p->gamma * G; }
     free(z); free(w); free(dG);

@@ -31,7 +31,7 @@ def build(force: bool = False) -> str:
 class _Problem(_c.Structure):
     _fields_ = [("V", _c.c_int64), ("N", _c.c_int64), ("R", _c.c_int64), ("C", _c.c_int64),
                 ("row_ptr", _P), ("col", _P), ("val", _P), ("T", _P), ("alpha", _P), ("beta", _P),
-                ("theta", _P), ("delta", _c.c_int32), ("gamma", _c.c_double)]
+                ("theta", _P), ("delta", _c.c_int32), ("gamma", _c.c_double), ("g_occupied_only", _c.c_int32)]
 
 
 class _MasterInfo(_c.Structure):
@@ -67,6 +67,8 @@ def _load():
         L.vo_penalty.restype = _c.c_double
         L.vo_smooth.argtypes = [_c.c_int64, _P, _P, _P]
         L.vo_smooth.restype = _c.c_double
+        L.vo_smooth_occ.argtypes = [_c.c_int64, _P, _P, _P, _P]
+        L.vo_smooth_occ.restype = _c.c_double
         L.vo_prices.argtypes = [PP, _P, _P, _P]
         L.vo_prices.restype = None
         L.vo_quantise.argtypes = [_c.c_int64, _P, _P]
@@ -127,6 +129,15 @@ def smooth(y, theta_deg):
     return float(G), dG
 
 
+def smooth_occ(y, theta_deg, occ):
+    """The other reading of Eq. 2 (S2): smoothing over successive OCCUPIED beams only.  Returns (G, dG); dG at an
+    un-occupied beam is the derivative at y_k = 0 of G with that beam put into the arc."""
+    y, th, occ = _as(y, np.float64), _as(theta_deg, np.float64), _as(occ, np.uint8)
+    dG = np.empty_like(y)
+    G = _load().vo_smooth_occ(y.size, _ptr(y), _ptr(th), _ptr(occ), _ptr(dG))
+    return float(G), dG
+
+
 def quantise(g32):
     g32 = _as(g32, np.float32)
     q = np.empty(g32.size, np.int64)
@@ -172,7 +183,8 @@ class Trace:
 class Oracle:
     """The oracle bound to one problem instance (a vmat_inputs.Phantom or raw arrays)."""
 
-    def __init__(self, row_ptr, col_idx, val, T, alpha, beta, theta_deg, n_rows, n_cols, max_leaf_travel, gamma):
+    def __init__(self, row_ptr, col_idx, val, T, alpha, beta, theta_deg, n_rows, n_cols, max_leaf_travel, gamma,
+                 occupied_only_G=False):
         self.row_ptr = _as(row_ptr, np.int64)
         self.col = _as(col_idx, np.int32)
         self.val = _as(val, np.float32)
@@ -182,16 +194,18 @@ class Oracle:
         self.B = self.N * self.R * self.C
         assert self.row_ptr.size == self.B + 1
         self.delta, self.gamma = int(max_leaf_travel), float(gamma)
+        self.occupied_only_G = bool(occupied_only_G)
         self._p = _Problem(self.V, self.N, self.R, self.C, _ptr(self.row_ptr), _ptr(self.col), _ptr(self.val),
-                           _ptr(self.T), _ptr(self.alpha), _ptr(self.beta), _ptr(self.theta), self.delta, self.gamma)
+                           _ptr(self.T), _ptr(self.alpha), _ptr(self.beta), _ptr(self.theta), self.delta, self.gamma,
+                           int(self.occupied_only_G))
         self._L = _load()
 
     @classmethod
-    def from_phantom(cls, ph, gamma=None, max_leaf_travel=None):
+    def from_phantom(cls, ph, gamma=None, max_leaf_travel=None, occupied_only_G=False):
         c = ph.config
         return cls(ph.row_ptr, ph.col_idx, ph.val, ph.T, ph.alpha, ph.beta, ph.theta_deg, c.n_rows, c.n_cols,
                    c.max_leaf_travel if max_leaf_travel is None else max_leaf_travel,
-                   c.gamma if gamma is None else gamma)
+                   c.gamma if gamma is None else gamma, occupied_only_G=occupied_only_G)
 
     # plan helpers -----------------------------------------------------------------------------
     def empty_plan(self):
@@ -213,13 +227,16 @@ class Oracle:
     def penalty(self, z):
         return penalty(z, self.T, self.alpha, self.beta)
 
-    def smooth(self, y):
+    def smooth(self, y, occ=None):
+        """G and dG in the problem's reading of Eq. 2 (occ is needed for the occupied-only reading)."""
+        if self.occupied_only_G:
+            return smooth_occ(y, self.theta, occ)
         return smooth(y, self.theta)
 
     def cost(self, occ, left, right, y):
         z = self.dose(occ, left, right, y)
         F, _ = self.penalty(z)
-        G, _ = self.smooth(y)
+        G, _ = self.smooth(y, occ)
         return F, G, F + self.gamma * G
 
     # O4 ----------------------------------------------------------------------------------------

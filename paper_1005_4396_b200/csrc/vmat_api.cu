@@ -138,6 +138,7 @@ void vmat_default_options(vmat_options *opt) {
     opt->master_mode = 1;
     opt->stop_when_priced_out = 0;
     opt->master_unstaged_lists = 1;
+    opt->occupied_only_G = 0;
 }
 
 int vmat_create(const vmat_problem *pb, const vmat_options *options, void *cuda_stream, vmat_plan **out) {

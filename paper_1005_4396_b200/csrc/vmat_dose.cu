@@ -26,6 +26,23 @@ constexpr int kDoseThreads = 256;
 constexpr int kDoseLanes = 16;    // lanes per beamlet
 constexpr int kDoseEntries = 8;   // 4-byte loads of values and of indices in flight per lane
 
+// this thread's share of Eq. 2: the pairs (k, next(k)) for k = first, first + stride, ..; next(k) = k + 1 with
+// y = 0 at un-occupied beams (S2), or the next occupied beam (the other reading, occ_only)
+__device__ __forceinline__ double smooth_share(const uint8_t *occ, const double *y, const double *theta, int N, int occ_only,
+                                               int first, int stride) {
+    double g = 0.0;
+    for (int k = first; k + 1 < N; k += stride) {
+        if (occ_only && !occ[k]) continue;
+        int n = k + 1;
+        if (occ_only)
+            while (n < N && !occ[n]) ++n;
+        if (n >= N) continue;
+        const double y0 = occ[k] ? y[k] : 0.0, y1 = occ[n] ? y[n] : 0.0, dv = y1 - y0;
+        g += dv * dv / (theta[n] - theta[k]);
+    }
+    return g;
+}
+
 struct DoseScale {
     double scale, inv;            // fixed-point scale of y_k * D_ij and its inverse (powers of two)
     double G;                     // Eq. 2
@@ -40,7 +57,7 @@ struct DoseScale {
 __global__ void __launch_bounds__(kDoseThreads)
 k_dose_prepare(const uint8_t *__restrict__ occ, const int32_t *__restrict__ left, const int32_t *__restrict__ right,
                const double *__restrict__ y, const double *__restrict__ theta, int N, int R, int C, double fx_scale,
-               DoseScale *__restrict__ out, int32_t *__restrict__ exp_list) {
+               int occ_only, DoseScale *__restrict__ out, int32_t *__restrict__ exp_list) {
     pdl_trigger();   // the scatter may be scheduled; it waits for the list and the scale itself
     __shared__ double s_max[kDoseThreads / 32], s_sum[kDoseThreads / 32];
     __shared__ int s_cnt[kDoseThreads / 32];
@@ -71,15 +88,8 @@ k_dose_prepare(const uint8_t *__restrict__ occ, const int32_t *__restrict__ left
     int32_t *dst = exp_list + s_base + before + incl - n;
     for (int c = 0; c < n; ++c) dst[c] = kr * C + l + c;
     if (blockIdx.x != 0) return;
-    double mx = 0.0, g = 0.0;
-    for (int k = threadIdx.x; k < N; k += kDoseThreads) {
-        const double yk = occ[k] ? y[k] : 0.0;
-        mx = fmax(mx, fabs(yk));
-        if (k + 1 < N) {
-            const double yn = occ[k + 1] ? y[k + 1] : 0.0, dv = yn - yk;
-            g += dv * dv / (theta[k + 1] - theta[k]);
-        }
-    }
+    double mx = 0.0, g = smooth_share(occ, y, theta, N, occ_only, threadIdx.x, kDoseThreads);
+    for (int k = threadIdx.x; k < N; k += kDoseThreads) mx = fmax(mx, occ[k] ? fabs(y[k]) : 0.0);
 #pragma unroll
     for (int o = 16; o; o >>= 1) {
         mx = fmax(mx, __shfl_xor_sync(kFull, mx, o));
@@ -209,7 +219,7 @@ k_dose_columns(const float *__restrict__ Dd, int N, int nchunks, const uint8_t *
                const double *__restrict__ y, const double *__restrict__ theta, const uint32_t *__restrict__ touch,
                int touch_words, const float *__restrict__ T, const float *__restrict__ alpha,
                const float *__restrict__ beta, float *__restrict__ z, float *__restrict__ w, double *__restrict__ partF,
-               unsigned int *__restrict__ ticket, double F_out, double gamma, double *__restrict__ cost3) {
+               unsigned int *__restrict__ ticket, double F_out, double gamma, int occ_only, double *__restrict__ cost3) {
     __shared__ int s_list[2048];           // vmat_create: N <= 2048
     __shared__ float s_coef[2048];
     __shared__ int s_wcnt[kColWarps], s_n;
@@ -289,12 +299,9 @@ k_dose_columns(const float *__restrict__ Dd, int N, int nchunks, const uint8_t *
     __syncthreads();
     if (!s_last) return;
     __threadfence();
-    double f = 0.0, g = 0.0;
+    double f = 0.0;
     for (int i = threadIdx.x; i < nchunks; i += kDoseThreads) f += __ldcg(partF + i);
-    for (int k = threadIdx.x; k + 1 < N; k += kDoseThreads) {   // Eq. 2 (S2: y = 0 at un-occupied beams)
-        const double y0 = occ[k] ? y[k] : 0.0, y1 = occ[k + 1] ? y[k + 1] : 0.0, dv = y1 - y0;
-        g += dv * dv / (theta[k + 1] - theta[k]);
-    }
+    const double g = smooth_share(occ, y, theta, N, occ_only, threadIdx.x, kDoseThreads);
     __shared__ double s_g[kDoseThreads];
     s_f[threadIdx.x] = f;
     s_g[threadIdx.x] = g;
@@ -337,7 +344,8 @@ int launch_columns_dose(vmat_plan *p) {
     k_dose_columns<<<(unsigned)nchunks, kDoseThreads, 0, p->stream>>>(p->Dd, (int)p->N, nchunks, p->occ, p->y, p->theta,
                                                                      p->col_touch, p->touch_words, p->T_s, p->alpha_s,
                                                                      p->beta_s, p->z_s, p->w_s, p->part_dose2, &ds->ticket2,
-                                                                     p->F_out, p->gamma, p->cost3);
+                                                                     p->F_out, p->gamma, p->opt.occupied_only_G ? 1 : 0,
+                                                                     p->cost3);
     ++p->launches;
     VMAT_CUDA(p, cudaGetLastError());
     return VMAT_OK;
@@ -349,7 +357,8 @@ int launch_direct_dose(vmat_plan *p) {
     DoseScale *ds = (DoseScale *)p->dose_scale;
     const unsigned pblocks = (unsigned)((p->N * p->R + kDoseThreads - 1) / kDoseThreads);
     k_dose_prepare<<<pblocks, kDoseThreads, 0, p->stream>>>(p->occ, p->left, p->right, p->y, p->theta, (int)p->N, (int)p->R,
-                                                            (int)p->C, p->fx_scale, ds, p->dose_list);
+                                                            (int)p->C, p->fx_scale, p->opt.occupied_only_G ? 1 : 0, ds,
+                                                            p->dose_list);
     if (p->B > 0) {
         // a fixed grid (a few blocks per SM) walks the list: its length is known on the device only
         const unsigned blocks = (unsigned)(p->sm_count * 6);

@@ -308,6 +308,7 @@ struct MasterArgs {
     int N;
     double gamma, F_out, eps, fx_inv, stall_rel;
     double lb, ub;              // bounds on the dose rates of occupied beams (default 0, +inf)
+    int occ_only;               // reading of Eq. 2: smoothing over successive occupied beams only (vmat_options.occupied_only_G)
     int stall_count;
     float Tmax, abmax;
     int max_inner;
@@ -455,6 +456,7 @@ struct Smem {
     float *rz0, *rz1, *rq, *rT, *ral, *rbe;   // resident copies of the block's own slots (a.rslots each), or unused
     float *rom;               // k_newton: resident copy of a.omref (written through)
     float *tile;       // staged 512-byte segments of the block's part of Dd, kSeg floats apart
+    int *nx, *pv;      // neighbours of beam k in Eq. 2 (-1: none): k + 1, k - 1, or the next / previous occupied beam
     int *sk, *lo, *hi, *ik;   // lo, hi: block-local range of chunks (j of b + jG) that may hold entries of column i
     int *nseg;         // how many of them really do
     unsigned long long *lmask;   // which: bit (j & 63) of word lmask[(j >> 6) * N + i]
@@ -899,10 +901,11 @@ __device__ __forceinline__ void ctl_reduce(double (&s)[MS], double &mx, double *
 __device__ __forceinline__ double smooth_part(const double *v, const Smem &sm, int N, int CT, bool want_dG) {
     double s = 0.0;
     for (int k = threadIdx.x; k < N; k += CT) {
-        const double e1 = k + 1 < N ? (v[k + 1] - v[k]) * sm.rdt[k] : 0.0;      // (v_{k+1}-v_k)/dtheta_k
-        if (k + 1 < N) s += (v[k + 1] - v[k]) * e1;
+        const int nx = sm.nx[k], pv = sm.pv[k];
+        const double e1 = nx >= 0 ? (v[nx] - v[k]) * sm.rdt[k] : 0.0;      // (v_next - v_k) / dtheta
+        if (nx >= 0) s += (v[nx] - v[k]) * e1;
         if (want_dG) {
-            const double e0 = k > 0 ? (v[k] - v[k - 1]) * sm.rdt[k - 1] : 0.0;
+            const double e0 = pv >= 0 ? (v[k] - v[pv]) * sm.rdt[pv] : 0.0;
             sm.dG[k] = 2.0 * (e0 - e1);
         }
     }
@@ -961,7 +964,9 @@ __device__ __forceinline__ Setup master_setup(const MasterArgs &a, Smem &sm, flo
     sm.lo = sm.sk + N;
     sm.hi = sm.lo + N;
     sm.ik = sm.hi + N;
-    sm.base = sm.ik + N;
+    sm.nx = sm.ik + N;
+    sm.pv = sm.nx + N;
+    sm.base = sm.pv + N;
     sm.unc = sm.base + N;
     sm.cseg = sm.unc + N;
     sm.gseg = sm.cseg + a.cache_segs;
@@ -1001,7 +1006,18 @@ __device__ __forceinline__ Setup master_setup(const MasterArgs &a, Smem &sm, flo
         else if (yk > a.ub) yk = a.ub;
         sm.y[k] = yk;
         sm.d[k] = 0.0;
-        sm.rdt[k] = k + 1 < N ? 1.0 / (a.theta[k + 1] - a.theta[k]) : 0.0;
+        // neighbours in Eq. 2: the angles next to k (S2), or the nearest occupied beams (the other reading)
+        int nxk = k + 1 < N ? k + 1 : -1, pvk = k - 1;
+        if (a.occ_only) {
+            if (!a.occ[k]) nxk = pvk = -1;
+            else {
+                while (nxk >= 0 && !a.occ[nxk]) nxk = nxk + 1 < N ? nxk + 1 : -1;
+                while (pvk >= 0 && !a.occ[pvk]) --pvk;
+            }
+        }
+        sm.nx[k] = nxk;
+        sm.pv[k] = pvk;
+        sm.rdt[k] = nxk >= 0 ? 1.0 / (a.theta[nxk] - a.theta[k]) : 0.0;
     }
     __syncthreads();
     const int K = sK;
@@ -1342,8 +1358,8 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
             s[0] += sm.grad[k] * dk;
             s[1] += fabs(dk) * lf;
             s[2] += fabs(yk) * lf;
-            if (k + 1 < N) {
-                const double dv = sm.d[k + 1] - dk;
+            if (sm.nx[k] >= 0) {
+                const double dv = sm.d[sm.nx[k]] - dk;
                 s[3] += dv * dv * sm.rdt[k];
             }
             if (dk < 0.0) ntl = fmax(ntl, -((yk - lb) / (-dk)));
@@ -2010,7 +2026,8 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
     double *vgn = vyn + N, *vp = vgn + N, *linf = vp + N, *rdt = linf + N, *Minv = rdt + N, *dGb = Minv + N;
     double *redb = dGb + N;                                  // 2 x kMasterWarps x kSolveRed
     int *sk = reinterpret_cast<int *>(redb + 2 * kMasterWarps * kSolveRed), *ik = sk + N, *freeo = ik + N, *freen = freeo + N;
-    float *dc = reinterpret_cast<float *>((reinterpret_cast<uintptr_t>(freen + N) + 15) & ~(uintptr_t)15);   // compact direction
+    int *nxl = freen + N, *pvl = nxl + N;   // neighbours of beam k in Eq. 2 (as in master_setup)
+    float *dc = reinterpret_cast<float *>((reinterpret_cast<uintptr_t>(pvl + N) + 15) & ~(uintptr_t)15);   // compact direction
     const int Np = ((N + 3) / 4) | 1;                        // float4s per row at K = N
     float *cgb = dc + 4 * Np;                                // 2 x 8 x kCgRow floats: scratch of cg_reduce
     float *hpart = cgb + 2 * 8 * kCgRow;                     // the product with the matrix, and the part of its second half
@@ -2041,7 +2058,17 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
         else if (yk > ub) yk = ub;
         vy[k] = yk;
         vd[k] = 0.0;
-        rdt[k] = k + 1 < N ? 1.0 / (a.theta[k + 1] - a.theta[k]) : 0.0;
+        int nxk = k + 1 < N ? k + 1 : -1, pvk = k - 1;
+        if (a.occ_only) {
+            if (!on) nxk = pvk = -1;
+            else {
+                while (nxk >= 0 && !a.occ[nxk]) nxk = nxk + 1 < N ? nxk + 1 : -1;
+                while (pvk >= 0 && !a.occ[pvk]) --pvk;
+            }
+        }
+        nxl[k] = nxk;
+        pvl[k] = pvk;
+        rdt[k] = nxk >= 0 ? 1.0 / (a.theta[nxk] - a.theta[k]) : 0.0;
         double lf = 0.0;
         if (on) {
             const ColStat cs = a.colstat[k];
@@ -2073,9 +2100,10 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
     auto smooth_of = [&](const double *v, double &G, double &zb) {
         double s[2] = {0.0, 0.0}, mx = 0.0;
         for (int k = tid; k < N; k += kMasterThreads) {
-            const double e1 = k + 1 < N ? (v[k + 1] - v[k]) * rdt[k] : 0.0;
-            const double e0 = k > 0 ? (v[k] - v[k - 1]) * rdt[k - 1] : 0.0;
-            if (k + 1 < N) s[0] += (v[k + 1] - v[k]) * e1;
+            const int nx = nxl[k], pv = pvl[k];
+            const double e1 = nx >= 0 ? (v[nx] - v[k]) * rdt[k] : 0.0;
+            const double e0 = pv >= 0 ? (v[k] - v[pv]) * rdt[pv] : 0.0;
+            if (nx >= 0) s[0] += (v[nx] - v[k]) * e1;
             dGb[k] = 2.0 * (e0 - e1);
             s[1] += fabs(v[k]) * linf[k];
         }
@@ -2204,7 +2232,7 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
         for (int k = tid; k < N; k += kMasterThreads) {
             const int i = ik[k];
             double m = 0.0;
-            if (i >= 0) m = 2.0 * (double)H32[i * Kp + i] + 2.0 * a.gamma * ((k > 0 ? rdt[k - 1] : 0.0) + rdt[k]);
+            if (i >= 0) m = 2.0 * (double)H32[i * Kp + i] + 2.0 * a.gamma * ((pvl[k] >= 0 ? rdt[pvl[k]] : 0.0) + rdt[k]);
             Minv[k] = m > 0.0 ? 1.0 / m : 1.0;
         }
         const long long c1 = clock64();
@@ -2278,8 +2306,9 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
             double hdk = 0.0;
             float s5[5] = {0.f, 0.f, 0.f, 0.f, 0.f}, ntl = -CUDART_INF_F;
             if (mine) {
-                const double e1 = k + 1 < N ? (vd[k + 1] - dk) * rdt[k] : 0.0;
-                const double e0 = k > 0 ? (dk - vd[k - 1]) * rdt[k - 1] : 0.0;
+                const int nx = nxl[k], pv = pvl[k];
+                const double e1 = nx >= 0 ? (vd[nx] - dk) * rdt[k] : 0.0;
+                const double e0 = pv >= 0 ? (dk - vd[pv]) * rdt[pv] : 0.0;
                 hdk = 2.0 * (double)hpart[ik[k]] + 2.0 * a.gamma * (e0 - e1);
                 s5[0] = (float)(dk * hdk);
                 s5[1] = (float)(rk * dk);
@@ -2541,7 +2570,7 @@ size_t master_smem_bytes(int64_t N, int64_t rslots, int64_t cache_segs, int64_t 
     return (size_t)(2 * kGroup * kChunk + (1 + 2 * f1) * kGroup * kSeg + f1 * kGroup * kChunk + (6 + f1) * rslots) * 4   // part2, wbuf (ombuf, ubuf, fl_dw), resident slots
            + (size_t)cache_segs * seg_bytes(newton)                                          // tile and the lists over it
            + (size_t)((13 + 2 * f1) * N + 2 * N + 2 + kMasterWarps + 2 * kMasterWarps * kRedSlots) * 8 + sizeof(Ctl)   // K-vectors (gaccu), recv, red, cred, ctl
-           + (size_t)N * 4 * 8 + (size_t)(ngroups * kGroup + 1) * 4           // coef, sk, lo, hi, ik, base, unc, nseg; coff
+           + (size_t)N * 4 * 10 + (size_t)(ngroups * kGroup + 1) * 4          // coef, sk, lo, hi, ik, nx, pv, base, unc, nseg; coff
            + (size_t)ngroups * (kGroup + 1) * 4                               // wst
            + (size_t)((ngroups * kGroup + 63) / 64) * N * 8                   // lmask
            + (size_t)f1 * ((size_t)2 * N * 4 + (kGroup * 4 + 4) * 4 + kGroup * kChunk)   // hm, hv, fl_wc, fl_slot
@@ -2551,7 +2580,7 @@ size_t master_smem_bytes(int64_t N, int64_t rslots, int64_t cache_segs, int64_t 
 // shared memory of k_newton's solving block (newton_solver's carve-up)
 size_t solver_smem_bytes(int64_t N) {
     const int64_t Np = ((N + 3) / 4) | 1;
-    return (size_t)(14 * N + 2 * kMasterWarps * kSolveRed) * 8 + (size_t)4 * N * 4 + 16 + (size_t)4 * Np * 4 +
+    return (size_t)(14 * N + 2 * kMasterWarps * kSolveRed) * 8 + (size_t)6 * N * 4 + 16 + (size_t)4 * Np * 4 +
            (size_t)(kMasterThreads + 2 * 8 * 8) * 4 + (size_t)4 * Np * 4 * Np * 4;
 }
 
@@ -2722,6 +2751,7 @@ static int launch_master_impl(vmat_plan *p, int max_inner, int trace_it, int war
     a.eps = p->opt.master_eps;
     a.stall_rel = p->opt.master_stall_rel;
     a.stall_count = p->opt.master_stall_count;
+    a.occ_only = p->opt.occupied_only_G ? 1 : 0;
     a.lb = p->y_min;
     a.ub = p->y_max;
     a.max_inner = max_inner;

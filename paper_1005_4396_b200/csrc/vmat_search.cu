@@ -137,6 +137,7 @@ struct SearchArgs {
     double *y;
     const double *theta;
     int N, R, C, delta;
+    int occ_only;                      // reading of Eq. 2: smoothing over successive occupied beams only
     double gamma;
     int32_t *cand_left, *cand_right;   // N*R row optima
     double *beam_price;                // N
@@ -247,13 +248,16 @@ __global__ void __launch_bounds__(kSearchThreads) k_leaf_search(const SearchArgs
                 a.beam_ticket[k] = 0u;
                 // price_k = 2^-30 * total + gamma * dG/dy_k, every operation individually rounded
                 // (Eq. 2; reading S10); same order of operations as the definition
+                // (the neighbours of beam k in Eq. 2: the angles next to it, or, in the occupied-only reading, the
+                // nearest occupied beams, between which an aperture at k would enter the arc; y_k = 0 here)
+                const int pm = a.occ_only ? s_km : k - 1, pp = a.occ_only ? s_kp : k + 1;
                 double dG = 0.0;
-                if (k > 0)
-                    dG = __dadd_rn(dG, __ddiv_rn(__dmul_rn(2.0, __dsub_rn(a.y[k], a.y[k - 1])),
-                                                 __dsub_rn(a.theta[k], a.theta[k - 1])));
-                if (k + 1 < N)
-                    dG = __dsub_rn(dG, __ddiv_rn(__dmul_rn(2.0, __dsub_rn(a.y[k + 1], a.y[k])),
-                                                 __dsub_rn(a.theta[k + 1], a.theta[k])));
+                if (pm >= 0)
+                    dG = __dadd_rn(dG, __ddiv_rn(__dmul_rn(2.0, __dsub_rn(a.y[k], a.y[pm])),
+                                                 __dsub_rn(a.theta[k], a.theta[pm])));
+                if (pp < N)
+                    dG = __dsub_rn(dG, __ddiv_rn(__dmul_rn(2.0, __dsub_rn(a.y[pp], a.y[k])),
+                                                 __dsub_rn(a.theta[pp], a.theta[k])));
                 const double smooth = __dmul_rn(a.gamma, dG);
                 const bool undeliverable = (seen >> 31) != 0u || s_bad;
                 const double price = undeliverable ? CUDART_INF : __dadd_rn(ldexp(__ll2double_rn(total), -30), smooth);
@@ -367,6 +371,7 @@ int launch_leaf_search(vmat_plan *p, const float *g, int32_t *all_left, int32_t 
     a.C = (int)p->C;
     a.delta = p->delta;
     a.gamma = p->gamma;
+    a.occ_only = p->opt.occupied_only_G ? 1 : 0;
     a.cand_left = p->cand_left;
     a.cand_right = p->cand_right;
     a.beam_price = p->beam_price;

@@ -554,6 +554,44 @@ def test_solve_with_dose_rate_bounds_matches_oracle(torch_cuda, vm, tiny_oracle,
         plan.destroy()
 
 
+@pytest.mark.parametrize("mode", [0, 1])
+def test_occupied_only_smoothing_option(torch_cuda, vm, tiny_phantom, mode):
+    """vmat_options.occupied_only_G (the other reading of S2: Eq. 2 over successive occupied beams only): beam prices
+    bit-exact on the oracle's prices along its own trajectory, master cost and G on the same apertures, and the free
+    run against the oracle's with the same option."""
+    from oracle import Oracle
+
+    o = Oracle.from_phantom(tiny_phantom, occupied_only_G=True)
+    opt = mode_options(vm, mode)
+    opt.occupied_only_G = 1
+    plan = make_plan(vm, o, options=opt)
+    for occ, left, right, y in oracle_states(o, 18, every=6):
+        z = o.dose(occ, left, right, y)
+        _, w = o.penalty(z)
+        g32 = o.prices(w, occ).astype(np.float32)
+        check_search(torch_cuda, plan, o, occ, left, right, y, g32)             # beam prices carry gamma dG/dy_k
+        if occ.any():
+            check_master(plan, o, occ, left, right, np.zeros(o.N))
+            check_master(plan, o, occ, left, right, y * 0.7)
+            for path in (0, 1):                                                 # G of both dose passes
+                plan.set_plan(occ, left, right, y)
+                plan.dose_recompute(path)
+                F, G, cost = plan.dose()
+                assert abs(G - o.smooth(y, occ)[0]) <= 1e-12 * max(1.0, abs(G))
+    occ_r, left_r, right_r, y_r, z_r, tr = o.solve(40)
+    fresh = make_plan(vm, o, options=opt)
+    st = fresh.solve(40)
+    occ, left, right, y = fresh.get_plan()
+    assert st.iters == o.N and occ.all()
+    check_free_run_against_oracle(o, st, (occ, left, right, y), tr, lambda n: o.solve(n)[:4] if n else o.empty_plan())
+    # with every beam occupied the two readings are one: the default plan prices this arc alike
+    ref = make_plan(vm, Oracle.from_phantom(tiny_phantom))
+    ref.set_plan(occ, left, right, y)
+    assert abs(ref.dose()[2] - st.cost) <= 1e-6 * abs(st.cost)
+    for q in (plan, fresh, ref):
+        q.destroy()
+
+
 def test_solve_stop_when_priced_out_option(torch_cuda, vm):
     """Option of reading S5: vmat_solve ends as soon as no aperture has a negative price; the default goes on until
     every beam holds an aperture.  Same stop iteration, apertures and cost as the oracle's."""

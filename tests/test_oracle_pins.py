@@ -174,6 +174,99 @@ def test_smooth_is_laplacian_quadratic_form_and_gradient():
 # ------------------------------------------------------------------------------------------------
 # O5 leaf-row interval search: brute force over every (l, r') in the box
 # ------------------------------------------------------------------------------------------------
+# ------------------------------------------------------------------------------------------------
+# the other reading of S2: Eq. 2 over successive OCCUPIED beams only (option, default off)
+# ------------------------------------------------------------------------------------------------
+def test_smooth_occupied_only_closed_forms_and_subpath_laplacian():
+    rng = np.random.default_rng(12)
+    N = 11
+    theta = np.cumsum(rng.uniform(1.0, 3.0, N))
+    occ = np.zeros(N, np.uint8)
+    occ[[1, 2, 5, 6, 9]] = 1
+    ks = np.flatnonzero(occ)
+    # a constant over the occupied beams costs nothing, whatever sits at the un-occupied ones
+    y = np.where(occ, 3.7, 0.0)
+    G, dG = orc.smooth_occ(y, theta, occ)
+    assert G == 0.0 and np.all(dG[ks] == 0.0)
+    # a ramp in the angle over the occupied beams: G = sum (dtheta)^2 / dtheta = theta_last - theta_first
+    y = np.where(occ, theta, 0.0)
+    G, dG = orc.smooth_occ(y, theta, occ)
+    assert G == pytest.approx(theta[9] - theta[1], rel=1e-13)
+    np.testing.assert_allclose(dG[ks], [-2.0, 0.0, 0.0, 0.0, 2.0], atol=1e-12)   # interior terms cancel
+    # G = y^T L y and dG = 2 L y with the weighted path-graph Laplacian of the occupied SUB-path, built here
+    y = rng.uniform(0.0, 2.0, N) * occ
+    L = np.zeros((N, N))
+    for a, b in zip(ks[:-1], ks[1:]):
+        s = 1.0 / (theta[b] - theta[a])
+        L[a, a] += s; L[b, b] += s; L[a, b] -= s; L[b, a] -= s
+    G, dG = orc.smooth_occ(y, theta, occ)
+    assert G == pytest.approx(float(y @ L @ y), rel=1e-13)
+    np.testing.assert_allclose(dG[ks], (2.0 * L @ y)[ks], rtol=1e-12, atol=1e-13)
+    # at an un-occupied beam: the derivative at y_k = 0 of G with the beam put into the arc (finite difference)
+    for k in (0, 3, 7, 10):
+        occ2 = occ.copy()
+        occ2[k] = 1
+        h = 1e-6
+        yp, ym = y.copy(), y.copy()
+        yp[k], ym[k] = h, -h
+        fd = (orc.smooth_occ(yp, theta, occ2)[0] - orc.smooth_occ(ym, theta, occ2)[0]) / (2 * h)
+        assert dG[k] == pytest.approx(fd, rel=1e-6, abs=1e-9)
+    # every beam occupied: the reading of the paper's Eq. 2 over all N angles
+    full = np.ones(N, np.uint8)
+    y = rng.uniform(0.0, 2.0, N)
+    Ga, dGa = orc.smooth(y, theta)
+    Gb, dGb = orc.smooth_occ(y, theta, full)
+    assert Ga == Gb and np.array_equal(dGa, dGb)
+
+
+def test_occupied_only_price_is_the_finite_difference_of_the_cost_and_master_is_nnls():
+    """With the option on: (i) price_k is still the reduced cost, the one-sided finite difference of Phi for the
+    chosen aperture put into the arc (S10); (ii) the master on alpha = beta problems is the non-negative least squares
+    with the difference operator of the occupied sub-path (scipy.optimize.nnls); (iii) the loop runs, ends with every
+    beam occupied and agrees with the default reading from then on (all beams occupied: the readings coincide)."""
+    base, D, rng = small_problem(31, V=60, N=7, R=2, C=6, gamma=0.6, delta=2, nonuniform_theta=True)
+    om = rng.uniform(0.5, 2.0, base.V).astype(np.float32)
+    o = Oracle(base.row_ptr, base.col, base.val, base.T, om, om, base.theta, base.R, base.C, base.delta, base.gamma,
+               occupied_only_G=True)
+    occ, left, right, y = random_plan(o, rng, 3)
+    ks = np.flatnonzero(occ)
+    for k in ks[1:]:
+        left[k], right[k] = left[ks[0]], right[ks[0]]            # mutually deliverable
+    # (ii) master = NNLS over the occupied beams
+    y_opt, z, info = o.master(occ, left, right, eps=1e-11)
+    Dc = np.einsum("krc,krcv->kv", open_mask(o, occ, left, right), D.reshape(o.N, o.R, o.C, o.V))[ks]
+    E = np.zeros((len(ks) - 1, len(ks)))
+    for i in range(len(ks) - 1):
+        s = 1.0 / np.sqrt(o.theta[ks[i + 1]] - o.theta[ks[i]])
+        E[i, i], E[i, i + 1] = -s, s
+    sq = np.sqrt(om.astype(np.float64))
+    A = np.vstack([sq[:, None] * Dc.T, np.sqrt(o.gamma) * E])
+    b = np.concatenate([sq * o.T.astype(np.float64), np.zeros(len(ks) - 1)])
+    y_ref, rnorm = scipy.optimize.nnls(A, b)
+    assert info.cost == pytest.approx(rnorm ** 2, rel=1e-9)
+    np.testing.assert_allclose(y_opt[ks], y_ref, rtol=1e-5, atol=1e-7)
+    # (i) the price of the chosen aperture at the master's optimum
+    zz = o.dose(occ, left, right, y_opt)
+    _, w = o.penalty(zz)
+    g32 = o.prices(w, occ).astype(np.float32)
+    out = o.price_step(g32, occ, left, right, y_opt)
+    k = out["beam"]
+    occ2, l2, r2 = occ.copy(), left.copy(), right.copy()
+    occ2[k] = 1
+    l2[k], r2[k] = out["left"], out["right"]
+    h = 1e-7
+    yh = y_opt.copy()
+    yh[k] = h
+    fd = (o.cost(occ2, l2, r2, yh)[2] - o.cost(occ2, l2, r2, y_opt)[2]) / h      # both WITH beam k in the arc
+    assert out["price"] == pytest.approx(fd, rel=2e-4, abs=1e-6)
+    # (iii) the loop
+    occ_f, left_f, right_f, y_f, z_f, tr = o.solve(20)
+    assert occ_f.all() and tr.iters == o.N
+    d = Oracle(base.row_ptr, base.col, base.val, base.T, om, om, base.theta, base.R, base.C, base.delta, base.gamma)
+    assert o.cost(occ_f, left_f, right_f, y_f)[2] == pytest.approx(d.cost(occ_f, left_f, right_f, y_f)[2], rel=1e-14)
+    assert d.master(occ_f, left_f, right_f, y0=y_f, eps=1e-10)[2].cost == pytest.approx(tr.cost[-1], rel=1e-8)
+
+
 def brute_force_row(q, Lmin, Lmax, Rmin, Rmax):
     """Enumerate all admissible leaf pairs; key = (sum of open prices, open count, l) (S8, S9)."""
     C = len(q)
