@@ -273,6 +273,28 @@ int vmat_get_plan(vmat_plan *plan, uint8_t *occupied, int32_t *left, int32_t *ri
 int vmat_set_plan(vmat_plan *plan, const uint8_t *occupied, const int32_t *left, const int32_t *right,
                   const double *y);
 
+/* Dose-deposition matrix on the device: a stand-in for the paper's GPU dose engine ("We calculate D_ij's
+ * using our in-house dose calculation engine implemented on a ... GPU", ref 17, a finite-size pencil-beam engine that is
+ * another paper).  It evaluates the ray / Gaussian / exponential model of BASELINE.json:configs:
+ * parallel rays in the axial plane, gantry axis = grid z through the grid centre, beam k at k 360/n_beams degrees,
+ * D = exp(-mu depth) exp(-rho^2 / 2 sigma^2) (1 + noise U(-1,1)) inside a body cylinder of radius body_radius_mm,
+ * sigma = sigma_beamlets x beamlet_mm, support rho <= 4.5 sigma, entries below cutoff x (row maximum) dropped, U a
+ * counter-based hash of (seed, beamlet, voxel).  Voxel j = (iz ny + iy) nx + ix, beamlet i = (k n_rows + r) n_cols + c.
+ * Outputs: DEVICE arrays owned by the caller afterwards (release each with vmat_engine_free), beamlet-major CSR with
+ * strictly ascending voxel ids in a row, ready for vmat_create with mem_space = VMAT_DEVICE.  Synchronises the stream
+ * once (the number of entries decides the allocation).  Input generation only: none of the method's arithmetic.     */
+typedef struct {
+    int32_t nx, ny, nz;          /* voxel grid, x fastest                                        */
+    double  voxel_mm;
+    int32_t n_beams, n_rows, n_cols;
+    double  beamlet_mm;
+    double  body_radius_mm, mu_per_mm, sigma_beamlets, noise, cutoff;
+    uint64_t seed;
+} vmat_engine_geometry;
+int vmat_engine_dose_matrix(const vmat_engine_geometry *geometry, void *cuda_stream, int64_t **row_ptr_dev,
+                            int32_t **col_idx_dev, float **val_dev, int64_t *nnz);
+int vmat_engine_free(void *dev_ptr, void *cuda_stream);
+
 /* Number of kernel launches this plan has issued since vmat_create (bench bookkeeping).     */
 int64_t vmat_launch_count(const vmat_plan *plan);
 

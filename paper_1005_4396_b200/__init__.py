@@ -30,6 +30,7 @@ SYMBOLS = (
     "vmat_price",
     "vmat_price_spmv", "vmat_leaf_search", "vmat_master", "vmat_enforce_dose_rate", "vmat_solve", "vmat_get_plan", "vmat_set_plan",
     "vmat_launch_count", "vmat_last_error", "vmat_release_memory", "vmat_set_dose_rate_bounds",
+    "vmat_engine_dose_matrix", "vmat_engine_free",
 )
 
 _P = C.c_void_p
@@ -81,6 +82,13 @@ class _Info(C.Structure):
                                          "nnz_padded", "n_support", "device_bytes", "pricing_bytes")]
 
 
+class EngineGeometry(C.Structure):
+    _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32), ("voxel_mm", C.c_double),
+                ("n_beams", C.c_int32), ("n_rows", C.c_int32), ("n_cols", C.c_int32), ("beamlet_mm", C.c_double),
+                ("body_radius_mm", C.c_double), ("mu_per_mm", C.c_double), ("sigma_beamlets", C.c_double),
+                ("noise", C.c_double), ("cutoff", C.c_double), ("seed", C.c_uint64)]
+
+
 class VmatError(RuntimeError):
     def __init__(self, code: int, msg: str):
         super().__init__(f"vmat error {code}: {msg}")
@@ -117,6 +125,11 @@ def load_library():
     L.vmat_launch_count.argtypes = [_P]
     L.vmat_release_memory.argtypes = []
     L.vmat_set_dose_rate_bounds.argtypes = [_P, C.c_double, C.c_double]
+    L.vmat_engine_dose_matrix.argtypes = [C.POINTER(EngineGeometry), _P, C.POINTER(_P), C.POINTER(_P), C.POINTER(_P),
+                                          C.POINTER(C.c_int64)]
+    L.vmat_engine_dose_matrix.restype = C.c_int
+    L.vmat_engine_free.argtypes = [_P, _P]
+    L.vmat_engine_free.restype = C.c_int
     L.vmat_launch_count.restype = C.c_int64
     L.vmat_last_error.argtypes = [_P]
     L.vmat_last_error.restype = C.c_char_p
@@ -134,6 +147,47 @@ def release_memory() -> None:
     rc = load_library().vmat_release_memory()
     if rc != 0:
         raise RuntimeError(f"vmat_release_memory failed ({rc})")
+
+
+class EngineMatrix:
+    """D as vmat_engine_dose_matrix left it on the device.  row_ptr / col_idx / val are CUDA torch tensors that view
+    the library's buffers (no copy); release() hands the buffers back.  Marshalling only."""
+
+    def __init__(self, geometry: EngineGeometry, stream: Optional[int] = None):
+        import torch
+
+        L = load_library()
+        if stream is None:
+            if not torch.cuda.is_available():
+                raise VmatError(VMAT_ECUDA, "no CUDA device (there is no CPU fallback)")
+            stream = torch.cuda.current_stream().cuda_stream
+        self._stream = stream
+        rp, ci, va, nnz = _P(), _P(), _P(), C.c_int64(0)
+        rc = L.vmat_engine_dose_matrix(C.byref(geometry), _P(stream), C.byref(rp), C.byref(ci), C.byref(va), C.byref(nnz))
+        if rc != VMAT_OK:
+            raise VmatError(rc, (L.vmat_last_error(None) or b"").decode())
+        self._ptrs = (rp.value, ci.value, va.value)
+        self.nnz = int(nnz.value)
+        B = geometry.n_beams * geometry.n_rows * geometry.n_cols
+        self.n_beamlets = B
+
+        def view(ptr, n, dtype, typestr):
+            class _Arr:   # __cuda_array_interface__ carrier: torch wraps the memory without copying
+                pass
+            a = _Arr()
+            a.__cuda_array_interface__ = {"shape": (n,), "typestr": typestr, "data": (ptr, False), "version": 3}
+            return torch.as_tensor(a, device="cuda")
+
+        self.row_ptr = view(rp.value, B + 1, None, "<i8")
+        self.col_idx = view(ci.value, max(self.nnz, 1), None, "<i4")[:self.nnz]
+        self.val = view(va.value, max(self.nnz, 1), None, "<f4")[:self.nnz]
+
+    def release(self):
+        L = load_library()
+        for ptr in self._ptrs:
+            L.vmat_engine_free(_P(ptr), _P(self._stream))
+        self._ptrs = ()
+        self.row_ptr = self.col_idx = self.val = None
 
 
 def default_options() -> Options:

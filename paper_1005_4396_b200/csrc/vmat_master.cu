@@ -1610,7 +1610,13 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(const MasterArgs a
                     hit = 0;
                     ++backtracks;
                     state = kRunTrial;
-                    if (++half >= 60) {
+                    if (-t * phi1 <= stall_threshold(Phi) * fabs(Phi)) {
+                        // whatever shorter step might pass the test, it cannot lower the cost by more than -t phi'(0),
+                        // which is below what fp32 dose arithmetic resolves: the solve has ended (measured on configs[4]:
+                        // without this, late solves spent 35 halvings per step on a slope lost in the noise of the cost)
+                        stop = 4;
+                        state = kFinish;
+                    } else if (++half >= 60) {
                         stop = 3;
                         state = kFinish;
                     } else prepare_trial();
@@ -2409,6 +2415,10 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
             }
             t *= 0.5;
             ++backtracks;
+            if (-t * slope <= stall_threshold(Phi) * fabs(Phi)) {   // no shorter step can lower the cost by more than fp32 resolves
+                stop = 4;
+                break;
+            }
             if (++half >= 40) {
                 stop = 3;
                 break;
@@ -2605,7 +2615,7 @@ int master_configure(vmat_plan *p) {
     // costs every group of every pass a round trip
     const int64_t ngroups = (nchunks + grid * kGroup - 1) / (grid * kGroup);
     int64_t rslots = ngroups * kGroup * kChunk;
-    if (rslots * 7 * 4 > 128 * 1024) rslots = 0;
+    if (rslots * (newton ? 7 : 6) * 4 > 128 * 1024) rslots = 0;
     p->master_rslots = (int)rslots;
     // what is left of the SM's opt-in shared memory (minus static use and room for L1) holds the tile of Dd
     const bool mode = newton;

@@ -592,6 +592,33 @@ def test_occupied_only_smoothing_option(torch_cuda, vm, tiny_phantom, mode):
         q.destroy()
 
 
+def test_mixed_resolution_phantom_runs_through_the_same_path(torch_cuda, vm):
+    """unspecified tissue at twice the voxel size (vmat_inputs.make_phantom(mixed_resolution=True)): a
+    support whose voxels carry penalty weights 1 x and 8 x.  Every step teacher-forced along the oracle's trajectory,
+    then the free run."""
+    import vmat_inputs
+    from oracle import Oracle
+
+    ph = vmat_inputs.make_phantom("tiny", seed=0, mixed_resolution=True)
+    o = Oracle.from_phantom(ph)
+    plan = vm.Plan.from_phantom(ph)
+    for occ, left, right, y in oracle_states(o, 12, every=6):
+        check_dose(torch_cuda, plan, o, occ, left, right, y, 0)
+        check_dose(torch_cuda, plan, o, occ, left, right, y, 1)
+        _, w = o.penalty(o.dose(occ, left, right, y))
+        check_prices(torch_cuda, plan, o, w, occ)
+        check_search(torch_cuda, plan, o, occ, left, right, y, o.prices(w, occ).astype(np.float32))
+        if occ.any():
+            check_master(plan, o, occ, left, right, np.zeros(o.N))
+    occ_r, left_r, right_r, y_r, z_r, tr = o.solve(40)
+    fresh = vm.Plan.from_phantom(ph)
+    st = fresh.solve(40)
+    occ, left, right, y = fresh.get_plan()
+    check_free_run_against_oracle(o, st, (occ, left, right, y), tr, lambda n: o.solve(n)[:4] if n else o.empty_plan())
+    plan.destroy()
+    fresh.destroy()
+
+
 def test_solve_stop_when_priced_out_option(torch_cuda, vm):
     """Option of reading S5: vmat_solve ends as soon as no aperture has a negative price; the default goes on until
     every beam holds an aperture.  Same stop iteration, apertures and cost as the oracle's."""
@@ -740,6 +767,51 @@ def test_enforce_dose_rate_matches_oracle(torch_cuda, vm, tiny_oracle, tiny_solu
     st = plan.enforce_dose_rate(1e-9 * r0, max_rounds=2)
     assert st["rounds"] == 2 and not st["feasible"] and st["gamma"] == o.gamma * 4.0
     plan.destroy()
+
+
+# ------------------------------------------------------------------------------------------------
+# D on the device (stand-in for the paper's GPU dose engine)
+# ------------------------------------------------------------------------------------------------
+def test_device_dose_engine_matches_the_host_generator(torch_cuda, vm, tiny_phantom):
+    """vmat_engine_dose_matrix evaluates the model of DESIGN.md section 5 on the GPU; vmat_inputs evaluates it on the
+    host.  Same pattern and values up to the ulp of exp / sin / cos: entries that differ sit at the cutoff, values agree
+    to fp32 rounding.  The oracle, fed the DEVICE matrix, and a plan created from it without leaving the device agree
+    like any other input (the same D feeds both sides)."""
+    import vmat_inputs
+    from oracle import Oracle
+
+    ph = tiny_phantom
+    c = ph.config
+    nx, ny, nz = c.grid
+    g = vm.EngineGeometry(nx, ny, nz, c.voxel_mm, c.n_beams, c.n_rows, c.n_cols, c.beamlet_mm,
+                          vmat_inputs.body_radius_mm(c), 0.05, 0.6, 0.02, 1e-3, ph.seed)
+    eng = vm.EngineMatrix(g)
+    rp, ci, va = eng.row_ptr.cpu().numpy(), eng.col_idx.cpu().numpy(), eng.val.cpu().numpy()
+    assert rp[0] == 0 and rp[-1] == eng.nnz and np.all(np.diff(rp) >= 0)
+    D_dev = sp.csr_matrix((va.astype(np.float64), ci, rp), shape=(ph.n_beamlets, ph.n_voxels))
+    D_host = sp.csr_matrix((ph.val.astype(np.float64), ph.col_idx, ph.row_ptr), shape=(ph.n_beamlets, ph.n_voxels))
+    diff = abs(D_dev - D_host)
+    assert abs(eng.nnz - ph.nnz) <= 1e-4 * ph.nnz
+    assert diff.max() <= 2e-3 * D_host.max()                    # an entry present on one side only is at the 1e-3 cutoff
+    both = D_dev.multiply(D_host != 0)
+    rel = abs(both - D_host.multiply(D_dev != 0))
+    assert rel.max() <= 1e-6 * D_host.max()
+    for i in range(0, ph.n_beamlets, 97):                        # strictly ascending voxel ids in every sampled row
+        assert np.all(np.diff(ci[rp[i]:rp[i + 1]]) > 0)
+    # a plan straight from the device arrays, the oracle on the same matrix
+    T, al, be = (torch_cuda.from_numpy(a).cuda() for a in (ph.T, ph.alpha, ph.beta))
+    plan = vm.Plan.create(eng.row_ptr, eng.col_idx, eng.val, T, al, be, ph.theta_deg, c.n_rows, c.n_cols,
+                          c.max_leaf_travel, c.gamma)
+    o = Oracle(rp, ci, va, ph.T, ph.alpha, ph.beta, ph.theta_deg, c.n_rows, c.n_cols, c.max_leaf_travel, c.gamma)
+    st = plan.solve(8)
+    occ_r, left_r, right_r, y_r, z_r, tr = o.solve(8)
+    occ, left, right, y = plan.get_plan()
+    check_free_run_against_oracle(o, st, (occ, left, right, y), tr, lambda n: o.solve(n)[:4] if n else o.empty_plan())
+    plan.destroy()
+    eng.release()
+    with pytest.raises(vm.VmatError):
+        vm.EngineMatrix(vm.EngineGeometry(0, ny, nz, c.voxel_mm, c.n_beams, c.n_rows, c.n_cols, c.beamlet_mm, 80.0, 0.05,
+                                          0.6, 0.02, 1e-3, 0))
 
 
 # ------------------------------------------------------------------------------------------------

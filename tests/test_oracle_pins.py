@@ -781,6 +781,36 @@ def test_solve_resumes_from_a_plan(tiny_oracle, tiny_solution):
 # ------------------------------------------------------------------------------------------------
 # shapes of the synthetic stand-ins vs. the paper's Table 1 (context only)
 # ------------------------------------------------------------------------------------------------
+def test_mixed_resolution_phantom_conserves_dose_and_penalty(tiny_phantom):
+    """Input preprocessing of PAPER.md:131 (unspecified tissue at twice the voxel size): the coarse column of D is the
+    mean of its eight fine columns, so every beamlet deposits the same dose x volume; a dose that is constant on every
+    coarsened block costs the same on both grids (weights x 8); structures keep their voxels."""
+    import vmat_inputs
+
+    ph = tiny_phantom
+    pm = vmat_inputs.make_phantom("tiny", seed=0, mixed_resolution=True)
+    assert pm.n_voxels < 0.5 * ph.n_voxels and pm.n_beamlets == ph.n_beamlets
+    assert set(np.unique(pm.volume)) == {1.0, 8.0}
+    D = sp.csr_matrix((ph.val.astype(np.float64), ph.col_idx, ph.row_ptr), shape=(ph.n_beamlets, ph.n_voxels))
+    Dm = sp.csr_matrix((pm.val.astype(np.float64), pm.col_idx, pm.row_ptr), shape=(pm.n_beamlets, pm.n_voxels))
+    np.testing.assert_allclose(Dm @ pm.volume.astype(np.float64), np.asarray(D.sum(axis=1)).ravel(), rtol=1e-6)
+    assert np.all(np.diff(pm.col_idx)[np.diff(np.repeat(np.arange(pm.n_beamlets), np.diff(pm.row_ptr))) == 0] > 0)
+    # structures are untouched: as many target / organ-at-risk voxels as before, all of volume 1
+    for T, al in ((1.0, 1.0), (0.3, 0.0)):
+        fine = (ph.T == np.float32(T)) & (ph.alpha == np.float32(al)) & (ph.beta > 0.1)
+        mix = (pm.T == np.float32(T)) & (pm.alpha == np.float32(al)) & (pm.beta > 0.1) & (pm.volume == 1.0)
+        assert fine.sum() == mix.sum() > 0
+    # the penalty of a uniform dose is the same on both grids
+    for zc in (0.2, 0.7):
+        Ff, _ = orc.penalty(np.full(ph.n_voxels, zc), ph.T, ph.alpha, ph.beta)
+        Fm, _ = orc.penalty(np.full(pm.n_voxels, zc), pm.T, pm.alpha, pm.beta)
+        assert Fm == pytest.approx(Ff, rel=1e-6)
+    # the loop runs on it and keeps its invariants
+    o = Oracle.from_phantom(pm)
+    occ, left, right, y, z, tr = o.solve(6)
+    assert tr.iters == 6 and np.all(np.diff(tr.cost) <= 1e-9 * tr.cost[:-1])
+
+
 def test_phantom_shape_is_in_the_range_of_table1():
     import os
 

@@ -167,6 +167,7 @@ class Phantom:
     theta_deg: np.ndarray      # float64 [N]
     body: np.ndarray           # bool [V]
     structures: List[Structure] = field(default_factory=list)
+    volume: Optional[np.ndarray] = None   # float32 [V]: fine voxels a voxel stands for (mixed resolution), None = all 1
 
     @property
     def nnz(self) -> int:
@@ -216,8 +217,59 @@ def paint_structures(cfg: PhantomConfig, seed: int = 0):
     return T.reshape(-1), alpha.reshape(-1), beta.reshape(-1), np.ascontiguousarray(body).reshape(-1), structs
 
 
-def make_phantom(config="tiny", seed: int = 0, check_reach: bool = True) -> Phantom:
-    """Build a phantom (structures + D).  `config` is a name in CONFIGS or a PhantomConfig."""
+def coarsen_unspecified_tissue(ph: "Phantom") -> "Phantom":
+    """Mixed voxel resolution ("For unspecified tissue ... we increased the voxel size in each dimension
+    by a factor of 2 to reduce the optimization problem size"): every 2 x 2 x 2 block of the grid whose eight voxels all
+    carry the config's `other` parameters (or all lie outside the body) becomes ONE voxel.  Its column of D is the mean
+    of the eight columns (the dose of the coarse voxel), its penalty weights are 8 x (it stands for eight voxels'
+    worth of volume), T is unchanged.  Voxels of blocks that touch a structure or the body contour stay as they are.
+    Voxel ids keep the raster order of the fine grid (a coarse voxel sits where its first fine voxel sat).  This is
+    input preprocessing only: none of the method's arithmetic."""
+    cfg = ph.config
+    nx, ny, nz = cfg.grid
+    assert nx % 2 == 0 and ny % 2 == 0 and nz % 2 == 0, "mixed resolution needs even grid dimensions"
+    V = ph.n_voxels
+    To, ao, bo = (np.float32(v) for v in cfg.other)
+    tissue = (ph.T == To) & (ph.alpha == ao) & (ph.beta == bo) & ph.body
+    outside = (ph.T == 0) & (ph.alpha == 0) & (ph.beta == 0) & ~ph.body
+
+    def blocks(mask):
+        return mask.reshape(nz // 2, 2, ny // 2, 2, nx // 2, 2).all(axis=(1, 3, 5))
+
+    merge = blocks(tissue) | blocks(outside)                         # [nz/2, ny/2, nx/2]
+    merge_fine = np.repeat(np.repeat(np.repeat(merge, 2, 0), 2, 1), 2, 2).reshape(-1)
+    idx = np.arange(V).reshape(nz, ny, nx)
+    first = (idx[0::2, 0::2, 0::2])                                  # first fine voxel of every block
+    first_fine = np.repeat(np.repeat(np.repeat(first, 2, 0), 2, 1), 2, 2).reshape(-1)
+    rep = np.where(merge_fine, first_fine, np.arange(V))             # representative fine voxel of every voxel
+    keep = rep == np.arange(V)
+    new_id = np.cumsum(keep) - 1
+    col_new = new_id[rep[ph.col_idx]]
+    scale = np.where(merge_fine[ph.col_idx], np.float64(0.125), np.float64(1.0))
+    rows = np.repeat(np.arange(ph.n_beamlets, dtype=np.int64), np.diff(ph.row_ptr))
+    Vn = int(keep.sum())
+    key = rows * Vn + col_new
+    order = np.argsort(key, kind="stable")
+    key_s = key[order]
+    val_s = ph.val[order].astype(np.float64) * scale[order]
+    start = np.flatnonzero(np.concatenate([[True], key_s[1:] != key_s[:-1]])) if key_s.size else np.zeros(0, np.int64)
+    val_n = np.add.reduceat(val_s, start).astype(np.float32) if key_s.size else np.zeros(0, np.float32)
+    key_u = key_s[start] if key_s.size else key_s
+    row_u, col_u = key_u // Vn, (key_u % Vn).astype(np.int32)
+    row_ptr = np.zeros(ph.n_beamlets + 1, np.int64)
+    np.add.at(row_ptr, row_u + 1, 1)
+    row_ptr = np.cumsum(row_ptr)
+    w8 = np.where(merge_fine[keep], np.float32(8.0), np.float32(1.0))
+    return Phantom(cfg, ph.seed, Vn, ph.n_beamlets, row_ptr, col_u, val_n, ph.T[keep].copy(),
+                   (ph.alpha[keep] * w8).astype(np.float32), (ph.beta[keep] * w8).astype(np.float32), ph.theta_deg,
+                   ph.body[keep].copy(), ph.structures, w8)
+
+
+def make_phantom(config="tiny", seed: int = 0, check_reach: bool = True, mixed_resolution: bool = False) -> Phantom:
+    """Build a phantom (structures + D).  `config` is a name in CONFIGS or a PhantomConfig.  mixed_resolution: coarsen
+    the unspecified tissue by a factor of 2 per dimension (coarsen_unspecified_tissue)."""
+    if mixed_resolution:
+        return coarsen_unspecified_tissue(make_phantom(config, seed, check_reach))
     cfg = CONFIGS[config] if isinstance(config, str) else config
     lib = _load()
     nx, ny, nz = cfg.grid
