@@ -40,8 +40,8 @@ def load_peaks():
 # A number cited from a committed capture, not measured by the run that prints it: `ncu --set full` of k_price_spmv on
 # configs[1], dram__bytes_read.sum + dram__bytes_write.sum of the FIRST pricing launch of a plan (all 180 beams
 # un-occupied; 994,678,664 algorithmic bytes).  The kernel and the layout of D have not changed since that capture.
-NCU_TRAFFIC_BYTES_FIRST_LAUNCH = {"prostate": 992094720 + 4436224}
-NCU_TRAFFIC_SOURCE = "profiles/r01j_price_spmv.md (ncu --set full, commit d77c9b3)"
+NCU_TRAFFIC_BYTES_FIRST_LAUNCH = {"prostate": 992094976 + 4541440}
+NCU_TRAFFIC_SOURCE = "profiles/r02_price_spmv.md (ncu --set full of k_price_spmv<16,4,128>, round 2)"
 
 
 class ClockSampler:
@@ -292,6 +292,8 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--master-mode", type=int, default=None, choices=[0, 1],
                     help="vmat_options.master_mode: 0 conjugate directions, 1 Newton on the reduced problem (the library's default)")
+    ap.add_argument("--d-format", type=int, default=None, choices=[0, 1],
+                    help="vmat_options.d_format: 0 fp32 CSR (the headline layout), 1 aligned slot pairs with 16-bit ids")
     ap.add_argument("--sweep", action="store_true", help="configs[3]: isolated pricing / search kernel sweep")
     ap.add_argument("--sweep-nnz", default="5e7,1e8,2.5e8,5e8,1e9")
     ap.add_argument("--sweep-voxels", default="1048576,2097152,4194304")
@@ -335,6 +337,8 @@ def main():
         opt.record_phases = record_phases
         if args.master_mode is not None:
             opt.master_mode = args.master_mode
+        if args.d_format is not None:
+            opt.d_format = args.d_format
         return vm.Plan.create(*[t.numpy() for t in host], ph.theta_deg, c.n_rows, c.n_cols, c.max_leaf_travel, c.gamma,
                               options=opt)
 
@@ -462,7 +466,8 @@ def main():
     phases = {k + "_us_per_step": v for k, v in ph_us.items()}
     phases["master_inner_iterations_per_step"] = inner_total / args.steps
     info = {"nnz": plan.nnz, "nnz_padded": plan.nnz_padded, "support_voxels": plan.n_support,
-            "device_bytes": plan.device_bytes}
+            "device_bytes": plan.device_bytes, "d_format": int(args.d_format or 0), "pricing_bytes": plan.pricing_bytes,
+            "pricing_bytes_per_entry": plan.pricing_bytes / max(plan.nnz, 1)}
     plan.destroy()
 
     # ---- end-to-end leg from pinned host buffers ----------------------------------------------------

@@ -361,7 +361,7 @@ int launch_direct_dose(vmat_plan *p) {
                                                             p->dose_list);
     if (p->B > 0) {
         // a fixed grid (a few blocks per SM) walks the list: its length is known on the device only
-        const unsigned blocks = (unsigned)(p->sm_count * 6);
+        const unsigned blocks = (unsigned)(p->sm_count * 6);   // (16 per SM measured the same: the reductions bound the pass)
         VMAT_CUDA(p, launch_pdl(k_dose_scatter, dim3(blocks), dim3(kDoseThreads), p->stream, p->rowq, p->val4, p->col4, p->y,
                                 (int)p->RC, ds, p->dose_list, p->acc));
     }
