@@ -153,6 +153,17 @@ def test_teacher_forced_steps_stress():
         _, _, cost1 = plan.dose(z1)
         assert relnorm(z1.cpu().numpy(), z_ref) <= TOL
         assert abs(cost1 - (F_ref + o.gamma * G_ref)) <= TOL * abs(F_ref + o.gamma * G_ref)
+        # P3 on a short prefix: the oracle's own free run over the first 8 iterations against vmat_solve(8)
+        from test_gpu_parity import check_free_run_against_oracle
+
+        n = 8
+        occ_r, left_r, right_r, y_r, z_r, tr = o.solve(n, eps=1e-9)
+        e = o.empty_plan()
+        plan.set_plan(e[0], e[1], e[2], e[3])
+        st = plan.solve(n)
+        occ, left, right, y = plan.get_plan()
+        check_free_run_against_oracle(o, st, (occ, left, right, y), tr,
+                                      lambda m: o.solve(m, eps=1e-9)[:4] if m else o.empty_plan())
     finally:
         s[4].destroy()
 
