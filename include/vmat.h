@@ -295,6 +295,23 @@ int vmat_engine_dose_matrix(const vmat_engine_geometry *geometry, void *cuda_str
                             int32_t **col_idx_dev, float **val_dev, int64_t *nnz);
 int vmat_engine_free(void *dev_ptr, void *cuda_stream);
 
+/* Step (b) alone, allocation free (Eq. 1): w_j = dF/dz_j and F = sum_j alpha_j max(0, T_j - z_j)^2 +
+ * beta_j max(0, z_j - T_j)^2 for a caller's dose vector, for callers that cannot call cudaMalloc (code under CUDA graph
+ * capture, tight serving loops).  No plan is needed and nothing is allocated, by this call or by a library routine under
+ * it: the per-block partial sums of F live in a fixed array in the library's device image (64 KB + 256 B, held by every
+ * GPU that loads the library until the process exits), which bounds the size: n_voxels > VMAT_NOALLOC_MAX_VOXELS returns
+ * VMAT_EINVAL and launches nothing.
+ *   z_dev, T_dev, alpha_dev, beta_dev   DEVICE, n_voxels floats, memory of the CURRENT device (checked for z_dev)
+ *   w_dev   DEVICE n_voxels floats or NULL;  F_dev   DEVICE one double or NULL (not both NULL)
+ * Stream-ordered on cuda_stream, no host synchronisation; F is summed in a fixed order (the same bits every call).
+ * Every call on a device shares that device's array, which keeps the last call's contents (the call clears what must
+ * start at zero): two calls that OVERLAP on one GPU (different streams, or two graphs in flight) race on it and give a
+ * wrong F - serialise them.  The first call on a device looks the array's address up (cudaGetSymbolAddress): make it
+ * outside stream capture.  Errors: VMAT_EINVAL / VMAT_ECUDA, text from vmat_last_error(NULL).                       */
+#define VMAT_NOALLOC_MAX_VOXELS (1 << 24)
+int vmat_penalty_noalloc(const float *z_dev, const float *T_dev, const float *alpha_dev, const float *beta_dev,
+                         int64_t n_voxels, float *w_dev, double *F_dev, void *cuda_stream);
+
 /* Number of kernel launches this plan has issued since vmat_create (bench bookkeeping).     */
 int64_t vmat_launch_count(const vmat_plan *plan);
 

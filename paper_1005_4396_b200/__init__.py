@@ -30,7 +30,7 @@ SYMBOLS = (
     "vmat_price",
     "vmat_price_spmv", "vmat_leaf_search", "vmat_master", "vmat_enforce_dose_rate", "vmat_solve", "vmat_get_plan", "vmat_set_plan",
     "vmat_launch_count", "vmat_last_error", "vmat_release_memory", "vmat_set_dose_rate_bounds",
-    "vmat_engine_dose_matrix", "vmat_engine_free",
+    "vmat_engine_dose_matrix", "vmat_engine_free", "vmat_penalty_noalloc",
 )
 
 _P = C.c_void_p
@@ -130,6 +130,8 @@ def load_library():
     L.vmat_engine_dose_matrix.restype = C.c_int
     L.vmat_engine_free.argtypes = [_P, _P]
     L.vmat_engine_free.restype = C.c_int
+    L.vmat_penalty_noalloc.argtypes = [_P, _P, _P, _P, C.c_int64, _P, _P, _P]
+    L.vmat_penalty_noalloc.restype = C.c_int
     L.vmat_launch_count.restype = C.c_int64
     L.vmat_last_error.argtypes = [_P]
     L.vmat_last_error.restype = C.c_char_p
@@ -258,6 +260,27 @@ def _dev_ptr(t, dtype_name: str, n: Optional[int] = None) -> int:
     if n is not None and t.numel() != n:
         raise ValueError(f"expected {n} elements, got {t.numel()}")
     return t.data_ptr()
+
+
+NOALLOC_MAX_VOXELS = 1 << 24   # VMAT_NOALLOC_MAX_VOXELS of include/vmat.h
+
+
+def penalty_noalloc(z, T, alpha, beta, w=None, F=None, stream: Optional[int] = None) -> None:
+    """vmat_penalty_noalloc: step (b) on a caller's dose, allocating nothing (its scratch is a fixed array in the
+    library's device image: at most NOALLOC_MAX_VOXELS voxels, calls that overlap on one GPU race).  z, T, alpha, beta:
+    CUDA float32[n]; w: CUDA float32[n] or None; F: CUDA float64[1] or None.  Stream-ordered (default: torch's current
+    stream); argument marshalling only."""
+    import torch
+
+    n = int(z.numel())
+    if stream is None:
+        stream = torch.cuda.current_stream().cuda_stream
+    L = load_library()
+    rc = L.vmat_penalty_noalloc(_dev_ptr(z, "float32", n), _dev_ptr(T, "float32", n), _dev_ptr(alpha, "float32", n),
+                                _dev_ptr(beta, "float32", n), n, _dev_ptr(w, "float32", n), _dev_ptr(F, "float64", 1),
+                                _P(stream))
+    if rc < 0:
+        raise VmatError(rc, (L.vmat_last_error(None) or b"").decode())
 
 
 class Plan:
