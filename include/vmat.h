@@ -105,7 +105,10 @@ typedef struct {
                                       one thread block solves the K-dimensional box-constrained quadratic by conjugate
                                       gradients on its faces, the other blocks evaluate the true cost and gradient at
                                       the point it proposes: two or three passes per solve instead of about twenty.
-                                      Needs n_beams <= 256 and N^2 floats of shared memory; otherwise mode 0 runs.   */
+                                      Needs n_beams <= 512 (one thread per beam) and, at each launch, K <= 256 occupied
+                                      beams whose K x K fp32 matrix fits the block's shared memory next to 14 N
+                                      doubles (K <= about 200 at N = 360); a launch past that runs mode 0's kernel from
+                                      the point the solve before it left, and so does every launch after it.          */
     int32_t stop_when_priced_out; /* vmat_solve stops as soon as the best aperture's price is >= 0 (the textbook
                                   column-generation stop).  Default 0: the loop goes on until every beam holds an
                                   aperture, as the paper wants (reading S5).  With 1 the
@@ -120,6 +123,9 @@ typedef struct {
                                   derivative of G with its beam put into the arc, a beam that enters at y_k = 0 changes
                                   G, and the post-master cost of vmat_solve is no longer guaranteed non-increasing.
                                   vmat_enforce_dose_rate tests all N - 1 successive pairs in either reading.          */
+    int32_t master_newton_max_beams; /* 0 (default): mode 1 runs while the occupied beams fit its solving block (above);
+                                  > 0: and while there are at most this many of them (lets a small test reach the
+                                  hand-over to mode 0's kernel; same minimiser either way).                          */
 } vmat_options;
 
 /* One deliverable aperture: a beam and one leaf pair per row. */

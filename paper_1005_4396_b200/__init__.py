@@ -46,7 +46,8 @@ class Options(C.Structure):
     _fields_ = [("validate", C.c_int32), ("d_format", C.c_int32), ("dose_path", C.c_int32),
                 ("master_eps", C.c_double), ("master_max_inner", C.c_int32), ("master_stall_rel", C.c_double),
                 ("master_stall_count", C.c_int32), ("record_phases", C.c_int32), ("master_mode", C.c_int32), ("stop_when_priced_out", C.c_int32),
-                ("master_unstaged_lists", C.c_int32), ("occupied_only_G", C.c_int32)]
+                ("master_unstaged_lists", C.c_int32), ("occupied_only_G", C.c_int32),
+                ("master_newton_max_beams", C.c_int32)]
 
 
 class _Aperture(C.Structure):

@@ -139,6 +139,7 @@ void vmat_default_options(vmat_options *opt) {
     opt->stop_when_priced_out = 0;
     opt->master_unstaged_lists = 1;
     opt->occupied_only_G = 0;
+    opt->master_newton_max_beams = 0;
 }
 
 int vmat_create(const vmat_problem *pb, const vmat_options *options, void *cuda_stream, vmat_plan **out) {
@@ -412,7 +413,7 @@ int vmat_master(vmat_plan *p, const vmat_master_opts *opts, vmat_master_stats *o
         if (opts->stall_rel > 0.0) p->opt.master_stall_rel = opts->stall_rel;
         if (opts->stall_count > 0) p->opt.master_stall_count = opts->stall_count;
     }
-    rc = launch_master(p, -1, 0);
+    rc = launch_master(p, -1, 0, (int)(p->N - unoccupied(p)));
     p->opt = keep;
     if (rc) return rc;
     p->state_valid = true;
@@ -466,7 +467,7 @@ int vmat_enforce_dose_rate(vmat_plan *p, double rho, double factor, double tol, 
     while (ratio > 1.0 + tol && rounds < max_rounds) {
         p->gamma *= factor;                          // "gamma ... will be automatically increased"
         if (!std::isfinite(p->gamma)) return fail(p, VMAT_ESTATE, "gamma overflowed while enforcing the dose-rate limit");
-        if ((rc = launch_master(p, -1, 0))) return rc;  // "the intensity for each aperture will be re-optimized"
+        if ((rc = launch_master(p, -1, 0, (int)(p->N - unoccupied(p))))) return rc;  // "the intensity for each aperture will be re-optimized"
         MasterOut h;
         VMAT_CUDA(p, cudaMemcpyAsync(&h, p->mout, sizeof(MasterOut), cudaMemcpyDeviceToHost, p->stream));
         if ((rc = test(ratio))) return rc;           // "till the solution is feasible"
@@ -552,7 +553,7 @@ int vmat_solve(vmat_plan *p, int32_t max_iters, vmat_solve_stats *out) {
         if (phases) TRYC(cudaEventRecord(evs[it * 5 + 2], st));
         TRY(launch_column_build(p, -1));                                           // d_k of the new aperture
         if (phases) TRYC(cudaEventRecord(evs[it * 5 + 3], st));
-        TRY(launch_master(p, (int)it, p->warm_ok ? 1 : 0));                        // (e), leaves z, w current
+        TRY(launch_master(p, (int)it, p->warm_ok ? 1 : 0, (int)(p->N - n_free0 + it + 1)));                      // (e), leaves z, w current
         p->warm_ok = true;
         if (phases) TRYC(cudaEventRecord(evs[it * 5 + 4], st));
         done = it + 1;

@@ -102,14 +102,19 @@ struct vmat_plan {
     int touch_words = 0;
     unsigned int *vbounds = nullptr;   // bit patterns of max|T|, max(alpha, beta)
     float Tmax = 0.f, abmax = 0.f;
-    int master_grid = 0;
-    size_t master_smem = 0;
-    int master_cache_segs = 0;         // 512-byte segments of Dd a master block stages in shared memory
-    int master_rslots = 0;             // slots per master block kept resident in shared memory (0: none)
-    int master_ul_cap = 0;             // capacity of the master's per-chunk lists of unstaged beams (0: masked loops)
+    // launch shape of one master kernel: mcfg[0] k_master, mcfg[1] k_newton (grid == 0: the plan cannot run it)
+    struct MasterCfg {
+        int grid = 0;                  // blocks launched
+        int nblk = 0;                  // blocks that own chunks (k_newton: all but the solving block)
+        size_t smem = 0;               // dynamic shared memory of a working block
+        int cache_segs = 0;            // 512-byte segments of Dd a master block stages in shared memory
+        int rslots = 0;                // slots per master block kept resident in shared memory (0: none)
+        int ul_cap = 0;                // capacity of the per-chunk lists of unstaged beams (0: masked loops)
+    } mcfg[2];
     // mode 1 of the master (k_newton): the Hessian of F over the occupied beams, kept on the device from solve to solve
-    bool master_newton = false;        // the plan runs k_newton (master_mode 1 and the reduced problem fits one block)
-    int master_nblk = 0;               // blocks of the master grid that own chunks (k_newton: all but the solving block)
+    bool master_newton = false;        // the plan can run k_newton (master_mode 1, n_beams <= one thread per beam)
+    int newton_kmax = 0;               // most occupied beams whose reduced problem fits the solving block
+    bool newton_retired = false;       // a solve has outgrown it: H_F is no longer kept up (until the next reset)
     long long *hess = nullptr;         // N x N fixed point
     float *omref = nullptr;            // Sp: the omega (alpha, beta or 0 per slot) the matrix was built with
     uint8_t *hvalid = nullptr;         // N: column k is in the matrix
@@ -216,7 +221,8 @@ int launch_leaf_search(vmat_plan *p, const float *g, int32_t *all_left, int32_t 
 int master_configure(vmat_plan *p);
 int reset_hessian(vmat_plan *p);
 int launch_column_build(vmat_plan *p, int beam /* -1: read p->sel */);
-int launch_master(vmat_plan *p, int trace_it, int warm /* 1: inside vmat_solve, right after a committed search */);
+int launch_master(vmat_plan *p, int trace_it, int warm /* 1: inside vmat_solve, right after a committed search */,
+                  int k_occ /* occupied beams at the launch, or an upper bound of them */);
 int launch_expand(vmat_plan *p, const float *src_s, float *dst_V, int what /*0 z, 1 w*/);
 int launch_compress(vmat_plan *p, const float *src_V, float *dst_s);
 int launch_rate_ratio(vmat_plan *p, double rho, double *ratio_dev);

@@ -164,9 +164,9 @@ k_column_finish(unsigned long long *__restrict__ acc, long long Sp, const Sel *_
         }
     }
     // ---- the new column's row of the Hessian (mode 1) ------------------------------------------------
-    if (hr.hess == nullptr || !*hr.hlive || N > 256) return;   // the same for the whole grid
+    if (hr.hess == nullptr || !*hr.hlive || N > kMasterThreads) return;   // the same for the whole grid
     if (blockIdx.x == 0 && threadIdx.x == 0) hr.hvalid[k] = 1;   // (no block reads the flag of k itself)
-    __shared__ int s_live[2], s_cnt[2], s_list[2][256];
+    __shared__ int s_live[2], s_cnt[2], s_list[2][kMasterThreads];
     __shared__ float4 s_u[2][kChunk / 4], s_d[2][kChunk / 4];
     const int lane = threadIdx.x & 31, half = threadIdx.x >> 7;   // warps 0-3: the block's first chunk, 4-7: its second
     const int sl = threadIdx.x & (kChunk - 1);
@@ -178,11 +178,12 @@ k_column_finish(unsigned long long *__restrict__ acc, long long Sp, const Sel *_
     if (__any_sync(kFull, u != 0.f) && lane == 0) s_live[half] = 1;
     __syncthreads();
     // the columns in the matrix that touch the chunk (any order: what each adds is an integer)
-    if ((int)threadIdx.x < N && (int)threadIdx.x != k && hr.occ[threadIdx.x] && hr.hvalid[threadIdx.x]) {
-        const uint32_t *tw = touch + (size_t)threadIdx.x * touch_words;
+    for (int i = threadIdx.x; i < N; i += 256) {
+        if (i == k || !hr.occ[i] || !hr.hvalid[i]) continue;
+        const uint32_t *tw = touch + (size_t)i * touch_words;
         for (int h = 0; h < 2; ++h) {
             const int c = 2 * (int)blockIdx.x + h;
-            if (s_live[h] && (long long)c * kChunk < Sp && ((tw[c >> 5] >> (c & 31)) & 1u)) s_list[h][atomicAdd(&s_cnt[h], 1)] = (int)threadIdx.x;
+            if (s_live[h] && (long long)c * kChunk < Sp && ((tw[c >> 5] >> (c & 31)) & 1u)) s_list[h][atomicAdd(&s_cnt[h], 1)] = i;
         }
     }
     __syncthreads();
@@ -1937,7 +1938,7 @@ __device__ __forceinline__ void newton_pass(const MasterArgs &a, const Smem &sm,
 // ---- the solving block ---------------------------------------------------------------------------------
 constexpr int kSolveRed = 8;   // values per warp row of the solver's reduction scratch
 
-// sums s[0..MS) and one maximum over the block, every thread receives them; fixed order.  Only the first nv <= 8
+// sums s[0..MS) and one maximum over the block, every thread receives them; fixed order.  Only the first nv <= 16
 // warps hold data (one beam per thread); the others skip the first level.
 template <int MS>
 __device__ __forceinline__ void solver_reduce(double (&s)[MS], double &mx, double *buf, int &tog, int nv) {
@@ -1959,31 +1960,31 @@ __device__ __forceinline__ void solver_reduce(double (&s)[MS], double &mx, doubl
         }
     }
     __syncthreads();
-    const int row = lane & 7;   // every group of eight lanes reads the (at most) eight rows
+    const int row = lane & 15;   // each half of a warp reads the (at most) sixteen rows
     const bool in = row < nv;
 #pragma unroll
     for (int m = 0; m < MS; ++m) {
         double v = in ? b[row * kSolveRed + m] : 0.0;
 #pragma unroll
-        for (int o = 4; o; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
+        for (int o = 8; o; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
         s[m] = v;
     }
     double v = in ? b[row * kSolveRed + kSolveRed - 1] : -CUDART_INF;
 #pragma unroll
-    for (int o = 4; o; o >>= 1) v = fmax(v, __shfl_xor_sync(kFull, v, o));
+    for (int o = 8; o; o >>= 1) v = fmax(v, __shfl_xor_sync(kFull, v, o));
     mx = v;
 }
 
 // Sums of the conjugate-gradient step over the block, in fp32 (the iteration corrects itself: the residual is updated
 // with the step actually taken): s[0..MS) are added, mx is maximised, the three low bits of flags are OR-ed.  Only the
-// first nv <= 8 warps hold data; they receive everything, the other warps the flags only (loop control).  One
+// first nv <= 16 warps hold data; they receive everything, the other warps the flags only (loop control).  One
 // barrier; both levels are warp shuffles in a fixed order; the scratch alternates between calls.
 constexpr int kCgRow = 8;   // floats per warp row of the scratch
 template <int MS>
 __device__ __forceinline__ void cg_reduce(float (&s)[MS], float &mx, int &flags, float *buf, int &tog, int nv) {
     static_assert(MS + 2 <= kCgRow, "scratch row too short");
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    float *b = buf + tog * (8 * kCgRow);
+    float *b = buf + tog * (kMasterWarps * kCgRow);
     tog ^= 1;
     if (warp < nv) {
 #pragma unroll
@@ -2001,7 +2002,7 @@ __device__ __forceinline__ void cg_reduce(float (&s)[MS], float &mx, int &flags,
         }
     }
     __syncthreads();
-    const int row = lane & 7;   // every group of eight lanes reads the (at most) eight rows
+    const int row = lane & 15;   // each half of a warp reads the (at most) sixteen rows
     const bool in = row < nv;
     flags = __reduce_or_sync(kFull, in ? __float_as_int(b[row * kCgRow + MS + 1]) : 0);
     if (warp < nv) {
@@ -2009,7 +2010,7 @@ __device__ __forceinline__ void cg_reduce(float (&s)[MS], float &mx, int &flags,
 #pragma unroll
         for (int m = 0; m < MS; ++m) v[m] = in ? b[row * kCgRow + m] : 0.f;
 #pragma unroll
-        for (int o = 4; o; o >>= 1) {
+        for (int o = 8; o; o >>= 1) {
 #pragma unroll
             for (int m = 0; m < MS; ++m) v[m] += __shfl_xor_sync(kFull, v[m], o);
             m2 = fmaxf(m2, __shfl_xor_sync(kFull, m2, o));
@@ -2035,8 +2036,8 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
     int *nxl = freen + N, *pvl = nxl + N;   // neighbours of beam k in Eq. 2 (as in master_setup)
     float *dc = reinterpret_cast<float *>((reinterpret_cast<uintptr_t>(pvl + N) + 15) & ~(uintptr_t)15);   // compact direction
     const int Np = ((N + 3) / 4) | 1;                        // float4s per row at K = N
-    float *cgb = dc + 4 * Np;                                // 2 x 8 x kCgRow floats: scratch of cg_reduce
-    float *hpart = cgb + 2 * 8 * kCgRow;                     // the product with the matrix, and the part of its second half
+    float *cgb = dc + 4 * Np;                                // 2 x kMasterWarps x kCgRow floats: scratch of cg_reduce
+    float *hpart = cgb + 2 * kMasterWarps * kCgRow;                     // the product with the matrix, and the part of its second half
     float *hpart2 = hpart + kMasterThreads / 2;
     float *H32 = hpart2 + kMasterThreads / 2;                // Kp x Kp floats, Kp = 4 Kp4 >= K
     // occupied beams, ascending
@@ -2588,69 +2589,90 @@ size_t master_smem_bytes(int64_t N, int64_t rslots, int64_t cache_segs, int64_t 
 }
 
 // shared memory of k_newton's solving block (newton_solver's carve-up)
-size_t solver_smem_bytes(int64_t N) {
-    const int64_t Np = ((N + 3) / 4) | 1;
+// for N beams of which at most K are occupied
+size_t solver_smem_bytes(int64_t N, int64_t K) {
+    const int64_t Np = ((N + 3) / 4) | 1, Kp = 4 * (((K + 3) / 4) | 1);
     return (size_t)(14 * N + 2 * kMasterWarps * kSolveRed) * 8 + (size_t)6 * N * 4 + 16 + (size_t)4 * Np * 4 +
-           (size_t)(kMasterThreads + 2 * 8 * 8) * 4 + (size_t)4 * Np * 4 * Np * 4;
+           (size_t)(kMasterThreads + 2 * kMasterWarps * kCgRow) * 4 + (size_t)Kp * Kp * 4;
 }
 
 }  // namespace
 
-int master_configure(vmat_plan *p) {
+// launch shape of one of the two master kernels for this plan; cfg->grid stays 0 if it does not fit
+static int configure_kernel(vmat_plan *p, bool newton, size_t budget, vmat_plan::MasterCfg *cfg) {
     const int64_t nchunks = p->Sp / kChunk;
-    int optin = 0;
-    VMAT_CUDA(p, cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, p->device));
-    const size_t budget = (size_t)optin > 8 * 1024 ? (size_t)optin - 8 * 1024 : 0;
-    // mode 1 (k_newton) gives one block of the grid to the reduced problems: its matrix must fit that block's shared
-    // memory and its vectors take one thread per beam; larger problems run mode 0
-    bool newton = p->opt.master_mode == 1 && p->sm_count >= 2 && p->N <= kMasterThreads / 2 && solver_smem_bytes(p->N) <= budget;
-    p->master_newton = newton;
+    *cfg = vmat_plan::MasterCfg();
     int64_t grid = p->sm_count - (newton ? 1 : 0);    // one block per SM, chunks dealt round-robin
     if (grid > nchunks) grid = nchunks;
     if (grid < 1) grid = 1;
-    p->master_nblk = (int)grid;
-    p->master_grid = (int)grid + (newton ? 1 : 0);
     // resident slot data (z, z trial, q, T, alpha, beta of a block's own slots) if it fits in 128 KB: on a large
     // support the tile holds a few per cent of the columns whatever its size, while slot data read from L2 / HBM
     // costs every group of every pass a round trip
     const int64_t ngroups = (nchunks + grid * kGroup - 1) / (grid * kGroup);
     int64_t rslots = ngroups * kGroup * kChunk;
     if (rslots * (newton ? 7 : 6) * 4 > 128 * 1024) rslots = 0;
-    p->master_rslots = (int)rslots;
-    // what is left of the SM's opt-in shared memory (minus static use and room for L1) holds the tile of Dd
-    const bool mode = newton;
     // per-chunk lists of the unstaged beams (one entry per column and local chunk at most) if they fit in 64 KB
     int64_t ul_cap = p->N * ngroups * kGroup;
     if (ul_cap * 2 > 64 * 1024 || p->N > 65535) ul_cap = 0;
     if (!p->opt.master_unstaged_lists) ul_cap = 0;         // option: force the fallback path (tests)
-    size_t fixed = master_smem_bytes(p->N, rslots, 0, ngroups, mode, ul_cap);
+    size_t fixed = master_smem_bytes(p->N, rslots, 0, ngroups, newton, ul_cap);
     if (fixed > budget) {
-        p->master_rslots = 0;
-        fixed = master_smem_bytes(p->N, 0, 0, ngroups, mode, ul_cap);
+        rslots = 0;
+        fixed = master_smem_bytes(p->N, 0, 0, ngroups, newton, ul_cap);
     }
     if (fixed > budget) {
         ul_cap = 0;
-        fixed = master_smem_bytes(p->N, 0, 0, ngroups, mode, 0);
+        fixed = master_smem_bytes(p->N, 0, 0, ngroups, newton, 0);
     }
-    p->master_ul_cap = (int)ul_cap;
-    if (fixed > budget) return fail(p, VMAT_EINVAL, "n_beams too large for the master kernel's shared memory");
-    p->master_cache_segs = (int)((budget - fixed) / seg_bytes(mode));
-    if (p->master_cache_segs > 65535 || ngroups * kGroup > 32767) p->master_cache_segs = 0;   // 16-bit fields of the lists
-    p->master_smem = master_smem_bytes(p->N, p->master_rslots, p->master_cache_segs, ngroups, mode, ul_cap);
-    if (newton && solver_smem_bytes(p->N) > p->master_smem) p->master_smem = solver_smem_bytes(p->N);
+    if (fixed > budget) return VMAT_OK;
+    // what is left of the SM's opt-in shared memory (minus static use and room for L1) holds the tile of Dd
+    int64_t cache_segs = (int64_t)((budget - fixed) / seg_bytes(newton));
+    if (cache_segs > 65535 || ngroups * kGroup > 32767) cache_segs = 0;   // 16-bit fields of the lists
+    cfg->smem = master_smem_bytes(p->N, rslots, cache_segs, ngroups, newton, ul_cap);
+    int per_sm = 0;
+    if (newton) VMAT_CUDA(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_newton, kMasterThreads, cfg->smem));
+    else VMAT_CUDA(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_master, kMasterThreads, cfg->smem));
+    if (per_sm < 1) return VMAT_OK;
+    cfg->nblk = (int)grid;
+    cfg->grid = (int)grid + (newton ? 1 : 0);
+    cfg->rslots = (int)rslots;
+    cfg->ul_cap = (int)ul_cap;
+    cfg->cache_segs = (int)cache_segs;
+    return VMAT_OK;
+}
+
+int master_configure(vmat_plan *p) {
+    const int64_t nchunks = p->Sp / kChunk;
+    int optin = 0;
+    VMAT_CUDA(p, cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, p->device));
+    const size_t budget = (size_t)optin > 8 * 1024 ? (size_t)optin - 8 * 1024 : 0;
     // The attribute is a per-function, per-device setting shared by every plan of the process: it is set to the
     // device's opt-in maximum (the same value from every vmat_create), never to this plan's own size, so that a plan
-    // created later cannot shrink it under a live one.  Each launch passes its own p->master_smem <= optin.
+    // created later cannot shrink it under a live one.  Each launch passes its own size <= optin.
     cudaFuncAttributes fa0, fa1;
     VMAT_CUDA(p, cudaFuncGetAttributes(&fa0, k_master));
     VMAT_CUDA(p, cudaFuncGetAttributes(&fa1, k_newton));
     VMAT_CUDA(p, cudaFuncSetAttribute(k_master, cudaFuncAttributeMaxDynamicSharedMemorySize, optin - (int)fa0.sharedSizeBytes));
     VMAT_CUDA(p, cudaFuncSetAttribute(k_newton, cudaFuncAttributeMaxDynamicSharedMemorySize, optin - (int)fa1.sharedSizeBytes));
-    int per_sm = 0;
-    if (newton) VMAT_CUDA(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_newton, kMasterThreads, p->master_smem));
-    else VMAT_CUDA(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_master, kMasterThreads, p->master_smem));
-    if (per_sm < 1) return fail(p, VMAT_ECUDA, "master kernel does not fit on an SM");
     int rc;
+    if ((rc = configure_kernel(p, false, budget, &p->mcfg[0]))) return rc;
+    if (p->mcfg[0].grid == 0) return fail(p, VMAT_EINVAL, "n_beams too large for the master kernel's shared memory");
+    // mode 1 (k_newton) gives one block of the grid to the reduced problems: its vectors take one thread per beam, the
+    // product with its matrix one thread per occupied beam and half of the columns, and the matrix must fit that
+    // block's shared memory.  The last two bound the number of OCCUPIED beams: a launch with more of them runs k_master.
+    p->newton_kmax = 0;
+    p->newton_retired = false;
+    if (p->opt.master_mode == 1 && p->sm_count >= 2 && p->N <= kMasterThreads) {
+        if ((rc = configure_kernel(p, true, budget, &p->mcfg[1]))) return rc;
+        if (p->mcfg[1].grid > 0) {
+            int64_t kmax = p->N < kMasterThreads / 2 ? p->N : kMasterThreads / 2;
+            while (kmax > 0 && solver_smem_bytes(p->N, kmax) > budget) --kmax;
+            if (p->opt.master_newton_max_beams > 0 && kmax > p->opt.master_newton_max_beams) kmax = p->opt.master_newton_max_beams;
+            p->newton_kmax = (int)kmax;
+        }
+    }
+    const bool newton = p->newton_kmax > 0;
+    p->master_newton = newton;
     if ((rc = dev_alloc(p, &p->accbuf, 3 * kSumGroups * (2 * p->N + 2)))) return rc;
     if ((rc = dev_alloc(p, &p->phase, 2))) return rc;
     if ((rc = dev_alloc(p, &p->mcount, 16))) return rc;
@@ -2708,6 +2730,7 @@ int master_configure(vmat_plan *p) {
 // behind the columns may all have changed)
 int reset_hessian(vmat_plan *p) {
     if (!p->master_newton) return VMAT_OK;
+    p->newton_retired = false;
     VMAT_CUDA(p, cudaMemsetAsync(p->hess, 0, (size_t)p->N * p->N * 8, p->stream));
     VMAT_CUDA(p, cudaMemsetAsync(p->omref, 0, (size_t)p->Sp * 4, p->stream));
     VMAT_CUDA(p, cudaMemsetAsync(p->hvalid, 0, (size_t)p->N, p->stream));
@@ -2735,7 +2758,19 @@ int launch_column_build(vmat_plan *p, int beam) {
     return VMAT_OK;
 }
 
-static int launch_master_impl(vmat_plan *p, int max_inner, int trace_it, int warm) {
+static int launch_master_impl(vmat_plan *p, int max_inner, int trace_it, int warm, int k_occ) {
+    // which kernel: k_newton while the occupied beams (k_occ: an upper bound) fit its solving block.  Past that the
+    // plan runs k_master; H_F is then no longer kept up, so k_column_finish is told to stop adding rows to it.
+    bool newton = p->master_newton && k_occ <= p->newton_kmax;
+    if (p->master_newton && !newton && !p->newton_retired) {
+        VMAT_CUDA(p, cudaMemsetAsync(p->hlive, 0, 4, p->stream));
+        VMAT_CUDA(p, cudaMemsetAsync(p->hvalid, 0, (size_t)p->N, p->stream));
+        p->newton_retired = true;
+    } else if (newton && p->newton_retired) {
+        int rc = reset_hessian(p);   // back under the bound (apertures were removed): the matrix is rebuilt from empty
+        if (rc) return rc;
+    }
+    const vmat_plan::MasterCfg &cfg = p->mcfg[newton ? 1 : 0];
     MasterArgs a;
     a.warm = warm;
     a.sel = p->sel;
@@ -2765,9 +2800,9 @@ static int launch_master_impl(vmat_plan *p, int max_inner, int trace_it, int war
     a.lb = p->y_min;
     a.ub = p->y_max;
     a.max_inner = max_inner;
-    a.rslots = p->master_rslots;
-    a.cache_segs = p->master_cache_segs;
-    a.ul_cap = p->master_ul_cap;
+    a.rslots = cfg.rslots;
+    a.cache_segs = cfg.cache_segs;
+    a.ul_cap = cfg.ul_cap;
     a.colstat = p->colstat;
     a.touch = p->col_touch;
     a.touch_words = p->touch_words;
@@ -2784,7 +2819,7 @@ static int launch_master_impl(vmat_plan *p, int max_inner, int trace_it, int war
     a.trC = p->tr_cost;
     a.trInner = p->tr_inner;
     a.trace_it = trace_it;
-    a.nblk = p->master_nblk;
+    a.nblk = cfg.nblk;
     a.hess = p->hess;
     a.omref = p->omref;
     a.hvalid = p->hvalid;
@@ -2795,15 +2830,16 @@ static int launch_master_impl(vmat_plan *p, int max_inner, int trace_it, int war
     a.mail = (Mail *)p->mail;
     a.sync = p->nsync;
     void *args[] = {&a};
-    const void *fn = p->master_newton ? (const void *)k_newton : (const void *)k_master;
-    VMAT_CUDA(p, cudaLaunchCooperativeKernel(fn, dim3((unsigned)p->master_grid), dim3(kMasterThreads), args,
-                                             p->master_smem, p->stream));
+    const void *fn = newton ? (const void *)k_newton : (const void *)k_master;
+    size_t smem = cfg.smem;
+    if (newton && solver_smem_bytes(p->N, k_occ) > smem) smem = solver_smem_bytes(p->N, k_occ);
+    VMAT_CUDA(p, cudaLaunchCooperativeKernel(fn, dim3((unsigned)cfg.grid), dim3(kMasterThreads), args, smem, p->stream));
     ++p->launches;
     return VMAT_OK;
 }
 
-int launch_master(vmat_plan *p, int trace_it, int warm) {
-    return launch_master_impl(p, p->opt.master_max_inner, trace_it, warm);
+int launch_master(vmat_plan *p, int trace_it, int warm, int k_occ) {
+    return launch_master_impl(p, p->opt.master_max_inner, trace_it, warm, k_occ);
 }
 
 int launch_rate_ratio(vmat_plan *p, double rho, double *ratio_dev) {

@@ -592,6 +592,40 @@ def test_occupied_only_smoothing_option(torch_cuda, vm, tiny_phantom, mode):
         q.destroy()
 
 
+def test_newton_master_hands_over_when_the_arc_outgrows_its_block(torch_cuda, vm, tiny_phantom):
+    """vmat_options.master_mode 1 runs k_newton while the occupied beams fit its solving block and k_master from then on
+    (master_newton_max_beams makes a small arc reach the hand-over): the free run is the oracle's across the switch, in
+    one call or split around it, and a plan brought back under the bound goes back to k_newton from an empty matrix."""
+    from oracle import Oracle
+
+    o = Oracle.from_phantom(tiny_phantom)
+    opt = mode_options(vm, 1)
+    opt.master_newton_max_beams = 7
+    occ_r, left_r, right_r, y_r, z_r, tr = o.solve(40)
+    states = lambda n: o.solve(n)[:4] if n else o.empty_plan()
+    plan = make_plan(vm, o, options=opt)
+    st = plan.solve(40)
+    got = plan.get_plan()
+    assert st.iters == o.N and got[0].all()
+    check_free_run_against_oracle(o, st, got, tr, states)
+    split = make_plan(vm, o, options=opt)
+    a = split.solve(5)
+    b = split.solve(4)      # 9 occupied beams: the switch falls inside this call
+    c = split.solve(40)
+    assert (a.iters, b.iters, c.iters) == (5, 4, o.N - 9)
+    assert a.master_cg_steps > 0 and b.master_cg_steps > 0 and c.master_cg_steps == 0    # which kernel ran
+    occ, left, right, y = split.get_plan()
+    assert np.array_equal(left, got[1]) and np.array_equal(right, got[2])
+    assert np.max(np.abs(y - got[3])) <= TIE * max(1.0, np.max(np.abs(y)))
+    assert abs(c.cost - st.cost) <= TIE * abs(st.cost)
+    # back under the bound: the master of a 6-beam plan (k_newton again) against the oracle's
+    occ6, left6, right6, y6 = states(6)
+    split.set_plan(occ6, left6, right6, y6 * 0.5)
+    check_master(split, o, occ6, left6, right6, y6 * 0.5)
+    plan.destroy()
+    split.destroy()
+
+
 def test_mixed_resolution_phantom_runs_through_the_same_path(torch_cuda, vm):
     """unspecified tissue at twice the voxel size (vmat_inputs.make_phantom(mixed_resolution=True)): a
     support whose voxels carry penalty weights 1 x and 8 x.  Every step teacher-forced along the oracle's trajectory,
