@@ -106,8 +106,8 @@ typedef struct {
                                       gradients on its faces, the other blocks evaluate the true cost and gradient at
                                       the point it proposes: two or three passes per solve instead of about twenty.
                                       Needs n_beams <= 512 (one thread per beam) and, at each launch, K <= 256 occupied
-                                      beams whose K x K fp32 matrix fits the block's shared memory next to 14 N
-                                      doubles (K <= about 200 at N = 360); a launch past that runs mode 0's kernel from
+                                      beams whose K x K fp32 matrix fits the block's shared memory next to 11 N
+                                      doubles (K <= 212 at N = 360); a launch past that runs mode 0's kernel from
                                       the point the solve before it left, and so does every launch after it.          */
     int32_t stop_when_priced_out; /* vmat_solve stops as soon as the best aperture's price is >= 0 (the textbook
                                   column-generation stop).  Default 0: the loop goes on until every beam holds an

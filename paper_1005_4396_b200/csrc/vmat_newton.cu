@@ -331,11 +331,11 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
     // vectors over the beams (fp64), then the matrix (fp32, K x Kp, Kp / 4 odd: rows 16-byte aligned and conflict free
     // for one thread per row), then the maps
     double *vy = reinterpret_cast<double *>(smem_raw);
-    double *vg = vy + N, *yc = vg + N, *vr = yc + N, *vd = vr + N, *vHd = vd + N, *vpo = vHd + N, *vyn = vpo + N;
+    double *vg = vy + N, *yc = vg + N, *vd = yc + N, *vyn = vd + N;
     double *vgn = vyn + N, *vp = vgn + N, *linf = vp + N, *rdt = linf + N, *Minv = rdt + N, *dGb = Minv + N;
     double *redb = dGb + N;                                  // 2 x kMasterWarps x kSolveRed
-    int *sk = reinterpret_cast<int *>(redb + 2 * kMasterWarps * kSolveRed), *ik = sk + N, *freeo = ik + N, *freen = freeo + N;
-    int *nxl = freen + N, *pvl = nxl + N;   // neighbours of beam k in Eq. 2 (as in master_setup)
+    int *sk = reinterpret_cast<int *>(redb + 2 * kMasterWarps * kSolveRed), *ik = sk + N;
+    int *nxl = ik + N, *pvl = nxl + N;   // neighbours of beam k in Eq. 2 (as in master_setup)
     float *dc = reinterpret_cast<float *>((reinterpret_cast<uintptr_t>(pvl + N) + 15) & ~(uintptr_t)15);   // compact direction
     const int Np = ((N + 3) / 4) | 1;                        // float4s per row at K = N
     float *cgb = dc + 4 * Np;                                // 2 x kMasterWarps x kCgRow floats: scratch of cg_reduce
@@ -531,10 +531,7 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
         for (int e = tid; e < (Kp - K) * Kp; e += kMasterThreads) H32[(size_t)K * Kp + e] = 0.f;   // rows K..Kp-1 (read with d = 0)
         for (int k = tid; k < N; k += kMasterThreads) {
             yc[k] = vy[k];
-            vr[k] = vg[k];
             vd[k] = 0.0;
-            vpo[k] = 0.0;
-            freeo[k] = 0;
         }
         for (int i = tid; i < Kp; i += kMasterThreads) dc[i] = 0.f;
         __syncthreads();
@@ -879,7 +876,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_newton(const MasterArgs a
 // for N beams of which at most K are occupied
 size_t solver_smem_bytes(int64_t N, int64_t K) {
     const int64_t Np = ((N + 3) / 4) | 1, Kp = 4 * (((K + 3) / 4) | 1);
-    return (size_t)(14 * N + 2 * kMasterWarps * kSolveRed) * 8 + (size_t)6 * N * 4 + 16 + (size_t)4 * Np * 4 +
+    return (size_t)(11 * N + 2 * kMasterWarps * kSolveRed) * 8 + (size_t)4 * N * 4 + 16 + (size_t)4 * Np * 4 +
            (size_t)(kMasterThreads + 2 * kMasterWarps * kCgRow) * 4 + (size_t)Kp * Kp * 4;
 }
 
