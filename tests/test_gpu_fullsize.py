@@ -64,6 +64,10 @@ def test_free_run_matches_oracle_fullsize(setup):
     torch, vm, ph, o, plan = setup
     n = o.N
     occ_r, left_r, right_r, y_r, z_r, tr = o.solve(n, eps=1e-9)
+    # the stored copy of this run (tests/golden/fullsize_run_prostate.txt) is the oracle's as it stands
+    g = _stored_run("prostate")
+    assert np.array_equal(g.beam, tr.beam) and np.array_equal(g.left, tr.left) and np.array_equal(g.right, tr.right)
+    assert relnorm(g.cost, tr.cost) <= 1e-9
     e = o.empty_plan()
     plan.set_plan(e[0], e[1], e[2], e[3])
     st = plan.solve(n)
@@ -88,6 +92,55 @@ def test_free_run_prefix_matches_oracle_head_and_neck(setup_hn):
     occ, left, right, y = plan.get_plan()
     check_free_run_against_oracle(o, st, (occ, left, right, y), tr,
                                   lambda m: o.solve(m, eps=1e-9)[:4] if m else o.empty_plan())
+
+
+def _stored_run(name):
+    """tests/golden/fullsize_run_<name>.txt (written by tests/golden/make_fullsize_runs.py from the oracle alone)."""
+    import os
+    import types
+
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", f"fullsize_run_{name}.txt")
+    beam, price, F, G, cost, left, right, y = [], [], [], [], [], [], [], None
+    for line in open(path):
+        if line.startswith("#"):
+            continue
+        if line.startswith("y "):
+            y = np.array([float(v) for v in line.split()[1:]])
+            continue
+        head, l, r = line.split("|")
+        h = head.split()
+        assert int(h[0]) == len(beam)
+        beam.append(int(h[1]))
+        price.append(float(h[2]))
+        F.append(float(h[3]))
+        G.append(float(h[4]))
+        cost.append(float(h[5]))
+        left.append([int(v) for v in l.split()])
+        right.append([int(v) for v in r.split()])
+    return types.SimpleNamespace(iters=len(beam), beam=np.array(beam, np.int32), price=np.array(price), F=np.array(F),
+                                 G=np.array(G), cost=np.array(cost), left=np.array(left, np.int32),
+                                 right=np.array(right, np.int32), y=y)
+
+
+def test_whole_plan_matches_the_stored_oracle_run_head_and_neck(setup_hn):
+    """P3 at BASELINE.json configs[2] over the WHOLE plan: the oracle's own free run of all 180 iterations takes minutes
+    of host time, so it is stored (tests/golden/fullsize_run_hn.txt, written by tests/golden/make_fullsize_runs.py, which
+    calls only oracle/): vmat_solve(180) must pick the same beams and leaf pairs with the cost trace within 1e-4, or part
+    from it at a tie within fp32 noise (then the live oracle is run up to that iteration for its prices)."""
+    from test_gpu_parity import check_free_run_against_oracle
+
+    torch, vm, ph, o, plan = setup_hn
+    tr = _stored_run("hn")
+    assert tr.iters == o.N
+    e = o.empty_plan()
+    plan.set_plan(e[0], e[1], e[2], e[3])
+    st = plan.solve(o.N)
+    occ, left, right, y = plan.get_plan()
+    assert st.iters == o.N and occ.all()
+    it = check_free_run_against_oracle(o, st, (occ, left, right, y), tr,
+                                       lambda m: o.solve(m, eps=1e-9)[:4] if m else o.empty_plan())
+    if it < 0:
+        assert np.max(np.abs(y - tr.y)) <= 1e-4 * np.max(tr.y)
 
 
 @pytest.mark.parametrize("seed", [0, 1, 2, 3])
