@@ -163,8 +163,8 @@ __device__ __forceinline__ void take_better(double &bp, int &bk, double op, int 
 
 template <int M>
 __global__ void __launch_bounds__(kSearchThreads) k_leaf_search(const SearchArgs a) {
-    pdl_wait();      // the prices (launched behind the pricing product by programmatic dependent launch)
-    pdl_trigger();   // the column build may be scheduled; it waits for the choice itself
+    // Launched behind the pricing product by programmatic dependent launch: everything up to pdl_wait() below runs
+    // while that grid drains and may read only what earlier launches of the stream left (occupancy, leaves), not g.
     __shared__ int s_km, s_kp, s_last, s_bad;
     __shared__ unsigned long long s_total;
     __shared__ double s_price[kRowsPerBlock];
@@ -177,6 +177,10 @@ __global__ void __launch_bounds__(kSearchThreads) k_leaf_search(const SearchArgs
     const bool occupied = a.occ[k] != 0;
     if (occupied && rb > 0) return;                               // block 0 of an occupied beam reports +inf
     bool beam_done = false;                                       // this block finishes its beam (thread 0)
+    if (occupied) {
+        pdl_wait();
+        pdl_trigger();
+    }
 
     if (!occupied) {
         if (tid == 0) {
@@ -202,8 +206,8 @@ __global__ void __launch_bounds__(kSearchThreads) k_leaf_search(const SearchArgs
         __syncthreads();
         const int km = s_km, kp = s_kp;
         const int r = rb * kRowsPerBlock + warp;
+        int Lmin = 0, Lmax = C, Rmin = 0, Rmax = C;
         if (r < R) {
-            int Lmin = 0, Lmax = C, Rmin = 0, Rmax = C;
             if (km >= 0) {
                 const int b = a.delta * (k - km), l = a.left[km * R + r], rr = a.right[km * R + r];
                 Lmin = max(Lmin, l - b);
@@ -218,6 +222,10 @@ __global__ void __launch_bounds__(kSearchThreads) k_leaf_search(const SearchArgs
                 Rmin = max(Rmin, rr - b);
                 Rmax = min(Rmax, rr + b);
             }
+        }
+        pdl_wait();      // the prices
+        pdl_trigger();   // the column build may be scheduled; it waits for the choice itself
+        if (r < R) {
             long long value;
             int bl, br;
             row_search_warp<M>(a.g + ((size_t)k * R + r) * C, C, Lmin, Lmax, Rmin, Rmax, lane, value, bl, br);
