@@ -1,9 +1,9 @@
 """Writes tests/golden/fullsize_run_<config>.txt: the ORACLE's own free run (oracle.Oracle.solve, fp64, eps = 1e-9) of
 the whole column-generation loop of PAPER.md:111-117 on a full-size seeded phantom (BASELINE.json configs[1] "prostate",
-configs[2] "hn"; seed 0), one line per iteration: the beam chosen, its price, F, G, F + gamma G after the master solve,
+configs[2] "hn", configs[4] "stress"; seed 0; 102 s, 271 s and 2508 s on 8 cores), one line per iteration: the beam chosen, its price, F, G, F + gamma G after the master solve,
 and the leaf pairs of the committed aperture.
 
-    python tests/golden/make_fullsize_runs.py [prostate] [hn]
+    python tests/golden/make_fullsize_runs.py [prostate] [hn] [stress]     (default: prostate hn)
 
 It imports only `oracle` and `vmat_inputs` (never the CUDA package): the stored values are the oracle's.  The GPU test
 tests/test_gpu_fullsize.py::test_whole_plan_matches_the_stored_oracle_run compares the device's whole run with them,

@@ -33,7 +33,7 @@ def load(name):
     return meta, rows, y
 
 
-@pytest.mark.parametrize("name", ["prostate", "hn"])
+@pytest.mark.parametrize("name", ["prostate", "hn", "stress"])
 def test_stored_run_is_a_run_of_the_loop(name):
     meta, rows, y = load(name)
     N, R, C, gamma, delta = int(meta["N"]), int(meta["R"]), int(meta["C"]), meta["gamma"], int(meta["delta"])

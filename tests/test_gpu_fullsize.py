@@ -217,6 +217,21 @@ def test_teacher_forced_steps_stress():
         occ, left, right, y = plan.get_plan()
         check_free_run_against_oracle(o, st, (occ, left, right, y), tr,
                                       lambda m: o.solve(m, eps=1e-9)[:4] if m else o.empty_plan())
+        # P3 over the WHOLE plan: all 360 iterations against the oracle's stored run (42 minutes of oracle on 8 cores:
+        # tests/golden/fullsize_run_stress.txt, written by tests/golden/make_fullsize_runs.py from oracle/ alone).  The
+        # first 212 master solves run k_newton, the other 148 k_master (observed: the same 360 apertures, cost traces
+        # 1.4e-9 apart).  The stored run's first 8 iterations are the live oracle's above.
+        g = _stored_run("stress")
+        assert g.iters == o.N and np.array_equal(g.beam[:n], tr.beam) and np.array_equal(g.left[:n], tr.left)
+        assert np.array_equal(g.right[:n], tr.right) and relnorm(g.cost[:n], tr.cost) <= 1e-9
+        plan.set_plan(e[0], e[1], e[2], e[3])
+        st = plan.solve(o.N)
+        occ, left, right, y = plan.get_plan()
+        assert st.iters == o.N and occ.all()
+        it = check_free_run_against_oracle(o, st, (occ, left, right, y), g,
+                                           lambda m: o.solve(m, eps=1e-9)[:4] if m else o.empty_plan())
+        if it < 0:
+            assert np.max(np.abs(y - g.y)) <= 1e-4 * np.max(g.y)
     finally:
         s[4].destroy()
 
