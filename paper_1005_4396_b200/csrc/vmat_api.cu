@@ -130,7 +130,7 @@ void vmat_default_options(vmat_options *opt) {
     opt->validate = 1;
     opt->d_format = 0;
     opt->dose_path = 0;
-    opt->master_eps = 1e-5;
+    opt->master_eps = 1e-4;
     opt->master_max_inner = 500;
     opt->master_stall_rel = 1e-6;    // 100x inside the 1e-4 parity tolerance on the master cost (S11)
     opt->master_stall_count = 2;
@@ -179,7 +179,7 @@ int vmat_create(const vmat_problem *pb, const vmat_options *options, void *cuda_
     };
     if (options) p->opt = *options;
     else vmat_default_options(&p->opt);
-    if (!(p->opt.master_eps > 0.0)) p->opt.master_eps = 1e-5;
+    if (!(p->opt.master_eps > 0.0)) p->opt.master_eps = 1e-4;
     if (p->opt.master_max_inner < 0) p->opt.master_max_inner = 0;
     if (!(p->opt.master_stall_rel >= 0.0)) p->opt.master_stall_rel = 1e-6;
     if (p->opt.master_stall_count < 1) p->opt.master_stall_count = 2;
