@@ -87,7 +87,8 @@ typedef struct {
                                   about 0.8 x the memory of D on top.                                    */
     int32_t dose_path;         /* how vmat_dose forms z: 0 from the aperture-dose columns d_k the
                                   master keeps (default), 1 straight from D (fixed-point atomics)  */
-    double  master_eps;        /* stop when max|projected gradient| <= eps*max(1, value at entry) */
+    double  master_eps;        /* stop when max|projected gradient| <= eps*max(1, value at entry);
+                                  default 1e-4 (S11: chosen against whole plans of the oracle) */
     int32_t master_max_inner;  /* cap on inner iterations of one master solve                     */
     double  master_stall_rel;  /* a step that lowers the cost by <= this fraction of it is a stall:
                                   the decrease is below what fp32 dose arithmetic resolves.  Once a
@@ -234,7 +235,7 @@ typedef struct {
 /* Step (e): solve model (3) for y >= 0 over the occupied beams, warm-started
  * from the plan's y.  Leaves z, w current.  opts may be NULL (the plan's options); out may be NULL.
  * y is kept in double precision on both sides of the boundary: the dose rates carry the plan from one
- * solve to the next, and fp32 would add 6e-8 relative noise per hand-over to a 1e-5 stop test.      */
+ * solve to the next, and fp32 would add 6e-8 relative noise per hand-over to a 1e-4 stop test.        */
 int vmat_master(vmat_plan *plan, const vmat_master_opts *opts, vmat_master_stats *out);
 
 /* The column-generation loop (S5): up to max_iters iterations of
