@@ -705,6 +705,35 @@ def test_solve_is_reproducible(torch_cuda, vm, tiny_oracle, mode):
         assert np.array_equal(a, b)
 
 
+@pytest.mark.parametrize("mode", [0, 1])
+def test_two_live_plans_interleaved_give_what_each_gives_alone(torch_cuda, vm, tiny_oracle, mode):
+    """Two plans of different shapes alive in one process, their loops advanced in turns: the master kernels' opt-in
+    shared-memory attribute is one per-function, per-device setting (every plan sets it to the device maximum, each launch
+    passes its own size), and mode 1 keeps its hand-over counters and its reduced Hessian per plan.  Each plan must end
+    exactly where it ends when it runs alone."""
+    small = random_problem(47, V=500, N=11, R=3, C=13, gamma=0.2)
+    alone = []
+    for o in (tiny_oracle, small):
+        p = make_plan(vm, o, options=mode_options(vm, mode))
+        st = p.solve(40)
+        alone.append((st.cost, p.get_plan()))
+        p.destroy()
+    a = make_plan(vm, tiny_oracle, options=mode_options(vm, mode))
+    b = make_plan(vm, small, options=mode_options(vm, mode))
+    done_a = done_b = 0
+    while done_a < tiny_oracle.N or done_b < small.N:
+        if done_a < tiny_oracle.N:
+            done_a += a.solve(3).iters
+        if done_b < small.N:
+            done_b += b.solve(2).iters
+    for p, (cost, ref) in ((a, alone[0]), (b, alone[1])):
+        got = p.get_plan()
+        assert np.array_equal(got[1], ref[1]) and np.array_equal(got[2], ref[2])      # the same apertures
+        assert np.max(np.abs(got[3] - ref[3])) <= TIE * max(1.0, np.max(np.abs(ref[3])))
+        assert abs(p.dose()[2] - cost) <= TIE * abs(cost)
+        p.destroy()
+
+
 def test_device_resident_inputs_give_the_same_plan(torch_cuda, vm, tiny_phantom, tiny_oracle):
     o = tiny_oracle
     a = make_plan(vm, o)
