@@ -626,6 +626,23 @@ def test_newton_master_hands_over_when_the_arc_outgrows_its_block(torch_cuda, vm
     split.destroy()
 
 
+def test_arc_of_more_beams_than_the_newton_master_takes(torch_cuda, vm):
+    """n_beams = 520 > 512: master_mode 1 cannot give one thread to every beam, the plan runs k_master throughout (and the
+    leaf search and the beam choice take several trips of their 256-thread loops over beams).  A short free run against
+    the oracle's, then teacher-forced master solves on its states."""
+    o = random_problem(61, V=260, N=520, R=2, C=7, density=0.2, gamma=0.05, delta=3)
+    plan = make_plan(vm, o)
+    n = 30
+    occ_r, left_r, right_r, y_r, z_r, tr = o.solve(n)
+    st = plan.solve(n)
+    got = plan.get_plan()
+    assert st.iters == n and st.master_cg_steps == 0                      # k_master, not k_newton
+    check_free_run_against_oracle(o, st, got, tr, lambda m: o.solve(m)[:4] if m else o.empty_plan())
+    check_master(plan, o, occ_r, left_r, right_r, y_r * 0.5)
+    check_master(plan, o, occ_r, left_r, right_r, np.zeros(o.N))
+    plan.destroy()
+
+
 def test_mixed_resolution_phantom_runs_through_the_same_path(torch_cuda, vm):
     """unspecified tissue at twice the voxel size (vmat_inputs.make_phantom(mixed_resolution=True)): a
     support whose voxels carry penalty weights 1 x and 8 x.  Every step teacher-forced along the oracle's trajectory,
