@@ -336,7 +336,9 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
     double *redb = dGb + N;                                  // 2 x kMasterWarps x kSolveRed
     int *sk = reinterpret_cast<int *>(redb + 2 * kMasterWarps * kSolveRed), *ik = sk + N;
     int *nxl = ik + N, *pvl = nxl + N;   // neighbours of beam k in Eq. 2 (as in master_setup)
-    float *dc = reinterpret_cast<float *>((reinterpret_cast<uintptr_t>(pvl + N) + 15) & ~(uintptr_t)15);   // compact direction
+    int *pk = pvl + N;                   // row / column of beam k in H32 (free beams first: see the Newton loop), -1 if un-occupied
+    int *pp = pk + N;                    // the same for the i-th occupied beam: pp[i] = pk[sk[i]]
+    float *dc = reinterpret_cast<float *>((reinterpret_cast<uintptr_t>(pp + N) + 15) & ~(uintptr_t)15);   // direction, in H32's order
     const int Np = ((N + 3) / 4) | 1;                        // float4s per row at K = N
     float *cgb = dc + 4 * Np;                                // 2 x kMasterWarps x kCgRow floats: scratch of cg_reduce
     float *hpart = cgb + 2 * kMasterWarps * kCgRow;                     // the product with the matrix, and the part of its second half
@@ -498,8 +500,34 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
 
     // ---- Newton iterations ------------------------------------------------------------------------------
     while (state != kFinish && !stop && pgmax > tol) {
-        // the matrix of the current piece: H32 = H_F over the occupied beams
+        // The matrix of the current piece: H32 = H_F over the occupied beams, the beams that are FREE at this point first
+        // (ascending), the ones held at a bound after them: the direction of the conjugate gradients is zero at a held
+        // beam, so the product with the matrix walks the columns of the free beams only (about half of an arc's beams
+        // sit at y = 0), up to the last beam released since.
         const long long c0 = clock64();
+        __shared__ int s_nA, s_cF[kMasterWarps], s_cH[kMasterWarps];
+        {
+            const int k = tid;                               // one beam per thread (N <= kMasterThreads)
+            const bool on = k < N && ik[k] >= 0, fre = on && !at_bound(vy[k], vg[k]);
+            const unsigned mF = __ballot_sync(kFull, fre), mH = __ballot_sync(kFull, on && !fre), lt = (1u << lane) - 1u;
+            if (lane == 0) {
+                s_cF[warp] = __popc(mF);
+                s_cH[warp] = __popc(mH);
+            }
+            __syncthreads();
+            int bF = 0, bH = 0, nF = 0;
+#pragma unroll
+            for (int w2 = 0; w2 < kMasterWarps; ++w2) {
+                const int cf = s_cF[w2], ch = s_cH[w2];
+                if (w2 < warp) bF += cf, bH += ch;
+                nF += cf;
+            }
+            const int p = fre ? bF + __popc(mF & lt) : (on ? nF + bH + __popc(mH & lt) : -1);
+            if (k < N) pk[k] = p;
+            if (on) pp[ik[k]] = p;
+            if (tid == 0) s_nA = nF;
+        }
+        __syncthreads();
         {
             const int npair = K * (K + 1) / 2;
             for (int e0 = 0; e0 < npair; e0 += 8 * kMasterThreads) {
@@ -523,8 +551,9 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
                 for (int u = 0; u < 8; ++u)
                     if (ri[u] >= 0) {
                         const float f = (float)((double)v[u] * a.hinv);
-                        H32[ri[u] * Kp + ci[u]] = f;
-                        H32[ci[u] * Kp + ri[u]] = f;
+                        const int pr = pp[ri[u]], pc = pp[ci[u]];
+                        H32[pr * Kp + pc] = f;
+                        H32[pc * Kp + pr] = f;
                     }
             }
         }
@@ -536,7 +565,7 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
         for (int i = tid; i < Kp; i += kMasterThreads) dc[i] = 0.f;
         __syncthreads();
         for (int k = tid; k < N; k += kMasterThreads) {
-            const int i = ik[k];
+            const int i = pk[k];
             double m = 0.0;
             if (i >= 0) m = 2.0 * (double)H32[i * Kp + i] + 2.0 * a.gamma * ((pvl[k] >= 0 ? rdt[pvl[k]] : 0.0) + rdt[k]);
             Minv[k] = m > 0.0 ? 1.0 / m : 1.0;
@@ -555,6 +584,7 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
         const double qtol = fmax(0.5 * tol, 0.05 * pgmax);
         const int k = tid;                                   // this thread's beam (k < N: checked on the host)
         const bool mine = k < N && ik[k] >= 0;
+        const int myp = mine ? pk[k] : 0;                    // this beam's row and column of H32
         const int nv = (N + 31) / 32;                        // warps that hold beams
         auto ratio = [](double num, double den) { return (double)__fdividef((float)num, (float)den); };
         __shared__ int s_fl[2];
@@ -581,7 +611,7 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
         int fl = any_flags(fabs(prk) > qtol ? 2 : 0);
         while ((fl & 2) && !(fl & 4) && it < maxcg) {
             if (k < N) vd[k] = dk;
-            if (mine) dc[ik[k]] = (float)dk;
+            if (mine) dc[myp] = (float)dk;
             __syncthreads();
             ++cg_steps;
             ++it;
@@ -590,7 +620,8 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
             // d_c is the same word for the whole warp.  Two halves: threads 0..255 and 256..511.
             {
                 const int r = tid & (kMasterThreads / 2 - 1), h = tid / (kMasterThreads / 2);
-                const int q0 = h * ((Kp4 + 1) / 2), q1 = min(Kp4, q0 + (Kp4 + 1) / 2);   // float4s of d of this half
+                const int nA4 = (s_nA + 3) / 4;              // float4s of d that can hold a non-zero entry
+                const int q0 = h * ((nA4 + 1) / 2), q1 = min(nA4, q0 + (nA4 + 1) / 2);   // float4s of d of this half
                 float acc0 = 0.f, acc1 = 0.f;
                 if (r < K) {
                     const float4 *d4 = reinterpret_cast<const float4 *>(dc);
@@ -615,7 +646,7 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
                 const int nx = nxl[k], pv = pvl[k];
                 const double e1 = nx >= 0 ? (vd[nx] - dk) * rdt[k] : 0.0;
                 const double e0 = pv >= 0 ? (dk - vd[pv]) * rdt[pv] : 0.0;
-                hdk = 2.0 * (double)hpart[ik[k]] + 2.0 * a.gamma * (e0 - e1);
+                hdk = 2.0 * (double)hpart[myp] + 2.0 * a.gamma * (e0 - e1);
                 s5[0] = (float)(dk * hdk);
                 s5[1] = (float)(rk * dk);
                 if (fr) {
@@ -655,6 +686,7 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
             }
             const int fn = mine && !at_bound(yk, rk);
             prk = fn ? rk : 0.0;
+            if (fn && !fr) atomicMax(&s_nA, myp + 1);        // a released beam: its column joins the product (read after the barrier)
             fl = any_flags(warp >= nv ? 0 : (fn != fr || hit || t == 0.0 ? 1 : 0) | (fabs(prk) > qtol ? 2 : 0) | (halt ? 4 : 0));
             // (only the warps that hold beams know the sums; `halt` and the rest of the loop control travel as flags)
             beta = (fl & 1) || !(s5[2] > 0.f) ? 0.0 : (double)fmaxf(0.f, __fdividef((float)t * (s5[3] + (float)t * s5[4]), s5[2]));
@@ -876,7 +908,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_newton(const MasterArgs a
 // for N beams of which at most K are occupied
 size_t solver_smem_bytes(int64_t N, int64_t K) {
     const int64_t Np = ((N + 3) / 4) | 1, Kp = 4 * (((K + 3) / 4) | 1);
-    return (size_t)(11 * N + 2 * kMasterWarps * kSolveRed) * 8 + (size_t)4 * N * 4 + 16 + (size_t)4 * Np * 4 +
+    return (size_t)(11 * N + 2 * kMasterWarps * kSolveRed) * 8 + (size_t)6 * N * 4 + 16 + (size_t)4 * Np * 4 +
            (size_t)(kMasterThreads + 2 * kMasterWarps * kCgRow) * 4 + (size_t)Kp * Kp * 4;
 }
 
