@@ -336,8 +336,8 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
     double *redb = dGb + N;                                  // 2 x kMasterWarps x kSolveRed
     int *sk = reinterpret_cast<int *>(redb + 2 * kMasterWarps * kSolveRed), *ik = sk + N;
     int *nxl = ik + N, *pvl = nxl + N;   // neighbours of beam k in Eq. 2 (as in master_setup)
-    int *pk = pvl + N;                   // row / column of beam k in H32 (free beams first: see the Newton loop), -1 if un-occupied
-    int *pp = pk + N;                    // the same for the i-th occupied beam: pp[i] = pk[sk[i]]
+    int *pk = pvl + N;                   // row / column of beam k in H32 (the free beams of a Newton step: see its loop), else -1
+    int *pp = pk + N;                    // the beam of row p
     float *dc = reinterpret_cast<float *>((reinterpret_cast<uintptr_t>(pp + N) + 15) & ~(uintptr_t)15);   // direction, in H32's order
     const int Np = ((N + 3) / 4) | 1;                        // float4s per row at K = N
     float *cgb = dc + 4 * Np;                                // 2 x kMasterWarps x kCgRow floats: scratch of cg_reduce
@@ -500,36 +500,34 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
 
     // ---- Newton iterations ------------------------------------------------------------------------------
     while (state != kFinish && !stop && pgmax > tol) {
-        // The matrix of the current piece: H32 = H_F over the occupied beams, the beams that are FREE at this point first
-        // (ascending), the ones held at a bound after them: the direction of the conjugate gradients is zero at a held
-        // beam, so the product with the matrix walks the columns of the free beams only (about half of an arc's beams
-        // sit at y = 0), up to the last beam released since.
+        // The face of this Newton step: the occupied beams that are not at a bound with the gradient pointing outwards.
+        // The model is solved on it (a beam that reaches a bound on the way stays there; a held beam is released, if
+        // the TRUE gradient says so, when the next step forms its face), so only the free beams take part: H32 = H_F
+        // over the free beams, in ascending order (about half of an arc's beams sit at y = 0 and are left out).
         const long long c0 = clock64();
-        __shared__ int s_nA, s_cF[kMasterWarps], s_cH[kMasterWarps];
+        __shared__ int s_nF, s_cF[kMasterWarps];
         {
             const int k = tid;                               // one beam per thread (N <= kMasterThreads)
-            const bool on = k < N && ik[k] >= 0, fre = on && !at_bound(vy[k], vg[k]);
-            const unsigned mF = __ballot_sync(kFull, fre), mH = __ballot_sync(kFull, on && !fre), lt = (1u << lane) - 1u;
-            if (lane == 0) {
-                s_cF[warp] = __popc(mF);
-                s_cH[warp] = __popc(mH);
-            }
+            const bool fre = k < N && ik[k] >= 0 && !at_bound(vy[k], vg[k]);
+            const unsigned mF = __ballot_sync(kFull, fre);
+            if (lane == 0) s_cF[warp] = __popc(mF);
             __syncthreads();
-            int bF = 0, bH = 0, nF = 0;
+            int bF = 0, nFt = 0;
 #pragma unroll
             for (int w2 = 0; w2 < kMasterWarps; ++w2) {
-                const int cf = s_cF[w2], ch = s_cH[w2];
-                if (w2 < warp) bF += cf, bH += ch;
-                nF += cf;
+                const int cf = s_cF[w2];
+                if (w2 < warp) bF += cf;
+                nFt += cf;
             }
-            const int p = fre ? bF + __popc(mF & lt) : (on ? nF + bH + __popc(mH & lt) : -1);
-            if (k < N) pk[k] = p;
-            if (on) pp[ik[k]] = p;
-            if (tid == 0) s_nA = nF;
+            const int p = fre ? bF + __popc(mF & ((1u << lane) - 1u)) : -1;
+            if (k < N) pk[k] = p;                            // row / column of beam k in H32, -1 if it is not free
+            if (fre) pp[p] = k;                              // and the beam of row p
+            if (tid == 0) s_nF = nFt;
         }
         __syncthreads();
+        const int nF = s_nF, nF4 = (nF + 3) / 4;
         {
-            const int npair = K * (K + 1) / 2;
+            const int npair = nF * (nF + 1) / 2;
             for (int e0 = 0; e0 < npair; e0 += 8 * kMasterThreads) {
                 long long v[8];
                 int ri[8], ci[8];
@@ -538,26 +536,25 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
                     const int e = e0 + u * kMasterThreads + tid;
                     ri[u] = -1;
                     v[u] = 0;
-                    if (e < npair) {   // row i of the upper triangle starts at i K - i (i - 1) / 2
-                        int i = (int)((2.0f * K + 1.0f - sqrtf((2.0f * K + 1.0f) * (2.0f * K + 1.0f) - 8.0f * (float)e)) * 0.5f);
-                        while (i > 0 && i * K - i * (i - 1) / 2 > e) --i;
-                        while ((i + 1) * K - (i + 1) * i / 2 <= e) ++i;
+                    if (e < npair) {   // row i of the upper triangle starts at i nF - i (i - 1) / 2
+                        int i = (int)((2.0f * nF + 1.0f - sqrtf((2.0f * nF + 1.0f) * (2.0f * nF + 1.0f) - 8.0f * (float)e)) * 0.5f);
+                        while (i > 0 && i * nF - i * (i - 1) / 2 > e) --i;
+                        while ((i + 1) * nF - (i + 1) * i / 2 <= e) ++i;
                         ri[u] = i;
-                        ci[u] = i + e - (i * K - i * (i - 1) / 2);
-                        v[u] = __ldcg(a.hess + (size_t)sk[i] * N + sk[ci[u]]);
+                        ci[u] = i + e - (i * nF - i * (i - 1) / 2);
+                        v[u] = __ldcg(a.hess + (size_t)pp[i] * N + pp[ci[u]]);   // pp ascending: the upper triangle
                     }
                 }
 #pragma unroll
                 for (int u = 0; u < 8; ++u)
                     if (ri[u] >= 0) {
                         const float f = (float)((double)v[u] * a.hinv);
-                        const int pr = pp[ri[u]], pc = pp[ci[u]];
-                        H32[pr * Kp + pc] = f;
-                        H32[pc * Kp + pr] = f;
+                        H32[ri[u] * Kp + ci[u]] = f;
+                        H32[ci[u] * Kp + ri[u]] = f;
                     }
             }
         }
-        for (int e = tid; e < (Kp - K) * Kp; e += kMasterThreads) H32[(size_t)K * Kp + e] = 0.f;   // rows K..Kp-1 (read with d = 0)
+        for (int e = tid; e < (4 * nF4 - nF) * Kp; e += kMasterThreads) H32[(size_t)nF * Kp + e] = 0.f;   // rows nF..4 nF4 - 1 (read with d = 0)
         for (int k = tid; k < N; k += kMasterThreads) {
             yc[k] = vy[k];
             vd[k] = 0.0;
@@ -572,8 +569,8 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
         }
         const long long c1 = clock64();
         clk_load += c1 - c0;
-        // Conjugate gradients on the faces of the box for the quadratic model at (vy, vg): one beam per thread (the
-        // first nv warps), all warps on the product with the matrix.  One sum over the beams per step: with the
+        // Conjugate gradients on that face of the box for the quadratic model at (vy, vg), and on its sub-faces as beams
+        // reach a bound: one beam per thread (the first nv warps), all warps on the product with the matrix.  One sum over the beams per step: with the
         // residual r, the preconditioner M, the direction d and H d at hand, A = sum M r^2, B = sum M r (H d) and
         // C = sum M (H d)^2 over the face give the Polak-Ribiere numerator of the NEXT residual r + t H d without a
         // second sum, (r+ - r) M r+ = t (B + t C), and its denominator is A.  Whether the face changed, whether any
@@ -583,8 +580,8 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
         // set on it explicitly.
         const double qtol = fmax(0.5 * tol, 0.05 * pgmax);
         const int k = tid;                                   // this thread's beam (k < N: checked on the host)
-        const bool mine = k < N && ik[k] >= 0;
-        const int myp = mine ? pk[k] : 0;                    // this beam's row and column of H32
+        const bool mine = k < N && pk[k] >= 0;               // a beam of the face
+        const int myp = mine ? pk[k] : 0;                    // its row and column of H32
         const int nv = (N + 31) / 32;                        // warps that hold beams
         auto ratio = [](double num, double den) { return (double)__fdividef((float)num, (float)den); };
         __shared__ int s_fl[2];
@@ -603,10 +600,10 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
         // state of this thread's beam
         double yk = mine ? vy[k] : 0.0, rk = mine ? vg[k] : 0.0, beta = 0.0;
         const double mk = mine ? Minv[k] : 1.0;
-        int fr = mine && !at_bound(yk, rk);
+        int fr = mine;                                       // still free (a beam that reaches a bound leaves the face for good)
         double prk = fr ? rk : 0.0, dk = -mk * prk;
         bool halt = false;
-        const int maxcg = 4 * K + 20;
+        const int maxcg = 4 * nF + 20;
         int it = 0;
         int fl = any_flags(fabs(prk) > qtol ? 2 : 0);
         while ((fl & 2) && !(fl & 4) && it < maxcg) {
@@ -620,10 +617,9 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
             // d_c is the same word for the whole warp.  Two halves: threads 0..255 and 256..511.
             {
                 const int r = tid & (kMasterThreads / 2 - 1), h = tid / (kMasterThreads / 2);
-                const int nA4 = (s_nA + 3) / 4;              // float4s of d that can hold a non-zero entry
-                const int q0 = h * ((nA4 + 1) / 2), q1 = min(nA4, q0 + (nA4 + 1) / 2);   // float4s of d of this half
+                const int q0 = h * ((nF4 + 1) / 2), q1 = min(nF4, q0 + (nF4 + 1) / 2);   // float4s of d of this half
                 float acc0 = 0.f, acc1 = 0.f;
-                if (r < K) {
+                if (r < nF) {
                     const float4 *d4 = reinterpret_cast<const float4 *>(dc);
                     const float *hc = H32 + r;
                     for (int q = q0; q < q1; ++q) {
@@ -635,9 +631,9 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
                         acc1 = fmaf(h4[3 * Kp], dv.w, acc1);
                     }
                 }
-                if (h == 1 && r < K) hpart2[r] = acc0 + acc1;
+                if (h == 1 && r < nF) hpart2[r] = acc0 + acc1;
                 __syncthreads();
-                if (h == 0 && r < K) hpart[r] = (acc0 + acc1) + hpart2[r];
+                if (h == 0 && r < nF) hpart[r] = (acc0 + acc1) + hpart2[r];
             }
             __syncthreads();
             double hdk = 0.0;
@@ -684,16 +680,15 @@ __device__ void newton_solver(const MasterArgs &a, float4 *smem_raw, unsigned lo
                     }
                 }
             }
-            const int fn = mine && !at_bound(yk, rk);
+            const int fn = fr && !at_bound(yk, rk);
             prk = fn ? rk : 0.0;
-            if (fn && !fr) atomicMax(&s_nA, myp + 1);        // a released beam: its column joins the product (read after the barrier)
             fl = any_flags(warp >= nv ? 0 : (fn != fr || hit || t == 0.0 ? 1 : 0) | (fabs(prk) > qtol ? 2 : 0) | (halt ? 4 : 0));
             // (only the warps that hold beams know the sums; `halt` and the rest of the loop control travel as flags)
             beta = (fl & 1) || !(s5[2] > 0.f) ? 0.0 : (double)fmaxf(0.f, __fdividef((float)t * (s5[3] + (float)t * s5[4]), s5[2]));
             dk = fn ? -mk * prk + beta * dk : 0.0;
             fr = fn;
         }
-        if (k < N) yc[k] = yk;
+        if (mine) yc[k] = yk;
         __syncthreads();
         clk_cg += clock64() - c1;
         // the step and its slope on the true gradient
