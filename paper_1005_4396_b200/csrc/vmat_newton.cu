@@ -13,8 +13,10 @@ namespace vmat {
 //     min_{lb <= y <= ub}  g.(y' - y) + 1/2 (y' - y)^T (2 H_F + 2 gamma L) (y' - y),
 //     H_F[k][k'] = sum_s omega_s d_k[s] d_k'[s],  omega_s = alpha_s (z_s < T_s), beta_s (z_s > T_s), else 0,
 // over the K <= N occupied beams: a problem in K unknowns that needs no pass over the columns at all once H_F is
-// known.  One block of the grid (the last one) holds H_F in its shared memory and solves that quadratic by
-// conjugate gradients on the faces of the box (Jacobi-preconditioned, fp64 vectors); the other blocks evaluate the
+// known.  One block of the grid (the last one) solves that quadratic, step by step: it forms the face of the box the
+// step starts from (the occupied beams not at a bound with the true gradient pointing outwards: about half of an
+// arc's beams sit at y = 0), holds H_F over those free beams in its shared memory and runs conjugate gradients on the
+// face (Jacobi-preconditioned, fp64 vectors; a beam that reaches a bound leaves it); the other blocks evaluate the
 // TRUE cost and gradient at the point it proposes, in one pass each (z = sum_k y_k d_k formed from y itself, so
 // there is no z += t q drift and no closing pass).  The piece changes only where a voxel crosses its T_s, so a
 // master solve takes two or three such passes instead of the twenty-odd of mode 0 (same minimiser: reading S11).
